@@ -1,0 +1,178 @@
+"""Seeded synthetic sprinklings (inputs only -- none of the method's arithmetic).
+
+This module is the one piece shared by the oracle-side tests and the CUDA
+path: it draws point coordinates with a counter-based SplitMix64 generator,
+sorts them by time, and hands the same fp64 buffer to both sides.  It never
+evaluates a causal relation, an interval or an action.
+
+The paper's workloads are themselves synthetic Poisson sprinklings
+(App. A.1); `N` is fixed instead of
+Poisson-distributed (reading A10).  Recipes:
+
+  config 1/2  1+1 flat diamond in light-cone coordinates, u,v ~ U[0,1)
+              (PAPER.md:3715-3729), sorted by ((u+v)/2, u, index)
+  config 3/5  3+1 flat diamond |t|+|x|<=1 by rejection from the cube
+              [-1,1)^4 (same distribution as PAPER.md:3745-3759 up to shift and
+              scale; reading A11), sorted by (t, x, index)
+  config 4    1+1 de Sitter slab, eta in [-1.2,-0.2] with density ~ sec^2(eta):
+              eta = atan(tan a + u (tan b - tan a)), theta = 2 pi u
+              (PAPER.md:3781-3795 generalised to an asymmetric slab; A12),
+              sorted by (eta, theta, index)
+"""
+from __future__ import annotations
+
+import dataclasses
+
+import numpy as np
+
+GEOM_MINK2_LIGHTCONE = 0
+GEOM_MINK_CONE = 1
+GEOM_DS2_SLAB = 2
+
+_GAMMA = np.uint64(0x9E3779B97F4A7C15)
+_M1 = np.uint64(0xBF58476D1CE4E5B9)
+_M2 = np.uint64(0x94D049BB133111EB)
+_MASK = (1 << 64) - 1
+
+SEED_BASE = 180504463 * 10
+
+
+def splitmix64(seed: int, start: int, count: int) -> np.ndarray:
+    """Outputs number start .. start+count-1 of SplitMix64 seeded with `seed`
+    (output n is mix(seed + (n+1)*gamma)); returned as uint64."""
+    n = np.arange(start + 1, start + count + 1, dtype=np.uint64)
+    with np.errstate(over="ignore"):
+        z = np.uint64(seed & _MASK) + n * _GAMMA
+        z = (z ^ (z >> np.uint64(30))) * _M1
+        z = (z ^ (z >> np.uint64(27))) * _M2
+        z = z ^ (z >> np.uint64(31))
+    return z
+
+
+def uniform01(seed: int, start: int, count: int) -> np.ndarray:
+    """fp64 uniforms in [0,1): (z >> 11) * 2^-53."""
+    z = splitmix64(seed, start, count)
+    return (z >> np.uint64(11)).astype(np.float64) * (1.0 / 9007199254740992.0)
+
+
+def _sort_rows(coords: np.ndarray, k0: np.ndarray, k1: np.ndarray) -> np.ndarray:
+    idx = np.arange(coords.shape[0])
+    order = np.lexsort((idx, k1, k0))  # primary k0, then k1, then original index
+    return np.ascontiguousarray(coords[order])
+
+
+def sprinkle_mink2_lightcone(N: int, seed: int) -> np.ndarray:
+    """[N][2] = (u, v), draws per point in the order u, v."""
+    r = uniform01(seed, 0, 2 * N).reshape(N, 2)
+    t = (r[:, 0] + r[:, 1]) / 2.0
+    return _sort_rows(r, t, r[:, 0])
+
+
+def sprinkle_mink4_diamond(N: int, seed: int) -> np.ndarray:
+    """[N][4] = (t, x, y, z); trial n uses draws 4n..4n+3 as t,x,y,z = 2u-1 and
+    is accepted iff |t| + sqrt(x^2+y^2+z^2) <= 1; the first N accepted trials."""
+    out = np.empty((N, 4), dtype=np.float64)
+    have = 0
+    trial = 0
+    while have < N:
+        batch = max(4096, int((N - have) * 8.5))
+        r = 2.0 * uniform01(seed, 4 * trial, 4 * batch).reshape(batch, 4) - 1.0
+        ok = np.abs(r[:, 0]) + np.sqrt(r[:, 1] ** 2 + r[:, 2] ** 2 + r[:, 3] ** 2) <= 1.0
+        acc = r[ok]
+        take = min(N - have, acc.shape[0])
+        out[have:have + take] = acc[:take]
+        have += take
+        trial += batch
+    return _sort_rows(out, out[:, 0], out[:, 1])
+
+
+def sprinkle_ds2_slab(N: int, seed: int, eta_a: float = -1.2, eta_b: float = -0.2) -> np.ndarray:
+    """[N][2] = (eta, theta), draws per point in the order eta, theta."""
+    r = uniform01(seed, 0, 2 * N).reshape(N, 2)
+    ta, tb = np.tan(eta_a), np.tan(eta_b)
+    eta = np.arctan(ta + r[:, 0] * (tb - ta))
+    theta = (2.0 * np.pi) * r[:, 1]
+    c = np.stack([eta, theta], axis=1)
+    return _sort_rows(c, eta, theta)
+
+
+def chain_lightcone(N: int) -> np.ndarray:
+    """Total order: u_i = v_i = i/N (sorted already)."""
+    u = np.arange(N, dtype=np.float64) / max(N, 1)
+    return np.ascontiguousarray(np.stack([u, u], axis=1))
+
+
+def antichain_lightcone(N: int) -> np.ndarray:
+    """Mutually unrelated points: u_i = i/N, v_i = 1 - i/N, sorted by time."""
+    u = np.arange(N, dtype=np.float64) / max(N, 1)
+    c = np.stack([u, 1.0 - u], axis=1)
+    return _sort_rows(c, (c[:, 0] + c[:, 1]) / 2.0, c[:, 0])
+
+
+@dataclasses.dataclass(frozen=True)
+class Config:
+    """One BASELINE.json workload."""
+    index: int          # 1..5
+    name: str
+    N: int
+    dim: int
+    geometry: int
+    batch: int = 1      # >1: independent causets (config 5)
+    kmax: int = -1      # -1: full histogram (k = 0..N-2)
+
+    @property
+    def seed(self) -> int:
+        return SEED_BASE + self.index
+
+
+CONFIGS = {
+    1: Config(1, "mink2_diamond_N1024", 1024, 2, GEOM_MINK2_LIGHTCONE),
+    2: Config(2, "mink2_diamond_N16384", 16384, 2, GEOM_MINK2_LIGHTCONE),
+    3: Config(3, "mink4_diamond_N65536", 65536, 4, GEOM_MINK_CONE),
+    4: Config(4, "ds2_slab_N131072", 131072, 2, GEOM_DS2_SLAB),
+    5: Config(5, "mink4_ensemble_4096xN2048", 2048, 4, GEOM_MINK_CONE, batch=4096, kmax=3),
+}
+
+
+def sprinkle(geometry: int, dim: int, N: int, seed: int) -> np.ndarray:
+    if geometry == GEOM_MINK2_LIGHTCONE and dim == 2:
+        return sprinkle_mink2_lightcone(N, seed)
+    if geometry == GEOM_MINK_CONE and dim == 4:
+        return sprinkle_mink4_diamond(N, seed)
+    if geometry == GEOM_MINK_CONE and dim in (2, 3):
+        # lower-dimensional flat diamonds: take the first `dim` coordinates of a
+        # cube rejection restricted to those coordinates
+        return _sprinkle_mink_low(N, dim, seed)
+    if geometry == GEOM_DS2_SLAB and dim == 2:
+        return sprinkle_ds2_slab(N, seed)
+    raise ValueError("no sprinkler for geometry=%d dim=%d" % (geometry, dim))
+
+
+def _sprinkle_mink_low(N: int, dim: int, seed: int) -> np.ndarray:
+    out = np.empty((N, dim), dtype=np.float64)
+    have = 0
+    trial = 0
+    while have < N:
+        batch = max(4096, int((N - have) * 4))
+        r = 2.0 * uniform01(seed, dim * trial, dim * batch).reshape(batch, dim) - 1.0
+        ok = np.abs(r[:, 0]) + np.sqrt((r[:, 1:] ** 2).sum(axis=1)) <= 1.0
+        acc = r[ok]
+        take = min(N - have, acc.shape[0])
+        out[have:have + take] = acc[:take]
+        have += take
+        trial += batch
+    return _sort_rows(out, out[:, 0], out[:, 1])
+
+
+def make_config_coords(cfg: Config, N: int | None = None, batch_index: int = 0) -> np.ndarray:
+    """Coordinates of config `cfg` (optionally at a reduced N, for tests).
+    Config 5: causet `batch_index` uses seed cfg.seed*4096 + batch_index."""
+    n = cfg.N if N is None else N
+    seed = cfg.seed if cfg.batch == 1 else cfg.seed * 4096 + batch_index
+    return sprinkle(cfg.geometry, cfg.dim, n, seed)
+
+
+def make_ensemble_coords(cfg: Config, B: int | None = None, N: int | None = None) -> np.ndarray:
+    """[B][N][dim] for the batched config."""
+    b = cfg.batch if B is None else B
+    return np.ascontiguousarray(np.stack([make_config_coords(cfg, N, i) for i in range(b)], axis=0))

@@ -1,0 +1,388 @@
+"""Pins for the oracle (CPU only).  Each test checks oracle/ against something
+other than itself: a closed form, an invariant, brute force on tiny inputs, an
+independent algorithm, or a number PAPER.md prints.  Citations: PAPER.md lines.
+"""
+import itertools
+import math
+import os
+from fractions import Fraction
+
+import numpy as np
+import pytest
+
+from paper_1805_04463_b200 import inputs as inp
+
+GOLDEN = os.path.join(os.path.dirname(__file__), "golden")
+
+
+# ----------------------------------------------------------------------------- helpers
+def brute_force_hist(C):
+    """Interval sizes by explicit set membership: |J+(i) & J-(j)|."""
+    N = C.shape[0]
+    future = [set(np.nonzero(C[i])[0].tolist()) for i in range(N)]
+    past = [set(np.nonzero(C[:, j])[0].tolist()) for j in range(N)]
+    hist = np.zeros(max(N - 1, 0), dtype=np.int64)
+    for i in range(N):
+        for j in future[i]:
+            hist[len(future[i] & past[j])] += 1
+    return hist
+
+
+def transitive_closure(C):
+    C = C.astype(bool)
+    N = C.shape[0]
+    for k in range(N):
+        C = C | (C[:, k:k + 1] & C[k:k + 1, :])
+    return C.astype(np.uint8)
+
+
+def hist_both_tiers(orc, C):
+    N = C.shape[0]
+    h0 = orc.interval_hist_alg19(C)
+    bits = orc.pack_bytes(C)
+    h1, wops, _ = orc.interval_hist_alg20(bits, N)
+    return h0, h1, bits, wops
+
+
+def all_geoms():
+    return [
+        (inp.GEOM_MINK2_LIGHTCONE, 2, 11),
+        (inp.GEOM_MINK_CONE, 2, 12),
+        (inp.GEOM_MINK_CONE, 3, 13),
+        (inp.GEOM_MINK_CONE, 4, 14),
+        (inp.GEOM_DS2_SLAB, 2, 15),
+    ]
+
+
+# ----------------------------------------------------------------------------- stage 1
+def test_relation_hand_cases(oracle):
+    L, Cn, D = inp.GEOM_MINK2_LIGHTCONE, inp.GEOM_MINK_CONE, inp.GEOM_DS2_SLAB
+    # light cone (ds^2 = -2 du dv): strict in both coordinates
+    assert oracle.relation([0.1, 0.2], [0.3, 0.4], L)
+    assert not oracle.relation([0.1, 0.5], [0.3, 0.4], L)
+    assert not oracle.relation([0.1, 0.2], [0.1, 0.4], L)      # du = 0: null, not related
+    assert not oracle.relation([0.3, 0.4], [0.1, 0.2], L)      # wrong time order
+    # flat cone: dt^2 >= |dx|^2, null related (reading A1), past not related
+    assert oracle.relation([0, 0, 0, 0], [1.0, 0.5, 0.5, 0.5], Cn)          # 1 >= 0.75
+    assert not oracle.relation([0, 0, 0, 0], [1.0, 0.6, 0.6, 0.6], Cn)      # 1 < 1.08
+    assert oracle.relation([0.0, 0.0], [1.0, 1.0], Cn)                      # null
+    assert oracle.relation([0.0, 0.0], [1.0, -1.0], Cn)
+    assert not oracle.relation([1.0, 0.0], [0.0, 0.0], Cn)                  # dt < 0
+    assert oracle.relation([0, 0, 0], [5.0, 3.0, 4.0], Cn)                  # 25 >= 25
+    assert not oracle.relation([0, 0, 0], [5.0, 3.0, 4.5], Cn)
+    # de Sitter slab: angular distance wraps around the circle
+    assert oracle.relation([-1.0, 0.1], [-0.7, 6.2], D)        # min(6.1, 0.183..) = 0.183 <= 0.3
+    assert not oracle.relation([-1.0, 0.1], [-0.9, 6.2], D)    # 0.183 > 0.1
+    assert not oracle.relation([-1.0, 1.0], [-0.5, 3.0], D)    # 2.0 > 0.5
+    assert oracle.relation([-1.0, 1.0], [-0.5, 1.5], D)        # 0.5 >= 0.5 (null related)
+
+
+def test_ds_relation_matches_paper_form(oracle):
+    """The paper's form pi - |pi - |dtheta|| equals min(a, 2pi-a)
+    in exact arithmetic; away from the null cone both give the same relation."""
+    rng = np.random.default_rng(5)
+    n_checked = 0
+    for _ in range(4000):
+        e1, e2 = np.sort(rng.uniform(-1.2, -0.2, 2))
+        t1, t2 = rng.uniform(0, 2 * np.pi, 2)
+        paper = np.pi - abs(np.pi - abs(t1 - t2))
+        if abs(paper - (e2 - e1)) < 1e-9:
+            continue
+        n_checked += 1
+        assert oracle.relation([e1, t1], [e2, t2], inp.GEOM_DS2_SLAB) == (paper <= e2 - e1)
+    assert n_checked > 3900
+
+
+@pytest.mark.parametrize("geom,dim,seed", all_geoms())
+def test_matrix_structure_transitive_acyclic(oracle, geom, dim, seed):
+    """Upper triangular (acyclic under the time order) and
+    transitive: (C.C > 0) => C."""
+    N = 700
+    coords = inp.sprinkle(geom, dim, N, seed)
+    C = oracle.causal_matrix_bytes(coords, geom)
+    assert np.array_equal(C, np.triu(C, 1))
+    two_step = (C.astype(np.float32) @ C.astype(np.float32)) > 0
+    assert not np.any(two_step & (C == 0))
+    # direct re-evaluation of the predicate in numpy for the flat cone (different code path)
+    if geom == inp.GEOM_MINK_CONE:
+        d = coords[None, :, :] - coords[:, None, :]
+        s = np.zeros((N, N))
+        for a in range(1, dim):
+            s = s + d[:, :, a] * d[:, :, a]
+        ref = (d[:, :, 0] >= 0) & (d[:, :, 0] * d[:, :, 0] >= s)
+        ref = np.triu(ref, 1)
+        assert np.array_equal(C.astype(bool), ref)
+
+
+@pytest.mark.parametrize("N", [0, 1, 2, 63, 64, 65, 130, 1000])
+def test_bit_layout_and_padding(oracle, N):
+    """LSB-first blocks, zero padding, pack/unpack/transposes agree."""
+    coords = inp.sprinkle(inp.GEOM_MINK2_LIGHTCONE, 2, N, 3) if N else np.zeros((0, 2))
+    C = oracle.causal_matrix_bytes(coords, inp.GEOM_MINK2_LIGHTCONE)
+    bits = oracle.causal_matrix_bits(coords, inp.GEOM_MINK2_LIGHTCONE)
+    stride = oracle.row_stride_words(N)
+    assert bits.shape == (N, stride) and stride % 2 == 0 and stride * 64 >= N
+    assert np.array_equal(bits, oracle.pack_bytes(C))
+    assert np.array_equal(oracle.unpack_bits(bits, N), C)
+    # independent unpack with numpy: little-endian bit order
+    if N:
+        nb = np.unpackbits(bits.view(np.uint8), axis=1, bitorder="little")
+        assert np.array_equal(nb[:, :N], C)
+        assert not nb[:, N:].any()
+        bT = oracle.transpose_bits(bits, N)
+        assert np.array_equal(oracle.unpack_bits(bT, N), C.T)
+
+
+# ----------------------------------------------------------------------------- stage 2
+@pytest.mark.parametrize("N", [2, 3, 5, 64, 65, 300])
+def test_chain_closed_form(oracle, N):
+    """Total order: pair (i,j) has j-i-1 interior elements => N_k = N-1-k."""
+    coords = inp.chain_lightcone(N)
+    C = oracle.causal_matrix_bytes(coords, inp.GEOM_MINK2_LIGHTCONE)
+    assert C.sum() == N * (N - 1) // 2
+    h0, h1, _, _ = hist_both_tiers(oracle, C)
+    expect = np.arange(N - 1, 0, -1, dtype=np.int64)
+    assert np.array_equal(h0, expect)
+    assert np.array_equal(h1, expect)
+    # actions of the chain: I2 = N, I4 = N-1 (N >= 5), from N_k = N-1-k
+    S2, I2 = oracle.bd_action(h0, N, 2)
+    assert I2 == N - 2 * max(N - 1, 0) + 4 * max(N - 2, 0) - 2 * max(N - 3, 0)
+    if N >= 4:
+        assert I2 == N and S2 == 2.0 * N
+    S4, I4 = oracle.bd_action(h0, N, 4)
+    if N >= 5:
+        assert I4 == N - 1
+        assert S4 == pytest.approx(4 / math.sqrt(6) * (N - 1), rel=1e-15)
+
+
+@pytest.mark.parametrize("N", [1, 2, 64, 257])
+def test_antichain(oracle, N):
+    coords = inp.antichain_lightcone(N)
+    C = oracle.causal_matrix_bytes(coords, inp.GEOM_MINK2_LIGHTCONE)
+    assert C.sum() == 0
+    h0, h1, _, _ = hist_both_tiers(oracle, C)
+    assert not h0.any() and not h1.any()
+    for dim in (2, 4):
+        _, I = oracle.bd_action(h0, N, dim)
+        assert I == N
+
+
+def test_exhaustive_small_posets(oracle):
+    """Every transitive strictly-upper-triangular 0/1 matrix with N <= 5."""
+    n_posets = 0
+    for N in range(2, 6):
+        pairs = [(i, j) for i in range(N) for j in range(i + 1, N)]
+        for mask in range(1 << len(pairs)):
+            C = np.zeros((N, N), dtype=np.uint8)
+            for b, (i, j) in enumerate(pairs):
+                if (mask >> b) & 1:
+                    C[i, j] = 1
+            if not np.array_equal(transitive_closure(C), C):
+                continue
+            n_posets += 1
+            expect = brute_force_hist(C)
+            h0, h1, _, _ = hist_both_tiers(oracle, C)
+            assert np.array_equal(h0, expect), (N, mask)
+            assert np.array_equal(h1, expect), (N, mask)
+    # labelled-by-linear-extension partial orders on 2..5 points: 2, 7, 40, 357
+    assert n_posets == 2 + 7 + 40 + 357
+
+
+@pytest.mark.parametrize("N,p,seed", [(8, 0.5, 0), (33, 0.2, 1), (64, 0.1, 2), (64, 0.03, 3), (100, 0.05, 4)])
+def test_random_transitive_closures_bruteforce(oracle, N, p, seed):
+    rng = np.random.default_rng(seed)
+    C = np.triu((rng.random((N, N)) < p).astype(np.uint8), 1)
+    C = transitive_closure(C)
+    expect = brute_force_hist(C)
+    h0, h1, bits, wops = hist_both_tiers(oracle, C)
+    assert np.array_equal(h0, expect)
+    assert np.array_equal(h1, expect)
+    R, W = oracle.count_relations(bits, N)
+    assert R == int(C.sum()) == int(expect.sum())
+    ii, jj = np.nonzero(C)
+    assert W == wops == int(((jj >> 6) - (ii >> 6) + 1).sum())
+
+
+def test_nontransitive_input_follows_alg19_definition(oracle):
+    """Alg. 19 counts k with i<k and k<j as matrix entries; on a non-transitive
+    matrix tier-0 and tier-1 still agree with the matrix-product definition."""
+    rng = np.random.default_rng(9)
+    N = 90
+    C = np.triu((rng.random((N, N)) < 0.3).astype(np.uint8), 1)
+    prod = C.astype(np.int64) @ C.astype(np.int64)
+    expect = np.bincount(prod[C == 1], minlength=N - 1).astype(np.int64)
+    h0, h1, _, _ = hist_both_tiers(oracle, C)
+    assert np.array_equal(h0, expect)
+    assert np.array_equal(h1, expect)
+
+
+@pytest.mark.parametrize("geom,dim,seed", all_geoms())
+@pytest.mark.parametrize("N", [64, 1000])
+def test_tier1_equals_tier0_and_moments(oracle, geom, dim, seed, N):
+    """Alg. 20 == Alg. 19 on every geometry (N=1000 is not a multiple of 64), and
+    sum_k N_k = R,  sum_k k N_k = sum_m indeg(m) outdeg(m) (number of 3-chains)."""
+    coords = inp.sprinkle(geom, dim, N, seed + N)
+    C = oracle.causal_matrix_bytes(coords, geom)
+    h0, h1, bits, _ = hist_both_tiers(oracle, C)
+    assert np.array_equal(h0, h1)
+    R = int(C.sum())
+    assert int(h0.sum()) == R
+    indeg = C.sum(axis=0).astype(np.int64)
+    outdeg = C.sum(axis=1).astype(np.int64)
+    assert int((np.arange(N - 1) * h0).sum()) == int((indeg * outdeg).sum())
+    # row-range additivity of tier-1 (used for sampled parity at full size)
+    ha, wa, _ = oracle.interval_hist_alg20(bits, N, 0, N // 3)
+    hb, wb, _ = oracle.interval_hist_alg20(bits, N, N // 3, N)
+    assert np.array_equal(ha + hb, h1)
+
+
+def test_tier1_equals_tier0_N2048(oracle):
+    cfg = inp.CONFIGS[5]
+    coords = inp.make_config_coords(cfg, batch_index=1)
+    C = oracle.causal_matrix_bytes(coords, cfg.geometry)
+    h0, h1, _, _ = hist_both_tiers(oracle, C)
+    assert np.array_equal(h0, h1)
+    # soft sanity: ordering fraction of the 3+1 diamond is about 1/10 (Myrheim-Meyer; not in PAPER.md)
+    frac = C.sum() / (cfg.N * (cfg.N - 1) / 2)
+    assert 0.07 < frac < 0.13
+
+
+# ----------------------------------------------------------------------------- 1+1 diamond: independent algorithms
+def count_inversions(a):
+    """Textbook merge-sort inversion count."""
+    a = list(a)
+    if len(a) < 2:
+        return 0, a
+    mid = len(a) // 2
+    il, left = count_inversions(a[:mid])
+    ir, right = count_inversions(a[mid:])
+    merged, i, j, inv = [], 0, 0, il + ir
+    while i < len(left) and j < len(right):
+        if left[i] <= right[j]:
+            merged.append(left[i]); i += 1
+        else:
+            merged.append(right[j]); j += 1; inv += len(left) - i
+    merged += left[i:] + right[j:]
+    return inv, merged
+
+
+def sat_histogram(coords):
+    """Interval sizes in the light-cone diamond from a summed-area table over the
+    rank grid: |I(i,j)| = points strictly inside the rectangle (u_i,u_j)x(v_i,v_j)."""
+    N = coords.shape[0]
+    ru = np.argsort(np.argsort(coords[:, 0], kind="stable"), kind="stable")
+    rv = np.argsort(np.argsort(coords[:, 1], kind="stable"), kind="stable")
+    G = np.zeros((N + 1, N + 1), dtype=np.int32)
+    G[ru + 1, rv + 1] = 1
+    P = G.cumsum(axis=0, dtype=np.int32).cumsum(axis=1, dtype=np.int32)  # P[a][b] = #{ru<a, rv<b}
+    hist = np.zeros(N - 1, dtype=np.int64)
+    R = 0
+    for i in range(N):
+        rel = (ru > ru[i]) & (rv > rv[i])
+        a0, b0 = ru[i] + 1, rv[i] + 1
+        a1, b1 = ru[rel], rv[rel]
+        cnt = P[a1, b1] - P[a0, b1] - P[a1, b0] + P[a0, b0]
+        hist += np.bincount(cnt, minlength=N - 1)
+        R += int(rel.sum())
+    return hist, R
+
+
+@pytest.mark.parametrize("N,tier", [(1024, 0), (4096, 1)])
+def test_lightcone_diamond_sat_and_inversions(oracle, N, tier):
+    cfg = inp.CONFIGS[1]
+    coords = inp.make_config_coords(cfg, N=N)
+    bits = oracle.causal_matrix_bits(coords, cfg.geometry)
+    R, _ = oracle.count_relations(bits, N)
+    # R = N(N-1)/2 - inversions of the v-ranks taken in u-order
+    order = np.argsort(coords[:, 0], kind="stable")
+    inv, _ = count_inversions(coords[order, 1].tolist())
+    assert R == N * (N - 1) // 2 - inv
+    # expected relation fraction of the 2-D diamond: E[R] = N(N-1)/4, Kendall variance
+    sd = math.sqrt(N * (N - 1) * (2 * N + 5) / 72)
+    assert abs(R - N * (N - 1) / 4) < 4.5 * sd
+    expect, R_sat = sat_histogram(coords)
+    assert R_sat == R
+    if tier == 0:
+        hist = oracle.interval_hist_alg19(oracle.unpack_bits(bits, N))
+    else:
+        hist, _, _ = oracle.interval_hist_alg20(bits, N)
+    assert np.array_equal(hist, expect)
+
+
+# ----------------------------------------------------------------------------- stage 3
+def _read_table(name):
+    rows = []
+    with open(os.path.join(GOLDEN, name)) as f:
+        for line in f:
+            line = line.split("#")[0].strip()
+            if line:
+                rows.append(line.split())
+    return rows
+
+
+def _prefactor(dim):
+    return {2: 2.0,
+            3: (1 / math.gamma(5 / 3)) * (math.pi / (3 * math.sqrt(2))) ** (2 / 3),
+            4: 4 / math.sqrt(6)}[dim]
+
+
+def test_action_coefficients_three_statements(oracle):
+    """Eq. 4.10-4.12 (golden), Eq. 4.5-4.7 (golden, sign flipped) and the eps -> 1
+    limit of Eq. 4.16-4.18 agree, and the oracle reproduces them term by term."""
+    act = {int(r[0]): [Fraction(x) for x in r[2:6]] for r in _read_table("bd_action_coefficients.txt")}
+    dal = {int(r[0]): (Fraction(r[1]), [Fraction(x) for x in r[2:6]]) for r in _read_table("dalembertian_coefficients.txt")}
+    N = 1000
+    for dim in (2, 3, 4):
+        a, b = dal[dim]
+        assert [-(a * x) for x in b] == act[dim]                      # statement 2 vs statement 1
+        for m in range(0, 8):                                           # statement 3
+            f = oracle.smear_f(dim, m, 1.0)
+            # S_eps at eps=1: bracket N - a*sum n_m f(m-1)  =>  c_{m+1} = -a f(m)
+            c = float(act[dim][m]) if m < 4 else 0.0
+            assert -float(a) * f == pytest.approx(c, abs=1e-15), (dim, m)
+        S0, _ = oracle.bd_action(np.zeros(4, dtype=np.int64), N, dim)
+        assert S0 == pytest.approx(_prefactor(dim) * N, rel=1e-15)
+        for m in range(4):
+            h = np.zeros(6, dtype=np.int64)
+            h[m] = 7
+            S, _ = oracle.bd_action(h, N, dim)
+            assert S == pytest.approx(_prefactor(dim) * (N + 7 * float(act[dim][m])), rel=1e-14)
+        h = np.zeros(6, dtype=np.int64); h[4] = 5; h[5] = 9             # n_5, n_6 do not enter
+        assert oracle.bd_action(h, N, dim)[0] == S0
+
+
+def test_action_short_hist_and_int64_range(oracle):
+    # missing entries are zero (reading A9)
+    assert oracle.bd_action(np.array([3], dtype=np.int64), 10, 4)[1] == 10 - 3
+    assert oracle.bd_action(np.zeros(0, dtype=np.int64), 10, 2)[1] == 10
+    # counts far above 2^31 stay exact in the integer bracket
+    h = np.array([3_000_000_000, 2_500_000_000, 2_000_000_001, 1_999_999_999], dtype=np.int64)
+    _, I = oracle.bd_action(h, 131072, 4)
+    assert I == 131072 - 3_000_000_000 + 9 * 2_500_000_000 - 16 * 2_000_000_001 + 8 * 1_999_999_999
+
+
+def test_smeared_action_reduces_to_local_at_eps_1(oracle):
+    coords = inp.sprinkle(inp.GEOM_DS2_SLAB, 2, 600, 77)
+    bits = oracle.causal_matrix_bits(coords, inp.GEOM_DS2_SLAB)
+    hist, _, _ = oracle.interval_hist_alg20(bits, 600)
+    for dim in (2, 3, 4):
+        S, _ = oracle.bd_action(hist, 600, dim)
+        assert oracle.smeared_action(hist, 600, dim, 1.0) == pytest.approx(S, rel=1e-12)
+
+
+def test_smear_f_against_paper_form(oracle):
+    """Eq. 4.16-4.18 as printed (with the 1/(1-eps) factors), rational arithmetic."""
+    for eps in (Fraction(1, 64), Fraction(1, 3)):
+        q = 1 - eps
+        for m in (0, 1, 2, 3, 10, 40):
+            f2 = q ** m * (1 - 2 * m * eps / q + Fraction(m * (m - 1), 2) * eps ** 2 / q ** 2)
+            f3 = q ** m * (1 - Fraction(27, 8) * m * eps / q + Fraction(9, 8) * m * (m - 1) * eps ** 2 / q ** 2)
+            f4 = q ** m * (1 - 9 * m * eps / q + 8 * m * (m - 1) * eps ** 2 / q ** 2
+                           - Fraction(4, 3) * m * (m - 1) * (m - 2) * eps ** 3 / q ** 3)
+            for dim, f in ((2, f2), (3, f3), (4, f4)):
+                assert oracle.smear_f(dim, m, float(eps)) == pytest.approx(float(f), rel=1e-12, abs=1e-15)
+
+
+def test_seh_golden():
+    eta0, printed, _ = _read_table("ds_slab_seh.txt")[0]
+    assert round(4 * math.pi * math.tan(float(eta0)), 3) == float(printed)
