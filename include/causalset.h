@@ -1,0 +1,163 @@
+/*
+ * causalset.h -- C ABI of libcausalset.so: the causal-set action hot path of
+ * W. J. Cunningham, "High Performance Algorithms for Quantum Gravity and
+ * Cosmology" (arXiv:1805.04463), hand-written CUDA for sm_100a (B200).
+ *
+ * Path (citations are PAPER.md line numbers; readings A1..A15 are in DESIGN.md):
+ *   a1  cs_causal_matrix   coordinates -> bit-packed causal matrix
+ *   a2  cs_interval_hist   bits -> interval abundances N_k           (Alg. 19/20)
+ *   a3  cs_bd_action       N_k -> Benincasa-Dowker action            (Eq. 4.10-4.12)
+ *
+ * Conventions common to every entry point
+ *   - "device" pointers are caller-owned CUDA device memory (e.g. from torch);
+ *     "host" pointers are ordinary host memory.  The library never allocates
+ *     or frees an output and keeps no pointer after the call returns.
+ *   - `stream` is a cudaStream_t passed as void* (NULL = legacy default
+ *     stream).  Device-pointer calls only enqueue work and return; results are
+ *     valid after the stream is synchronised.  *_host calls synchronise.
+ *   - every call returns a cs_status (0 = ok, <0 = error); nothing throws.
+ *     On error no output is guaranteed.  There is no CPU fallback: without a
+ *     CUDA device every compute call returns CS_ERR_CUDA.
+ *   - bit layout (FastBitset): a matrix is N rows
+ *     of `stride = cs_row_stride_words(N)` uint64 blocks; element j of a row is
+ *     bit (j & 63) of block (j >> 6), LSB first; padding bits are zero.
+ *   - elements must be sorted by non-decreasing time coordinate
+ *     so that i -< j implies i < j; only pairs i < j are ever tested.
+ */
+#ifndef CAUSALSET_H
+#define CAUSALSET_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+/* Geometry of the sprinkled region = the pairwise predicate "i precedes j". */
+enum cs_geometry {
+    /* dim = 2, coords (u,v) light-cone coordinates, ds^2 = -2 du dv:
+       i -< j  <=>  u_i < u_j && v_i < v_j. */
+    CS_GEOM_MINK2_LIGHTCONE = 0,
+    /* dim = 2..4, coords (t,x[,y[,z]]) (squared form of Eq. 7.7):
+       dt = t_j - t_i, d_a = x^a_j - x^a_i, s = ((dx*dx) + (dy*dy)) + (dz*dz),
+       i -< j  <=>  dt >= 0 && dt*dt >= s        (fp64, no FMA contraction). */
+    CS_GEOM_MINK_CONE = 1,
+    /* dim = 2, coords (eta,theta) of the 1+1 de Sitter slab (Eq. 4.19):
+       a = |theta_j - theta_i|, b = 2pi - a, m = a < b ? a : b,
+       i -< j  <=>  eta_j - eta_i >= m           (2pi = 0x401921FB54442D18). */
+    CS_GEOM_DS2_SLAB = 2
+};
+
+enum cs_status {
+    CS_OK = 0,
+    CS_ERR_ARG = -1,        /* NULL pointer, negative size, misaligned buffer */
+    CS_ERR_DIM = -2,        /* dim not valid for the geometry / action */
+    CS_ERR_GEOM = -3,       /* unknown geometry */
+    CS_ERR_UNSORTED = -4,   /* reserved (the library does not check sortedness) */
+    CS_ERR_WORKSPACE = -5,  /* workspace NULL or smaller than the *_workspace() query */
+    CS_ERR_CUDA = -6        /* a CUDA runtime call or launch failed; see cs_last_cuda_error() */
+};
+
+/* How a2 is computed.  Both routes give identical integers. */
+enum cs_route {
+    CS_ROUTE_AUTO = 0,      /* the library's default for this N */
+    CS_ROUTE_POPC = 1,      /* shared-memory tiled AND + POPC (Alg. 20 restated for the GPU) */
+    CS_ROUTE_TENSOR = 2     /* count matrix C.C as a 0/1 int8 contraction on tcgen05 tensor cores */
+};
+
+const char *cs_version(void);
+const char *cs_status_string(int status);
+/* Text of the last CUDA error seen by this thread's calls ("" if none). Host string, static storage. */
+const char *cs_last_cuda_error(void);
+
+/* Row stride in uint64 blocks: ceil(N/64) rounded up to an even count (rows are 128-bit aligned). */
+int64_t cs_row_stride_words(int64_t N);
+
+/* a1: causal matrix.
+ *   coords  device, [N][dim] fp64, time coordinate first, sorted by time; 16-byte aligned.
+ *   bits    device, [N][stride] uint64, overwritten: bit j of row i = (i < j && i -< j)
+ *           (upper triangular: "future of i"); lower triangle and padding are written as zero.
+ *   bitsT   device or NULL, [N][stride] uint64, overwritten with the transpose
+ *           (bit i of row j = i -< j: "past of j").
+ * Errors: CS_ERR_ARG (NULL coords/bits, N < 0), CS_ERR_GEOM, CS_ERR_DIM, CS_ERR_CUDA.  N = 0 is a no-op. */
+int cs_causal_matrix(const double *coords, int64_t N, int dim, int geometry,
+                     uint64_t *bits, uint64_t *bitsT, void *stream);
+
+/* Same for B independent causets: coords [B][N][dim], bits/bitsT [B][N][stride]. */
+int cs_causal_matrix_batched(const double *coords, int64_t B, int64_t N, int dim, int geometry,
+                             uint64_t *bits, uint64_t *bitsT, void *stream);
+
+/* bitsT <- transpose(bits) (both device, [N][stride]); for callers that kept only `bits`. */
+int cs_transpose_bits(const uint64_t *bits, int64_t N, uint64_t *bitsT, void *stream);
+
+/* Relation count R = popcount(bits) and the algorithmic work of Alg. 20,
+ * W_alg = sum over related pairs of ((j>>6) - (i>>6) + 1) 64-bit blocks.
+ *   out  device, int64[2] = {R, W_alg}, overwritten. */
+int cs_relation_stats(const uint64_t *bits, int64_t N, int64_t *out, void *stream);
+
+/* a2: interval abundances (Alg. 19; Alg. 20).
+ * For every related pair i -< j:  c = |{k : i -< k -< j}| = popcount(bits[i] & bitsT[j]);  hist[c] += 1.
+ * hist[k] = n_{k+1} in the paper's notation (Eq. 4.8).
+ *   bits, bitsT  device, as produced by cs_causal_matrix.  bitsT may be NULL: it is then
+ *                rebuilt inside the workspace (query the size with have_bitsT = 0).
+ *   kmax         largest interval size kept; kmax < 0 or kmax > N-2 means N-2.
+ *   hist         device, int64[kmax+1] (after clamping; at least 1 entry), overwritten.
+ *                Pairs with c > kmax are dropped from hist but counted in *n_relations.
+ *   n_relations  device int64[1] or NULL: number of related pairs (restricted to the row range).
+ *   workspace    device, >= cs_interval_hist_workspace() bytes, 256-byte aligned; scratch.
+ * cs_interval_hist_ex restricts the outer element i to [row_begin, row_end) (hist then holds
+ * the contribution of those rows only: partial histograms add up) and selects the route.
+ * Errors: CS_ERR_ARG, CS_ERR_WORKSPACE, CS_ERR_CUDA.  N < 2 zeroes the outputs. */
+size_t cs_interval_hist_workspace(int64_t N, int64_t kmax, int have_bitsT, int route);
+int cs_interval_hist(const uint64_t *bits, const uint64_t *bitsT, int64_t N, int64_t kmax,
+                     int64_t *hist, int64_t *n_relations,
+                     void *workspace, size_t workspace_bytes, void *stream);
+int cs_interval_hist_ex(const uint64_t *bits, const uint64_t *bitsT, int64_t N, int64_t kmax,
+                        int64_t row_begin, int64_t row_end, int route,
+                        int64_t *hist, int64_t *n_relations,
+                        void *workspace, size_t workspace_bytes, void *stream);
+/* Route CS_ROUTE_AUTO resolves to for this N (CS_ROUTE_POPC or CS_ROUTE_TENSOR). */
+int cs_default_route(int64_t N);
+
+/* a3: Benincasa-Dowker action, Eq. 4.10-4.12 with l/l_p = 1:
+ *   dim 2: S = 2 (N - 2 N_0 + 4 N_1 - 2 N_2)
+ *   dim 3: S = (1/Gamma(5/3)) (pi/(3 sqrt 2))^(2/3) (N - N_0 + (27/8) N_1 - (9/4) N_2)
+ *   dim 4: S = (4/sqrt 6) (N - N_0 + 9 N_1 - 16 N_2 + 8 N_3)
+ *   hist     device, int64[kmax+1]; entries beyond kmax are taken as 0.
+ *   action   device, double[1], overwritten.
+ *   bracket  device int64[1] or NULL: the exact integer bracket (dim 2, 4) or 8 x bracket (dim 3).
+ * Errors: CS_ERR_ARG, CS_ERR_DIM, CS_ERR_CUDA. */
+int cs_bd_action(const int64_t *hist, int64_t kmax, int64_t N, int dim,
+                 double *action, int64_t *bracket, void *stream);
+
+/* Batched ensemble (Monte-Carlo use): B independent causets of N points each,
+ * one action per causet.
+ *   coords   device, [B][N][dim] fp64, each causet sorted by time.
+ *   actions  device, double[B], overwritten.
+ *   hist4    device int64[B][4] or NULL: N_0..N_3 of every causet.
+ *   workspace device, >= cs_bd_action_batched_workspace(B, N) bytes, 256-byte aligned. */
+size_t cs_bd_action_batched_workspace(int64_t B, int64_t N);
+int cs_bd_action_batched(const double *coords, int64_t B, int64_t N, int dim, int geometry,
+                         double *actions, int64_t *hist4,
+                         void *workspace, size_t workspace_bytes, void *stream);
+
+/* End-to-end with HOST buffers: copies coords host->device, runs a1, a2, a3, copies hist and
+ * the action back, and synchronises the stream before returning.
+ *   coords_host  host, [N][dim] fp64 (pinned memory makes the copy asynchronous).
+ *   hist_host    host, int64[kmax+1] (after clamping), overwritten.
+ *   action_host  host, double[1], overwritten.
+ *   workspace    device, >= cs_action_host_workspace(N, kmax) bytes, 256-byte aligned. */
+size_t cs_action_host_workspace(int64_t N, int64_t kmax);
+int cs_action_host(const double *coords_host, int64_t N, int dim, int geometry, int64_t kmax,
+                   int64_t *hist_host, double *action_host,
+                   void *workspace, size_t workspace_bytes, void *stream);
+
+/* Number of kernel launches issued by this library in this process so far (for bench.py's
+ * `gpu_launches`). */
+int64_t cs_launch_count(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* CAUSALSET_H */

@@ -15,6 +15,7 @@ from .oracle import (  # noqa: F401
     causal_matrix_bytes,
     causal_matrix_bits,
     transpose_bits,
+    degrees,
     pack_bytes,
     unpack_bits,
     interval_hist_alg19,

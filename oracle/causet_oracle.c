@@ -122,9 +122,29 @@ void orc_transpose_bits(const uint64_t *bits, int64_t N, int64_t stride, uint64_
 {
     memset(bitsT, 0, (size_t)N * (size_t)stride * sizeof(uint64_t));
     for (int64_t i = 0; i < N; i++)
-        for (int64_t j = 0; j < N; j++)
-            if ((bits[i * stride + (j >> 6)] >> (j & 63)) & 1)
-                bitsT[j * stride + (i >> 6)] |= (uint64_t)1 << (i & 63);
+        for (int64_t b = 0; b < stride; b++) {
+            uint64_t w = bits[i * stride + b];
+            while (w) {                                   /* visit the set bits of the block */
+                int64_t j = b * 64 + __builtin_ctzll(w);
+                w &= w - 1;
+                if (j < N) bitsT[j * stride + (i >> 6)] |= (uint64_t)1 << (i & 63);
+            }
+        }
+}
+
+/* out-degree (row sums) and in-degree (column sums) of the relation. */
+void orc_degrees(const uint64_t *bits, int64_t N, int64_t stride, int64_t *outdeg, int64_t *indeg)
+{
+    for (int64_t i = 0; i < N; i++) { outdeg[i] = 0; indeg[i] = 0; }
+    for (int64_t i = 0; i < N; i++)
+        for (int64_t b = 0; b < stride; b++) {
+            uint64_t w = bits[i * stride + b];
+            while (w) {
+                int64_t j = b * 64 + __builtin_ctzll(w);
+                w &= w - 1;
+                if (j < N) { outdeg[i]++; indeg[j]++; }
+            }
+        }
 }
 
 void orc_pack_bytes(const uint8_t *C, int64_t N, uint64_t *bits, int64_t stride)

@@ -50,6 +50,8 @@ def _load():
         lib.orc_causal_matrix_bits.argtypes = [_p, _i64, ctypes.c_int, ctypes.c_int, _p, _i64]
         lib.orc_transpose_bits.restype = None
         lib.orc_transpose_bits.argtypes = [_p, _i64, _i64, _p]
+        lib.orc_degrees.restype = None
+        lib.orc_degrees.argtypes = [_p, _i64, _i64, _p, _p]
         lib.orc_pack_bytes.restype = None
         lib.orc_pack_bytes.argtypes = [_p, _i64, _p, _i64]
         lib.orc_unpack_bits.restype = None
@@ -121,6 +123,15 @@ def transpose_bits(bits: np.ndarray, N: int) -> np.ndarray:
     out = np.zeros_like(bits)
     _load().orc_transpose_bits(_ptr(bits), N, bits.shape[1], _ptr(out))
     return out
+
+
+def degrees(bits: np.ndarray, N: int):
+    """(outdeg, indeg) int64 arrays of the relation."""
+    bits = np.ascontiguousarray(bits, dtype=np.uint64)
+    o = np.zeros(N, dtype=np.int64)
+    i = np.zeros(N, dtype=np.int64)
+    _load().orc_degrees(_ptr(bits), N, bits.shape[1], _ptr(o), _ptr(i))
+    return o, i
 
 
 def pack_bytes(C: np.ndarray, stride: int | None = None) -> np.ndarray:

@@ -1,0 +1,261 @@
+// cs_api.cu -- the extern "C" boundary of libcausalset.so (include/causalset.h).
+// Argument checking, workspace carving and kernel sequencing only; the arithmetic lives in
+// cs_build.cu (a1), cs_interval_popc.cu / cs_interval_tensor.cu (a2) and cs_action.cu (a3).
+#include "cs_common.cuh"
+
+namespace cs {
+
+thread_local char g_cuda_err[256] = "";
+long long g_launches = 0;
+
+int sm_count()
+{
+    static int cached = 0;
+    if (cached <= 0) {
+        int dev = 0, n = 0;
+        if (cudaGetDevice(&dev) == cudaSuccess &&
+            cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && n > 0)
+            cached = n;
+        else
+            return 148;
+    }
+    return cached;
+}
+
+static int resolve_route(int64_t N, int route)
+{
+    if (route == CS_ROUTE_AUTO) route = cs_default_route(N);
+    if (route == CS_ROUTE_TENSOR && !interval_tensor_available()) return -1;
+    return route;
+}
+
+static size_t interval_ws_bytes(int64_t B, int64_t N, int have_bitsT, int route)
+{
+    size_t ws = 256;   // tile counter etc.
+    if (!have_bitsT) ws += align_up((size_t)B * N * row_stride_words(N) * 8, 256);
+    if (route == CS_ROUTE_TENSOR) ws += align_up(interval_tensor_scratch_bytes(B, N), 256);
+    return ws;
+}
+
+// hist: int64[B][kmax+1]; shared by the single and the batched entry points
+static int interval_hist_impl(const uint64_t *bits, const uint64_t *bitsT, int64_t B, int64_t N, int64_t kmax,
+                              int64_t row_begin, int64_t row_end, int route, int64_t *hist, int64_t *nrel,
+                              void *workspace, size_t workspace_bytes, cudaStream_t st)
+{
+    kmax = clamp_kmax(N, kmax);
+    CS_CUDA(cudaMemsetAsync(hist, 0, (size_t)B * (kmax + 1) * sizeof(int64_t), st));
+    if (nrel) CS_CUDA(cudaMemsetAsync(nrel, 0, sizeof(int64_t), st));
+    if (N < 2) return CS_OK;
+    if (row_begin < 0) row_begin = 0;
+    if (row_end > N) row_end = N;
+    if (row_begin >= row_end) return CS_OK;
+    route = resolve_route(N, route);
+    if (route < 0) return CS_ERR_ARG;
+    const size_t need = interval_ws_bytes(B, N, bitsT != nullptr, route);
+    if (!workspace || workspace_bytes < need || ((uintptr_t)workspace & 255)) return CS_ERR_WORKSPACE;
+    unsigned char *ws = static_cast<unsigned char *>(workspace);
+    void *scratch = ws;
+    ws += 256;
+    if (!bitsT) {
+        uint64_t *t = reinterpret_cast<uint64_t *>(ws);
+        ws += align_up((size_t)B * N * row_stride_words(N) * 8, 256);
+        int rc = launch_transpose_bits(bits, B, N, t, st);
+        if (rc) return rc;
+        bitsT = t;
+    }
+    if (route == CS_ROUTE_TENSOR)
+        return launch_interval_tensor(bits, bitsT, B, N, kmax, row_begin, row_end, hist, nrel, ws,
+                                      workspace_bytes - (size_t)(ws - static_cast<unsigned char *>(workspace)), st);
+    return launch_interval_popc(bits, bitsT, B, N, kmax, row_begin, row_end, hist, nrel, scratch, st);
+}
+
+}  // namespace cs
+
+using namespace cs;
+
+extern "C" {
+
+const char *cs_version(void) { return "causalset-b200 0.1 (sm_100a)"; }
+
+const char *cs_status_string(int status)
+{
+    switch (status) {
+    case CS_OK: return "ok";
+    case CS_ERR_ARG: return "invalid argument";
+    case CS_ERR_DIM: return "dimension not valid for this geometry/action";
+    case CS_ERR_GEOM: return "unknown geometry";
+    case CS_ERR_UNSORTED: return "elements not sorted by time";
+    case CS_ERR_WORKSPACE: return "workspace missing, misaligned or too small";
+    case CS_ERR_CUDA: return "CUDA error";
+    default: return "unknown status";
+    }
+}
+
+const char *cs_last_cuda_error(void) { return g_cuda_err; }
+
+int64_t cs_row_stride_words(int64_t N) { return N < 0 ? 0 : row_stride_words(N); }
+
+int64_t cs_launch_count(void) { return g_launches; }
+
+int cs_default_route(int64_t N)
+{
+    (void)N;
+    return interval_tensor_available() && N >= 1024 ? CS_ROUTE_TENSOR : CS_ROUTE_POPC;
+}
+
+int cs_causal_matrix_batched(const double *coords, int64_t B, int64_t N, int dim, int geometry,
+                             uint64_t *bits, uint64_t *bitsT, void *stream)
+{
+    if (N < 0 || B < 0) return CS_ERR_ARG;
+    if (geometry < CS_GEOM_MINK2_LIGHTCONE || geometry > CS_GEOM_DS2_SLAB) return CS_ERR_GEOM;
+    if (geometry == CS_GEOM_MINK_CONE ? (dim < 2 || dim > 4) : (dim != 2)) return CS_ERR_DIM;
+    if (N == 0 || B == 0) return CS_OK;
+    if (!coords || !bits) return CS_ERR_ARG;
+    return launch_causal_matrix(coords, B, N, dim, geometry, bits, bitsT, static_cast<cudaStream_t>(stream));
+}
+
+int cs_causal_matrix(const double *coords, int64_t N, int dim, int geometry,
+                     uint64_t *bits, uint64_t *bitsT, void *stream)
+{
+    return cs_causal_matrix_batched(coords, 1, N, dim, geometry, bits, bitsT, stream);
+}
+
+int cs_transpose_bits(const uint64_t *bits, int64_t N, uint64_t *bitsT, void *stream)
+{
+    if (N < 0) return CS_ERR_ARG;
+    if (N == 0) return CS_OK;
+    if (!bits || !bitsT) return CS_ERR_ARG;
+    return launch_transpose_bits(bits, 1, N, bitsT, static_cast<cudaStream_t>(stream));
+}
+
+int cs_relation_stats(const uint64_t *bits, int64_t N, int64_t *out, void *stream)
+{
+    if (N < 0 || !out || (N > 0 && !bits)) return CS_ERR_ARG;
+    return launch_relation_stats(bits, N, out, static_cast<cudaStream_t>(stream));
+}
+
+size_t cs_interval_hist_workspace(int64_t N, int64_t kmax, int have_bitsT, int route)
+{
+    (void)kmax;
+    if (N < 0) return 0;
+    int r = resolve_route(N, route);
+    if (r < 0) r = CS_ROUTE_POPC;
+    return interval_ws_bytes(1, N, have_bitsT, r);
+}
+
+int cs_interval_hist_ex(const uint64_t *bits, const uint64_t *bitsT, int64_t N, int64_t kmax,
+                        int64_t row_begin, int64_t row_end, int route,
+                        int64_t *hist, int64_t *n_relations,
+                        void *workspace, size_t workspace_bytes, void *stream)
+{
+    if (N < 0 || !hist || (N > 0 && !bits)) return CS_ERR_ARG;
+    if (route < CS_ROUTE_AUTO || route > CS_ROUTE_TENSOR) return CS_ERR_ARG;
+    return interval_hist_impl(bits, bitsT, 1, N, kmax, row_begin, row_end, route, hist, n_relations,
+                              workspace, workspace_bytes, static_cast<cudaStream_t>(stream));
+}
+
+int cs_interval_hist(const uint64_t *bits, const uint64_t *bitsT, int64_t N, int64_t kmax,
+                     int64_t *hist, int64_t *n_relations,
+                     void *workspace, size_t workspace_bytes, void *stream)
+{
+    return cs_interval_hist_ex(bits, bitsT, N, kmax, 0, N, CS_ROUTE_AUTO, hist, n_relations,
+                               workspace, workspace_bytes, stream);
+}
+
+int cs_bd_action(const int64_t *hist, int64_t kmax, int64_t N, int dim,
+                 double *action, int64_t *bracket, void *stream)
+{
+    if (!hist || !action || N < 0) return CS_ERR_ARG;
+    if (dim < 2 || dim > 4) return CS_ERR_DIM;
+    if (kmax < 0) kmax = clamp_kmax(N, kmax);
+    return launch_bd_action(hist, kmax + 1, 1, kmax, N, dim, action, bracket, nullptr,
+                            static_cast<cudaStream_t>(stream));
+}
+
+// ---- batched ensemble ----------------------------------------------------------------------
+// workspace: [bits B*N*stride][bitsT B*N*stride][hist B*4 int64][interval scratch]
+size_t cs_bd_action_batched_workspace(int64_t B, int64_t N)
+{
+    if (B < 0 || N < 0) return 0;
+    const size_t mat = align_up((size_t)B * N * row_stride_words(N) * 8, 256);
+    int r = cs_default_route(N);
+    return 2 * mat + align_up((size_t)B * 4 * 8, 256) + interval_ws_bytes(B, N, 1, r);
+}
+
+int cs_bd_action_batched(const double *coords, int64_t B, int64_t N, int dim, int geometry,
+                         double *actions, int64_t *hist4,
+                         void *workspace, size_t workspace_bytes, void *stream)
+{
+    if (B < 0 || N < 0) return CS_ERR_ARG;
+    if (B == 0) return CS_OK;
+    if (!coords || !actions) return CS_ERR_ARG;
+    if (!workspace || workspace_bytes < cs_bd_action_batched_workspace(B, N) || ((uintptr_t)workspace & 255))
+        return CS_ERR_WORKSPACE;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    const size_t mat = align_up((size_t)B * N * row_stride_words(N) * 8, 256);
+    unsigned char *ws = static_cast<unsigned char *>(workspace);
+    uint64_t *bits = reinterpret_cast<uint64_t *>(ws);
+    uint64_t *bitsT = reinterpret_cast<uint64_t *>(ws + mat);
+    int64_t *hist = reinterpret_cast<int64_t *>(ws + 2 * mat);
+    unsigned char *iws = ws + 2 * mat + align_up((size_t)B * 4 * 8, 256);
+    int rc = cs_causal_matrix_batched(coords, B, N, dim, geometry, bits, bitsT, stream);
+    if (rc) return rc;
+    const int64_t kmax = clamp_kmax(N, 3);
+    if (kmax < 3) CS_CUDA(cudaMemsetAsync(hist, 0, (size_t)B * 4 * 8, st));
+    // hist rows are kmax+1 long; with kmax = 3 that is the [B][4] layout asked for
+    int64_t *hist_k = hist;
+    rc = interval_hist_impl(bits, bitsT, B, N, kmax, 0, N, CS_ROUTE_AUTO, hist_k, nullptr, iws,
+                            workspace_bytes - (size_t)(iws - ws), st);
+    if (rc) return rc;
+    return launch_bd_action(hist_k, kmax + 1, B, kmax, N, dim, actions, nullptr, hist4, st);
+}
+
+// ---- end to end with host buffers ----------------------------------------------------------
+// workspace: [coords][bits][bitsT][hist][action+pad][interval scratch]
+size_t cs_action_host_workspace(int64_t N, int64_t kmax)
+{
+    if (N < 0) return 0;
+    kmax = clamp_kmax(N, kmax);
+    const size_t mat = align_up((size_t)N * row_stride_words(N) * 8, 256);
+    return align_up((size_t)N * 4 * 8, 256) + 2 * mat + align_up((size_t)(kmax + 1) * 8, 256) + 256 +
+           interval_ws_bytes(1, N, 1, cs_default_route(N));
+}
+
+int cs_action_host(const double *coords_host, int64_t N, int dim, int geometry, int64_t kmax,
+                   int64_t *hist_host, double *action_host,
+                   void *workspace, size_t workspace_bytes, void *stream)
+{
+    if (N < 0 || !hist_host || !action_host || (N > 0 && !coords_host)) return CS_ERR_ARG;
+    if (dim < 2 || dim > 4) return CS_ERR_DIM;
+    if (!workspace || workspace_bytes < cs_action_host_workspace(N, kmax) || ((uintptr_t)workspace & 255))
+        return CS_ERR_WORKSPACE;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    kmax = clamp_kmax(N, kmax);
+    const size_t mat = align_up((size_t)N * row_stride_words(N) * 8, 256);
+    unsigned char *ws = static_cast<unsigned char *>(workspace);
+    double *coords = reinterpret_cast<double *>(ws);
+    ws += align_up((size_t)N * 4 * 8, 256);
+    uint64_t *bits = reinterpret_cast<uint64_t *>(ws);
+    ws += mat;
+    uint64_t *bitsT = reinterpret_cast<uint64_t *>(ws);
+    ws += mat;
+    int64_t *hist = reinterpret_cast<int64_t *>(ws);
+    ws += align_up((size_t)(kmax + 1) * 8, 256);
+    double *action = reinterpret_cast<double *>(ws);
+    ws += 256;
+    const size_t left = workspace_bytes - (size_t)(ws - static_cast<unsigned char *>(workspace));
+
+    if (N > 0) CS_CUDA(cudaMemcpyAsync(coords, coords_host, (size_t)N * dim * 8, cudaMemcpyHostToDevice, st));
+    int rc = cs_causal_matrix(coords, N, dim, geometry, bits, bitsT, stream);
+    if (rc) return rc;
+    rc = cs_interval_hist(bits, bitsT, N, kmax, hist, nullptr, ws, left, stream);
+    if (rc) return rc;
+    rc = cs_bd_action(hist, kmax, N, dim, action, nullptr, stream);
+    if (rc) return rc;
+    CS_CUDA(cudaMemcpyAsync(hist_host, hist, (size_t)(kmax + 1) * 8, cudaMemcpyDeviceToHost, st));
+    CS_CUDA(cudaMemcpyAsync(action_host, action, 8, cudaMemcpyDeviceToHost, st));
+    CS_CUDA(cudaStreamSynchronize(st));
+    return CS_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,287 @@
+// cs_build.cu -- stage a1: causal-matrix build, plus the
+// bit-matrix transpose and the relation statistics (R, W_alg).
+//
+// One CTA owns one BT x BT tile (I <= J) of the pair space.  The BT "past" points x_i of the
+// tile are staged in shared memory (the paper's Alg. 16 idea, for both
+// elements: PAPER.md:1695); every lane keeps one "future" point x_j in registers and sweeps
+// 32 rows at a time.  The predicate is evaluated ONCE per pair and yields both outputs:
+//   bits  (row i, bit j)  through a warp ballot     -> "future of i"
+//   bitsT (row j, bit i)  accumulated in the lane   -> "past of j"
+// Both tiles are assembled in shared memory and written with full 32-byte row segments.
+// The same CTA zero-fills the mirrored tile (lower triangle), so no separate memset is needed.
+//
+// Floating point: explicit round-to-nearest intrinsics (__dsub_rn, __dmul_rn, __dadd_rn), which
+// the compiler never contracts into FMA, in exactly the order stated in include/causalset.h.
+#include "cs_common.cuh"
+
+namespace cs {
+
+constexpr int BT = 256;          // tile edge in elements
+constexpr int BUILD_THREADS = 256;
+
+template <int GEOM, int DIM>
+struct Pred;
+
+template <>
+struct Pred<CS_GEOM_MINK2_LIGHTCONE, 2> {
+    __device__ static __forceinline__ bool rel(const double *xi, const double *xj)
+    {
+        return (xi[0] < xj[0]) && (xi[1] < xj[1]);
+    }
+};
+
+template <int DIM>
+struct Pred<CS_GEOM_MINK_CONE, DIM> {
+    __device__ static __forceinline__ bool rel(const double *xi, const double *xj)
+    {
+        double dt = __dsub_rn(xj[0], xi[0]);
+        double dx = __dsub_rn(xj[1], xi[1]);
+        double s = __dmul_rn(dx, dx);
+        if (DIM >= 3) {
+            double dy = __dsub_rn(xj[2], xi[2]);
+            s = __dadd_rn(s, __dmul_rn(dy, dy));
+        }
+        if (DIM >= 4) {
+            double dz = __dsub_rn(xj[3], xi[3]);
+            s = __dadd_rn(s, __dmul_rn(dz, dz));
+        }
+        return (dt >= 0.0) && (__dmul_rn(dt, dt) >= s);
+    }
+};
+
+template <>
+struct Pred<CS_GEOM_DS2_SLAB, 2> {
+    __device__ static __forceinline__ bool rel(const double *xi, const double *xj)
+    {
+        const double two_pi = __longlong_as_double(0x401921FB54442D18LL);
+        double deta = __dsub_rn(xj[0], xi[0]);
+        double a = fabs(__dsub_rn(xj[1], xi[1]));
+        double b = __dsub_rn(two_pi, a);
+        double m = (a < b) ? a : b;
+        return deta >= m;
+    }
+};
+
+template <int GEOM, int DIM>
+__global__ void __launch_bounds__(BUILD_THREADS)
+k_causal_matrix(const double *__restrict__ coords, int64_t N, int64_t stride,
+                uint64_t *__restrict__ bits, uint64_t *__restrict__ bitsT)
+{
+    const int J = blockIdx.x, I = blockIdx.y;
+    if (I > J) return;
+    const int64_t b = blockIdx.z;
+    coords += b * N * DIM;
+    bits += b * N * stride;
+    if (bitsT) bitsT += b * N * stride;
+
+    __shared__ double s_xi[DIM][BT];
+    __shared__ uint32_t s_U[BT][9];   // row i_local, 32-bit word = 32 columns j
+    __shared__ uint32_t s_L[BT][9];   // row j_local, 32-bit word = 32 rows i
+
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const double qnan = __longlong_as_double(0x7FF8000000000000LL);   // compares false: unrelated
+
+    {   // stage the tile's past points (SoA), NaN beyond N
+        int64_t gi = (int64_t)I * BT + tid;
+#pragma unroll
+        for (int d = 0; d < DIM; d++) s_xi[d][tid] = (gi < N) ? coords[gi * DIM + d] : qnan;
+    }
+    double xj[DIM];
+    const int jl = warp * 32 + lane;
+    {
+        int64_t gj = (int64_t)J * BT + jl;
+#pragma unroll
+        for (int d = 0; d < DIM; d++) xj[d] = (gj < N) ? coords[gj * DIM + d] : qnan;
+    }
+    __syncthreads();
+
+    const bool diag = (I == J);
+#pragma unroll 1
+    for (int sb = 0; sb < BT / 32; sb++) {
+        uint32_t uw = 0, lw = 0;
+#pragma unroll 8
+        for (int ii = 0; ii < 32; ii++) {
+            const int il = sb * 32 + ii;
+            double xi[DIM];
+#pragma unroll
+            for (int d = 0; d < DIM; d++) xi[d] = s_xi[d][il];
+            bool r = Pred<GEOM, DIM>::rel(xi, xj);
+            if (diag) r = r && (il < jl);
+            uint32_t bal = __ballot_sync(0xffffffffu, r);
+            if (lane == ii) uw = bal;
+            lw |= (r ? 1u : 0u) << ii;
+        }
+        s_U[sb * 32 + lane][warp] = uw;
+        s_L[jl][sb] = lw;
+    }
+    __syncthreads();
+
+    // write-out: BT rows x 4 uint64 per tile; 4 consecutive threads cover one 32-byte row segment
+    const int q = tid & 3;
+#pragma unroll
+    for (int pass = 0; pass < 4; pass++) {
+        const int r = (tid >> 2) + 64 * pass;
+        const int64_t ri = (int64_t)I * BT + r, rj = (int64_t)J * BT + r;
+        const int64_t wi = (int64_t)I * (BT / 64) + q, wj = (int64_t)J * (BT / 64) + q;
+        const uint64_t u = (uint64_t)s_U[r][2 * q] | ((uint64_t)s_U[r][2 * q + 1] << 32);
+        const uint64_t l = (uint64_t)s_L[r][2 * q] | ((uint64_t)s_L[r][2 * q + 1] << 32);
+        if (ri < N && wj < stride) bits[ri * stride + wj] = u;
+        if (bitsT && rj < N && wi < stride) bitsT[rj * stride + wi] = l;
+        if (!diag) {   // mirrored tile is identically zero
+            if (rj < N && wi < stride) bits[rj * stride + wi] = 0;
+            if (bitsT && ri < N && wj < stride) bitsT[ri * stride + wj] = 0;
+        }
+    }
+}
+
+// Columns of the last tile may stop short of the row stride (stride is rounded up to an even
+// word count); those padding words are zeroed here.
+__global__ void k_zero_tail(uint64_t *bits, uint64_t *bitsT, int64_t rows, int64_t stride, int64_t first_word)
+{
+    int64_t r = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (r >= rows) return;
+    for (int64_t w = first_word; w < stride; w++) {
+        bits[r * stride + w] = 0;
+        if (bitsT) bitsT[r * stride + w] = 0;
+    }
+}
+
+template <int GEOM, int DIM>
+static int launch_build_t(const double *coords, int64_t B, int64_t N, int64_t stride,
+                          uint64_t *bits, uint64_t *bitsT, cudaStream_t st)
+{
+    const int nT = (int)((N + BT - 1) / BT);
+    dim3 grid(nT, nT, (unsigned)B);
+    k_causal_matrix<GEOM, DIM><<<grid, BUILD_THREADS, 0, st>>>(coords, N, stride, bits, bitsT);
+    CS_LAUNCHED("k_causal_matrix");
+    const int64_t covered = (int64_t)nT * (BT / 64);
+    if (covered < stride) {
+        int64_t rows = B * N;
+        k_zero_tail<<<(unsigned)((rows + 255) / 256), 256, 0, st>>>(bits, bitsT, rows, stride, covered);
+        CS_LAUNCHED("k_zero_tail");
+    }
+    return CS_OK;
+}
+
+int launch_causal_matrix(const double *coords, int64_t B, int64_t N, int dim, int geometry,
+                         uint64_t *bits, uint64_t *bitsT, cudaStream_t st)
+{
+    const int64_t stride = row_stride_words(N);
+    if (N > (int64_t)BT * 65535 || B > 65535) return CS_ERR_ARG;
+    switch (geometry) {
+    case CS_GEOM_MINK2_LIGHTCONE:
+        if (dim != 2) return CS_ERR_DIM;
+        return launch_build_t<CS_GEOM_MINK2_LIGHTCONE, 2>(coords, B, N, stride, bits, bitsT, st);
+    case CS_GEOM_MINK_CONE:
+        if (dim == 2) return launch_build_t<CS_GEOM_MINK_CONE, 2>(coords, B, N, stride, bits, bitsT, st);
+        if (dim == 3) return launch_build_t<CS_GEOM_MINK_CONE, 3>(coords, B, N, stride, bits, bitsT, st);
+        if (dim == 4) return launch_build_t<CS_GEOM_MINK_CONE, 4>(coords, B, N, stride, bits, bitsT, st);
+        return CS_ERR_DIM;
+    case CS_GEOM_DS2_SLAB:
+        if (dim != 2) return CS_ERR_DIM;
+        return launch_build_t<CS_GEOM_DS2_SLAB, 2>(coords, B, N, stride, bits, bitsT, st);
+    default:
+        return CS_ERR_GEOM;
+    }
+}
+
+// ---- transpose -----------------------------------------------------------------------------
+// One warp transposes one 32x32 bit block with the 5-step butterfly; blocks are read as 32-bit
+// halves of the uint64 rows.
+__device__ __forceinline__ uint32_t transpose32(uint32_t x, int lane)
+{
+    const uint32_t mlo[5] = {0x0000FFFFu, 0x00FF00FFu, 0x0F0F0F0Fu, 0x33333333u, 0x55555555u};
+#pragma unroll
+    for (int t = 0; t < 5; t++) {
+        const int s = 16 >> t;
+        const uint32_t o = __shfl_xor_sync(0xffffffffu, x, s);
+        if (lane & s) x = (x & ~mlo[t]) | ((o >> s) & mlo[t]);
+        else          x = (x & mlo[t]) | ((o << s) & ~mlo[t]);
+    }
+    return x;
+}
+
+__global__ void __launch_bounds__(256)
+k_transpose_bits(const uint64_t *__restrict__ bits, int64_t N, int64_t stride, uint64_t *__restrict__ bitsT)
+{
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int64_t b = blockIdx.z;
+    const uint32_t *src = reinterpret_cast<const uint32_t *>(bits + b * N * stride);
+    uint32_t *dst = reinterpret_cast<uint32_t *>(bitsT + b * N * stride);
+    const int64_t cb = (int64_t)blockIdx.x * 8 + warp;   // 32-column block
+    const int64_t rb = blockIdx.y;                       // 32-row block
+    const int64_t s32 = stride * 2;
+    if (cb >= s32) return;
+    const int64_t r = rb * 32 + lane;
+    uint32_t x = (r < N) ? src[r * s32 + cb] : 0u;
+    x = transpose32(x, lane);
+    const int64_t orow = cb * 32 + lane;
+    if (orow < N && rb < s32) dst[orow * s32 + rb] = x;
+}
+
+__global__ void k_zero_words(uint64_t *p, int64_t n)
+{
+    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) p[i] = 0;
+}
+
+int launch_transpose_bits(const uint64_t *bits, int64_t B, int64_t N, uint64_t *bitsT, cudaStream_t st)
+{
+    const int64_t stride = row_stride_words(N);
+    if (N == 0) return CS_OK;
+    const int64_t s32 = stride * 2;
+    const int64_t rblocks = (N + 31) / 32;
+    if (rblocks > 65535 || B > 65535) return CS_ERR_ARG;
+    if (rblocks < s32) {   // 32-bit words no row block maps to (row padding): clear everything first
+        int64_t n = B * N * stride;
+        k_zero_words<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(bitsT, n);
+        CS_LAUNCHED("k_zero_words");
+    }
+    dim3 grid((unsigned)((s32 + 7) / 8), (unsigned)rblocks, (unsigned)B);
+    k_transpose_bits<<<grid, 256, 0, st>>>(bits, N, stride, bitsT);
+    CS_LAUNCHED("k_transpose_bits");
+    return CS_OK;
+}
+
+// ---- relation statistics ------------------------------------------------------------------
+// out[0] = R = popcount(bits); out[1] = W_alg = sum_{i -< j} ((j>>6) - (i>>6) + 1)
+__global__ void __launch_bounds__(256)
+k_relation_stats(const uint64_t *__restrict__ bits, int64_t N, int64_t stride, unsigned long long *out)
+{
+    const int lane = threadIdx.x & 31;
+    const int64_t warp_global = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    const int64_t nwarps = ((int64_t)gridDim.x * blockDim.x) >> 5;
+    unsigned long long R = 0, W = 0;
+    for (int64_t i = warp_global; i < N; i += nwarps) {
+        const int64_t wi = i >> 6;
+        for (int64_t w = wi + lane; w < stride; w += 32) {
+            unsigned long long p = __popcll(bits[i * stride + w]);
+            R += p;
+            W += p * (unsigned long long)(w - wi + 1);
+        }
+    }
+#pragma unroll
+    for (int s = 16; s >= 1; s >>= 1) {
+        R += __shfl_xor_sync(0xffffffffu, R, s);
+        W += __shfl_xor_sync(0xffffffffu, W, s);
+    }
+    if (lane == 0 && (R | W)) {
+        atomicAdd(&out[0], R);
+        atomicAdd(&out[1], W);
+    }
+}
+
+int launch_relation_stats(const uint64_t *bits, int64_t N, int64_t *out, cudaStream_t st)
+{
+    CS_CUDA(cudaMemsetAsync(out, 0, 2 * sizeof(int64_t), st));
+    if (N == 0) return CS_OK;
+    const int64_t stride = row_stride_words(N);
+    int blocks = sm_count() * 8;
+    int64_t need = (N + 7) / 8;
+    if (need < blocks) blocks = (int)need;
+    k_relation_stats<<<blocks, 256, 0, st>>>(bits, N, stride, reinterpret_cast<unsigned long long *>(out));
+    CS_LAUNCHED("k_relation_stats");
+    return CS_OK;
+}
+
+}  // namespace cs

@@ -1,0 +1,73 @@
+// cs_common.cuh -- shared declarations of the CUDA side of libcausalset.so (sm_100a).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <stdio.h>
+#include <string.h>
+
+#include "../../include/causalset.h"
+
+namespace cs {
+
+extern thread_local char g_cuda_err[256];
+extern long long g_launches;   // kernels launched by this library (host counter)
+
+inline int cuda_fail(cudaError_t e, const char *what)
+{
+    snprintf(g_cuda_err, sizeof(g_cuda_err), "%s: %s", what, cudaGetErrorString(e));
+    return CS_ERR_CUDA;
+}
+
+#define CS_CUDA(call)                                               \
+    do {                                                            \
+        cudaError_t e__ = (call);                                   \
+        if (e__ != cudaSuccess) return cs::cuda_fail(e__, #call);   \
+    } while (0)
+
+#define CS_LAUNCHED(name)                                           \
+    do {                                                            \
+        cs::g_launches++;                                           \
+        cudaError_t e__ = cudaGetLastError();                       \
+        if (e__ != cudaSuccess) return cs::cuda_fail(e__, name);    \
+    } while (0)
+
+inline int64_t row_stride_words(int64_t N)
+{
+    int64_t w = (N + 63) / 64;
+    return w + (w & 1);
+}
+
+inline int64_t clamp_kmax(int64_t N, int64_t kmax)
+{
+    int64_t top = N - 2;
+    if (top < 0) top = 0;
+    if (kmax < 0 || kmax > top) kmax = top;
+    return kmax;
+}
+
+inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+
+int sm_count();   // SMs of the current device (cached)
+
+// ---- stage launchers (defined in the .cu files) ---------------------------------------------
+int launch_causal_matrix(const double *coords, int64_t B, int64_t N, int dim, int geometry,
+                         uint64_t *bits, uint64_t *bitsT, cudaStream_t st);
+int launch_transpose_bits(const uint64_t *bits, int64_t B, int64_t N, uint64_t *bitsT, cudaStream_t st);
+int launch_relation_stats(const uint64_t *bits, int64_t N, int64_t *out, cudaStream_t st);
+
+// hist (int64[B][kmax+1]) and nrel (int64[B] or NULL) must be zeroed by the caller.
+int launch_interval_popc(const uint64_t *bits, const uint64_t *bitsT, int64_t B, int64_t N, int64_t kmax,
+                         int64_t row_begin, int64_t row_end, int64_t *hist, int64_t *nrel,
+                         void *scratch, cudaStream_t st);
+size_t interval_popc_scratch_bytes();
+
+int launch_interval_tensor(const uint64_t *bits, const uint64_t *bitsT, int64_t B, int64_t N, int64_t kmax,
+                           int64_t row_begin, int64_t row_end, int64_t *hist, int64_t *nrel,
+                           void *scratch, size_t scratch_bytes, cudaStream_t st);
+size_t interval_tensor_scratch_bytes(int64_t B, int64_t N);
+bool interval_tensor_available();
+
+int launch_bd_action(const int64_t *hist, int64_t hist_stride, int64_t B, int64_t kmax, int64_t N, int dim,
+                     double *action, int64_t *bracket, int64_t *hist4, cudaStream_t st);
+
+}  // namespace cs

@@ -1,0 +1,58 @@
+"""The C-ABI library builds, loads on a CPU-only host and exports every symbol the header declares."""
+import ctypes
+import re
+
+import pytest
+
+from paper_1805_04463_b200 import api, build
+
+
+@pytest.fixture(scope="module")
+def lib():
+    build.build()
+    return api.load()
+
+
+def declared_symbols():
+    text = open(api.HEADER_PATH).read()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    return sorted(set(re.findall(r"\b(cs_[a-z0-9_]+)\s*\(", text)))
+
+
+def test_header_symbols_exported(lib):
+    names = declared_symbols()
+    assert len(names) >= 15
+    for n in names:
+        assert hasattr(lib, n), "libcausalset.so does not export %s" % n
+    # the binding marshals exactly the declared entry points
+    assert sorted(api._SIGNATURES) == names
+
+
+def test_host_only_entry_points(lib):
+    assert b"sm_100a" in lib.cs_version()
+    assert lib.cs_status_string(0) == b"ok"
+    assert lib.cs_status_string(-5).startswith(b"workspace")
+    for N, want in [(0, 0), (1, 2), (64, 2), (65, 2), (128, 2), (129, 4), (1000, 16), (65536, 1024), (131072, 2048)]:
+        assert lib.cs_row_stride_words(N) == want
+    assert lib.cs_launch_count() >= 0
+
+
+def test_argument_errors_need_no_gpu(lib):
+    # argument validation happens before any CUDA call
+    assert lib.cs_causal_matrix(None, -1, 2, 0, None, None, None) == -1          # CS_ERR_ARG
+    assert lib.cs_causal_matrix(None, 8, 2, 7, None, None, None) == -3           # CS_ERR_GEOM
+    assert lib.cs_causal_matrix(None, 8, 3, 0, None, None, None) == -2           # CS_ERR_DIM
+    assert lib.cs_causal_matrix(None, 8, 5, 1, None, None, None) == -2
+    assert lib.cs_causal_matrix(None, 8, 2, 0, None, None, None) == -1           # NULL buffers
+    assert lib.cs_causal_matrix(None, 0, 2, 0, None, None, None) == 0            # N = 0 is a no-op
+    assert lib.cs_bd_action(None, 3, 10, 4, None, None, None) == -1
+    assert lib.cs_interval_hist(None, None, 10, -1, None, None, None, 0, None) == -1
+    assert lib.cs_interval_hist_workspace(65536, -1, 1, 1) >= 256
+    assert lib.cs_interval_hist_workspace(1024, -1, 0, 1) >= 256 + 1024 * 16 * 8
+
+
+def test_missing_library_fails_loudly(monkeypatch, tmp_path):
+    monkeypatch.setattr(api, "_lib", None)
+    monkeypatch.setattr(api, "LIB_PATH", str(tmp_path / "nope.so"))
+    with pytest.raises(RuntimeError, match="no CPU fallback"):
+        api.load()

@@ -1,0 +1,247 @@
+"""Parity of the CUDA path (through the C ABI) with the oracle -- bit-exact.
+
+Run on the B200 box:  python -m pytest tests -m gpu -x -q
+Every input is seeded and synthetic (paper_1805_04463_b200.inputs); nothing
+reads /root/reference at run time.
+"""
+import numpy as np
+import pytest
+
+torch = pytest.importorskip("torch")
+
+from paper_1805_04463_b200 import inputs as inp  # noqa: E402
+
+pytestmark = pytest.mark.gpu
+
+GEOMS = [
+    (inp.GEOM_MINK2_LIGHTCONE, 2),
+    (inp.GEOM_MINK_CONE, 2),
+    (inp.GEOM_MINK_CONE, 3),
+    (inp.GEOM_MINK_CONE, 4),
+    (inp.GEOM_DS2_SLAB, 2),
+]
+
+
+@pytest.fixture(scope="module")
+def api():
+    if not torch.cuda.is_available():
+        pytest.fail("gpu tests need a CUDA device")
+    from paper_1805_04463_b200 import api as _api
+    _api.load()
+    torch.cuda.set_device(0)
+    return _api
+
+
+def routes(api):
+    r = [api.ROUTE_POPC]
+    try:
+        x = torch.zeros((128, 2), dtype=torch.int64, device="cuda")
+        api.interval_hist(x, x, 128, route=api.ROUTE_TENSOR)
+        r.append(api.ROUTE_TENSOR)
+    except RuntimeError:
+        pass
+    return r
+
+
+def to_u64(t):
+    return t.cpu().numpy().view(np.uint64)
+
+
+def gpu_bits(api, coords, geom):
+    d = torch.from_numpy(np.ascontiguousarray(coords)).cuda()
+    bits, bitsT = api.causal_matrix(d, geom)
+    torch.cuda.synchronize()
+    return bits, bitsT
+
+
+# ----------------------------------------------------------------------------- a1
+@pytest.mark.parametrize("geom,dim", GEOMS)
+@pytest.mark.parametrize("N", [1, 2, 63, 64, 65, 255, 256, 257, 1000, 1024, 3001])
+def test_causal_matrix_bit_exact(api, oracle, geom, dim, N):
+    coords = inp.sprinkle(geom, dim, N, 100 + N + dim)
+    o_bits = oracle.causal_matrix_bits(coords, geom)
+    bits, bitsT = gpu_bits(api, coords, geom)
+    assert np.array_equal(to_u64(bits), o_bits)
+    assert np.array_equal(to_u64(bitsT), oracle.transpose_bits(o_bits, N))
+    # bits-only call, then the stand-alone transpose
+    d = torch.from_numpy(coords).cuda()
+    b2, none = api.causal_matrix(d, geom, want_transpose=False)
+    assert none is None and torch.equal(b2, bits)
+    assert torch.equal(api.transpose_bits(b2, N), bitsT)
+
+
+def test_causal_matrix_near_null_pairs(api, oracle):
+    """Pairs exactly on and one ulp either side of the light cone decide identically."""
+    rng = np.random.default_rng(1)
+    base = rng.uniform(-0.5, 0.5, (200, 4))
+    base[:, 0] = np.sort(rng.uniform(-1, 0, 200))
+    fut = base.copy()
+    r = np.sqrt((rng.uniform(0.1, 0.4, (200, 3)) ** 2).sum(axis=1))
+    dx = rng.normal(size=(200, 3))
+    dx = dx / np.linalg.norm(dx, axis=1)[:, None] * r[:, None]
+    fut[:, 1:] = base[:, 1:] + dx
+    fut[:, 0] = base[:, 0] + r                      # (nearly) null separated partners
+    fut2 = fut.copy(); fut2[:, 0] = np.nextafter(fut[:, 0], 10.0)
+    fut3 = fut.copy(); fut3[:, 0] = np.nextafter(fut[:, 0], -10.0)
+    coords = np.concatenate([base, fut, fut2, fut3])
+    coords = coords[np.lexsort((coords[:, 1], coords[:, 0]))]
+    o_bits = oracle.causal_matrix_bits(coords, inp.GEOM_MINK_CONE)
+    bits, _ = gpu_bits(api, coords, inp.GEOM_MINK_CONE)
+    assert np.array_equal(to_u64(bits), o_bits)
+
+
+def test_degenerate_inputs(api, oracle):
+    # identical points, NaN coordinates, N = 0
+    coords = np.zeros((70, 4)); coords[10:20, 1] = np.nan
+    o_bits = oracle.causal_matrix_bits(coords, inp.GEOM_MINK_CONE)
+    bits, bitsT = gpu_bits(api, coords, inp.GEOM_MINK_CONE)
+    assert np.array_equal(to_u64(bits), o_bits)
+    for r in routes(api):
+        h = api.interval_hist(bits, bitsT, 70, route=r)
+        assert np.array_equal(h.cpu().numpy(), oracle.interval_hist_alg20(o_bits, 70)[0])
+    empty = torch.zeros((0, 2), dtype=torch.float64, device="cuda")
+    b, bT = api.causal_matrix(empty, inp.GEOM_DS2_SLAB)
+    assert b.numel() == 0
+    for N in (0, 1):
+        z = torch.zeros((N, api.row_stride_words(N)), dtype=torch.int64, device="cuda")
+        h = api.interval_hist(z, z, N)
+        assert h.shape == (1,) and int(h[0]) == 0
+        assert float(api.bd_action(h, N, 2)[0]) == 2.0 * N
+
+
+# ----------------------------------------------------------------------------- a2
+@pytest.mark.parametrize("geom,dim", GEOMS)
+@pytest.mark.parametrize("N", [2, 64, 129, 1000, 2048])
+def test_interval_hist_bit_exact(api, oracle, geom, dim, N):
+    coords = inp.sprinkle(geom, dim, N, 7 * N + dim)
+    o_bits = oracle.causal_matrix_bits(coords, geom)
+    if N <= 1000:
+        o_hist = oracle.interval_hist_alg19(oracle.unpack_bits(o_bits, N))      # tier-0
+    else:
+        o_hist, _, _ = oracle.interval_hist_alg20(o_bits, N)                    # tier-1
+    R, W = oracle.count_relations(o_bits, N)
+    bits, bitsT = gpu_bits(api, coords, geom)
+    stats = api.relation_stats(bits, N).cpu().numpy()
+    assert (int(stats[0]), int(stats[1])) == (R, W)
+    for r in routes(api):
+        hist, nrel = api.interval_hist(bits, bitsT, N, route=r, return_relations=True)
+        assert np.array_equal(hist.cpu().numpy(), o_hist), "route %d" % r
+        assert int(nrel[0]) == R
+        # without bitsT (rebuilt in the workspace)
+        assert np.array_equal(api.interval_hist(bits, None, N, route=r).cpu().numpy(), o_hist)
+        # truncated histogram: larger intervals dropped, still counted as relations
+        h3, n3 = api.interval_hist(bits, bitsT, N, kmax=3, route=r, return_relations=True)
+        k = min(3, max(N - 2, 0))
+        assert np.array_equal(h3.cpu().numpy(), o_hist[:k + 1]) and int(n3[0]) == R
+        # row ranges add up
+        cut = N // 3 + 1
+        ha = api.interval_hist(bits, bitsT, N, route=r, row_begin=0, row_end=cut)
+        hb = api.interval_hist(bits, bitsT, N, route=r, row_begin=cut, row_end=N)
+        assert np.array_equal((ha + hb).cpu().numpy(), o_hist)
+        assert np.array_equal(ha.cpu().numpy(), oracle.interval_hist_alg20(o_bits, N, 0, cut)[0])
+
+
+@pytest.mark.parametrize("N", [2, 300, 1025])
+def test_chain_and_antichain_on_gpu(api, N):
+    for r in routes(api):
+        bits, bitsT = gpu_bits(api, inp.chain_lightcone(N), inp.GEOM_MINK2_LIGHTCONE)
+        h = api.interval_hist(bits, bitsT, N, route=r).cpu().numpy()
+        assert np.array_equal(h, np.arange(N - 1, 0, -1))          # N_k = N-1-k
+        bits, bitsT = gpu_bits(api, inp.antichain_lightcone(N), inp.GEOM_MINK2_LIGHTCONE)
+        assert int(api.interval_hist(bits, bitsT, N, route=r).sum()) == 0
+
+
+# ----------------------------------------------------------------------------- a3
+@pytest.mark.parametrize("dim", [2, 3, 4])
+def test_bd_action_matches_oracle(api, oracle, dim):
+    rng = np.random.default_rng(dim)
+    for n_entries in (1, 2, 3, 4, 9):
+        hist = rng.integers(0, 3_000_000_000, n_entries).astype(np.int64)
+        N = 131072
+        S, I = api.bd_action(torch.from_numpy(hist).cuda(), N, dim, return_bracket=True)
+        oS, oI = oracle.bd_action(hist, N, dim)
+        assert int(I[0]) == oI
+        if dim == 3:   # the prefactor needs Gamma and pow: libm vs correctly rounded constant
+            assert float(S[0]) == pytest.approx(oS, rel=1e-15)
+        else:
+            assert float(S[0]) == oS
+
+
+# ----------------------------------------------------------------------------- whole path
+@pytest.mark.parametrize("cfg_index,N", [(1, 1024), (3, 1500), (4, 2000)])
+def test_pipeline_device_and_host_entry(api, oracle, cfg_index, N):
+    cfg = inp.CONFIGS[cfg_index]
+    coords = inp.make_config_coords(cfg, N=N)
+    o_bits, o_hist, o_S, o_I = oracle.action_pipeline(coords, cfg.geometry, tier=0 if N <= 1024 else 1)
+    bits, bitsT = gpu_bits(api, coords, cfg.geometry)
+    hist = api.interval_hist(bits, bitsT, N)
+    S, I = api.bd_action(hist, N, cfg.dim, return_bracket=True)
+    assert np.array_equal(to_u64(bits), o_bits)
+    assert np.array_equal(hist.cpu().numpy(), o_hist)
+    assert int(I[0]) == o_I and float(S[0]) == o_S
+    # the host-buffer entry point (H2D + a1 + a2 + a3 + D2H)
+    h_host, s_host = api.action_host(torch.from_numpy(coords).pin_memory(), cfg.geometry)
+    assert np.array_equal(h_host.numpy(), o_hist) and float(s_host[0]) == o_S
+    h_host3, s3 = api.action_host(torch.from_numpy(coords), cfg.geometry, kmax=3)
+    assert np.array_equal(h_host3.numpy(), o_hist[:4]) and float(s3[0]) == o_S
+
+
+def test_batched_ensemble(api, oracle):
+    cfg = inp.CONFIGS[5]
+    B, N = 6, 2048
+    coords = inp.make_ensemble_coords(cfg, B=B)
+    actions, hist4 = api.bd_action_batched(torch.from_numpy(coords).cuda(), cfg.geometry, return_hist4=True)
+    actions = actions.cpu().numpy(); hist4 = hist4.cpu().numpy()
+    for b in range(B):
+        _, o_hist, o_S, _ = oracle.action_pipeline(coords[b], cfg.geometry, tier=1)
+        assert np.array_equal(hist4[b], o_hist[:4])
+        assert actions[b] == o_S
+    # ragged batched size
+    coords = inp.make_ensemble_coords(cfg, B=3, N=333)
+    actions = api.bd_action_batched(torch.from_numpy(coords).cuda(), cfg.geometry).cpu().numpy()
+    for b in range(3):
+        assert actions[b] == oracle.action_pipeline(coords[b], cfg.geometry)[2]
+
+
+# ----------------------------------------------------------------------------- full sizes
+def _full_size_check(api, oracle, cfg, full_hist):
+    """Bits compared in full; histogram compared in full (tier-1) or on sampled row ranges plus
+    the two moment identities that hold at any size."""
+    N = cfg.N
+    coords = inp.make_config_coords(cfg)
+    o_bits = oracle.causal_matrix_bits(coords, cfg.geometry)
+    bits, bitsT = gpu_bits(api, coords, cfg.geometry)
+    assert np.array_equal(to_u64(bits), o_bits)
+    R, W = oracle.count_relations(o_bits, N)
+    stats = api.relation_stats(bits, N).cpu().numpy()
+    assert (int(stats[0]), int(stats[1])) == (R, W)
+    hist, nrel = api.interval_hist(bits, bitsT, N, return_relations=True)
+    h = hist.cpu().numpy()
+    assert int(nrel[0]) == R and int(h.sum()) == R
+    outdeg, indeg = oracle.degrees(o_bits, N)
+    assert int((np.arange(N - 1, dtype=np.int64) * h).sum()) == int((outdeg * indeg).sum())
+    if full_hist:
+        o_hist, _, _ = oracle.interval_hist_alg20(o_bits, N)
+        assert np.array_equal(h, o_hist)
+    else:
+        rng = np.random.default_rng(cfg.index)
+        for r0 in sorted(rng.integers(0, N - 64, 3).tolist()):
+            part = api.interval_hist(bits, bitsT, N, row_begin=r0, row_end=r0 + 40).cpu().numpy()
+            assert np.array_equal(part, oracle.interval_hist_alg20(o_bits, N, r0, r0 + 40)[0])
+    S, I = api.bd_action(hist, N, cfg.dim, return_bracket=True)
+    oS, oI = oracle.bd_action(h, N, cfg.dim)
+    assert int(I[0]) == oI and float(S[0]) == oS
+
+
+def test_config2_full(api, oracle):
+    _full_size_check(api, oracle, inp.CONFIGS[2], full_hist=True)
+
+
+@pytest.mark.slow
+def test_config3_full_size(api, oracle):
+    _full_size_check(api, oracle, inp.CONFIGS[3], full_hist=False)
+
+
+@pytest.mark.slow
+def test_config4_full_size(api, oracle):
+    _full_size_check(api, oracle, inp.CONFIGS[4], full_hist=False)

@@ -386,3 +386,10 @@ def test_smear_f_against_paper_form(oracle):
 def test_seh_golden():
     eta0, printed, _ = _read_table("ds_slab_seh.txt")[0]
     assert round(4 * math.pi * math.tan(float(eta0)), 3) == float(printed)
+
+
+def test_degrees_helper(oracle):
+    coords = inp.sprinkle(inp.GEOM_MINK_CONE, 3, 333, 21)
+    C = oracle.causal_matrix_bytes(coords, inp.GEOM_MINK_CONE)
+    o, i = oracle.degrees(oracle.pack_bytes(C), 333)
+    assert np.array_equal(o, C.sum(axis=1)) and np.array_equal(i, C.sum(axis=0))
