@@ -188,16 +188,18 @@ void orc_interval_hist_alg19(const uint8_t *C, int64_t N, int64_t *hist)
  * = popcount of (A[i] AND A[j]) restricted to bit positions i..j, everything
  * outside zeroed.  Bits i and j themselves are 0
  * (irreflexive), so the closed range counts exactly the open interval.
- * Restricted to rows i in [row_begin, row_end).  Per-thread histograms, then
- * the reduction of lines 12-14.  *word_ops accumulates the number of 64-bit
- * blocks touched, sum over related pairs of (j>>6)-(i>>6)+1.
+ * Restricted to rows i = row_begin, row_begin+row_step, ... < row_end.
+ * Per-thread histograms, then the reduction of lines 12-14.  *word_ops
+ * accumulates the number of 64-bit blocks touched, sum over related pairs of
+ * (j>>6)-(i>>6)+1; *loop_seconds is the wall time of the pair loop alone (the
+ * paper's linker already delivers the symmetrised matrix).
  */
 static uint64_t orc_mask_from(int b) { return ~(uint64_t)0 << b; }              /* bits b..63 */
 static uint64_t orc_mask_upto(int b) { return ~(uint64_t)0 >> (63 - b); }       /* bits 0..b  */
 
 int orc_interval_hist_alg20(const uint64_t *bits, int64_t N, int64_t stride,
-                            int64_t row_begin, int64_t row_end,
-                            int64_t *hist, int64_t *word_ops, int nthreads)
+                            int64_t row_begin, int64_t row_end, int64_t row_step,
+                            int64_t *hist, int64_t *word_ops, double *loop_seconds, int nthreads)
 {
     if (N < 0 || stride * 64 < N) return -1;
     int64_t nh = N > 1 ? N - 1 : 0;
@@ -206,6 +208,8 @@ int orc_interval_hist_alg20(const uint64_t *bits, int64_t N, int64_t stride,
     if (N < 2) return 0;
     if (row_begin < 0) row_begin = 0;
     if (row_end > N) row_end = N;
+    if (row_step < 1) row_step = 1;
+    if (loop_seconds) *loop_seconds = 0.0;
 
     /* A = P + P^T */
     uint64_t *A = (uint64_t *)malloc((size_t)N * (size_t)stride * sizeof(uint64_t));
@@ -223,8 +227,11 @@ int orc_interval_hist_alg20(const uint64_t *bits, int64_t N, int64_t stride,
     int64_t *wops = (int64_t *)calloc((size_t)T, sizeof(int64_t));
     if (!n || !wops) { free(A); free(n); free(wops); return -2; }
 
+#ifdef _OPENMP
+    double t0 = omp_get_wtime();
+#endif
 #pragma omp parallel for schedule(dynamic, 1) num_threads(T)
-    for (int64_t i = row_begin; i < row_end; i++) {
+    for (int64_t i = row_begin; i < row_end; i += row_step) {
 #ifdef _OPENMP
         int t = omp_get_thread_num();
 #else
@@ -248,6 +255,9 @@ int orc_interval_hist_alg20(const uint64_t *bits, int64_t N, int64_t stride,
             wops[t] += y - x + 1;
         }
     }
+#ifdef _OPENMP
+    if (loop_seconds) *loop_seconds = omp_get_wtime() - t0;
+#endif
     for (int t = 0; t < T; t++) {
         for (int64_t m = 0; m < nh; m++) hist[m] += n[(int64_t)t * nh + m];
         if (word_ops) *word_ops += wops[t];

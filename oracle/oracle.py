@@ -59,7 +59,7 @@ def _load():
         lib.orc_interval_hist_alg19.restype = None
         lib.orc_interval_hist_alg19.argtypes = [_p, _i64, _p]
         lib.orc_interval_hist_alg20.restype = ctypes.c_int
-        lib.orc_interval_hist_alg20.argtypes = [_p, _i64, _i64, _i64, _i64, _p, _p, ctypes.c_int]
+        lib.orc_interval_hist_alg20.argtypes = [_p, _i64, _i64, _i64, _i64, _i64, _p, _p, _p, ctypes.c_int]
         lib.orc_count_relations.restype = None
         lib.orc_count_relations.argtypes = [_p, _i64, _i64, _p, _p]
         lib.orc_bd_action.restype = ctypes.c_double
@@ -161,14 +161,18 @@ def interval_hist_alg19(C: np.ndarray) -> np.ndarray:
 
 
 def interval_hist_alg20(bits: np.ndarray, N: int, row_begin: int = 0, row_end: int | None = None,
-                        nthreads: int = 0):
-    """Tier-1: Algorithm 20 on bit rows.  Returns (hist[0..N-2], word_ops, threads)."""
+                        nthreads: int = 0, row_step: int = 1, timing: dict | None = None):
+    """Tier-1: Algorithm 20 on bit rows i = row_begin, row_begin+row_step, ... < row_end.
+    Returns (hist[0..N-2], word_ops, threads); timing["loop_seconds"] gets the pair-loop wall time."""
     bits = np.ascontiguousarray(bits, dtype=np.uint64)
     row_end = N if row_end is None else row_end
     hist = np.zeros(max(N - 1, 0), dtype=np.int64)
     wops = np.zeros(1, dtype=np.int64)
-    T = _load().orc_interval_hist_alg20(_ptr(bits), N, bits.shape[1], row_begin, row_end,
-                                        _ptr(hist), _ptr(wops), nthreads)
+    secs = ctypes.c_double(0.0)
+    T = _load().orc_interval_hist_alg20(_ptr(bits), N, bits.shape[1], row_begin, row_end, row_step,
+                                        _ptr(hist), _ptr(wops), ctypes.byref(secs), nthreads)
+    if timing is not None:
+        timing["loop_seconds"] = secs.value
     if T < 0:
         raise RuntimeError("oracle: alg20 failed (%d)" % T)
     return hist, int(wops[0]), int(T)
