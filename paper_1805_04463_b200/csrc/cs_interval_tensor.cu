@@ -1,14 +1,372 @@
-// cs_interval_tensor.cu -- stage a2, tensor route (placeholder until the tcgen05 kernel lands).
+// cs_interval_tensor.cu -- stage a2, tensor route: the count matrix C = U . U as a genuine dense
+// 0/1 contraction on the 5th-generation tensor cores (tcgen05.mma kind::i8, accumulators in TMEM).
+//
+//   count(i,j) = |{k : i -< k -< j}| = sum_k U[i][k] * L[j][k],   U = bits ("future of i"),
+//                                                                  L = bitsT ("past of j"),
+// which is exactly the paper's inner product of rows i and j between columns i and j
+// (Fig. 4.2 caption PAPER.md:1768; Alg. 20 line 9) with AND/popcount replaced by an
+// integer multiply-accumulate.  Only K blocks between the I block and the J block are visited.
+//
+// Operands never exist as bytes in HBM: the bit rows are read from global memory (16 bytes = 128
+// k per row per k-step) and expanded in registers straight into the shared-memory layout the MMA
+// reads (no-swizzle K-major canonical layout: [16-byte k chunk][row][16 B]; SBO = 128 B,
+// LBO = rows*16 B).  A bit becomes the byte 0x80 (u8 128): with x a 32-bit slice of the row,
+// output word m = (x << (7-m)) & 0x80808080, i.e. byte p = 4m+b of the 32-byte K slice holds bit
+// m+8b.  That is a fixed permutation of k inside each 32-wide slice, applied identically to both
+// operands, so the sum over k is unchanged and the expansion costs one shift and one AND per
+// four bytes.  Every match contributes 128*128 = 2^14; the int32 accumulator holds count * 2^14
+// exactly for counts < 2^17 (N <= 131072; checked by the launcher), and count = acc >> 14.
+//
+// CTA = one SM (512 TMEM columns), persistent over 128 x 256 tiles (rows i x rows j), 17 warps:
+//   warps 0-3   epilogue: tcgen05.ld the accumulator rows, test the relation bit U[i][j], update the
+//               shared-memory histogram (global atomics for rare large intervals)
+//   warp  4     TMEM allocation + the single MMA-issuing thread
+//   warps 5-16  expanders: 384 threads, one operand row each (128 rows of U, 256 rows of L)
+// Pipelines: NS shared-memory stages (full/empty mbarriers; the MMA warp releases a stage with
+// tcgen05.commit), two TMEM accumulator buffers (tmem_full / tmem_empty).
 #include "cs_common.cuh"
 
 namespace cs {
 
-bool interval_tensor_available() { return false; }
-size_t interval_tensor_scratch_bytes(int64_t, int64_t) { return 0; }
-int launch_interval_tensor(const uint64_t *, const uint64_t *, int64_t, int64_t, int64_t, int64_t, int64_t,
-                           int64_t *, int64_t *, void *, size_t, cudaStream_t)
+namespace {
+
+constexpr int TM = 128;                 // tile rows i (MMA M)
+constexpr int TN = 256;                 // tile rows j (MMA N)
+constexpr int KSTEP = 128;              // k per stage = 128 bytes of int8 = 4 MMAs of K = 32
+constexpr int NS = 4;                   // shared-memory stages
+constexpr int A_BYTES = TM * KSTEP;     // 16 KiB
+constexpr int B_BYTES = TN * KSTEP;     // 32 KiB
+constexpr int STAGE_BYTES = A_BYTES + B_BYTES;
+constexpr int HS = 2048;                // shared-memory histogram bins
+constexpr int EPI_WARPS = 4, MMA_WARP = 4, EXP_WARP0 = 5, EXP_WARPS = 12;
+constexpr int THREADS = (EPI_WARPS + 1 + EXP_WARPS) * 32;   // 544
+constexpr int EXP_THREADS = EXP_WARPS * 32;                 // 384 = TM + TN
+constexpr int SMEM_BYTES = NS * STAGE_BYTES + HS * 4 + 256 + 1024;
+constexpr int SCALE_SHIFT = 14;         // every match adds 128 * 128
+
+static_assert(EXP_THREADS == TM + TN, "one expander thread per operand row");
+
+// instruction descriptor, kind::i8: D = S32 (2 at bit 4), A = B = U8 (0), both K-major,
+// N >> 3 at bit 17, M >> 4 at bit 24
+constexpr uint32_t IDESC = (2u << 4) | ((uint32_t)(TN >> 3) << 17) | ((uint32_t)(TM >> 4) << 24);
+
+__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(uint64_t *bar, uint32_t count)
 {
-    return CS_ERR_ARG;
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t *bar)
+{
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity)
+{
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "LAB_WAIT:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra LAB_DONE;\n"
+        "bra LAB_WAIT;\n"
+        "LAB_DONE:\n"
+        "}\n" ::"r"(smem_u32(bar)),
+        "r"(parity)
+        : "memory");
+}
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+__device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
+
+// shared-memory matrix descriptor: no swizzle, K-major; addresses and offsets in 16-byte units
+__device__ __forceinline__ uint64_t make_desc(uint32_t saddr, uint32_t lbo_bytes, uint32_t sbo_bytes)
+{
+    uint64_t d = 0;
+    d |= (uint64_t)((saddr >> 4) & 0x3FFF);
+    d |= (uint64_t)((lbo_bytes >> 4) & 0x3FFF) << 16;
+    d |= (uint64_t)((sbo_bytes >> 4) & 0x3FFF) << 32;
+    d |= (uint64_t)1 << 46;   // descriptor version (Blackwell)
+    return d;                 // layout_type = 0 (SWIZZLE_NONE), base_offset = 0, lbo_mode = 0
+}
+
+__device__ __forceinline__ void mma_i8(uint32_t d_tmem, uint64_t adesc, uint64_t bdesc, uint32_t idesc, uint32_t accum)
+{
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "setp.ne.b32 p, %4, 0;\n"
+        "tcgen05.mma.cta_group::1.kind::i8 [%0], %1, %2, %3, p;\n"
+        "}\n" ::"r"(d_tmem),
+        "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accum)
+        : "memory");
+}
+__device__ __forceinline__ void mma_commit(uint64_t *bar)
+{
+    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(smem_u32(bar))
+                 : "memory");
+}
+
+__device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t (&v)[32])
+{
+    asm volatile(
+        "tcgen05.ld.sync.aligned.32x32b.x32.b32 "
+        "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, "
+        "%16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31}, [%32];\n"
+        : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]),
+          "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15]),
+          "=r"(v[16]), "=r"(v[17]), "=r"(v[18]), "=r"(v[19]), "=r"(v[20]), "=r"(v[21]), "=r"(v[22]), "=r"(v[23]),
+          "=r"(v[24]), "=r"(v[25]), "=r"(v[26]), "=r"(v[27]), "=r"(v[28]), "=r"(v[29]), "=r"(v[30]), "=r"(v[31])
+        : "r"(taddr)
+        : "memory");
+    asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+}
+
+struct Tile {
+    int I, J;   // 128-row block of i, 256-row block of j
+};
+// tiles of one causet ordered by decreasing number of k-steps (2J + 2 - I); nTJ(nTJ+1) tiles
+__device__ __forceinline__ Tile tile_from_index(int64_t t, int nTJ)
+{
+    int64_t q = (int64_t)((sqrt(4.0 * (double)t + 1.0) - 1.0) * 0.5);
+    while ((q + 1) * (q + 2) <= t) q++;
+    while (q * (q + 1) > t) q--;
+    const int r = (int)(t - q * (q + 1));
+    const int p = nTJ - 1 - (int)q;
+    if (r < (int)q + 1) return Tile{2 * r, p + r};                 // d = 2p+1
+    const int idx = r - ((int)q + 1);
+    return Tile{2 * idx + 1, p + idx};                             // d = 2p
+}
+
+__global__ void __launch_bounds__(THREADS, 1)
+k_interval_tensor(const uint64_t *__restrict__ bits, const uint64_t *__restrict__ bitsT,
+                  int64_t B, int64_t N, int64_t stride, int64_t kmax,
+                  int64_t row_begin, int64_t row_end,
+                  unsigned long long *__restrict__ hist, unsigned long long *__restrict__ nrel)
+{
+    extern __shared__ unsigned char smem_raw[];
+    unsigned char *smem = reinterpret_cast<unsigned char *>(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
+    unsigned char *s_stage = smem;
+    uint32_t *s_hist = reinterpret_cast<uint32_t *>(smem + NS * STAGE_BYTES);
+    uint64_t *s_full = reinterpret_cast<uint64_t *>(smem + NS * STAGE_BYTES + HS * 4);
+    uint64_t *s_empty = s_full + NS;
+    uint64_t *s_tfull = s_empty + NS;     // [2]
+    uint64_t *s_tempty = s_tfull + 2;     // [2]
+    uint32_t *s_tmem = reinterpret_cast<uint32_t *>(s_tempty + 2);
+    unsigned long long *s_nrel = reinterpret_cast<unsigned long long *>(s_tmem + 2);
+
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const int nTJ = (int)((N + TN - 1) / TN);
+    const int64_t tiles_per = (int64_t)nTJ * (nTJ + 1);
+    const int64_t total_tiles = tiles_per * B;
+    const int hs = (int)((kmax + 1 < HS) ? (kmax + 1) : HS);
+    const int64_t hist_len = kmax + 1;
+
+    if (tid == 0) {
+        for (int s = 0; s < NS; s++) {
+            mbar_init(&s_full[s], EXP_THREADS);
+            mbar_init(&s_empty[s], 1);
+        }
+        for (int a = 0; a < 2; a++) {
+            mbar_init(&s_tfull[a], 1);
+            mbar_init(&s_tempty[a], EPI_WARPS * 32);
+        }
+        *s_nrel = 0;
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    for (int b = tid; b < HS; b += THREADS) s_hist[b] = 0;
+    if (warp == MMA_WARP) {   // allocate all 512 TMEM columns (one CTA per SM by shared-memory size)
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 512;" ::"r"(smem_u32(s_tmem)));
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
+    }
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    const uint32_t tmem_base = *s_tmem;
+
+    // every role walks the same static schedule: tile t = blockIdx.x, + gridDim.x, ...
+    if (warp >= EXP_WARP0) {
+        // ===================================== expanders =====================================
+        const int e = tid - EXP_WARP0 * 32;
+        const bool isA = e < TM;
+        const int r = isA ? e : e - TM;
+        const uint32_t rows = isA ? TM : TN;
+        uint32_t it = 0;   // global k-step counter (stage ring position)
+        for (int64_t t = blockIdx.x; t < total_tiles; t += gridDim.x) {
+            const int64_t bidx = t / tiles_per;
+            const Tile tc = tile_from_index(t - bidx * tiles_per, nTJ);
+            if ((int64_t)tc.I * TM >= row_end || (int64_t)(tc.I + 1) * TM <= row_begin) continue;
+            const int64_t grow = isA ? (int64_t)tc.I * TM + r : (int64_t)tc.J * TN + r;
+            const uint64_t *src = (isA ? bits : bitsT) + bidx * N * stride + grow * stride;
+            const bool row_ok = grow < N;
+            const int ks0 = tc.I, ks1 = 2 * tc.J + 1;            // inclusive k-step range
+            const int64_t max_ks = stride / 2;                    // 16-byte chunks per row
+            auto load = [&](int ks) -> uint4 {
+                if (row_ok && ks <= ks1 && ks < max_ks) return __ldg(reinterpret_cast<const uint4 *>(src) + ks);
+                return make_uint4(0u, 0u, 0u, 0u);
+            };
+            uint4 nxt0 = load(ks0), nxt1 = load(ks0 + 1);
+            for (int ks = ks0; ks <= ks1; ks++, it++) {
+                const uint4 cur = nxt0;
+                nxt0 = nxt1;
+                nxt1 = load(ks + 2);
+                const int s = it % NS;
+                mbar_wait(&s_empty[s], ((it / NS) & 1) ^ 1);
+                unsigned char *dst = s_stage + s * STAGE_BYTES + (isA ? 0 : A_BYTES) + r * 16;
+                const uint32_t xs[4] = {cur.x, cur.y, cur.z, cur.w};
+#pragma unroll
+                for (int q = 0; q < 4; q++) {
+                    const uint32_t x = xs[q];
+                    uint4 lo, hi;
+                    lo.x = (x << 7) & 0x80808080u;
+                    lo.y = (x << 6) & 0x80808080u;
+                    lo.z = (x << 5) & 0x80808080u;
+                    lo.w = (x << 4) & 0x80808080u;
+                    hi.x = (x << 3) & 0x80808080u;
+                    hi.y = (x << 2) & 0x80808080u;
+                    hi.z = (x << 1) & 0x80808080u;
+                    hi.w = x & 0x80808080u;
+                    *reinterpret_cast<uint4 *>(dst + (2 * q) * rows * 16) = lo;
+                    *reinterpret_cast<uint4 *>(dst + (2 * q + 1) * rows * 16) = hi;
+                }
+                fence_proxy_async();          // generic-proxy stores -> visible to the tensor core
+                mbar_arrive(&s_full[s]);
+            }
+        }
+    } else if (warp == MMA_WARP) {
+        // ===================================== MMA issuer ====================================
+        if (lane == 0) {
+            uint32_t it = 0, tile_seq = 0;
+            for (int64_t t = blockIdx.x; t < total_tiles; t += gridDim.x) {
+                const int64_t bidx = t / tiles_per;
+                const Tile tc = tile_from_index(t - bidx * tiles_per, nTJ);
+                if ((int64_t)tc.I * TM >= row_end || (int64_t)(tc.I + 1) * TM <= row_begin) continue;
+                const int ks0 = tc.I, ks1 = 2 * tc.J + 1;
+                const uint32_t a = tile_seq & 1;
+                mbar_wait(&s_tempty[a], ((tile_seq >> 1) & 1) ^ 1);      // epilogue has drained buffer a
+                tc_fence_after();
+                const uint32_t d_tmem = tmem_base + a * TN;
+                for (int ks = ks0; ks <= ks1; ks++, it++) {
+                    const int s = it % NS;
+                    mbar_wait(&s_full[s], (it / NS) & 1);
+                    tc_fence_after();
+                    const uint32_t a_addr = smem_u32(s_stage + s * STAGE_BYTES);
+                    const uint32_t b_addr = a_addr + A_BYTES;
+#pragma unroll
+                    for (int q = 0; q < KSTEP / 32; q++) {
+                        const uint64_t ad = make_desc(a_addr + q * 2 * TM * 16, TM * 16, 128);
+                        const uint64_t bd = make_desc(b_addr + q * 2 * TN * 16, TN * 16, 128);
+                        mma_i8(d_tmem, ad, bd, IDESC, (ks > ks0 || q > 0) ? 1u : 0u);
+                    }
+                    mma_commit(&s_empty[s]);                              // stage s free once these MMAs retire
+                }
+                mma_commit(&s_tfull[a]);                                  // accumulator complete
+                tile_seq++;
+            }
+        }
+    } else {
+        // ===================================== epilogue ======================================
+        uint32_t tile_seq = 0;
+        unsigned long long my_nrel = 0;
+        int64_t cur_batch = -1;
+        for (int64_t t = blockIdx.x; t < total_tiles; t += gridDim.x) {
+            const int64_t bidx = t / tiles_per;
+            const Tile tc = tile_from_index(t - bidx * tiles_per, nTJ);
+            if ((int64_t)tc.I * TM >= row_end || (int64_t)(tc.I + 1) * TM <= row_begin) continue;
+            if (bidx != cur_batch) {   // per-causet histograms: flush before switching
+                if (cur_batch >= 0 && B > 1) {
+                    asm volatile("bar.sync 1, 128;");
+                    for (int b = tid; b < hs; b += EPI_WARPS * 32) {
+                        uint32_t v = s_hist[b];
+                        if (v) { atomicAdd(&hist[cur_batch * hist_len + b], (unsigned long long)v); s_hist[b] = 0; }
+                    }
+                    asm volatile("bar.sync 1, 128;");
+                }
+                cur_batch = bidx;
+            }
+            const int64_t i = (int64_t)tc.I * TM + tid;          // this thread's row = TMEM lane
+            const bool row_ok = i < N && i >= row_begin && i < row_end;
+            uint64_t rel[4] = {0, 0, 0, 0};
+            if (row_ok) {
+                const uint64_t *urow = bits + bidx * N * stride + i * stride;
+#pragma unroll
+                for (int w = 0; w < 4; w++) {
+                    const int64_t wi = (int64_t)tc.J * 4 + w;
+                    if (wi < stride) rel[w] = __ldg(urow + wi);
+                }
+            }
+            const uint32_t a = tile_seq & 1;
+            mbar_wait(&s_tfull[a], (tile_seq >> 1) & 1);
+            tc_fence_after();
+            const uint32_t taddr = tmem_base + ((uint32_t)(warp * 32) << 16) + a * TN;
+#pragma unroll 1
+            for (int c8 = 0; c8 < TN / 32; c8++) {
+                const uint32_t rel32 = (uint32_t)(rel[c8 >> 1] >> (32 * (c8 & 1)));
+                if (!__any_sync(0xffffffffu, rel32 != 0)) continue;
+                uint32_t v[32];
+                tmem_ld32(taddr + c8 * 32, v);
+                if (rel32 == 0) continue;
+                my_nrel += __popc(rel32);
+#pragma unroll
+                for (int c = 0; c < 32; c++) {
+                    if (rel32 & (1u << c)) {
+                        const uint32_t cnt = v[c] >> SCALE_SHIFT;
+                        if (cnt < (uint32_t)hs) atomicAdd(&s_hist[cnt], 1u);
+                        else if ((int64_t)cnt <= kmax) atomicAdd(&hist[cur_batch * hist_len + cnt], 1ULL);
+                    }
+                }
+            }
+            tc_fence_before();
+            mbar_arrive(&s_tempty[a]);
+            tile_seq++;
+        }
+        // final flush by the epilogue warps
+        asm volatile("bar.sync 1, 128;");
+        if (cur_batch >= 0) {
+            for (int b = tid; b < hs; b += EPI_WARPS * 32) {
+                uint32_t v = s_hist[b];
+                if (v) atomicAdd(&hist[cur_batch * hist_len + b], (unsigned long long)v);
+            }
+        }
+        if (nrel && B == 1) {
+#pragma unroll
+            for (int s = 16; s >= 1; s >>= 1) my_nrel += __shfl_xor_sync(0xffffffffu, my_nrel, s);
+            if (lane == 0 && my_nrel) atomicAdd(nrel, my_nrel);
+        }
+    }
+
+    tc_fence_before();
+    __syncthreads();
+    if (warp == MMA_WARP) {
+        asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 512;" ::"r"(tmem_base));
+    }
+}
+
+}  // namespace
+
+bool interval_tensor_available() { return true; }
+size_t interval_tensor_scratch_bytes(int64_t, int64_t) { return 0; }
+
+int launch_interval_tensor(const uint64_t *bits, const uint64_t *bitsT, int64_t B, int64_t N, int64_t kmax,
+                           int64_t row_begin, int64_t row_end, int64_t *hist, int64_t *nrel,
+                           void *, size_t, cudaStream_t st)
+{
+    if (N > ((int64_t)1 << 17)) return CS_ERR_ARG;   // count * 2^14 must stay below 2^31
+    static bool attr_set = false;
+    if (!attr_set) {
+        CS_CUDA(cudaFuncSetAttribute(k_interval_tensor, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES));
+        attr_set = true;
+    }
+    const int64_t stride = row_stride_words(N);
+    const int64_t nTJ = (N + TN - 1) / TN;
+    const int64_t total = nTJ * (nTJ + 1) * B;
+    int64_t grid = sm_count();
+    if (grid > total) grid = total;
+    if (grid < 1) grid = 1;
+    k_interval_tensor<<<(unsigned)grid, THREADS, SMEM_BYTES, st>>>(
+        bits, bitsT, B, N, stride, kmax, row_begin, row_end,
+        reinterpret_cast<unsigned long long *>(hist), reinterpret_cast<unsigned long long *>(nrel));
+    CS_LAUNCHED("k_interval_tensor");
+    return CS_OK;
 }
 
 }  // namespace cs
