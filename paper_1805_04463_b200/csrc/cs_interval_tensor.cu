@@ -17,13 +17,17 @@
 // four bytes.  Every match contributes 128*128 = 2^14; the int32 accumulator holds count * 2^14
 // exactly for counts < 2^17 (N <= 131072; checked by the launcher), and count = acc >> 14.
 //
-// CTA = one SM (512 TMEM columns), persistent over 128 x 256 tiles (rows i x rows j), 17 warps:
+// CTA = one SM (512 TMEM columns), persistent over 128 x 256 tiles (rows i x rows j), 18 warps:
 //   warps 0-3   epilogue: tcgen05.ld the accumulator rows, test the relation bit U[i][j], update the
 //               shared-memory histogram (global atomics for rare large intervals)
 //   warp  4     TMEM allocation + the single MMA-issuing thread
-//   warps 5-16  expanders: 384 threads, one operand row each (128 rows of U, 256 rows of L)
-// Pipelines: NS shared-memory stages (full/empty mbarriers; the MMA warp releases a stage with
-// tcgen05.commit), two TMEM accumulator buffers (tmem_full / tmem_empty).
+//   warp  5     loader: one thread issues the TMA tensor copies (cp.async.bulk.tensor, 64B swizzle)
+//               that stage the bit rows, GK k-steps (64 bytes per row) at a time
+//   warps 6-17  expanders: 384 threads, one operand row each (128 rows of U, 256 rows of L)
+// Pipelines: NB bit-row buffers (bfull/bempty), NS shared-memory operand stages (full/empty; the
+// MMA warp releases a stage with tcgen05.commit), two TMEM accumulator buffers (tfull/tempty).
+#include <cuda.h>
+
 #include "cs_common.cuh"
 
 namespace cs {
@@ -33,18 +37,25 @@ namespace {
 constexpr int TM = 128;                 // tile rows i (MMA M)
 constexpr int TN = 256;                 // tile rows j (MMA N)
 constexpr int KSTEP = 128;              // k per stage = 128 bytes of int8 = 4 MMAs of K = 32
-constexpr int NS = 4;                   // shared-memory stages
+constexpr int NS = 3;                   // shared-memory stages of expanded operands
+constexpr int GK = 4;                   // k-steps per staged group of bit rows (64 bytes per row)
+constexpr int BROW = GK * 16;           // bytes per staged bit row (TMA box inner extent, 64B swizzle)
+constexpr int NB = 3;                   // bit-row buffers
+constexpr int BITS_BYTES = (TM + TN) * BROW;
 constexpr int A_BYTES = TM * KSTEP;     // 16 KiB
 constexpr int B_BYTES = TN * KSTEP;     // 32 KiB
 constexpr int STAGE_BYTES = A_BYTES + B_BYTES;
 constexpr int HS = 2048;                // shared-memory histogram bins
-constexpr int EPI_WARPS = 4, MMA_WARP = 4, EXP_WARP0 = 5, EXP_WARPS = 12;
-constexpr int THREADS = (EPI_WARPS + 1 + EXP_WARPS) * 32;   // 544
+constexpr int EPI_WARPS = 4, MMA_WARP = 4, LOAD_WARP = 5, EXP_WARP0 = 6, EXP_WARPS = 12;
+constexpr int THREADS = (EPI_WARPS + 2 + EXP_WARPS) * 32;   // 576
 constexpr int EXP_THREADS = EXP_WARPS * 32;                 // 384 = TM + TN
-constexpr int SMEM_BYTES = NS * STAGE_BYTES + HS * 4 + 256 + 1024;
+constexpr int SMEM_BYTES = NS * STAGE_BYTES + NB * BITS_BYTES + HS * 4 + 256;
 constexpr int SCALE_SHIFT = 14;         // every match adds 128 * 128
 
 static_assert(EXP_THREADS == TM + TN, "one expander thread per operand row");
+// a thread may run at most NS k-steps ahead of the slowest warp; keeping that below one group keeps
+// every thread within one phase of the bit-buffer barriers
+static_assert(NS <= GK, "stage ring must not outrun a bit-row group");
 
 // instruction descriptor, kind::i8: D = S32 (2 at bit 4), A = B = U8 (0), both K-major,
 // N >> 3 at bit 17, M >> 4 at bit 24
@@ -72,6 +83,18 @@ __device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity)
         "LAB_DONE:\n"
         "}\n" ::"r"(smem_u32(bar)),
         "r"(parity)
+        : "memory");
+}
+__device__ __forceinline__ void mbar_arrive_expect_tx(uint64_t *bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void tma_load_3d(void *dst, const CUtensorMap *map, int c0, int c1, int c2, uint64_t *bar)
+{
+    asm volatile(
+        "cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];" ::"r"(
+            smem_u32(dst)),
+        "l"(map), "r"(c0), "r"(c1), "r"(c2), "r"(smem_u32(bar))
         : "memory");
 }
 __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
@@ -138,20 +161,23 @@ __device__ __forceinline__ Tile tile_from_index(int64_t t, int nTJ)
 }
 
 __global__ void __launch_bounds__(THREADS, 1)
-k_interval_tensor(const uint64_t *__restrict__ bits, const uint64_t *__restrict__ bitsT,
+k_interval_tensor(const __grid_constant__ CUtensorMap mapU, const __grid_constant__ CUtensorMap mapL,
+                  const uint64_t *__restrict__ bits,
                   int64_t B, int64_t N, int64_t stride, int64_t kmax,
                   int64_t row_begin, int64_t row_end,
                   unsigned long long *__restrict__ hist, unsigned long long *__restrict__ nrel)
 {
-    extern __shared__ unsigned char smem_raw[];
-    unsigned char *smem = reinterpret_cast<unsigned char *>(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
+    extern __shared__ __align__(1024) unsigned char smem[];   // typed shared base: STS/ATOMS, not generic
     unsigned char *s_stage = smem;
-    uint32_t *s_hist = reinterpret_cast<uint32_t *>(smem + NS * STAGE_BYTES);
-    uint64_t *s_full = reinterpret_cast<uint64_t *>(smem + NS * STAGE_BYTES + HS * 4);
+    unsigned char *s_bits = smem + NS * STAGE_BYTES;
+    uint32_t *s_hist = reinterpret_cast<uint32_t *>(smem + NS * STAGE_BYTES + NB * BITS_BYTES);
+    uint64_t *s_full = reinterpret_cast<uint64_t *>(smem + NS * STAGE_BYTES + NB * BITS_BYTES + HS * 4);
     uint64_t *s_empty = s_full + NS;
     uint64_t *s_tfull = s_empty + NS;     // [2]
     uint64_t *s_tempty = s_tfull + 2;     // [2]
-    uint32_t *s_tmem = reinterpret_cast<uint32_t *>(s_tempty + 2);
+    uint64_t *s_bfull = s_tempty + 2;     // [NB] staged bit rows have landed
+    uint64_t *s_bempty = s_bfull + NB;    // [NB] every expander warp is done with the buffer
+    uint32_t *s_tmem = reinterpret_cast<uint32_t *>(s_bempty + NB);
     unsigned long long *s_nrel = reinterpret_cast<unsigned long long *>(s_tmem + 2);
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
@@ -163,8 +189,12 @@ k_interval_tensor(const uint64_t *__restrict__ bits, const uint64_t *__restrict_
 
     if (tid == 0) {
         for (int s = 0; s < NS; s++) {
-            mbar_init(&s_full[s], EXP_THREADS);
+            mbar_init(&s_full[s], EXP_WARPS);
             mbar_init(&s_empty[s], 1);
+        }
+        for (int b = 0; b < NB; b++) {
+            mbar_init(&s_bfull[b], 1);
+            mbar_init(&s_bempty[b], EXP_WARPS);
         }
         for (int a = 0; a < 2; a++) {
             mbar_init(&s_tfull[a], 1);
@@ -191,45 +221,71 @@ k_interval_tensor(const uint64_t *__restrict__ bits, const uint64_t *__restrict_
         const int r = isA ? e : e - TM;
         const uint32_t rows = isA ? TM : TN;
         uint32_t it = 0;   // global k-step counter (stage ring position)
+        uint32_t grp = 0;  // global group counter (bit-buffer ring position)
+        // TMA 64B swizzle: 16-byte chunk c of row e sits at chunk c ^ ((e >> 1) & 3)
+        const unsigned char *my_bits = s_bits + (isA ? 0 : TM * BROW) + r * BROW;
+        const int swz = (r >> 1) & 3;
         for (int64_t t = blockIdx.x; t < total_tiles; t += gridDim.x) {
             const int64_t bidx = t / tiles_per;
             const Tile tc = tile_from_index(t - bidx * tiles_per, nTJ);
             if ((int64_t)tc.I * TM >= row_end || (int64_t)(tc.I + 1) * TM <= row_begin) continue;
-            const int64_t grow = isA ? (int64_t)tc.I * TM + r : (int64_t)tc.J * TN + r;
-            const uint64_t *src = (isA ? bits : bitsT) + bidx * N * stride + grow * stride;
-            const bool row_ok = grow < N;
             const int ks0 = tc.I, ks1 = 2 * tc.J + 1;            // inclusive k-step range
-            const int64_t max_ks = stride / 2;                    // 16-byte chunks per row
-            auto load = [&](int ks) -> uint4 {
-                if (row_ok && ks <= ks1 && ks < max_ks) return __ldg(reinterpret_cast<const uint4 *>(src) + ks);
-                return make_uint4(0u, 0u, 0u, 0u);
-            };
-            uint4 nxt0 = load(ks0), nxt1 = load(ks0 + 1);
-            for (int ks = ks0; ks <= ks1; ks++, it++) {
-                const uint4 cur = nxt0;
-                nxt0 = nxt1;
-                nxt1 = load(ks + 2);
-                const int s = it % NS;
-                mbar_wait(&s_empty[s], ((it / NS) & 1) ^ 1);
-                unsigned char *dst = s_stage + s * STAGE_BYTES + (isA ? 0 : A_BYTES) + r * 16;
-                const uint32_t xs[4] = {cur.x, cur.y, cur.z, cur.w};
+            const int ngroups = (ks1 - ks0 + GK) / GK;
+            for (int g = 0; g < ngroups; g++, grp++) {
+                const int b = grp % NB;
+                mbar_wait(&s_bfull[b], (grp / NB) & 1);
+                const int kcount = (ks1 - (ks0 + g * GK) + 1 < GK) ? (ks1 - (ks0 + g * GK) + 1) : GK;
+                for (int c = 0; c < kcount; c++, it++) {
+                    const uint4 cur = *reinterpret_cast<const uint4 *>(my_bits + b * BITS_BYTES + ((c ^ swz) << 4));
+                    const int s = it % NS;
+                    mbar_wait(&s_empty[s], ((it / NS) & 1) ^ 1);
+                    unsigned char *dst = s_stage + s * STAGE_BYTES + (isA ? 0 : A_BYTES) + r * 16;
+                    const uint32_t xs[4] = {cur.x, cur.y, cur.z, cur.w};
 #pragma unroll
-                for (int q = 0; q < 4; q++) {
-                    const uint32_t x = xs[q];
-                    uint4 lo, hi;
-                    lo.x = (x << 7) & 0x80808080u;
-                    lo.y = (x << 6) & 0x80808080u;
-                    lo.z = (x << 5) & 0x80808080u;
-                    lo.w = (x << 4) & 0x80808080u;
-                    hi.x = (x << 3) & 0x80808080u;
-                    hi.y = (x << 2) & 0x80808080u;
-                    hi.z = (x << 1) & 0x80808080u;
-                    hi.w = x & 0x80808080u;
-                    *reinterpret_cast<uint4 *>(dst + (2 * q) * rows * 16) = lo;
-                    *reinterpret_cast<uint4 *>(dst + (2 * q + 1) * rows * 16) = hi;
+                    for (int q = 0; q < 4; q++) {
+                        const uint32_t x = xs[q];
+                        uint4 lo, hi;
+                        lo.x = (x << 7) & 0x80808080u;
+                        lo.y = (x << 6) & 0x80808080u;
+                        lo.z = (x << 5) & 0x80808080u;
+                        lo.w = (x << 4) & 0x80808080u;
+                        hi.x = (x << 3) & 0x80808080u;
+                        hi.y = (x << 2) & 0x80808080u;
+                        hi.z = (x << 1) & 0x80808080u;
+                        hi.w = x & 0x80808080u;
+                        *reinterpret_cast<uint4 *>(dst + (2 * q) * rows * 16) = lo;
+                        *reinterpret_cast<uint4 *>(dst + (2 * q + 1) * rows * 16) = hi;
+                    }
+                    fence_proxy_async();          // generic-proxy stores -> visible to the tensor core
+                    __syncwarp();
+                    if (lane == 0) {
+                        mbar_arrive(&s_full[s]);                          // one arrival per warp
+                        // last chunk of the buffer has been loaded AND consumed by every lane (the
+                        // stores above depend on it): hand the bit buffer back to the loader
+                        if (c == kcount - 1) mbar_arrive(&s_bempty[b]);
+                    }
                 }
-                fence_proxy_async();          // generic-proxy stores -> visible to the tensor core
-                mbar_arrive(&s_full[s]);
+            }
+        }
+    } else if (warp == LOAD_WARP) {
+        // ===================================== TMA loader ====================================
+        if (lane == 0) {
+            uint32_t grp = 0;
+            for (int64_t t = blockIdx.x; t < total_tiles; t += gridDim.x) {
+                const int64_t bidx = t / tiles_per;
+                const Tile tc = tile_from_index(t - bidx * tiles_per, nTJ);
+                if ((int64_t)tc.I * TM >= row_end || (int64_t)(tc.I + 1) * TM <= row_begin) continue;
+                const int ks0 = tc.I, ks1 = 2 * tc.J + 1;
+                const int ngroups = (ks1 - ks0 + GK) / GK;
+                for (int g = 0; g < ngroups; g++, grp++) {
+                    const int b = grp % NB;
+                    mbar_wait(&s_bempty[b], ((grp / NB) & 1) ^ 1);
+                    mbar_arrive_expect_tx(&s_bfull[b], (uint32_t)BITS_BYTES);   // out-of-bounds is zero-filled
+                    unsigned char *dst = s_bits + b * BITS_BYTES;
+                    const int c0 = (ks0 + g * GK) * 16;
+                    tma_load_3d(dst, &mapU, c0, tc.I * TM, (int)bidx, &s_bfull[b]);
+                    tma_load_3d(dst + TM * BROW, &mapL, c0, tc.J * TN, (int)bidx, &s_bfull[b]);
+                }
             }
         }
     } else if (warp == MMA_WARP) {
@@ -298,7 +354,7 @@ k_interval_tensor(const uint64_t *__restrict__ bits, const uint64_t *__restrict_
             mbar_wait(&s_tfull[a], (tile_seq >> 1) & 1);
             tc_fence_after();
             const uint32_t taddr = tmem_base + ((uint32_t)(warp * 32) << 16) + a * TN;
-#pragma unroll 1
+#pragma unroll
             for (int c8 = 0; c8 < TN / 32; c8++) {
                 const uint32_t rel32 = (uint32_t)(rel[c8 >> 1] >> (32 * (c8 & 1)));
                 if (!__any_sync(0xffffffffu, rel32 != 0)) continue;
@@ -346,6 +402,46 @@ k_interval_tensor(const uint64_t *__restrict__ bits, const uint64_t *__restrict_
 bool interval_tensor_available() { return true; }
 size_t interval_tensor_scratch_bytes(int64_t, int64_t) { return 0; }
 
+// cuTensorMapEncodeTiled through the runtime's driver entry point (no link against libcuda)
+typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
+                                  const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+static EncodeTiledFn encode_fn()
+{
+    static EncodeTiledFn fn = nullptr;
+    if (!fn) {
+        void *p = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess &&
+            q == cudaDriverEntryPointSuccess)
+            fn = reinterpret_cast<EncodeTiledFn>(p);
+    }
+    return fn;
+}
+
+// bit matrix [B][N][stride uint64] seen as bytes: dims {stride*8, N, B}; box {64 bytes, rows, 1}
+static int make_bits_map(CUtensorMap *map, const uint64_t *base, int64_t B, int64_t N, int64_t stride, int rows)
+{
+    EncodeTiledFn fn = encode_fn();
+    if (!fn) {
+        snprintf(g_cuda_err, sizeof(g_cuda_err), "cuTensorMapEncodeTiled entry point not available");
+        return CS_ERR_CUDA;
+    }
+    cuuint64_t gdim[3] = {(cuuint64_t)(stride * 8), (cuuint64_t)N, (cuuint64_t)B};
+    cuuint64_t gstr[2] = {(cuuint64_t)(stride * 8), (cuuint64_t)(N * stride * 8)};
+    cuuint32_t box[3] = {(cuuint32_t)BROW, (cuuint32_t)rows, 1};
+    cuuint32_t estr[3] = {1, 1, 1};
+    CUresult r = fn(map, CU_TENSOR_MAP_DATA_TYPE_UINT8, 3, const_cast<uint64_t *>(base), gdim, gstr, box, estr,
+                    CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_64B, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+                    CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) {
+        snprintf(g_cuda_err, sizeof(g_cuda_err), "cuTensorMapEncodeTiled failed (%d)", (int)r);
+        return CS_ERR_CUDA;
+    }
+    return CS_OK;
+}
+
 int launch_interval_tensor(const uint64_t *bits, const uint64_t *bitsT, int64_t B, int64_t N, int64_t kmax,
                            int64_t row_begin, int64_t row_end, int64_t *hist, int64_t *nrel,
                            void *, size_t, cudaStream_t st)
@@ -357,13 +453,18 @@ int launch_interval_tensor(const uint64_t *bits, const uint64_t *bitsT, int64_t 
         attr_set = true;
     }
     const int64_t stride = row_stride_words(N);
+    CUtensorMap mapU, mapL;
+    int rc = make_bits_map(&mapU, bits, B, N, stride, TM);
+    if (rc) return rc;
+    rc = make_bits_map(&mapL, bitsT, B, N, stride, TN);
+    if (rc) return rc;
     const int64_t nTJ = (N + TN - 1) / TN;
     const int64_t total = nTJ * (nTJ + 1) * B;
     int64_t grid = sm_count();
     if (grid > total) grid = total;
     if (grid < 1) grid = 1;
     k_interval_tensor<<<(unsigned)grid, THREADS, SMEM_BYTES, st>>>(
-        bits, bitsT, B, N, stride, kmax, row_begin, row_end,
+        mapU, mapL, bits, B, N, stride, kmax, row_begin, row_end,
         reinterpret_cast<unsigned long long *>(hist), reinterpret_cast<unsigned long long *>(nrel));
     CS_LAUNCHED("k_interval_tensor");
     return CS_OK;
