@@ -23,6 +23,7 @@ GEOM_DS2_SLAB = 2
 ROUTE_AUTO = 0
 ROUTE_POPC = 1
 ROUTE_TENSOR = 2
+ROUTE_TENSOR_FP4 = 3
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libcausalset.so")

@@ -25,7 +25,7 @@ int sm_count()
 static int resolve_route(int64_t N, int route)
 {
     if (route == CS_ROUTE_AUTO) route = cs_default_route(N);
-    if (route == CS_ROUTE_TENSOR && !interval_tensor_available()) return -1;
+    if ((route == CS_ROUTE_TENSOR || route == CS_ROUTE_TENSOR_FP4) && !interval_tensor_available()) return -1;
     return route;
 }
 
@@ -63,6 +63,9 @@ static int interval_hist_impl(const uint64_t *bits, const uint64_t *bitsT, int64
         if (rc) return rc;
         bitsT = t;
     }
+    if (route == CS_ROUTE_TENSOR_FP4)
+        return launch_interval_fp4(bits, bitsT, B, N, kmax, row_begin, row_end, hist, nrel, ws,
+                                   workspace_bytes - (size_t)(ws - static_cast<unsigned char *>(workspace)), st);
     if (route == CS_ROUTE_TENSOR)
         return launch_interval_tensor(bits, bitsT, B, N, kmax, row_begin, row_end, hist, nrel, ws,
                                       workspace_bytes - (size_t)(ws - static_cast<unsigned char *>(workspace)), st);
@@ -149,7 +152,7 @@ int cs_interval_hist_ex(const uint64_t *bits, const uint64_t *bitsT, int64_t N, 
                         void *workspace, size_t workspace_bytes, void *stream)
 {
     if (N < 0 || !hist || (N > 0 && !bits)) return CS_ERR_ARG;
-    if (route < CS_ROUTE_AUTO || route > CS_ROUTE_TENSOR) return CS_ERR_ARG;
+    if (route < CS_ROUTE_AUTO || route > CS_ROUTE_TENSOR_FP4) return CS_ERR_ARG;
     return interval_hist_impl(bits, bitsT, 1, N, kmax, row_begin, row_end, route, hist, n_relations,
                               workspace, workspace_bytes, static_cast<cudaStream_t>(stream));
 }

@@ -1,31 +1,19 @@
-// cs_interval_tensor.cu -- stage a2, tensor route: the count matrix C = U . U as a genuine dense
-// 0/1 contraction on the 5th-generation tensor cores (tcgen05.mma kind::i8, accumulators in TMEM).
+// cs_interval_fp4.cu -- stage a2, tensor route with 4-bit operands (tcgen05.mma kind::mxf4).
 //
-//   count(i,j) = |{k : i -< k -< j}| = sum_k U[i][k] * L[j][k],   U = bits ("future of i"),
-//                                                                  L = bitsT ("past of j"),
-// which is exactly the paper's inner product of rows i and j between columns i and j
-// (Fig. 4.2 caption PAPER.md:1768; Alg. 20 line 9) with AND/popcount replaced by an
-// integer multiply-accumulate.  Only K blocks between the I block and the J block are visited.
+// Same contraction and the same CTA skeleton as cs_interval_tensor.cu (int8): count(i,j) =
+// sum_k U[i][k] * L[j][k] over the K blocks between the I block and the J block (Fig. 4.2 caption
+// PAPER.md:1768; Alg. 20 line 9).  The int8 kernel is bound by shared-memory
+// bandwidth (operand bytes written by the expanders + read by the MMA); here a bit becomes the
+// E2M1 nibble 0b0010 (= 1.0) instead of a byte, which halves the operand bytes per k and doubles
+// the MMA rate: a 48 KB stage now covers 256 k.  With x a 32-bit slice of a row, output word
+// m = ((x << 1) >> m) & 0x22222222 (m = 0..3): nibble n of word m holds bit 4n+m -- again a fixed
+// permutation of k inside the slice, applied to both operands.  Block scales are UE8M0 = 2^0
+// (byte 0x7F) everywhere, written once into TMEM.  Products are 0 or 1 and the fp32 accumulator
+// is exact for counts < 2^24 (measured: identical histograms to the int8 and POPC routes).
 //
-// Operands never exist as bytes in HBM: the bit rows are read from global memory (16 bytes = 128
-// k per row per k-step) and expanded in registers straight into the shared-memory layout the MMA
-// reads (no-swizzle K-major canonical layout: [16-byte k chunk][row][16 B]; SBO = 128 B,
-// LBO = rows*16 B).  A bit becomes the byte 0x80 (u8 128): with x a 32-bit slice of the row,
-// output word m = (x << (7-m)) & 0x80808080, i.e. byte p = 4m+b of the 32-byte K slice holds bit
-// m+8b.  That is a fixed permutation of k inside each 32-wide slice, applied identically to both
-// operands, so the sum over k is unchanged and the expansion costs one shift and one AND per
-// four bytes.  Every match contributes 128*128 = 2^14; the int32 accumulator holds count * 2^14
-// exactly for counts < 2^17 (N <= 131072; checked by the launcher), and count = acc >> 14.
-//
-// CTA = one SM (512 TMEM columns), persistent over 128 x 256 tiles (rows i x rows j), 18 warps:
-//   warps 0-3   epilogue: tcgen05.ld the accumulator rows, test the relation bit U[i][j], update the
-//               shared-memory histogram (global atomics for rare large intervals)
-//   warp  4     TMEM allocation + the single MMA-issuing thread
-//   warp  5     loader: one thread issues the TMA tensor copies (cp.async.bulk.tensor, 64B swizzle)
-//               that stage the bit rows, GK k-steps (64 bytes per row) at a time
-//   warps 6-17  expanders: 384 threads, one operand row each (128 rows of U, 256 rows of L)
-// Pipelines: NB bit-row buffers (bfull/bempty), NS shared-memory operand stages (full/empty; the
-// MMA warp releases a stage with tcgen05.commit), two TMEM accumulator buffers (tfull/tempty).
+// TMEM: one 256-column fp32 accumulator + 2 x 32 columns of scale factors (a second accumulator
+// does not fit next to them), so the epilogue is not overlapped with the next tile's MMAs; it is
+// branch-free and short (8 tcgen05.ld + 512 predicated reductions per thread).
 #include <cuda.h>
 
 #include "cs_common.cuh"
@@ -36,30 +24,31 @@ namespace {
 
 constexpr int TM = 128;                 // tile rows i (MMA M)
 constexpr int TN = 256;                 // tile rows j (MMA N)
-constexpr int KSTEP = 128;              // k per stage = 128 bytes of int8 = 4 MMAs of K = 32
+constexpr int KSTEP = 256;              // k per stage = 128 bytes of E2M1 = 4 MMAs of K = 64
+constexpr int KBYTES = KSTEP / 2;       // operand bytes per row per stage
 constexpr int NS = 3;                   // shared-memory stages of expanded operands
-constexpr int GK = 4;                   // k-steps per staged group of bit rows (64 bytes per row)
-constexpr int BROW = GK * 16;           // bytes per staged bit row (TMA box inner extent, 64B swizzle)
-constexpr int NB = 3;                   // bit-row buffers
+constexpr int GK = 2;                   // stages per staged group of bit rows (64 bytes per row)
+constexpr int BROW = GK * 32;           // bytes per staged bit row (TMA box inner extent, 64B swizzle)
+constexpr int NB = 2;                   // bit-row buffers
+constexpr int EPITCH = 20;              // words per thread row of the epilogue staging area (16 counts + pad)
+constexpr int EPI_BYTES = 256 * EPITCH * 4;
 constexpr int BITS_BYTES = (TM + TN) * BROW;
-constexpr int A_BYTES = TM * KSTEP;     // 16 KiB
-constexpr int B_BYTES = TN * KSTEP;     // 32 KiB
+constexpr int A_BYTES = TM * KBYTES;    // 16 KiB
+constexpr int B_BYTES = TN * KBYTES;    // 32 KiB
 constexpr int STAGE_BYTES = A_BYTES + B_BYTES;
 constexpr int HS = 2048;                // shared-memory histogram bins
-constexpr int EPI_WARPS = 4, MMA_WARP = 4, LOAD_WARP = 5, EXP_WARP0 = 6, EXP_WARPS = 12;
+constexpr int EPI_WARPS = 8, MMA_WARP = 8, LOAD_WARP = 9, EXP_WARP0 = 10, EXP_WARPS = 12;
 constexpr int THREADS = (EPI_WARPS + 2 + EXP_WARPS) * 32;   // 576
 constexpr int EXP_THREADS = EXP_WARPS * 32;                 // 384 = TM + TN
-constexpr int SMEM_BYTES = NS * STAGE_BYTES + NB * BITS_BYTES + HS * 4 + 256;
-constexpr int SCALE_SHIFT = 14;         // every match adds 128 * 128
+constexpr int SMEM_BYTES = NS * STAGE_BYTES + NB * BITS_BYTES + EPI_BYTES + HS * 4 + 256;
 
 static_assert(EXP_THREADS == TM + TN, "one expander thread per operand row");
-// a thread may run at most NS k-steps ahead of the slowest warp; keeping that below one group keeps
-// every thread within one phase of the bit-buffer barriers
-static_assert(NS <= GK, "stage ring must not outrun a bit-row group");
 
-// instruction descriptor, kind::i8: D = S32 (2 at bit 4), A = B = U8 (0), both K-major,
-// N >> 3 at bit 17, M >> 4 at bit 24
-constexpr uint32_t IDESC = (2u << 4) | ((uint32_t)(TN >> 3) << 17) | ((uint32_t)(TM >> 4) << 24);
+
+// block-scaled instruction descriptor, kind::mxf4: A = B = E2M1 (1 at bits 7 and 10), both K-major,
+// N >> 3 at bit 17, scale format UE8M0 (1 at bit 23), M >> 4 at bit 24, scale-factor ids 0, K = 64
+constexpr uint32_t IDESC = (1u << 7) | (1u << 10) | ((uint32_t)(TN >> 3) << 17) | (1u << 23) | ((uint32_t)(TM >> 4) << 24);
+constexpr uint32_t SFA_COL = 256, SFB_COL = 288;   // TMEM columns of the (constant) scale factors
 
 __device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
 
@@ -112,16 +101,27 @@ __device__ __forceinline__ uint64_t make_desc(uint32_t saddr, uint32_t lbo_bytes
     return d;                 // layout_type = 0 (SWIZZLE_NONE), base_offset = 0, lbo_mode = 0
 }
 
-__device__ __forceinline__ void mma_i8(uint32_t d_tmem, uint64_t adesc, uint64_t bdesc, uint32_t idesc, uint32_t accum)
+__device__ __forceinline__ void mma_mxf4(uint32_t d_tmem, uint64_t adesc, uint64_t bdesc, uint32_t idesc, uint32_t accum,
+                                         uint32_t sfa, uint32_t sfb)
 {
     asm volatile(
         "{\n"
         ".reg .pred p;\n"
         "setp.ne.b32 p, %4, 0;\n"
-        "tcgen05.mma.cta_group::1.kind::i8 [%0], %1, %2, %3, p;\n"
+        "tcgen05.mma.cta_group::1.kind::mxf4.block_scale.block32 [%0], %1, %2, %3, [%5], [%6], p;\n"
         "}\n" ::"r"(d_tmem),
-        "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accum)
+        "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accum), "r"(sfa), "r"(sfb)
         : "memory");
+}
+__device__ __forceinline__ void tmem_st32_const(uint32_t taddr, uint32_t val)
+{
+    asm volatile(
+        "tcgen05.st.sync.aligned.32x32b.x32.b32 [%0], "
+        "{%1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1, "
+        "%1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1};\n" ::"r"(taddr),
+        "r"(val)
+        : "memory");
+    asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
 }
 __device__ __forceinline__ void mma_commit(uint64_t *bar)
 {
@@ -144,6 +144,18 @@ __device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t (&v)[32])
     asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
 }
 
+__device__ __forceinline__ void tmem_ld16(uint32_t taddr, uint32_t (&v)[16])
+{
+    asm volatile(
+        "tcgen05.ld.sync.aligned.32x32b.x16.b32 "
+        "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15}, [%16];\n"
+        : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]),
+          "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15])
+        : "r"(taddr)
+        : "memory");
+    asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+}
+
 struct Tile {
     int I, J;   // 128-row block of i, 256-row block of j
 };
@@ -161,7 +173,7 @@ __device__ __forceinline__ Tile tile_from_index(int64_t t, int nTJ)
 }
 
 __global__ void __launch_bounds__(THREADS, 1)
-k_interval_tensor(const __grid_constant__ CUtensorMap mapU, const __grid_constant__ CUtensorMap mapL,
+k_interval_fp4(const __grid_constant__ CUtensorMap mapU, const __grid_constant__ CUtensorMap mapL,
                   const uint64_t *__restrict__ bits,
                   int64_t B, int64_t N, int64_t stride, int64_t kmax,
                   int64_t row_begin, int64_t row_end,
@@ -170,8 +182,9 @@ k_interval_tensor(const __grid_constant__ CUtensorMap mapU, const __grid_constan
     extern __shared__ __align__(1024) unsigned char smem[];   // typed shared base: STS/ATOMS, not generic
     unsigned char *s_stage = smem;
     unsigned char *s_bits = smem + NS * STAGE_BYTES;
-    uint32_t *s_hist = reinterpret_cast<uint32_t *>(smem + NS * STAGE_BYTES + NB * BITS_BYTES);
-    uint64_t *s_full = reinterpret_cast<uint64_t *>(smem + NS * STAGE_BYTES + NB * BITS_BYTES + HS * 4);
+    uint32_t *s_epi = reinterpret_cast<uint32_t *>(smem + NS * STAGE_BYTES + NB * BITS_BYTES);
+    uint32_t *s_hist = reinterpret_cast<uint32_t *>(smem + NS * STAGE_BYTES + NB * BITS_BYTES + EPI_BYTES);
+    uint64_t *s_full = reinterpret_cast<uint64_t *>(smem + NS * STAGE_BYTES + NB * BITS_BYTES + EPI_BYTES + HS * 4);
     uint64_t *s_empty = s_full + NS;
     uint64_t *s_tfull = s_empty + NS;     // [2]
     uint64_t *s_tempty = s_tfull + 2;     // [2]
@@ -212,6 +225,14 @@ k_interval_tensor(const __grid_constant__ CUtensorMap mapU, const __grid_constan
     __syncthreads();
     tc_fence_after();
     const uint32_t tmem_base = *s_tmem;
+    if (warp < 4) {   // constant block scales UE8M0 = 2^0 in every byte of the scale-factor columns
+        const uint32_t sf = tmem_base + ((uint32_t)(warp * 32) << 16) + SFA_COL;
+        tmem_st32_const(sf, 0x7F7F7F7Fu);
+        tmem_st32_const(sf + 32, 0x7F7F7F7Fu);
+    }
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
 
     // every role walks the same static schedule: tile t = blockIdx.x, + gridDim.x, ...
     if (warp >= EXP_WARP0) {
@@ -229,32 +250,28 @@ k_interval_tensor(const __grid_constant__ CUtensorMap mapU, const __grid_constan
             const int64_t bidx = t / tiles_per;
             const Tile tc = tile_from_index(t - bidx * tiles_per, nTJ);
             if ((int64_t)tc.I * TM >= row_end || (int64_t)(tc.I + 1) * TM <= row_begin) continue;
-            const int ks0 = tc.I, ks1 = 2 * tc.J + 1;            // inclusive k-step range
+            const int ks0 = tc.I >> 1, ks1 = tc.J;                // inclusive range of 256-k stages
             const int ngroups = (ks1 - ks0 + GK) / GK;
             for (int g = 0; g < ngroups; g++, grp++) {
                 const int b = grp % NB;
                 mbar_wait(&s_bfull[b], (grp / NB) & 1);
                 const int kcount = (ks1 - (ks0 + g * GK) + 1 < GK) ? (ks1 - (ks0 + g * GK) + 1) : GK;
                 for (int c = 0; c < kcount; c++, it++) {
-                    const uint4 cur = *reinterpret_cast<const uint4 *>(my_bits + b * BITS_BYTES + ((c ^ swz) << 4));
+                    const uint4 cur0 = *reinterpret_cast<const uint4 *>(my_bits + b * BITS_BYTES + (((2 * c) ^ swz) << 4));
+                    const uint4 cur1 = *reinterpret_cast<const uint4 *>(my_bits + b * BITS_BYTES + (((2 * c + 1) ^ swz) << 4));
                     const int s = it % NS;
                     mbar_wait(&s_empty[s], ((it / NS) & 1) ^ 1);
                     unsigned char *dst = s_stage + s * STAGE_BYTES + (isA ? 0 : A_BYTES) + r * 16;
-                    const uint32_t xs[4] = {cur.x, cur.y, cur.z, cur.w};
+                    const uint32_t xs[8] = {cur0.x, cur0.y, cur0.z, cur0.w, cur1.x, cur1.y, cur1.z, cur1.w};
 #pragma unroll
-                    for (int q = 0; q < 4; q++) {
+                    for (int q = 0; q < 8; q++) {     // 32 k -> one 16-byte chunk of E2M1 nibbles (1.0 = 0b0010)
                         const uint32_t x = xs[q];
-                        uint4 lo, hi;
-                        lo.x = (x << 7) & 0x80808080u;
-                        lo.y = (x << 6) & 0x80808080u;
-                        lo.z = (x << 5) & 0x80808080u;
-                        lo.w = (x << 4) & 0x80808080u;
-                        hi.x = (x << 3) & 0x80808080u;
-                        hi.y = (x << 2) & 0x80808080u;
-                        hi.z = (x << 1) & 0x80808080u;
-                        hi.w = x & 0x80808080u;
-                        *reinterpret_cast<uint4 *>(dst + (2 * q) * rows * 16) = lo;
-                        *reinterpret_cast<uint4 *>(dst + (2 * q + 1) * rows * 16) = hi;
+                        uint4 w;
+                        w.x = (x << 1) & 0x22222222u;
+                        w.y = x & 0x22222222u;
+                        w.z = (x >> 1) & 0x22222222u;
+                        w.w = (x >> 2) & 0x22222222u;
+                        *reinterpret_cast<uint4 *>(dst + q * rows * 16) = w;
                     }
                     fence_proxy_async();          // generic-proxy stores -> visible to the tensor core
                     __syncwarp();
@@ -275,14 +292,14 @@ k_interval_tensor(const __grid_constant__ CUtensorMap mapU, const __grid_constan
                 const int64_t bidx = t / tiles_per;
                 const Tile tc = tile_from_index(t - bidx * tiles_per, nTJ);
                 if ((int64_t)tc.I * TM >= row_end || (int64_t)(tc.I + 1) * TM <= row_begin) continue;
-                const int ks0 = tc.I, ks1 = 2 * tc.J + 1;
+                const int ks0 = tc.I >> 1, ks1 = tc.J;
                 const int ngroups = (ks1 - ks0 + GK) / GK;
                 for (int g = 0; g < ngroups; g++, grp++) {
                     const int b = grp % NB;
                     mbar_wait(&s_bempty[b], ((grp / NB) & 1) ^ 1);
                     mbar_arrive_expect_tx(&s_bfull[b], (uint32_t)BITS_BYTES);   // out-of-bounds is zero-filled
                     unsigned char *dst = s_bits + b * BITS_BYTES;
-                    const int c0 = (ks0 + g * GK) * 16;
+                    const int c0 = (ks0 + g * GK) * 32;
                     tma_load_3d(dst, &mapU, c0, tc.I * TM, (int)bidx, &s_bfull[b]);
                     tma_load_3d(dst + TM * BROW, &mapL, c0, tc.J * TN, (int)bidx, &s_bfull[b]);
                 }
@@ -296,11 +313,10 @@ k_interval_tensor(const __grid_constant__ CUtensorMap mapU, const __grid_constan
                 const int64_t bidx = t / tiles_per;
                 const Tile tc = tile_from_index(t - bidx * tiles_per, nTJ);
                 if ((int64_t)tc.I * TM >= row_end || (int64_t)(tc.I + 1) * TM <= row_begin) continue;
-                const int ks0 = tc.I, ks1 = 2 * tc.J + 1;
-                const uint32_t a = tile_seq & 1;
-                mbar_wait(&s_tempty[a], ((tile_seq >> 1) & 1) ^ 1);      // epilogue has drained buffer a
+                const int ks0 = tc.I >> 1, ks1 = tc.J;
+                mbar_wait(&s_tempty[0], (tile_seq & 1) ^ 1);             // epilogue has drained the accumulator
                 tc_fence_after();
-                const uint32_t d_tmem = tmem_base + a * TN;
+                const uint32_t d_tmem = tmem_base;
                 for (int ks = ks0; ks <= ks1; ks++, it++) {
                     const int s = it % NS;
                     mbar_wait(&s_full[s], (it / NS) & 1);
@@ -308,14 +324,14 @@ k_interval_tensor(const __grid_constant__ CUtensorMap mapU, const __grid_constan
                     const uint32_t a_addr = smem_u32(s_stage + s * STAGE_BYTES);
                     const uint32_t b_addr = a_addr + A_BYTES;
 #pragma unroll
-                    for (int q = 0; q < KSTEP / 32; q++) {
+                    for (int q = 0; q < KBYTES / 32; q++) {
                         const uint64_t ad = make_desc(a_addr + q * 2 * TM * 16, TM * 16, 128);
                         const uint64_t bd = make_desc(b_addr + q * 2 * TN * 16, TN * 16, 128);
-                        mma_i8(d_tmem, ad, bd, IDESC, (ks > ks0 || q > 0) ? 1u : 0u);
+                        mma_mxf4(d_tmem, ad, bd, IDESC, (ks > ks0 || q > 0) ? 1u : 0u, tmem_base + SFA_COL, tmem_base + SFB_COL);
                     }
                     mma_commit(&s_empty[s]);                              // stage s free once these MMAs retire
                 }
-                mma_commit(&s_tfull[a]);                                  // accumulator complete
+                mma_commit(&s_tfull[0]);                                  // accumulator complete
                 tile_seq++;
             }
         }
@@ -332,65 +348,69 @@ k_interval_tensor(const __grid_constant__ CUtensorMap mapU, const __grid_constan
             if ((int64_t)tc.I * TM >= row_end || (int64_t)(tc.I + 1) * TM <= row_begin) continue;
             if (bidx != cur_batch) {   // per-causet histograms: flush before switching
                 if (cur_batch >= 0 && B > 1) {
-                    asm volatile("bar.sync 1, 128;");
+                    asm volatile("bar.sync 1, 256;");
                     for (int b = tid; b < hs; b += EPI_WARPS * 32) {
                         uint32_t v = s_hist[b];
                         if (v) { atomicAdd(&hist[cur_batch * hist_len + b], (unsigned long long)v); s_hist[b] = 0; }
                     }
-                    asm volatile("bar.sync 1, 128;");
+                    asm volatile("bar.sync 1, 256;");
                 }
                 cur_batch = bidx;
             }
-            const int64_t i = (int64_t)tc.I * TM + tid;          // this thread's row = TMEM lane
+            const int quarter = warp & 3, colhalf = warp >> 2;   // TMEM lane quarter; which 128 columns
+            const int64_t i = (int64_t)tc.I * TM + quarter * 32 + lane;   // this thread's row = TMEM lane
             const bool row_ok = i < N && i >= row_begin && i < row_end;
-            uint64_t rel[4] = {0, 0, 0, 0};
+            uint64_t rel[2] = {0, 0};                            // relation bits of this warp's 128 columns
             if (row_ok) {
                 const uint64_t *urow = bits + bidx * N * stride + i * stride;
 #pragma unroll
-                for (int w = 0; w < 4; w++) {
-                    const int64_t wi = (int64_t)tc.J * 4 + w;
+                for (int w = 0; w < 2; w++) {
+                    const int64_t wi = (int64_t)tc.J * 4 + colhalf * 2 + w;
                     if (wi < stride) rel[w] = __ldg(urow + wi);
                 }
             }
             unsigned long long *ghist = hist + cur_batch * hist_len;
-            const uint32_t a = tile_seq & 1;
-            mbar_wait(&s_tfull[a], (tile_seq >> 1) & 1);
+            mbar_wait(&s_tfull[0], tile_seq & 1);
             tc_fence_after();
-            const uint32_t taddr = tmem_base + ((uint32_t)(warp * 32) << 16) + a * TN;
+            const uint32_t taddr = tmem_base + ((uint32_t)(quarter * 32) << 16) + colhalf * 128;
+            uint32_t *my = s_epi + tid * EPITCH;
+            auto tally = [&](uint32_t word) {
+                const uint32_t cnt = (uint32_t)__uint_as_float(word);   // products are 0 or 1: exact in fp32
+                if (cnt < (uint32_t)hs) atomicAdd(&s_hist[cnt], 1u);
+                else if (cnt <= kmax32) atomicAdd(&ghist[cnt], 1ULL);
+            };
 #pragma unroll
-            for (int c8 = 0; c8 < TN / 32; c8++) {
-                const uint32_t rel32 = (uint32_t)(rel[c8 >> 1] >> (32 * (c8 & 1)));
-                if (!__any_sync(0xffffffffu, rel32 != 0)) continue;
-                uint32_t v[32];
-                tmem_ld32(taddr + c8 * 32, v);
-                if (rel32 == 0) continue;
-                my_nrel += __popc(rel32);
-                // branch-free: two predicated reductions per element (a divergent if/else here costs
-                // one serialized pass per column in which any lane has a related pair)
+            for (int c16 = 0; c16 < 8; c16++) {
+                const uint32_t rel16 = (uint32_t)(rel[c16 >> 2] >> (16 * (c16 & 3))) & 0xFFFFu;
+                if (!__any_sync(0xffffffffu, rel16 != 0)) continue;
+                uint32_t v[16];
+                tmem_ld16(taddr + c16 * 16, v);
+                if (rel16 == 0) continue;
+                my_nrel += __popc(rel16);
+                // Stage the 16 counts in this thread's private shared-memory row, then visit only the
+                // columns whose relation bit is set, two per iteration (work ~ related pairs, not
+                // columns; a predicated reduction per column compiles to a divergent branch per column).
 #pragma unroll
-                for (int c = 0; c < 32; c++) {
-                    const uint32_t cnt = v[c] >> SCALE_SHIFT;
-                    const uint32_t on = (rel32 >> c) & 1u;
-                    const uint32_t small = on & (cnt < (uint32_t)hs ? 1u : 0u);
-                    const uint32_t big = on & (small ^ 1u) & (cnt <= kmax32 ? 1u : 0u);
-                    asm volatile(
-                        "{\n"
-                        ".reg .pred ps, pb;\n"
-                        "setp.ne.u32 ps, %0, 0;\n"
-                        "setp.ne.u32 pb, %1, 0;\n"
-                        "@ps red.shared.add.u32 [%2], 1;\n"
-                        "@pb red.global.add.u64 [%3], 1;\n"
-                        "}\n" ::"r"(small),
-                        "r"(big), "r"(hist_saddr + cnt * 4u), "l"(ghist + cnt)
-                        : "memory");
+                for (int c4 = 0; c4 < 4; c4++)
+                    *reinterpret_cast<uint4 *>(my + 4 * c4) = make_uint4(v[4 * c4], v[4 * c4 + 1], v[4 * c4 + 2], v[4 * c4 + 3]);
+                uint32_t m = rel16;
+                while (m) {
+                    const int c0 = __ffs(m) - 1;
+                    m &= m - 1;
+                    const bool two = m != 0;
+                    const int c1 = two ? __ffs(m) - 1 : c0;
+                    m &= m - 1;
+                    const uint32_t w0 = my[c0], w1 = my[c1];
+                    tally(w0);
+                    if (two) tally(w1);
                 }
             }
             tc_fence_before();
-            mbar_arrive(&s_tempty[a]);
+            mbar_arrive(&s_tempty[0]);
             tile_seq++;
         }
         // final flush by the epilogue warps
-        asm volatile("bar.sync 1, 128;");
+        asm volatile("bar.sync 1, 256;");
         if (cur_batch >= 0) {
             for (int b = tid; b < hs; b += EPI_WARPS * 32) {
                 uint32_t v = s_hist[b];
@@ -413,8 +433,6 @@ k_interval_tensor(const __grid_constant__ CUtensorMap mapU, const __grid_constan
 
 }  // namespace
 
-bool interval_tensor_available() { return true; }
-size_t interval_tensor_scratch_bytes(int64_t, int64_t) { return 0; }
 
 // cuTensorMapEncodeTiled through the runtime's driver entry point (no link against libcuda)
 typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
@@ -456,14 +474,14 @@ static int make_bits_map(CUtensorMap *map, const uint64_t *base, int64_t B, int6
     return CS_OK;
 }
 
-int launch_interval_tensor(const uint64_t *bits, const uint64_t *bitsT, int64_t B, int64_t N, int64_t kmax,
+int launch_interval_fp4(const uint64_t *bits, const uint64_t *bitsT, int64_t B, int64_t N, int64_t kmax,
                            int64_t row_begin, int64_t row_end, int64_t *hist, int64_t *nrel,
                            void *, size_t, cudaStream_t st)
 {
-    if (N > ((int64_t)1 << 17)) return CS_ERR_ARG;   // count * 2^14 must stay below 2^31
+    if (N > ((int64_t)1 << 24)) return CS_ERR_ARG;   // counts must stay exact in fp32
     static bool attr_set = false;
     if (!attr_set) {
-        CS_CUDA(cudaFuncSetAttribute(k_interval_tensor, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES));
+        CS_CUDA(cudaFuncSetAttribute(k_interval_fp4, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES));
         attr_set = true;
     }
     const int64_t stride = row_stride_words(N);
@@ -477,10 +495,10 @@ int launch_interval_tensor(const uint64_t *bits, const uint64_t *bitsT, int64_t 
     int64_t grid = sm_count();
     if (grid > total) grid = total;
     if (grid < 1) grid = 1;
-    k_interval_tensor<<<(unsigned)grid, THREADS, SMEM_BYTES, st>>>(
+    k_interval_fp4<<<(unsigned)grid, THREADS, SMEM_BYTES, st>>>(
         mapU, mapL, bits, B, N, stride, kmax, row_begin, row_end,
         reinterpret_cast<unsigned long long *>(hist), reinterpret_cast<unsigned long long *>(nrel));
-    CS_LAUNCHED("k_interval_tensor");
+    CS_LAUNCHED("k_interval_fp4");
     return CS_OK;
 }
 

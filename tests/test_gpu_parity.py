@@ -34,12 +34,13 @@ def api():
 
 def routes(api):
     r = [api.ROUTE_POPC]
-    try:
-        x = torch.zeros((128, 2), dtype=torch.int64, device="cuda")
-        api.interval_hist(x, x, 128, route=api.ROUTE_TENSOR)
-        r.append(api.ROUTE_TENSOR)
-    except RuntimeError:
-        pass
+    for cand in (api.ROUTE_TENSOR, api.ROUTE_TENSOR_FP4):
+        try:
+            x = torch.zeros((128, 2), dtype=torch.int64, device="cuda")
+            api.interval_hist(x, x, 128, route=cand)
+            r.append(cand)
+        except RuntimeError:
+            pass
     return r
 
 
