@@ -38,8 +38,14 @@ UNIT = "word-ops/s"
 
 # ALU roofline of the POPC route: 16 POPC.32 /clk/SM, two per 64-bit word
 POPC_PER_CLK_SM = 16.0
-# int8 tensor peak = measured bf16 dense peak x nominal ratio 2 (guide: 4.5 / 2.25 PFLOP/s)
-INT8_OVER_BF16 = 2.0
+# dram__bytes_read.sum + dram__bytes_write.sum of one launch of the a2 kernel at config 3, from the
+# `ncu --set full` captures summarised under profiles/ (bytes per launch; None = not captured)
+NCU_TRAFFIC = {1: 78.28e9, 2: 51.14e9, 3: None}
+# tensor peaks = measured bf16 dense peak x the guide's nominal ratio (bf16 2.25, int8/fp8 4.5, fp4 9 PFLOP/s)
+TENSOR_OVER_BF16 = {2: 2.0, 3: 4.0}
+ROUTE_NAME = {1: "popc", 2: "tensor_int8", 3: "tensor_fp4"}
+ROUTE_DTYPE = {1: "u64", 2: "int8", 3: "fp4_e2m1"}
+ROUTE_KERNEL = {1: "k_interval_popc", 2: "k_interval_tensor", 3: "k_interval_fp4"}
 
 
 def measured_peaks():
@@ -181,7 +187,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=3, help="BASELINE.json workload 1..4 (default 3: N=65536, 3+1)")
     ap.add_argument("--N", type=int, default=0, help="override N (debug only; the line then names it)")
-    ap.add_argument("--route", type=int, default=0, help="0 auto, 1 popc, 2 tensor")
+    ap.add_argument("--route", type=int, default=0, help="0 auto, 1 popc, 2 tensor int8, 3 tensor fp4")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=12.0)
     ap.add_argument("--ref-seconds", type=float, default=6.0)
@@ -282,20 +288,21 @@ def main():
     # ---- roofline of the dominant kernel (a2) -----------------------------------------------
     hist_s = statistics.mean(hist_ms) / 1e3
     sm_mhz = clocks.get("sm_mhz") or peaks.get("sm_max_mhz", 1965.0)
-    if route == api.ROUTE_TENSOR:
+    if route in TENSOR_OVER_BF16:
         ops = tensor_ops_algorithmic(N)
         burst = hist_s < 1.0
-        peak = INT8_OVER_BF16 * (peaks["bf16_tflops"] if burst else peaks.get("bf16_tflops_sustained", peaks["bf16_tflops"]))
+        ratio = TENSOR_OVER_BF16[route]
+        peak = ratio * (peaks["bf16_tflops"] if burst else peaks.get("bf16_tflops_sustained", peaks["bf16_tflops"]))
         roofline = {"bound": "tensor", "achieved": ops / hist_s / 1e12, "peak": peak, "unit": "TFLOP/s",
-                    "frac": ops / hist_s / 1e12 / peak, "traffic": None,
-                    "kernel": "k_interval_tensor", "peak_source": "%s bf16 %s x %.0f (int8:bf16 nominal ratio)" %
-                    (peaks["_source"], "burst" if burst else "sustained", INT8_OVER_BF16),
+                    "frac": ops / hist_s / 1e12 / peak, "traffic": NCU_TRAFFIC.get(route),
+                    "kernel": ROUTE_KERNEL[route], "peak_source": "%s bf16 %s x %.0f (%s:bf16 nominal ratio)" %
+                    (peaks["_source"], "burst" if burst else "sustained", ratio, ROUTE_DTYPE[route]),
                     "algorithmic_ops": ops}
     else:
         peak = 148 * POPC_PER_CLK_SM / 2.0 * peaks.get("sm_max_mhz", 1965.0) * 1e6 / 1e12   # T word-ops/s
         executed = dense_triangular_word_ops(N)
         roofline = {"bound": "alu", "achieved": W_alg / hist_s / 1e12, "peak": peak, "unit": "Tword-op/s",
-                    "frac": W_alg / hist_s / 1e12 / peak, "traffic": None, "kernel": "k_interval_popc",
+                    "frac": W_alg / hist_s / 1e12 / peak, "traffic": NCU_TRAFFIC.get(route), "kernel": "k_interval_popc",
                     "peak_source": "derived: 148 SM x 16 POPC.32/clk/SM / 2 per 64-bit word x sm_max_mhz (DESIGN.md)",
                     "executed_word_ops": executed, "executed_frac": executed / hist_s / 1e12 / peak}
     build_s = statistics.mean(build_ms) / 1e3
@@ -309,9 +316,9 @@ def main():
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-        "dtype": "u64" if route != api.ROUTE_TENSOR else "int8", "data": "synthetic",
+        "dtype": ROUTE_DTYPE[route], "data": "synthetic",
         "config": {"workload": cfg.name, "N": N, "dim": cfg.dim, "geometry": cfg.geometry, "seed": cfg.seed,
-                   "route": {1: "popc", 2: "tensor"}[route], "kmax": kmax, "relations": R, "W_alg": W_alg,
+                   "route": ROUTE_NAME[route], "kmax": kmax, "relations": R, "W_alg": W_alg,
                    "l2": "inputs larger than L2 (bits+bitsT = %.0f MiB vs 126 MB)" % (2.0 * N * stride * 8 / 2 ** 20),
                    "parallelism": "replicas x%d" % world, "action": S_dev},
         "action_time_ms": ms_per_step, "stages": stages, "roofline": roofline,

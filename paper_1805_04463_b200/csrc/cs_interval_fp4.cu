@@ -26,7 +26,7 @@ constexpr int TM = 128;                 // tile rows i (MMA M)
 constexpr int TN = 256;                 // tile rows j (MMA N)
 constexpr int KSTEP = 256;              // k per stage = 128 bytes of E2M1 = 4 MMAs of K = 64
 constexpr int KBYTES = KSTEP / 2;       // operand bytes per row per stage
-constexpr int NS = 3;                   // shared-memory stages of expanded operands
+constexpr int NS = 4;                   // stages: B operand in shared memory, A operand in TMEM
 constexpr int GK = 2;                   // stages per staged group of bit rows (64 bytes per row)
 constexpr int BROW = GK * 32;           // bytes per staged bit row (TMA box inner extent, 64B swizzle)
 constexpr int NB = 2;                   // bit-row buffers
@@ -35,7 +35,7 @@ constexpr int EPI_BYTES = 256 * EPITCH * 4;
 constexpr int BITS_BYTES = (TM + TN) * BROW;
 constexpr int A_BYTES = TM * KBYTES;    // 16 KiB
 constexpr int B_BYTES = TN * KBYTES;    // 32 KiB
-constexpr int STAGE_BYTES = A_BYTES + B_BYTES;
+constexpr int STAGE_BYTES = B_BYTES;     // the A operand of a stage lives in 32 TMEM columns
 constexpr int HS = 2048;                // shared-memory histogram bins
 constexpr int EPI_WARPS = 8, MMA_WARP = 8, LOAD_WARP = 9, EXP_WARP0 = 10, EXP_WARPS = 12;
 constexpr int THREADS = (EPI_WARPS + 2 + EXP_WARPS) * 32;   // 576
@@ -49,6 +49,8 @@ static_assert(EXP_THREADS == TM + TN, "one expander thread per operand row");
 // N >> 3 at bit 17, scale format UE8M0 (1 at bit 23), M >> 4 at bit 24, scale-factor ids 0, K = 64
 constexpr uint32_t IDESC = (1u << 7) | (1u << 10) | ((uint32_t)(TN >> 3) << 17) | (1u << 23) | ((uint32_t)(TM >> 4) << 24);
 constexpr uint32_t SFA_COL = 256, SFB_COL = 288;   // TMEM columns of the (constant) scale factors
+constexpr uint32_t A_COL = 320;                    // TMEM ring of the A operand: NS x 32 columns
+static_assert(A_COL + NS * 32 <= 512, "TMEM columns");
 
 __device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
 
@@ -101,16 +103,16 @@ __device__ __forceinline__ uint64_t make_desc(uint32_t saddr, uint32_t lbo_bytes
     return d;                 // layout_type = 0 (SWIZZLE_NONE), base_offset = 0, lbo_mode = 0
 }
 
-__device__ __forceinline__ void mma_mxf4(uint32_t d_tmem, uint64_t adesc, uint64_t bdesc, uint32_t idesc, uint32_t accum,
+__device__ __forceinline__ void mma_mxf4(uint32_t d_tmem, uint32_t a_tmem, uint64_t bdesc, uint32_t idesc, uint32_t accum,
                                          uint32_t sfa, uint32_t sfb)
 {
     asm volatile(
         "{\n"
         ".reg .pred p;\n"
         "setp.ne.b32 p, %4, 0;\n"
-        "tcgen05.mma.cta_group::1.kind::mxf4.block_scale.block32 [%0], %1, %2, %3, [%5], [%6], p;\n"
+        "tcgen05.mma.cta_group::1.kind::mxf4.block_scale.block32 [%0], [%1], %2, %3, [%5], [%6], p;\n"
         "}\n" ::"r"(d_tmem),
-        "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accum), "r"(sfa), "r"(sfb)
+        "r"(a_tmem), "l"(bdesc), "r"(idesc), "r"(accum), "r"(sfa), "r"(sfb)
         : "memory");
 }
 __device__ __forceinline__ void tmem_st32_const(uint32_t taddr, uint32_t val)
@@ -129,21 +131,6 @@ __device__ __forceinline__ void mma_commit(uint64_t *bar)
                  : "memory");
 }
 
-__device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t (&v)[32])
-{
-    asm volatile(
-        "tcgen05.ld.sync.aligned.32x32b.x32.b32 "
-        "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, "
-        "%16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31}, [%32];\n"
-        : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]),
-          "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15]),
-          "=r"(v[16]), "=r"(v[17]), "=r"(v[18]), "=r"(v[19]), "=r"(v[20]), "=r"(v[21]), "=r"(v[22]), "=r"(v[23]),
-          "=r"(v[24]), "=r"(v[25]), "=r"(v[26]), "=r"(v[27]), "=r"(v[28]), "=r"(v[29]), "=r"(v[30]), "=r"(v[31])
-        : "r"(taddr)
-        : "memory");
-    asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
-}
-
 __device__ __forceinline__ void tmem_ld16(uint32_t taddr, uint32_t (&v)[16])
 {
     asm volatile(
@@ -154,6 +141,20 @@ __device__ __forceinline__ void tmem_ld16(uint32_t taddr, uint32_t (&v)[16])
         : "r"(taddr)
         : "memory");
     asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+}
+
+__device__ __forceinline__ void tmem_st32(uint32_t taddr, const uint32_t (&v)[32])
+{
+    asm volatile(
+        "tcgen05.st.sync.aligned.32x32b.x32.b32 [%0], "
+        "{%1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, %16, "
+        "%17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31, %32};\n" ::"r"(taddr),
+        "r"(v[0]), "r"(v[1]), "r"(v[2]), "r"(v[3]), "r"(v[4]), "r"(v[5]), "r"(v[6]), "r"(v[7]), "r"(v[8]), "r"(v[9]),
+        "r"(v[10]), "r"(v[11]), "r"(v[12]), "r"(v[13]), "r"(v[14]), "r"(v[15]), "r"(v[16]), "r"(v[17]), "r"(v[18]),
+        "r"(v[19]), "r"(v[20]), "r"(v[21]), "r"(v[22]), "r"(v[23]), "r"(v[24]), "r"(v[25]), "r"(v[26]), "r"(v[27]),
+        "r"(v[28]), "r"(v[29]), "r"(v[30]), "r"(v[31])
+        : "memory");
+    asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
 }
 
 struct Tile {
@@ -237,10 +238,11 @@ k_interval_fp4(const __grid_constant__ CUtensorMap mapU, const __grid_constant__
     // every role walks the same static schedule: tile t = blockIdx.x, + gridDim.x, ...
     if (warp >= EXP_WARP0) {
         // ===================================== expanders =====================================
-        const int e = tid - EXP_WARP0 * 32;
-        const bool isA = e < TM;
-        const int r = isA ? e : e - TM;
-        const uint32_t rows = isA ? TM : TN;
+        // expander warps 0-3 own the A rows (row = TMEM lane: warp w may only touch lanes 32 (w % 4) ..),
+        // warps 4-11 the B rows
+        const int ew = warp - EXP_WARP0;
+        const bool isA = ew < 4;
+        const int r = isA ? ((warp & 3) * 32 + lane) : ((ew - 4) * 32 + lane);
         uint32_t it = 0;   // global k-step counter (stage ring position)
         uint32_t grp = 0;  // global group counter (bit-buffer ring position)
         // TMA 64B swizzle: 16-byte chunk c of row e sits at chunk c ^ ((e >> 1) & 3)
@@ -261,19 +263,34 @@ k_interval_fp4(const __grid_constant__ CUtensorMap mapU, const __grid_constant__
                     const uint4 cur1 = *reinterpret_cast<const uint4 *>(my_bits + b * BITS_BYTES + (((2 * c + 1) ^ swz) << 4));
                     const int s = it % NS;
                     mbar_wait(&s_empty[s], ((it / NS) & 1) ^ 1);
-                    unsigned char *dst = s_stage + s * STAGE_BYTES + (isA ? 0 : A_BYTES) + r * 16;
                     const uint32_t xs[8] = {cur0.x, cur0.y, cur0.z, cur0.w, cur1.x, cur1.y, cur1.z, cur1.w};
+                    if (isA) {
+                        // 32 k -> 4 words of E2M1 nibbles (1.0 = 0b0010); 8 slices -> the 32 TMEM columns of stage s
+                        uint32_t w[32];
 #pragma unroll
-                    for (int q = 0; q < 8; q++) {     // 32 k -> one 16-byte chunk of E2M1 nibbles (1.0 = 0b0010)
-                        const uint32_t x = xs[q];
-                        uint4 w;
-                        w.x = (x << 1) & 0x22222222u;
-                        w.y = x & 0x22222222u;
-                        w.z = (x >> 1) & 0x22222222u;
-                        w.w = (x >> 2) & 0x22222222u;
-                        *reinterpret_cast<uint4 *>(dst + q * rows * 16) = w;
+                        for (int q = 0; q < 8; q++) {
+                            const uint32_t x = xs[q];
+                            w[4 * q + 0] = (x << 1) & 0x22222222u;
+                            w[4 * q + 1] = x & 0x22222222u;
+                            w[4 * q + 2] = (x >> 1) & 0x22222222u;
+                            w[4 * q + 3] = (x >> 2) & 0x22222222u;
+                        }
+                        tmem_st32(tmem_base + ((uint32_t)((warp & 3) * 32) << 16) + A_COL + s * 32, w);
+                        tc_fence_before();
+                    } else {
+                        unsigned char *dst = s_stage + s * STAGE_BYTES + r * 16;
+#pragma unroll
+                        for (int q = 0; q < 8; q++) {     // 32 k -> one 16-byte chunk of E2M1 nibbles
+                            const uint32_t x = xs[q];
+                            uint4 w;
+                            w.x = (x << 1) & 0x22222222u;
+                            w.y = x & 0x22222222u;
+                            w.z = (x >> 1) & 0x22222222u;
+                            w.w = (x >> 2) & 0x22222222u;
+                            *reinterpret_cast<uint4 *>(dst + q * TN * 16) = w;
+                        }
+                        fence_proxy_async();          // generic-proxy stores -> visible to the tensor core
                     }
-                    fence_proxy_async();          // generic-proxy stores -> visible to the tensor core
                     __syncwarp();
                     if (lane == 0) {
                         mbar_arrive(&s_full[s]);                          // one arrival per warp
@@ -321,13 +338,12 @@ k_interval_fp4(const __grid_constant__ CUtensorMap mapU, const __grid_constant__
                     const int s = it % NS;
                     mbar_wait(&s_full[s], (it / NS) & 1);
                     tc_fence_after();
-                    const uint32_t a_addr = smem_u32(s_stage + s * STAGE_BYTES);
-                    const uint32_t b_addr = a_addr + A_BYTES;
+                    const uint32_t b_addr = smem_u32(s_stage + s * STAGE_BYTES);
 #pragma unroll
-                    for (int q = 0; q < KBYTES / 32; q++) {
-                        const uint64_t ad = make_desc(a_addr + q * 2 * TM * 16, TM * 16, 128);
+                    for (int q = 0; q < KBYTES / 32; q++) {       // K = 64 per MMA: 8 TMEM columns of A, 2 chunks of B
                         const uint64_t bd = make_desc(b_addr + q * 2 * TN * 16, TN * 16, 128);
-                        mma_mxf4(d_tmem, ad, bd, IDESC, (ks > ks0 || q > 0) ? 1u : 0u, tmem_base + SFA_COL, tmem_base + SFB_COL);
+                        mma_mxf4(d_tmem, tmem_base + A_COL + s * 32 + q * 8, bd, IDESC, (ks > ks0 || q > 0) ? 1u : 0u,
+                                 tmem_base + SFA_COL, tmem_base + SFB_COL);
                     }
                     mma_commit(&s_empty[s]);                              // stage s free once these MMAs retire
                 }
@@ -339,7 +355,6 @@ k_interval_fp4(const __grid_constant__ CUtensorMap mapU, const __grid_constant__
         // ===================================== epilogue ======================================
         uint32_t tile_seq = 0;
         unsigned long long my_nrel = 0;
-        const uint32_t hist_saddr = smem_u32(s_hist);
         const uint32_t kmax32 = (uint32_t)kmax;
         int64_t cur_batch = -1;
         for (int64_t t = blockIdx.x; t < total_tiles; t += gridDim.x) {
