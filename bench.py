@@ -45,7 +45,7 @@ NCU_TRAFFIC = {1: 78.28e9, 2: 51.14e9, 3: None}
 TENSOR_OVER_BF16 = {2: 2.0, 3: 4.0}
 ROUTE_NAME = {1: "popc", 2: "tensor_int8", 3: "tensor_fp4"}
 ROUTE_DTYPE = {1: "u64", 2: "int8", 3: "fp4_e2m1"}
-ROUTE_KERNEL = {1: "k_interval_popc", 2: "k_interval_tensor", 3: "k_interval_fp4"}
+ROUTE_KERNEL = {1: "k_interval_popc", 2: "k_interval_tensor", 3: "k_interval_fp4", 4: "k_interval_pair"}
 
 
 def measured_peaks():

@@ -64,7 +64,9 @@ enum cs_route {
     CS_ROUTE_AUTO = 0,      /* the library's default for this N */
     CS_ROUTE_POPC = 1,      /* shared-memory tiled AND + POPC (Alg. 20 restated for the GPU) */
     CS_ROUTE_TENSOR = 2,    /* count matrix C.C as a 0/1 int8 contraction on tcgen05 tensor cores */
-    CS_ROUTE_TENSOR_FP4 = 3 /* the same contraction with 4-bit (E2M1, unit block scales) operands, fp32 accumulators */
+    CS_ROUTE_TENSOR_FP4 = 3,/* the same contraction with 4-bit (E2M1, unit block scales) operands, fp32 accumulators */
+    CS_ROUTE_TENSOR_PAIR = 4/* 4-bit operands on CTA pairs (cta_group::2, 256 x 256 tiles), shift-free expansion with
+                               constant power-of-two block scales, L2-aware tile order */
 };
 
 const char *cs_version(void);
@@ -118,7 +120,7 @@ int cs_interval_hist_ex(const uint64_t *bits, const uint64_t *bitsT, int64_t N, 
                         int64_t row_begin, int64_t row_end, int route,
                         int64_t *hist, int64_t *n_relations,
                         void *workspace, size_t workspace_bytes, void *stream);
-/* Route CS_ROUTE_AUTO resolves to for this N (one of the three concrete routes). */
+/* Route CS_ROUTE_AUTO resolves to for this N (one of the concrete routes). */
 int cs_default_route(int64_t N);
 
 /* a3: Benincasa-Dowker action, Eq. 4.10-4.12 with l/l_p = 1:

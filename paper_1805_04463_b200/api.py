@@ -24,6 +24,7 @@ ROUTE_AUTO = 0
 ROUTE_POPC = 1
 ROUTE_TENSOR = 2
 ROUTE_TENSOR_FP4 = 3
+ROUTE_TENSOR_PAIR = 4
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libcausalset.so")

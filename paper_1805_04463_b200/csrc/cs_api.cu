@@ -1,6 +1,6 @@
 // cs_api.cu -- the extern "C" boundary of libcausalset.so (include/causalset.h).
 // Argument checking, workspace carving and kernel sequencing only; the arithmetic lives in
-// cs_build.cu (a1), cs_interval_popc.cu / cs_interval_tensor.cu / cs_interval_fp4.cu (a2) and cs_action.cu (a3).
+// cs_build.cu (a1), cs_interval_popc.cu / cs_interval_tensor.cu / cs_interval_fp4.cu / cs_interval_pair.cu (a2) and cs_action.cu (a3).
 #include "cs_common.cuh"
 
 namespace cs {
@@ -25,7 +25,7 @@ int sm_count()
 static int resolve_route(int64_t N, int route)
 {
     if (route == CS_ROUTE_AUTO) route = cs_default_route(N);
-    if ((route == CS_ROUTE_TENSOR || route == CS_ROUTE_TENSOR_FP4) && !interval_tensor_available()) return -1;
+    if (route >= CS_ROUTE_TENSOR && !interval_tensor_available()) return -1;
     return route;
 }
 
@@ -34,6 +34,7 @@ static size_t interval_ws_bytes(int64_t B, int64_t N, int have_bitsT, int route)
     size_t ws = 256;   // tile counter etc.
     if (!have_bitsT) ws += align_up((size_t)B * N * row_stride_words(N) * 8, 256);
     if (route == CS_ROUTE_TENSOR) ws += align_up(interval_tensor_scratch_bytes(B, N), 256);
+    if (route == CS_ROUTE_TENSOR_PAIR) ws += align_up(interval_pair_scratch_bytes(N), 256);
     return ws;
 }
 
@@ -63,6 +64,9 @@ static int interval_hist_impl(const uint64_t *bits, const uint64_t *bitsT, int64
         if (rc) return rc;
         bitsT = t;
     }
+    if (route == CS_ROUTE_TENSOR_PAIR)
+        return launch_interval_pair(bits, bitsT, B, N, kmax, row_begin, row_end, hist, nrel, ws,
+                                    workspace_bytes - (size_t)(ws - static_cast<unsigned char *>(workspace)), st);
     if (route == CS_ROUTE_TENSOR_FP4)
         return launch_interval_fp4(bits, bitsT, B, N, kmax, row_begin, row_end, hist, nrel, ws,
                                    workspace_bytes - (size_t)(ws - static_cast<unsigned char *>(workspace)), st);
@@ -153,7 +157,7 @@ int cs_interval_hist_ex(const uint64_t *bits, const uint64_t *bitsT, int64_t N, 
                         void *workspace, size_t workspace_bytes, void *stream)
 {
     if (N < 0 || !hist || (N > 0 && !bits)) return CS_ERR_ARG;
-    if (route < CS_ROUTE_AUTO || route > CS_ROUTE_TENSOR_FP4) return CS_ERR_ARG;
+    if (route < CS_ROUTE_AUTO || route > CS_ROUTE_TENSOR_PAIR) return CS_ERR_ARG;
     return interval_hist_impl(bits, bitsT, 1, N, kmax, row_begin, row_end, route, hist, n_relations,
                               workspace, workspace_bytes, static_cast<cudaStream_t>(stream));
 }

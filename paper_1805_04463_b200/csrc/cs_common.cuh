@@ -68,6 +68,10 @@ size_t interval_tensor_scratch_bytes(int64_t B, int64_t N);
 int launch_interval_fp4(const uint64_t *bits, const uint64_t *bitsT, int64_t B, int64_t N, int64_t kmax,
                         int64_t row_begin, int64_t row_end, int64_t *hist, int64_t *nrel,
                         void *scratch, size_t scratch_bytes, cudaStream_t st);
+int launch_interval_pair(const uint64_t *bits, const uint64_t *bitsT, int64_t B, int64_t N, int64_t kmax,
+                         int64_t row_begin, int64_t row_end, int64_t *hist, int64_t *nrel,
+                         void *scratch, size_t scratch_bytes, cudaStream_t st);
+size_t interval_pair_scratch_bytes(int64_t N);
 bool interval_tensor_available();
 
 int launch_bd_action(const int64_t *hist, int64_t hist_stride, int64_t B, int64_t kmax, int64_t N, int dim,

@@ -1,0 +1,629 @@
+// cs_interval_pair.cu -- stage a2, tensor route on CTA pairs (tcgen05.mma.cta_group::2, kind::mxf4).
+//
+// count(i,j) = sum_k U[i][k] * L[j][k] over the K blocks between the I block and the J block
+// (Fig. 4.2 caption PAPER.md:1768; Alg. 20 line 9), histogrammed over related pairs.
+// Same contraction as cs_interval_fp4.cu, re-cut for the two SMs of a TPC:
+//
+//  * a cluster of two CTAs owns a 256 (i) x 256 (j) tile.  CTA r expands the 128 U rows
+//    I*256 + r*128 .. into its TMEM (A operand) and the 128 L rows J*256 + r*128 .. into its shared
+//    memory (its half of the B operand); one thread of CTA 0 issues M=256 N=256 K=64 MMAs for the
+//    pair.  Per SM and per k this halves the B expansion and the B shared-memory reads of the
+//    single-CTA kernel (the two tensor cores share each B half), and a third of the ALU work.
+//  * expansion without shifts: with x a 32-bit slice of a bit row, x & 0x11111111, x & 0x22222222 and
+//    x & 0x44444444 are already E2M1 nibbles (0.5, 1.0, 2.0 where the bit is set); only bit 3 of
+//    every nibble needs a shift ((x >> 3) & 0x11111111).  Each K=64 MMA takes one nibble position
+//    of eight slices, so its products are all 0.25, 1 or 4 -- undone exactly by constant UE8M0
+//    block scales 2^1, 2^0, 2^-1 kept in three TMEM regions.  k is permuted inside a 256-k stage,
+//    identically for both operands, which leaves the contraction unchanged.
+//  * tiles are visited in a table order (longest K first in bands of 8 diagonals, I-major inside
+//    a band) so that the ~74 tiles in flight share a few row panels in L2.
+//
+// Products are 0 or 1 and the fp32 accumulators are exact for counts < 2^24.
+#include <cuda.h>
+
+#include "cs_common.cuh"
+
+namespace cs {
+
+namespace {
+
+constexpr int TM = 128;                 // A rows (i) per CTA; the pair covers 256
+constexpr int TNH = 128;                // B rows (j) per CTA; the pair covers 256
+constexpr int TILE = 256;               // tile edge of the pair
+constexpr int KSTEP = 256;              // k per stage = 4 MMAs of K = 64
+constexpr int NS = 6;                   // operand stages (B in shared memory, A in TMEM)
+constexpr int GK = 2;                   // stages per staged group of bit rows
+constexpr int BROW = GK * 32;           // bytes per staged bit row (TMA box inner extent, 64B swizzle)
+constexpr int NB = 4;                   // bit-row buffers
+constexpr int EPITCH = 20;              // words per thread row of the epilogue staging area
+constexpr int EPI_BYTES = 256 * EPITCH * 4;
+constexpr int BITS_BYTES = (TM + TNH) * BROW;       // 16 KiB
+constexpr int STAGE_BYTES = TNH * (KSTEP / 2);      // 16 KiB: this CTA's half of B
+constexpr int HS = 2048;                // shared-memory histogram bins
+constexpr int BANDW = 8;                // diagonals per band of the tile order
+constexpr int EPI_WARPS = 8, MMA_WARP = 8, LOAD_WARP = 9, EXP_WARP0 = 10, EXP_WARPS = 8;
+constexpr int THREADS = (EPI_WARPS + 2 + EXP_WARPS) * 32;   // 576
+constexpr int SMEM_BYTES = NS * STAGE_BYTES + NB * BITS_BYTES + EPI_BYTES + HS * 4 + 512;
+
+// block-scaled instruction descriptor, kind::mxf4: A = B = E2M1 (1 at bits 7 and 10), both K-major,
+// N >> 3 at bit 17, scale format UE8M0 (bit 23), M >> 4 at bit 24 (M = 256 over the pair), K = 64
+constexpr uint32_t IDESC = (1u << 7) | (1u << 10) | ((uint32_t)(256 >> 3) << 17) | (1u << 23) | ((uint32_t)(256 >> 4) << 24);
+constexpr uint32_t SF_COL = 256;        // three 16-column regions of constant scale factors: 2^1, 2^0, 2^-1
+constexpr uint32_t A_COL = 320;         // TMEM ring of the A operand: NS x 32 columns
+static_assert(A_COL + NS * 32 <= 512, "TMEM columns");
+static_assert(SMEM_BYTES <= 227 * 1024, "shared memory");
+
+__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(uint64_t *bar, uint32_t count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t *bar)
+{
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+// arrive on the barrier at the same shared-memory offset in CTA `cta` of the cluster.  Default
+// (CTA-scope) release: what the arrival publishes is consumed by the tensor cores, for which the
+// writers have already issued fence.proxy.async / tcgen05.wait::st + fence::before_thread_sync;
+// a cluster-scope release compiles to MEMBAR.ALL.GPU and a cluster-scope acquire to CCTL.IVALL
+// (measured: 28.3 ms instead of 20 ms at N = 65536).
+__device__ __forceinline__ void mbar_arrive_cluster(uint64_t *bar, uint32_t cta)
+{
+    uint32_t ra;
+    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(ra) : "r"(smem_u32(bar)), "r"(cta));
+    asm volatile("mbarrier.arrive.shared::cluster.b64 _, [%0];" ::"r"(ra) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity)
+{
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "LAB_WAIT:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra LAB_DONE;\n"
+        "bra LAB_WAIT;\n"
+        "LAB_DONE:\n"
+        "}\n" ::"r"(smem_u32(bar)),
+        "r"(parity)
+        : "memory");
+}
+// wait on a barrier that also receives arrivals from the peer CTA (see mbar_arrive_cluster)
+__device__ __forceinline__ void mbar_wait_cluster(uint64_t *bar, uint32_t parity)
+{
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "LAB_WAIT:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra LAB_DONE;\n"
+        "bra LAB_WAIT;\n"
+        "LAB_DONE:\n"
+        "}\n" ::"r"(smem_u32(bar)),
+        "r"(parity)
+        : "memory");
+}
+__device__ __forceinline__ void mbar_arrive_expect_tx(uint64_t *bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void tma_load_3d(void *dst, const CUtensorMap *map, int c0, int c1, int c2, uint64_t *bar)
+{
+    asm volatile(
+        "cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];" ::"r"(
+            smem_u32(dst)),
+        "l"(map), "r"(c0), "r"(c1), "r"(c2), "r"(smem_u32(bar))
+        : "memory");
+}
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+__device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void cluster_sync()
+{
+    asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory");
+    asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
+__device__ __forceinline__ uint32_t cluster_ctarank()
+{
+    uint32_t r;
+    asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r));
+    return r;
+}
+__device__ __forceinline__ uint32_t cluster_id_x()
+{
+    uint32_t r;
+    asm volatile("mov.u32 %0, %%clusterid.x;" : "=r"(r));
+    return r;
+}
+__device__ __forceinline__ uint32_t num_clusters_x()
+{
+    uint32_t r;
+    asm volatile("mov.u32 %0, %%nclusterid.x;" : "=r"(r));
+    return r;
+}
+
+// shared-memory matrix descriptor: no swizzle, K-major; addresses and offsets in 16-byte units
+__device__ __forceinline__ uint64_t make_desc(uint32_t saddr, uint32_t lbo_bytes, uint32_t sbo_bytes)
+{
+    uint64_t d = 0;
+    d |= (uint64_t)((saddr >> 4) & 0x3FFF);
+    d |= (uint64_t)((lbo_bytes >> 4) & 0x3FFF) << 16;
+    d |= (uint64_t)((sbo_bytes >> 4) & 0x3FFF) << 32;
+    d |= (uint64_t)1 << 46;   // descriptor version (Blackwell)
+    return d;                 // layout_type = 0 (SWIZZLE_NONE), base_offset = 0, lbo_mode = 0
+}
+
+// D[tmem] (+)= A[tmem] . B[smem], M = 256 over the CTA pair; issued by one thread of CTA 0
+__device__ __forceinline__ void mma_mxf4_pair(uint32_t d_tmem, uint32_t a_tmem, uint64_t bdesc, uint32_t idesc,
+                                              uint32_t accum, uint32_t sfa, uint32_t sfb)
+{
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "setp.ne.b32 p, %4, 0;\n"
+        "tcgen05.mma.cta_group::2.kind::mxf4.block_scale.block32 [%0], [%1], %2, %3, [%5], [%6], p;\n"
+        "}\n" ::"r"(d_tmem),
+        "r"(a_tmem), "l"(bdesc), "r"(idesc), "r"(accum), "r"(sfa), "r"(sfb)
+        : "memory");
+}
+// the barrier at this shared-memory offset in both CTAs of the pair gets one arrival when the
+// MMAs issued so far have retired
+__device__ __forceinline__ void mma_commit_pair(uint64_t *bar)
+{
+    asm volatile(
+        "tcgen05.commit.cta_group::2.mbarrier::arrive::one.shared::cluster.multicast::cluster.b64 [%0], %1;" ::"r"(
+            smem_u32(bar)),
+        "h"((uint16_t)3)
+        : "memory");
+}
+
+__device__ __forceinline__ void tmem_st16_const(uint32_t taddr, uint32_t val)
+{
+    asm volatile(
+        "tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], "
+        "{%1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1, %1};\n" ::"r"(taddr),
+        "r"(val)
+        : "memory");
+    asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
+}
+__device__ __forceinline__ void tmem_ld16(uint32_t taddr, uint32_t (&v)[16])
+{
+    asm volatile(
+        "tcgen05.ld.sync.aligned.32x32b.x16.b32 "
+        "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15}, [%16];\n"
+        : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]),
+          "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15])
+        : "r"(taddr)
+        : "memory");
+    asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+}
+__device__ __forceinline__ void tmem_st32(uint32_t taddr, const uint32_t (&v)[32])
+{
+    asm volatile(
+        "tcgen05.st.sync.aligned.32x32b.x32.b32 [%0], "
+        "{%1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, %16, "
+        "%17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31, %32};\n" ::"r"(taddr),
+        "r"(v[0]), "r"(v[1]), "r"(v[2]), "r"(v[3]), "r"(v[4]), "r"(v[5]), "r"(v[6]), "r"(v[7]), "r"(v[8]), "r"(v[9]),
+        "r"(v[10]), "r"(v[11]), "r"(v[12]), "r"(v[13]), "r"(v[14]), "r"(v[15]), "r"(v[16]), "r"(v[17]), "r"(v[18]),
+        "r"(v[19]), "r"(v[20]), "r"(v[21]), "r"(v[22]), "r"(v[23]), "r"(v[24]), "r"(v[25]), "r"(v[26]), "r"(v[27]),
+        "r"(v[28]), "r"(v[29]), "r"(v[30]), "r"(v[31])
+        : "memory");
+    asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
+}
+
+// E2M1 nibbles of nibble position Q of a 32-bit slice (values 0.5, 1, 2, 0.5 where the bit is set)
+template <int Q>
+__device__ __forceinline__ uint32_t nib(uint32_t x)
+{
+    if (Q == 0) return x & 0x11111111u;
+    if (Q == 1) return x & 0x22222222u;
+    if (Q == 2) return x & 0x44444444u;
+    return (x >> 3) & 0x11111111u;
+}
+// UE8M0 block scale that turns the products of nibble position q into exactly 1: 2^1, 2^0, 2^-1, 2^1
+__device__ __forceinline__ uint32_t sf_col(int q) { return SF_COL + (q == 1 ? 16u : q == 2 ? 32u : 0u); }
+
+// ---- tile order ---------------------------------------------------------------------------------
+// Tiles (I, J = I + d), 0 <= I, I + d < nT, in bands of BANDW diagonals, longest (largest d) first;
+// inside a band I-major, then d ascending.  Entry = (I << 16) | J.  nT (nT + 1) / 2 entries.
+__host__ __device__ inline int64_t band_tiles(int nT, int dlo, int dhi)   // sum over d of (nT - d)
+{
+    const int64_t w = dhi - dlo + 1;
+    return w * nT - w * (int64_t)(dlo + dhi) / 2;
+}
+
+__global__ void k_pair_tile_order(int nT, uint32_t *__restrict__ tab)
+{
+    const int b = blockIdx.x;
+    const int dhi = nT - 1 - b * BANDW;
+    const int dlo = dhi - BANDW + 1 > 0 ? dhi - BANDW + 1 : 0;
+    const int w = dhi - dlo + 1;
+    int64_t off = 0;
+    for (int bb = 0; bb < b; bb++) {
+        const int h = nT - 1 - bb * BANDW;
+        const int l = h - BANDW + 1 > 0 ? h - BANDW + 1 : 0;
+        off += band_tiles(nT, l, h);
+    }
+    const int full = nT - dhi;   // rows I < full have all w diagonals inside the matrix
+    for (int I = threadIdx.x; I + dlo < nT; I += blockDim.x) {
+        int64_t pos;
+        if (I <= full) pos = (int64_t)I * w;
+        else {
+            const int64_t m = I - full;   // rows full .. I-1 hold nT - dlo - I' entries each
+            pos = (int64_t)full * w + m * (nT - dlo) - (int64_t)(full + I - 1) * m / 2;
+        }
+        for (int d = dlo; d <= dhi && I + d < nT; d++) tab[off + pos + (d - dlo)] = ((uint32_t)I << 16) | (uint32_t)(I + d);
+    }
+}
+
+struct Tile {
+    int I, J;      // 256-row blocks of i and of j
+    int64_t b;     // causet
+    bool skip;     // no row of the tile inside [row_begin, row_end)
+};
+
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(THREADS, 1)
+k_interval_pair(const __grid_constant__ CUtensorMap mapU, const __grid_constant__ CUtensorMap mapL,
+                const uint64_t *__restrict__ bits, const uint32_t *__restrict__ tile_tab,
+                int64_t B, int64_t N, int64_t stride, int64_t kmax,
+                int64_t row_begin, int64_t row_end,
+                unsigned long long *__restrict__ hist, unsigned long long *__restrict__ nrel)
+{
+    extern __shared__ __align__(1024) unsigned char smem[];
+    unsigned char *s_stage = smem;
+    unsigned char *s_bits = smem + NS * STAGE_BYTES;
+    uint32_t *s_epi = reinterpret_cast<uint32_t *>(smem + NS * STAGE_BYTES + NB * BITS_BYTES);
+    uint32_t *s_hist = reinterpret_cast<uint32_t *>(smem + NS * STAGE_BYTES + NB * BITS_BYTES + EPI_BYTES);
+    uint64_t *s_full = reinterpret_cast<uint64_t *>(smem + NS * STAGE_BYTES + NB * BITS_BYTES + EPI_BYTES + HS * 4);
+    uint64_t *s_empty = s_full + NS;      // [NS] stage free again (multicast commit from CTA 0)
+    uint64_t *s_tfull = s_empty + NS;     // [1] accumulator complete (multicast commit)
+    uint64_t *s_tempty = s_tfull + 1;     // [1] accumulator drained (used in CTA 0 only)
+    uint64_t *s_bfull = s_tempty + 1;     // [NB] staged bit rows have landed
+    uint64_t *s_bempty = s_bfull + NB;    // [NB] every expander warp is done with the buffer
+    uint32_t *s_tmem = reinterpret_cast<uint32_t *>(s_bempty + NB);
+
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const uint32_t rank = cluster_ctarank();
+    const int nT = (int)((N + TILE - 1) / TILE);
+    const int64_t tiles_per = (int64_t)nT * (nT + 1) / 2;
+    const int64_t total_tiles = tiles_per * B;
+    const int64_t t0 = cluster_id_x(), tstep = num_clusters_x();
+    const int hs = (int)((kmax + 1 < HS) ? (kmax + 1) : HS);
+    const int64_t hist_len = kmax + 1;
+
+    auto get_tile = [&](int64_t t) {
+        Tile tc;
+        tc.b = t / tiles_per;
+        const uint32_t e = __ldg(tile_tab + (t - tc.b * tiles_per));
+        tc.I = (int)(e >> 16);
+        tc.J = (int)(e & 0xFFFFu);
+        tc.skip = (int64_t)tc.I * TILE >= row_end || (int64_t)(tc.I + 1) * TILE <= row_begin;
+        return tc;
+    };
+
+    if (tid == 0) {
+        for (int s = 0; s < NS; s++) {
+            mbar_init(&s_full[s], 2 * EXP_WARPS);   // expander warps of both CTAs (counted in CTA 0)
+            mbar_init(&s_empty[s], 1);
+        }
+        for (int b = 0; b < NB; b++) {
+            mbar_init(&s_bfull[b], 1);
+            mbar_init(&s_bempty[b], EXP_WARPS);
+        }
+        mbar_init(s_tfull, 1);
+        mbar_init(s_tempty, 2 * EPI_WARPS);         // epilogue warps of both CTAs (counted in CTA 0)
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    for (int b = tid; b < HS; b += THREADS) s_hist[b] = 0;
+    if (warp == MMA_WARP) {   // all 512 TMEM columns of both SMs of the pair
+        asm volatile("tcgen05.alloc.cta_group::2.sync.aligned.shared::cta.b32 [%0], 512;" ::"r"(smem_u32(s_tmem)));
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::2.sync.aligned;");
+    }
+    tc_fence_before();
+    __syncthreads();
+    cluster_sync();           // barriers of the peer are initialised before anyone arrives on them
+    tc_fence_after();
+    const uint32_t tmem_base = *s_tmem;
+    if (warp < 4) {           // constant UE8M0 block scales: 2^1, 2^0, 2^-1 in every byte of their region
+        const uint32_t sf = tmem_base + ((uint32_t)(warp * 32) << 16) + SF_COL;
+        tmem_st16_const(sf, 0x80808080u);
+        tmem_st16_const(sf + 16, 0x7F7F7F7Fu);
+        tmem_st16_const(sf + 32, 0x7E7E7E7Eu);
+    }
+    tc_fence_before();
+    __syncthreads();
+    cluster_sync();
+    tc_fence_after();
+
+    // every role of both CTAs walks the same static schedule: tile t = cluster id, + number of clusters, ...
+    if (warp >= EXP_WARP0) {
+        // ===================================== expanders =====================================
+        // warps 0-3 own this CTA's 128 A rows (row = TMEM lane: warp w may only touch lanes 32 (w % 4) ..),
+        // warps 4-7 its 128 B rows
+        const int ew = warp - EXP_WARP0;
+        const bool isA = ew < 4;
+        const int r = isA ? ((warp & 3) * 32 + lane) : ((ew - 4) * 32 + lane);
+        uint32_t it = 0;   // global stage counter (operand ring position)
+        uint32_t grp = 0;  // global group counter (bit-buffer ring position)
+        // TMA 64B swizzle: 16-byte chunk c of row e sits at chunk c ^ ((e >> 1) & 3)
+        const unsigned char *my_bits = s_bits + (isA ? 0 : TM * BROW) + r * BROW;
+        const int swz = (r >> 1) & 3;
+        for (int64_t t = t0; t < total_tiles; t += tstep) {
+            const Tile tc = get_tile(t);
+            if (tc.skip) continue;
+            const int nstages = tc.J - tc.I + 1;
+            const int ngroups = (nstages + GK - 1) / GK;
+            for (int g = 0; g < ngroups; g++, grp++) {
+                const int b = grp % NB;
+                mbar_wait(&s_bfull[b], (grp / NB) & 1);
+                const int kcount = (nstages - g * GK < GK) ? (nstages - g * GK) : GK;
+                for (int c = 0; c < kcount; c++, it++) {
+                    const uint4 cur0 = *reinterpret_cast<const uint4 *>(my_bits + b * BITS_BYTES + (((2 * c) ^ swz) << 4));
+                    const uint4 cur1 = *reinterpret_cast<const uint4 *>(my_bits + b * BITS_BYTES + (((2 * c + 1) ^ swz) << 4));
+                    const int s = it % NS;
+                    const uint32_t xs[8] = {cur0.x, cur0.y, cur0.z, cur0.w, cur1.x, cur1.y, cur1.z, cur1.w};
+                    if (isA) {
+                        // TMEM column 8 q + j of stage s = nibble position q of slice j
+                        uint32_t w[32];
+#pragma unroll
+                        for (int j = 0; j < 8; j++) {
+                            w[j] = nib<0>(xs[j]);
+                            w[8 + j] = nib<1>(xs[j]);
+                            w[16 + j] = nib<2>(xs[j]);
+                            w[24 + j] = nib<3>(xs[j]);
+                        }
+                        mbar_wait(&s_empty[s], ((it / NS) & 1) ^ 1);
+                        tc_fence_after();
+                        tmem_st32(tmem_base + ((uint32_t)((warp & 3) * 32) << 16) + A_COL + s * 32, w);
+                        tc_fence_before();
+                    } else {
+                        // 16-byte chunk 2 q + h of this row = nibble position q of slices 4 h .. 4 h + 3
+                        uint4 w[8];
+#pragma unroll
+                        for (int h = 0; h < 2; h++) {
+                            w[0 + h] = make_uint4(nib<0>(xs[4 * h]), nib<0>(xs[4 * h + 1]), nib<0>(xs[4 * h + 2]), nib<0>(xs[4 * h + 3]));
+                            w[2 + h] = make_uint4(nib<1>(xs[4 * h]), nib<1>(xs[4 * h + 1]), nib<1>(xs[4 * h + 2]), nib<1>(xs[4 * h + 3]));
+                            w[4 + h] = make_uint4(nib<2>(xs[4 * h]), nib<2>(xs[4 * h + 1]), nib<2>(xs[4 * h + 2]), nib<2>(xs[4 * h + 3]));
+                            w[6 + h] = make_uint4(nib<3>(xs[4 * h]), nib<3>(xs[4 * h + 1]), nib<3>(xs[4 * h + 2]), nib<3>(xs[4 * h + 3]));
+                        }
+                        mbar_wait(&s_empty[s], ((it / NS) & 1) ^ 1);
+                        unsigned char *dst = s_stage + s * STAGE_BYTES + r * 16;
+#pragma unroll
+                        for (int q = 0; q < 8; q++) *reinterpret_cast<uint4 *>(dst + q * TNH * 16) = w[q];
+                        fence_proxy_async();          // generic-proxy stores -> visible to the tensor cores
+                    }
+                    __syncwarp();
+                    if (lane == 0) {
+                        mbar_arrive_cluster(&s_full[s], 0);               // one arrival per warp, in CTA 0
+                        // last stage of the buffer has been loaded AND consumed by every lane (the
+                        // stores above depend on it): hand the bit buffer back to the loader
+                        if (c == kcount - 1) mbar_arrive(&s_bempty[b]);
+                    }
+                }
+            }
+        }
+    } else if (warp == LOAD_WARP) {
+        // ===================================== TMA loader ====================================
+        if (lane == 0) {
+            uint32_t grp = 0;
+            for (int64_t t = t0; t < total_tiles; t += tstep) {
+                const Tile tc = get_tile(t);
+                if (tc.skip) continue;
+                const int nstages = tc.J - tc.I + 1;
+                const int ngroups = (nstages + GK - 1) / GK;
+                for (int g = 0; g < ngroups; g++, grp++) {
+                    const int b = grp % NB;
+                    mbar_wait(&s_bempty[b], ((grp / NB) & 1) ^ 1);
+                    mbar_arrive_expect_tx(&s_bfull[b], (uint32_t)BITS_BYTES);   // out-of-bounds is zero-filled
+                    unsigned char *dst = s_bits + b * BITS_BYTES;
+                    const int c0 = (tc.I * (KSTEP / 8)) + g * BROW;             // byte column of the first k
+                    tma_load_3d(dst, &mapU, c0, tc.I * TILE + (int)rank * TM, (int)tc.b, &s_bfull[b]);
+                    tma_load_3d(dst + TM * BROW, &mapL, c0, tc.J * TILE + (int)rank * TNH, (int)tc.b, &s_bfull[b]);
+                }
+            }
+        }
+    } else if (warp == MMA_WARP) {
+        // ===================================== MMA issuer (CTA 0 only) =======================
+        if (rank == 0 && lane == 0) {
+            uint32_t it = 0, tile_seq = 0;
+            for (int64_t t = t0; t < total_tiles; t += tstep) {
+                const Tile tc = get_tile(t);
+                if (tc.skip) continue;
+                const int nstages = tc.J - tc.I + 1;
+                mbar_wait_cluster(s_tempty, (tile_seq & 1) ^ 1);          // both epilogues have drained the accumulator
+                tc_fence_after();
+                for (int ks = 0; ks < nstages; ks++, it++) {
+                    const int s = it % NS;
+                    mbar_wait_cluster(&s_full[s], (it / NS) & 1);
+                    tc_fence_after();
+                    const uint32_t b_addr = smem_u32(s_stage + s * STAGE_BYTES);
+#pragma unroll
+                    for (int q = 0; q < 4; q++) {     // K = 64 per MMA: 8 TMEM columns of A, 2 chunks of B
+                        const uint64_t bd = make_desc(b_addr + q * 2 * TNH * 16, TNH * 16, 128);
+                        const uint32_t sf = tmem_base + sf_col(q);
+                        mma_mxf4_pair(tmem_base, tmem_base + A_COL + s * 32 + q * 8, bd, IDESC, (ks > 0 || q > 0) ? 1u : 0u, sf, sf);
+                    }
+                    mma_commit_pair(&s_empty[s]);                         // stage s free in both CTAs once these MMAs retire
+                }
+                mma_commit_pair(s_tfull);                                 // accumulator complete, both CTAs
+                tile_seq++;
+            }
+        }
+    } else {
+        // ===================================== epilogue ======================================
+        // this CTA's accumulator: rows I*256 + rank*128 + TMEM lane, columns J*256 ..
+        uint32_t tile_seq = 0;
+        unsigned long long my_nrel = 0;
+        const uint32_t kmax32 = (uint32_t)kmax;
+        int64_t cur_batch = -1;
+        const int quarter = warp & 3, colhalf = warp >> 2;   // TMEM lane quarter; which 128 columns
+        for (int64_t t = t0; t < total_tiles; t += tstep) {
+            const Tile tc = get_tile(t);
+            if (tc.skip) continue;
+            if (tc.b != cur_batch) {   // per-causet histograms: flush before switching
+                if (cur_batch >= 0 && B > 1) {
+                    asm volatile("bar.sync 1, 256;");
+                    for (int b = tid; b < hs; b += EPI_WARPS * 32) {
+                        uint32_t v = s_hist[b];
+                        if (v) { atomicAdd(&hist[cur_batch * hist_len + b], (unsigned long long)v); s_hist[b] = 0; }
+                    }
+                    asm volatile("bar.sync 1, 256;");
+                }
+                cur_batch = tc.b;
+            }
+            const int64_t i = (int64_t)tc.I * TILE + rank * TM + quarter * 32 + lane;   // this thread's row
+            const bool row_ok = i < N && i >= row_begin && i < row_end;
+            uint64_t rel[2] = {0, 0};                            // relation bits of this warp's 128 columns
+            if (row_ok) {
+                const uint64_t *urow = bits + tc.b * N * stride + i * stride;
+#pragma unroll
+                for (int w = 0; w < 2; w++) {
+                    const int64_t wi = (int64_t)tc.J * 4 + colhalf * 2 + w;
+                    if (wi < stride) rel[w] = __ldg(urow + wi);
+                }
+            }
+            unsigned long long *ghist = hist + cur_batch * hist_len;
+            mbar_wait(s_tfull, tile_seq & 1);
+            tc_fence_after();
+            const uint32_t taddr = tmem_base + ((uint32_t)(quarter * 32) << 16) + colhalf * 128;
+            uint32_t *my = s_epi + tid * EPITCH;
+            auto tally = [&](uint32_t word) {
+                const uint32_t cnt = (uint32_t)__uint_as_float(word);   // products are 0 or 1: exact in fp32
+                if (cnt < (uint32_t)hs) atomicAdd(&s_hist[cnt], 1u);
+                else if (cnt <= kmax32) atomicAdd(&ghist[cnt], 1ULL);
+            };
+#pragma unroll
+            for (int c16 = 0; c16 < 8; c16++) {
+                const uint32_t rel16 = (uint32_t)(rel[c16 >> 2] >> (16 * (c16 & 3))) & 0xFFFFu;
+                if (!__any_sync(0xffffffffu, rel16 != 0)) continue;
+                uint32_t v[16];
+                tmem_ld16(taddr + c16 * 16, v);
+                if (rel16 == 0) continue;
+                my_nrel += __popc(rel16);
+                // stage the 16 counts in this thread's private shared-memory row, then visit only the
+                // columns whose relation bit is set, two per iteration
+#pragma unroll
+                for (int c4 = 0; c4 < 4; c4++)
+                    *reinterpret_cast<uint4 *>(my + 4 * c4) = make_uint4(v[4 * c4], v[4 * c4 + 1], v[4 * c4 + 2], v[4 * c4 + 3]);
+                uint32_t m = rel16;
+                while (m) {
+                    const int c0 = __ffs(m) - 1;
+                    m &= m - 1;
+                    const bool two = m != 0;
+                    const int c1 = two ? __ffs(m) - 1 : c0;
+                    m &= m - 1;
+                    const uint32_t w0 = my[c0], w1 = my[c1];
+                    tally(w0);
+                    if (two) tally(w1);
+                }
+            }
+            tc_fence_before();
+            __syncwarp();
+            if (lane == 0) mbar_arrive_cluster(s_tempty, 0);   // one arrival per warp, in CTA 0
+            tile_seq++;
+        }
+        // final flush by the epilogue warps
+        asm volatile("bar.sync 1, 256;");
+        if (cur_batch >= 0) {
+            for (int b = tid; b < hs; b += EPI_WARPS * 32) {
+                uint32_t v = s_hist[b];
+                if (v) atomicAdd(&hist[cur_batch * hist_len + b], (unsigned long long)v);
+            }
+        }
+        if (nrel && B == 1) {
+#pragma unroll
+            for (int s = 16; s >= 1; s >>= 1) my_nrel += __shfl_xor_sync(0xffffffffu, my_nrel, s);
+            if (lane == 0 && my_nrel) atomicAdd(nrel, my_nrel);
+        }
+    }
+
+    // neither CTA may leave (or free its TMEM) while the peer can still reach it
+    tc_fence_before();
+    __syncthreads();
+    cluster_sync();
+    if (warp == MMA_WARP) {
+        asm volatile("tcgen05.dealloc.cta_group::2.sync.aligned.b32 %0, 512;" ::"r"(tmem_base));
+    }
+}
+
+}  // namespace
+
+// cuTensorMapEncodeTiled through the runtime's driver entry point (no link against libcuda)
+typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
+                                  const cuuint64_t *, const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+static EncodeTiledFn pair_encode_fn()
+{
+    static EncodeTiledFn fn = nullptr;
+    if (!fn) {
+        void *p = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess &&
+            q == cudaDriverEntryPointSuccess)
+            fn = reinterpret_cast<EncodeTiledFn>(p);
+    }
+    return fn;
+}
+
+// bit matrix [B][N][stride uint64] seen as bytes: dims {stride*8, N, B}; box {BROW bytes, rows, 1}
+static int pair_bits_map(CUtensorMap *map, const uint64_t *base, int64_t B, int64_t N, int64_t stride, int rows)
+{
+    EncodeTiledFn fn = pair_encode_fn();
+    if (!fn) {
+        snprintf(g_cuda_err, sizeof(g_cuda_err), "cuTensorMapEncodeTiled entry point not available");
+        return CS_ERR_CUDA;
+    }
+    cuuint64_t gdim[3] = {(cuuint64_t)(stride * 8), (cuuint64_t)N, (cuuint64_t)B};
+    cuuint64_t gstr[2] = {(cuuint64_t)(stride * 8), (cuuint64_t)(N * stride * 8)};
+    cuuint32_t box[3] = {(cuuint32_t)BROW, (cuuint32_t)rows, 1};
+    cuuint32_t estr[3] = {1, 1, 1};
+    CUresult r = fn(map, CU_TENSOR_MAP_DATA_TYPE_UINT8, 3, const_cast<uint64_t *>(base), gdim, gstr, box, estr,
+                    CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_64B, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+                    CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) {
+        snprintf(g_cuda_err, sizeof(g_cuda_err), "cuTensorMapEncodeTiled failed (%d)", (int)r);
+        return CS_ERR_CUDA;
+    }
+    return CS_OK;
+}
+
+size_t interval_pair_scratch_bytes(int64_t N)
+{
+    const int64_t nT = (N + TILE - 1) / TILE;
+    return (size_t)(nT * (nT + 1) / 2) * sizeof(uint32_t);
+}
+
+int launch_interval_pair(const uint64_t *bits, const uint64_t *bitsT, int64_t B, int64_t N, int64_t kmax,
+                         int64_t row_begin, int64_t row_end, int64_t *hist, int64_t *nrel,
+                         void *scratch, size_t scratch_bytes, cudaStream_t st)
+{
+    if (N > ((int64_t)1 << 24)) return CS_ERR_ARG;   // counts must stay exact in fp32; tile ids are 16 bits
+    if (!scratch || scratch_bytes < interval_pair_scratch_bytes(N)) return CS_ERR_WORKSPACE;
+    static bool attr_set = false;
+    if (!attr_set) {
+        CS_CUDA(cudaFuncSetAttribute(k_interval_pair, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES));
+        attr_set = true;
+    }
+    const int64_t stride = row_stride_words(N);
+    CUtensorMap mapU, mapL;
+    int rc = pair_bits_map(&mapU, bits, B, N, stride, TM);
+    if (rc) return rc;
+    rc = pair_bits_map(&mapL, bitsT, B, N, stride, TNH);
+    if (rc) return rc;
+    const int nT = (int)((N + TILE - 1) / TILE);
+    uint32_t *tab = static_cast<uint32_t *>(scratch);
+    k_pair_tile_order<<<(nT + BANDW - 1) / BANDW, 128, 0, st>>>(nT, tab);
+    CS_LAUNCHED("k_pair_tile_order");
+    const int64_t total = (int64_t)nT * (nT + 1) / 2 * B;
+    int64_t clusters = sm_count() / 2;
+    if (clusters > total) clusters = total;
+    if (clusters < 1) clusters = 1;
+    k_interval_pair<<<(unsigned)(2 * clusters), THREADS, SMEM_BYTES, st>>>(
+        mapU, mapL, bits, tab, B, N, stride, kmax, row_begin, row_end,
+        reinterpret_cast<unsigned long long *>(hist), reinterpret_cast<unsigned long long *>(nrel));
+    CS_LAUNCHED("k_interval_pair");
+    return CS_OK;
+}
+
+}  // namespace cs

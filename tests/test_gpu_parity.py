@@ -34,7 +34,7 @@ def api():
 
 def routes(api):
     r = [api.ROUTE_POPC]
-    for cand in (api.ROUTE_TENSOR, api.ROUTE_TENSOR_FP4):
+    for cand in (api.ROUTE_TENSOR, api.ROUTE_TENSOR_FP4, api.ROUTE_TENSOR_PAIR):
         try:
             x = torch.zeros((128, 2), dtype=torch.int64, device="cuda")
             api.interval_hist(x, x, 128, route=cand)
