@@ -40,11 +40,11 @@ UNIT = "word-ops/s"
 POPC_PER_CLK_SM = 16.0
 # dram__bytes_read.sum + dram__bytes_write.sum of one launch of the a2 kernel at config 3, from the
 # `ncu --set full` captures summarised under profiles/ (bytes per launch; None = not captured)
-NCU_TRAFFIC = {1: 78.28e9, 2: 51.14e9, 3: None}
+NCU_TRAFFIC = {1: 78.28e9, 2: 51.14e9, 3: 38.12e9, 4: None}
 # tensor peaks = measured bf16 dense peak x the guide's nominal ratio (bf16 2.25, int8/fp8 4.5, fp4 9 PFLOP/s)
-TENSOR_OVER_BF16 = {2: 2.0, 3: 4.0}
-ROUTE_NAME = {1: "popc", 2: "tensor_int8", 3: "tensor_fp4"}
-ROUTE_DTYPE = {1: "u64", 2: "int8", 3: "fp4_e2m1"}
+TENSOR_OVER_BF16 = {2: 2.0, 3: 4.0, 4: 4.0}
+ROUTE_NAME = {1: "popc", 2: "tensor_int8", 3: "tensor_fp4", 4: "tensor_fp4_pair"}
+ROUTE_DTYPE = {1: "u64", 2: "int8", 3: "fp4_e2m1", 4: "fp4_e2m1"}
 ROUTE_KERNEL = {1: "k_interval_popc", 2: "k_interval_tensor", 3: "k_interval_fp4", 4: "k_interval_pair"}
 
 
@@ -187,7 +187,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=3, help="BASELINE.json workload 1..4 (default 3: N=65536, 3+1)")
     ap.add_argument("--N", type=int, default=0, help="override N (debug only; the line then names it)")
-    ap.add_argument("--route", type=int, default=0, help="0 auto, 1 popc, 2 tensor int8, 3 tensor fp4")
+    ap.add_argument("--route", type=int, default=0, help="0 auto, 1 popc, 2 tensor int8, 3 tensor fp4, 4 tensor fp4 on CTA pairs")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=12.0)
     ap.add_argument("--ref-seconds", type=float, default=6.0)

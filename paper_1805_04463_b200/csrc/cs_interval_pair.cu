@@ -35,15 +35,22 @@ constexpr int NS = 6;                   // operand stages (B in shared memory, A
 constexpr int GK = 2;                   // stages per staged group of bit rows
 constexpr int BROW = GK * 32;           // bytes per staged bit row (TMA box inner extent, 64B swizzle)
 constexpr int NB = 4;                   // bit-row buffers
-constexpr int EPITCH = 20;              // words per thread row of the epilogue staging area
-constexpr int EPI_BYTES = 256 * EPITCH * 4;
 constexpr int BITS_BYTES = (TM + TNH) * BROW;       // 16 KiB
 constexpr int STAGE_BYTES = TNH * (KSTEP / 2);      // 16 KiB: this CTA's half of B
 constexpr int HS = 2048;                // shared-memory histogram bins
 constexpr int BANDW = 8;                // diagonals per band of the tile order
-constexpr int EPI_WARPS = 8, MMA_WARP = 8, LOAD_WARP = 9, EXP_WARP0 = 10, EXP_WARPS = 8;
-constexpr int THREADS = (EPI_WARPS + 2 + EXP_WARPS) * 32;   // 576
-constexpr int SMEM_BYTES = NS * STAGE_BYTES + NB * BITS_BYTES + EPI_BYTES + HS * 4 + 512;
+#ifndef CS_PAIR_DIAG
+#define CS_PAIR_DIAG 0      // timing experiments only (results are wrong): 1 no B stores, 2 no A stores, 4 no tally
+#endif
+#ifndef CS_PAIR_ROT_IMAD
+#define CS_PAIR_ROT_IMAD 0
+#endif
+// five warpgroups: 0-1 epilogue (warp & 3 = TMEM lane quarter, warp >> 2 = column half), 2 A expanders,
+// 3 B expanders, 4 = MMA issuer, TMA loader and two idle warps.  The epilogue keeps a whole accumulator
+// row slice (128 columns) in registers, so registers are re-split by warpgroup with setmaxnreg.
+constexpr int EPI_WARPS = 8, EXPA_WARP0 = 8, EXPB_WARP0 = 12, EXP_WARPS = 8, MMA_WARP = 16, LOAD_WARP = 17;
+constexpr int THREADS = 20 * 32;
+constexpr int SMEM_BYTES = NS * STAGE_BYTES + NB * BITS_BYTES + HS * 4 + 512;
 
 // block-scaled instruction descriptor, kind::mxf4: A = B = E2M1 (1 at bits 7 and 10), both K-major,
 // N >> 3 at bit 17, scale format UE8M0 (bit 23), M >> 4 at bit 24 (M = 256 over the pair), K = 64
@@ -186,39 +193,39 @@ __device__ __forceinline__ void tmem_st16_const(uint32_t taddr, uint32_t val)
         : "memory");
     asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
 }
-__device__ __forceinline__ void tmem_ld16(uint32_t taddr, uint32_t (&v)[16])
+// 32 lanes x 32 columns -> 32 registers per thread; the caller issues tcgen05.wait::ld
+__device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t *v)
 {
     asm volatile(
-        "tcgen05.ld.sync.aligned.32x32b.x16.b32 "
-        "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15}, [%16];\n"
+        "tcgen05.ld.sync.aligned.32x32b.x32.b32 "
+        "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, "
+        "%16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31}, [%32];\n"
         : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]),
-          "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15])
+          "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15]),
+          "=r"(v[16]), "=r"(v[17]), "=r"(v[18]), "=r"(v[19]), "=r"(v[20]), "=r"(v[21]), "=r"(v[22]), "=r"(v[23]),
+          "=r"(v[24]), "=r"(v[25]), "=r"(v[26]), "=r"(v[27]), "=r"(v[28]), "=r"(v[29]), "=r"(v[30]), "=r"(v[31])
         : "r"(taddr)
         : "memory");
-    asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
 }
-__device__ __forceinline__ void tmem_st32(uint32_t taddr, const uint32_t (&v)[32])
+// 32 lanes x 16 columns <- 16 registers per thread; the caller issues tcgen05.wait::st
+__device__ __forceinline__ void tmem_st16(uint32_t taddr, const uint32_t (&v)[16])
 {
     asm volatile(
-        "tcgen05.st.sync.aligned.32x32b.x32.b32 [%0], "
-        "{%1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, %16, "
-        "%17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31, %32};\n" ::"r"(taddr),
+        "tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], "
+        "{%1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, %16};\n" ::"r"(taddr),
         "r"(v[0]), "r"(v[1]), "r"(v[2]), "r"(v[3]), "r"(v[4]), "r"(v[5]), "r"(v[6]), "r"(v[7]), "r"(v[8]), "r"(v[9]),
-        "r"(v[10]), "r"(v[11]), "r"(v[12]), "r"(v[13]), "r"(v[14]), "r"(v[15]), "r"(v[16]), "r"(v[17]), "r"(v[18]),
-        "r"(v[19]), "r"(v[20]), "r"(v[21]), "r"(v[22]), "r"(v[23]), "r"(v[24]), "r"(v[25]), "r"(v[26]), "r"(v[27]),
-        "r"(v[28]), "r"(v[29]), "r"(v[30]), "r"(v[31])
+        "r"(v[10]), "r"(v[11]), "r"(v[12]), "r"(v[13]), "r"(v[14]), "r"(v[15])
         : "memory");
-    asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
 }
 
-// E2M1 nibbles of nibble position Q of a 32-bit slice (values 0.5, 1, 2, 0.5 where the bit is set)
+// E2M1 nibbles of nibble position Q = 0, 1, 2 of a 32-bit slice (values 0.5, 1, 2 where the bit is set)
 template <int Q>
 __device__ __forceinline__ uint32_t nib(uint32_t x)
 {
+    if (CS_PAIR_DIAG & 8) return x;
     if (Q == 0) return x & 0x11111111u;
     if (Q == 1) return x & 0x22222222u;
-    if (Q == 2) return x & 0x44444444u;
-    return (x >> 3) & 0x11111111u;
+    return x & 0x44444444u;
 }
 // UE8M0 block scale that turns the products of nibble position q into exactly 1: 2^1, 2^0, 2^-1, 2^1
 __device__ __forceinline__ uint32_t sf_col(int q) { return SF_COL + (q == 1 ? 16u : q == 2 ? 32u : 0u); }
@@ -258,7 +265,7 @@ __global__ void k_pair_tile_order(int nT, uint32_t *__restrict__ tab)
 
 struct Tile {
     int I, J;      // 256-row blocks of i and of j
-    int64_t b;     // causet
+    int b;         // causet
     bool skip;     // no row of the tile inside [row_begin, row_end)
 };
 
@@ -272,9 +279,8 @@ k_interval_pair(const __grid_constant__ CUtensorMap mapU, const __grid_constant_
     extern __shared__ __align__(1024) unsigned char smem[];
     unsigned char *s_stage = smem;
     unsigned char *s_bits = smem + NS * STAGE_BYTES;
-    uint32_t *s_epi = reinterpret_cast<uint32_t *>(smem + NS * STAGE_BYTES + NB * BITS_BYTES);
-    uint32_t *s_hist = reinterpret_cast<uint32_t *>(smem + NS * STAGE_BYTES + NB * BITS_BYTES + EPI_BYTES);
-    uint64_t *s_full = reinterpret_cast<uint64_t *>(smem + NS * STAGE_BYTES + NB * BITS_BYTES + EPI_BYTES + HS * 4);
+    uint32_t *s_hist = reinterpret_cast<uint32_t *>(smem + NS * STAGE_BYTES + NB * BITS_BYTES);
+    uint64_t *s_full = reinterpret_cast<uint64_t *>(smem + NS * STAGE_BYTES + NB * BITS_BYTES + HS * 4);
     uint64_t *s_empty = s_full + NS;      // [NS] stage free again (multicast commit from CTA 0)
     uint64_t *s_tfull = s_empty + NS;     // [1] accumulator complete (multicast commit)
     uint64_t *s_tempty = s_tfull + 1;     // [1] accumulator drained (used in CTA 0 only)
@@ -285,19 +291,22 @@ k_interval_pair(const __grid_constant__ CUtensorMap mapU, const __grid_constant_
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const uint32_t rank = cluster_ctarank();
     const int nT = (int)((N + TILE - 1) / TILE);
-    const int64_t tiles_per = (int64_t)nT * (nT + 1) / 2;
-    const int64_t total_tiles = tiles_per * B;
-    const int64_t t0 = cluster_id_x(), tstep = num_clusters_x();
+    // 32-bit schedule state (the launcher rejects more than 2^31 tiles): the expander and issuer
+    // warps run on 64 and 40 registers
+    const uint32_t tiles_per = (uint32_t)nT * (uint32_t)(nT + 1) / 2;
+    const uint32_t total_tiles = tiles_per * (uint32_t)B;
+    const uint32_t t0 = cluster_id_x(), tstep = num_clusters_x();
+    const int ib0 = (int)(row_begin / TILE), ib1 = (int)((row_end + TILE - 1) / TILE);   // I blocks inside the row range
     const int hs = (int)((kmax + 1 < HS) ? (kmax + 1) : HS);
     const int64_t hist_len = kmax + 1;
 
-    auto get_tile = [&](int64_t t) {
+    auto get_tile = [&](uint32_t t) {
         Tile tc;
-        tc.b = t / tiles_per;
-        const uint32_t e = __ldg(tile_tab + (t - tc.b * tiles_per));
+        tc.b = (int)(t / tiles_per);
+        const uint32_t e = __ldg(tile_tab + (t - (uint32_t)tc.b * tiles_per));
         tc.I = (int)(e >> 16);
         tc.J = (int)(e & 0xFFFFu);
-        tc.skip = (int64_t)tc.I * TILE >= row_end || (int64_t)(tc.I + 1) * TILE <= row_begin;
+        tc.skip = tc.I < ib0 || tc.I >= ib1;
         return tc;
     };
 
@@ -336,77 +345,112 @@ k_interval_pair(const __grid_constant__ CUtensorMap mapU, const __grid_constant_
     tc_fence_after();
 
     // every role of both CTAs walks the same static schedule: tile t = cluster id, + number of clusters, ...
-    if (warp >= EXP_WARP0) {
+    // 640 threads x 96 registers at launch = the CTA's pool (setmaxnreg.inc only draws on what the CTA's
+    // own warps released): 256 x 152 (epilogue) + 256 x 64 (expanders) + 128 x 40 = 61440.  Each
+    // setmaxnreg sits inside its role's branch: ptxas budgets a region by the setmaxnreg that dominates it.
+    if (warp >= EXPA_WARP0 && warp < MMA_WARP) {
+        asm volatile("setmaxnreg.dec.sync.aligned.u32 64;");
         // ===================================== expanders =====================================
-        // warps 0-3 own this CTA's 128 A rows (row = TMEM lane: warp w may only touch lanes 32 (w % 4) ..),
-        // warps 4-7 its 128 B rows
-        const int ew = warp - EXP_WARP0;
-        const bool isA = ew < 4;
-        const int r = isA ? ((warp & 3) * 32 + lane) : ((ew - 4) * 32 + lane);
-        uint32_t it = 0;   // global stage counter (operand ring position)
-        uint32_t grp = 0;  // global group counter (bit-buffer ring position)
+        // warpgroup 2 owns this CTA's 128 A rows (row = TMEM lane: warp w may only touch lanes
+        // 32 (w % 4) ..), warpgroup 3 its 128 B rows.  One thread per row.
+        const bool isA = warp < EXPB_WARP0;
+        const int r = (warp & 3) * 32 + lane;
         // TMA 64B swizzle: 16-byte chunk c of row e sits at chunk c ^ ((e >> 1) & 3)
         const unsigned char *my_bits = s_bits + (isA ? 0 : TM * BROW) + r * BROW;
         const int swz = (r >> 1) & 3;
-        for (int64_t t = t0; t < total_tiles; t += tstep) {
+        const int off0 = (0 ^ swz) << 4, off1 = (1 ^ swz) << 4, off2 = (2 ^ swz) << 4, off3 = (3 ^ swz) << 4;
+        // bit 3 of every nibble: rotate left by one, then mask; the rotation is an IMAD.WIDE by a 2
+        // the compiler cannot see (FMA pipe) so that the ALU pipe only runs the 32 masks per stage
+        const uint32_t two = 2u | (uint32_t)((uint64_t)N >> 40);
+        auto nib3 = [&](uint32_t x) {
+#if CS_PAIR_ROT_IMAD
+            const uint64_t p = (uint64_t)x * two;
+            return ((uint32_t)p | (uint32_t)(p >> 32)) & 0x11111111u;
+#else
+            (void)two;
+            return (x >> 3) & 0x11111111u;
+#endif
+        };
+        uint32_t s = 0, ph = 0;    // operand ring position and phase
+        uint32_t b = 0, bph = 0;   // bit-buffer ring position and phase
+        const uint32_t a_taddr = tmem_base + ((uint32_t)((warp & 3) * 32) << 16) + A_COL;
+        unsigned char *b_dst = s_stage + r * 16;
+
+        auto stage_A = [&](const uint4 &c0, const uint4 &c1) {
+            const uint32_t xs[8] = {c0.x, c0.y, c0.z, c0.w, c1.x, c1.y, c1.z, c1.w};
+            // TMEM column 8 q + j of stage s = nibble position q of slice j; two 16-column stores
+            uint32_t lo[16], hi[16];
+#pragma unroll
+            for (int j = 0; j < 8; j++) {
+                lo[j] = nib<0>(xs[j]);
+                lo[8 + j] = nib<1>(xs[j]);
+            }
+            mbar_wait(&s_empty[s], ph ^ 1);
+            tc_fence_after();
+            if (!(CS_PAIR_DIAG & 2)) tmem_st16(a_taddr + s * 32, lo);
+#pragma unroll
+            for (int j = 0; j < 8; j++) {
+                hi[j] = nib<2>(xs[j]);
+                hi[8 + j] = (CS_PAIR_DIAG & 8) ? xs[j] : nib3(xs[j]);
+            }
+            if (!(CS_PAIR_DIAG & 2)) tmem_st16(a_taddr + s * 32 + 16, hi);
+            asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
+            tc_fence_before();
+            __syncwarp();
+            if (lane == 0) mbar_arrive_cluster(&s_full[s], 0);    // one arrival per warp, in CTA 0
+            if (++s == NS) { s = 0; ph ^= 1; }
+        };
+        auto stage_B = [&](const uint4 &c0, const uint4 &c1) {
+            const uint32_t xs[8] = {c0.x, c0.y, c0.z, c0.w, c1.x, c1.y, c1.z, c1.w};
+            uint4 w[8];       // 16-byte chunk 2 q + h of this row = nibble position q of slices 4 h .. 4 h + 3
+#pragma unroll
+            for (int h = 0; h < 2; h++) {
+                w[0 + h] = make_uint4(nib<0>(xs[4 * h]), nib<0>(xs[4 * h + 1]), nib<0>(xs[4 * h + 2]), nib<0>(xs[4 * h + 3]));
+                w[2 + h] = make_uint4(nib<1>(xs[4 * h]), nib<1>(xs[4 * h + 1]), nib<1>(xs[4 * h + 2]), nib<1>(xs[4 * h + 3]));
+                w[4 + h] = make_uint4(nib<2>(xs[4 * h]), nib<2>(xs[4 * h + 1]), nib<2>(xs[4 * h + 2]), nib<2>(xs[4 * h + 3]));
+                if (CS_PAIR_DIAG & 8) w[6 + h] = make_uint4(xs[4 * h], xs[4 * h + 1], xs[4 * h + 2], xs[4 * h + 3]);
+                else w[6 + h] = make_uint4(nib3(xs[4 * h]), nib3(xs[4 * h + 1]), nib3(xs[4 * h + 2]), nib3(xs[4 * h + 3]));
+            }
+            mbar_wait(&s_empty[s], ph ^ 1);
+            unsigned char *dst = b_dst + s * STAGE_BYTES;
+#pragma unroll
+            for (int q = 0; q < 8; q++)
+                if (!(CS_PAIR_DIAG & 1)) *reinterpret_cast<uint4 *>(dst + q * TNH * 16) = w[q];
+            if (!(CS_PAIR_DIAG & 16)) fence_proxy_async();   // generic-proxy stores -> visible to the tensor cores
+            __syncwarp();
+            if (lane == 0) mbar_arrive_cluster(&s_full[s], 0);
+            if (++s == NS) { s = 0; ph ^= 1; }
+        };
+
+        for (uint32_t t = t0; t < total_tiles; t += tstep) {
             const Tile tc = get_tile(t);
             if (tc.skip) continue;
             const int nstages = tc.J - tc.I + 1;
-            const int ngroups = (nstages + GK - 1) / GK;
-            for (int g = 0; g < ngroups; g++, grp++) {
-                const int b = grp % NB;
-                mbar_wait(&s_bfull[b], (grp / NB) & 1);
-                const int kcount = (nstages - g * GK < GK) ? (nstages - g * GK) : GK;
-                for (int c = 0; c < kcount; c++, it++) {
-                    const uint4 cur0 = *reinterpret_cast<const uint4 *>(my_bits + b * BITS_BYTES + (((2 * c) ^ swz) << 4));
-                    const uint4 cur1 = *reinterpret_cast<const uint4 *>(my_bits + b * BITS_BYTES + (((2 * c + 1) ^ swz) << 4));
-                    const int s = it % NS;
-                    const uint32_t xs[8] = {cur0.x, cur0.y, cur0.z, cur0.w, cur1.x, cur1.y, cur1.z, cur1.w};
-                    if (isA) {
-                        // TMEM column 8 q + j of stage s = nibble position q of slice j
-                        uint32_t w[32];
-#pragma unroll
-                        for (int j = 0; j < 8; j++) {
-                            w[j] = nib<0>(xs[j]);
-                            w[8 + j] = nib<1>(xs[j]);
-                            w[16 + j] = nib<2>(xs[j]);
-                            w[24 + j] = nib<3>(xs[j]);
-                        }
-                        mbar_wait(&s_empty[s], ((it / NS) & 1) ^ 1);
-                        tc_fence_after();
-                        tmem_st32(tmem_base + ((uint32_t)((warp & 3) * 32) << 16) + A_COL + s * 32, w);
-                        tc_fence_before();
-                    } else {
-                        // 16-byte chunk 2 q + h of this row = nibble position q of slices 4 h .. 4 h + 3
-                        uint4 w[8];
-#pragma unroll
-                        for (int h = 0; h < 2; h++) {
-                            w[0 + h] = make_uint4(nib<0>(xs[4 * h]), nib<0>(xs[4 * h + 1]), nib<0>(xs[4 * h + 2]), nib<0>(xs[4 * h + 3]));
-                            w[2 + h] = make_uint4(nib<1>(xs[4 * h]), nib<1>(xs[4 * h + 1]), nib<1>(xs[4 * h + 2]), nib<1>(xs[4 * h + 3]));
-                            w[4 + h] = make_uint4(nib<2>(xs[4 * h]), nib<2>(xs[4 * h + 1]), nib<2>(xs[4 * h + 2]), nib<2>(xs[4 * h + 3]));
-                            w[6 + h] = make_uint4(nib<3>(xs[4 * h]), nib<3>(xs[4 * h + 1]), nib<3>(xs[4 * h + 2]), nib<3>(xs[4 * h + 3]));
-                        }
-                        mbar_wait(&s_empty[s], ((it / NS) & 1) ^ 1);
-                        unsigned char *dst = s_stage + s * STAGE_BYTES + r * 16;
-#pragma unroll
-                        for (int q = 0; q < 8; q++) *reinterpret_cast<uint4 *>(dst + q * TNH * 16) = w[q];
-                        fence_proxy_async();          // generic-proxy stores -> visible to the tensor cores
-                    }
-                    __syncwarp();
-                    if (lane == 0) {
-                        mbar_arrive_cluster(&s_full[s], 0);               // one arrival per warp, in CTA 0
-                        // last stage of the buffer has been loaded AND consumed by every lane (the
-                        // stores above depend on it): hand the bit buffer back to the loader
-                        if (c == kcount - 1) mbar_arrive(&s_bempty[b]);
-                    }
+            for (int k = 0; k < nstages; k += GK) {
+                mbar_wait(&s_bfull[b], bph);
+                const unsigned char *src = my_bits + b * BITS_BYTES;
+                const bool second = k + 1 < nstages;
+                if (isA) {
+                    stage_A(*reinterpret_cast<const uint4 *>(src + off0), *reinterpret_cast<const uint4 *>(src + off1));
+                    if (second) stage_A(*reinterpret_cast<const uint4 *>(src + off2), *reinterpret_cast<const uint4 *>(src + off3));
+                } else {
+                    stage_B(*reinterpret_cast<const uint4 *>(src + off0), *reinterpret_cast<const uint4 *>(src + off1));
+                    if (second) stage_B(*reinterpret_cast<const uint4 *>(src + off2), *reinterpret_cast<const uint4 *>(src + off3));
                 }
+                // the buffer has been loaded AND consumed by every lane (the stores above depend on
+                // it): hand it back to the loader
+                __syncwarp();
+                if (lane == 0) mbar_arrive(&s_bempty[b]);
+                if (++b == NB) { b = 0; bph ^= 1; }
             }
         }
-    } else if (warp == LOAD_WARP) {
-        // ===================================== TMA loader ====================================
-        if (lane == 0) {
+    } else if (warp >= MMA_WARP) {
+        asm volatile("setmaxnreg.dec.sync.aligned.u32 40;");
+        if (warp == LOAD_WARP && lane == 0) {
+            // ===================================== TMA loader ====================================
+            {
             uint32_t grp = 0;
-            for (int64_t t = t0; t < total_tiles; t += tstep) {
+            for (uint32_t t = t0; t < total_tiles; t += tstep) {
                 const Tile tc = get_tile(t);
                 if (tc.skip) continue;
                 const int nstages = tc.J - tc.I + 1;
@@ -417,16 +461,16 @@ k_interval_pair(const __grid_constant__ CUtensorMap mapU, const __grid_constant_
                     mbar_arrive_expect_tx(&s_bfull[b], (uint32_t)BITS_BYTES);   // out-of-bounds is zero-filled
                     unsigned char *dst = s_bits + b * BITS_BYTES;
                     const int c0 = (tc.I * (KSTEP / 8)) + g * BROW;             // byte column of the first k
-                    tma_load_3d(dst, &mapU, c0, tc.I * TILE + (int)rank * TM, (int)tc.b, &s_bfull[b]);
-                    tma_load_3d(dst + TM * BROW, &mapL, c0, tc.J * TILE + (int)rank * TNH, (int)tc.b, &s_bfull[b]);
+                    tma_load_3d(dst, &mapU, c0, tc.I * TILE + (int)rank * TM, tc.b, &s_bfull[b]);
+                    tma_load_3d(dst + TM * BROW, &mapL, c0, tc.J * TILE + (int)rank * TNH, tc.b, &s_bfull[b]);
                 }
             }
         }
-    } else if (warp == MMA_WARP) {
-        // ===================================== MMA issuer (CTA 0 only) =======================
-        if (rank == 0 && lane == 0) {
+        } else if (warp == MMA_WARP && rank == 0 && lane == 0) {
+            // ===================================== MMA issuer (CTA 0 only) =======================
+            {
             uint32_t it = 0, tile_seq = 0;
-            for (int64_t t = t0; t < total_tiles; t += tstep) {
+            for (uint32_t t = t0; t < total_tiles; t += tstep) {
                 const Tile tc = get_tile(t);
                 if (tc.skip) continue;
                 const int nstages = tc.J - tc.I + 1;
@@ -448,16 +492,21 @@ k_interval_pair(const __grid_constant__ CUtensorMap mapU, const __grid_constant_
                 mma_commit_pair(s_tfull);                                 // accumulator complete, both CTAs
                 tile_seq++;
             }
+            }
         }
     } else {
         // ===================================== epilogue ======================================
-        // this CTA's accumulator: rows I*256 + rank*128 + TMEM lane, columns J*256 ..
+        // This CTA's accumulator: rows I*256 + rank*128 + TMEM lane, columns J*256 ...  A warp drains its
+        // 32 lanes x 128 columns into registers, hands the accumulator back to the MMA issuer at
+        // once, and only then tallies the related pairs -- while the next tile's MMAs run.
+        asm volatile("setmaxnreg.inc.sync.aligned.u32 152;");
         uint32_t tile_seq = 0;
         unsigned long long my_nrel = 0;
         const uint32_t kmax32 = (uint32_t)kmax;
-        int64_t cur_batch = -1;
+        int cur_batch = -1;
         const int quarter = warp & 3, colhalf = warp >> 2;   // TMEM lane quarter; which 128 columns
-        for (int64_t t = t0; t < total_tiles; t += tstep) {
+        const uint32_t taddr = tmem_base + ((uint32_t)(quarter * 32) << 16) + colhalf * 128;
+        for (uint32_t t = t0; t < total_tiles; t += tstep) {
             const Tile tc = get_tile(t);
             if (tc.skip) continue;
             if (tc.b != cur_batch) {   // per-causet histograms: flush before switching
@@ -465,7 +514,7 @@ k_interval_pair(const __grid_constant__ CUtensorMap mapU, const __grid_constant_
                     asm volatile("bar.sync 1, 256;");
                     for (int b = tid; b < hs; b += EPI_WARPS * 32) {
                         uint32_t v = s_hist[b];
-                        if (v) { atomicAdd(&hist[cur_batch * hist_len + b], (unsigned long long)v); s_hist[b] = 0; }
+                        if (v) { atomicAdd(&hist[(int64_t)cur_batch * hist_len + b], (unsigned long long)v); s_hist[b] = 0; }
                     }
                     asm volatile("bar.sync 1, 256;");
                 }
@@ -475,59 +524,46 @@ k_interval_pair(const __grid_constant__ CUtensorMap mapU, const __grid_constant_
             const bool row_ok = i < N && i >= row_begin && i < row_end;
             uint64_t rel[2] = {0, 0};                            // relation bits of this warp's 128 columns
             if (row_ok) {
-                const uint64_t *urow = bits + tc.b * N * stride + i * stride;
+                const uint64_t *urow = bits + ((int64_t)tc.b * N + i) * stride;
 #pragma unroll
                 for (int w = 0; w < 2; w++) {
                     const int64_t wi = (int64_t)tc.J * 4 + colhalf * 2 + w;
                     if (wi < stride) rel[w] = __ldg(urow + wi);
                 }
             }
-            unsigned long long *ghist = hist + cur_batch * hist_len;
+            unsigned long long *ghist = hist + (int64_t)cur_batch * hist_len;
+            uint32_t v[128];
             mbar_wait(s_tfull, tile_seq & 1);
             tc_fence_after();
-            const uint32_t taddr = tmem_base + ((uint32_t)(quarter * 32) << 16) + colhalf * 128;
-            uint32_t *my = s_epi + tid * EPITCH;
-            auto tally = [&](uint32_t word) {
-                const uint32_t cnt = (uint32_t)__uint_as_float(word);   // products are 0 or 1: exact in fp32
-                if (cnt < (uint32_t)hs) atomicAdd(&s_hist[cnt], 1u);
-                else if (cnt <= kmax32) atomicAdd(&ghist[cnt], 1ULL);
-            };
 #pragma unroll
-            for (int c16 = 0; c16 < 8; c16++) {
-                const uint32_t rel16 = (uint32_t)(rel[c16 >> 2] >> (16 * (c16 & 3))) & 0xFFFFu;
-                if (!__any_sync(0xffffffffu, rel16 != 0)) continue;
-                uint32_t v[16];
-                tmem_ld16(taddr + c16 * 16, v);
-                if (rel16 == 0) continue;
-                my_nrel += __popc(rel16);
-                // stage the 16 counts in this thread's private shared-memory row, then visit only the
-                // columns whose relation bit is set, two per iteration
-#pragma unroll
-                for (int c4 = 0; c4 < 4; c4++)
-                    *reinterpret_cast<uint4 *>(my + 4 * c4) = make_uint4(v[4 * c4], v[4 * c4 + 1], v[4 * c4 + 2], v[4 * c4 + 3]);
-                uint32_t m = rel16;
-                while (m) {
-                    const int c0 = __ffs(m) - 1;
-                    m &= m - 1;
-                    const bool two = m != 0;
-                    const int c1 = two ? __ffs(m) - 1 : c0;
-                    m &= m - 1;
-                    const uint32_t w0 = my[c0], w1 = my[c1];
-                    tally(w0);
-                    if (two) tally(w1);
-                }
-            }
+            for (int c = 0; c < 4; c++) tmem_ld32(taddr + c * 32, &v[c * 32]);
+            asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
             tc_fence_before();
             __syncwarp();
             if (lane == 0) mbar_arrive_cluster(s_tempty, 0);   // one arrival per warp, in CTA 0
             tile_seq++;
+            if (CS_PAIR_DIAG & 4) continue;
+            my_nrel += __popcll(rel[0]) + __popcll(rel[1]);
+#pragma unroll
+            for (int c16 = 0; c16 < 8; c16++) {
+                const uint32_t rel16 = (uint32_t)(rel[c16 >> 2] >> (16 * (c16 & 3))) & 0xFFFFu;
+                if (!__any_sync(0xffffffffu, rel16 != 0)) continue;
+#pragma unroll
+                for (int c = 0; c < 16; c++) {
+                    if (rel16 & (1u << c)) {
+                        const uint32_t cnt = (uint32_t)__uint_as_float(v[c16 * 16 + c]);   // 0/1 products: exact in fp32
+                        if (cnt < (uint32_t)hs) atomicAdd(&s_hist[cnt], 1u);
+                        else if (cnt <= kmax32) atomicAdd(&ghist[cnt], 1ULL);
+                    }
+                }
+            }
         }
         // final flush by the epilogue warps
         asm volatile("bar.sync 1, 256;");
         if (cur_batch >= 0) {
             for (int b = tid; b < hs; b += EPI_WARPS * 32) {
                 uint32_t v = s_hist[b];
-                if (v) atomicAdd(&hist[cur_batch * hist_len + b], (unsigned long long)v);
+                if (v) atomicAdd(&hist[(int64_t)cur_batch * hist_len + b], (unsigned long long)v);
             }
         }
         if (nrel && B == 1) {
@@ -599,6 +635,10 @@ int launch_interval_pair(const uint64_t *bits, const uint64_t *bitsT, int64_t B,
                          void *scratch, size_t scratch_bytes, cudaStream_t st)
 {
     if (N > ((int64_t)1 << 24)) return CS_ERR_ARG;   // counts must stay exact in fp32; tile ids are 16 bits
+    {
+        const int64_t nT64 = (N + TILE - 1) / TILE;
+        if (B > 0 && nT64 * (nT64 + 1) / 2 > (((int64_t)1 << 31) - 1) / B) return CS_ERR_ARG;   // 32-bit tile schedule
+    }
     if (!scratch || scratch_bytes < interval_pair_scratch_bytes(N)) return CS_ERR_WORKSPACE;
     static bool attr_set = false;
     if (!attr_set) {
