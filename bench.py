@@ -40,9 +40,11 @@ UNIT = "word-ops/s"
 POPC_PER_CLK_SM = 16.0
 # dram__bytes_read.sum + dram__bytes_write.sum of one launch of the a2 kernel at config 3, from the
 # `ncu --set full` captures summarised under profiles/ (bytes per launch; None = not captured)
-NCU_TRAFFIC = {1: 78.28e9, 2: 51.14e9, 3: 38.12e9, 4: None}
+NCU_TRAFFIC = {1: 78.28e9, 2: 51.14e9, 3: 38.12e9, 4: 10.30e9}
 # tensor peaks = measured bf16 dense peak x the guide's nominal ratio (bf16 2.25, int8/fp8 4.5, fp4 9 PFLOP/s)
 TENSOR_OVER_BF16 = {2: 2.0, 3: 4.0, 4: 4.0}
+# dense issue rate of one SM's tensor pipe in op/clk (2 per multiply-add): kind::i8 16384, kind::mxf4 32768
+TENSOR_OPS_PER_CLK_SM = {2: 16384.0, 3: 32768.0, 4: 32768.0}
 ROUTE_NAME = {1: "popc", 2: "tensor_int8", 3: "tensor_fp4", 4: "tensor_fp4_pair"}
 ROUTE_DTYPE = {1: "u64", 2: "int8", 3: "fp4_e2m1", 4: "fp4_e2m1"}
 ROUTE_KERNEL = {1: "k_interval_popc", 2: "k_interval_tensor", 3: "k_interval_fp4", 4: "k_interval_pair"}
@@ -288,21 +290,27 @@ def main():
     # ---- roofline of the dominant kernel (a2) -----------------------------------------------
     hist_s = statistics.mean(hist_ms) / 1e3
     sm_mhz = clocks.get("sm_mhz") or peaks.get("sm_max_mhz", 1965.0)
+    traffic = NCU_TRAFFIC.get(route) if (args.config == 3 and N == cfg.N) else None   # captured at config 3 only
     if route in TENSOR_OVER_BF16:
         ops = tensor_ops_algorithmic(N)
         burst = hist_s < 1.0
         ratio = TENSOR_OVER_BF16[route]
         peak = ratio * (peaks["bf16_tflops"] if burst else peaks.get("bf16_tflops_sustained", peaks["bf16_tflops"]))
         roofline = {"bound": "tensor", "achieved": ops / hist_s / 1e12, "peak": peak, "unit": "TFLOP/s",
-                    "frac": ops / hist_s / 1e12 / peak, "traffic": NCU_TRAFFIC.get(route),
+                    "frac": ops / hist_s / 1e12 / peak, "traffic": traffic,
                     "kernel": ROUTE_KERNEL[route], "peak_source": "%s bf16 %s x %.0f (%s:bf16 nominal ratio)" %
                     (peaks["_source"], "burst" if burst else "sustained", ratio, ROUTE_DTYPE[route]),
                     "algorithmic_ops": ops}
+        # the pipe's own issue rate, for reading frac > 1: the library bf16 GEMM behind `peak` runs power-capped
+        # (MEASURED_PEAKS clocks_under_load), this kernel at full clock.  DESIGN.md section 5.
+        pipe = 148 * TENSOR_OPS_PER_CLK_SM[route] * peaks.get("sm_max_mhz", 1965.0) * 1e6 / 1e12
+        roofline["pipe_peak"] = pipe
+        roofline["frac_of_pipe"] = ops / hist_s / 1e12 / pipe
     else:
         peak = 148 * POPC_PER_CLK_SM / 2.0 * peaks.get("sm_max_mhz", 1965.0) * 1e6 / 1e12   # T word-ops/s
         executed = dense_triangular_word_ops(N)
         roofline = {"bound": "alu", "achieved": W_alg / hist_s / 1e12, "peak": peak, "unit": "Tword-op/s",
-                    "frac": W_alg / hist_s / 1e12 / peak, "traffic": NCU_TRAFFIC.get(route), "kernel": "k_interval_popc",
+                    "frac": W_alg / hist_s / 1e12 / peak, "traffic": traffic, "kernel": "k_interval_popc",
                     "peak_source": "derived: 148 SM x 16 POPC.32/clk/SM / 2 per 64-bit word x sm_max_mhz (DESIGN.md)",
                     "executed_word_ops": executed, "executed_frac": executed / hist_s / 1e12 / peak}
     build_s = statistics.mean(build_ms) / 1e3

@@ -120,6 +120,13 @@ int cs_interval_hist_ex(const uint64_t *bits, const uint64_t *bitsT, int64_t N, 
                         int64_t row_begin, int64_t row_end, int route,
                         int64_t *hist, int64_t *n_relations,
                         void *workspace, size_t workspace_bytes, void *stream);
+/* a2 over B causets in one launch (the Monte-Carlo ensemble): bits/bitsT are
+ * [B][N][stride] as written by cs_causal_matrix_batched (bitsT required), hist is int64[B][kmax+1]
+ * (kmax clamped as above), overwritten.  Workspace: cs_interval_hist_batched_workspace() bytes.
+ * Errors: CS_ERR_ARG, CS_ERR_WORKSPACE, CS_ERR_CUDA. */
+size_t cs_interval_hist_batched_workspace(int64_t B, int64_t N, int route);
+int cs_interval_hist_batched(const uint64_t *bits, const uint64_t *bitsT, int64_t B, int64_t N, int64_t kmax,
+                             int route, int64_t *hist, void *workspace, size_t workspace_bytes, void *stream);
 /* Route CS_ROUTE_AUTO resolves to for this N (one of the concrete routes). */
 int cs_default_route(int64_t N);
 

@@ -47,6 +47,8 @@ _SIGNATURES = {
     "cs_interval_hist_workspace": (_sz, [_i64, _i64, _int, _int]),
     "cs_interval_hist": (_int, [_p, _p, _i64, _i64, _p, _p, _p, _sz, _p]),
     "cs_interval_hist_ex": (_int, [_p, _p, _i64, _i64, _i64, _i64, _int, _p, _p, _p, _sz, _p]),
+    "cs_interval_hist_batched_workspace": (_sz, [_i64, _i64, _int]),
+    "cs_interval_hist_batched": (_int, [_p, _p, _i64, _i64, _i64, _int, _p, _p, _sz, _p]),
     "cs_default_route": (_int, [_i64]),
     "cs_bd_action": (_int, [_p, _i64, _i64, _int, _p, _p, _p]),
     "cs_bd_action_batched_workspace": (_sz, [_i64, _i64]),
@@ -182,6 +184,21 @@ def interval_hist(bits: torch.Tensor, bitsT, N: int, kmax: int = -1, route: int 
                                       _dptr(hist), _dptr(nrel), _dptr(ws), ws.numel(), _stream()),
            "cs_interval_hist_ex")
     return (hist, nrel) if return_relations else hist
+
+
+def interval_hist_batched(bits: torch.Tensor, bitsT: torch.Tensor, N: int, kmax: int = -1,
+                          route: int = ROUTE_AUTO, workspace: torch.Tensor | None = None) -> torch.Tensor:
+    """bits, bitsT [B][N][stride] -> hist int64[B][kmax+1] (CUDA), one launch for all causets."""
+    _need_cuda(bits, torch.int64, "bits")
+    _need_cuda(bitsT, torch.int64, "bitsT")
+    B = bits.shape[0]
+    k = clamp_kmax(N, kmax)
+    hist = torch.empty((B, k + 1), dtype=torch.int64, device=bits.device)
+    need = int(load().cs_interval_hist_batched_workspace(B, N, route))
+    ws = workspace if workspace is not None else _workspace(need, bits.device)
+    _check(load().cs_interval_hist_batched(_dptr(bits), _dptr(bitsT), B, N, kmax, route, _dptr(hist),
+                                           _dptr(ws), ws.numel(), _stream()), "cs_interval_hist_batched")
+    return hist
 
 
 def bd_action(hist: torch.Tensor, N: int, dim: int, return_bracket: bool = False):
