@@ -62,6 +62,47 @@ struct Pred<CS_GEOM_DS2_SLAB, 2> {
     }
 };
 
+// ---- exact single-precision prefilter (flat cone) ----------------------------------------------
+// With h = (t^2 - |x|^2) / 2 the sign of the interval is the sign of
+//     T = ((t_j - t_i)^2 - |x_j - x_i|^2) / 2 = h_i + h_j - t_i t_j + x_i . x_j ,
+// four FFMA and one FADD per pair in fp32 instead of twelve fp64-pipe instructions.  The fp32 value a
+// differs from T by at most 34 u C^2 (u = 2^-24, C = largest |coordinate| of the tile: 8 input
+// roundings <= 8.04 u C^2, two roundings of h <= 3 u C^2, five result roundings of partial sums
+// bounded by 2.5, 3.5, 4.5, 5.5 and 7 C^2), so with m = 64 u C^2
+//     a >  m  =>  T >  30 u C^2  : related     (the fp64 expression errs by < 2^-46 C^2, and dt >= 0
+//     a < -m  =>  T < -30 u C^2  : unrelated    holds for the whole tile, checked below)
+// and anything else -- including NaN -- is re-evaluated with the fp64 expression of the header for
+// the whole 32 x 32 block.  The output is therefore bit-identical to the plain fp64 evaluation.
+// The tile takes this path only if it is off the diagonal, max t_i <= min t_j (so the header's
+// dt >= 0 holds for every pair; always the case for time-sorted input) and 2^-40 <= C <= 2^40 (no
+// overflow or underflow in the fp32 products).
+template <int GEOM, int DIM>
+struct FastCone { static constexpr bool ok = false; };
+template <int DIM>
+struct FastCone<CS_GEOM_MINK_CONE, DIM> { static constexpr bool ok = true; };
+
+__device__ __forceinline__ double warp_max(double v)
+{
+#pragma unroll
+    for (int s = 16; s >= 1; s >>= 1) v = fmax(v, __shfl_xor_sync(0xffffffffu, v, s));
+    return v;
+}
+
+// 32 x 32 bit block held one word per lane (lane = column, bit = row) -> one word per lane
+// (lane = row, bit = column): the 5-step butterfly
+__device__ __forceinline__ uint32_t transpose32(uint32_t x, int lane)
+{
+    const uint32_t mlo[5] = {0x0000FFFFu, 0x00FF00FFu, 0x0F0F0F0Fu, 0x33333333u, 0x55555555u};
+#pragma unroll
+    for (int t = 0; t < 5; t++) {
+        const int s = 16 >> t;
+        const uint32_t o = __shfl_xor_sync(0xffffffffu, x, s);
+        if (lane & s) x = (x & ~mlo[t]) | ((o >> s) & mlo[t]);
+        else          x = (x & mlo[t]) | ((o << s) & ~mlo[t]);
+    }
+    return x;
+}
+
 template <int GEOM, int DIM>
 __global__ void __launch_bounds__(BUILD_THREADS)
 k_causal_matrix(const double *__restrict__ coords, int64_t N, int64_t stride,
@@ -74,17 +115,26 @@ k_causal_matrix(const double *__restrict__ coords, int64_t N, int64_t stride,
     bits += b * N * stride;
     if (bitsT) bitsT += b * N * stride;
 
+    constexpr bool FAST = FastCone<GEOM, DIM>::ok;
     __shared__ double s_xi[DIM][BT];
+    __shared__ __align__(16) float4 s_fi[FAST ? BT : 1];   // (t, x, y, z) of the past points in fp32
+    __shared__ __align__(16) float s_hi[FAST ? BT : 4];    // h of the past points in fp32
+    __shared__ double s_red[3][BUILD_THREADS / 32];
     __shared__ uint32_t s_U[BT][9];   // row i_local, 32-bit word = 32 columns j
     __shared__ uint32_t s_L[BT][9];   // row j_local, 32-bit word = 32 rows i
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const double qnan = __longlong_as_double(0x7FF8000000000000LL);   // compares false: unrelated
+    const bool diag = (I == J);
 
+    double xi0[DIM];
     {   // stage the tile's past points (SoA), NaN beyond N
         int64_t gi = (int64_t)I * BT + tid;
 #pragma unroll
-        for (int d = 0; d < DIM; d++) s_xi[d][tid] = (gi < N) ? coords[gi * DIM + d] : qnan;
+        for (int d = 0; d < DIM; d++) {
+            xi0[d] = (gi < N) ? coords[gi * DIM + d] : qnan;
+            s_xi[d][tid] = xi0[d];
+        }
     }
     double xj[DIM];
     const int jl = warp * 32 + lane;
@@ -93,26 +143,81 @@ k_causal_matrix(const double *__restrict__ coords, int64_t N, int64_t stride,
 #pragma unroll
         for (int d = 0; d < DIM; d++) xj[d] = (gj < N) ? coords[gj * DIM + d] : qnan;
     }
-    __syncthreads();
 
-    const bool diag = (I == J);
+    bool fast = false;
+    float fj[4] = {0.f, 0.f, 0.f, 0.f}, hj = 0.f, m = 0.f;
+    if (FAST && !diag) {
+        // tile summaries: C = max |coordinate| (fmax ignores NaN), max t_i, min t_j
+        double c = 0.0, si = 0.0, sj = 0.0;
+#pragma unroll
+        for (int d = 0; d < DIM; d++) {
+            c = fmax(c, fmax(fabs(xi0[d]), fabs(xj[d])));
+            if (d > 0) { si += xi0[d] * xi0[d]; sj += xj[d] * xj[d]; }
+        }
+        const double wc = warp_max(c), wti = warp_max(xi0[0]), wtj = warp_max(-xj[0]);
+        if (lane == 0) { s_red[0][warp] = wc; s_red[1][warp] = wti; s_red[2][warp] = wtj; }
+        s_fi[tid] = make_float4((float)xi0[0], DIM > 1 ? (float)xi0[1 % DIM] : 0.f, DIM > 2 ? (float)xi0[2 % DIM] : 0.f,
+                                DIM > 3 ? (float)xi0[3 % DIM] : 0.f);
+        s_hi[tid] = (float)(0.5 * (xi0[0] * xi0[0] - si));
+#pragma unroll
+        for (int d = 0; d < DIM; d++) fj[d] = (float)xj[d];
+        hj = (float)(0.5 * (xj[0] * xj[0] - sj));
+        __syncthreads();
+        double C = s_red[0][0], tmaxI = s_red[1][0], ntminJ = s_red[2][0];
+#pragma unroll
+        for (int w = 1; w < BUILD_THREADS / 32; w++) {
+            C = fmax(C, s_red[0][w]);
+            tmaxI = fmax(tmaxI, s_red[1][w]);
+            ntminJ = fmax(ntminJ, s_red[2][w]);
+        }
+        fast = (tmaxI <= -ntminJ) && (C >= 0x1p-40) && (C <= 0x1p40);
+        m = __double2float_ru(C * C * (0x1p-18 * 1.001));
+    } else {
+        __syncthreads();
+    }
+
 #pragma unroll 1
     for (int sb = 0; sb < BT / 32; sb++) {
-        uint32_t uw = 0, lw = 0;
-#pragma unroll 8
-        for (int ii = 0; ii < 32; ii++) {
-            const int il = sb * 32 + ii;
-            double xi[DIM];
+        uint32_t lw = 0;
+        bool slow = !fast;
+        if (FAST && fast) {
+            bool unc = false;
 #pragma unroll
-            for (int d = 0; d < DIM; d++) xi[d] = s_xi[d][il];
-            bool r = Pred<GEOM, DIM>::rel(xi, xj);
-            if (diag) r = r && (il < jl);
-            uint32_t bal = __ballot_sync(0xffffffffu, r);
-            if (lane == ii) uw = bal;
-            lw |= (r ? 1u : 0u) << ii;
+            for (int i4 = 0; i4 < 32; i4 += 4) {
+                const float4 h4 = *reinterpret_cast<const float4 *>(&s_hi[sb * 32 + i4]);
+                const float hq[4] = {h4.x, h4.y, h4.z, h4.w};
+#pragma unroll
+                for (int q = 0; q < 4; q++) {
+                    const float4 p = s_fi[sb * 32 + i4 + q];
+                    float a = fmaf(-p.x, fj[0], hq[q]);
+                    if (DIM > 1) a = fmaf(p.y, fj[1], a);
+                    if (DIM > 2) a = fmaf(p.z, fj[2], a);
+                    if (DIM > 3) a = fmaf(p.w, fj[3], a);
+                    a = a + hj;
+                    if (a > m) lw |= 1u << (i4 + q);
+                    unc = unc || !(fabsf(a) > m);
+                }
+            }
+            slow = __any_sync(0xffffffffu, unc);
+            if (slow) lw = 0;
         }
-        s_U[sb * 32 + lane][warp] = uw;
-        s_L[jl][sb] = lw;
+        if (slow) {
+#pragma unroll 8
+            for (int ii = 0; ii < 32; ii++) {
+                const int il = sb * 32 + ii;
+                double xi[DIM];
+#pragma unroll
+                for (int d = 0; d < DIM; d++) xi[d] = s_xi[d][il];
+                const bool r = Pred<GEOM, DIM>::rel(xi, xj);
+                lw |= (r ? 1u : 0u) << ii;
+            }
+            if (diag) {   // only i < j inside the diagonal tile
+                const int lo = jl - sb * 32;   // rows sb*32 + ii with ii < lo are kept
+                lw &= lo <= 0 ? 0u : (lo >= 32 ? 0xffffffffu : ((1u << lo) - 1u));
+            }
+        }
+        s_L[jl][sb] = lw;                                   // past of j: bit = row i
+        s_U[sb * 32 + lane][warp] = transpose32(lw, lane);  // future of i: bit = column j
     }
     __syncthreads();
 
@@ -186,21 +291,8 @@ int launch_causal_matrix(const double *coords, int64_t B, int64_t N, int dim, in
 }
 
 // ---- transpose -----------------------------------------------------------------------------
-// One warp transposes one 32x32 bit block with the 5-step butterfly; blocks are read as 32-bit
-// halves of the uint64 rows.
-__device__ __forceinline__ uint32_t transpose32(uint32_t x, int lane)
-{
-    const uint32_t mlo[5] = {0x0000FFFFu, 0x00FF00FFu, 0x0F0F0F0Fu, 0x33333333u, 0x55555555u};
-#pragma unroll
-    for (int t = 0; t < 5; t++) {
-        const int s = 16 >> t;
-        const uint32_t o = __shfl_xor_sync(0xffffffffu, x, s);
-        if (lane & s) x = (x & ~mlo[t]) | ((o >> s) & mlo[t]);
-        else          x = (x & mlo[t]) | ((o << s) & ~mlo[t]);
-    }
-    return x;
-}
-
+// One warp transposes one 32x32 bit block (transpose32 above); blocks are read as 32-bit halves of the
+// uint64 rows.
 __global__ void __launch_bounds__(256)
 k_transpose_bits(const uint64_t *__restrict__ bits, int64_t N, int64_t stride, uint64_t *__restrict__ bitsT)
 {

@@ -21,6 +21,8 @@
 // Products are 0 or 1 and the fp32 accumulators are exact for counts < 2^24.
 #include <cuda.h>
 
+#include <type_traits>
+
 #include "cs_common.cuh"
 
 namespace cs {
@@ -37,7 +39,8 @@ constexpr int BROW = GK * 32;           // bytes per staged bit row (TMA box inn
 constexpr int NB = 4;                   // bit-row buffers
 constexpr int BITS_BYTES = (TM + TNH) * BROW;       // 16 KiB
 constexpr int STAGE_BYTES = TNH * (KSTEP / 2);      // 16 KiB: this CTA's half of B
-constexpr int HS = 2048;                // shared-memory histogram bins
+constexpr int HS_MAX = 16896;            // shared-memory histogram bins that fit beside the operand rings
+constexpr int HS_BATCHED = 2048;        // bins when several causets share a CTA (flushed at every switch)
 constexpr int BANDW = 8;                // diagonals per band of the tile order
 #ifndef CS_PAIR_DIAG
 #define CS_PAIR_DIAG 0      // timing experiments only (results are wrong): 1 no B stores, 2 no A stores, 4 no tally
@@ -50,7 +53,8 @@ constexpr int BANDW = 8;                // diagonals per band of the tile order
 // row slice (128 columns) in registers, so registers are re-split by warpgroup with setmaxnreg.
 constexpr int EPI_WARPS = 8, EXPA_WARP0 = 8, EXPB_WARP0 = 12, EXP_WARPS = 8, MMA_WARP = 16, LOAD_WARP = 17;
 constexpr int THREADS = 20 * 32;
-constexpr int SMEM_BYTES = NS * STAGE_BYTES + NB * BITS_BYTES + HS * 4 + 512;
+constexpr int SMEM_FIXED = NS * STAGE_BYTES + NB * BITS_BYTES + 512;      // + 4 bytes per histogram bin
+constexpr int SMEM_BYTES = SMEM_FIXED + HS_MAX * 4;
 
 // block-scaled instruction descriptor, kind::mxf4: A = B = E2M1 (1 at bits 7 and 10), both K-major,
 // N >> 3 at bit 17, scale format UE8M0 (bit 23), M >> 4 at bit 24 (M = 256 over the pair), K = 64
@@ -269,24 +273,27 @@ struct Tile {
     bool skip;     // no row of the tile inside [row_begin, row_end)
 };
 
+// SMALL: kmax <= 3 (the Monte-Carlo case, only N_0..N_3 enter Eq. 4.10-4.12): the tally keeps packed
+// counters in registers and never touches the shared histogram (hs = 0).
+template <bool SMALL>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(THREADS, 1)
 k_interval_pair(const __grid_constant__ CUtensorMap mapU, const __grid_constant__ CUtensorMap mapL,
                 const uint64_t *__restrict__ bits, const uint32_t *__restrict__ tile_tab,
-                int64_t B, int64_t N, int64_t stride, int64_t kmax,
+                int64_t B, int64_t N, int64_t stride, int64_t kmax, int hs,
                 int64_t row_begin, int64_t row_end,
                 unsigned long long *__restrict__ hist, unsigned long long *__restrict__ nrel)
 {
     extern __shared__ __align__(1024) unsigned char smem[];
     unsigned char *s_stage = smem;
     unsigned char *s_bits = smem + NS * STAGE_BYTES;
-    uint32_t *s_hist = reinterpret_cast<uint32_t *>(smem + NS * STAGE_BYTES + NB * BITS_BYTES);
-    uint64_t *s_full = reinterpret_cast<uint64_t *>(smem + NS * STAGE_BYTES + NB * BITS_BYTES + HS * 4);
+    uint64_t *s_full = reinterpret_cast<uint64_t *>(smem + NS * STAGE_BYTES + NB * BITS_BYTES);
     uint64_t *s_empty = s_full + NS;      // [NS] stage free again (multicast commit from CTA 0)
     uint64_t *s_tfull = s_empty + NS;     // [1] accumulator complete (multicast commit)
     uint64_t *s_tempty = s_tfull + 1;     // [1] accumulator drained (used in CTA 0 only)
     uint64_t *s_bfull = s_tempty + 1;     // [NB] staged bit rows have landed
     uint64_t *s_bempty = s_bfull + NB;    // [NB] every expander warp is done with the buffer
     uint32_t *s_tmem = reinterpret_cast<uint32_t *>(s_bempty + NB);
+    uint32_t *s_hist = reinterpret_cast<uint32_t *>(smem + SMEM_FIXED);   // [hs], sized by the launcher
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const uint32_t rank = cluster_ctarank();
@@ -297,7 +304,6 @@ k_interval_pair(const __grid_constant__ CUtensorMap mapU, const __grid_constant_
     const uint32_t total_tiles = tiles_per * (uint32_t)B;
     const uint32_t t0 = cluster_id_x(), tstep = num_clusters_x();
     const int ib0 = (int)(row_begin / TILE), ib1 = (int)((row_end + TILE - 1) / TILE);   // I blocks inside the row range
-    const int hs = (int)((kmax + 1 < HS) ? (kmax + 1) : HS);
     const int64_t hist_len = kmax + 1;
 
     auto get_tile = [&](uint32_t t) {
@@ -323,7 +329,7 @@ k_interval_pair(const __grid_constant__ CUtensorMap mapU, const __grid_constant_
         mbar_init(s_tempty, 2 * EPI_WARPS);         // epilogue warps of both CTAs (counted in CTA 0)
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
-    for (int b = tid; b < HS; b += THREADS) s_hist[b] = 0;
+    for (int b = tid; b < hs; b += THREADS) s_hist[b] = 0;
     if (warp == MMA_WARP) {   // all 512 TMEM columns of both SMs of the pair
         asm volatile("tcgen05.alloc.cta_group::2.sync.aligned.shared::cta.b32 [%0], 512;" ::"r"(smem_u32(s_tmem)));
         asm volatile("tcgen05.relinquish_alloc_permit.cta_group::2.sync.aligned;");
@@ -502,21 +508,37 @@ k_interval_pair(const __grid_constant__ CUtensorMap mapU, const __grid_constant_
         asm volatile("setmaxnreg.inc.sync.aligned.u32 152;");
         uint32_t tile_seq = 0;
         unsigned long long my_nrel = 0;
-        const uint32_t kmax32 = (uint32_t)kmax;
         int cur_batch = -1;
         const int quarter = warp & 3, colhalf = warp >> 2;   // TMEM lane quarter; which 128 columns
         const uint32_t taddr = tmem_base + ((uint32_t)(quarter * 32) << 16) + colhalf * 128;
+        // Counts are exact small integers held as fp32: adding 2^23 leaves the count in the low mantissa
+        // bits (one FADD, no F2I), and comparisons are taken on the float itself.
+        const uint32_t kmax32 = (uint32_t)kmax;
+        uint32_t small[4] = {0, 0, 0, 0};                    // SMALL: this thread's tallies of counts 0..3
+        auto flush_small = [&](int batch) {                  // one warp reduction, <= 4 global atomics per warp
+#pragma unroll
+            for (int q = 0; q < 4; q++) {
+                uint32_t c = small[q];
+#pragma unroll
+                for (int sft = 16; sft >= 1; sft >>= 1) c += __shfl_xor_sync(0xffffffffu, c, sft);
+                if (lane == 0 && c && q <= kmax) atomicAdd(&hist[(int64_t)batch * hist_len + q], (unsigned long long)c);
+                small[q] = 0;
+            }
+        };
         for (uint32_t t = t0; t < total_tiles; t += tstep) {
             const Tile tc = get_tile(t);
             if (tc.skip) continue;
             if (tc.b != cur_batch) {   // per-causet histograms: flush before switching
                 if (cur_batch >= 0 && B > 1) {
-                    asm volatile("bar.sync 1, 256;");
-                    for (int b = tid; b < hs; b += EPI_WARPS * 32) {
-                        uint32_t v = s_hist[b];
-                        if (v) { atomicAdd(&hist[(int64_t)cur_batch * hist_len + b], (unsigned long long)v); s_hist[b] = 0; }
+                    if (SMALL) flush_small(cur_batch);
+                    else {
+                        asm volatile("bar.sync 1, 256;" ::: "memory");
+                        for (int b = tid; b < hs; b += EPI_WARPS * 32) {
+                            uint32_t v = s_hist[b];
+                            if (v) { atomicAdd(&hist[(int64_t)cur_batch * hist_len + b], (unsigned long long)v); s_hist[b] = 0; }
+                        }
+                        asm volatile("bar.sync 1, 256;" ::: "memory");
                     }
-                    asm volatile("bar.sync 1, 256;");
                 }
                 cur_batch = tc.b;
             }
@@ -544,26 +566,60 @@ k_interval_pair(const __grid_constant__ CUtensorMap mapU, const __grid_constant_
             tile_seq++;
             if (CS_PAIR_DIAG & 4) continue;
             my_nrel += __popcll(rel[0]) + __popcll(rel[1]);
+            // Tally over the 128 columns in registers; 32 columns at a time are skipped when no lane of
+            // the warp has a related pair there.  SMALL is branch-free (a branch per related pair
+            // serialises on the latency of every step with two warps per scheduler: measured 7x the MMA
+            // time of a 2048-point causet).  The general path needs one branch per column -- ptxas never
+            // predicates an atomic -- and a second one only in tiles long enough to hold counts >= hs.
+            uint32_t acc0 = 0, acc1 = 0;                         // SMALL: four 8-bit fields, <= 64 increments each
+            const bool maybe_big = (uint32_t)(tc.J - tc.I + 1) * TILE > (uint32_t)hs;   // counts < (J-I+1) 256
+            auto tally = [&](auto big_tag) {
+                constexpr bool BIG = decltype(big_tag)::value;
 #pragma unroll
-            for (int c16 = 0; c16 < 8; c16++) {
-                const uint32_t rel16 = (uint32_t)(rel[c16 >> 2] >> (16 * (c16 & 3))) & 0xFFFFu;
-                if (!__any_sync(0xffffffffu, rel16 != 0)) continue;
+                for (int w = 0; w < 4; w++) {
+                    const uint32_t relw = (uint32_t)(rel[w >> 1] >> (32 * (w & 1)));
+                    if (!__any_sync(0xffffffffu, relw != 0)) continue;
 #pragma unroll
-                for (int c = 0; c < 16; c++) {
-                    if (rel16 & (1u << c)) {
-                        const uint32_t cnt = (uint32_t)__uint_as_float(v[c16 * 16 + c]);   // 0/1 products: exact in fp32
-                        if (cnt < (uint32_t)hs) atomicAdd(&s_hist[cnt], 1u);
-                        else if (cnt <= kmax32) atomicAdd(&ghist[cnt], 1ULL);
+                    for (int c = 0; c < 32; c++) {
+                        const float f = __uint_as_float(v[w * 32 + c]);
+                        const uint32_t ub = __float_as_uint(f + 8388608.0f);        // 0x4B000000 + count
+                        if (SMALL) {
+                            // inc = 1 << 8 count; shl.b32 clamps the shift amount, so counts >= 4 give 0.
+                            // FADD, LEA, SHF, R2P (7 columns at once), SEL, 1/2 IADD3 per column.
+                            uint32_t &acc = (c & 1) ? acc1 : acc0;
+                            asm("{\n"
+                                ".reg .pred r;\n"
+                                ".reg .u32 t, i;\n"
+                                "and.b32 t, %1, %2;\n"
+                                "setp.ne.u32 r, t, 0;\n"
+                                "shl.b32 i, 1, %3;\n"
+                                "@r add.u32 %0, %0, i;\n"
+                                "}\n" : "+r"(acc) : "r"(relw), "r"(1u << c), "r"((ub - 0x4B000000u) * 8u));
+                        } else if (relw & (1u << c)) {
+                            const uint32_t cnt = ub - 0x4B000000u;
+                            if (!BIG || cnt < (uint32_t)hs) atomicAdd(&s_hist[cnt], 1u);
+                            else if (cnt <= kmax32) atomicAdd(&ghist[cnt], 1ULL);
+                        }
                     }
                 }
+            };
+            if (!SMALL && maybe_big) tally(std::true_type{});
+            else tally(std::false_type{});
+            if (SMALL) {
+#pragma unroll
+                for (int q = 0; q < 4; q++) small[q] += ((acc0 >> (8 * q)) & 0xFFu) + ((acc1 >> (8 * q)) & 0xFFu);
             }
         }
         // final flush by the epilogue warps
-        asm volatile("bar.sync 1, 256;");
-        if (cur_batch >= 0) {
-            for (int b = tid; b < hs; b += EPI_WARPS * 32) {
-                uint32_t v = s_hist[b];
-                if (v) atomicAdd(&hist[(int64_t)cur_batch * hist_len + b], (unsigned long long)v);
+        if (SMALL) {
+            if (cur_batch >= 0) flush_small(cur_batch);
+        } else {
+            asm volatile("bar.sync 1, 256;" ::: "memory");
+            if (cur_batch >= 0) {
+                for (int b = tid; b < hs; b += EPI_WARPS * 32) {
+                    uint32_t v = s_hist[b];
+                    if (v) atomicAdd(&hist[(int64_t)cur_batch * hist_len + b], (unsigned long long)v);
+                }
             }
         }
         if (nrel && B == 1) {
@@ -642,7 +698,8 @@ int launch_interval_pair(const uint64_t *bits, const uint64_t *bitsT, int64_t B,
     if (!scratch || scratch_bytes < interval_pair_scratch_bytes(N)) return CS_ERR_WORKSPACE;
     static bool attr_set = false;
     if (!attr_set) {
-        CS_CUDA(cudaFuncSetAttribute(k_interval_pair, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES));
+        CS_CUDA(cudaFuncSetAttribute(k_interval_pair<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES));
+        CS_CUDA(cudaFuncSetAttribute(k_interval_pair<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_FIXED));
         attr_set = true;
     }
     const int64_t stride = row_stride_words(N);
@@ -659,9 +716,18 @@ int launch_interval_pair(const uint64_t *bits, const uint64_t *bitsT, int64_t B,
     int64_t clusters = sm_count() / 2;
     if (clusters > total) clusters = total;
     if (clusters < 1) clusters = 1;
-    k_interval_pair<<<(unsigned)(2 * clusters), THREADS, SMEM_BYTES, st>>>(
-        mapU, mapL, bits, tab, B, N, stride, kmax, row_begin, row_end,
-        reinterpret_cast<unsigned long long *>(hist), reinterpret_cast<unsigned long long *>(nrel));
+    // shared histogram: every bin up to kmax if it fits (N <= 16384 then needs no global atomics at all)
+    const bool small = kmax <= 3;
+    const int64_t hs_cap = B > 1 ? HS_BATCHED : HS_MAX;
+    const int hs = small ? 0 : (int)(kmax + 1 < hs_cap ? kmax + 1 : hs_cap);
+    if (small)
+        k_interval_pair<true><<<(unsigned)(2 * clusters), THREADS, SMEM_FIXED, st>>>(
+            mapU, mapL, bits, tab, B, N, stride, kmax, hs, row_begin, row_end,
+            reinterpret_cast<unsigned long long *>(hist), reinterpret_cast<unsigned long long *>(nrel));
+    else
+        k_interval_pair<false><<<(unsigned)(2 * clusters), THREADS, SMEM_FIXED + hs * 4, st>>>(
+            mapU, mapL, bits, tab, B, N, stride, kmax, hs, row_begin, row_end,
+            reinterpret_cast<unsigned long long *>(hist), reinterpret_cast<unsigned long long *>(nrel));
     CS_LAUNCHED("k_interval_pair");
     return CS_OK;
 }
