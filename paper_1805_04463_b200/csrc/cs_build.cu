@@ -73,9 +73,9 @@ struct Pred<CS_GEOM_DS2_SLAB, 2> {
 //     a < -m  =>  T < -30 u C^2  : unrelated    holds for the whole tile, checked below)
 // and anything else -- including NaN -- is re-evaluated with the fp64 expression of the header for
 // the whole 32 x 32 block.  The output is therefore bit-identical to the plain fp64 evaluation.
-// The tile takes this path only if it is off the diagonal, max t_i <= min t_j (so the header's
-// dt >= 0 holds for every pair; always the case for time-sorted input) and 2^-40 <= C <= 2^40 (no
-// overflow or underflow in the fp32 products).
+// The tile takes this path only if the header's dt >= 0 holds for every pair it keeps (off the
+// diagonal: max t_i <= min t_j; diagonal tile: its points are in time order -- always the case for
+// time-sorted input) and 2^-40 <= C <= 2^40 (no overflow or underflow in the fp32 products).
 template <int GEOM, int DIM>
 struct FastCone { static constexpr bool ok = false; };
 template <int DIM>
@@ -146,8 +146,9 @@ k_causal_matrix(const double *__restrict__ coords, int64_t N, int64_t stride,
 
     bool fast = false;
     float fj[4] = {0.f, 0.f, 0.f, 0.f}, hj = 0.f, m = 0.f;
-    if (FAST && !diag) {
-        // tile summaries: C = max |coordinate| (fmax ignores NaN), max t_i, min t_j
+    if (FAST) {
+        // tile summaries: C = max |coordinate| (fmax ignores NaN), max t_i, min t_j; inside the diagonal
+        // tile i < j must imply t_i <= t_j instead, i.e. the tile's own points are in time order
         double c = 0.0, si = 0.0, sj = 0.0;
 #pragma unroll
         for (int d = 0; d < DIM; d++) {
@@ -170,7 +171,14 @@ k_causal_matrix(const double *__restrict__ coords, int64_t N, int64_t stride,
             tmaxI = fmax(tmaxI, s_red[1][w]);
             ntminJ = fmax(ntminJ, s_red[2][w]);
         }
-        fast = (tmaxI <= -ntminJ) && (C >= 0x1p-40) && (C <= 0x1p40);
+        bool ordered;
+        if (diag) {   // points beyond N are NaN and only ever sit at the end: their pairs read unrelated either way
+            const bool last = tid == BT - 1 || (int64_t)I * BT + tid + 1 >= N;
+            ordered = __syncthreads_and(last || xi0[0] <= s_xi[0][last ? tid : tid + 1]) != 0;
+        } else {
+            ordered = tmaxI <= -ntminJ;
+        }
+        fast = ordered && (C >= 0x1p-40) && (C <= 0x1p40);
         m = __double2float_ru(C * C * (0x1p-18 * 1.001));
     } else {
         __syncthreads();
@@ -180,7 +188,8 @@ k_causal_matrix(const double *__restrict__ coords, int64_t N, int64_t stride,
     for (int sb = 0; sb < BT / 32; sb++) {
         uint32_t lw = 0;
         bool slow = !fast;
-        if (FAST && fast) {
+        if (diag && sb > warp) slow = false;      // rows all at or below the diagonal: nothing to evaluate
+        else if (FAST && fast) {
             bool unc = false;
 #pragma unroll
             for (int i4 = 0; i4 < 32; i4 += 4) {
@@ -211,10 +220,10 @@ k_causal_matrix(const double *__restrict__ coords, int64_t N, int64_t stride,
                 const bool r = Pred<GEOM, DIM>::rel(xi, xj);
                 lw |= (r ? 1u : 0u) << ii;
             }
-            if (diag) {   // only i < j inside the diagonal tile
-                const int lo = jl - sb * 32;   // rows sb*32 + ii with ii < lo are kept
-                lw &= lo <= 0 ? 0u : (lo >= 32 ? 0xffffffffu : ((1u << lo) - 1u));
-            }
+        }
+        if (diag) {   // only i < j inside the diagonal tile
+            const int lo = jl - sb * 32;   // rows sb*32 + ii with ii < lo are kept
+            lw &= lo <= 0 ? 0u : (lo >= 32 ? 0xffffffffu : ((1u << lo) - 1u));
         }
         s_L[jl][sb] = lw;                                   // past of j: bit = row i
         s_U[sb * 32 + lane][warp] = transpose32(lw, lane);  // future of i: bit = column j

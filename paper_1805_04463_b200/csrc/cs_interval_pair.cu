@@ -39,7 +39,10 @@ constexpr int BROW = GK * 32;           // bytes per staged bit row (TMA box inn
 constexpr int NB = 4;                   // bit-row buffers
 constexpr int BITS_BYTES = (TM + TNH) * BROW;       // 16 KiB
 constexpr int STAGE_BYTES = TNH * (KSTEP / 2);      // 16 KiB: this CTA's half of B
-constexpr int HS_MAX = 16896;            // shared-memory histogram bins that fit beside the operand rings
+#ifndef CS_PAIR_HS_MAX
+#define CS_PAIR_HS_MAX 16896
+#endif
+constexpr int HS_MAX = CS_PAIR_HS_MAX;   // shared-memory histogram bins that fit beside the operand rings
 constexpr int HS_BATCHED = 2048;        // bins when several causets share a CTA (flushed at every switch)
 constexpr int BANDW = 8;                // diagonals per band of the tile order
 #ifndef CS_PAIR_DIAG

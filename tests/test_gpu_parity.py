@@ -91,6 +91,54 @@ def test_causal_matrix_near_null_pairs(api, oracle):
     assert np.array_equal(to_u64(bits), o_bits)
 
 
+def _near_null_set(rng, n, dim):
+    """n base points and, for each, partners on the cone and one ulp either side of it (time-sorted)."""
+    base = rng.uniform(-0.5, 0.5, (n, dim))
+    base[:, 0] = rng.uniform(-1, 0, n)
+    r = rng.uniform(0.05, 0.6, n)
+    dx = rng.normal(size=(n, dim - 1))
+    dx = dx / np.linalg.norm(dx, axis=1)[:, None] * r[:, None]
+    fut = base.copy()
+    fut[:, 1:] = base[:, 1:] + dx
+    fut[:, 0] = base[:, 0] + np.sqrt((dx ** 2).sum(axis=1))
+    fut2 = fut.copy(); fut2[:, 0] = np.nextafter(fut[:, 0], 10.0)
+    fut3 = fut.copy(); fut3[:, 0] = np.nextafter(fut[:, 0], -10.0)
+    coords = np.concatenate([base, fut, fut2, fut3])
+    return np.ascontiguousarray(coords[np.lexsort((coords[:, 1], coords[:, 0]))])
+
+
+@pytest.mark.parametrize("dim", [2, 3, 4])
+@pytest.mark.parametrize("scale", [1.0, 2.0 ** 30, 2.0 ** -30, 2.0 ** 45, 2.0 ** -45, 2.0 ** 600, 2.0 ** -600])
+def test_causal_matrix_prefilter_bands(api, oracle, dim, scale):
+    """The single-precision prefilter of the flat cone never decides a pair the fp64 expression would
+    decide differently: thousands of pairs within an ulp of the cone spread over many tiles, at
+    coordinate scales inside and outside the prefilter's range (|x| in 2^-40 .. 2^40)."""
+    rng = np.random.default_rng(7 + dim)
+    coords = _near_null_set(rng, 700, dim) * scale          # N = 2800: 11 tiles per side
+    o_bits = oracle.causal_matrix_bits(coords, inp.GEOM_MINK_CONE)
+    bits, bitsT = gpu_bits(api, coords, inp.GEOM_MINK_CONE)
+    assert np.array_equal(to_u64(bits), o_bits)
+    assert np.array_equal(to_u64(bitsT), oracle.transpose_bits(o_bits, coords.shape[0]))
+
+
+def test_causal_matrix_prefilter_unsorted_inf_nan(api, oracle):
+    """Inputs that break the prefilter's preconditions fall back to the fp64 expression: elements not
+    sorted by time (dt < 0 must read unrelated), infinite and NaN coordinates, a tile of identical points."""
+    rng = np.random.default_rng(11)
+    N = 1500
+    coords = inp.sprinkle(inp.GEOM_MINK_CONE, 4, N, 5)
+    shuffled = np.ascontiguousarray(coords[rng.permutation(N)])
+    weird = coords.copy()
+    weird[300, 0] = np.inf; weird[301, 2] = -np.inf; weird[700, 0] = np.nan; weird[701, 3] = np.nan
+    weird[900:1200] = weird[900]                            # more than one tile of identical points
+    late = coords.copy(); late[5, 0] = 2.0                  # one element far out of time order
+    for c in (shuffled, weird, late):
+        o_bits = oracle.causal_matrix_bits(c, inp.GEOM_MINK_CONE)
+        bits, bitsT = gpu_bits(api, c, inp.GEOM_MINK_CONE)
+        assert np.array_equal(to_u64(bits), o_bits)
+        assert np.array_equal(to_u64(bitsT), oracle.transpose_bits(o_bits, N))
+
+
 def test_degenerate_inputs(api, oracle):
     # identical points, NaN coordinates, N = 0
     coords = np.zeros((70, 4)); coords[10:20, 1] = np.nan
@@ -246,3 +294,19 @@ def test_config3_full_size(api, oracle):
 @pytest.mark.slow
 def test_config4_full_size(api, oracle):
     _full_size_check(api, oracle, inp.CONFIGS[4], full_hist=False)
+
+
+@pytest.mark.slow
+def test_config5_full_size(api, oracle):
+    """The whole ensemble (4096 x N=2048) in the one launch bench-style callers use; every causet's
+    N_0..N_3 and action against the oracle (tier-1, itself pinned to tier-0 at this N)."""
+    cfg = inp.CONFIGS[5]
+    coords = inp.make_ensemble_coords(cfg)
+    B = coords.shape[0]
+    assert B == 4096 and coords.shape[1] == 2048
+    actions, hist4 = api.bd_action_batched(torch.from_numpy(coords).cuda(), cfg.geometry, return_hist4=True)
+    actions = actions.cpu().numpy(); hist4 = hist4.cpu().numpy()
+    for b in range(B):
+        _, o_hist, o_S, _ = oracle.action_pipeline(coords[b], cfg.geometry, tier=1)
+        assert np.array_equal(hist4[b], o_hist[:4]), "causet %d" % b
+        assert actions[b] == o_S, "causet %d" % b
