@@ -103,29 +103,87 @@ __device__ __forceinline__ uint32_t transpose32(uint32_t x, int lane)
     return x;
 }
 
+constexpr int NJ = 2;            // future points per lane: a CTA covers 256 rows x 512 columns
+
+// One 32 x 32 block per future point k < NK of this lane: bit ii of lw[k] = (row i0 + ii  -<  point k),
+// decided by the fp32 prefilter; unc[k] is set if any of the lane's 32 decisions is inside the error
+// band.  The row's (t, x, y, z) and h are loaded once (LDS.128 broadcasts) for all NK points.
+template <int DIM, int NK>
+__device__ __forceinline__ void fast_block(const float4 *__restrict__ fi, const float *__restrict__ hi,
+                                           const float (*fj)[4], const float *hj, const float *m,
+                                           uint32_t *lw, bool *unc)
+{
+#pragma unroll
+    for (int i4 = 0; i4 < 32; i4 += 4) {
+        const float4 h4 = *reinterpret_cast<const float4 *>(hi + i4);
+        const float hq[4] = {h4.x, h4.y, h4.z, h4.w};
+#pragma unroll
+        for (int q = 0; q < 4; q++) {
+            const float4 p = fi[i4 + q];
+#pragma unroll
+            for (int k = 0; k < NK; k++) {
+                float a = fmaf(-p.x, fj[k][0], hq[q]);
+                if (DIM > 1) a = fmaf(p.y, fj[k][1], a);
+                if (DIM > 2) a = fmaf(p.z, fj[k][2], a);
+                if (DIM > 3) a = fmaf(p.w, fj[k][3], a);
+                a = a + hj[k];
+                if (a > m[k]) lw[k] |= 1u << (i4 + q);
+                unc[k] = unc[k] || !(fabsf(a) > m[k]);
+            }
+        }
+    }
+}
+
+// The same block with the fp64 expression of include/causalset.h (the definition).
+template <int GEOM, int DIM, int NK>
+__device__ __forceinline__ void exact_block(const double (*xi_s)[BT], int i0, const double (*xj)[DIM], uint32_t *lw)
+{
+#pragma unroll 8
+    for (int ii = 0; ii < 32; ii++) {
+        double xi[DIM];
+#pragma unroll
+        for (int d = 0; d < DIM; d++) xi[d] = xi_s[d][i0 + ii];
+#pragma unroll
+        for (int k = 0; k < NK; k++) lw[k] |= (Pred<GEOM, DIM>::rel(xi, xj[k]) ? 1u : 0u) << ii;
+    }
+}
+
 template <int GEOM, int DIM>
 __global__ void __launch_bounds__(BUILD_THREADS)
 k_causal_matrix(const double *__restrict__ coords, int64_t N, int64_t stride,
                 uint64_t *__restrict__ bits, uint64_t *__restrict__ bitsT)
 {
-    const int J = blockIdx.x, I = blockIdx.y;
-    if (I > J) return;
+    const int JS = blockIdx.x, I = blockIdx.y;
+    const int nT = gridDim.y;
+    if (JS * NJ + NJ - 1 < I) return;             // every column tile of this CTA lies below the diagonal
     const int64_t b = blockIdx.z;
     coords += b * N * DIM;
     bits += b * N * stride;
     if (bitsT) bitsT += b * N * stride;
 
     constexpr bool FAST = FastCone<GEOM, DIM>::ok;
+    constexpr int NW = BUILD_THREADS / 32;
     __shared__ double s_xi[DIM][BT];
     __shared__ __align__(16) float4 s_fi[FAST ? BT : 1];   // (t, x, y, z) of the past points in fp32
     __shared__ __align__(16) float s_hi[FAST ? BT : 4];    // h of the past points in fp32
-    __shared__ double s_red[3][BUILD_THREADS / 32];
-    __shared__ uint32_t s_U[BT][9];   // row i_local, 32-bit word = 32 columns j
-    __shared__ uint32_t s_L[BT][9];   // row j_local, 32-bit word = 32 rows i
+    __shared__ __align__(16) uint32_t s_U[BT][NJ * 8 + 1]; // row i_local, 32-bit word = 32 columns j
+    __shared__ uint32_t s_L[NJ * BT][9];                   // row j_local, 32-bit word = 32 rows i
+    double (*s_red)[NW] = reinterpret_cast<double (*)[NW]>(&s_U[0][0]);   // [2 + 2 NJ][NW], dead before s_U is written
+    static_assert((2 + 2 * NJ) * NW * sizeof(double) <= sizeof(uint32_t) * BT * (NJ * 8 + 1), "s_red fits in s_U");
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const double qnan = __longlong_as_double(0x7FF8000000000000LL);   // compares false: unrelated
-    const bool diag = (I == J);
+    const int jl = warp * 32 + lane;
+
+    bool act[NJ], dg[NJ];
+    bool any_diag = false;
+#pragma unroll
+    for (int k = 0; k < NJ; k++) {
+        const int J = JS * NJ + k;
+        act[k] = J >= I && J < nT;
+        dg[k] = J == I;
+        any_diag = any_diag || dg[k];
+    }
 
     double xi0[DIM];
     {   // stage the tile's past points (SoA), NaN beyond N
@@ -136,114 +194,144 @@ k_causal_matrix(const double *__restrict__ coords, int64_t N, int64_t stride,
             s_xi[d][tid] = xi0[d];
         }
     }
-    double xj[DIM];
-    const int jl = warp * 32 + lane;
-    {
-        int64_t gj = (int64_t)J * BT + jl;
+    double xj[NJ][DIM];
 #pragma unroll
-        for (int d = 0; d < DIM; d++) xj[d] = (gj < N) ? coords[gj * DIM + d] : qnan;
+    for (int k = 0; k < NJ; k++) {
+        int64_t gj = (int64_t)(JS * NJ + k) * BT + jl;
+#pragma unroll
+        for (int d = 0; d < DIM; d++) xj[k][d] = (act[k] && gj < N) ? coords[gj * DIM + d] : qnan;
     }
 
-    bool fast = false;
-    float fj[4] = {0.f, 0.f, 0.f, 0.f}, hj = 0.f, m = 0.f;
+    bool fast[NJ];
+    float fj[NJ][4], hj[NJ], m[NJ];
+#pragma unroll
+    for (int k = 0; k < NJ; k++) { fast[k] = false; hj[k] = 0.f; m[k] = 0.f; fj[k][0] = fj[k][1] = fj[k][2] = fj[k][3] = 0.f; }
     if (FAST) {
-        // tile summaries: C = max |coordinate| (fmax ignores NaN), max t_i, min t_j; inside the diagonal
-        // tile i < j must imply t_i <= t_j instead, i.e. the tile's own points are in time order
-        double c = 0.0, si = 0.0, sj = 0.0;
+        // tile summaries: largest |coordinate| of the past points and of each set of future points (fmax
+        // ignores NaN), max t_i, min t_j; inside the diagonal tile i < j must imply t_i <= t_j instead,
+        // i.e. the tile's own points are in time order
+        double ci = 0.0, si = 0.0;
 #pragma unroll
         for (int d = 0; d < DIM; d++) {
-            c = fmax(c, fmax(fabs(xi0[d]), fabs(xj[d])));
-            if (d > 0) { si += xi0[d] * xi0[d]; sj += xj[d] * xj[d]; }
+            ci = fmax(ci, fabs(xi0[d]));
+            if (d > 0) si += xi0[d] * xi0[d];
         }
-        const double wc = warp_max(c), wti = warp_max(xi0[0]), wtj = warp_max(-xj[0]);
-        if (lane == 0) { s_red[0][warp] = wc; s_red[1][warp] = wti; s_red[2][warp] = wtj; }
         s_fi[tid] = make_float4((float)xi0[0], DIM > 1 ? (float)xi0[1 % DIM] : 0.f, DIM > 2 ? (float)xi0[2 % DIM] : 0.f,
                                 DIM > 3 ? (float)xi0[3 % DIM] : 0.f);
         s_hi[tid] = (float)(0.5 * (xi0[0] * xi0[0] - si));
+        const double wci = warp_max(ci), wti = warp_max(xi0[0]);
+        if (lane == 0) { s_red[0][warp] = wci; s_red[1][warp] = wti; }
 #pragma unroll
-        for (int d = 0; d < DIM; d++) fj[d] = (float)xj[d];
-        hj = (float)(0.5 * (xj[0] * xj[0] - sj));
+        for (int k = 0; k < NJ; k++) {
+            double cj = 0.0, sj = 0.0;
+#pragma unroll
+            for (int d = 0; d < DIM; d++) {
+                cj = fmax(cj, fabs(xj[k][d]));
+                if (d > 0) sj += xj[k][d] * xj[k][d];
+                fj[k][d] = (float)xj[k][d];
+            }
+            hj[k] = (float)(0.5 * (xj[k][0] * xj[k][0] - sj));
+            const double wcj = warp_max(cj), wtj = warp_max(-xj[k][0]);
+            if (lane == 0) { s_red[2 + 2 * k][warp] = wcj; s_red[3 + 2 * k][warp] = wtj; }
+        }
         __syncthreads();
-        double C = s_red[0][0], tmaxI = s_red[1][0], ntminJ = s_red[2][0];
+        double Ci = s_red[0][0], tmaxI = s_red[1][0], Cj[NJ], ntminJ[NJ];
 #pragma unroll
-        for (int w = 1; w < BUILD_THREADS / 32; w++) {
-            C = fmax(C, s_red[0][w]);
+        for (int k = 0; k < NJ; k++) { Cj[k] = s_red[2 + 2 * k][0]; ntminJ[k] = s_red[3 + 2 * k][0]; }
+#pragma unroll
+        for (int w = 1; w < NW; w++) {
+            Ci = fmax(Ci, s_red[0][w]);
             tmaxI = fmax(tmaxI, s_red[1][w]);
-            ntminJ = fmax(ntminJ, s_red[2][w]);
+#pragma unroll
+            for (int k = 0; k < NJ; k++) { Cj[k] = fmax(Cj[k], s_red[2 + 2 * k][w]); ntminJ[k] = fmax(ntminJ[k], s_red[3 + 2 * k][w]); }
         }
-        bool ordered;
-        if (diag) {   // points beyond N are NaN and only ever sit at the end: their pairs read unrelated either way
+        bool tile_ordered = false;
+        if (any_diag) {   // points beyond N are NaN and only ever sit at the end: their pairs read unrelated either way
             const bool last = tid == BT - 1 || (int64_t)I * BT + tid + 1 >= N;
-            ordered = __syncthreads_and(last || xi0[0] <= s_xi[0][last ? tid : tid + 1]) != 0;
-        } else {
-            ordered = tmaxI <= -ntminJ;
+            tile_ordered = __syncthreads_and(last || xi0[0] <= s_xi[0][last ? tid : tid + 1]) != 0;
         }
-        fast = ordered && (C >= 0x1p-40) && (C <= 0x1p40);
-        m = __double2float_ru(C * C * (0x1p-18 * 1.001));
-    } else {
-        __syncthreads();
+#pragma unroll
+        for (int k = 0; k < NJ; k++) {
+            const double C = fmax(Ci, Cj[k]);
+            const bool ordered = dg[k] ? tile_ordered : (tmaxI <= -ntminJ[k]);
+            fast[k] = act[k] && ordered && (C >= 0x1p-40) && (C <= 0x1p40);
+            m[k] = __double2float_ru(C * C * (0x1p-18 * 1.001));
+        }
     }
+    __syncthreads();    // s_xi / s_fi / s_hi visible; s_red (aliased on s_U) no longer read
 
 #pragma unroll 1
     for (int sb = 0; sb < BT / 32; sb++) {
-        uint32_t lw = 0;
-        bool slow = !fast;
-        if (diag && sb > warp) slow = false;      // rows all at or below the diagonal: nothing to evaluate
-        else if (FAST && fast) {
-            bool unc = false;
+        uint32_t lw[NJ];
+        bool need[NJ], slow[NJ];
 #pragma unroll
-            for (int i4 = 0; i4 < 32; i4 += 4) {
-                const float4 h4 = *reinterpret_cast<const float4 *>(&s_hi[sb * 32 + i4]);
-                const float hq[4] = {h4.x, h4.y, h4.z, h4.w};
-#pragma unroll
-                for (int q = 0; q < 4; q++) {
-                    const float4 p = s_fi[sb * 32 + i4 + q];
-                    float a = fmaf(-p.x, fj[0], hq[q]);
-                    if (DIM > 1) a = fmaf(p.y, fj[1], a);
-                    if (DIM > 2) a = fmaf(p.z, fj[2], a);
-                    if (DIM > 3) a = fmaf(p.w, fj[3], a);
-                    a = a + hj;
-                    if (a > m) lw |= 1u << (i4 + q);
-                    unc = unc || !(fabsf(a) > m);
-                }
-            }
-            slow = __any_sync(0xffffffffu, unc);
-            if (slow) lw = 0;
+        for (int k = 0; k < NJ; k++) {
+            lw[k] = 0;
+            need[k] = act[k] && !(dg[k] && sb > warp);   // rows all at or below the diagonal: nothing to evaluate
+            slow[k] = need[k] && !fast[k];
         }
-        if (slow) {
-#pragma unroll 8
-            for (int ii = 0; ii < 32; ii++) {
-                const int il = sb * 32 + ii;
-                double xi[DIM];
+        if (FAST) {
+            bool unc[NJ] = {false, false};
+            const bool f0 = need[0] && fast[0], f1 = need[1] && fast[1];
+            if (f0 && f1) fast_block<DIM, 2>(s_fi + sb * 32, s_hi + sb * 32, fj, hj, m, lw, unc);
+            else if (f0) fast_block<DIM, 1>(s_fi + sb * 32, s_hi + sb * 32, fj, hj, m, lw, unc);
+            else if (f1) fast_block<DIM, 1>(s_fi + sb * 32, s_hi + sb * 32, fj + 1, hj + 1, m + 1, lw + 1, unc + 1);
 #pragma unroll
-                for (int d = 0; d < DIM; d++) xi[d] = s_xi[d][il];
-                const bool r = Pred<GEOM, DIM>::rel(xi, xj);
-                lw |= (r ? 1u : 0u) << ii;
+            for (int k = 0; k < NJ; k++) {
+                if (__any_sync(0xffffffffu, unc[k])) { slow[k] = true; lw[k] = 0; }
             }
         }
-        if (diag) {   // only i < j inside the diagonal tile
-            const int lo = jl - sb * 32;   // rows sb*32 + ii with ii < lo are kept
-            lw &= lo <= 0 ? 0u : (lo >= 32 ? 0xffffffffu : ((1u << lo) - 1u));
+        if (slow[0] && slow[1]) exact_block<GEOM, DIM, 2>(s_xi, sb * 32, xj, lw);
+        else if (slow[0]) exact_block<GEOM, DIM, 1>(s_xi, sb * 32, xj, lw);
+        else if (slow[1]) exact_block<GEOM, DIM, 1>(s_xi, sb * 32, xj + 1, lw + 1);
+#pragma unroll
+        for (int k = 0; k < NJ; k++) {
+            if (dg[k]) {   // only i < j inside the diagonal tile
+                const int lo = jl - sb * 32;   // rows sb*32 + ii with ii < lo are kept
+                lw[k] &= lo <= 0 ? 0u : (lo >= 32 ? 0xffffffffu : ((1u << lo) - 1u));
+            }
+            if (act[k]) {
+                s_L[k * BT + jl][sb] = lw[k];                                   // past of j: bit = row i
+                s_U[sb * 32 + lane][k * 8 + warp] = transpose32(lw[k], lane);   // future of i: bit = column j
+            }
         }
-        s_L[jl][sb] = lw;                                   // past of j: bit = row i
-        s_U[sb * 32 + lane][warp] = transpose32(lw, lane);  // future of i: bit = column j
     }
     __syncthreads();
 
-    // write-out: BT rows x 4 uint64 per tile; 4 consecutive threads cover one 32-byte row segment
-    const int q = tid & 3;
+    // write-out.  Rows of the I tile: NJ x 4 uint64 per row, 8 consecutive threads cover one 64-byte segment
+    // (bits: the tile; bitsT: zeros, the mirrored tile of an off-diagonal tile is identically zero).
+    {
+        const int q8 = tid & 7, k = q8 >> 2, q = q8 & 3;
+        const int J = JS * NJ + k;
+        const int64_t wj = (int64_t)J * (BT / 64) + q;
+        if (J >= I && J < nT && wj < stride) {
 #pragma unroll
-    for (int pass = 0; pass < 4; pass++) {
-        const int r = (tid >> 2) + 64 * pass;
-        const int64_t ri = (int64_t)I * BT + r, rj = (int64_t)J * BT + r;
-        const int64_t wi = (int64_t)I * (BT / 64) + q, wj = (int64_t)J * (BT / 64) + q;
-        const uint64_t u = (uint64_t)s_U[r][2 * q] | ((uint64_t)s_U[r][2 * q + 1] << 32);
-        const uint64_t l = (uint64_t)s_L[r][2 * q] | ((uint64_t)s_L[r][2 * q + 1] << 32);
-        if (ri < N && wj < stride) bits[ri * stride + wj] = u;
-        if (bitsT && rj < N && wi < stride) bitsT[rj * stride + wi] = l;
-        if (!diag) {   // mirrored tile is identically zero
-            if (rj < N && wi < stride) bits[rj * stride + wi] = 0;
-            if (bitsT && ri < N && wj < stride) bitsT[ri * stride + wj] = 0;
+            for (int pass = 0; pass < 8; pass++) {
+                const int r = (tid >> 3) + 32 * pass;
+                const int64_t ri = (int64_t)I * BT + r;
+                if (ri < N) {
+                    bits[ri * stride + wj] = (uint64_t)s_U[r][k * 8 + 2 * q] | ((uint64_t)s_U[r][k * 8 + 2 * q + 1] << 32);
+                    if (bitsT && J != I) bitsT[ri * stride + wj] = 0;
+                }
+            }
+        }
+    }
+    // Rows of the J tiles: 4 uint64 per row, 4 consecutive threads cover one 32-byte segment
+    {
+        const int q = tid & 3;
+        const int64_t wi = (int64_t)I * (BT / 64) + q;
+        if (wi < stride) {
+#pragma unroll
+            for (int pass = 0; pass < NJ * 4; pass++) {
+                const int r2 = (tid >> 2) + 64 * pass;          // 0 .. NJ*256-1
+                const int k = r2 / BT, r = r2 % BT;
+                const int J = JS * NJ + k;
+                const int64_t rj = (int64_t)J * BT + r;
+                if (J >= I && J < nT && rj < N) {
+                    if (bitsT) bitsT[rj * stride + wi] = (uint64_t)s_L[r2][2 * q] | ((uint64_t)s_L[r2][2 * q + 1] << 32);
+                    if (J != I) bits[rj * stride + wi] = 0;
+                }
+            }
         }
     }
 }
@@ -265,7 +353,7 @@ static int launch_build_t(const double *coords, int64_t B, int64_t N, int64_t st
                           uint64_t *bits, uint64_t *bitsT, cudaStream_t st)
 {
     const int nT = (int)((N + BT - 1) / BT);
-    dim3 grid(nT, nT, (unsigned)B);
+    dim3 grid((nT + NJ - 1) / NJ, nT, (unsigned)B);   // x: groups of NJ column tiles, y: row tile
     k_causal_matrix<GEOM, DIM><<<grid, BUILD_THREADS, 0, st>>>(coords, N, stride, bits, bitsT);
     CS_LAUNCHED("k_causal_matrix");
     const int64_t covered = (int64_t)nT * (BT / 64);
