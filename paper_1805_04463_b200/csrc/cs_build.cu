@@ -81,27 +81,47 @@ struct FastCone { static constexpr bool ok = false; };
 template <int DIM>
 struct FastCone<CS_GEOM_MINK_CONE, DIM> { static constexpr bool ok = true; };
 
-__device__ __forceinline__ double warp_max(double v)
+// order-preserving map float -> uint32 (NaN with the sign bit clear sorts above +inf, set below -inf)
+__device__ __forceinline__ uint32_t float_key(float f)
 {
-#pragma unroll
-    for (int s = 16; s >= 1; s >>= 1) v = fmax(v, __shfl_xor_sync(0xffffffffu, v, s));
-    return v;
+    const uint32_t u = __float_as_uint(f);
+    return u ^ ((uint32_t)((int32_t)u >> 31) | 0x80000000u);
+}
+__device__ __forceinline__ float key_float(uint32_t k)
+{
+    return __uint_as_float(k ^ ((k & 0x80000000u) ? 0x80000000u : 0xFFFFFFFFu));
 }
 
 // 32 x 32 bit block held one word per lane (lane = column, bit = row) -> one word per lane
-// (lane = row, bit = column): the 5-step butterfly
-__device__ __forceinline__ uint32_t transpose32(uint32_t x, int lane)
-{
-    const uint32_t mlo[5] = {0x0000FFFFu, 0x00FF00FFu, 0x0F0F0F0Fu, 0x33333333u, 0x55555555u};
+// (lane = row, bit = column): the 5-step butterfly.  Step t exchanges with lane ^ s (s = 16 >> t) and keeps
+// x & keep | rot(partner) & ~keep, where the partner word is shifted right by s in the lanes with bit s set
+// and left by s in the others; a rotation does both, the bits that wrap around land where ~keep is 0.
+// keep[t] and rot[t] depend on the lane only (TransposeLane, set up once per kernel).
+struct TransposeLane {
+    uint32_t keep[5], rot[5];
+    __device__ __forceinline__ explicit TransposeLane(int lane)
+    {
+        const uint32_t mlo[5] = {0x0000FFFFu, 0x00FF00FFu, 0x0F0F0F0Fu, 0x33333333u, 0x55555555u};
 #pragma unroll
-    for (int t = 0; t < 5; t++) {
-        const int s = 16 >> t;
-        const uint32_t o = __shfl_xor_sync(0xffffffffu, x, s);
-        if (lane & s) x = (x & ~mlo[t]) | ((o >> s) & mlo[t]);
-        else          x = (x & mlo[t]) | ((o << s) & ~mlo[t]);
+        for (int t = 0; t < 5; t++) {
+            const int s = 16 >> t;
+            keep[t] = (lane & s) ? ~mlo[t] : mlo[t];
+            rot[t] = (lane & s) ? 32 - s : s;           // rotate left by 32 - s = shift right by s
+        }
     }
-    return x;
-}
+    __device__ __forceinline__ uint32_t operator()(uint32_t x) const
+    {
+#pragma unroll
+        for (int t = 0; t < 5; t++) {
+            const uint32_t o = __shfl_xor_sync(0xffffffffu, x, 16 >> t);
+            const uint32_t r = __funnelshift_l(o, o, rot[t]);
+            x = (x & keep[t]) | (r & ~keep[t]);
+        }
+        return x;
+    }
+};
+
+__device__ __forceinline__ uint32_t transpose32(uint32_t x, int lane) { return TransposeLane(lane)(x); }
 
 constexpr int NJ = 2;            // future points per lane: a CTA covers 256 rows x 512 columns
 
@@ -168,13 +188,13 @@ k_causal_matrix(const double *__restrict__ coords, int64_t N, int64_t stride,
     __shared__ __align__(16) float s_hi[FAST ? BT : 4];    // h of the past points in fp32
     __shared__ __align__(16) uint32_t s_U[BT][NJ * 8 + 1]; // row i_local, 32-bit word = 32 columns j
     __shared__ uint32_t s_L[NJ * BT][9];                   // row j_local, 32-bit word = 32 rows i
-    double (*s_red)[NW] = reinterpret_cast<double (*)[NW]>(&s_U[0][0]);   // [2 + 2 NJ][NW], dead before s_U is written
-    static_assert((2 + 2 * NJ) * NW * sizeof(double) <= sizeof(uint32_t) * BT * (NJ * 8 + 1), "s_red fits in s_U");
+    uint32_t (*s_red)[NW] = reinterpret_cast<uint32_t (*)[NW]>(&s_U[0][0]);   // [2 + 2 NJ][NW], dead before s_U is written
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const double qnan = __longlong_as_double(0x7FF8000000000000LL);   // compares false: unrelated
     const int jl = warp * 32 + lane;
 
+    const TransposeLane transpose(lane);
     bool act[NJ], dg[NJ];
     bool any_diag = false;
 #pragma unroll
@@ -207,55 +227,60 @@ k_causal_matrix(const double *__restrict__ coords, int64_t N, int64_t stride,
 #pragma unroll
     for (int k = 0; k < NJ; k++) { fast[k] = false; hj[k] = 0.f; m[k] = 0.f; fj[k][0] = fj[k][1] = fj[k][2] = fj[k][3] = 0.f; }
     if (FAST) {
-        // tile summaries: largest |coordinate| of the past points and of each set of future points (fmax
-        // ignores NaN), max t_i, min t_j; inside the diagonal tile i < j must imply t_i <= t_j instead,
-        // i.e. the tile's own points are in time order
-        double ci = 0.0, si = 0.0;
+        // Tile summaries, all as floats reduced with redux.sync on order-preserving integer keys:
+        //   C   >= largest |coordinate| of the past points and of each set of future points (the fp32
+        //          conversions, NaN ignored by fmaxf; rounding to nearest is covered by m's 1.001),
+        //   max t_i rounded up and min t_j rounded down, so "max t_i <= min t_j" is only ever claimed when
+        //   it holds for the doubles (a NaN time makes the claim fail or is ignored; either is safe).
+        // Inside the diagonal tile i < j must imply t_i <= t_j instead: its points are in time order.
+        double si = 0.0;
+        float fi[4] = {0.f, 0.f, 0.f, 0.f}, ci = 0.f;
 #pragma unroll
         for (int d = 0; d < DIM; d++) {
-            ci = fmax(ci, fabs(xi0[d]));
+            fi[d] = (float)xi0[d];
+            ci = fmaxf(ci, fabsf(fi[d]));
             if (d > 0) si += xi0[d] * xi0[d];
         }
-        s_fi[tid] = make_float4((float)xi0[0], DIM > 1 ? (float)xi0[1 % DIM] : 0.f, DIM > 2 ? (float)xi0[2 % DIM] : 0.f,
-                                DIM > 3 ? (float)xi0[3 % DIM] : 0.f);
+        s_fi[tid] = make_float4(fi[0], fi[1], fi[2], fi[3]);
         s_hi[tid] = (float)(0.5 * (xi0[0] * xi0[0] - si));
-        const double wci = warp_max(ci), wti = warp_max(xi0[0]);
+        const uint32_t wci = __reduce_max_sync(0xffffffffu, __float_as_uint(ci));   // ci >= 0: bit order = value order
+        const uint32_t wti = __reduce_max_sync(0xffffffffu, float_key(__double2float_ru(xi0[0])));
         if (lane == 0) { s_red[0][warp] = wci; s_red[1][warp] = wti; }
 #pragma unroll
         for (int k = 0; k < NJ; k++) {
-            double cj = 0.0, sj = 0.0;
+            double sj = 0.0;
+            float cj = 0.f;
 #pragma unroll
             for (int d = 0; d < DIM; d++) {
-                cj = fmax(cj, fabs(xj[k][d]));
-                if (d > 0) sj += xj[k][d] * xj[k][d];
                 fj[k][d] = (float)xj[k][d];
+                cj = fmaxf(cj, fabsf(fj[k][d]));
+                if (d > 0) sj += xj[k][d] * xj[k][d];
             }
             hj[k] = (float)(0.5 * (xj[k][0] * xj[k][0] - sj));
-            const double wcj = warp_max(cj), wtj = warp_max(-xj[k][0]);
+            const uint32_t wcj = __reduce_max_sync(0xffffffffu, __float_as_uint(cj));
+            const uint32_t wtj = __reduce_max_sync(0xffffffffu, float_key(-__double2float_rd(xj[k][0])));   // -(min t_j)
             if (lane == 0) { s_red[2 + 2 * k][warp] = wcj; s_red[3 + 2 * k][warp] = wtj; }
         }
         __syncthreads();
-        double Ci = s_red[0][0], tmaxI = s_red[1][0], Cj[NJ], ntminJ[NJ];
+        uint32_t r[2 + 2 * NJ];
 #pragma unroll
-        for (int k = 0; k < NJ; k++) { Cj[k] = s_red[2 + 2 * k][0]; ntminJ[k] = s_red[3 + 2 * k][0]; }
+        for (int q = 0; q < 2 + 2 * NJ; q++) {
+            r[q] = s_red[q][0];
 #pragma unroll
-        for (int w = 1; w < NW; w++) {
-            Ci = fmax(Ci, s_red[0][w]);
-            tmaxI = fmax(tmaxI, s_red[1][w]);
-#pragma unroll
-            for (int k = 0; k < NJ; k++) { Cj[k] = fmax(Cj[k], s_red[2 + 2 * k][w]); ntminJ[k] = fmax(ntminJ[k], s_red[3 + 2 * k][w]); }
+            for (int w = 1; w < NW; w++) r[q] = max(r[q], s_red[q][w]);
         }
         bool tile_ordered = false;
         if (any_diag) {   // points beyond N are NaN and only ever sit at the end: their pairs read unrelated either way
             const bool last = tid == BT - 1 || (int64_t)I * BT + tid + 1 >= N;
             tile_ordered = __syncthreads_and(last || xi0[0] <= s_xi[0][last ? tid : tid + 1]) != 0;
         }
+        const float Ci = __uint_as_float(r[0]), tmaxI = key_float(r[1]);
 #pragma unroll
         for (int k = 0; k < NJ; k++) {
-            const double C = fmax(Ci, Cj[k]);
-            const bool ordered = dg[k] ? tile_ordered : (tmaxI <= -ntminJ[k]);
-            fast[k] = act[k] && ordered && (C >= 0x1p-40) && (C <= 0x1p40);
-            m[k] = __double2float_ru(C * C * (0x1p-18 * 1.001));
+            const float C = fmaxf(Ci, __uint_as_float(r[2 + 2 * k]));
+            const bool ordered = dg[k] ? tile_ordered : (tmaxI <= -key_float(r[3 + 2 * k]));
+            fast[k] = act[k] && ordered && (C >= 0x1p-40f) && (C <= 0x1p40f);
+            m[k] = __fmul_ru(__fmul_ru(C, C), 0x1p-18f * 1.001f);
         }
     }
     __syncthreads();    // s_xi / s_fi / s_hi visible; s_red (aliased on s_U) no longer read
@@ -292,7 +317,7 @@ k_causal_matrix(const double *__restrict__ coords, int64_t N, int64_t stride,
             }
             if (act[k]) {
                 s_L[k * BT + jl][sb] = lw[k];                                   // past of j: bit = row i
-                s_U[sb * 32 + lane][k * 8 + warp] = transpose32(lw[k], lane);   // future of i: bit = column j
+                s_U[sb * 32 + lane][k * 8 + warp] = transpose(lw[k]);   // future of i: bit = column j
             }
         }
     }
