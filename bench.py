@@ -181,14 +181,75 @@ def cpu_baseline(cfg, N, coords, W_alg, seconds):
                       (row_step, N, w, W_alg, timing["loop_seconds"], t_build)}
 
 
+def run_ensemble(args, cfg, rank, local_rank, world):
+    """Config 5: B independent causets per step through cs_bd_action_batched (one launch per stage).
+    Not the headline workload (BASELINE.json's metric is quoted on config 3); same line shape, metric
+    causets/s.  Every causet is distinct (own seed); 256 MiB of coordinates + 4 GiB of bit matrices per step,
+    all larger than L2."""
+    import torch
+    from paper_1805_04463_b200 import api, dist as csd, inputs as inp
+    torch.cuda.set_device(local_rank)
+    csd.init()
+    api.load()
+    B = args.B or cfg.batch
+    N = args.N or cfg.N
+    coords = np.ascontiguousarray(np.stack(
+        [inp.sprinkle(cfg.geometry, cfg.dim, N, cfg.seed * 4096 + b + 1000003 * rank) for b in range(B)]))
+    d_coords = torch.from_numpy(coords).cuda()
+    h_coords = torch.from_numpy(coords).pin_memory()
+    h_actions = torch.empty(B, dtype=torch.float64).pin_memory()
+    ws = torch.empty(api.bd_action_batched_workspace(B, N), dtype=torch.uint8, device="cuda")
+    for _ in range(args.warmup):
+        actions = api.bd_action_batched(d_coords, cfg.geometry, workspace=ws)
+    sampler = ClockSampler(local_rank); sampler.start()
+    csd.barrier(); torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    l0 = api.launch_count(); t0 = time.perf_counter()
+    e0.record()
+    for _ in range(args.steps):
+        actions = api.bd_action_batched(d_coords, cfg.geometry, workspace=ws)
+    e1.record(); torch.cuda.synchronize(); csd.barrier()
+    t1 = time.perf_counter()
+    launches = api.launch_count() - l0
+    clocks = sampler.stop(t0, t1)
+    units, secs, value = csd.aggregate(float(B) * args.steps, e0.elapsed_time(e1) / 1e3)
+    # e2e: coordinates from pinned host memory, actions back to the host, every step
+    d_in = torch.empty_like(d_coords)
+    for _ in range(2):
+        d_in.copy_(h_coords, non_blocking=True)
+        h_actions.copy_(api.bd_action_batched(d_in, cfg.geometry, workspace=ws), non_blocking=True)
+    csd.barrier(); torch.cuda.synchronize()
+    e0.record()
+    for _ in range(args.steps):
+        d_in.copy_(h_coords, non_blocking=True)
+        h_actions.copy_(api.bd_action_batched(d_in, cfg.geometry, workspace=ws), non_blocking=True)
+    e1.record(); torch.cuda.synchronize(); csd.barrier()
+    _, e2e_secs, e2e_value = csd.aggregate(float(B) * args.steps, e0.elapsed_time(e1) / 1e3)
+    assert np.array_equal(h_actions.numpy(), actions.cpu().numpy())
+    if rank == 0:
+        print(json.dumps({
+            "metric": "ensemble_causets_per_s", "value": value, "unit": "causets/s", "n_gpus": world,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * secs / args.steps,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "fp4_e2m1", "data": "synthetic",
+            "config": {"workload": cfg.name, "B": B, "N": N, "dim": cfg.dim, "geometry": cfg.geometry, "kmax": 3,
+                       "l2": "inputs larger than L2 (coords %.0f MiB, bit matrices %.0f MiB)" %
+                             (coords.nbytes / 2 ** 20, 2.0 * B * N * api.row_stride_words(N) * 8 / 2 ** 20),
+                       "parallelism": "replicas x%d" % world, "mean_action": float(actions.mean().item())},
+            "e2e": {"value": e2e_value, "unit": "causets/s", "h2d_bytes_per_step": int(coords.nbytes),
+                    "d2h_bytes_per_step": int(B * 8), "ms_per_step": 1e3 * e2e_secs / args.steps},
+            "gpu_launches": int(launches), "clocks": clocks, "roofline": None, "cpu_baseline": None}))
+    csd.shutdown()
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--config", type=int, default=3, help="BASELINE.json workload 1..4 (default 3: N=65536, 3+1)")
+    ap.add_argument("--config", type=int, default=3, help="BASELINE.json workload 1..5 (default 3: N=65536, 3+1, the headline; 5 = batched ensemble, causets/s)")
     ap.add_argument("--N", type=int, default=0, help="override N (debug only; the line then names it)")
+    ap.add_argument("--B", type=int, default=0, help="config 5 only: number of causets per step (default 4096)")
     ap.add_argument("--route", type=int, default=0, help="0 auto, 1 popc, 2 tensor int8, 3 tensor fp4, 4 tensor fp4 on CTA pairs")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=12.0)
@@ -207,6 +268,9 @@ def main():
     from paper_1805_04463_b200 import api
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device (there is no CPU fallback)")
+    if cfg.batch > 1:
+        run_ensemble(args, cfg, rank, local_rank, world)
+        return
     torch.cuda.set_device(local_rank)
     csd.init()
     api.load()

@@ -141,6 +141,23 @@ int cs_default_route(int64_t N);
 int cs_bd_action(const int64_t *hist, int64_t kmax, int64_t N, int dim,
                  double *action, int64_t *bracket, void *stream);
 
+/* Smeared (non-local) action S_eps, Eq. 4.13-4.15 with the smearing functions of Eq. 4.16-4.18
+ * (PAPER.md:1783-1795), l/l_p = 1, from the FULL interval histogram:
+ *   dim 2: S = 2 eps [ N - 2 eps sum_k hist[k] f_2(k, eps) ]
+ *   dim 3: S = (1/Gamma(5/3)) (pi eps/(3 sqrt 2))^(2/3) [ N - eps sum_k hist[k] f_3(k, eps) ]
+ *   dim 4: S = 4 sqrt(eps/6) [ N - eps sum_k hist[k] f_4(k, eps) ]
+ * (the paper's n_m f(m-1) with m = k+1).  f_d is evaluated in the polynomial form
+ * (1-eps)^k - c1 k eps (1-eps)^(k-1) + ..., which is also defined at eps = 1, where S_eps equals the
+ * local action of cs_bd_action.  The sum is carried in double-double arithmetic (it cancels to a small
+ * fraction of its terms) and rounded to fp64 once at the end.
+ *   hist    device, int64[kmax+1] (kmax clamped as in cs_interval_hist; entries beyond kmax count as 0,
+ *           so pass the whole histogram, kmax = N-2, for the paper's S_eps).
+ *   eps     0 < eps <= 1.
+ *   action  device, double[1], overwritten.
+ * Errors: CS_ERR_ARG (eps out of range, N > 131073), CS_ERR_DIM, CS_ERR_CUDA. */
+int cs_smeared_action(const int64_t *hist, int64_t kmax, int64_t N, int dim, double eps,
+                      double *action, void *stream);
+
 /* Batched ensemble (Monte-Carlo use): B independent causets of N points each,
  * one action per causet.
  *   coords   device, [B][N][dim] fp64, each causet sorted by time.

@@ -331,7 +331,7 @@ static long double orc_powl_nonneg(long double b, int64_t e)
     return powl(b, (long double)e);
 }
 
-double orc_smear_f(int dim, int64_t m, double eps)
+static long double orc_smear_fl(int dim, int64_t m, double eps)
 {
     long double e = eps, q = 1.0L - e, M = (long double)m;
     long double f = orc_powl_nonneg(q, m);
@@ -346,10 +346,12 @@ double orc_smear_f(int dim, int64_t m, double eps)
         if (m >= 2) f += 8.0L * M * (M - 1) * e * e * orc_powl_nonneg(q, m - 2);
         if (m >= 3) f -= (4.0L / 3.0L) * M * (M - 1) * (M - 2) * e * e * e * orc_powl_nonneg(q, m - 3);
     } else {
-        return NAN;
+        return (long double)NAN;
     }
-    return (double)f;
+    return f;
 }
+
+double orc_smear_f(int dim, int64_t m, double eps) { return (double)orc_smear_fl(dim, m, eps); }
 
 /* Smeared action, Eq. 4.13-4.15; sum over m = 1..N-1 of
  * n_m f_d(m-1, eps) = sum_k hist[k] f_d(k, eps); long double accumulation. */
@@ -357,7 +359,7 @@ double orc_smeared_action(const int64_t *hist, int64_t nhist, int64_t N, int dim
 {
     long double sum = 0.0L;
     for (int64_t k = 0; k < nhist; k++)
-        if (hist[k]) sum += (long double)hist[k] * (long double)orc_smear_f(dim, k, eps);
+        if (hist[k]) sum += (long double)hist[k] * orc_smear_fl(dim, k, eps);   /* f_d kept in long double */
     long double e = eps;
     if (dim == 2) return (double)(2.0L * e * ((long double)N - 2.0L * e * sum));
     if (dim == 3) {

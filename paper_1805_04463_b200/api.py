@@ -51,6 +51,7 @@ _SIGNATURES = {
     "cs_interval_hist_batched": (_int, [_p, _p, _i64, _i64, _i64, _int, _p, _p, _sz, _p]),
     "cs_default_route": (_int, [_i64]),
     "cs_bd_action": (_int, [_p, _i64, _i64, _int, _p, _p, _p]),
+    "cs_smeared_action": (_int, [_p, _i64, _i64, _int, ctypes.c_double, _p, _p]),
     "cs_bd_action_batched_workspace": (_sz, [_i64, _i64]),
     "cs_bd_action_batched": (_int, [_p, _i64, _i64, _int, _int, _p, _p, _p, _sz, _p]),
     "cs_action_host_workspace": (_sz, [_i64, _i64]),
@@ -209,6 +210,15 @@ def bd_action(hist: torch.Tensor, N: int, dim: int, return_bracket: bool = False
     _check(load().cs_bd_action(_dptr(hist), hist.numel() - 1, N, dim, _dptr(action), _dptr(bracket), _stream()),
            "cs_bd_action")
     return (action, bracket) if return_bracket else action
+
+
+def smeared_action(hist: torch.Tensor, N: int, dim: int, eps: float) -> torch.Tensor:
+    """Smeared action S_eps (Eq. 4.13-4.18) from the full histogram -> fp64[1] CUDA tensor."""
+    _need_cuda(hist, torch.int64, "hist")
+    action = torch.empty(1, dtype=torch.float64, device=hist.device)
+    _check(load().cs_smeared_action(_dptr(hist), hist.numel() - 1, N, dim, float(eps), _dptr(action), _stream()),
+           "cs_smeared_action")
+    return action
 
 
 def bd_action_batched_workspace(B: int, N: int) -> int:

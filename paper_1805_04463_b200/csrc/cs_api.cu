@@ -200,6 +200,14 @@ int cs_bd_action(const int64_t *hist, int64_t kmax, int64_t N, int dim,
                             static_cast<cudaStream_t>(stream));
 }
 
+int cs_smeared_action(const int64_t *hist, int64_t kmax, int64_t N, int dim, double eps,
+                      double *action, void *stream)
+{
+    if (!hist || !action || N < 0) return CS_ERR_ARG;
+    kmax = clamp_kmax(N, kmax);
+    return launch_smeared_action(hist, kmax + 1, 1, kmax, N, dim, eps, action, static_cast<cudaStream_t>(stream));
+}
+
 // ---- batched ensemble ----------------------------------------------------------------------
 // workspace: [bits B*N*stride][bitsT B*N*stride][hist B*4 int64][interval scratch]
 size_t cs_bd_action_batched_workspace(int64_t B, int64_t N)

@@ -77,4 +77,7 @@ bool interval_tensor_available();
 int launch_bd_action(const int64_t *hist, int64_t hist_stride, int64_t B, int64_t kmax, int64_t N, int dim,
                      double *action, int64_t *bracket, int64_t *hist4, cudaStream_t st);
 
+int launch_smeared_action(const int64_t *hist, int64_t hist_stride, int64_t B, int64_t kmax, int64_t N, int dim,
+                          double eps, double *action, cudaStream_t st);
+
 }  // namespace cs

@@ -310,3 +310,78 @@ def test_config5_full_size(api, oracle):
         _, o_hist, o_S, _ = oracle.action_pipeline(coords[b], cfg.geometry, tier=1)
         assert np.array_equal(hist4[b], o_hist[:4]), "causet %d" % b
         assert actions[b] == o_S, "causet %d" % b
+
+
+# ----------------------------------------------------------------------------- NEXT-1: smeared action
+_SMEAR_C = {2: (2.0, 0.5, 0.0, 2.0), 3: (27.0 / 8, 9.0 / 8, 0.0, 1.0), 4: (9.0, 8.0, 4.0 / 3, 1.0)}
+
+
+def _smear_prefactor(dim, eps):
+    import math
+    if dim == 2:
+        return 2.0 * eps
+    if dim == 3:
+        return (1.0 / math.gamma(5.0 / 3.0)) * (math.pi * eps / (3.0 * math.sqrt(2.0))) ** (2.0 / 3.0)
+    return 4.0 * math.sqrt(eps / 6.0)
+
+
+def _smear_tolerance(hist, dim, eps, S):
+    """Bound on |CUDA - oracle| derived from the arithmetic: the CUDA sum is carried
+    in double-double (~2^-100) and rounded once (2^-53 |S|, plus the fp64 prefactor: 2^-51 |S| in all); the
+    oracle works in x87 long double, u = 2^-64: q = 1 - eps is rounded once, so q^(k-j) is off by <= (k+1) u, and
+    each of the <= 4 sub-terms of f_d and their sums round with u -- in all <= (k+8) u A(k), with A(k) the sum of
+    the absolute values of the sub-terms of f_d(k, eps)."""
+    c1, c2, c3, a = _SMEAR_C[dim]
+    k = np.arange(hist.shape[0], dtype=np.float64)
+    q = 1.0 - eps
+
+    def qp(j):                      # q^(k-j), 0 where the falling factorial vanishes
+        return np.where(k >= j, np.power(q, np.maximum(k - j, 0.0)), 0.0)
+    A = qp(0) + c1 * k * eps * qp(1) + c2 * k * (k - 1) * eps ** 2 * qp(2) + c3 * k * (k - 1) * (k - 2) * eps ** 3 * qp(3)
+    bound = float((hist.astype(np.float64) * A * (k + 8.0)).sum()) * 2.0 ** -63
+    return _smear_prefactor(dim, eps) * a * eps * bound + 2.0 ** -51 * abs(S)
+
+
+@pytest.mark.parametrize("cfg_id,N,dim", [(2, 1500, 2), (3, 2048, 4), (4, 2000, 2), (3, 1200, 3)])
+def test_smeared_action_vs_oracle(api, oracle, cfg_id, N, dim):
+    cfg = inp.CONFIGS[cfg_id]
+    coords = inp.sprinkle(cfg.geometry, dim, N, 77 + N)
+    _, o_hist, _, _ = oracle.action_pipeline(coords, cfg.geometry, tier=1)
+    d_hist = torch.from_numpy(o_hist).cuda()
+    for eps in (1.0, 0.5, 0.25, 0.1, 2.0 ** -6, 0.013):
+        o_S = oracle.smeared_action(o_hist, N, dim, eps)
+        S = float(api.smeared_action(d_hist, N, dim, eps)[0])
+        assert abs(S - o_S) <= _smear_tolerance(o_hist, dim, eps, o_S), (eps, S, o_S)
+    # eps = 1 is the local action (Eq. 4.16-4.18 reduce to the coefficients of Eq. 4.10-4.12)
+    S1 = float(api.smeared_action(d_hist, N, dim, 1.0)[0])
+    S_local = float(api.bd_action(d_hist, N, dim)[0])
+    assert S1 == pytest.approx(S_local, rel=4e-16, abs=0.0)
+    # on the device pipeline's own histogram too
+    bits, bitsT = gpu_bits(api, coords, cfg.geometry)
+    h = api.interval_hist(bits, bitsT, N)
+    assert float(api.smeared_action(h, N, dim, 2.0 ** -6)[0]) == float(api.smeared_action(d_hist, N, dim, 2.0 ** -6)[0])
+
+
+@pytest.mark.parametrize("dim", [2, 3, 4])
+def test_smeared_action_long_histogram(api, oracle, dim):
+    """Every bin up to k = N - 2 at the largest N the entry point takes, large counts, small eps: the terms
+    reach ~1e21 while they cancel; still inside the derived bound."""
+    N = 131072
+    rng = np.random.default_rng(dim)
+    k = np.arange(N - 1)
+    hist = (rng.integers(1, 1 << 40, N - 1) * np.exp(-k / 30000.0)).astype(np.int64)
+    d_hist = torch.from_numpy(hist).cuda()
+    for eps in (2.0 ** -10, 2.0 ** -6, 0.37):
+        o_S = oracle.smeared_action(hist, N, dim, eps)
+        S = float(api.smeared_action(d_hist, N, dim, eps)[0])
+        assert abs(S - o_S) <= _smear_tolerance(hist, dim, eps, o_S), (eps, S, o_S)
+
+
+def test_smeared_action_arguments(api):
+    h = torch.zeros(10, dtype=torch.int64, device="cuda")
+    for bad in (0.0, -0.5, 1.5, float("nan")):
+        with pytest.raises(RuntimeError):
+            api.smeared_action(h, 11, 2, bad)
+    with pytest.raises(RuntimeError):
+        api.smeared_action(h, 11, 5, 0.5)
+    assert float(api.smeared_action(h, 11, 4, 0.5)[0]) == 4.0 * (0.5 / 6.0) ** 0.5 * 11

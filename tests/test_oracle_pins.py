@@ -383,6 +383,34 @@ def test_smear_f_against_paper_form(oracle):
                 assert oracle.smear_f(dim, m, float(eps)) == pytest.approx(float(f), rel=1e-12, abs=1e-15)
 
 
+def test_smeared_action_against_exact_rational(oracle):
+    """Eq. 4.13-4.15 with Eq. 4.16-4.18 exactly as printed, in rational arithmetic, on a real histogram
+    (the bracket cancels to ~1e-3 of its terms here): pins the oracle's long-double sum, index shift
+    n_m f(m-1) and prefactors.  Irrational prefactors are applied in floating point at the end."""
+    N = 400
+    coords = inp.sprinkle(inp.GEOM_DS2_SLAB, 2, N, 5)
+    hist, _, _ = oracle.interval_hist_alg20(oracle.causal_matrix_bits(coords, inp.GEOM_DS2_SLAB), N)
+    for eps in (Fraction(1, 64), Fraction(1, 5), Fraction(3, 4)):
+        q = 1 - eps
+        sums = {2: Fraction(0), 3: Fraction(0), 4: Fraction(0)}
+        for mm in range(1, N):                                   # the paper's m = 1 .. N-1, n_m = hist[m-1]
+            n_m = int(hist[mm - 1]) if mm - 1 < hist.shape[0] else 0
+            if n_m == 0:
+                continue
+            m = mm - 1
+            sums[2] += n_m * q ** m * (1 - 2 * m * eps / q + Fraction(m * (m - 1), 2) * eps ** 2 / q ** 2)
+            sums[3] += n_m * q ** m * (1 - Fraction(27, 8) * m * eps / q + Fraction(9, 8) * m * (m - 1) * eps ** 2 / q ** 2)
+            sums[4] += n_m * q ** m * (1 - 9 * m * eps / q + 8 * m * (m - 1) * eps ** 2 / q ** 2
+                                       - Fraction(4, 3) * m * (m - 1) * (m - 2) * eps ** 3 / q ** 3)
+        e = float(eps)
+        want = {2: float(2 * eps * (N - 2 * eps * sums[2])),
+                3: (1 / math.gamma(5 / 3)) * (math.pi * e / (3 * math.sqrt(2))) ** (2 / 3) * float(N - eps * sums[3]),
+                4: 4 * math.sqrt(e / 6) * float(N - eps * sums[4])}
+        for dim in (2, 3, 4):
+            got = oracle.smeared_action(hist, N, dim, e)
+            assert got == pytest.approx(want[dim], rel=1e-11, abs=1e-9), (dim, eps)
+
+
 def test_seh_golden():
     eta0, printed, _ = _read_table("ds_slab_seh.txt")[0]
     assert round(4 * math.pi * math.tan(float(eta0)), 3) == float(printed)
