@@ -252,6 +252,23 @@ def test_batched_ensemble(api, oracle):
         assert actions[b] == oracle.action_pipeline(coords[b], cfg.geometry)[2]
 
 
+def test_interval_hist_batched_routes(api, oracle):
+    """cs_interval_hist_batched: every route, full and truncated histograms, causets of a ragged size."""
+    cfg = inp.CONFIGS[5]
+    for B, N in ((5, 1300), (3, 2048)):
+        coords = inp.make_ensemble_coords(cfg, B=B, N=N)
+        bits, bitsT = api.causal_matrix_batched(torch.from_numpy(coords).cuda(), cfg.geometry)
+        want = [oracle.action_pipeline(coords[b], cfg.geometry, tier=1)[1] for b in range(B)]
+        for r in routes(api) + [api.ROUTE_AUTO]:
+            full = api.interval_hist_batched(bits, bitsT, N, route=r).cpu().numpy()
+            k3 = api.interval_hist_batched(bits, bitsT, N, kmax=3, route=r).cpu().numpy()
+            k100 = api.interval_hist_batched(bits, bitsT, N, kmax=100, route=r).cpu().numpy()
+            for b in range(B):
+                assert np.array_equal(full[b], want[b]), (r, b)
+                assert np.array_equal(k3[b], want[b][:4]), (r, b)
+                assert np.array_equal(k100[b], want[b][:101]), (r, b)
+
+
 # ----------------------------------------------------------------------------- full sizes
 def _full_size_check(api, oracle, cfg, full_hist):
     """Bits compared in full; histogram compared in full (tier-1) or on sampled row ranges plus
@@ -385,3 +402,28 @@ def test_smeared_action_arguments(api):
     with pytest.raises(RuntimeError):
         api.smeared_action(h, 11, 5, 0.5)
     assert float(api.smeared_action(h, 11, 4, 0.5)[0]) == 4.0 * (0.5 / 6.0) ** 0.5 * 11
+
+
+@pytest.mark.slow
+def test_smeared_action_tends_to_einstein_hilbert(api):
+    """The paper's convergence experiment (Eq. 4.20, Fig. 4.5 right): 1+1 de Sitter slab,
+    symmetric cutoff eta0 = 0.5, eps = 2^-6, ten sprinklings; the mean smeared action 'begins to converge' to
+    S_EH = 4 pi tan(eta0) = 6.865 around N >= 2^14 while single terms of the series are orders of magnitude
+    larger, and sigma_S grows like sqrt(N).  Statistical, but deterministic: the seeds are fixed.  The whole
+    pipeline (a1, a2, smeared a3) runs on the device."""
+    import math
+    target = 4.0 * math.pi * math.tan(0.5)
+    sds = {}
+    for N in (1 << 14, 1 << 15):
+        vals = []
+        for seed in range(10):
+            c = inp.sprinkle_ds2_slab(N, 9000 + seed, -0.5, 0.5)
+            bits, bitsT = api.causal_matrix(torch.from_numpy(c).cuda(), inp.GEOM_DS2_SLAB)
+            h = api.interval_hist(bits, bitsT, N)
+            vals.append(float(api.smeared_action(h, N, 2, 2.0 ** -6)[0]))
+            assert int(h[:3].sum()) > 1000 * abs(vals[-1])           # the series' terms dwarf the result
+        mean, sd = float(np.mean(vals)), float(np.std(vals, ddof=1))
+        sds[N] = sd
+        assert abs(mean - target) < 3.5 * sd / math.sqrt(10), (N, mean, sd)
+        assert mean > 0.5 * target                                    # N = 2^12 gives 0.4 +- 0.3: not yet converged
+    assert 0.8 < sds[1 << 15] / sds[1 << 14] < 2.5                    # ~ sqrt(2), ten samples each
