@@ -30,21 +30,38 @@ namespace cs {
 namespace {
 
 constexpr int TM = 128;                 // A rows (i) per CTA; the pair covers 256
-constexpr int TNH = 128;                // B rows (j) per CTA; the pair covers 256
-constexpr int TILE = 256;               // tile edge of the pair
+constexpr int TILE = 256;               // rows (i) of a tile: 128 per CTA of the pair
 constexpr int KSTEP = 256;              // k per stage = 4 MMAs of K = 64
 constexpr int NS = 6;                   // operand stages (B in shared memory, A in TMEM)
 constexpr int GK = 2;                   // stages per staged group of bit rows
 constexpr int BROW = GK * 32;           // bytes per staged bit row (TMA box inner extent, 64B swizzle)
 constexpr int NB = 4;                   // bit-row buffers
-constexpr int BITS_BYTES = (TM + TNH) * BROW;       // 16 KiB
-constexpr int STAGE_BYTES = TNH * (KSTEP / 2);      // 16 KiB: this CTA's half of B
+// Tile width TN (columns j of a tile): 256, one accumulator, or 128, two accumulators that ping-pong
+// so that the epilogue drains one (TMEM reads run at 64 B/clk: 2048 clk for 128 lanes x 256 columns)
+// while the MMAs of the next tile fill the other.  TN = 128 expands every A stage for half the MMA work,
+// which only pays when tiles are short (small N, batched ensembles).
+template <int TN>
+struct Shape {
+    static constexpr int TNH = TN / 2;                          // B rows (j) per CTA
+    static constexpr int NACC = 256 / TN;                       // accumulators of TN columns
+    static constexpr int CW = TN / 2;                           // columns drained per epilogue warp
+    static constexpr int BITS_BYTES = (TM + TNH) * BROW;        // staged bit rows per buffer
+    static constexpr int STAGE_BYTES = TNH * (KSTEP / 2);       // this CTA's half of B, one stage
+    static constexpr int SMEM_FIXED = NS * STAGE_BYTES + NB * BITS_BYTES + 512;      // + 4 bytes per histogram bin
+    // block-scaled instruction descriptor, kind::mxf4: A = B = E2M1 (1 at bits 7 and 10), both K-major,
+    // N >> 3 at bit 17, scale format UE8M0 (bit 23), M >> 4 at bit 24 (M = 256 over the pair), K = 64
+    static constexpr uint32_t IDESC =
+        (1u << 7) | (1u << 10) | ((uint32_t)(TN >> 3) << 17) | (1u << 23) | ((uint32_t)(256 >> 4) << 24);
+};
 #ifndef CS_PAIR_HS_MAX
 #define CS_PAIR_HS_MAX 16896
 #endif
 constexpr int HS_MAX = CS_PAIR_HS_MAX;   // shared-memory histogram bins that fit beside the operand rings
 constexpr int HS_BATCHED = 2048;        // bins when several causets share a CTA (flushed at every switch)
-constexpr int BANDW = 8;                // diagonals per band of the tile order
+constexpr int BANDW = 8;                // diagonals (in 256-column units) per band of the tile order
+#ifndef CS_PAIR_TN128_MAX_N
+#define CS_PAIR_TN128_MAX_N 4096        // largest N that runs on 128-column tiles (two accumulators)
+#endif
 #ifndef CS_PAIR_DIAG
 #define CS_PAIR_DIAG 0      // timing experiments only (results are wrong): 1 no B stores, 2 no A stores, 4 no tally
 #endif
@@ -56,12 +73,7 @@ constexpr int BANDW = 8;                // diagonals per band of the tile order
 // row slice (128 columns) in registers, so registers are re-split by warpgroup with setmaxnreg.
 constexpr int EPI_WARPS = 8, EXPA_WARP0 = 8, EXPB_WARP0 = 12, EXP_WARPS = 8, MMA_WARP = 16, LOAD_WARP = 17;
 constexpr int THREADS = 20 * 32;
-constexpr int SMEM_FIXED = NS * STAGE_BYTES + NB * BITS_BYTES + 512;      // + 4 bytes per histogram bin
-constexpr int SMEM_BYTES = SMEM_FIXED + HS_MAX * 4;
-
-// block-scaled instruction descriptor, kind::mxf4: A = B = E2M1 (1 at bits 7 and 10), both K-major,
-// N >> 3 at bit 17, scale format UE8M0 (bit 23), M >> 4 at bit 24 (M = 256 over the pair), K = 64
-constexpr uint32_t IDESC = (1u << 7) | (1u << 10) | ((uint32_t)(256 >> 3) << 17) | (1u << 23) | ((uint32_t)(256 >> 4) << 24);
+constexpr int SMEM_BYTES = Shape<256>::SMEM_FIXED + HS_MAX * 4;
 constexpr uint32_t SF_COL = 256;        // three 16-column regions of constant scale factors: 2^1, 2^0, 2^-1
 constexpr uint32_t A_COL = 320;         // TMEM ring of the A operand: NS x 32 columns
 static_assert(A_COL + NS * 32 <= 512, "TMEM columns");
@@ -136,6 +148,19 @@ __device__ __forceinline__ void cluster_sync()
 {
     asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory");
     asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
+// one lane of the (converged) warp; the same lane every time
+__device__ __forceinline__ bool elect_one()
+{
+    uint32_t p;
+    asm volatile(
+        "{\n"
+        ".reg .pred q;\n"
+        "elect.sync _|q, 0xffffffff;\n"
+        "selp.u32 %0, 1, 0, q;\n"
+        "}\n"
+        : "=r"(p));
+    return p != 0;
 }
 __device__ __forceinline__ uint32_t cluster_ctarank()
 {
@@ -238,72 +263,87 @@ __device__ __forceinline__ uint32_t nib(uint32_t x)
 __device__ __forceinline__ uint32_t sf_col(int q) { return SF_COL + (q == 1 ? 16u : q == 2 ? 32u : 0u); }
 
 // ---- tile order ---------------------------------------------------------------------------------
-// Tiles (I, J = I + d), 0 <= I, I + d < nT, in bands of BANDW diagonals, longest (largest d) first;
-// inside a band I-major, then d ascending.  Entry = (I << 16) | J.  nT (nT + 1) / 2 entries.
-__host__ __device__ inline int64_t band_tiles(int nT, int dlo, int dhi)   // sum over d of (nT - d)
+// Row tile I (256 rows) meets column tiles Jc (TN columns) with Jc >= R I, R = 256 / TN; d = Jc - R I
+// measures the K length.  Tiles are listed in bands of BANDW R values of d, longest first; inside a
+// band I-major, then d ascending.  Entry = (I << 16) | Jc.
+__host__ __device__ inline int64_t row_tiles_in_band(int nTc, int R, int I, int dlo, int dhi)
 {
-    const int64_t w = dhi - dlo + 1;
-    return w * nT - w * (int64_t)(dlo + dhi) / 2;
+    const int dmax = nTc - R * I - 1;             // largest d of row I
+    if (dmax < dlo) return 0;
+    return (dmax < dhi ? dmax : dhi) - dlo + 1;
+}
+inline int64_t pair_tiles_per_causet(int64_t N, int TN)
+{
+    const int64_t nT = (N + TILE - 1) / TILE, nTc = (N + TN - 1) / TN, R = TILE / TN;
+    int64_t n = 0;
+    for (int64_t I = 0; I < nT; I++) n += nTc - R * I > 0 ? nTc - R * I : 0;
+    return n;
 }
 
-__global__ void k_pair_tile_order(int nT, uint32_t *__restrict__ tab)
+__global__ void k_pair_tile_order(int nT, int nTc, int R, uint32_t *__restrict__ tab)
 {
+    __shared__ unsigned long long s_off;
+    const int bw = BANDW * R;
     const int b = blockIdx.x;
-    const int dhi = nT - 1 - b * BANDW;
-    const int dlo = dhi - BANDW + 1 > 0 ? dhi - BANDW + 1 : 0;
-    const int w = dhi - dlo + 1;
-    int64_t off = 0;
-    for (int bb = 0; bb < b; bb++) {
-        const int h = nT - 1 - bb * BANDW;
-        const int l = h - BANDW + 1 > 0 ? h - BANDW + 1 : 0;
-        off += band_tiles(nT, l, h);
+    const int dhi = nTc - 1 - b * bw;
+    const int dlo = dhi - bw + 1 > 0 ? dhi - bw + 1 : 0;
+    if (threadIdx.x == 0) s_off = 0;
+    __syncthreads();
+    // tiles of all earlier bands: thread bb sums band bb over the rows
+    unsigned long long part = 0;
+    for (int bb = threadIdx.x; bb < b; bb += blockDim.x) {
+        const int h = nTc - 1 - bb * bw;
+        const int l = h - bw + 1 > 0 ? h - bw + 1 : 0;
+        for (int I = 0; I < nT; I++) part += (unsigned long long)row_tiles_in_band(nTc, R, I, l, h);
     }
-    const int full = nT - dhi;   // rows I < full have all w diagonals inside the matrix
-    for (int I = threadIdx.x; I + dlo < nT; I += blockDim.x) {
-        int64_t pos;
-        if (I <= full) pos = (int64_t)I * w;
-        else {
-            const int64_t m = I - full;   // rows full .. I-1 hold nT - dlo - I' entries each
-            pos = (int64_t)full * w + m * (nT - dlo) - (int64_t)(full + I - 1) * m / 2;
-        }
-        for (int d = dlo; d <= dhi && I + d < nT; d++) tab[off + pos + (d - dlo)] = ((uint32_t)I << 16) | (uint32_t)(I + d);
+    if (part) atomicAdd(&s_off, part);
+    __syncthreads();
+    const int64_t off = (int64_t)s_off;
+    for (int I = threadIdx.x; I < nT; I += blockDim.x) {
+        const int64_t cnt = row_tiles_in_band(nTc, R, I, dlo, dhi);
+        if (cnt == 0) continue;
+        int64_t pos = 0;
+        for (int Ip = 0; Ip < I; Ip++) pos += row_tiles_in_band(nTc, R, Ip, dlo, dhi);
+        for (int64_t d = 0; d < cnt; d++) tab[off + pos + d] = ((uint32_t)I << 16) | (uint32_t)(R * I + dlo + d);
     }
 }
 
 struct Tile {
-    int I, J;      // 256-row blocks of i and of j
+    int I, J;      // 256-row block of i, TN-column block of j
+    int nstages;   // 256-k stages from the first row of I to the last column of J
     int b;         // causet
     bool skip;     // no row of the tile inside [row_begin, row_end)
 };
 
 // SMALL: kmax <= 3 (the Monte-Carlo case, only N_0..N_3 enter Eq. 4.10-4.12): the tally keeps packed
 // counters in registers and never touches the shared histogram (hs = 0).
-template <bool SMALL>
+template <bool SMALL, int TN>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(THREADS, 1)
 k_interval_pair(const __grid_constant__ CUtensorMap mapU, const __grid_constant__ CUtensorMap mapL,
-                const uint64_t *__restrict__ bits, const uint32_t *__restrict__ tile_tab,
+                const uint64_t *__restrict__ bits, const uint32_t *__restrict__ tile_tab, uint32_t tiles_per,
                 int64_t B, int64_t N, int64_t stride, int64_t kmax, int hs,
                 int64_t row_begin, int64_t row_end,
                 unsigned long long *__restrict__ hist, unsigned long long *__restrict__ nrel)
 {
     extern __shared__ __align__(1024) unsigned char smem[];
     unsigned char *s_stage = smem;
+    using SH = Shape<TN>;
+    constexpr int TNH = SH::TNH, NACC = SH::NACC, CW = SH::CW;
+    constexpr int BITS_BYTES = SH::BITS_BYTES, STAGE_BYTES = SH::STAGE_BYTES, SMEM_FIXED = SH::SMEM_FIXED;
     unsigned char *s_bits = smem + NS * STAGE_BYTES;
     uint64_t *s_full = reinterpret_cast<uint64_t *>(smem + NS * STAGE_BYTES + NB * BITS_BYTES);
     uint64_t *s_empty = s_full + NS;      // [NS] stage free again (multicast commit from CTA 0)
-    uint64_t *s_tfull = s_empty + NS;     // [1] accumulator complete (multicast commit)
-    uint64_t *s_tempty = s_tfull + 1;     // [1] accumulator drained (used in CTA 0 only)
-    uint64_t *s_bfull = s_tempty + 1;     // [NB] staged bit rows have landed
+    uint64_t *s_tfull = s_empty + NS;     // [2] accumulator complete (multicast commit)
+    uint64_t *s_tempty = s_tfull + 2;     // [2] accumulator drained (used in CTA 0 only)
+    uint64_t *s_bfull = s_tempty + 2;     // [NB] staged bit rows have landed
     uint64_t *s_bempty = s_bfull + NB;    // [NB] every expander warp is done with the buffer
     uint32_t *s_tmem = reinterpret_cast<uint32_t *>(s_bempty + NB);
     uint32_t *s_hist = reinterpret_cast<uint32_t *>(smem + SMEM_FIXED);   // [hs], sized by the launcher
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const uint32_t rank = cluster_ctarank();
-    const int nT = (int)((N + TILE - 1) / TILE);
     // 32-bit schedule state (the launcher rejects more than 2^31 tiles): the expander and issuer
     // warps run on 64 and 40 registers
-    const uint32_t tiles_per = (uint32_t)nT * (uint32_t)(nT + 1) / 2;
     const uint32_t total_tiles = tiles_per * (uint32_t)B;
     const uint32_t t0 = cluster_id_x(), tstep = num_clusters_x();
     const int ib0 = (int)(row_begin / TILE), ib1 = (int)((row_end + TILE - 1) / TILE);   // I blocks inside the row range
@@ -315,6 +355,7 @@ k_interval_pair(const __grid_constant__ CUtensorMap mapU, const __grid_constant_
         const uint32_t e = __ldg(tile_tab + (t - (uint32_t)tc.b * tiles_per));
         tc.I = (int)(e >> 16);
         tc.J = (int)(e & 0xFFFFu);
+        tc.nstages = ((tc.J + 1) * TN - tc.I * TILE + KSTEP - 1) / KSTEP;
         tc.skip = tc.I < ib0 || tc.I >= ib1;
         return tc;
     };
@@ -328,8 +369,10 @@ k_interval_pair(const __grid_constant__ CUtensorMap mapU, const __grid_constant_
             mbar_init(&s_bfull[b], 1);
             mbar_init(&s_bempty[b], EXP_WARPS);
         }
-        mbar_init(s_tfull, 1);
-        mbar_init(s_tempty, 2 * EPI_WARPS);         // epilogue warps of both CTAs (counted in CTA 0)
+        for (int a = 0; a < 2; a++) {
+            mbar_init(&s_tfull[a], 1);
+            mbar_init(&s_tempty[a], 2 * EPI_WARPS);     // epilogue warps of both CTAs (counted in CTA 0)
+        }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     for (int b = tid; b < hs; b += THREADS) s_hist[b] = 0;
@@ -362,8 +405,12 @@ k_interval_pair(const __grid_constant__ CUtensorMap mapU, const __grid_constant_
         // ===================================== expanders =====================================
         // warpgroup 2 owns this CTA's 128 A rows (row = TMEM lane: warp w may only touch lanes
         // 32 (w % 4) ..), warpgroup 3 its 128 B rows.  One thread per row.
+        // With TN = 128 a CTA has only 64 B rows: two threads share a row, thread half h expanding the
+        // 16-byte chunks h (first stage of a group) and 2 + h (second stage).
         const bool isA = warp < EXPB_WARP0;
-        const int r = (warp & 3) * 32 + lane;
+        const int r128 = (warp & 3) * 32 + lane;
+        const int r = isA ? r128 : (r128 & (TNH - 1));
+        const int bhalf = r128 / TNH;                     // 0 unless TNH = 64
         // TMA 64B swizzle: 16-byte chunk c of row e sits at chunk c ^ ((e >> 1) & 3)
         const unsigned char *my_bits = s_bits + (isA ? 0 : TM * BROW) + r * BROW;
         const int swz = (r >> 1) & 3;
@@ -385,6 +432,24 @@ k_interval_pair(const __grid_constant__ CUtensorMap mapU, const __grid_constant_
         const uint32_t a_taddr = tmem_base + ((uint32_t)((warp & 3) * 32) << 16) + A_COL;
         unsigned char *b_dst = s_stage + r * 16;
 
+        // A stage is published (arrival on its full barrier) only after its stores have landed: TMEM
+        // stores need tcgen05.wait::st, shared-memory stores a generic->async proxy fence.  Both waits are
+        // deferred until the NEXT stage's bits have been loaded and expanded, so that the store latency
+        // overlaps that work instead of sitting on the one-stage-at-a-time critical path of the warp.
+        bool pend = false;
+        uint32_t pend_s = 0;
+        auto publish = [&]() {
+            if (!pend) return;
+            if (isA) {
+                asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
+                tc_fence_before();
+            } else if (!(CS_PAIR_DIAG & 16)) {
+                fence_proxy_async();   // generic-proxy stores -> visible to the tensor cores
+            }
+            __syncwarp();
+            if (lane == 0) mbar_arrive_cluster(&s_full[pend_s], 0);    // one arrival per warp, in CTA 0
+            pend = false;
+        };
         auto stage_A = [&](const uint4 &c0, const uint4 &c1) {
             const uint32_t xs[8] = {c0.x, c0.y, c0.z, c0.w, c1.x, c1.y, c1.z, c1.w};
             // TMEM column 8 q + j of stage s = nibble position q of slice j; two 16-column stores
@@ -394,6 +459,7 @@ k_interval_pair(const __grid_constant__ CUtensorMap mapU, const __grid_constant_
                 lo[j] = nib<0>(xs[j]);
                 lo[8 + j] = nib<1>(xs[j]);
             }
+            publish();
             mbar_wait(&s_empty[s], ph ^ 1);
             tc_fence_after();
             if (!(CS_PAIR_DIAG & 2)) tmem_st16(a_taddr + s * 32, lo);
@@ -403,10 +469,25 @@ k_interval_pair(const __grid_constant__ CUtensorMap mapU, const __grid_constant_
                 hi[8 + j] = (CS_PAIR_DIAG & 8) ? xs[j] : nib3(xs[j]);
             }
             if (!(CS_PAIR_DIAG & 2)) tmem_st16(a_taddr + s * 32 + 16, hi);
-            asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
-            tc_fence_before();
-            __syncwarp();
-            if (lane == 0) mbar_arrive_cluster(&s_full[s], 0);    // one arrival per warp, in CTA 0
+            pend = true; pend_s = s;
+            if (++s == NS) { s = 0; ph ^= 1; }
+        };
+        // one thread, half a row: chunk c = slices 4 h .. 4 h + 3 of the stage -> 16-byte chunks 2 q + h
+        auto stage_B_half = [&](const uint4 &c) {
+            const uint32_t xs[4] = {c.x, c.y, c.z, c.w};
+            uint4 w[4];
+            w[0] = make_uint4(nib<0>(xs[0]), nib<0>(xs[1]), nib<0>(xs[2]), nib<0>(xs[3]));
+            w[1] = make_uint4(nib<1>(xs[0]), nib<1>(xs[1]), nib<1>(xs[2]), nib<1>(xs[3]));
+            w[2] = make_uint4(nib<2>(xs[0]), nib<2>(xs[1]), nib<2>(xs[2]), nib<2>(xs[3]));
+            if (CS_PAIR_DIAG & 8) w[3] = c;
+            else w[3] = make_uint4(nib3(xs[0]), nib3(xs[1]), nib3(xs[2]), nib3(xs[3]));
+            publish();
+            mbar_wait(&s_empty[s], ph ^ 1);
+            unsigned char *dst = b_dst + s * STAGE_BYTES + bhalf * TNH * 16;
+#pragma unroll
+            for (int q = 0; q < 4; q++)
+                if (!(CS_PAIR_DIAG & 1)) *reinterpret_cast<uint4 *>(dst + 2 * q * TNH * 16) = w[q];
+            pend = true; pend_s = s;
             if (++s == NS) { s = 0; ph ^= 1; }
         };
         auto stage_B = [&](const uint4 &c0, const uint4 &c1) {
@@ -420,21 +501,20 @@ k_interval_pair(const __grid_constant__ CUtensorMap mapU, const __grid_constant_
                 if (CS_PAIR_DIAG & 8) w[6 + h] = make_uint4(xs[4 * h], xs[4 * h + 1], xs[4 * h + 2], xs[4 * h + 3]);
                 else w[6 + h] = make_uint4(nib3(xs[4 * h]), nib3(xs[4 * h + 1]), nib3(xs[4 * h + 2]), nib3(xs[4 * h + 3]));
             }
+            publish();
             mbar_wait(&s_empty[s], ph ^ 1);
             unsigned char *dst = b_dst + s * STAGE_BYTES;
 #pragma unroll
             for (int q = 0; q < 8; q++)
                 if (!(CS_PAIR_DIAG & 1)) *reinterpret_cast<uint4 *>(dst + q * TNH * 16) = w[q];
-            if (!(CS_PAIR_DIAG & 16)) fence_proxy_async();   // generic-proxy stores -> visible to the tensor cores
-            __syncwarp();
-            if (lane == 0) mbar_arrive_cluster(&s_full[s], 0);
+            pend = true; pend_s = s;
             if (++s == NS) { s = 0; ph ^= 1; }
         };
 
         for (uint32_t t = t0; t < total_tiles; t += tstep) {
             const Tile tc = get_tile(t);
             if (tc.skip) continue;
-            const int nstages = tc.J - tc.I + 1;
+            const int nstages = tc.nstages;
             for (int k = 0; k < nstages; k += GK) {
                 mbar_wait(&s_bfull[b], bph);
                 const unsigned char *src = my_bits + b * BITS_BYTES;
@@ -442,6 +522,9 @@ k_interval_pair(const __grid_constant__ CUtensorMap mapU, const __grid_constant_
                 if (isA) {
                     stage_A(*reinterpret_cast<const uint4 *>(src + off0), *reinterpret_cast<const uint4 *>(src + off1));
                     if (second) stage_A(*reinterpret_cast<const uint4 *>(src + off2), *reinterpret_cast<const uint4 *>(src + off3));
+                } else if (TNH == 64) {
+                    stage_B_half(*reinterpret_cast<const uint4 *>(src + (bhalf ? off1 : off0)));
+                    if (second) stage_B_half(*reinterpret_cast<const uint4 *>(src + (bhalf ? off3 : off2)));
                 } else {
                     stage_B(*reinterpret_cast<const uint4 *>(src + off0), *reinterpret_cast<const uint4 *>(src + off1));
                     if (second) stage_B(*reinterpret_cast<const uint4 *>(src + off2), *reinterpret_cast<const uint4 *>(src + off3));
@@ -452,6 +535,9 @@ k_interval_pair(const __grid_constant__ CUtensorMap mapU, const __grid_constant_
                 if (lane == 0) mbar_arrive(&s_bempty[b]);
                 if (++b == NB) { b = 0; bph ^= 1; }
             }
+            // the last stage of a tile is published at once: the epilogue of this tile waits on it, and the
+            // next tile's first bits may be a DRAM miss away
+            publish();
         }
     } else if (warp >= MMA_WARP) {
         asm volatile("setmaxnreg.dec.sync.aligned.u32 40;");
@@ -462,7 +548,7 @@ k_interval_pair(const __grid_constant__ CUtensorMap mapU, const __grid_constant_
             for (uint32_t t = t0; t < total_tiles; t += tstep) {
                 const Tile tc = get_tile(t);
                 if (tc.skip) continue;
-                const int nstages = tc.J - tc.I + 1;
+                const int nstages = tc.nstages;
                 const int ngroups = (nstages + GK - 1) / GK;
                 for (int g = 0; g < ngroups; g++, grp++) {
                     const int b = grp % NB;
@@ -471,36 +557,49 @@ k_interval_pair(const __grid_constant__ CUtensorMap mapU, const __grid_constant_
                     unsigned char *dst = s_bits + b * BITS_BYTES;
                     const int c0 = (tc.I * (KSTEP / 8)) + g * BROW;             // byte column of the first k
                     tma_load_3d(dst, &mapU, c0, tc.I * TILE + (int)rank * TM, tc.b, &s_bfull[b]);
-                    tma_load_3d(dst + TM * BROW, &mapL, c0, tc.J * TILE + (int)rank * TNH, tc.b, &s_bfull[b]);
+                    tma_load_3d(dst + TM * BROW, &mapL, c0, tc.J * TN + (int)rank * TNH, tc.b, &s_bfull[b]);
                 }
             }
         }
-        } else if (warp == MMA_WARP && rank == 0 && lane == 0) {
+        } else if (warp == MMA_WARP && rank == 0) {
             // ===================================== MMA issuer (CTA 0 only) =======================
-            {
-            uint32_t it = 0, tile_seq = 0;
+            // The whole warp walks the schedule and polls the barriers; one elected lane issues.  Kept
+            // warp-uniform on purpose: with the loop inside an `if (lane == 0)` ptxas holds every MMA
+            // operand in vector registers and spends ~19 instructions (R2UR, ELECT, PLOP3 ...) per MMA,
+            // ~600 clk per 512-clk stage for the one issuing thread -- the kernel was bound by that
+            // (ncu source view).  The shared-memory descriptor of (stage, k-slice) is the stage-0 one plus a
+            // constant: the start-address field never carries out of its 14 bits (addresses < 2^18).
+            const uint64_t bdesc0 = make_desc(smem_u32(s_stage), TNH * 16, 128);
+            const uint32_t a_tmem0 = tmem_base + A_COL;
+            const uint32_t sf0 = tmem_base + sf_col(0), sf1 = tmem_base + sf_col(1), sf2 = tmem_base + sf_col(2);
+            uint32_t s = 0, ph = 0, tile_seq = 0;
             for (uint32_t t = t0; t < total_tiles; t += tstep) {
                 const Tile tc = get_tile(t);
                 if (tc.skip) continue;
-                const int nstages = tc.J - tc.I + 1;
-                mbar_wait_cluster(s_tempty, (tile_seq & 1) ^ 1);          // both epilogues have drained the accumulator
+                const int nstages = tc.nstages;
+                const uint32_t acc = tile_seq % NACC, use = tile_seq / NACC;     // accumulator and how often it was used
+                mbar_wait_cluster(&s_tempty[acc], (use & 1) ^ 1);         // both epilogues have drained this accumulator
                 tc_fence_after();
-                for (int ks = 0; ks < nstages; ks++, it++) {
-                    const int s = it % NS;
-                    mbar_wait_cluster(&s_full[s], (it / NS) & 1);
+                const uint32_t d_tmem = tmem_base + acc * TN;
+                for (int ks = 0; ks < nstages; ks++) {
+                    mbar_wait_cluster(&s_full[s], ph);
                     tc_fence_after();
-                    const uint32_t b_addr = smem_u32(s_stage + s * STAGE_BYTES);
-#pragma unroll
-                    for (int q = 0; q < 4; q++) {     // K = 64 per MMA: 8 TMEM columns of A, 2 chunks of B
-                        const uint64_t bd = make_desc(b_addr + q * 2 * TNH * 16, TNH * 16, 128);
-                        const uint32_t sf = tmem_base + sf_col(q);
-                        mma_mxf4_pair(tmem_base, tmem_base + A_COL + s * 32 + q * 8, bd, IDESC, (ks > 0 || q > 0) ? 1u : 0u, sf, sf);
+                    if (elect_one()) {
+                        const uint64_t bd = bdesc0 + (uint64_t)((s * STAGE_BYTES) >> 4);
+                        const uint32_t at = a_tmem0 + s * 32;
+                        // K = 64 per MMA: 8 TMEM columns of A, 2 chunks of B
+                        mma_mxf4_pair(d_tmem, at, bd, SH::IDESC, ks > 0 ? 1u : 0u, sf0, sf0);
+                        mma_mxf4_pair(d_tmem, at + 8, bd + ((2 * TNH * 16) >> 4), SH::IDESC, 1u, sf1, sf1);
+                        mma_mxf4_pair(d_tmem, at + 16, bd + ((4 * TNH * 16) >> 4), SH::IDESC, 1u, sf2, sf2);
+                        mma_mxf4_pair(d_tmem, at + 24, bd + ((6 * TNH * 16) >> 4), SH::IDESC, 1u, sf0, sf0);
+                        mma_commit_pair(&s_empty[s]);                     // stage s free in both CTAs once these MMAs retire
                     }
-                    mma_commit_pair(&s_empty[s]);                         // stage s free in both CTAs once these MMAs retire
+                    __syncwarp();
+                    if (++s == NS) { s = 0; ph ^= 1; }
                 }
-                mma_commit_pair(s_tfull);                                 // accumulator complete, both CTAs
+                if (elect_one()) mma_commit_pair(&s_tfull[acc]);          // accumulator complete, both CTAs
+                __syncwarp();
                 tile_seq++;
-            }
             }
         }
     } else {
@@ -512,8 +611,8 @@ k_interval_pair(const __grid_constant__ CUtensorMap mapU, const __grid_constant_
         uint32_t tile_seq = 0;
         unsigned long long my_nrel = 0;
         int cur_batch = -1;
-        const int quarter = warp & 3, colhalf = warp >> 2;   // TMEM lane quarter; which 128 columns
-        const uint32_t taddr = tmem_base + ((uint32_t)(quarter * 32) << 16) + colhalf * 128;
+        const int quarter = warp & 3, colhalf = warp >> 2;   // TMEM lane quarter; which CW = TN/2 columns
+        const uint32_t taddr0 = tmem_base + ((uint32_t)(quarter * 32) << 16) + colhalf * CW;
         // Counts are exact small integers held as fp32: adding 2^23 leaves the count in the low mantissa
         // bits (one FADD, no F2I), and comparisons are taken on the float itself.
         const uint32_t kmax32 = (uint32_t)kmax;
@@ -547,25 +646,27 @@ k_interval_pair(const __grid_constant__ CUtensorMap mapU, const __grid_constant_
             }
             const int64_t i = (int64_t)tc.I * TILE + rank * TM + quarter * 32 + lane;   // this thread's row
             const bool row_ok = i < N && i >= row_begin && i < row_end;
-            uint64_t rel[2] = {0, 0};                            // relation bits of this warp's 128 columns
+            uint64_t rel[2] = {0, 0};                            // relation bits of this warp's CW columns
             if (row_ok) {
                 const uint64_t *urow = bits + ((int64_t)tc.b * N + i) * stride;
 #pragma unroll
-                for (int w = 0; w < 2; w++) {
-                    const int64_t wi = (int64_t)tc.J * 4 + colhalf * 2 + w;
+                for (int w = 0; w < CW / 64; w++) {
+                    const int64_t wi = ((int64_t)tc.J * TN + colhalf * CW) / 64 + w;
                     if (wi < stride) rel[w] = __ldg(urow + wi);
                 }
             }
             unsigned long long *ghist = hist + (int64_t)cur_batch * hist_len;
-            uint32_t v[128];
-            mbar_wait(s_tfull, tile_seq & 1);
+            uint32_t v[CW];
+            const uint32_t acc = tile_seq % NACC, use = tile_seq / NACC;
+            const uint32_t taddr = taddr0 + acc * TN;
+            mbar_wait(&s_tfull[acc], use & 1);
             tc_fence_after();
 #pragma unroll
-            for (int c = 0; c < 4; c++) tmem_ld32(taddr + c * 32, &v[c * 32]);
+            for (int c = 0; c < CW / 32; c++) tmem_ld32(taddr + c * 32, &v[c * 32]);
             asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
             tc_fence_before();
             __syncwarp();
-            if (lane == 0) mbar_arrive_cluster(s_tempty, 0);   // one arrival per warp, in CTA 0
+            if (lane == 0) mbar_arrive_cluster(&s_tempty[acc], 0);   // one arrival per warp, in CTA 0
             tile_seq++;
             if (CS_PAIR_DIAG & 4) continue;
             my_nrel += __popcll(rel[0]) + __popcll(rel[1]);
@@ -575,11 +676,11 @@ k_interval_pair(const __grid_constant__ CUtensorMap mapU, const __grid_constant_
             // time of a 2048-point causet).  The general path needs one branch per column -- ptxas never
             // predicates an atomic -- and a second one only in tiles long enough to hold counts >= hs.
             uint32_t acc0 = 0, acc1 = 0;                         // SMALL: four 8-bit fields, <= 64 increments each
-            const bool maybe_big = (uint32_t)(tc.J - tc.I + 1) * TILE > (uint32_t)hs;   // counts < (J-I+1) 256
+            const bool maybe_big = (uint32_t)tc.nstages * KSTEP > (uint32_t)hs;   // counts < 256 nstages
             auto tally = [&](auto big_tag) {
                 constexpr bool BIG = decltype(big_tag)::value;
 #pragma unroll
-                for (int w = 0; w < 4; w++) {
+                for (int w = 0; w < CW / 32; w++) {
                     const uint32_t relw = (uint32_t)(rel[w >> 1] >> (32 * (w & 1)));
                     if (!__any_sync(0xffffffffu, relw != 0)) continue;
 #pragma unroll
@@ -683,39 +784,58 @@ static int pair_bits_map(CUtensorMap *map, const uint64_t *base, int64_t B, int6
     return CS_OK;
 }
 
+// TN = 128 (two ping-pong accumulators) when the tiles are short enough for the accumulator drain to
+// matter more than the doubled A expansion; measured on B200
+static int pair_tile_width(int64_t B, int64_t N)
+{
+    (void)B;
+    return N <= CS_PAIR_TN128_MAX_N ? 128 : 256;
+}
+
 size_t interval_pair_scratch_bytes(int64_t N)
 {
-    const int64_t nT = (N + TILE - 1) / TILE;
-    return (size_t)(nT * (nT + 1) / 2) * sizeof(uint32_t);
+    return (size_t)pair_tiles_per_causet(N, 128) * sizeof(uint32_t);   // the longer of the two tables
+}
+
+template <bool SMALL, int TN>
+static int launch_pair_t(const CUtensorMap &mapU, const CUtensorMap &mapL, const uint64_t *bits, const uint32_t *tab,
+                         uint32_t tiles_per, int64_t clusters, int64_t B, int64_t N, int64_t stride, int64_t kmax, int hs,
+                         int64_t row_begin, int64_t row_end, int64_t *hist, int64_t *nrel, cudaStream_t st)
+{
+    static bool attr_set = false;
+    if (!attr_set) {
+        CS_CUDA(cudaFuncSetAttribute(k_interval_pair<SMALL, TN>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                     Shape<TN>::SMEM_FIXED + (SMALL ? 0 : HS_MAX * 4)));
+        attr_set = true;
+    }
+    k_interval_pair<SMALL, TN><<<(unsigned)(2 * clusters), THREADS, Shape<TN>::SMEM_FIXED + hs * 4, st>>>(
+        mapU, mapL, bits, tab, tiles_per, B, N, stride, kmax, hs, row_begin, row_end,
+        reinterpret_cast<unsigned long long *>(hist), reinterpret_cast<unsigned long long *>(nrel));
+    CS_LAUNCHED("k_interval_pair");
+    return CS_OK;
 }
 
 int launch_interval_pair(const uint64_t *bits, const uint64_t *bitsT, int64_t B, int64_t N, int64_t kmax,
                          int64_t row_begin, int64_t row_end, int64_t *hist, int64_t *nrel,
                          void *scratch, size_t scratch_bytes, cudaStream_t st)
 {
-    if (N > ((int64_t)1 << 24)) return CS_ERR_ARG;   // counts must stay exact in fp32; tile ids are 16 bits
-    {
-        const int64_t nT64 = (N + TILE - 1) / TILE;
-        if (B > 0 && nT64 * (nT64 + 1) / 2 > (((int64_t)1 << 31) - 1) / B) return CS_ERR_ARG;   // 32-bit tile schedule
-    }
+    if (N > ((int64_t)1 << 22)) return CS_ERR_ARG;   // counts must stay exact in fp32; tile ids are 16 bits
+    const int TN = pair_tile_width(B, N);
+    const int64_t tiles_per = pair_tiles_per_causet(N, TN);
+    if (B > 0 && tiles_per > (((int64_t)1 << 31) - 1) / B) return CS_ERR_ARG;   // 32-bit tile schedule
     if (!scratch || scratch_bytes < interval_pair_scratch_bytes(N)) return CS_ERR_WORKSPACE;
-    static bool attr_set = false;
-    if (!attr_set) {
-        CS_CUDA(cudaFuncSetAttribute(k_interval_pair<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES));
-        CS_CUDA(cudaFuncSetAttribute(k_interval_pair<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_FIXED));
-        attr_set = true;
-    }
     const int64_t stride = row_stride_words(N);
     CUtensorMap mapU, mapL;
     int rc = pair_bits_map(&mapU, bits, B, N, stride, TM);
     if (rc) return rc;
-    rc = pair_bits_map(&mapL, bitsT, B, N, stride, TNH);
+    rc = pair_bits_map(&mapL, bitsT, B, N, stride, TN / 2);
     if (rc) return rc;
-    const int nT = (int)((N + TILE - 1) / TILE);
+    const int nT = (int)((N + TILE - 1) / TILE), nTc = (int)((N + TN - 1) / TN), R = TILE / TN;
     uint32_t *tab = static_cast<uint32_t *>(scratch);
-    k_pair_tile_order<<<(nT + BANDW - 1) / BANDW, 128, 0, st>>>(nT, tab);
+    const int bands = (nTc + BANDW * R - 1) / (BANDW * R);
+    k_pair_tile_order<<<bands, 256, 0, st>>>(nT, nTc, R, tab);
     CS_LAUNCHED("k_pair_tile_order");
-    const int64_t total = (int64_t)nT * (nT + 1) / 2 * B;
+    const int64_t total = tiles_per * B;
     int64_t clusters = sm_count() / 2;
     if (clusters > total) clusters = total;
     if (clusters < 1) clusters = 1;
@@ -723,16 +843,11 @@ int launch_interval_pair(const uint64_t *bits, const uint64_t *bitsT, int64_t B,
     const bool small = kmax <= 3;
     const int64_t hs_cap = B > 1 ? HS_BATCHED : HS_MAX;
     const int hs = small ? 0 : (int)(kmax + 1 < hs_cap ? kmax + 1 : hs_cap);
-    if (small)
-        k_interval_pair<true><<<(unsigned)(2 * clusters), THREADS, SMEM_FIXED, st>>>(
-            mapU, mapL, bits, tab, B, N, stride, kmax, hs, row_begin, row_end,
-            reinterpret_cast<unsigned long long *>(hist), reinterpret_cast<unsigned long long *>(nrel));
-    else
-        k_interval_pair<false><<<(unsigned)(2 * clusters), THREADS, SMEM_FIXED + hs * 4, st>>>(
-            mapU, mapL, bits, tab, B, N, stride, kmax, hs, row_begin, row_end,
-            reinterpret_cast<unsigned long long *>(hist), reinterpret_cast<unsigned long long *>(nrel));
-    CS_LAUNCHED("k_interval_pair");
-    return CS_OK;
+#define CS_PAIR_LAUNCH(S, T) \
+    launch_pair_t<S, T>(mapU, mapL, bits, tab, (uint32_t)tiles_per, clusters, B, N, stride, kmax, hs, row_begin, row_end, hist, nrel, st)
+    if (TN == 128) return small ? CS_PAIR_LAUNCH(true, 128) : CS_PAIR_LAUNCH(false, 128);
+    return small ? CS_PAIR_LAUNCH(true, 256) : CS_PAIR_LAUNCH(false, 256);
+#undef CS_PAIR_LAUNCH
 }
 
 }  // namespace cs
