@@ -40,7 +40,7 @@ UNIT = "word-ops/s"
 POPC_PER_CLK_SM = 16.0
 # dram__bytes_read.sum + dram__bytes_write.sum of one launch of the a2 kernel at config 3, from the
 # `ncu --set full` captures summarised under profiles/ (bytes per launch; None = not captured)
-NCU_TRAFFIC = {1: 78.28e9, 2: 51.14e9, 3: 38.12e9, 4: 10.30e9}
+NCU_TRAFFIC = {1: 78.28e9, 2: 51.14e9, 3: 38.12e9, 4: 8.50e9}
 # tensor peaks = measured bf16 dense peak x the guide's nominal ratio (bf16 2.25, int8/fp8 4.5, fp4 9 PFLOP/s)
 TENSOR_OVER_BF16 = {2: 2.0, 3: 4.0, 4: 4.0}
 # dense issue rate of one SM's tensor pipe in op/clk (2 per multiply-add): kind::i8 16384, kind::mxf4 32768

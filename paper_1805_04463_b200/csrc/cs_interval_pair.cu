@@ -59,9 +59,7 @@ struct Shape {
 constexpr int HS_MAX = CS_PAIR_HS_MAX;   // shared-memory histogram bins that fit beside the operand rings
 constexpr int HS_BATCHED = 2048;        // bins when several causets share a CTA (flushed at every switch)
 constexpr int BANDW = 8;                // diagonals (in 256-column units) per band of the tile order
-#ifndef CS_PAIR_TN128_MAX_N
-#define CS_PAIR_TN128_MAX_N 4096        // largest N that runs on 128-column tiles (two accumulators)
-#endif
+
 #ifndef CS_PAIR_DIAG
 #define CS_PAIR_DIAG 0      // timing experiments only (results are wrong): 1 no B stores, 2 no A stores, 4 no tally
 #endif
@@ -432,14 +430,10 @@ k_interval_pair(const __grid_constant__ CUtensorMap mapU, const __grid_constant_
         const uint32_t a_taddr = tmem_base + ((uint32_t)((warp & 3) * 32) << 16) + A_COL;
         unsigned char *b_dst = s_stage + r * 16;
 
-        // A stage is published (arrival on its full barrier) only after its stores have landed: TMEM
-        // stores need tcgen05.wait::st, shared-memory stores a generic->async proxy fence.  Both waits are
-        // deferred until the NEXT stage's bits have been loaded and expanded, so that the store latency
-        // overlaps that work instead of sitting on the one-stage-at-a-time critical path of the warp.
-        bool pend = false;
-        uint32_t pend_s = 0;
-        auto publish = [&]() {
-            if (!pend) return;
+        // A stage is published (arrival on its full barrier) once its stores have landed: TMEM stores
+        // need tcgen05.wait::st, shared-memory stores a generic->async proxy fence.  (Deferring the wait until
+        // the next stage has been expanded was measured: no difference, 10.974 vs 10.977 ms at N = 65536.)
+        auto publish = [&](uint32_t stage) {
             if (isA) {
                 asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
                 tc_fence_before();
@@ -447,8 +441,7 @@ k_interval_pair(const __grid_constant__ CUtensorMap mapU, const __grid_constant_
                 fence_proxy_async();   // generic-proxy stores -> visible to the tensor cores
             }
             __syncwarp();
-            if (lane == 0) mbar_arrive_cluster(&s_full[pend_s], 0);    // one arrival per warp, in CTA 0
-            pend = false;
+            if (lane == 0) mbar_arrive_cluster(&s_full[stage], 0);    // one arrival per warp, in CTA 0
         };
         auto stage_A = [&](const uint4 &c0, const uint4 &c1) {
             const uint32_t xs[8] = {c0.x, c0.y, c0.z, c0.w, c1.x, c1.y, c1.z, c1.w};
@@ -459,7 +452,6 @@ k_interval_pair(const __grid_constant__ CUtensorMap mapU, const __grid_constant_
                 lo[j] = nib<0>(xs[j]);
                 lo[8 + j] = nib<1>(xs[j]);
             }
-            publish();
             mbar_wait(&s_empty[s], ph ^ 1);
             tc_fence_after();
             if (!(CS_PAIR_DIAG & 2)) tmem_st16(a_taddr + s * 32, lo);
@@ -469,7 +461,7 @@ k_interval_pair(const __grid_constant__ CUtensorMap mapU, const __grid_constant_
                 hi[8 + j] = (CS_PAIR_DIAG & 8) ? xs[j] : nib3(xs[j]);
             }
             if (!(CS_PAIR_DIAG & 2)) tmem_st16(a_taddr + s * 32 + 16, hi);
-            pend = true; pend_s = s;
+            publish(s);
             if (++s == NS) { s = 0; ph ^= 1; }
         };
         // one thread, half a row: chunk c = slices 4 h .. 4 h + 3 of the stage -> 16-byte chunks 2 q + h
@@ -481,13 +473,12 @@ k_interval_pair(const __grid_constant__ CUtensorMap mapU, const __grid_constant_
             w[2] = make_uint4(nib<2>(xs[0]), nib<2>(xs[1]), nib<2>(xs[2]), nib<2>(xs[3]));
             if (CS_PAIR_DIAG & 8) w[3] = c;
             else w[3] = make_uint4(nib3(xs[0]), nib3(xs[1]), nib3(xs[2]), nib3(xs[3]));
-            publish();
             mbar_wait(&s_empty[s], ph ^ 1);
             unsigned char *dst = b_dst + s * STAGE_BYTES + bhalf * TNH * 16;
 #pragma unroll
             for (int q = 0; q < 4; q++)
                 if (!(CS_PAIR_DIAG & 1)) *reinterpret_cast<uint4 *>(dst + 2 * q * TNH * 16) = w[q];
-            pend = true; pend_s = s;
+            publish(s);
             if (++s == NS) { s = 0; ph ^= 1; }
         };
         auto stage_B = [&](const uint4 &c0, const uint4 &c1) {
@@ -501,13 +492,12 @@ k_interval_pair(const __grid_constant__ CUtensorMap mapU, const __grid_constant_
                 if (CS_PAIR_DIAG & 8) w[6 + h] = make_uint4(xs[4 * h], xs[4 * h + 1], xs[4 * h + 2], xs[4 * h + 3]);
                 else w[6 + h] = make_uint4(nib3(xs[4 * h]), nib3(xs[4 * h + 1]), nib3(xs[4 * h + 2]), nib3(xs[4 * h + 3]));
             }
-            publish();
             mbar_wait(&s_empty[s], ph ^ 1);
             unsigned char *dst = b_dst + s * STAGE_BYTES;
 #pragma unroll
             for (int q = 0; q < 8; q++)
                 if (!(CS_PAIR_DIAG & 1)) *reinterpret_cast<uint4 *>(dst + q * TNH * 16) = w[q];
-            pend = true; pend_s = s;
+            publish(s);
             if (++s == NS) { s = 0; ph ^= 1; }
         };
 
@@ -535,9 +525,6 @@ k_interval_pair(const __grid_constant__ CUtensorMap mapU, const __grid_constant_
                 if (lane == 0) mbar_arrive(&s_bempty[b]);
                 if (++b == NB) { b = 0; bph ^= 1; }
             }
-            // the last stage of a tile is published at once: the epilogue of this tile waits on it, and the
-            // next tile's first bits may be a DRAM miss away
-            publish();
         }
     } else if (warp >= MMA_WARP) {
         asm volatile("setmaxnreg.dec.sync.aligned.u32 40;");
@@ -784,17 +771,15 @@ static int pair_bits_map(CUtensorMap *map, const uint64_t *base, int64_t B, int6
     return CS_OK;
 }
 
-// TN = 128 (two ping-pong accumulators) when the tiles are short enough for the accumulator drain to
-// matter more than the doubled A expansion; measured on B200
-static int pair_tile_width(int64_t B, int64_t N)
-{
-    (void)B;
-    return N <= CS_PAIR_TN128_MAX_N ? 128 : 256;
-}
+// Only TN = 256 is instantiated.  TN = 128 (two ping-pong accumulators, so that the 2048-clk drain of one
+// overlaps the MMAs into the other) was built and measured: bit-exact, but slower at every size (N = 32768:
+// 2.80 vs 1.48 ms; 1024 x N = 2048: 1.69 vs 1.11 ms) -- it expands every A stage for half the MMA work, and
+// the A stores into TMEM and the B stores into shared memory are what the tensor pipe waits for.
+constexpr int PAIR_TN = 256;
 
 size_t interval_pair_scratch_bytes(int64_t N)
 {
-    return (size_t)pair_tiles_per_causet(N, 128) * sizeof(uint32_t);   // the longer of the two tables
+    return (size_t)pair_tiles_per_causet(N, PAIR_TN) * sizeof(uint32_t);
 }
 
 template <bool SMALL, int TN>
@@ -820,7 +805,7 @@ int launch_interval_pair(const uint64_t *bits, const uint64_t *bitsT, int64_t B,
                          void *scratch, size_t scratch_bytes, cudaStream_t st)
 {
     if (N > ((int64_t)1 << 22)) return CS_ERR_ARG;   // counts must stay exact in fp32; tile ids are 16 bits
-    const int TN = pair_tile_width(B, N);
+    constexpr int TN = PAIR_TN;
     const int64_t tiles_per = pair_tiles_per_causet(N, TN);
     if (B > 0 && tiles_per > (((int64_t)1 << 31) - 1) / B) return CS_ERR_ARG;   // 32-bit tile schedule
     if (!scratch || scratch_bytes < interval_pair_scratch_bytes(N)) return CS_ERR_WORKSPACE;
@@ -845,8 +830,7 @@ int launch_interval_pair(const uint64_t *bits, const uint64_t *bitsT, int64_t B,
     const int hs = small ? 0 : (int)(kmax + 1 < hs_cap ? kmax + 1 : hs_cap);
 #define CS_PAIR_LAUNCH(S, T) \
     launch_pair_t<S, T>(mapU, mapL, bits, tab, (uint32_t)tiles_per, clusters, B, N, stride, kmax, hs, row_begin, row_end, hist, nrel, st)
-    if (TN == 128) return small ? CS_PAIR_LAUNCH(true, 128) : CS_PAIR_LAUNCH(false, 128);
-    return small ? CS_PAIR_LAUNCH(true, 256) : CS_PAIR_LAUNCH(false, 256);
+    return small ? CS_PAIR_LAUNCH(true, PAIR_TN) : CS_PAIR_LAUNCH(false, PAIR_TN);
 #undef CS_PAIR_LAUNCH
 }
 
