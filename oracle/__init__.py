@@ -22,6 +22,9 @@ from .oracle import (  # noqa: F401
     interval_hist_alg20,
     count_relations,
     bd_action,
+    chain_pair,
+    chain_heights,
+    greedy_antichain,
     smear_f,
     smeared_action,
     max_threads,

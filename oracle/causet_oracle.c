@@ -20,6 +20,8 @@
  *      paper's notation L_m = {i : |A_ij| = m-1} (Eq. 4.8).
  *   3. Benincasa-Dowker action, Eq. 4.10-4.12, l/l_p := 1.
  *   4. (NEXT-1) smeared action, Eq. 4.13-4.18.
+ *   5. (NEXT-3) longest chains (Algorithm 11) and the greedy maximal antichain
+ *      (Algorithm 13).
  *
  * Floating point: every predicate is evaluated in fp64 exactly in the order
  * written below; compile with -ffp-contract=off (no FMA), no -ffast-math.
@@ -368,6 +370,114 @@ double orc_smeared_action(const int64_t *hist, int64_t nhist, int64_t N, int dim
     }
     if (dim == 4) return (double)(4.0L * sqrtl(e / 6.0L) * ((long double)N - e * sum));
     return NAN;
+}
+
+/* ---- NEXT-3: chains and antichains -------------------------------------
+ * All three work on the byte matrix C[i*N + j] = (i -< j) of stage 1 (tier-0 style: plain loops).
+ *
+ * orc_chain_pair: Algorithm 11 literally (text 1326, 1353): for i -< j the
+ * recursion moves through the Alexandroff set A_ij = J+(i) & J-(j), L[k] memoises the distance from
+ * k to j, unvisited entries are -1.  With l starting at 0 the procedure returns
+ * l + 1 = the number of LINKS of the longest chain from i to j (1 if A_ij is empty), i.e. the number
+ * of elements of that chain minus one.  Returns 0 if i is not related to j.  (The listing's recursive
+ * call passes "A_ki"; the set being scanned must be A_kj, the one formed on the line before it.)
+ */
+static int64_t orc_chain_rec(const uint8_t *C, int64_t N, int64_t *L, int64_t i, int64_t j)
+{
+    int64_t l = 0;
+    for (int64_t k = i + 1; k < j; k++) {
+        if (!(C[i * N + k] && C[k * N + j])) continue;          /* k in A_ij */
+        int64_t kappa;
+        if (L[k] == -1) {
+            int nonempty = 0;
+            for (int64_t m = k + 1; m < j && !nonempty; m++) nonempty = C[k * N + m] && C[m * N + j];
+            if (nonempty) kappa = orc_chain_rec(C, N, L, k, j);
+            else kappa = 1;
+            L[k] = kappa;
+        } else {
+            kappa = L[k];
+        }
+        if (kappa > l) l = kappa;
+    }
+    return l + 1;
+}
+
+int64_t orc_chain_pair(const uint8_t *C, int64_t N, int64_t i, int64_t j)
+{
+    if (i < 0 || j >= N || i >= j || !C[i * N + j]) return 0;
+    int64_t *L = (int64_t *)malloc((size_t)N * sizeof(int64_t));
+    for (int64_t k = 0; k < N; k++) L[k] = -1;
+    int64_t r = orc_chain_rec(C, N, L, i, j);
+    free(L);
+    return r;
+}
+
+/* orc_chain_heights: the definition the recursion reaches, written out for every element at once.
+ * height[k] = number of elements of the longest chain that ends at k; with source >= 0 only chains
+ * that start at `source` count (height[source] = 1, 0 for elements outside J+(source)).  Elements
+ * are in time order, so predecessors come first.  Returns the largest height (0 for N = 0). */
+int64_t orc_chain_heights(const uint8_t *C, int64_t N, int64_t source, int32_t *height)
+{
+    int64_t best = 0;
+    for (int64_t j = 0; j < N; j++) {
+        int32_t h;
+        if (source < 0) {
+            h = 1;
+            for (int64_t i = 0; i < j; i++)
+                if (C[i * N + j] && height[i] + 1 > h) h = height[i] + 1;
+        } else if (j == source) {
+            h = 1;
+        } else if (j < source || !C[source * N + j]) {
+            h = 0;
+        } else {
+            h = 2;                                              /* source -< j */
+            for (int64_t i = source + 1; i < j; i++)
+                if (height[i] > 0 && C[i * N + j] && height[i] + 1 > h) h = height[i] + 1;
+        }
+        height[j] = h;
+        if (h > best) best = h;
+    }
+    return best;
+}
+
+/* orc_greedy_antichain: Algorithm 13 literally (text 1355-1359).  J(j) = J+(j) | J-(j).
+ * Candidates Xi = P \ J(seed) \ {seed}, A = {seed} | Xi; while Xi is not empty: for j in Xi in index
+ * order c = |A \ J(j)|, keep the FIRST j with the largest c (the listing's strict "c > sigma"), then
+ * A = A \ J(k), Xi = Xi \ (J(k) | {k}).  member[] gets 0/1; returns |A|. */
+int64_t orc_greedy_antichain(const uint8_t *C, int64_t N, int64_t seed, uint8_t *member)
+{
+    if (N <= 0 || seed < 0 || seed >= N) return 0;
+    uint8_t *xi = (uint8_t *)calloc((size_t)N, 1);
+    int64_t nxi = 0;
+#define ORC_REL(a, b) (C[(a) * N + (b)] || C[(b) * N + (a)])
+    for (int64_t j = 0; j < N; j++) {
+        xi[j] = (j != seed) && !ORC_REL(seed, j);
+        member[j] = (j == seed) || xi[j];
+        nxi += xi[j];
+    }
+    while (nxi > 0) {
+        int64_t sigma = 0, k = -1;
+        for (int64_t j = 0; j < N; j++) {
+            if (!xi[j]) continue;
+            int64_t c = 0;
+            for (int64_t a = 0; a < N; a++) c += member[a] && !ORC_REL(j, a);
+            if (c > sigma) { sigma = c; k = j; }
+        }
+        /* c >= 1 always (j itself is in A and not in J(j)), so k is set */
+        for (int64_t a = 0; a < N; a++) {
+            if (ORC_REL(k, a)) {
+                member[a] = 0;
+                if (xi[a]) { xi[a] = 0; nxi--; }
+            }
+        }
+        xi[k] = 0;
+        nxi--;
+    }
+#undef ORC_REL
+    free(xi);
+    int64_t size = 0;
+    for (int64_t a = 0; a < N; a++) size += member[a];
+    return size;
 }
 
 int orc_max_threads(void)

@@ -64,6 +64,12 @@ def _load():
         lib.orc_count_relations.argtypes = [_p, _i64, _i64, _p, _p]
         lib.orc_bd_action.restype = ctypes.c_double
         lib.orc_bd_action.argtypes = [_p, _i64, _i64, ctypes.c_int, _p]
+        lib.orc_chain_pair.restype = _i64
+        lib.orc_chain_pair.argtypes = [_p, _i64, _i64, _i64]
+        lib.orc_chain_heights.restype = _i64
+        lib.orc_chain_heights.argtypes = [_p, _i64, _i64, _p]
+        lib.orc_greedy_antichain.restype = _i64
+        lib.orc_greedy_antichain.argtypes = [_p, _i64, _i64, _p]
         lib.orc_smear_f.restype = ctypes.c_double
         lib.orc_smear_f.argtypes = [ctypes.c_int, _i64, ctypes.c_double]
         lib.orc_smeared_action.restype = ctypes.c_double
@@ -192,6 +198,30 @@ def bd_action(hist: np.ndarray, N: int, dim: int):
     br = np.zeros(1, dtype=np.int64)
     S = _load().orc_bd_action(_ptr(hist), hist.shape[0], N, dim, _ptr(br))
     return float(S), int(br[0])
+
+
+def chain_pair(C: np.ndarray, i: int, j: int) -> int:
+    """Algorithm 11: links of the longest chain from i to j (0 if unrelated)."""
+    C = np.ascontiguousarray(C, dtype=np.uint8)
+    return int(_load().orc_chain_pair(_ptr(C), C.shape[0], i, j))
+
+
+def chain_heights(C: np.ndarray, source: int = -1):
+    """-> (height int32[N], longest): elements of the longest chain ending at each element."""
+    C = np.ascontiguousarray(C, dtype=np.uint8)
+    N = C.shape[0]
+    h = np.zeros(N, dtype=np.int32)
+    best = int(_load().orc_chain_heights(_ptr(C), N, source, _ptr(h)))
+    return h, best
+
+
+def greedy_antichain(C: np.ndarray, seed: int) -> np.ndarray:
+    """Algorithm 13 -> member uint8[N]."""
+    C = np.ascontiguousarray(C, dtype=np.uint8)
+    N = C.shape[0]
+    m = np.zeros(N, dtype=np.uint8)
+    _load().orc_greedy_antichain(_ptr(C), N, seed, _ptr(m))
+    return m
 
 
 def smear_f(dim: int, m: int, eps: float) -> float:
