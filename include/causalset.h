@@ -120,6 +120,29 @@ int cs_interval_hist_ex(const uint64_t *bits, const uint64_t *bitsT, int64_t N, 
                         int64_t row_begin, int64_t row_end, int route,
                         int64_t *hist, int64_t *n_relations,
                         void *workspace, size_t workspace_bytes, void *stream);
+/* NEXT-3: chains and antichains on the bit matrix (Algorithms 11-13).
+ * Both take bits and bitsT as written by cs_causal_matrix and a workspace of cs_poset_workspace(N) bytes
+ * (256-byte aligned).
+ *
+ * cs_chain_heights: height[k] = number of elements of the longest chain that ends at element k (1 for a
+ * minimal element).  With source >= 0 only chains starting at `source` count: height[source] = 1, 0 for
+ * elements outside the future of `source`; then height[j] - 1 is the result of Algorithm 11 for the pair
+ * (source, j): the number of links of the longest chain between them.  source = -1: all chains.
+ *   height   device, int32[N], overwritten.
+ *   longest  device, int64[1] or NULL: the largest height (0 for N = 0).
+ *
+ * cs_greedy_antichain: Algorithm 13 with seed element `seed`: candidates = elements unrelated to the seed;
+ * repeatedly keep the candidate j that leaves the most elements, c = |A \ J(j)|, J(j) = future | past of j
+ * (the first such j in index order), and drop its relatives, until no candidate is left.
+ *   member   device, uint64[cs_row_stride_words(N)], overwritten: bit k set iff element k is in the antichain.
+ *   size     device, int64[1] or NULL: number of members.
+ * Errors: CS_ERR_ARG (source/seed out of range), CS_ERR_WORKSPACE, CS_ERR_CUDA. */
+size_t cs_poset_workspace(int64_t N);
+int cs_chain_heights(const uint64_t *bits, const uint64_t *bitsT, int64_t N, int64_t source,
+                     int32_t *height, int64_t *longest, void *workspace, size_t workspace_bytes, void *stream);
+int cs_greedy_antichain(const uint64_t *bits, const uint64_t *bitsT, int64_t N, int64_t seed,
+                        uint64_t *member, int64_t *size, void *workspace, size_t workspace_bytes, void *stream);
+
 /* a2 over B causets in one launch (the Monte-Carlo ensemble): bits/bitsT are
  * [B][N][stride] as written by cs_causal_matrix_batched (bitsT required), hist is int64[B][kmax+1]
  * (kmax clamped as above), overwritten.  Workspace: cs_interval_hist_batched_workspace() bytes.

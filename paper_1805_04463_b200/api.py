@@ -51,6 +51,9 @@ _SIGNATURES = {
     "cs_interval_hist_batched": (_int, [_p, _p, _i64, _i64, _i64, _int, _p, _p, _sz, _p]),
     "cs_default_route": (_int, [_i64]),
     "cs_bd_action": (_int, [_p, _i64, _i64, _int, _p, _p, _p]),
+    "cs_poset_workspace": (_sz, [_i64]),
+    "cs_chain_heights": (_int, [_p, _p, _i64, _i64, _p, _p, _p, _sz, _p]),
+    "cs_greedy_antichain": (_int, [_p, _p, _i64, _i64, _p, _p, _p, _sz, _p]),
     "cs_smeared_action": (_int, [_p, _i64, _i64, _int, ctypes.c_double, _p, _p]),
     "cs_bd_action_batched_workspace": (_sz, [_i64, _i64]),
     "cs_bd_action_batched": (_int, [_p, _i64, _i64, _int, _int, _p, _p, _p, _sz, _p]),
@@ -210,6 +213,31 @@ def bd_action(hist: torch.Tensor, N: int, dim: int, return_bracket: bool = False
     _check(load().cs_bd_action(_dptr(hist), hist.numel() - 1, N, dim, _dptr(action), _dptr(bracket), _stream()),
            "cs_bd_action")
     return (action, bracket) if return_bracket else action
+
+
+def chain_heights(bits: torch.Tensor, bitsT: torch.Tensor, N: int, source: int = -1):
+    """-> (height int32[N], longest int64[1]) on the device: elements of the longest chain ending at each
+    element (starting at `source` if >= 0); Algorithm 11 for the pair (source, j) is height[j] - 1."""
+    _need_cuda(bits, torch.int64, "bits")
+    _need_cuda(bitsT, torch.int64, "bitsT")
+    height = torch.empty(N, dtype=torch.int32, device=bits.device)
+    longest = torch.empty(1, dtype=torch.int64, device=bits.device)
+    ws = _workspace(int(load().cs_poset_workspace(N)), bits.device)
+    _check(load().cs_chain_heights(_dptr(bits), _dptr(bitsT), N, source, _dptr(height), _dptr(longest),
+                                   _dptr(ws), ws.numel(), _stream()), "cs_chain_heights")
+    return height, longest
+
+
+def greedy_antichain(bits: torch.Tensor, bitsT: torch.Tensor, N: int, seed: int):
+    """Algorithm 13 -> (member int64[stride] holding the uint64 bitset, size int64[1]) on the device."""
+    _need_cuda(bits, torch.int64, "bits")
+    _need_cuda(bitsT, torch.int64, "bitsT")
+    member = torch.empty(row_stride_words(N), dtype=torch.int64, device=bits.device)
+    size = torch.empty(1, dtype=torch.int64, device=bits.device)
+    ws = _workspace(int(load().cs_poset_workspace(N)), bits.device)
+    _check(load().cs_greedy_antichain(_dptr(bits), _dptr(bitsT), N, seed, _dptr(member), _dptr(size),
+                                      _dptr(ws), ws.numel(), _stream()), "cs_greedy_antichain")
+    return member, size
 
 
 def smeared_action(hist: torch.Tensor, N: int, dim: int, eps: float) -> torch.Tensor:

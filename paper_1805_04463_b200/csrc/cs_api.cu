@@ -1,6 +1,6 @@
 // cs_api.cu -- the extern "C" boundary of libcausalset.so (include/causalset.h).
 // Argument checking, workspace carving and kernel sequencing only; the arithmetic lives in
-// cs_build.cu (a1), cs_interval_popc.cu / cs_interval_tensor.cu / cs_interval_fp4.cu / cs_interval_pair.cu (a2) and cs_action.cu (a3).
+// cs_poset.cu (NEXT-3), cs_build.cu (a1), cs_interval_popc.cu / cs_interval_tensor.cu / cs_interval_fp4.cu / cs_interval_pair.cu (a2) and cs_action.cu (a3).
 #include "cs_common.cuh"
 
 namespace cs {
@@ -206,6 +206,29 @@ int cs_smeared_action(const int64_t *hist, int64_t kmax, int64_t N, int dim, dou
     if (!hist || !action || N < 0) return CS_ERR_ARG;
     kmax = clamp_kmax(N, kmax);
     return launch_smeared_action(hist, kmax + 1, 1, kmax, N, dim, eps, action, static_cast<cudaStream_t>(stream));
+}
+
+size_t cs_poset_workspace(int64_t N) { return N < 0 ? 0 : poset_workspace_bytes(N); }
+
+int cs_chain_heights(const uint64_t *bits, const uint64_t *bitsT, int64_t N, int64_t source,
+                     int32_t *height, int64_t *longest, void *workspace, size_t workspace_bytes, void *stream)
+{
+    if (N < 0 || source < -1 || source >= N) return CS_ERR_ARG;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    if (longest) CS_CUDA(cudaMemsetAsync(longest, 0, sizeof(int64_t), st));
+    if (N == 0) return CS_OK;
+    if (!bits || !bitsT || !height) return CS_ERR_ARG;
+    if (!workspace || workspace_bytes < poset_workspace_bytes(N) || ((uintptr_t)workspace & 255)) return CS_ERR_WORKSPACE;
+    return launch_chain_heights(bits, bitsT, N, source, height, longest, workspace, st);
+}
+
+int cs_greedy_antichain(const uint64_t *bits, const uint64_t *bitsT, int64_t N, int64_t seed,
+                        uint64_t *member, int64_t *size, void *workspace, size_t workspace_bytes, void *stream)
+{
+    if (N <= 0 || seed < 0 || seed >= N) return CS_ERR_ARG;
+    if (!bits || !bitsT || !member) return CS_ERR_ARG;
+    if (!workspace || workspace_bytes < poset_workspace_bytes(N) || ((uintptr_t)workspace & 255)) return CS_ERR_WORKSPACE;
+    return launch_greedy_antichain(bits, bitsT, N, seed, member, size, workspace, static_cast<cudaStream_t>(stream));
 }
 
 // ---- batched ensemble ----------------------------------------------------------------------

@@ -77,6 +77,11 @@ bool interval_tensor_available();
 int launch_bd_action(const int64_t *hist, int64_t hist_stride, int64_t B, int64_t kmax, int64_t N, int dim,
                      double *action, int64_t *bracket, int64_t *hist4, cudaStream_t st);
 
+size_t poset_workspace_bytes(int64_t N);
+int launch_chain_heights(const uint64_t *bits, const uint64_t *bitsT, int64_t N, int64_t source,
+                         int32_t *height, int64_t *longest, void *ws, cudaStream_t st);
+int launch_greedy_antichain(const uint64_t *bits, const uint64_t *bitsT, int64_t N, int64_t seed,
+                            uint64_t *member, int64_t *size, void *ws, cudaStream_t st);
 int launch_smeared_action(const int64_t *hist, int64_t hist_stride, int64_t B, int64_t kmax, int64_t N, int dim,
                           double eps, double *action, cudaStream_t st);
 

@@ -427,3 +427,82 @@ def test_smeared_action_tends_to_einstein_hilbert(api):
         assert abs(mean - target) < 3.5 * sd / math.sqrt(10), (N, mean, sd)
         assert mean > 0.5 * target                                    # N = 2^12 gives 0.4 +- 0.3: not yet converged
     assert 0.8 < sds[1 << 15] / sds[1 << 14] < 2.5                    # ~ sqrt(2), ten samples each
+
+
+# ----------------------------------------------------------------------------- NEXT-3: chains, antichains
+def _unpack_member(member, N):
+    return np.unpackbits(member.cpu().numpy().view(np.uint8), bitorder="little")[:N]
+
+
+@pytest.mark.parametrize("geom,dim", GEOMS)
+@pytest.mark.parametrize("N", [1, 2, 65, 700, 1500])
+def test_chain_heights_bit_exact(api, oracle, geom, dim, N):
+    coords = inp.sprinkle(geom, dim, N, 31 * N + dim)
+    C = oracle.causal_matrix_bytes(coords, geom)
+    bits, bitsT = gpu_bits(api, coords, geom)
+    h, longest = api.chain_heights(bits, bitsT, N)
+    o_h, o_best = oracle.chain_heights(C)
+    assert np.array_equal(h.cpu().numpy(), o_h) and int(longest[0]) == o_best
+    rng = np.random.default_rng(N)
+    for source in {0, N // 2, int(rng.integers(0, N))}:
+        h, longest = api.chain_heights(bits, bitsT, N, source=source)
+        o_h, o_best = oracle.chain_heights(C, source=source)
+        assert np.array_equal(h.cpu().numpy(), o_h) and int(longest[0]) == o_best
+        # Algorithm 11 for a related pair = height - 1
+        js = np.flatnonzero(C[source])
+        if len(js):
+            j = int(js[len(js) // 2])
+            assert oracle.chain_pair(C, source, j) == int(h[j]) - 1
+
+
+def test_chain_heights_closed_forms(api, oracle):
+    for N in (300, 1025):
+        c = inp.chain_lightcone(N)
+        bits, bitsT = gpu_bits(api, c, inp.GEOM_MINK2_LIGHTCONE)
+        h, longest = api.chain_heights(bits, bitsT, N)
+        assert int(longest[0]) == N and np.array_equal(h.cpu().numpy(), np.arange(1, N + 1))
+        a = inp.antichain_lightcone(N)
+        bits, bitsT = gpu_bits(api, a, inp.GEOM_MINK2_LIGHTCONE)
+        h, longest = api.chain_heights(bits, bitsT, N)
+        assert int(longest[0]) == 1 and bool((h == 1).all())
+        m, size = api.greedy_antichain(bits, bitsT, N, 5)
+        assert int(size[0]) == N and _unpack_member(m, N).all()
+    z = torch.zeros((0, 0), dtype=torch.int64, device="cuda")
+    assert int(api.chain_heights(z, z, 0)[1][0]) == 0
+    with pytest.raises(RuntimeError):
+        api.chain_heights(bits, bitsT, N, source=N)
+    with pytest.raises(RuntimeError):
+        api.greedy_antichain(bits, bitsT, N, -1)
+
+
+@pytest.mark.parametrize("geom,dim,N", [(inp.GEOM_MINK2_LIGHTCONE, 2, 900), (inp.GEOM_MINK_CONE, 4, 1100),
+                                        (inp.GEOM_MINK_CONE, 3, 333), (inp.GEOM_DS2_SLAB, 2, 1000)])
+def test_greedy_antichain_bit_exact(api, oracle, geom, dim, N):
+    coords = inp.sprinkle(geom, dim, N, 17 + N)
+    C = oracle.causal_matrix_bytes(coords, geom)
+    bits, bitsT = gpu_bits(api, coords, geom)
+    for seed in (0, N // 3, N - 1):
+        m, size = api.greedy_antichain(bits, bitsT, N, seed)
+        want = oracle.greedy_antichain(C, seed)
+        assert np.array_equal(_unpack_member(m, N), want) and int(size[0]) == int(want.sum())
+        assert int(m.cpu().numpy().view(np.uint64)[(N + 63) // 64:].sum()) == 0     # padding words stay zero
+
+
+def test_longest_chain_config2_is_lis(api):
+    """Full config 2 (N = 16384): the longest chain of the 1+1 diamond is the longest increasing subsequence
+    (patience sorting on the host: a property that holds at any size)."""
+    import bisect
+    cfg = inp.CONFIGS[2]
+    coords = inp.make_config_coords(cfg)
+    bits, bitsT = gpu_bits(api, coords, cfg.geometry)
+    h, longest = api.chain_heights(bits, bitsT, cfg.N)
+    piles = []
+    for v in coords[np.argsort(coords[:, 0], kind="stable"), 1]:
+        k = bisect.bisect_left(piles, v)
+        if k == len(piles):
+            piles.append(v)
+        else:
+            piles[k] = v
+    assert int(longest[0]) == len(piles)
+    hh = h.cpu().numpy()
+    assert hh.min() == 1 and np.array_equal(np.unique(hh), np.arange(1, len(piles) + 1))
