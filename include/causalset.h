@@ -99,6 +99,13 @@ int cs_transpose_bits(const uint64_t *bits, int64_t N, uint64_t *bitsT, void *st
  *   out  device, int64[2] = {R, W_alg}, overwritten. */
 int cs_relation_stats(const uint64_t *bits, int64_t N, int64_t *out, void *stream);
 
+/* Degree vectors (the by-product of the paper's linker, Alg. 17):
+ *   outdeg[k] = number of elements in the future of k (row sum of bits),
+ *   indeg[k]  = number of elements in its past (row sum of bitsT).
+ * Both device, int64[N]; either may be NULL (indeg needs bitsT).  sum_k indeg[k] outdeg[k] is the number of
+ * 3-chains = sum_k k hist[k] (used as a whole-size check of a2). */
+int cs_degrees(const uint64_t *bits, const uint64_t *bitsT, int64_t N, int64_t *outdeg, int64_t *indeg, void *stream);
+
 /* a2: interval abundances (Alg. 19; Alg. 20).
  * For every related pair i -< j:  c = |{k : i -< k -< j}| = popcount(bits[i] & bitsT[j]);  hist[c] += 1.
  * hist[k] = n_{k+1} in the paper's notation (Eq. 4.8).

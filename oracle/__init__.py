@@ -9,6 +9,7 @@ from .oracle import (  # noqa: F401
     GEOM_MINK2_LIGHTCONE,
     GEOM_MINK_CONE,
     GEOM_DS2_SLAB,
+    GEOM_FLRW_POLAR,
     build,
     row_stride_words,
     relation,

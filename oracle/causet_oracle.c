@@ -41,7 +41,7 @@
 #include <omp.h>
 #endif
 
-enum { ORC_GEOM_MINK2_LIGHTCONE = 0, ORC_GEOM_MINK_CONE = 1, ORC_GEOM_DS2_SLAB = 2 };
+enum { ORC_GEOM_MINK2_LIGHTCONE = 0, ORC_GEOM_MINK_CONE = 1, ORC_GEOM_DS2_SLAB = 2, ORC_GEOM_FLRW_POLAR = 3 };
 
 /* 2*pi as the fp64 nearest to the real number (bit pattern 0x401921FB54442D18). */
 static const double ORC_TWO_PI = 6.283185307179586476925286766559;
@@ -56,6 +56,13 @@ static const double ORC_TWO_PI = 6.283185307179586476925286766559;
  *  DS2_SLAB:        (eta,theta), metric conformal to the cylinder (Eq. 4.19,
  *                   PAPER.md:1949-1951): d_eta >= min(|d_theta|, 2pi-|d_theta|)
  *                   (readings A1, A3).
+ *  FLRW_POLAR:      (NEXT-4) conformally flat 3+1 FLRW in conformal time and spherical coordinates,
+ *                   Eq. 7.7 as printed, strict:
+ *                     r_i^2 + r_j^2 - 2 r_i r_j (cos th_i cos th_j + sin th_i sin th_j cos(ph_i - ph_j)) < (eta_i - eta_j)^2
+ *                   A point is (eta, r, cos th, sin th, cos ph, sin ph): the trigonometric values are inputs
+ *                   (taken once per point, not once per pair), and cos(ph_i - ph_j) is expanded as
+ *                   cos ph_i cos ph_j + sin ph_i sin ph_j, so the predicate is additions and multiplications
+ *                   only (reading A17).  j is in the future of i only if eta_j > eta_i.
  */
 int orc_relation(const double *xi, const double *xj, int dim, int geom)
 {
@@ -80,6 +87,12 @@ int orc_relation(const double *xi, const double *xj, int dim, int geom)
         double b = ORC_TWO_PI - a;
         double m = (a < b) ? a : b;
         return deta >= m;
+    } else if (geom == ORC_GEOM_FLRW_POLAR) {
+        double deta = xj[0] - xi[0];
+        double cphi = (xi[4] * xj[4]) + (xi[5] * xj[5]);
+        double ang = (xi[2] * xj[2]) + ((xi[3] * xj[3]) * cphi);
+        double d2 = ((xi[1] * xi[1]) + (xj[1] * xj[1])) - ((2.0 * (xi[1] * xj[1])) * ang);
+        return (deta > 0.0) && (d2 < deta * deta);
     }
     return 0;
 }
@@ -89,6 +102,7 @@ static int orc_geom_ok(int dim, int geom)
     if (geom == ORC_GEOM_MINK2_LIGHTCONE) return dim == 2;
     if (geom == ORC_GEOM_MINK_CONE) return dim >= 2 && dim <= 4;
     if (geom == ORC_GEOM_DS2_SLAB) return dim == 2;
+    if (geom == ORC_GEOM_FLRW_POLAR) return dim == 6;
     return 0;
 }
 

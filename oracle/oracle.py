@@ -17,6 +17,7 @@ import numpy as np
 GEOM_MINK2_LIGHTCONE = 0
 GEOM_MINK_CONE = 1
 GEOM_DS2_SLAB = 2
+GEOM_FLRW_POLAR = 3
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "causet_oracle.c")
@@ -248,5 +249,5 @@ def action_pipeline(coords, geom: int, tier: int = 1):
     else:
         bits = causal_matrix_bits(c, geom)
         hist, _, _ = interval_hist_alg20(bits, N)
-    S, br = bd_action(hist, N, dim)
+    S, br = bd_action(hist, N, 4 if geom == GEOM_FLRW_POLAR else dim)    # six coordinates, 3+1 dimensions
     return bits, hist, S, br

@@ -43,6 +43,7 @@ _SIGNATURES = {
     "cs_causal_matrix": (_int, [_p, _i64, _int, _int, _p, _p, _p]),
     "cs_causal_matrix_batched": (_int, [_p, _i64, _i64, _int, _int, _p, _p, _p]),
     "cs_transpose_bits": (_int, [_p, _i64, _p, _p]),
+    "cs_degrees": (_int, [_p, _p, _i64, _p, _p, _p]),
     "cs_relation_stats": (_int, [_p, _i64, _p, _p]),
     "cs_interval_hist_workspace": (_sz, [_i64, _i64, _int, _int]),
     "cs_interval_hist": (_int, [_p, _p, _i64, _i64, _p, _p, _p, _sz, _p]),
@@ -213,6 +214,16 @@ def bd_action(hist: torch.Tensor, N: int, dim: int, return_bracket: bool = False
     _check(load().cs_bd_action(_dptr(hist), hist.numel() - 1, N, dim, _dptr(action), _dptr(bracket), _stream()),
            "cs_bd_action")
     return (action, bracket) if return_bracket else action
+
+
+def degrees(bits: torch.Tensor, bitsT: torch.Tensor, N: int):
+    """-> (outdeg, indeg) int64[N] on the device."""
+    _need_cuda(bits, torch.int64, "bits")
+    _need_cuda(bitsT, torch.int64, "bitsT")
+    outdeg = torch.empty(N, dtype=torch.int64, device=bits.device)
+    indeg = torch.empty(N, dtype=torch.int64, device=bits.device)
+    _check(load().cs_degrees(_dptr(bits), _dptr(bitsT), N, _dptr(outdeg), _dptr(indeg), _stream()), "cs_degrees")
+    return outdeg, indeg
 
 
 def chain_heights(bits: torch.Tensor, bitsT: torch.Tensor, N: int, source: int = -1):

@@ -143,6 +143,12 @@ int cs_relation_stats(const uint64_t *bits, int64_t N, int64_t *out, void *strea
     return launch_relation_stats(bits, N, out, static_cast<cudaStream_t>(stream));
 }
 
+int cs_degrees(const uint64_t *bits, const uint64_t *bitsT, int64_t N, int64_t *outdeg, int64_t *indeg, void *stream)
+{
+    if (N < 0 || (N > 0 && !bits) || (indeg && N > 0 && !bitsT)) return CS_ERR_ARG;
+    return launch_degrees(bits, indeg ? bitsT : nullptr, N, outdeg, indeg, static_cast<cudaStream_t>(stream));
+}
+
 size_t cs_interval_hist_workspace(int64_t N, int64_t kmax, int have_bitsT, int route)
 {
     (void)kmax;

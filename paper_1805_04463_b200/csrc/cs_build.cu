@@ -457,6 +457,46 @@ int launch_transpose_bits(const uint64_t *bits, int64_t B, int64_t N, uint64_t *
     return CS_OK;
 }
 
+// ---- degree vectors -----------------------------------------------------------------------
+// out-degree(k) = |J+(k)| = popcount(bits[k]), in-degree(k) = |J-(k)| = popcount(bitsT[k]): the vectors the
+// paper's linker accumulates next to the matrix (Alg. 17).  One warp per row.
+__global__ void __launch_bounds__(256)
+k_degrees(const uint64_t *__restrict__ bits, const uint64_t *__restrict__ bitsT, int64_t N, int64_t stride,
+          int64_t *__restrict__ outdeg, int64_t *__restrict__ indeg)
+{
+    const int lane = threadIdx.x & 31;
+    const int64_t warp_global = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    const int64_t nwarps = ((int64_t)gridDim.x * blockDim.x) >> 5;
+    for (int64_t k = warp_global; k < N; k += nwarps) {
+        long long o = 0, i = 0;
+        for (int64_t w = lane; w < stride; w += 32) {
+            o += __popcll(bits[k * stride + w]);
+            if (bitsT) i += __popcll(bitsT[k * stride + w]);
+        }
+#pragma unroll
+        for (int s = 16; s >= 1; s >>= 1) {
+            o += __shfl_xor_sync(0xffffffffu, o, s);
+            i += __shfl_xor_sync(0xffffffffu, i, s);
+        }
+        if (lane == 0) {
+            if (outdeg) outdeg[k] = o;
+            if (indeg) indeg[k] = i;
+        }
+    }
+}
+
+int launch_degrees(const uint64_t *bits, const uint64_t *bitsT, int64_t N, int64_t *outdeg, int64_t *indeg, cudaStream_t st)
+{
+    if (N == 0) return CS_OK;
+    const int64_t stride = row_stride_words(N);
+    int blocks = sm_count() * 8;
+    const int64_t need = (N + 7) / 8;
+    if (need < blocks) blocks = (int)need;
+    k_degrees<<<blocks, 256, 0, st>>>(bits, bitsT, N, stride, outdeg, indeg);
+    CS_LAUNCHED("k_degrees");
+    return CS_OK;
+}
+
 // ---- relation statistics ------------------------------------------------------------------
 // out[0] = R = popcount(bits); out[1] = W_alg = sum_{i -< j} ((j>>6) - (i>>6) + 1)
 __global__ void __launch_bounds__(256)

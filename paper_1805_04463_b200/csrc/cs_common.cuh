@@ -53,6 +53,7 @@ int sm_count();   // SMs of the current device (cached)
 int launch_causal_matrix(const double *coords, int64_t B, int64_t N, int dim, int geometry,
                          uint64_t *bits, uint64_t *bitsT, cudaStream_t st);
 int launch_transpose_bits(const uint64_t *bits, int64_t B, int64_t N, uint64_t *bitsT, cudaStream_t st);
+int launch_degrees(const uint64_t *bits, const uint64_t *bitsT, int64_t N, int64_t *outdeg, int64_t *indeg, cudaStream_t st);
 int launch_relation_stats(const uint64_t *bits, int64_t N, int64_t *out, cudaStream_t st);
 
 // hist (int64[B][kmax+1]) and nrel (int64[B] or NULL) must be zeroed by the caller.

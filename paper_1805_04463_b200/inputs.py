@@ -28,6 +28,7 @@ import numpy as np
 GEOM_MINK2_LIGHTCONE = 0
 GEOM_MINK_CONE = 1
 GEOM_DS2_SLAB = 2
+GEOM_FLRW_POLAR = 3
 
 _GAMMA = np.uint64(0x9E3779B97F4A7C15)
 _M1 = np.uint64(0xBF58476D1CE4E5B9)
@@ -96,6 +97,20 @@ def sprinkle_ds2_slab(N: int, seed: int, eta_a: float = -1.2, eta_b: float = -0.
     return _sort_rows(c, eta, theta)
 
 
+def sprinkle_flrw_polar(N: int, seed: int, eta0: float = 1.0, r0: float = 0.7) -> np.ndarray:
+    """[N][6] = (eta, r, cos th, sin th, cos ph, sin ph) for the Eq. 7.7 predicate: conformal time
+    eta ~ U[0, eta0), points uniform in the ball r < r0 (r = r0 u^(1/3), cos th = 2u - 1, ph = 2 pi u); draws per
+    point in the order eta, r, th, ph.  The trigonometric values are part of the input."""
+    r = uniform01(seed, 0, 4 * N).reshape(N, 4)
+    eta = eta0 * r[:, 0]
+    rad = r0 * np.cbrt(r[:, 1])
+    ct = 2.0 * r[:, 2] - 1.0
+    st = np.sqrt(np.maximum(0.0, 1.0 - ct * ct))
+    ph = (2.0 * np.pi) * r[:, 3]
+    c = np.stack([eta, rad, ct, st, np.cos(ph), np.sin(ph)], axis=1)
+    return _sort_rows(c, eta, rad)
+
+
 def chain_lightcone(N: int) -> np.ndarray:
     """Total order: u_i = v_i = i/N (sorted already)."""
     u = np.arange(N, dtype=np.float64) / max(N, 1)
@@ -145,6 +160,8 @@ def sprinkle(geometry: int, dim: int, N: int, seed: int) -> np.ndarray:
         return _sprinkle_mink_low(N, dim, seed)
     if geometry == GEOM_DS2_SLAB and dim == 2:
         return sprinkle_ds2_slab(N, seed)
+    if geometry == GEOM_FLRW_POLAR and dim == 6:
+        return sprinkle_flrw_polar(N, seed)
     raise ValueError("no sprinkler for geometry=%d dim=%d" % (geometry, dim))
 
 

@@ -429,6 +429,21 @@ def test_smeared_action_tends_to_einstein_hilbert(api):
     assert 0.8 < sds[1 << 15] / sds[1 << 14] < 2.5                    # ~ sqrt(2), ten samples each
 
 
+@pytest.mark.parametrize("geom,dim", GEOMS)
+def test_degree_vectors(api, oracle, geom, dim):
+    N = 1111
+    coords = inp.sprinkle(geom, dim, N, 5 + dim)
+    o_bits = oracle.causal_matrix_bits(coords, geom)
+    bits, bitsT = gpu_bits(api, coords, geom)
+    outdeg, indeg = api.degrees(bits, bitsT, N)
+    o_out, o_in = oracle.degrees(o_bits, N)
+    assert np.array_equal(outdeg.cpu().numpy(), o_out) and np.array_equal(indeg.cpu().numpy(), o_in)
+    # the 3-chain identity on the device's own histogram
+    h = api.interval_hist(bits, bitsT, N)
+    k = torch.arange(h.numel(), device="cuda", dtype=torch.int64)
+    assert int((k * h).sum()) == int((outdeg * indeg).sum())
+
+
 # ----------------------------------------------------------------------------- NEXT-3: chains, antichains
 def _unpack_member(member, N):
     return np.unpackbits(member.cpu().numpy().view(np.uint8), bitorder="little")[:N]

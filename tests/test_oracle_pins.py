@@ -421,3 +421,34 @@ def test_degrees_helper(oracle):
     C = oracle.causal_matrix_bytes(coords, inp.GEOM_MINK_CONE)
     o, i = oracle.degrees(oracle.pack_bytes(C), 333)
     assert np.array_equal(o, C.sum(axis=1)) and np.array_equal(i, C.sum(axis=0))
+
+
+def test_flrw_polar_relation(oracle):
+    """Eq. 7.7: hand cases (law of cosines along one ray, opposite rays, the null
+    pair is NOT related -- the paper's strict '<'), and agreement with the flat cone in Cartesian
+    coordinates for every pair away from the cone (FLRW is conformally flat)."""
+    def pt(eta, r, th, ph):
+        return np.array([eta, r, math.cos(th), math.sin(th), math.cos(ph), math.sin(ph)])
+    g = oracle.GEOM_FLRW_POLAR
+    assert oracle.relation(pt(0.0, 0.5, 0.3, 1.0), pt(0.25, 0.7, 0.3, 1.0), g)          # same ray: |dr| = 0.2 < 0.25
+    assert not oracle.relation(pt(0.0, 0.5, 0.3, 1.0), pt(0.15, 0.7, 0.3, 1.0), g)      # 0.2 > 0.15
+    assert not oracle.relation(pt(0.25, 0.7, 0.3, 1.0), pt(0.0, 0.5, 0.3, 1.0), g)      # time order
+    assert oracle.relation(pt(0.0, 0.25, 0.0, 0.0), pt(0.625, 0.25, math.pi, 0.0), g)   # opposite poles: 0.5 < 0.625
+    assert not oracle.relation(pt(0.0, 0.25, 0.0, 0.0), pt(0.5, 0.25, math.pi, 0.0), g) # null: strict
+    assert not oracle.relation(pt(0.0, 0.0, 0.0, 0.0), pt(0.0, 0.0, 0.0, 0.0), g)       # same event
+    N = 400
+    c = inp.sprinkle_flrw_polar(N, 12)
+    assert np.all(np.diff(c[:, 0]) >= 0) and np.allclose(c[:, 2] ** 2 + c[:, 3] ** 2, 1) and np.allclose(c[:, 4] ** 2 + c[:, 5] ** 2, 1)
+    C = oracle.causal_matrix_bytes(c, g)
+    x = c[:, 1] * c[:, 3] * c[:, 4]; y = c[:, 1] * c[:, 3] * c[:, 5]; z = c[:, 1] * c[:, 2]
+    dt = c[None, :, 0] - c[:, None, 0]
+    q = dt ** 2 - ((x[None] - x[:, None]) ** 2 + (y[None] - y[:, None]) ** 2 + (z[None] - z[:, None]) ** 2)
+    want = np.triu((dt > 0) & (q > 0), 1)
+    clear = np.triu(np.abs(q) > 1e-12, 1)
+    assert np.array_equal(C.astype(bool)[clear], want[clear]) and 0.02 < want.mean() < 0.4
+    # transitive and acyclic like every other geometry
+    Cb = C.astype(bool)
+    assert not (Cb.astype(np.int32) @ Cb.astype(np.int32) > 0)[~Cb & np.triu(np.ones_like(Cb), 1)].any()
+    # the action pipeline treats it as 3+1 dimensional
+    _, hist, S, I = oracle.action_pipeline(c, g)
+    assert I == N - hist[0] + 9 * hist[1] - 16 * hist[2] + 8 * hist[3]
