@@ -46,7 +46,15 @@ enum cs_geometry {
     /* dim = 2, coords (eta,theta) of the 1+1 de Sitter slab (Eq. 4.19):
        a = |theta_j - theta_i|, b = 2pi - a, m = a < b ? a : b,
        i -< j  <=>  eta_j - eta_i >= m           (2pi = 0x401921FB54442D18). */
-    CS_GEOM_DS2_SLAB = 2
+    CS_GEOM_DS2_SLAB = 2,
+    /* dim = 6, a point is (eta, r, cos th, sin th, cos ph, sin ph): conformally flat 3+1 FLRW in conformal
+       time and spherical coordinates, Eq. 7.7, strict as printed; cos(ph_i - ph_j) is
+       expanded, so the trigonometric values are taken once per point by the caller:
+       cphi = (cp_i*cp_j) + (sp_i*sp_j), ang = (ct_i*ct_j) + ((st_i*st_j)*cphi),
+       d2 = ((r_i*r_i) + (r_j*r_j)) - ((2*(r_i*r_j))*ang), deta = eta_j - eta_i,
+       i -< j  <=>  deta > 0 && d2 < deta*deta   (fp64, no FMA contraction).
+       The spacetime dimension (for the action entry points that take coordinates) is 4. */
+    CS_GEOM_FLRW_POLAR = 3
 };
 
 enum cs_status {

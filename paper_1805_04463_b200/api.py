@@ -20,6 +20,7 @@ GEOM_MINK2_LIGHTCONE = 0
 GEOM_MINK_CONE = 1
 GEOM_DS2_SLAB = 2
 
+GEOM_FLRW_POLAR = 3   # include/causalset.h
 ROUTE_AUTO = 0
 ROUTE_POPC = 1
 ROUTE_TENSOR = 2

@@ -22,6 +22,10 @@ int sm_count()
     return cached;
 }
 
+// spacetime dimension of a point set: the number of coordinates, except for the FLRW geometry whose six
+// numbers per point describe a 3+1 dimensional event
+static int spacetime_dim(int geometry, int dim) { return geometry == CS_GEOM_FLRW_POLAR ? 4 : dim; }
+
 static int resolve_route(int64_t N, int route)
 {
     if (route == CS_ROUTE_AUTO) route = cs_default_route(N);
@@ -116,8 +120,9 @@ int cs_causal_matrix_batched(const double *coords, int64_t B, int64_t N, int dim
                              uint64_t *bits, uint64_t *bitsT, void *stream)
 {
     if (N < 0 || B < 0) return CS_ERR_ARG;
-    if (geometry < CS_GEOM_MINK2_LIGHTCONE || geometry > CS_GEOM_DS2_SLAB) return CS_ERR_GEOM;
-    if (geometry == CS_GEOM_MINK_CONE ? (dim < 2 || dim > 4) : (dim != 2)) return CS_ERR_DIM;
+    if (geometry < CS_GEOM_MINK2_LIGHTCONE || geometry > CS_GEOM_FLRW_POLAR) return CS_ERR_GEOM;
+    if (geometry == CS_GEOM_MINK_CONE ? (dim < 2 || dim > 4) : (dim != (geometry == CS_GEOM_FLRW_POLAR ? 6 : 2)))
+        return CS_ERR_DIM;
     if (N == 0 || B == 0) return CS_OK;
     if (!coords || !bits) return CS_ERR_ARG;
     return launch_causal_matrix(coords, B, N, dim, geometry, bits, bitsT, static_cast<cudaStream_t>(stream));
@@ -272,7 +277,7 @@ int cs_bd_action_batched(const double *coords, int64_t B, int64_t N, int dim, in
     rc = interval_hist_impl(bits, bitsT, B, N, kmax, 0, N, CS_ROUTE_AUTO, hist_k, nullptr, iws,
                             workspace_bytes - (size_t)(iws - ws), st);
     if (rc) return rc;
-    return launch_bd_action(hist_k, kmax + 1, B, kmax, N, dim, actions, nullptr, hist4, st);
+    return launch_bd_action(hist_k, kmax + 1, B, kmax, N, spacetime_dim(geometry, dim), actions, nullptr, hist4, st);
 }
 
 // ---- end to end with host buffers ----------------------------------------------------------
@@ -282,7 +287,7 @@ size_t cs_action_host_workspace(int64_t N, int64_t kmax)
     if (N < 0) return 0;
     kmax = clamp_kmax(N, kmax);
     const size_t mat = align_up((size_t)N * row_stride_words(N) * 8, 256);
-    return align_up((size_t)N * 4 * 8, 256) + 2 * mat + align_up((size_t)(kmax + 1) * 8, 256) + 256 +
+    return align_up((size_t)N * 6 * 8, 256) + 2 * mat + align_up((size_t)(kmax + 1) * 8, 256) + 256 +
            interval_ws_bytes(1, N, 1, cs_default_route(N));
 }
 
@@ -291,7 +296,7 @@ int cs_action_host(const double *coords_host, int64_t N, int dim, int geometry, 
                    void *workspace, size_t workspace_bytes, void *stream)
 {
     if (N < 0 || !hist_host || !action_host || (N > 0 && !coords_host)) return CS_ERR_ARG;
-    if (dim < 2 || dim > 4) return CS_ERR_DIM;
+    if (dim < 2 || dim > 6) return CS_ERR_DIM;
     if (!workspace || workspace_bytes < cs_action_host_workspace(N, kmax) || ((uintptr_t)workspace & 255))
         return CS_ERR_WORKSPACE;
     cudaStream_t st = static_cast<cudaStream_t>(stream);
@@ -299,7 +304,7 @@ int cs_action_host(const double *coords_host, int64_t N, int dim, int geometry, 
     const size_t mat = align_up((size_t)N * row_stride_words(N) * 8, 256);
     unsigned char *ws = static_cast<unsigned char *>(workspace);
     double *coords = reinterpret_cast<double *>(ws);
-    ws += align_up((size_t)N * 4 * 8, 256);
+    ws += align_up((size_t)N * 6 * 8, 256);
     uint64_t *bits = reinterpret_cast<uint64_t *>(ws);
     ws += mat;
     uint64_t *bitsT = reinterpret_cast<uint64_t *>(ws);
@@ -315,7 +320,7 @@ int cs_action_host(const double *coords_host, int64_t N, int dim, int geometry, 
     if (rc) return rc;
     rc = cs_interval_hist(bits, bitsT, N, kmax, hist, nullptr, ws, left, stream);
     if (rc) return rc;
-    rc = cs_bd_action(hist, kmax, N, dim, action, nullptr, stream);
+    rc = cs_bd_action(hist, kmax, N, spacetime_dim(geometry, dim), action, nullptr, stream);
     if (rc) return rc;
     CS_CUDA(cudaMemcpyAsync(hist_host, hist, (size_t)(kmax + 1) * 8, cudaMemcpyDeviceToHost, st));
     CS_CUDA(cudaMemcpyAsync(action_host, action, 8, cudaMemcpyDeviceToHost, st));

@@ -62,6 +62,19 @@ struct Pred<CS_GEOM_DS2_SLAB, 2> {
     }
 };
 
+template <>
+struct Pred<CS_GEOM_FLRW_POLAR, 6> {
+    __device__ static __forceinline__ bool rel(const double *xi, const double *xj)
+    {
+        const double deta = __dsub_rn(xj[0], xi[0]);
+        const double cphi = __dadd_rn(__dmul_rn(xi[4], xj[4]), __dmul_rn(xi[5], xj[5]));
+        const double ang = __dadd_rn(__dmul_rn(xi[2], xj[2]), __dmul_rn(__dmul_rn(xi[3], xj[3]), cphi));
+        const double d2 = __dsub_rn(__dadd_rn(__dmul_rn(xi[1], xi[1]), __dmul_rn(xj[1], xj[1])),
+                                    __dmul_rn(__dmul_rn(2.0, __dmul_rn(xi[1], xj[1])), ang));
+        return (deta > 0.0) && (d2 < __dmul_rn(deta, deta));
+    }
+};
+
 // ---- exact single-precision prefilter (flat cone) ----------------------------------------------
 // With h = (t^2 - |x|^2) / 2 the sign of the interval is the sign of
 //     T = ((t_j - t_i)^2 - |x_j - x_i|^2) / 2 = h_i + h_j - t_i t_j + x_i . x_j ,
@@ -407,6 +420,9 @@ int launch_causal_matrix(const double *coords, int64_t B, int64_t N, int dim, in
     case CS_GEOM_DS2_SLAB:
         if (dim != 2) return CS_ERR_DIM;
         return launch_build_t<CS_GEOM_DS2_SLAB, 2>(coords, B, N, stride, bits, bitsT, st);
+    case CS_GEOM_FLRW_POLAR:
+        if (dim != 6) return CS_ERR_DIM;
+        return launch_build_t<CS_GEOM_FLRW_POLAR, 6>(coords, B, N, stride, bits, bitsT, st);
     default:
         return CS_ERR_GEOM;
     }

@@ -19,6 +19,7 @@ GEOMS = [
     (inp.GEOM_MINK_CONE, 3),
     (inp.GEOM_MINK_CONE, 4),
     (inp.GEOM_DS2_SLAB, 2),
+    (inp.GEOM_FLRW_POLAR, 6),          # NEXT-4: Eq. 7.7
 ]
 
 
@@ -442,6 +443,32 @@ def test_degree_vectors(api, oracle, geom, dim):
     h = api.interval_hist(bits, bitsT, N)
     k = torch.arange(h.numel(), device="cuda", dtype=torch.int64)
     assert int((k * h).sum()) == int((outdeg * indeg).sum())
+
+
+def test_flrw_polar_pipeline(api, oracle):
+    """NEXT-4 (Eq. 7.7): bits incl. pairs on and one ulp off the cone, histogram, 3+1 action, host entry point."""
+    N = 1800
+    coords = inp.sprinkle_flrw_polar(N, 3)
+    # partners along the same ray at exactly / just beyond / just short of null separation
+    extra = coords[:200].copy()
+    extra[:, 0] = coords[:200, 0] + 0.125
+    extra[:, 1] = coords[:200, 1] + 0.125
+    e2 = extra.copy(); e2[:, 0] = np.nextafter(extra[:, 0], 10.0)
+    e3 = extra.copy(); e3[:, 0] = np.nextafter(extra[:, 0], -10.0)
+    coords = np.concatenate([coords, extra, e2, e3])
+    coords = np.ascontiguousarray(coords[np.lexsort((coords[:, 1], coords[:, 0]))])
+    N = coords.shape[0]
+    o_bits, o_hist, o_S, o_I = oracle.action_pipeline(coords, inp.GEOM_FLRW_POLAR, tier=1)
+    bits, bitsT = gpu_bits(api, coords, inp.GEOM_FLRW_POLAR)
+    assert np.array_equal(to_u64(bits), o_bits)
+    hist = api.interval_hist(bits, bitsT, N)
+    assert np.array_equal(hist.cpu().numpy(), o_hist)
+    S, I = api.bd_action(hist, N, 4, return_bracket=True)
+    assert int(I[0]) == o_I and float(S[0]) == o_S
+    h_host, s_host = api.action_host(torch.from_numpy(coords).pin_memory(), inp.GEOM_FLRW_POLAR)
+    assert np.array_equal(h_host.numpy(), o_hist) and float(s_host[0]) == o_S
+    with pytest.raises(RuntimeError):
+        api.causal_matrix(torch.zeros((10, 4), dtype=torch.float64, device="cuda"), inp.GEOM_FLRW_POLAR)
 
 
 # ----------------------------------------------------------------------------- NEXT-3: chains, antichains
