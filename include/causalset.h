@@ -218,6 +218,20 @@ int cs_action_host(const double *coords_host, int64_t N, int dim, int geometry, 
                    int64_t *hist_host, double *action_host,
                    void *workspace, size_t workspace_bytes, void *stream);
 
+/* The ensemble end to end with HOST buffers (the Monte-Carlo use): B causets of N points each,
+ * processed in chunks of up to 512 causets; the coordinates of the next chunk are copied on a library-owned
+ * stream while `stream` builds and reduces the current one, so the PCIe time hides behind the kernels.  Copies the
+ * actions (and N_0..N_3 per causet) back and synchronises `stream` before returning.
+ *   coords_host   host, [B][N][dim] fp64; pinned memory is needed for the copies to overlap.
+ *   actions_host  host, double[B], overwritten.
+ *   hist4_host    host, int64[B][4] or NULL.
+ *   workspace     device, >= cs_bd_action_batched_host_workspace(B, N, dim) bytes, 256-byte aligned.
+ * Errors: CS_ERR_ARG, CS_ERR_DIM, CS_ERR_GEOM, CS_ERR_WORKSPACE, CS_ERR_CUDA. */
+size_t cs_bd_action_batched_host_workspace(int64_t B, int64_t N, int dim);
+int cs_bd_action_batched_host(const double *coords_host, int64_t B, int64_t N, int dim, int geometry,
+                              double *actions_host, int64_t *hist4_host,
+                              void *workspace, size_t workspace_bytes, void *stream);
+
 /* Number of kernel launches issued by this library in this process so far (for bench.py's
  * `gpu_launches`). */
 int64_t cs_launch_count(void);

@@ -59,6 +59,8 @@ _SIGNATURES = {
     "cs_smeared_action": (_int, [_p, _i64, _i64, _int, ctypes.c_double, _p, _p]),
     "cs_bd_action_batched_workspace": (_sz, [_i64, _i64]),
     "cs_bd_action_batched": (_int, [_p, _i64, _i64, _int, _int, _p, _p, _p, _sz, _p]),
+    "cs_bd_action_batched_host_workspace": (_sz, [_i64, _i64, _int]),
+    "cs_bd_action_batched_host": (_int, [_p, _i64, _i64, _int, _int, _p, _p, _p, _sz, _p]),
     "cs_action_host_workspace": (_sz, [_i64, _i64]),
     "cs_action_host": (_int, [_p, _i64, _int, _int, _i64, _p, _p, _p, _sz, _p]),
     "cs_launch_count": (_i64, []),
@@ -276,6 +278,26 @@ def bd_action_batched(coords: torch.Tensor, geometry: int, workspace: torch.Tens
     _check(load().cs_bd_action_batched(_dptr(coords), B, N, dim, geometry, _dptr(actions), _dptr(hist4),
                                        _dptr(ws), ws.numel(), _stream()), "cs_bd_action_batched")
     return (actions, hist4) if return_hist4 else actions
+
+
+def bd_action_batched_host(coords_host: torch.Tensor, geometry: int, workspace: torch.Tensor | None = None,
+                           actions_host: torch.Tensor | None = None, hist4_host: torch.Tensor | None = None,
+                           device="cuda"):
+    """Ensemble end to end from HOST buffers (pinned for overlap): coords [B][N][dim] -> (actions_host fp64[B],
+    hist4_host int64[B][4]); H2D copies overlap the kernels chunk by chunk."""
+    if coords_host.is_cuda or coords_host.dtype != torch.float64 or not coords_host.is_contiguous():
+        raise TypeError("coords_host must be a contiguous CPU float64 tensor")
+    B, N, dim = coords_host.shape
+    if actions_host is None:
+        actions_host = torch.empty(B, dtype=torch.float64).pin_memory()
+    if hist4_host is None:
+        hist4_host = torch.empty((B, 4), dtype=torch.int64).pin_memory()
+    need = int(load().cs_bd_action_batched_host_workspace(B, N, dim))
+    ws = workspace if workspace is not None else _workspace(need, device)
+    _check(load().cs_bd_action_batched_host(coords_host.data_ptr(), B, N, dim, geometry, actions_host.data_ptr(),
+                                            hist4_host.data_ptr(), _dptr(ws), ws.numel(), _stream()),
+           "cs_bd_action_batched_host")
+    return actions_host, hist4_host
 
 
 def action_host_workspace(N: int, kmax: int = -1) -> int:

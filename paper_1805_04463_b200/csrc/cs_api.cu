@@ -280,6 +280,90 @@ int cs_bd_action_batched(const double *coords, int64_t B, int64_t N, int dim, in
     return launch_bd_action(hist_k, kmax + 1, B, kmax, N, spacetime_dim(geometry, dim), actions, nullptr, hist4, st);
 }
 
+// ---- ensemble end to end with host buffers: chunked, copies overlapped with compute -------------
+// The coordinates of the next chunk of causets travel over PCIe on a library-owned copy stream while the
+// caller's stream builds and reduces the current chunk; two coordinate buffers alternate, the bit matrices
+// exist for one chunk only.
+// workspace: [coords chunk x2][bits chunk][bitsT chunk][hist CB*4][actions B][hist4 B*4][interval scratch]
+static int64_t ensemble_chunk(int64_t B) { return B < 512 ? B : 512; }
+
+size_t cs_bd_action_batched_host_workspace(int64_t B, int64_t N, int dim)
+{
+    if (B < 0 || N < 0 || dim < 2 || dim > 6) return 0;
+    const int64_t CB = ensemble_chunk(B);
+    const size_t cbuf = align_up((size_t)CB * N * dim * 8, 256);
+    const size_t mat = align_up((size_t)CB * N * row_stride_words(N) * 8, 256);
+    return 2 * cbuf + 2 * mat + align_up((size_t)CB * 4 * 8, 256) + align_up((size_t)B * 8, 256) +
+           align_up((size_t)B * 4 * 8, 256) + interval_ws_bytes(CB, N, 1, cs_default_route(N));
+}
+
+int cs_bd_action_batched_host(const double *coords_host, int64_t B, int64_t N, int dim, int geometry,
+                              double *actions_host, int64_t *hist4_host,
+                              void *workspace, size_t workspace_bytes, void *stream)
+{
+    if (B < 0 || N < 0) return CS_ERR_ARG;
+    if (B == 0) return CS_OK;
+    if (!coords_host || !actions_host) return CS_ERR_ARG;
+    if (dim < 2 || dim > 6) return CS_ERR_DIM;
+    if (!workspace || workspace_bytes < cs_bd_action_batched_host_workspace(B, N, dim) || ((uintptr_t)workspace & 255))
+        return CS_ERR_WORKSPACE;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    static cudaStream_t copy_stream = nullptr;
+    static cudaEvent_t copied[2] = {nullptr, nullptr}, consumed[2] = {nullptr, nullptr}, start = nullptr;
+    if (!copy_stream) {
+        CS_CUDA(cudaStreamCreateWithFlags(&copy_stream, cudaStreamNonBlocking));
+        for (int i = 0; i < 2; i++) {
+            CS_CUDA(cudaEventCreateWithFlags(&copied[i], cudaEventDisableTiming));
+            CS_CUDA(cudaEventCreateWithFlags(&consumed[i], cudaEventDisableTiming));
+        }
+        CS_CUDA(cudaEventCreateWithFlags(&start, cudaEventDisableTiming));
+    }
+    const int64_t CB = ensemble_chunk(B);
+    const size_t cbuf = align_up((size_t)CB * N * dim * 8, 256);
+    const size_t mat = align_up((size_t)CB * N * row_stride_words(N) * 8, 256);
+    unsigned char *ws = static_cast<unsigned char *>(workspace);
+    double *cdev[2] = {reinterpret_cast<double *>(ws), reinterpret_cast<double *>(ws + cbuf)};
+    ws += 2 * cbuf;
+    uint64_t *bits = reinterpret_cast<uint64_t *>(ws);
+    uint64_t *bitsT = reinterpret_cast<uint64_t *>(ws + mat);
+    ws += 2 * mat;
+    int64_t *hist = reinterpret_cast<int64_t *>(ws);
+    ws += align_up((size_t)CB * 4 * 8, 256);
+    double *actions = reinterpret_cast<double *>(ws);
+    ws += align_up((size_t)B * 8, 256);
+    int64_t *hist4 = reinterpret_cast<int64_t *>(ws);
+    ws += align_up((size_t)B * 4 * 8, 256);
+    const size_t left = workspace_bytes - (size_t)(ws - static_cast<unsigned char *>(workspace));
+    const int64_t kmax = clamp_kmax(N, 3);
+
+    // the copy stream may not touch the workspace before the caller's stream is done with earlier work on it
+    CS_CUDA(cudaEventRecord(start, st));
+    CS_CUDA(cudaStreamWaitEvent(copy_stream, start, 0));
+    int64_t c = 0;
+    for (int64_t b0 = 0; b0 < B; b0 += CB, c++) {
+        const int64_t nb = (B - b0 < CB) ? B - b0 : CB;
+        const int buf = (int)(c & 1);
+        if (c >= 2) CS_CUDA(cudaStreamWaitEvent(copy_stream, consumed[buf], 0));
+        CS_CUDA(cudaMemcpyAsync(cdev[buf], coords_host + b0 * N * dim, (size_t)nb * N * dim * 8,
+                                cudaMemcpyHostToDevice, copy_stream));
+        CS_CUDA(cudaEventRecord(copied[buf], copy_stream));
+        CS_CUDA(cudaStreamWaitEvent(st, copied[buf], 0));
+        int rc = cs_causal_matrix_batched(cdev[buf], nb, N, dim, geometry, bits, bitsT, stream);
+        if (rc) return rc;
+        CS_CUDA(cudaEventRecord(consumed[buf], st));
+        if (kmax < 3) CS_CUDA(cudaMemsetAsync(hist, 0, (size_t)nb * 4 * 8, st));
+        rc = interval_hist_impl(bits, bitsT, nb, N, kmax, 0, N, CS_ROUTE_AUTO, hist, nullptr, ws, left, st);
+        if (rc) return rc;
+        rc = launch_bd_action(hist, kmax + 1, nb, kmax, N, spacetime_dim(geometry, dim), actions + b0, nullptr,
+                              hist4 + b0 * 4, st);
+        if (rc) return rc;
+    }
+    CS_CUDA(cudaMemcpyAsync(actions_host, actions, (size_t)B * 8, cudaMemcpyDeviceToHost, st));
+    if (hist4_host) CS_CUDA(cudaMemcpyAsync(hist4_host, hist4, (size_t)B * 4 * 8, cudaMemcpyDeviceToHost, st));
+    CS_CUDA(cudaStreamSynchronize(st));
+    return CS_OK;
+}
+
 // ---- end to end with host buffers ----------------------------------------------------------
 // workspace: [coords][bits][bitsT][hist][action+pad][interval scratch]
 size_t cs_action_host_workspace(int64_t N, int64_t kmax)

@@ -261,48 +261,41 @@ __device__ __forceinline__ uint32_t nib(uint32_t x)
 __device__ __forceinline__ uint32_t sf_col(int q) { return SF_COL + (q == 1 ? 16u : q == 2 ? 32u : 0u); }
 
 // ---- tile order ---------------------------------------------------------------------------------
-// Row tile I (256 rows) meets column tiles Jc (TN columns) with Jc >= R I, R = 256 / TN; d = Jc - R I
-// measures the K length.  Tiles are listed in bands of BANDW R values of d, longest first; inside a
-// band I-major, then d ascending.  Entry = (I << 16) | Jc.
-__host__ __device__ inline int64_t row_tiles_in_band(int nTc, int R, int I, int dlo, int dhi)
+// Tiles (I, J = I + d), 0 <= I, I + d < nT, in bands of BANDW diagonals, longest (largest d) first;
+// inside a band I-major, then d ascending.  Entry = (I << 16) | J.  nT (nT + 1) / 2 entries.
+// (Square tiles only: TN = 256.  Closed forms, no loops over rows: 3.6 us at nT = 256.)
+__host__ __device__ inline int64_t band_tiles(int nT, int dlo, int dhi)   // sum over d of (nT - d)
 {
-    const int dmax = nTc - R * I - 1;             // largest d of row I
-    if (dmax < dlo) return 0;
-    return (dmax < dhi ? dmax : dhi) - dlo + 1;
+    const int64_t w = dhi - dlo + 1;
+    return w * nT - w * (int64_t)(dlo + dhi) / 2;
 }
-inline int64_t pair_tiles_per_causet(int64_t N, int TN)
+inline int64_t pair_tiles_per_causet(int64_t N)
 {
-    const int64_t nT = (N + TILE - 1) / TILE, nTc = (N + TN - 1) / TN, R = TILE / TN;
-    int64_t n = 0;
-    for (int64_t I = 0; I < nT; I++) n += nTc - R * I > 0 ? nTc - R * I : 0;
-    return n;
+    const int64_t nT = (N + TILE - 1) / TILE;
+    return nT * (nT + 1) / 2;
 }
 
-__global__ void k_pair_tile_order(int nT, int nTc, int R, uint32_t *__restrict__ tab)
+__global__ void k_pair_tile_order(int nT, uint32_t *__restrict__ tab)
 {
-    __shared__ unsigned long long s_off;
-    const int bw = BANDW * R;
     const int b = blockIdx.x;
-    const int dhi = nTc - 1 - b * bw;
-    const int dlo = dhi - bw + 1 > 0 ? dhi - bw + 1 : 0;
-    if (threadIdx.x == 0) s_off = 0;
-    __syncthreads();
-    // tiles of all earlier bands: thread bb sums band bb over the rows
-    unsigned long long part = 0;
-    for (int bb = threadIdx.x; bb < b; bb += blockDim.x) {
-        const int h = nTc - 1 - bb * bw;
-        const int l = h - bw + 1 > 0 ? h - bw + 1 : 0;
-        for (int I = 0; I < nT; I++) part += (unsigned long long)row_tiles_in_band(nTc, R, I, l, h);
+    const int dhi = nT - 1 - b * BANDW;
+    const int dlo = dhi - BANDW + 1 > 0 ? dhi - BANDW + 1 : 0;
+    const int w = dhi - dlo + 1;
+    int64_t off = 0;
+    for (int bb = 0; bb < b; bb++) {
+        const int h = nT - 1 - bb * BANDW;
+        const int l = h - BANDW + 1 > 0 ? h - BANDW + 1 : 0;
+        off += band_tiles(nT, l, h);
     }
-    if (part) atomicAdd(&s_off, part);
-    __syncthreads();
-    const int64_t off = (int64_t)s_off;
-    for (int I = threadIdx.x; I < nT; I += blockDim.x) {
-        const int64_t cnt = row_tiles_in_band(nTc, R, I, dlo, dhi);
-        if (cnt == 0) continue;
-        int64_t pos = 0;
-        for (int Ip = 0; Ip < I; Ip++) pos += row_tiles_in_band(nTc, R, Ip, dlo, dhi);
-        for (int64_t d = 0; d < cnt; d++) tab[off + pos + d] = ((uint32_t)I << 16) | (uint32_t)(R * I + dlo + d);
+    const int full = nT - dhi;   // rows I < full have all w diagonals inside the matrix
+    for (int I = threadIdx.x; I + dlo < nT; I += blockDim.x) {
+        int64_t pos;
+        if (I <= full) pos = (int64_t)I * w;
+        else {
+            const int64_t m = I - full;   // rows full .. I-1 hold nT - dlo - I' entries each
+            pos = (int64_t)full * w + m * (nT - dlo) - (int64_t)(full + I - 1) * m / 2;
+        }
+        for (int d = dlo; d <= dhi && I + d < nT; d++) tab[off + pos + (d - dlo)] = ((uint32_t)I << 16) | (uint32_t)(I + d);
     }
 }
 
@@ -779,7 +772,7 @@ constexpr int PAIR_TN = 256;
 
 size_t interval_pair_scratch_bytes(int64_t N)
 {
-    return (size_t)pair_tiles_per_causet(N, PAIR_TN) * sizeof(uint32_t);
+    return (size_t)pair_tiles_per_causet(N) * sizeof(uint32_t);
 }
 
 template <bool SMALL, int TN>
@@ -806,7 +799,8 @@ int launch_interval_pair(const uint64_t *bits, const uint64_t *bitsT, int64_t B,
 {
     if (N > ((int64_t)1 << 22)) return CS_ERR_ARG;   // counts must stay exact in fp32; tile ids are 16 bits
     constexpr int TN = PAIR_TN;
-    const int64_t tiles_per = pair_tiles_per_causet(N, TN);
+    static_assert(PAIR_TN == TILE, "the tile table lists square tiles");
+    const int64_t tiles_per = pair_tiles_per_causet(N);
     if (B > 0 && tiles_per > (((int64_t)1 << 31) - 1) / B) return CS_ERR_ARG;   // 32-bit tile schedule
     if (!scratch || scratch_bytes < interval_pair_scratch_bytes(N)) return CS_ERR_WORKSPACE;
     const int64_t stride = row_stride_words(N);
@@ -815,10 +809,9 @@ int launch_interval_pair(const uint64_t *bits, const uint64_t *bitsT, int64_t B,
     if (rc) return rc;
     rc = pair_bits_map(&mapL, bitsT, B, N, stride, TN / 2);
     if (rc) return rc;
-    const int nT = (int)((N + TILE - 1) / TILE), nTc = (int)((N + TN - 1) / TN), R = TILE / TN;
+    const int nT = (int)((N + TILE - 1) / TILE);
     uint32_t *tab = static_cast<uint32_t *>(scratch);
-    const int bands = (nTc + BANDW * R - 1) / (BANDW * R);
-    k_pair_tile_order<<<bands, 256, 0, st>>>(nT, nTc, R, tab);
+    k_pair_tile_order<<<(nT + BANDW - 1) / BANDW, 128, 0, st>>>(nT, tab);
     CS_LAUNCHED("k_pair_tile_order");
     const int64_t total = tiles_per * B;
     int64_t clusters = sm_count() / 2;

@@ -246,6 +246,14 @@ def test_batched_ensemble(api, oracle):
         _, o_hist, o_S, _ = oracle.action_pipeline(coords[b], cfg.geometry, tier=1)
         assert np.array_equal(hist4[b], o_hist[:4])
         assert actions[b] == o_S
+    # the chunked host-buffer entry point: more than one chunk of 512, pinned and pageable memory
+    coords = inp.make_ensemble_coords(cfg, B=20, N=300)
+    big = np.ascontiguousarray(np.tile(coords, (53, 1, 1))[:1050])
+    want = [oracle.action_pipeline(coords[b], cfg.geometry, tier=1) for b in range(20)]
+    for host in (torch.from_numpy(big).pin_memory(), torch.from_numpy(big)):
+        a_host, h4_host = api.bd_action_batched_host(host, cfg.geometry)
+        for b in range(1050):
+            assert a_host[b] == want[b % 20][2] and np.array_equal(h4_host[b].numpy(), want[b % 20][1][:4])
     # ragged batched size
     coords = inp.make_ensemble_coords(cfg, B=3, N=333)
     actions = api.bd_action_batched(torch.from_numpy(coords).cuda(), cfg.geometry).cpu().numpy()
