@@ -89,10 +89,18 @@ struct Pred<CS_GEOM_FLRW_POLAR, 6> {
 // The tile takes this path only if the header's dt >= 0 holds for every pair it keeps (off the
 // diagonal: max t_i <= min t_j; diagonal tile: its points are in time order -- always the case for
 // time-sorted input) and 2^-40 <= C <= 2^40 (no overflow or underflow in the fp32 products).
+//
+// de Sitter slab: the same scheme on D = (eta_j - eta_i) - min(|dtheta|, 2pi - |dtheta|), five fp32 operations.
+// With C = max(|eta|, |theta|, 2pi) over the tile: the two differences are each off by <= 4 u C (two input
+// roundings and the subtraction), b = 2pi - a by <= 8 u C, the minimum by no more, d = deta - m by
+// <= 17 u C; margin m = 32 u C.  d > m => D > 15 u C => the fp64 expression (errors ~2^-50 C) says related,
+// d < -m => unrelated, else fp64.  No time-order condition: the header's expression has none.
 template <int GEOM, int DIM>
 struct FastCone { static constexpr bool ok = false; };
 template <int DIM>
 struct FastCone<CS_GEOM_MINK_CONE, DIM> { static constexpr bool ok = true; };
+template <>
+struct FastCone<CS_GEOM_DS2_SLAB, 2> { static constexpr bool ok = true; };
 
 // order-preserving map float -> uint32 (NaN with the sign bit clear sorts above +inf, set below -inf)
 __device__ __forceinline__ uint32_t float_key(float f)
@@ -141,7 +149,7 @@ constexpr int NJ = 2;            // future points per lane: a CTA covers 256 row
 // One 32 x 32 block per future point k < NK of this lane: bit ii of lw[k] = (row i0 + ii  -<  point k),
 // decided by the fp32 prefilter; unc[k] is set if any of the lane's 32 decisions is inside the error
 // band.  The row's (t, x, y, z) and h are loaded once (LDS.128 broadcasts) for all NK points.
-template <int DIM, int NK>
+template <int GEOM, int DIM, int NK>
 __device__ __forceinline__ void fast_block(const float4 *__restrict__ fi, const float *__restrict__ hi,
                                            const float (*fj)[4], const float *hj, const float *m,
                                            uint32_t *lw, bool *unc)
@@ -155,11 +163,18 @@ __device__ __forceinline__ void fast_block(const float4 *__restrict__ fi, const 
             const float4 p = fi[i4 + q];
 #pragma unroll
             for (int k = 0; k < NK; k++) {
-                float a = fmaf(-p.x, fj[k][0], hq[q]);
-                if (DIM > 1) a = fmaf(p.y, fj[k][1], a);
-                if (DIM > 2) a = fmaf(p.z, fj[k][2], a);
-                if (DIM > 3) a = fmaf(p.w, fj[k][3], a);
-                a = a + hj[k];
+                float a;
+                if (GEOM == CS_GEOM_DS2_SLAB) {
+                    const float de = fj[k][0] - p.x;
+                    const float ab = fabsf(fj[k][1] - p.y);
+                    a = de - fminf(ab, 6.2831853071795865f - ab);
+                } else {
+                    a = fmaf(-p.x, fj[k][0], hq[q]);
+                    if (DIM > 1) a = fmaf(p.y, fj[k][1], a);
+                    if (DIM > 2) a = fmaf(p.z, fj[k][2], a);
+                    if (DIM > 3) a = fmaf(p.w, fj[k][3], a);
+                    a = a + hj[k];
+                }
                 if (a > m[k]) lw[k] |= 1u << (i4 + q);
                 unc[k] = unc[k] || !(fabsf(a) > m[k]);
             }
@@ -291,9 +306,15 @@ k_causal_matrix(const double *__restrict__ coords, int64_t N, int64_t stride,
 #pragma unroll
         for (int k = 0; k < NJ; k++) {
             const float C = fmaxf(Ci, __uint_as_float(r[2 + 2 * k]));
-            const bool ordered = dg[k] ? tile_ordered : (tmaxI <= -key_float(r[3 + 2 * k]));
-            fast[k] = act[k] && ordered && (C >= 0x1p-40f) && (C <= 0x1p40f);
-            m[k] = __fmul_ru(__fmul_ru(C, C), 0x1p-18f * 1.001f);
+            if (GEOM == CS_GEOM_DS2_SLAB) {
+                const float Cd = fmaxf(C, 6.2831855f);                     // >= 2 pi
+                fast[k] = act[k] && (Cd <= 0x1p100f);
+                m[k] = __fmul_ru(Cd, 0x1p-19f * 1.001f);
+            } else {
+                const bool ordered = dg[k] ? tile_ordered : (tmaxI <= -key_float(r[3 + 2 * k]));
+                fast[k] = act[k] && ordered && (C >= 0x1p-40f) && (C <= 0x1p40f);
+                m[k] = __fmul_ru(__fmul_ru(C, C), 0x1p-18f * 1.001f);
+            }
         }
     }
     __syncthreads();    // s_xi / s_fi / s_hi visible; s_red (aliased on s_U) no longer read
@@ -311,9 +332,9 @@ k_causal_matrix(const double *__restrict__ coords, int64_t N, int64_t stride,
         if (FAST) {
             bool unc[NJ] = {false, false};
             const bool f0 = need[0] && fast[0], f1 = need[1] && fast[1];
-            if (f0 && f1) fast_block<DIM, 2>(s_fi + sb * 32, s_hi + sb * 32, fj, hj, m, lw, unc);
-            else if (f0) fast_block<DIM, 1>(s_fi + sb * 32, s_hi + sb * 32, fj, hj, m, lw, unc);
-            else if (f1) fast_block<DIM, 1>(s_fi + sb * 32, s_hi + sb * 32, fj + 1, hj + 1, m + 1, lw + 1, unc + 1);
+            if (f0 && f1) fast_block<GEOM, DIM, 2>(s_fi + sb * 32, s_hi + sb * 32, fj, hj, m, lw, unc);
+            else if (f0) fast_block<GEOM, DIM, 1>(s_fi + sb * 32, s_hi + sb * 32, fj, hj, m, lw, unc);
+            else if (f1) fast_block<GEOM, DIM, 1>(s_fi + sb * 32, s_hi + sb * 32, fj + 1, hj + 1, m + 1, lw + 1, unc + 1);
 #pragma unroll
             for (int k = 0; k < NJ; k++) {
                 if (__any_sync(0xffffffffu, unc[k])) { slow[k] = true; lw[k] = 0; }

@@ -140,6 +140,41 @@ def test_causal_matrix_prefilter_unsorted_inf_nan(api, oracle):
         assert np.array_equal(to_u64(bitsT), oracle.transpose_bits(o_bits, N))
 
 
+def test_causal_matrix_prefilter_ds_slab(api, oracle):
+    """The de Sitter slab's single-precision prefilter: partners exactly on the cone and one ulp either side,
+    directly and through the 2 pi wrap-around, plus angles outside [0, 2 pi) and NaN / infinite coordinates."""
+    rng = np.random.default_rng(21)
+    n = 600
+    eta = rng.uniform(-1.2, -0.4, n); th = rng.uniform(0, 2 * np.pi, n)
+    d = rng.uniform(0.01, 0.35, n)
+    base = np.stack([eta, th], axis=1)
+    fwd = np.stack([eta + d, th + d], axis=1)                       # null, same side
+    wrap = np.stack([eta + d, np.mod(th - d, 2 * np.pi)], axis=1)   # null, may cross theta = 0
+    sets = [base]
+    for p in (fwd, wrap):
+        for k in (0.0, 10.0, -10.0):
+            q = p.copy()
+            if k:
+                q[:, 0] = np.nextafter(p[:, 0], k)
+            sets.append(q)
+    coords = np.concatenate(sets)
+    coords = np.ascontiguousarray(coords[np.lexsort((coords[:, 1], coords[:, 0]))])
+    N = coords.shape[0]
+    for variant in range(3):
+        c = coords.copy()
+        if variant == 1:
+            c[:, 1] += 100.0                                        # angles far outside [0, 2 pi)
+        if variant == 2:
+            c[7, 1] = np.nan; c[300, 0] = np.inf; c[900, 1] = -np.inf; c[1500:1900] = c[1500]
+        o_bits = oracle.causal_matrix_bits(c, inp.GEOM_DS2_SLAB)
+        bits, bitsT = gpu_bits(api, c, inp.GEOM_DS2_SLAB)
+        assert np.array_equal(to_u64(bits), o_bits), variant
+        assert np.array_equal(to_u64(bitsT), oracle.transpose_bits(o_bits, N)), variant
+    shuffled = np.ascontiguousarray(coords[rng.permutation(N)])     # not time-sorted: d_eta < 0 pairs
+    assert np.array_equal(to_u64(gpu_bits(api, shuffled, inp.GEOM_DS2_SLAB)[0]),
+                          oracle.causal_matrix_bits(shuffled, inp.GEOM_DS2_SLAB))
+
+
 def test_degenerate_inputs(api, oracle):
     # identical points, NaN coordinates, N = 0
     coords = np.zeros((70, 4)); coords[10:20, 1] = np.nan
