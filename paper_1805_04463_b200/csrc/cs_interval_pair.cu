@@ -312,7 +312,7 @@ template <bool SMALL, int TN>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(THREADS, 1)
 k_interval_pair(const __grid_constant__ CUtensorMap mapU, const __grid_constant__ CUtensorMap mapL,
                 const uint64_t *__restrict__ bits, const uint32_t *__restrict__ tile_tab, uint32_t tiles_per,
-                int64_t B, int64_t N, int64_t stride, int64_t kmax, int hs,
+                int64_t B, int64_t N, int64_t stride, int64_t kmax, int hs, int causet_major,
                 int64_t row_begin, int64_t row_end,
                 unsigned long long *__restrict__ hist, unsigned long long *__restrict__ nrel)
 {
@@ -335,15 +335,34 @@ k_interval_pair(const __grid_constant__ CUtensorMap mapU, const __grid_constant_
     const uint32_t rank = cluster_ctarank();
     // 32-bit schedule state (the launcher rejects more than 2^31 tiles): the expander and issuer
     // warps run on 64 and 40 registers
-    const uint32_t total_tiles = tiles_per * (uint32_t)B;
     const uint32_t t0 = cluster_id_x(), tstep = num_clusters_x();
     const int ib0 = (int)(row_begin / TILE), ib1 = (int)((row_end + TILE - 1) / TILE);   // I blocks inside the row range
     const int64_t hist_len = kmax + 1;
 
-    auto get_tile = [&](uint32_t t) {
+    // Every role of both CTAs walks the same static schedule, kept as (causet, tile index) and advanced
+    // without divisions.  Interleaved (one causet, or few): cluster c takes tiles c, c + #clusters, ... of the
+    // concatenated tile lists.  Causet-major (ensembles): cluster c takes whole causets c, c + #clusters, ...,
+    // so that the per-causet tallies are flushed once per causet, not once per tile (the ncu source view of
+    // the 4096 x 2048 ensemble had two thirds of the epilogue's samples in that flush).
+    struct Sched { uint32_t b, idx; };
+    auto sched_first = [&]() {
+        Sched sc;
+        if (causet_major) { sc.b = t0; sc.idx = 0; }
+        else { sc.b = t0 / tiles_per; sc.idx = t0 % tiles_per; }
+        return sc;
+    };
+    auto sched_next = [&](Sched &sc) {
+        if (causet_major) {
+            if (++sc.idx == tiles_per) { sc.idx = 0; sc.b += tstep; }
+        } else {
+            sc.idx += tstep;
+            while (sc.idx >= tiles_per) { sc.idx -= tiles_per; sc.b++; }
+        }
+    };
+    auto get_tile = [&](const Sched &sc) {
         Tile tc;
-        tc.b = (int)(t / tiles_per);
-        const uint32_t e = __ldg(tile_tab + (t - (uint32_t)tc.b * tiles_per));
+        tc.b = (int)sc.b;
+        const uint32_t e = __ldg(tile_tab + sc.idx);
         tc.I = (int)(e >> 16);
         tc.J = (int)(e & 0xFFFFu);
         tc.nstages = ((tc.J + 1) * TN - tc.I * TILE + KSTEP - 1) / KSTEP;
@@ -494,8 +513,8 @@ k_interval_pair(const __grid_constant__ CUtensorMap mapU, const __grid_constant_
             if (++s == NS) { s = 0; ph ^= 1; }
         };
 
-        for (uint32_t t = t0; t < total_tiles; t += tstep) {
-            const Tile tc = get_tile(t);
+        for (Sched sc = sched_first(); sc.b < (uint32_t)B; sched_next(sc)) {
+            const Tile tc = get_tile(sc);
             if (tc.skip) continue;
             const int nstages = tc.nstages;
             for (int k = 0; k < nstages; k += GK) {
@@ -525,8 +544,8 @@ k_interval_pair(const __grid_constant__ CUtensorMap mapU, const __grid_constant_
             // ===================================== TMA loader ====================================
             {
             uint32_t grp = 0;
-            for (uint32_t t = t0; t < total_tiles; t += tstep) {
-                const Tile tc = get_tile(t);
+            for (Sched sc = sched_first(); sc.b < (uint32_t)B; sched_next(sc)) {
+                const Tile tc = get_tile(sc);
                 if (tc.skip) continue;
                 const int nstages = tc.nstages;
                 const int ngroups = (nstages + GK - 1) / GK;
@@ -553,8 +572,8 @@ k_interval_pair(const __grid_constant__ CUtensorMap mapU, const __grid_constant_
             const uint32_t a_tmem0 = tmem_base + A_COL;
             const uint32_t sf0 = tmem_base + sf_col(0), sf1 = tmem_base + sf_col(1), sf2 = tmem_base + sf_col(2);
             uint32_t s = 0, ph = 0, tile_seq = 0;
-            for (uint32_t t = t0; t < total_tiles; t += tstep) {
-                const Tile tc = get_tile(t);
+            for (Sched sc = sched_first(); sc.b < (uint32_t)B; sched_next(sc)) {
+                const Tile tc = get_tile(sc);
                 if (tc.skip) continue;
                 const int nstages = tc.nstages;
                 const uint32_t acc = tile_seq % NACC, use = tile_seq / NACC;     // accumulator and how often it was used
@@ -607,8 +626,8 @@ k_interval_pair(const __grid_constant__ CUtensorMap mapU, const __grid_constant_
                 small[q] = 0;
             }
         };
-        for (uint32_t t = t0; t < total_tiles; t += tstep) {
-            const Tile tc = get_tile(t);
+        for (Sched sc = sched_first(); sc.b < (uint32_t)B; sched_next(sc)) {
+            const Tile tc = get_tile(sc);
             if (tc.skip) continue;
             if (tc.b != cur_batch) {   // per-causet histograms: flush before switching
                 if (cur_batch >= 0 && B > 1) {
@@ -786,8 +805,11 @@ static int launch_pair_t(const CUtensorMap &mapU, const CUtensorMap &mapL, const
                                      Shape<TN>::SMEM_FIXED + (SMALL ? 0 : HS_MAX * 4)));
         attr_set = true;
     }
+    // whole causets per cluster only if the last round of causets leaves at most 5 % of the clusters idle
+    const int64_t rounds = (B + clusters - 1) / clusters;
+    const int causet_major = (B > 1 && rounds * clusters * 20 <= B * 21) ? 1 : 0;
     k_interval_pair<SMALL, TN><<<(unsigned)(2 * clusters), THREADS, Shape<TN>::SMEM_FIXED + hs * 4, st>>>(
-        mapU, mapL, bits, tab, tiles_per, B, N, stride, kmax, hs, row_begin, row_end,
+        mapU, mapL, bits, tab, tiles_per, B, N, stride, kmax, hs, causet_major, row_begin, row_end,
         reinterpret_cast<unsigned long long *>(hist), reinterpret_cast<unsigned long long *>(nrel));
     CS_LAUNCHED("k_interval_pair");
     return CS_OK;
