@@ -175,6 +175,33 @@ def test_causal_matrix_prefilter_ds_slab(api, oracle):
                           oracle.causal_matrix_bits(shuffled, inp.GEOM_DS2_SLAB))
 
 
+def test_causal_matrix_lightcone_ties(api, oracle):
+    """1+1 light cone (two strict fp64 comparisons): coordinates that differ by one fp64 ulp, exact ties, values
+    beyond the fp32 range, denormals and NaN.  (An fp32 prefilter was measured for this predicate too and
+    dropped: two DSETP per pair are already cheaper than its set-up.)"""
+    rng = np.random.default_rng(5)
+    n = 500
+    u = rng.uniform(0, 1, n); v = rng.uniform(0, 1, n)
+    pts = [np.stack([u, v], 1)]
+    for du, dv in ((1, 1), (1, 0), (0, 1), (-1, 1), (1, -1)):
+        uu = u.copy(); vv = v.copy()
+        for _ in range(abs(du)):
+            uu = np.nextafter(uu, 2.0 * du)
+        for _ in range(abs(dv)):
+            vv = np.nextafter(vv, 2.0 * dv)
+        pts.append(np.stack([uu, vv], 1))
+    coords = np.concatenate(pts)
+    for scale in (1.0, 1e300, 1e-300, 1e-42):
+        c = coords * scale
+        c = np.ascontiguousarray(c[np.lexsort((c[:, 0], (c[:, 0] + c[:, 1]) / 2))])
+        if scale == 1.0:
+            c[17, 0] = np.nan; c[400, 1] = np.inf; c[1000:1300] = c[1000]
+        o_bits = oracle.causal_matrix_bits(c, inp.GEOM_MINK2_LIGHTCONE)
+        bits, bitsT = gpu_bits(api, c, inp.GEOM_MINK2_LIGHTCONE)
+        assert np.array_equal(to_u64(bits), o_bits), scale
+        assert np.array_equal(to_u64(bitsT), oracle.transpose_bits(o_bits, c.shape[0])), scale
+
+
 def test_degenerate_inputs(api, oracle):
     # identical points, NaN coordinates, N = 0
     coords = np.zeros((70, 4)); coords[10:20, 1] = np.nan
