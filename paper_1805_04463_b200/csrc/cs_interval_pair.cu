@@ -63,6 +63,9 @@ constexpr int BANDW = 8;                // diagonals (in 256-column units) per b
 #ifndef CS_PAIR_DIAG
 #define CS_PAIR_DIAG 0      // timing experiments only (results are wrong): 1 no B stores, 2 no A stores, 4 no tally
 #endif
+#ifndef CS_PAIR_SKIP
+#define CS_PAIR_SKIP 1      // skip K blocks whose bit block is empty (k_pair_block_flags)
+#endif
 #ifndef CS_PAIR_ROT_IMAD
 #define CS_PAIR_ROT_IMAD 0
 #endif
@@ -304,14 +307,65 @@ struct Tile {
     int nstages;   // 256-k stages from the first row of I to the last column of J
     int b;         // causet
     bool skip;     // no row of the tile inside [row_begin, row_end)
+    uint32_t head, tail;   // bit m: the bit block U[I][I+m] resp. U[J-m][J] holds a relation (m < SKIPM)
+    bool force0;           // no stage would run: stage 0 runs anyway (the accumulator must be written)
 };
+
+// ---- empty K blocks -----------------------------------------------------------------------------
+// Stage k of tile (I, J) multiplies U[rows I][cols I+k] with U[rows I+k][cols J]; if either 256 x 256 bit
+// block is empty the stage adds nothing.  In a time-sorted sprinkling the blocks next to the diagonal
+// are empty when relations need more separation in time than a few hundred elements span (3+1 flat cone at
+// N = 65536: 96 % of the diagonal blocks, half of those 5 blocks out, none beyond 16; 13.7 % of all stages).
+// flagU[I][m] = block (I, I+m) non-empty, flagT[J][m] = block (J-m, J) non-empty, m < SKIPM.
+constexpr int SKIPM = 16;
+
+__global__ void __launch_bounds__(256)
+k_pair_block_flags(const uint64_t *__restrict__ bits, int64_t N, int64_t stride, int nT,
+                   uint8_t *__restrict__ flagU, uint8_t *__restrict__ flagT)
+{
+    const int I = blockIdx.x, m = blockIdx.y, K = I + m;
+    if (K >= nT) return;
+    const int64_t r = (int64_t)I * TILE + threadIdx.x;
+    uint64_t any = 0;
+    if (r < N) {
+#pragma unroll
+        for (int w = 0; w < TILE / 64; w++) {
+            const int64_t wi = (int64_t)K * (TILE / 64) + w;
+            if (wi < stride) any |= bits[r * stride + wi];
+        }
+    }
+    const int nz = __syncthreads_or(any != 0);
+    if (threadIdx.x == 0) {
+        flagU[I * SKIPM + m] = (uint8_t)(nz != 0);
+        flagT[K * SKIPM + m] = (uint8_t)(nz != 0);
+    }
+}
+
+// sixteen 0/1 bytes -> sixteen bits
+__device__ __forceinline__ uint32_t flags_to_mask(uint4 f)
+{
+    return ((f.x * 0x01020408u) >> 24 & 0xFu) | ((f.y * 0x01020408u) >> 24 & 0xFu) << 4 |
+           ((f.z * 0x01020408u) >> 24 & 0xFu) << 8 | ((f.w * 0x01020408u) >> 24 & 0xFu) << 12;
+}
+
+#ifndef CS_PAIR_BYPASS
+#define CS_PAIR_BYPASS 0    // experiment: bit 0 expanders, 1 loader, 2 issuer, 3 get_tile treat every stage as live
+#endif
+// THE predicate every role uses to decide whether stage k of a tile runs
+__device__ __forceinline__ bool stage_live(const Tile &tc, int k)
+{
+    const int kt = tc.nstages - 1 - k;
+    const bool dead = (k < SKIPM && !((tc.head >> k) & 1u)) || (kt < SKIPM && !((tc.tail >> kt) & 1u));
+    return !dead || (tc.force0 && k == 0);
+}
 
 // SMALL: kmax <= 3 (the Monte-Carlo case, only N_0..N_3 enter Eq. 4.10-4.12): the tally keeps packed
 // counters in registers and never touches the shared histogram (hs = 0).
 template <bool SMALL, int TN>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(THREADS, 1)
 k_interval_pair(const __grid_constant__ CUtensorMap mapU, const __grid_constant__ CUtensorMap mapL,
-                const uint64_t *__restrict__ bits, const uint32_t *__restrict__ tile_tab, uint32_t tiles_per,
+                const uint64_t *__restrict__ bits, const uint32_t *__restrict__ tile_tab,
+                const uint8_t *__restrict__ flagU, const uint8_t *__restrict__ flagT, uint32_t tiles_per,
                 int64_t B, int64_t N, int64_t stride, int64_t kmax, int hs, int causet_major,
                 int64_t row_begin, int64_t row_end,
                 unsigned long long *__restrict__ hist, unsigned long long *__restrict__ nrel)
@@ -367,6 +421,17 @@ k_interval_pair(const __grid_constant__ CUtensorMap mapU, const __grid_constant_
         tc.J = (int)(e & 0xFFFFu);
         tc.nstages = ((tc.J + 1) * TN - tc.I * TILE + KSTEP - 1) / KSTEP;
         tc.skip = tc.I < ib0 || tc.I >= ib1;
+        tc.head = tc.tail = 0xFFFFu;
+        tc.force0 = false;
+        if (!(CS_PAIR_BYPASS & 8) && flagU) {
+            tc.head = flags_to_mask(__ldg(reinterpret_cast<const uint4 *>(flagU + tc.I * SKIPM)));
+            tc.tail = flags_to_mask(__ldg(reinterpret_cast<const uint4 *>(flagT + tc.J * SKIPM)));
+            if (tc.nstages <= 2 * SKIPM) {          // longer tiles always have a stage outside both windows
+                bool any = false;
+                for (int k = 0; k < tc.nstages; k++) any = any || stage_live(tc, k);
+                tc.force0 = !any;
+            }
+        }
         return tc;
     };
 
@@ -517,18 +582,17 @@ k_interval_pair(const __grid_constant__ CUtensorMap mapU, const __grid_constant_
             const Tile tc = get_tile(sc);
             if (tc.skip) continue;
             const int nstages = tc.nstages;
-            for (int k = 0; k < nstages; k += GK) {
+            auto do_group = [&](bool first, bool second) {
                 mbar_wait(&s_bfull[b], bph);
                 const unsigned char *src = my_bits + b * BITS_BYTES;
-                const bool second = k + 1 < nstages;
                 if (isA) {
-                    stage_A(*reinterpret_cast<const uint4 *>(src + off0), *reinterpret_cast<const uint4 *>(src + off1));
+                    if (first) stage_A(*reinterpret_cast<const uint4 *>(src + off0), *reinterpret_cast<const uint4 *>(src + off1));
                     if (second) stage_A(*reinterpret_cast<const uint4 *>(src + off2), *reinterpret_cast<const uint4 *>(src + off3));
                 } else if (TNH == 64) {
-                    stage_B_half(*reinterpret_cast<const uint4 *>(src + (bhalf ? off1 : off0)));
+                    if (first) stage_B_half(*reinterpret_cast<const uint4 *>(src + (bhalf ? off1 : off0)));
                     if (second) stage_B_half(*reinterpret_cast<const uint4 *>(src + (bhalf ? off3 : off2)));
                 } else {
-                    stage_B(*reinterpret_cast<const uint4 *>(src + off0), *reinterpret_cast<const uint4 *>(src + off1));
+                    if (first) stage_B(*reinterpret_cast<const uint4 *>(src + off0), *reinterpret_cast<const uint4 *>(src + off1));
                     if (second) stage_B(*reinterpret_cast<const uint4 *>(src + off2), *reinterpret_cast<const uint4 *>(src + off3));
                 }
                 // the buffer has been loaded AND consumed by every lane (the stores above depend on
@@ -536,6 +600,24 @@ k_interval_pair(const __grid_constant__ CUtensorMap mapU, const __grid_constant_
                 __syncwarp();
                 if (lane == 0) mbar_arrive(&s_bempty[b]);
                 if (++b == NB) { b = 0; bph ^= 1; }
+            };
+            // Only the first and the last SKIPM stages of a tile can be empty (stage_live): those zones test
+            // every stage, the stages in between run the plain loop (testing there cost 16 % at N = 65536:
+            // the expanders live on 64 registers).  Zone borders are even, so groups of GK = 2 never straddle.
+            auto checked = [&](int k) {
+                const bool first = stage_live(tc, k), second = k + 1 < nstages && stage_live(tc, k + 1);
+                if (first || second) do_group(first, second);            // the loader skips the same groups
+            };
+            static_assert(GK == 2 && SKIPM % GK == 0, "zone borders");
+            const int z1 = nstages < SKIPM ? nstages : SKIPM;            // [0, z1): head zone
+            int z2 = (nstages - SKIPM) & ~1;                              // [z2, nstages): tail zone
+            if (z2 < z1) z2 = z1;
+            if (!flagU) {
+                for (int k = 0; k < nstages; k += GK) do_group(true, k + 1 < nstages);
+            } else {
+                for (int k = 0; k < z1; k += GK) checked(k);
+                for (int k = z1; k < z2; k += GK) do_group(true, true);
+                for (int k = z2; k < nstages; k += GK) checked(k);
             }
         }
     } else if (warp >= MMA_WARP) {
@@ -549,7 +631,8 @@ k_interval_pair(const __grid_constant__ CUtensorMap mapU, const __grid_constant_
                 if (tc.skip) continue;
                 const int nstages = tc.nstages;
                 const int ngroups = (nstages + GK - 1) / GK;
-                for (int g = 0; g < ngroups; g++, grp++) {
+                for (int g = 0; g < ngroups; g++) {
+                    if (!(CS_PAIR_BYPASS & 2) && !stage_live(tc, GK * g) && !(GK * g + 1 < nstages && stage_live(tc, GK * g + 1))) continue;
                     const int b = grp % NB;
                     mbar_wait(&s_bempty[b], ((grp / NB) & 1) ^ 1);
                     mbar_arrive_expect_tx(&s_bfull[b], (uint32_t)BITS_BYTES);   // out-of-bounds is zero-filled
@@ -557,6 +640,7 @@ k_interval_pair(const __grid_constant__ CUtensorMap mapU, const __grid_constant_
                     const int c0 = (tc.I * (KSTEP / 8)) + g * BROW;             // byte column of the first k
                     tma_load_3d(dst, &mapU, c0, tc.I * TILE + (int)rank * TM, tc.b, &s_bfull[b]);
                     tma_load_3d(dst + TM * BROW, &mapL, c0, tc.J * TN + (int)rank * TNH, tc.b, &s_bfull[b]);
+                    grp++;
                 }
             }
         }
@@ -580,20 +664,23 @@ k_interval_pair(const __grid_constant__ CUtensorMap mapU, const __grid_constant_
                 mbar_wait_cluster(&s_tempty[acc], (use & 1) ^ 1);         // both epilogues have drained this accumulator
                 tc_fence_after();
                 const uint32_t d_tmem = tmem_base + acc * TN;
+                uint32_t accum = 0;                                       // the first stage that runs overwrites
                 for (int ks = 0; ks < nstages; ks++) {
+                    if (!(CS_PAIR_BYPASS & 4) && !stage_live(tc, ks)) continue;
                     mbar_wait_cluster(&s_full[s], ph);
                     tc_fence_after();
                     if (elect_one()) {
                         const uint64_t bd = bdesc0 + (uint64_t)((s * STAGE_BYTES) >> 4);
                         const uint32_t at = a_tmem0 + s * 32;
                         // K = 64 per MMA: 8 TMEM columns of A, 2 chunks of B
-                        mma_mxf4_pair(d_tmem, at, bd, SH::IDESC, ks > 0 ? 1u : 0u, sf0, sf0);
+                        mma_mxf4_pair(d_tmem, at, bd, SH::IDESC, accum, sf0, sf0);
                         mma_mxf4_pair(d_tmem, at + 8, bd + ((2 * TNH * 16) >> 4), SH::IDESC, 1u, sf1, sf1);
                         mma_mxf4_pair(d_tmem, at + 16, bd + ((4 * TNH * 16) >> 4), SH::IDESC, 1u, sf2, sf2);
                         mma_mxf4_pair(d_tmem, at + 24, bd + ((6 * TNH * 16) >> 4), SH::IDESC, 1u, sf0, sf0);
                         mma_commit_pair(&s_empty[s]);                     // stage s free in both CTAs once these MMAs retire
                     }
                     __syncwarp();
+                    accum = 1;
                     if (++s == NS) { s = 0; ph ^= 1; }
                 }
                 if (elect_one()) mma_commit_pair(&s_tfull[acc]);          // accumulator complete, both CTAs
@@ -791,12 +878,13 @@ constexpr int PAIR_TN = 256;
 
 size_t interval_pair_scratch_bytes(int64_t N)
 {
-    return (size_t)pair_tiles_per_causet(N) * sizeof(uint32_t);
+    const int64_t nT = (N + TILE - 1) / TILE;
+    return align_up((size_t)pair_tiles_per_causet(N) * sizeof(uint32_t), 256) + 2 * align_up((size_t)nT * SKIPM, 256);
 }
 
 template <bool SMALL, int TN>
 static int launch_pair_t(const CUtensorMap &mapU, const CUtensorMap &mapL, const uint64_t *bits, const uint32_t *tab,
-                         uint32_t tiles_per, int64_t clusters, int64_t B, int64_t N, int64_t stride, int64_t kmax, int hs,
+                         const uint8_t *flagU, const uint8_t *flagT, uint32_t tiles_per, int64_t clusters, int64_t B, int64_t N, int64_t stride, int64_t kmax, int hs,
                          int64_t row_begin, int64_t row_end, int64_t *hist, int64_t *nrel, cudaStream_t st)
 {
     static bool attr_set = false;
@@ -809,7 +897,7 @@ static int launch_pair_t(const CUtensorMap &mapU, const CUtensorMap &mapL, const
     const int64_t rounds = (B + clusters - 1) / clusters;
     const int causet_major = (B > 1 && rounds * clusters * 20 <= B * 21) ? 1 : 0;
     k_interval_pair<SMALL, TN><<<(unsigned)(2 * clusters), THREADS, Shape<TN>::SMEM_FIXED + hs * 4, st>>>(
-        mapU, mapL, bits, tab, tiles_per, B, N, stride, kmax, hs, causet_major, row_begin, row_end,
+        mapU, mapL, bits, tab, flagU, flagT, tiles_per, B, N, stride, kmax, hs, causet_major, row_begin, row_end,
         reinterpret_cast<unsigned long long *>(hist), reinterpret_cast<unsigned long long *>(nrel));
     CS_LAUNCHED("k_interval_pair");
     return CS_OK;
@@ -835,6 +923,15 @@ int launch_interval_pair(const uint64_t *bits, const uint64_t *bitsT, int64_t B,
     uint32_t *tab = static_cast<uint32_t *>(scratch);
     k_pair_tile_order<<<(nT + BANDW - 1) / BANDW, 128, 0, st>>>(nT, tab);
     CS_LAUNCHED("k_pair_tile_order");
+    // empty-block flags: one causet, and enough row tiles for blocks near the diagonal to be empty at all
+    uint8_t *flagU = nullptr, *flagT = nullptr;
+    if (CS_PAIR_SKIP && B == 1 && nT >= 2 * SKIPM) {
+        flagU = static_cast<uint8_t *>(scratch) + align_up((size_t)tiles_per * sizeof(uint32_t), 256);
+        flagT = flagU + align_up((size_t)nT * SKIPM, 256);
+        CS_CUDA(cudaMemsetAsync(flagU, 0, 2 * align_up((size_t)nT * SKIPM, 256), st));   // entries no block maps to
+        k_pair_block_flags<<<dim3(nT, SKIPM), 256, 0, st>>>(bits, N, stride, nT, flagU, flagT);
+        CS_LAUNCHED("k_pair_block_flags");
+    }
     const int64_t total = tiles_per * B;
     int64_t clusters = sm_count() / 2;
     if (clusters > total) clusters = total;
@@ -844,7 +941,7 @@ int launch_interval_pair(const uint64_t *bits, const uint64_t *bitsT, int64_t B,
     const int64_t hs_cap = B > 1 ? HS_BATCHED : HS_MAX;
     const int hs = small ? 0 : (int)(kmax + 1 < hs_cap ? kmax + 1 : hs_cap);
 #define CS_PAIR_LAUNCH(S, T) \
-    launch_pair_t<S, T>(mapU, mapL, bits, tab, (uint32_t)tiles_per, clusters, B, N, stride, kmax, hs, row_begin, row_end, hist, nrel, st)
+    launch_pair_t<S, T>(mapU, mapL, bits, tab, flagU, flagT, (uint32_t)tiles_per, clusters, B, N, stride, kmax, hs, row_begin, row_end, hist, nrel, st)
     return small ? CS_PAIR_LAUNCH(true, PAIR_TN) : CS_PAIR_LAUNCH(false, PAIR_TN);
 #undef CS_PAIR_LAUNCH
 }
