@@ -307,8 +307,10 @@ struct Tile {
     int nstages;   // 256-k stages from the first row of I to the last column of J
     int b;         // causet
     bool skip;     // no row of the tile inside [row_begin, row_end)
-    uint32_t head, tail;   // bit m: the bit block U[I][I+m] resp. U[J-m][J] holds a relation (m < SKIPM)
-    bool force0;           // no stage would run: stage 0 runs anyway (the accumulator must be written)
+    // Which stages run (see "empty K blocks"): stages [0, zA) by bit k of liveA, stages [zA, zB) all,
+    // stages [zB, nstages) by bit k - zB of liveB.  Without flags zA = 0, zB = nstages.
+    int zA, zB;
+    uint32_t liveA, liveB;
 };
 
 // ---- empty K blocks -----------------------------------------------------------------------------
@@ -348,15 +350,50 @@ __device__ __forceinline__ uint32_t flags_to_mask(uint4 f)
            ((f.z * 0x01020408u) >> 24 & 0xFu) << 8 | ((f.w * 0x01020408u) >> 24 & 0xFu) << 12;
 }
 
-#ifndef CS_PAIR_BYPASS
-#define CS_PAIR_BYPASS 0    // experiment: bit 0 expanders, 1 loader, 2 issuer, 3 get_tile treat every stage as live
-#endif
-// THE predicate every role uses to decide whether stage k of a tile runs
-__device__ __forceinline__ bool stage_live(const Tile &tc, int k)
+// Stage k of a tile with nstages = n runs unless its U block (head window, k < SKIPM) or its L block (tail
+// window, n-1-k < SKIPM) is empty.  Evaluated once per tile into the zone masks of Tile; the roles only
+// test bits (evaluating this per stage in the expanders, which live on 64 registers, cost 16 %).
+__device__ __forceinline__ bool stage_live(uint32_t head, uint32_t tail, int n, int k)
 {
-    const int kt = tc.nstages - 1 - k;
-    const bool dead = (k < SKIPM && !((tc.head >> k) & 1u)) || (kt < SKIPM && !((tc.tail >> kt) & 1u));
-    return !dead || (tc.force0 && k == 0);
+    const int kt = n - 1 - k;
+    const bool dead = (k < SKIPM && !((head >> k) & 1u)) || (kt < SKIPM && !((tail >> kt) & 1u));
+    return !dead;
+}
+__device__ __forceinline__ void tile_zones(Tile &tc, uint32_t head, uint32_t tail)
+{
+    const int n = tc.nstages;
+    if (n <= 2 * SKIPM) {                           // the windows meet: one zone over the whole tile
+        uint32_t live = 0;
+        for (int k = 0; k < n; k++) live |= (stage_live(head, tail, n, k) ? 1u : 0u) << k;
+        if (live == 0) live = 1;                    // nothing to add, but the accumulator must be written
+        tc.zA = tc.zB = n;
+        tc.liveA = live;
+        tc.liveB = 0;
+    } else {
+        tc.zA = SKIPM;
+        tc.zB = (n - SKIPM) & ~1;                   // even, so that groups of GK = 2 stages never straddle a border
+        tc.liveA = head & ((1u << SKIPM) - 1u);
+        uint32_t live = 0;
+        for (int k = tc.zB; k < n; k++) live |= (stage_live(head, tail, n, k) ? 1u : 0u) << (k - tc.zB);
+        tc.liveB = live;
+    }
+}
+// Calls f(k, first, second) for every group of two stages (k even) of which at least one runs; the
+// loader, the expanders and the MMA issuer all walk a tile with this, so they agree by construction.
+template <typename F>
+__device__ __forceinline__ void for_each_group(const Tile &tc, F f)
+{
+    static_assert(GK == 2 && SKIPM % GK == 0, "zone borders");
+    const int n = tc.nstages;
+    for (int k = 0; k < tc.zA; k += GK) {
+        const uint32_t pair = (tc.liveA >> k) & 3u;     // bits at or beyond nstages are 0
+        if (pair) f(k, (pair & 1u) != 0, (pair & 2u) != 0);
+    }
+    for (int k = tc.zA; k < tc.zB; k += GK) f(k, true, k + 1 < n);
+    for (int k = tc.zB; k < n; k += GK) {
+        const uint32_t pair = (tc.liveB >> (k - tc.zB)) & 3u;
+        if (pair) f(k, (pair & 1u) != 0, (pair & 2u) != 0);
+    }
 }
 
 // SMALL: kmax <= 3 (the Monte-Carlo case, only N_0..N_3 enter Eq. 4.10-4.12): the tally keeps packed
@@ -413,7 +450,7 @@ k_interval_pair(const __grid_constant__ CUtensorMap mapU, const __grid_constant_
             while (sc.idx >= tiles_per) { sc.idx -= tiles_per; sc.b++; }
         }
     };
-    auto get_tile = [&](const Sched &sc) {
+    auto get_tile = [&](const Sched &sc, bool with_zones = true) {
         Tile tc;
         tc.b = (int)sc.b;
         const uint32_t e = __ldg(tile_tab + sc.idx);
@@ -421,17 +458,12 @@ k_interval_pair(const __grid_constant__ CUtensorMap mapU, const __grid_constant_
         tc.J = (int)(e & 0xFFFFu);
         tc.nstages = ((tc.J + 1) * TN - tc.I * TILE + KSTEP - 1) / KSTEP;
         tc.skip = tc.I < ib0 || tc.I >= ib1;
-        tc.head = tc.tail = 0xFFFFu;
-        tc.force0 = false;
-        if (!(CS_PAIR_BYPASS & 8) && flagU) {
-            tc.head = flags_to_mask(__ldg(reinterpret_cast<const uint4 *>(flagU + tc.I * SKIPM)));
-            tc.tail = flags_to_mask(__ldg(reinterpret_cast<const uint4 *>(flagT + tc.J * SKIPM)));
-            if (tc.nstages <= 2 * SKIPM) {          // longer tiles always have a stage outside both windows
-                bool any = false;
-                for (int k = 0; k < tc.nstages; k++) any = any || stage_live(tc, k);
-                tc.force0 = !any;
-            }
-        }
+        tc.zA = 0;
+        tc.zB = tc.nstages;
+        tc.liveA = tc.liveB = 0;
+        if (with_zones && flagU)
+            tile_zones(tc, flags_to_mask(__ldg(reinterpret_cast<const uint4 *>(flagU + tc.I * SKIPM))),
+                       flags_to_mask(__ldg(reinterpret_cast<const uint4 *>(flagT + tc.J * SKIPM))));
         return tc;
     };
 
@@ -581,7 +613,6 @@ k_interval_pair(const __grid_constant__ CUtensorMap mapU, const __grid_constant_
         for (Sched sc = sched_first(); sc.b < (uint32_t)B; sched_next(sc)) {
             const Tile tc = get_tile(sc);
             if (tc.skip) continue;
-            const int nstages = tc.nstages;
             auto do_group = [&](bool first, bool second) {
                 mbar_wait(&s_bfull[b], bph);
                 const unsigned char *src = my_bits + b * BITS_BYTES;
@@ -601,24 +632,7 @@ k_interval_pair(const __grid_constant__ CUtensorMap mapU, const __grid_constant_
                 if (lane == 0) mbar_arrive(&s_bempty[b]);
                 if (++b == NB) { b = 0; bph ^= 1; }
             };
-            // Only the first and the last SKIPM stages of a tile can be empty (stage_live): those zones test
-            // every stage, the stages in between run the plain loop (testing there cost 16 % at N = 65536:
-            // the expanders live on 64 registers).  Zone borders are even, so groups of GK = 2 never straddle.
-            auto checked = [&](int k) {
-                const bool first = stage_live(tc, k), second = k + 1 < nstages && stage_live(tc, k + 1);
-                if (first || second) do_group(first, second);            // the loader skips the same groups
-            };
-            static_assert(GK == 2 && SKIPM % GK == 0, "zone borders");
-            const int z1 = nstages < SKIPM ? nstages : SKIPM;            // [0, z1): head zone
-            int z2 = (nstages - SKIPM) & ~1;                              // [z2, nstages): tail zone
-            if (z2 < z1) z2 = z1;
-            if (!flagU) {
-                for (int k = 0; k < nstages; k += GK) do_group(true, k + 1 < nstages);
-            } else {
-                for (int k = 0; k < z1; k += GK) checked(k);
-                for (int k = z1; k < z2; k += GK) do_group(true, true);
-                for (int k = z2; k < nstages; k += GK) checked(k);
-            }
+            for_each_group(tc, [&](int, bool first, bool second) { do_group(first, second); });
         }
     } else if (warp >= MMA_WARP) {
         asm volatile("setmaxnreg.dec.sync.aligned.u32 40;");
@@ -629,19 +643,16 @@ k_interval_pair(const __grid_constant__ CUtensorMap mapU, const __grid_constant_
             for (Sched sc = sched_first(); sc.b < (uint32_t)B; sched_next(sc)) {
                 const Tile tc = get_tile(sc);
                 if (tc.skip) continue;
-                const int nstages = tc.nstages;
-                const int ngroups = (nstages + GK - 1) / GK;
-                for (int g = 0; g < ngroups; g++) {
-                    if (!(CS_PAIR_BYPASS & 2) && !stage_live(tc, GK * g) && !(GK * g + 1 < nstages && stage_live(tc, GK * g + 1))) continue;
+                for_each_group(tc, [&](int k, bool, bool) {
                     const int b = grp % NB;
                     mbar_wait(&s_bempty[b], ((grp / NB) & 1) ^ 1);
                     mbar_arrive_expect_tx(&s_bfull[b], (uint32_t)BITS_BYTES);   // out-of-bounds is zero-filled
                     unsigned char *dst = s_bits + b * BITS_BYTES;
-                    const int c0 = (tc.I * (KSTEP / 8)) + g * BROW;             // byte column of the first k
+                    const int c0 = (tc.I * (KSTEP / 8)) + (k / GK) * BROW;      // byte column of the first k
                     tma_load_3d(dst, &mapU, c0, tc.I * TILE + (int)rank * TM, tc.b, &s_bfull[b]);
                     tma_load_3d(dst + TM * BROW, &mapL, c0, tc.J * TN + (int)rank * TNH, tc.b, &s_bfull[b]);
                     grp++;
-                }
+                });
             }
         }
         } else if (warp == MMA_WARP && rank == 0) {
@@ -659,14 +670,12 @@ k_interval_pair(const __grid_constant__ CUtensorMap mapU, const __grid_constant_
             for (Sched sc = sched_first(); sc.b < (uint32_t)B; sched_next(sc)) {
                 const Tile tc = get_tile(sc);
                 if (tc.skip) continue;
-                const int nstages = tc.nstages;
                 const uint32_t acc = tile_seq % NACC, use = tile_seq / NACC;     // accumulator and how often it was used
                 mbar_wait_cluster(&s_tempty[acc], (use & 1) ^ 1);         // both epilogues have drained this accumulator
                 tc_fence_after();
                 const uint32_t d_tmem = tmem_base + acc * TN;
                 uint32_t accum = 0;                                       // the first stage that runs overwrites
-                for (int ks = 0; ks < nstages; ks++) {
-                    if (!(CS_PAIR_BYPASS & 4) && !stage_live(tc, ks)) continue;
+                auto issue_stage = [&]() {
                     mbar_wait_cluster(&s_full[s], ph);
                     tc_fence_after();
                     if (elect_one()) {
@@ -682,7 +691,11 @@ k_interval_pair(const __grid_constant__ CUtensorMap mapU, const __grid_constant_
                     __syncwarp();
                     accum = 1;
                     if (++s == NS) { s = 0; ph ^= 1; }
-                }
+                };
+                for_each_group(tc, [&](int, bool first, bool second) {
+                    if (first) issue_stage();
+                    if (second) issue_stage();
+                });
                 if (elect_one()) mma_commit_pair(&s_tfull[acc]);          // accumulator complete, both CTAs
                 __syncwarp();
                 tile_seq++;
@@ -714,7 +727,7 @@ k_interval_pair(const __grid_constant__ CUtensorMap mapU, const __grid_constant_
             }
         };
         for (Sched sc = sched_first(); sc.b < (uint32_t)B; sched_next(sc)) {
-            const Tile tc = get_tile(sc);
+            const Tile tc = get_tile(sc, false);
             if (tc.skip) continue;
             if (tc.b != cur_batch) {   // per-causet histograms: flush before switching
                 if (cur_batch >= 0 && B > 1) {
