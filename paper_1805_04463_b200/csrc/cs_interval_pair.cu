@@ -320,10 +320,11 @@ struct Tile {
 // N = 65536: 96 % of the diagonal blocks, half of those 5 blocks out, none beyond 16; 13.7 % of all stages).
 // flagU[I][m] = block (I, I+m) non-empty, flagT[J][m] = block (J-m, J) non-empty, m < SKIPM.
 constexpr int SKIPM = 16;
+constexpr int SKIP_MIN_TILES = 96;      // N > 24320: below that the flag pass (~10 us) is several % of the whole call
 
 __global__ void __launch_bounds__(256)
 k_pair_block_flags(const uint64_t *__restrict__ bits, int64_t N, int64_t stride, int nT,
-                   uint8_t *__restrict__ flagU, uint8_t *__restrict__ flagT)
+                   uint8_t *__restrict__ flagU, uint8_t *__restrict__ flagT, unsigned int *__restrict__ n_empty)
 {
     const int I = blockIdx.x, m = blockIdx.y, K = I + m;
     if (K >= nT) return;
@@ -340,6 +341,7 @@ k_pair_block_flags(const uint64_t *__restrict__ bits, int64_t N, int64_t stride,
     if (threadIdx.x == 0) {
         flagU[I * SKIPM + m] = (uint8_t)(nz != 0);
         flagT[K * SKIPM + m] = (uint8_t)(nz != 0);
+        if (!nz) atomicAdd(n_empty, 1u);
     }
 }
 
@@ -350,32 +352,29 @@ __device__ __forceinline__ uint32_t flags_to_mask(uint4 f)
            ((f.z * 0x01020408u) >> 24 & 0xFu) << 8 | ((f.w * 0x01020408u) >> 24 & 0xFu) << 12;
 }
 
-// Stage k of a tile with nstages = n runs unless its U block (head window, k < SKIPM) or its L block (tail
-// window, n-1-k < SKIPM) is empty.  Evaluated once per tile into the zone masks of Tile; the roles only
-// test bits (evaluating this per stage in the expanders, which live on 64 registers, cost 16 %).
-__device__ __forceinline__ bool stage_live(uint32_t head, uint32_t tail, int n, int k)
-{
-    const int kt = n - 1 - k;
-    const bool dead = (k < SKIPM && !((head >> k) & 1u)) || (kt < SKIPM && !((tail >> kt) & 1u));
-    return !dead;
-}
+// Stage k of a tile with nstages = n runs unless its U block (head window: k < SKIPM and flagU[I][k] clear) or
+// its L block (tail window: t = n-1-k < SKIPM and flagT[J][t] clear) is empty.  Evaluated once per tile into the
+// zone masks of Tile with bit operations; the roles only test bits (evaluating the predicate per stage in
+// the expanders, which live on 64 registers, cost 16 %).
+__device__ __forceinline__ uint32_t low_mask(int x) { return x >= 32 ? 0xFFFFFFFFu : (1u << x) - 1u; }
 __device__ __forceinline__ void tile_zones(Tile &tc, uint32_t head, uint32_t tail)
 {
     const int n = tc.nstages;
-    if (n <= 2 * SKIPM) {                           // the windows meet: one zone over the whole tile
-        uint32_t live = 0;
-        for (int k = 0; k < n; k++) live |= (stage_live(head, tail, n, k) ? 1u : 0u) << k;
-        if (live == 0) live = 1;                    // nothing to add, but the accumulator must be written
+    const uint32_t deadH = ~head & 0xFFFFu;          // bit k: stage k dead through its U block
+    const uint32_t deadT = ~tail & 0xFFFFu;          // bit t: stage n-1-t dead through its L block
+    if (n <= 2 * SKIPM) {                            // the windows meet: one zone over the whole tile
+        // tail bit t -> stage n-1-t: reverse (bit 31-t), then down by 32-n
+        uint32_t live = ~(deadH | (__brev(deadT) >> (32 - n))) & low_mask(n);
+        if (live == 0) live = 1;                     // nothing to add, but the accumulator must be written
         tc.zA = tc.zB = n;
         tc.liveA = live;
         tc.liveB = 0;
     } else {
         tc.zA = SKIPM;
-        tc.zB = (n - SKIPM) & ~1;                   // even, so that groups of GK = 2 stages never straddle a border
-        tc.liveA = head & ((1u << SKIPM) - 1u);
-        uint32_t live = 0;
-        for (int k = tc.zB; k < n; k++) live |= (stage_live(head, tail, n, k) ? 1u : 0u) << (k - tc.zB);
-        tc.liveB = live;
+        tc.zB = (n - SKIPM) & ~1;                    // even, so that groups of GK = 2 stages never straddle a border
+        tc.liveA = head & 0xFFFFu;
+        const int D = n - 1 - tc.zB;                 // 15 or 16: stage zB + t has tail index D - t
+        tc.liveB = ~(__brev(deadT) >> (31 - D)) & low_mask(D + 1);
     }
 }
 // Calls f(k, first, second) for every group of two stages (k even) of which at least one runs; the
@@ -402,7 +401,8 @@ template <bool SMALL, int TN>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(THREADS, 1)
 k_interval_pair(const __grid_constant__ CUtensorMap mapU, const __grid_constant__ CUtensorMap mapL,
                 const uint64_t *__restrict__ bits, const uint32_t *__restrict__ tile_tab,
-                const uint8_t *__restrict__ flagU, const uint8_t *__restrict__ flagT, uint32_t tiles_per,
+                const uint8_t *__restrict__ flagU, const uint8_t *__restrict__ flagT,
+                const unsigned int *__restrict__ n_empty, int nT_flags, uint32_t tiles_per,
                 int64_t B, int64_t N, int64_t stride, int64_t kmax, int hs, int causet_major,
                 int64_t row_begin, int64_t row_end,
                 unsigned long long *__restrict__ hist, unsigned long long *__restrict__ nrel)
@@ -450,6 +450,9 @@ k_interval_pair(const __grid_constant__ CUtensorMap mapU, const __grid_constant_
             while (sc.idx >= tiles_per) { sc.idx -= tiles_per; sc.b++; }
         }
     };
+    // Testing stages costs a little even when nothing is empty (dS, 1+1 light cone): the flags are used only
+    // if at least 2 % of the examined blocks turned out empty (counted by k_pair_block_flags).
+    const bool use_flags = flagU != nullptr && (uint64_t)__ldg(n_empty) * 50 >= (uint64_t)nT_flags * SKIPM;
     auto get_tile = [&](const Sched &sc, bool with_zones = true) {
         Tile tc;
         tc.b = (int)sc.b;
@@ -461,7 +464,7 @@ k_interval_pair(const __grid_constant__ CUtensorMap mapU, const __grid_constant_
         tc.zA = 0;
         tc.zB = tc.nstages;
         tc.liveA = tc.liveB = 0;
-        if (with_zones && flagU)
+        if (with_zones && use_flags)
             tile_zones(tc, flags_to_mask(__ldg(reinterpret_cast<const uint4 *>(flagU + tc.I * SKIPM))),
                        flags_to_mask(__ldg(reinterpret_cast<const uint4 *>(flagT + tc.J * SKIPM))));
         return tc;
@@ -892,12 +895,12 @@ constexpr int PAIR_TN = 256;
 size_t interval_pair_scratch_bytes(int64_t N)
 {
     const int64_t nT = (N + TILE - 1) / TILE;
-    return align_up((size_t)pair_tiles_per_causet(N) * sizeof(uint32_t), 256) + 2 * align_up((size_t)nT * SKIPM, 256);
+    return align_up((size_t)pair_tiles_per_causet(N) * sizeof(uint32_t), 256) + 2 * align_up((size_t)nT * SKIPM, 256) + 256;
 }
 
 template <bool SMALL, int TN>
 static int launch_pair_t(const CUtensorMap &mapU, const CUtensorMap &mapL, const uint64_t *bits, const uint32_t *tab,
-                         const uint8_t *flagU, const uint8_t *flagT, uint32_t tiles_per, int64_t clusters, int64_t B, int64_t N, int64_t stride, int64_t kmax, int hs,
+                         const uint8_t *flagU, const uint8_t *flagT, const unsigned int *n_empty, int nT, uint32_t tiles_per, int64_t clusters, int64_t B, int64_t N, int64_t stride, int64_t kmax, int hs,
                          int64_t row_begin, int64_t row_end, int64_t *hist, int64_t *nrel, cudaStream_t st)
 {
     static bool attr_set = false;
@@ -910,7 +913,7 @@ static int launch_pair_t(const CUtensorMap &mapU, const CUtensorMap &mapL, const
     const int64_t rounds = (B + clusters - 1) / clusters;
     const int causet_major = (B > 1 && rounds * clusters * 20 <= B * 21) ? 1 : 0;
     k_interval_pair<SMALL, TN><<<(unsigned)(2 * clusters), THREADS, Shape<TN>::SMEM_FIXED + hs * 4, st>>>(
-        mapU, mapL, bits, tab, flagU, flagT, tiles_per, B, N, stride, kmax, hs, causet_major, row_begin, row_end,
+        mapU, mapL, bits, tab, flagU, flagT, n_empty, nT, tiles_per, B, N, stride, kmax, hs, causet_major, row_begin, row_end,
         reinterpret_cast<unsigned long long *>(hist), reinterpret_cast<unsigned long long *>(nrel));
     CS_LAUNCHED("k_interval_pair");
     return CS_OK;
@@ -936,13 +939,15 @@ int launch_interval_pair(const uint64_t *bits, const uint64_t *bitsT, int64_t B,
     uint32_t *tab = static_cast<uint32_t *>(scratch);
     k_pair_tile_order<<<(nT + BANDW - 1) / BANDW, 128, 0, st>>>(nT, tab);
     CS_LAUNCHED("k_pair_tile_order");
-    // empty-block flags: one causet, and enough row tiles for blocks near the diagonal to be empty at all
+    // empty-block flags: one causet, and large enough that the ~10 us of the flag pass cannot matter
     uint8_t *flagU = nullptr, *flagT = nullptr;
-    if (CS_PAIR_SKIP && B == 1 && nT >= 2 * SKIPM) {
+    unsigned int *n_empty = nullptr;
+    if (CS_PAIR_SKIP && B == 1 && nT >= SKIP_MIN_TILES) {
         flagU = static_cast<uint8_t *>(scratch) + align_up((size_t)tiles_per * sizeof(uint32_t), 256);
         flagT = flagU + align_up((size_t)nT * SKIPM, 256);
-        CS_CUDA(cudaMemsetAsync(flagU, 0, 2 * align_up((size_t)nT * SKIPM, 256), st));   // entries no block maps to
-        k_pair_block_flags<<<dim3(nT, SKIPM), 256, 0, st>>>(bits, N, stride, nT, flagU, flagT);
+        n_empty = reinterpret_cast<unsigned int *>(flagT + align_up((size_t)nT * SKIPM, 256));
+        CS_CUDA(cudaMemsetAsync(flagU, 0, 2 * align_up((size_t)nT * SKIPM, 256) + 256, st));   // entries no block maps to, counter
+        k_pair_block_flags<<<dim3(nT, SKIPM), 256, 0, st>>>(bits, N, stride, nT, flagU, flagT, n_empty);
         CS_LAUNCHED("k_pair_block_flags");
     }
     const int64_t total = tiles_per * B;
@@ -954,7 +959,7 @@ int launch_interval_pair(const uint64_t *bits, const uint64_t *bitsT, int64_t B,
     const int64_t hs_cap = B > 1 ? HS_BATCHED : HS_MAX;
     const int hs = small ? 0 : (int)(kmax + 1 < hs_cap ? kmax + 1 : hs_cap);
 #define CS_PAIR_LAUNCH(S, T) \
-    launch_pair_t<S, T>(mapU, mapL, bits, tab, flagU, flagT, (uint32_t)tiles_per, clusters, B, N, stride, kmax, hs, row_begin, row_end, hist, nrel, st)
+    launch_pair_t<S, T>(mapU, mapL, bits, tab, flagU, flagT, n_empty, nT, (uint32_t)tiles_per, clusters, B, N, stride, kmax, hs, row_begin, row_end, hist, nrel, st)
     return small ? CS_PAIR_LAUNCH(true, PAIR_TN) : CS_PAIR_LAUNCH(false, PAIR_TN);
 #undef CS_PAIR_LAUNCH
 }

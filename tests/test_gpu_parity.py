@@ -341,13 +341,13 @@ def test_interval_hist_batched_routes(api, oracle):
 
 
 def test_interval_hist_empty_block_skipping(api, oracle):
-    """N large enough for the pair route to skip K blocks whose 256 x 256 bit block is empty (32+ row tiles):
+    """N large enough for the pair route to skip K blocks whose 256 x 256 bit block is empty (96+ row tiles):
     a 3+1 diamond, the same points with space stretched (most blocks near the diagonal empty, many tiles with
     no live stage at all), a ragged N, row ranges and kmax = 3; all routes that take this size agree with tier-1."""
     cfg = inp.CONFIGS[3]
-    base = inp.sprinkle(cfg.geometry, cfg.dim, 9000, 41)
+    base = inp.sprinkle(cfg.geometry, cfg.dim, 25000, 41)
     stretched = base.copy(); stretched[:, 1:] *= 12.0
-    thin = base[:8300].copy(); thin[:, 1:] *= 3.0
+    thin = base[:24700].copy(); thin[:, 1:] *= 3.0
     for coords in (base, stretched, thin):
         N = coords.shape[0]
         o_bits = oracle.causal_matrix_bits(coords, cfg.geometry)
@@ -359,7 +359,7 @@ def test_interval_hist_empty_block_skipping(api, oracle):
             assert np.array_equal(hist.cpu().numpy(), o_hist)
             assert int(nrel[0]) == int(o_hist.sum())
             assert np.array_equal(api.interval_hist(bits, bitsT, N, kmax=3, route=r).cpu().numpy(), o_hist[:4])
-        cut = 4321
+        cut = 14321
         ha = api.interval_hist(bits, bitsT, N, row_begin=0, row_end=cut)
         hb = api.interval_hist(bits, bitsT, N, row_begin=cut, row_end=N)
         assert np.array_equal((ha + hb).cpu().numpy(), o_hist)
