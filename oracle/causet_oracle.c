@@ -22,11 +22,12 @@
  *   4. (NEXT-1) smeared action, Eq. 4.13-4.18.
  *   5. (NEXT-3) longest chains (Algorithm 11) and the greedy maximal antichain
  *      (Algorithm 13).
+ *   6. (NEXT-4) the FLRW relation of Eq. 7.7 as a fourth predicate of stage 1.
  *
  * Floating point: every predicate is evaluated in fp64 exactly in the order
  * written below; compile with -ffp-contract=off (no FMA), no -ffast-math.
  *
- * Pins (tests/test_oracle_*.py): chain / antichain closed forms, brute-force
+ * Pins (tests/test_oracle_pins.py, tests/test_oracle_chains.py): chain / antichain closed forms, brute-force
  * subset enumeration on N<=64, exhaustive N<=5, sum_k N_k = R,
  * sum_k k N_k = sum_m indeg(m) outdeg(m), inversion-count R and a summed-area
  * table histogram for the 1+1 light-cone diamond, three independent statements
