@@ -67,14 +67,16 @@ enum cs_status {
     CS_ERR_CUDA = -6        /* a CUDA runtime call or launch failed; see cs_last_cuda_error() */
 };
 
-/* How a2 is computed.  Both routes give identical integers. */
+/* How a2 is computed.  All routes give identical integers. */
 enum cs_route {
     CS_ROUTE_AUTO = 0,      /* the library's default for this N */
     CS_ROUTE_POPC = 1,      /* shared-memory tiled AND + POPC (Alg. 20 restated for the GPU) */
     CS_ROUTE_TENSOR = 2,    /* count matrix C.C as a 0/1 int8 contraction on tcgen05 tensor cores */
     CS_ROUTE_TENSOR_FP4 = 3,/* the same contraction with 4-bit (E2M1, unit block scales) operands, fp32 accumulators */
     CS_ROUTE_TENSOR_PAIR = 4/* 4-bit operands on CTA pairs (cta_group::2, 256 x 256 tiles), shift-free expansion with
-                               constant power-of-two block scales, L2-aware tile order */
+                               constant power-of-two block scales, L2-aware tile order; K blocks whose 256 x 256 bit
+                               block is empty are not executed (large single causets).  The default for N >= 1024.
+                               The tensor routes assume bits is upper triangular (as cs_causal_matrix writes it). */
 };
 
 const char *cs_version(void);
