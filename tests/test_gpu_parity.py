@@ -366,6 +366,49 @@ def test_interval_hist_empty_block_skipping(api, oracle):
         assert np.array_equal(ha.cpu().numpy(), oracle.interval_hist_alg20(o_bits, N, 0, cut)[0])
 
 
+def test_interval_hist_random_block_patterns(api, oracle):
+    """The empty-block logic on arbitrary patterns (a sprinkling only produces monotone ones): a random upper
+    triangular relation whose 256 x 256 blocks near the diagonal are emptied at random, a2 on the given bits
+    (count = sum_k U[i][k] U[k][j] over related pairs, whatever U is) against tier-1, incl. a row range."""
+    rng = np.random.default_rng(77)
+    for N, p_empty in ((25000, 0.5), (24900, 0.9), (26000, 0.15)):
+        stride = api.row_stride_words(N)
+        nT = (N + 255) // 256
+        bits = np.zeros((N, stride), dtype=np.uint64)
+        for I in range(nT):
+            r0, r1 = I * 256, min(N, I * 256 + 256)
+            for J in range(I, nT):
+                if J - I < 20 and rng.random() < p_empty:
+                    continue                                   # an empty block
+                if J - I >= 20 and rng.random() < 0.7:
+                    continue                                   # keep the matrix sparse: most far blocks empty too
+                blk = rng.integers(0, 2 ** 63, size=(r1 - r0, 4), dtype=np.int64).astype(np.uint64)
+                blk &= rng.integers(0, 2 ** 63, size=(r1 - r0, 4), dtype=np.int64).astype(np.uint64)
+                blk &= rng.integers(0, 2 ** 63, size=(r1 - r0, 4), dtype=np.int64).astype(np.uint64)   # density 1/8
+                w0 = J * 4
+                w1 = min(stride, w0 + 4)
+                bits[r0:r1, w0:w1] = blk[:, : w1 - w0]
+        # upper triangular (only the diagonal blocks hold bits at or below the diagonal), nothing at or beyond N
+        sh = np.arange(64, dtype=np.uint64)[None, :]
+        for I in range(nT):
+            r0, r1 = I * 256, min(N, I * 256 + 256)
+            rows = np.arange(r0, r1)
+            for w in range(I * 4, min(stride, I * 4 + 4)):
+                cols = np.arange(w * 64, w * 64 + 64)
+                keep = cols[None, :] > rows[:, None]
+                bits[r0:r1, w] &= (keep.astype(np.uint64) << sh).sum(axis=1, dtype=np.uint64)
+        for w in range(N // 64, stride):
+            cols = np.arange(w * 64, w * 64 + 64)
+            bits[:, w] &= np.uint64(((cols < N).astype(np.uint64) << sh[0]).sum(dtype=np.uint64))
+        o_hist, _, _ = oracle.interval_hist_alg20(bits, N)
+        d_bits = torch.from_numpy(bits.view(np.int64)).cuda()
+        d_bitsT = api.transpose_bits(d_bits, N)
+        hist = api.interval_hist(d_bits, d_bitsT, N, route=api.ROUTE_TENSOR_PAIR)
+        assert np.array_equal(hist.cpu().numpy(), o_hist), (N, p_empty)
+        part = api.interval_hist(d_bits, d_bitsT, N, route=api.ROUTE_TENSOR_PAIR, row_begin=5000, row_end=5300)
+        assert np.array_equal(part.cpu().numpy(), oracle.interval_hist_alg20(bits, N, 5000, 5300)[0])
+
+
 # ----------------------------------------------------------------------------- full sizes
 def _full_size_check(api, oracle, cfg, full_hist):
     """Bits compared in full; histogram compared in full (tier-1) or on sampled row ranges plus
