@@ -33,7 +33,6 @@ constexpr int NB = 2;                   // bit-row buffers
 constexpr int EPITCH = 20;              // words per thread row of the epilogue staging area (16 counts + pad)
 constexpr int EPI_BYTES = 256 * EPITCH * 4;
 constexpr int BITS_BYTES = (TM + TN) * BROW;
-constexpr int A_BYTES = TM * KBYTES;    // 16 KiB
 constexpr int B_BYTES = TN * KBYTES;    // 32 KiB
 constexpr int STAGE_BYTES = B_BYTES;     // the A operand of a stage lives in 32 TMEM columns
 constexpr int HS = 2048;                // shared-memory histogram bins
