@@ -23,6 +23,10 @@
  *     bit (j & 63) of block (j >> 6), LSB first; padding bits are zero.
  *   - elements must be sorted by non-decreasing time coordinate
  *     so that i -< j implies i < j; only pairs i < j are ever tested.
+ *   - threads and devices: calls may come from several host threads and for several devices of one
+ *     process (the device is the calling thread's current one; everything the library caches on the host
+ *     is keyed by it).  Two calls that share a workspace, or two *_host calls on the same device, must
+ *     not run concurrently.
  */
 #ifndef CAUSALSET_H
 #define CAUSALSET_H
@@ -119,7 +123,8 @@ int cs_degrees(const uint64_t *bits, const uint64_t *bitsT, int64_t N, int64_t *
 /* a2: interval abundances (Alg. 19; Alg. 20).
  * For every related pair i -< j:  c = |{k : i -< k -< j}| = popcount(bits[i] & bitsT[j]);  hist[c] += 1.
  * hist[k] = n_{k+1} in the paper's notation (Eq. 4.8).
- *   bits, bitsT  device, as produced by cs_causal_matrix.  bitsT may be NULL: it is then
+ *   bits, bitsT  device, as produced by cs_causal_matrix; 16-byte aligned (rows are read with 128-bit
+ *                loads, bulk copies and TMA; CS_ERR_ARG otherwise).  bitsT may be NULL: it is then
  *                rebuilt inside the workspace (query the size with have_bitsT = 0).
  *   kmax         largest interval size kept; kmax < 0 or kmax > N-2 means N-2.
  *   hist         device, int64[kmax+1] (after clamping; at least 1 entry), overwritten.
@@ -137,6 +142,15 @@ int cs_interval_hist_ex(const uint64_t *bits, const uint64_t *bitsT, int64_t N, 
                         int64_t row_begin, int64_t row_end, int route,
                         int64_t *hist, int64_t *n_relations,
                         void *workspace, size_t workspace_bytes, void *stream);
+/* What the last cs_interval_hist* call that used `workspace` executed (for the roofline on executed work):
+ *   stats_host  host, int64[4], overwritten:
+ *     [0] (tile, stage) pairs whose MMAs were issued: a stage is 256 rows x 256 columns x 256 k of the 0/1
+ *         contraction = 2 * 256^3 tensor ops (CS_ROUTE_TENSOR_PAIR; 0 for the other routes),
+ *     [1] the same count with no empty block skipped (the dense-triangular tile set of the row range),
+ *     [2] empty 256 x 256 bit blocks found by the flag pass, [3] blocks it examined (0 if it did not run).
+ * Copies 64 bytes device->host and synchronises `stream`.  Errors: CS_ERR_ARG, CS_ERR_CUDA. */
+int cs_interval_hist_stats(const void *workspace, int64_t *stats_host, void *stream);
+
 /* NEXT-3: chains and antichains on the bit matrix (Algorithms 11-13).
  * Both take bits and bitsT as written by cs_causal_matrix and a workspace of cs_poset_workspace(N) bytes
  * (256-byte aligned).
@@ -233,6 +247,30 @@ size_t cs_bd_action_batched_host_workspace(int64_t B, int64_t N, int dim);
 int cs_bd_action_batched_host(const double *coords_host, int64_t B, int64_t N, int dim, int geometry,
                               double *actions_host, int64_t *hist4_host,
                               void *workspace, size_t workspace_bytes, void *stream);
+
+/* Peak probes -- a measurement aid for the rooflines bench.py reports ("pipe utilisation vs the
+ * measured peaks"), not a step of the path.  Each probe saturates one unit with the instruction the path's
+ * kernels use on it and synchronises before returning.
+ *   iters      inner iterations (MMAs for the tensor probes); clamped to [4, 2^22].
+ *   workspace  device, 256-byte aligned, >= 64 KiB; the HBM probes stream over everything beyond the first
+ *              64 KiB and need >= 256 MiB there (CS_ERR_WORKSPACE otherwise).
+ *   out_host   host, double[3]: {units executed, seconds (CUDA events), units per clock per SM (in-kernel
+ *              clock64 of the slowest CTA; 0 for the HBM probes)}.  Units: tensor probes -- operations (2 per
+ *              multiply-add); POPC / DFMA / FFMA -- lane-instructions; FFMA2 -- fused multiply-adds (two per
+ *              lane-instruction); HBM -- bytes (copy: read + written); TMEM_LD -- bytes. */
+enum cs_peak_kind {
+    CS_PEAK_MXF4_PAIR = 0,  /* tcgen05.mma.cta_group::2.kind::mxf4.block_scale M=256 N=256 K=64 (k_interval_pair's) */
+    CS_PEAK_I8 = 1,         /* tcgen05.mma.cta_group::1.kind::i8 M=128 N=256 K=32 (k_interval_tensor's) */
+    CS_PEAK_POPC = 2,       /* POPC.32 */
+    CS_PEAK_DFMA = 3,       /* fp64 fused multiply-add */
+    CS_PEAK_FFMA = 4,       /* fp32 fused multiply-add */
+    CS_PEAK_FFMA2 = 5,      /* fma.rn.f32x2 */
+    CS_PEAK_HBM_WRITE = 6,  /* 128-bit stores */
+    CS_PEAK_HBM_COPY = 7,   /* 128-bit loads + stores */
+    CS_PEAK_TMEM_LD4 = 8,   /* tcgen05.ld 32x32b.x32, one warp per TMEM lane quarter */
+    CS_PEAK_TMEM_LD8 = 9    /* the same from two warps per lane quarter */
+};
+int cs_peak_probe(int kind, int64_t iters, void *workspace, size_t workspace_bytes, double *out_host, void *stream);
 
 /* Number of kernel launches issued by this library in this process so far (for bench.py's
  * `gpu_launches`). */

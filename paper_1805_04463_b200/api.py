@@ -49,6 +49,7 @@ _SIGNATURES = {
     "cs_interval_hist_workspace": (_sz, [_i64, _i64, _int, _int]),
     "cs_interval_hist": (_int, [_p, _p, _i64, _i64, _p, _p, _p, _sz, _p]),
     "cs_interval_hist_ex": (_int, [_p, _p, _i64, _i64, _i64, _i64, _int, _p, _p, _p, _sz, _p]),
+    "cs_interval_hist_stats": (_int, [_p, _p, _p]),
     "cs_interval_hist_batched_workspace": (_sz, [_i64, _i64, _int]),
     "cs_interval_hist_batched": (_int, [_p, _p, _i64, _i64, _i64, _int, _p, _p, _sz, _p]),
     "cs_default_route": (_int, [_i64]),
@@ -64,6 +65,7 @@ _SIGNATURES = {
     "cs_action_host_workspace": (_sz, [_i64, _i64]),
     "cs_action_host": (_int, [_p, _i64, _int, _int, _i64, _p, _p, _p, _sz, _p]),
     "cs_launch_count": (_i64, []),
+    "cs_peak_probe": (_int, [_int, _i64, _p, _sz, _p, _p]),
 }
 
 _lib = None
@@ -121,6 +123,18 @@ def launch_count() -> int:
 
 def default_route(N: int) -> int:
     return int(load().cs_default_route(N))
+
+
+PEAK_KINDS = {"mxf4_pair": 0, "i8": 1, "popc": 2, "dfma": 3, "ffma": 4, "ffma2": 5, "hbm_write": 6, "hbm_copy": 7,
+              "tmem_ld4": 8, "tmem_ld8": 9}
+
+
+def peak_probe(kind: str, iters: int, workspace: torch.Tensor):
+    """-> (units, seconds, units per clock per SM) of one peak probe (include/causalset.h, cs_peak_kind)."""
+    out = (ctypes.c_double * 3)()
+    _check(load().cs_peak_probe(PEAK_KINDS[kind], iters, _dptr(workspace), workspace.numel(), ctypes.addressof(out),
+                                _stream()), "cs_peak_probe")
+    return float(out[0]), float(out[1]), float(out[2])
 
 
 def causal_matrix(coords: torch.Tensor, geometry: int, want_transpose: bool = True):
@@ -192,6 +206,13 @@ def interval_hist(bits: torch.Tensor, bitsT, N: int, kmax: int = -1, route: int 
                                       _dptr(hist), _dptr(nrel), _dptr(ws), ws.numel(), _stream()),
            "cs_interval_hist_ex")
     return (hist, nrel) if return_relations else hist
+
+
+def interval_hist_stats(workspace: torch.Tensor):
+    """-> (stages_executed, stages_total, blocks_empty, blocks_examined) of the last a2 call on `workspace`."""
+    out = (ctypes.c_int64 * 4)()
+    _check(load().cs_interval_hist_stats(_dptr(workspace), ctypes.addressof(out), _stream()), "cs_interval_hist_stats")
+    return tuple(int(x) for x in out)
 
 
 def interval_hist_batched(bits: torch.Tensor, bitsT: torch.Tensor, N: int, kmax: int = -1,

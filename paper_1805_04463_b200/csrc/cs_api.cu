@@ -1,30 +1,36 @@
 // cs_api.cu -- the extern "C" boundary of libcausalset.so (include/causalset.h).
 // Argument checking, workspace carving and kernel sequencing only; the arithmetic lives in
 // cs_poset.cu (NEXT-3), cs_build.cu (a1), cs_interval_popc.cu / cs_interval_tensor.cu / cs_interval_fp4.cu / cs_interval_pair.cu (a2) and cs_action.cu (a3).
+#include <mutex>
+
 #include "cs_common.cuh"
 
 namespace cs {
 
 thread_local char g_cuda_err[256] = "";
-long long g_launches = 0;
+std::atomic<long long> g_launches{0};
 
 int sm_count()
 {
-    static int cached = 0;
-    if (cached <= 0) {
-        int dev = 0, n = 0;
-        if (cudaGetDevice(&dev) == cudaSuccess &&
-            cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && n > 0)
-            cached = n;
-        else
-            return 148;
+    static std::atomic<int> cached[MAX_DEVICES];
+    const int dev = current_device();
+    int n = cached[dev].load(std::memory_order_relaxed);
+    if (n <= 0) {
+        if (cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n <= 0) return 148;
+        cached[dev].store(n, std::memory_order_relaxed);
     }
-    return cached;
+    return n;
 }
 
 // spacetime dimension of a point set: the number of coordinates, except for the FLRW geometry whose six
 // numbers per point describe a 3+1 dimensional event
 static int spacetime_dim(int geometry, int dim) { return geometry == CS_GEOM_FLRW_POLAR ? 4 : dim; }
+
+// rows are read with 128-bit loads, bulk copies and TMA: the matrices must start on a 16-byte boundary
+static bool misaligned16(const void *a, const void *b)
+{
+    return (((uintptr_t)a | (uintptr_t)b) & 15) != 0;
+}
 
 static int resolve_route(int64_t N, int route)
 {
@@ -60,6 +66,7 @@ static int interval_hist_impl(const uint64_t *bits, const uint64_t *bitsT, int64
     if (!workspace || workspace_bytes < need || ((uintptr_t)workspace & 255)) return CS_ERR_WORKSPACE;
     unsigned char *ws = static_cast<unsigned char *>(workspace);
     void *scratch = ws;
+    CS_CUDA(cudaMemsetAsync(scratch, 0, 256, st));   // IntervalStats
     ws += 256;
     if (!bitsT) {
         uint64_t *t = reinterpret_cast<uint64_t *>(ws);
@@ -70,7 +77,8 @@ static int interval_hist_impl(const uint64_t *bits, const uint64_t *bitsT, int64
     }
     if (route == CS_ROUTE_TENSOR_PAIR)
         return launch_interval_pair(bits, bitsT, B, N, kmax, row_begin, row_end, hist, nrel, ws,
-                                    workspace_bytes - (size_t)(ws - static_cast<unsigned char *>(workspace)), st);
+                                    workspace_bytes - (size_t)(ws - static_cast<unsigned char *>(workspace)),
+                                    static_cast<IntervalStats *>(scratch), st);
     if (route == CS_ROUTE_TENSOR_FP4)
         return launch_interval_fp4(bits, bitsT, B, N, kmax, row_begin, row_end, hist, nrel, ws,
                                    workspace_bytes - (size_t)(ws - static_cast<unsigned char *>(workspace)), st);
@@ -106,7 +114,13 @@ const char *cs_last_cuda_error(void) { return g_cuda_err; }
 
 int64_t cs_row_stride_words(int64_t N) { return N < 0 ? 0 : row_stride_words(N); }
 
-int64_t cs_launch_count(void) { return g_launches; }
+int64_t cs_launch_count(void) { return g_launches.load(); }
+
+int cs_peak_probe(int kind, int64_t iters, void *workspace, size_t workspace_bytes, double *out_host, void *stream)
+{
+    if (!out_host) return CS_ERR_ARG;
+    return launch_peak_probe(kind, iters, workspace, workspace_bytes, out_host, static_cast<cudaStream_t>(stream));
+}
 
 int cs_default_route(int64_t N)
 {
@@ -170,6 +184,7 @@ int cs_interval_hist_ex(const uint64_t *bits, const uint64_t *bitsT, int64_t N, 
 {
     if (N < 0 || !hist || (N > 0 && !bits)) return CS_ERR_ARG;
     if (route < CS_ROUTE_AUTO || route > CS_ROUTE_TENSOR_PAIR) return CS_ERR_ARG;
+    if (misaligned16(bits, bitsT)) return CS_ERR_ARG;
     return interval_hist_impl(bits, bitsT, 1, N, kmax, row_begin, row_end, route, hist, n_relations,
                               workspace, workspace_bytes, static_cast<cudaStream_t>(stream));
 }
@@ -189,6 +204,7 @@ int cs_interval_hist_batched(const uint64_t *bits, const uint64_t *bitsT, int64_
     if (B == 0) return CS_OK;
     if (N > 0 && (!bits || !bitsT)) return CS_ERR_ARG;
     if (route < CS_ROUTE_AUTO || route > CS_ROUTE_TENSOR_PAIR) return CS_ERR_ARG;
+    if (misaligned16(bits, bitsT)) return CS_ERR_ARG;
     return interval_hist_impl(bits, bitsT, B, N, kmax, 0, N, route, hist, nullptr,
                               workspace, workspace_bytes, static_cast<cudaStream_t>(stream));
 }
@@ -199,6 +215,20 @@ int cs_interval_hist(const uint64_t *bits, const uint64_t *bitsT, int64_t N, int
 {
     return cs_interval_hist_ex(bits, bitsT, N, kmax, 0, N, CS_ROUTE_AUTO, hist, n_relations,
                                workspace, workspace_bytes, stream);
+}
+
+int cs_interval_hist_stats(const void *workspace, int64_t *stats_host, void *stream)
+{
+    if (!workspace || !stats_host || ((uintptr_t)workspace & 255)) return CS_ERR_ARG;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    IntervalStats h;
+    CS_CUDA(cudaMemcpyAsync(&h, workspace, sizeof(h), cudaMemcpyDeviceToHost, st));
+    CS_CUDA(cudaStreamSynchronize(st));
+    stats_host[0] = (int64_t)h.stages_executed;
+    stats_host[1] = (int64_t)h.stages_total;
+    stats_host[2] = (int64_t)h.blocks_empty;
+    stats_host[3] = (int64_t)h.blocks_examined;
+    return CS_OK;
 }
 
 int cs_bd_action(const int64_t *hist, int64_t kmax, int64_t N, int dim,
@@ -287,6 +317,42 @@ int cs_bd_action_batched(const double *coords, int64_t B, int64_t N, int dim, in
 // workspace: [coords chunk x2][bits chunk][bitsT chunk][hist CB*4][actions B][hist4 B*4][interval scratch]
 static int64_t ensemble_chunk(int64_t B) { return B < 512 ? B : 512; }
 
+// copy stream and events of the host pipeline, one set per device, created under a lock on first use;
+// a partial failure destroys what was created so that the next call starts over
+struct CopyPipe {
+    cudaStream_t stream = nullptr;
+    cudaEvent_t copied[2] = {nullptr, nullptr}, consumed[2] = {nullptr, nullptr}, start = nullptr;
+    bool ready = false;
+};
+static int copy_pipe(CopyPipe **out)
+{
+    static CopyPipe pipes[MAX_DEVICES];
+    static std::mutex mu;
+    std::lock_guard<std::mutex> lock(mu);
+    CopyPipe &p = pipes[current_device()];
+    if (!p.ready) {
+        cudaError_t e = cudaStreamCreateWithFlags(&p.stream, cudaStreamNonBlocking);
+        for (int i = 0; i < 2 && e == cudaSuccess; i++) {
+            e = cudaEventCreateWithFlags(&p.copied[i], cudaEventDisableTiming);
+            if (e == cudaSuccess) e = cudaEventCreateWithFlags(&p.consumed[i], cudaEventDisableTiming);
+        }
+        if (e == cudaSuccess) e = cudaEventCreateWithFlags(&p.start, cudaEventDisableTiming);
+        if (e != cudaSuccess) {
+            for (int i = 0; i < 2; i++) {
+                if (p.copied[i]) cudaEventDestroy(p.copied[i]);
+                if (p.consumed[i]) cudaEventDestroy(p.consumed[i]);
+            }
+            if (p.start) cudaEventDestroy(p.start);
+            if (p.stream) cudaStreamDestroy(p.stream);
+            p = CopyPipe();
+            return cuda_fail(e, "host pipeline set-up");
+        }
+        p.ready = true;
+    }
+    *out = &p;
+    return CS_OK;
+}
+
 size_t cs_bd_action_batched_host_workspace(int64_t B, int64_t N, int dim)
 {
     if (B < 0 || N < 0 || dim < 2 || dim > 6) return 0;
@@ -308,16 +374,11 @@ int cs_bd_action_batched_host(const double *coords_host, int64_t B, int64_t N, i
     if (!workspace || workspace_bytes < cs_bd_action_batched_host_workspace(B, N, dim) || ((uintptr_t)workspace & 255))
         return CS_ERR_WORKSPACE;
     cudaStream_t st = static_cast<cudaStream_t>(stream);
-    static cudaStream_t copy_stream = nullptr;
-    static cudaEvent_t copied[2] = {nullptr, nullptr}, consumed[2] = {nullptr, nullptr}, start = nullptr;
-    if (!copy_stream) {
-        CS_CUDA(cudaStreamCreateWithFlags(&copy_stream, cudaStreamNonBlocking));
-        for (int i = 0; i < 2; i++) {
-            CS_CUDA(cudaEventCreateWithFlags(&copied[i], cudaEventDisableTiming));
-            CS_CUDA(cudaEventCreateWithFlags(&consumed[i], cudaEventDisableTiming));
-        }
-        CS_CUDA(cudaEventCreateWithFlags(&start, cudaEventDisableTiming));
-    }
+    CopyPipe *pipe = nullptr;
+    int prc = copy_pipe(&pipe);
+    if (prc) return prc;
+    cudaStream_t copy_stream = pipe->stream;
+    cudaEvent_t *copied = pipe->copied, *consumed = pipe->consumed, start = pipe->start;
     const int64_t CB = ensemble_chunk(B);
     const size_t cbuf = align_up((size_t)CB * N * dim * 8, 256);
     const size_t mat = align_up((size_t)CB * N * row_stride_words(N) * 8, 256);

@@ -217,6 +217,9 @@ k_causal_matrix(const double *__restrict__ coords, int64_t N, int64_t stride,
     __shared__ __align__(16) uint32_t s_U[BT][NJ * 8 + 1]; // row i_local, 32-bit word = 32 columns j
     __shared__ uint32_t s_L[NJ * BT][9];                   // row j_local, 32-bit word = 32 rows i
     uint32_t (*s_red)[NW] = reinterpret_cast<uint32_t (*)[NW]>(&s_U[0][0]);   // [2 + 2 NJ][NW], dead before s_U is written
+    // static shared memory stops at 48 KB; the flat cone in 3+1 dimensions sits exactly on it
+    static_assert(sizeof(s_xi) + sizeof(s_fi) + sizeof(s_hi) + sizeof(s_U) + sizeof(s_L) <= 48 * 1024,
+                  "k_causal_matrix: static shared memory");
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const double qnan = __longlong_as_double(0x7FF8000000000000LL);   // compares false: unrelated

@@ -2,6 +2,8 @@
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
+
+#include <atomic>
 #include <stdio.h>
 #include <string.h>
 
@@ -10,7 +12,7 @@
 namespace cs {
 
 extern thread_local char g_cuda_err[256];
-extern long long g_launches;   // kernels launched by this library (host counter)
+extern std::atomic<long long> g_launches;   // kernels launched by this library (host counter)
 
 inline int cuda_fail(cudaError_t e, const char *what)
 {
@@ -47,7 +49,34 @@ inline int64_t clamp_kmax(int64_t N, int64_t kmax)
 
 inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 
-int sm_count();   // SMs of the current device (cached)
+// Per-device host state.  The library may be called from several threads and on several devices of one
+// process: everything cached on the host is keyed by the current device, and one-time set-up that is
+// idempotent (cudaFuncSetAttribute) is guarded by an atomic flag per device rather than a lock.
+constexpr int MAX_DEVICES = 64;
+inline int current_device()
+{
+    int d = 0;
+    if (cudaGetDevice(&d) != cudaSuccess || d < 0 || d >= MAX_DEVICES) d = 0;
+    return d;
+}
+struct PerDeviceFlag {
+    std::atomic<bool> done[MAX_DEVICES];
+    bool get(int dev) const { return done[dev].load(std::memory_order_acquire); }
+    void set(int dev) { done[dev].store(true, std::memory_order_release); }
+};
+
+int sm_count();   // SMs of the current device (cached per device)
+
+// First 256 bytes of every a2 workspace: scheduling counters of the route and what the launch executed
+// (read back through cs_interval_hist_stats).
+struct IntervalStats {
+    unsigned long long sched[4];          // route-private (POPC: the tile counter)
+    unsigned long long stages_executed;   // (tile, 256-k stage) pairs whose MMAs were issued (pair route)
+    unsigned long long stages_total;      // the same count with no empty block skipped
+    unsigned long long blocks_empty;      // empty 256 x 256 bit blocks among those examined (pair route)
+    unsigned long long blocks_examined;
+};
+static_assert(sizeof(IntervalStats) <= 256, "stats block");
 
 // ---- stage launchers (defined in the .cu files) ---------------------------------------------
 int launch_causal_matrix(const double *coords, int64_t B, int64_t N, int dim, int geometry,
@@ -71,12 +100,14 @@ int launch_interval_fp4(const uint64_t *bits, const uint64_t *bitsT, int64_t B, 
                         void *scratch, size_t scratch_bytes, cudaStream_t st);
 int launch_interval_pair(const uint64_t *bits, const uint64_t *bitsT, int64_t B, int64_t N, int64_t kmax,
                          int64_t row_begin, int64_t row_end, int64_t *hist, int64_t *nrel,
-                         void *scratch, size_t scratch_bytes, cudaStream_t st);
+                         void *scratch, size_t scratch_bytes, IntervalStats *stats, cudaStream_t st);
 size_t interval_pair_scratch_bytes(int64_t N);
 bool interval_tensor_available();
 
 int launch_bd_action(const int64_t *hist, int64_t hist_stride, int64_t B, int64_t kmax, int64_t N, int dim,
                      double *action, int64_t *bracket, int64_t *hist4, cudaStream_t st);
+
+int launch_peak_probe(int kind, int64_t iters, void *workspace, size_t workspace_bytes, double *out_host, cudaStream_t st);
 
 size_t poset_workspace_bytes(int64_t N);
 int launch_chain_heights(const uint64_t *bits, const uint64_t *bitsT, int64_t N, int64_t source,

@@ -493,10 +493,11 @@ int launch_interval_fp4(const uint64_t *bits, const uint64_t *bitsT, int64_t B, 
                            void *, size_t, cudaStream_t st)
 {
     if (N > ((int64_t)1 << 24)) return CS_ERR_ARG;   // counts must stay exact in fp32
-    static bool attr_set = false;
-    if (!attr_set) {
+    static PerDeviceFlag attr_set;
+    const int dev = current_device();
+    if (!attr_set.get(dev)) {
         CS_CUDA(cudaFuncSetAttribute(k_interval_fp4, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES));
-        attr_set = true;
+        attr_set.set(dev);
     }
     const int64_t stride = row_stride_words(N);
     CUtensorMap mapU, mapL;

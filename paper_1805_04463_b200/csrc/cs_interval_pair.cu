@@ -53,22 +53,10 @@ struct Shape {
     static constexpr uint32_t IDESC =
         (1u << 7) | (1u << 10) | ((uint32_t)(TN >> 3) << 17) | (1u << 23) | ((uint32_t)(256 >> 4) << 24);
 };
-#ifndef CS_PAIR_HS_MAX
-#define CS_PAIR_HS_MAX 16896
-#endif
-constexpr int HS_MAX = CS_PAIR_HS_MAX;   // shared-memory histogram bins that fit beside the operand rings
+constexpr int HS_MAX = 16896;           // shared-memory histogram bins that fit beside the operand rings
 constexpr int HS_BATCHED = 2048;        // bins when several causets share a CTA (flushed at every switch)
 constexpr int BANDW = 8;                // diagonals (in 256-column units) per band of the tile order
 
-#ifndef CS_PAIR_DIAG
-#define CS_PAIR_DIAG 0      // timing experiments only (results are wrong): 1 no B stores, 2 no A stores, 4 no tally
-#endif
-#ifndef CS_PAIR_SKIP
-#define CS_PAIR_SKIP 1      // skip K blocks whose bit block is empty (k_pair_block_flags)
-#endif
-#ifndef CS_PAIR_ROT_IMAD
-#define CS_PAIR_ROT_IMAD 0
-#endif
 // five warpgroups: 0-1 epilogue (warp & 3 = TMEM lane quarter, warp >> 2 = column half), 2 A expanders,
 // 3 B expanders, 4 = MMA issuer, TMA loader and two idle warps.  The epilogue keeps a whole accumulator
 // row slice (128 columns) in registers, so registers are re-split by warpgroup with setmaxnreg.
@@ -255,7 +243,6 @@ __device__ __forceinline__ void tmem_st16(uint32_t taddr, const uint32_t (&v)[16
 template <int Q>
 __device__ __forceinline__ uint32_t nib(uint32_t x)
 {
-    if (CS_PAIR_DIAG & 8) return x;
     if (Q == 0) return x & 0x11111111u;
     if (Q == 1) return x & 0x22222222u;
     return x & 0x44444444u;
@@ -405,7 +392,8 @@ k_interval_pair(const __grid_constant__ CUtensorMap mapU, const __grid_constant_
                 const unsigned int *__restrict__ n_empty, int nT_flags, uint32_t tiles_per,
                 int64_t B, int64_t N, int64_t stride, int64_t kmax, int hs, int causet_major,
                 int64_t row_begin, int64_t row_end,
-                unsigned long long *__restrict__ hist, unsigned long long *__restrict__ nrel)
+                unsigned long long *__restrict__ hist, unsigned long long *__restrict__ nrel,
+                IntervalStats *__restrict__ stats, unsigned long long stages_total, unsigned long long blocks_examined)
 {
     extern __shared__ __align__(1024) unsigned char smem[];
     unsigned char *s_stage = smem;
@@ -525,18 +513,8 @@ k_interval_pair(const __grid_constant__ CUtensorMap mapU, const __grid_constant_
         const unsigned char *my_bits = s_bits + (isA ? 0 : TM * BROW) + r * BROW;
         const int swz = (r >> 1) & 3;
         const int off0 = (0 ^ swz) << 4, off1 = (1 ^ swz) << 4, off2 = (2 ^ swz) << 4, off3 = (3 ^ swz) << 4;
-        // bit 3 of every nibble: rotate left by one, then mask; the rotation is an IMAD.WIDE by a 2
-        // the compiler cannot see (FMA pipe) so that the ALU pipe only runs the 32 masks per stage
-        const uint32_t two = 2u | (uint32_t)((uint64_t)N >> 40);
-        auto nib3 = [&](uint32_t x) {
-#if CS_PAIR_ROT_IMAD
-            const uint64_t p = (uint64_t)x * two;
-            return ((uint32_t)p | (uint32_t)(p >> 32)) & 0x11111111u;
-#else
-            (void)two;
-            return (x >> 3) & 0x11111111u;
-#endif
-        };
+        // bit 3 of every nibble is the only one that needs a shift
+        auto nib3 = [&](uint32_t x) { return (x >> 3) & 0x11111111u; };
         uint32_t s = 0, ph = 0;    // operand ring position and phase
         uint32_t b = 0, bph = 0;   // bit-buffer ring position and phase
         const uint32_t a_taddr = tmem_base + ((uint32_t)((warp & 3) * 32) << 16) + A_COL;
@@ -549,7 +527,7 @@ k_interval_pair(const __grid_constant__ CUtensorMap mapU, const __grid_constant_
             if (isA) {
                 asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
                 tc_fence_before();
-            } else if (!(CS_PAIR_DIAG & 16)) {
+            } else {
                 fence_proxy_async();   // generic-proxy stores -> visible to the tensor cores
             }
             __syncwarp();
@@ -566,13 +544,13 @@ k_interval_pair(const __grid_constant__ CUtensorMap mapU, const __grid_constant_
             }
             mbar_wait(&s_empty[s], ph ^ 1);
             tc_fence_after();
-            if (!(CS_PAIR_DIAG & 2)) tmem_st16(a_taddr + s * 32, lo);
+            tmem_st16(a_taddr + s * 32, lo);
 #pragma unroll
             for (int j = 0; j < 8; j++) {
                 hi[j] = nib<2>(xs[j]);
-                hi[8 + j] = (CS_PAIR_DIAG & 8) ? xs[j] : nib3(xs[j]);
+                hi[8 + j] = nib3(xs[j]);
             }
-            if (!(CS_PAIR_DIAG & 2)) tmem_st16(a_taddr + s * 32 + 16, hi);
+            tmem_st16(a_taddr + s * 32 + 16, hi);
             publish(s);
             if (++s == NS) { s = 0; ph ^= 1; }
         };
@@ -583,13 +561,12 @@ k_interval_pair(const __grid_constant__ CUtensorMap mapU, const __grid_constant_
             w[0] = make_uint4(nib<0>(xs[0]), nib<0>(xs[1]), nib<0>(xs[2]), nib<0>(xs[3]));
             w[1] = make_uint4(nib<1>(xs[0]), nib<1>(xs[1]), nib<1>(xs[2]), nib<1>(xs[3]));
             w[2] = make_uint4(nib<2>(xs[0]), nib<2>(xs[1]), nib<2>(xs[2]), nib<2>(xs[3]));
-            if (CS_PAIR_DIAG & 8) w[3] = c;
-            else w[3] = make_uint4(nib3(xs[0]), nib3(xs[1]), nib3(xs[2]), nib3(xs[3]));
+            w[3] = make_uint4(nib3(xs[0]), nib3(xs[1]), nib3(xs[2]), nib3(xs[3]));
             mbar_wait(&s_empty[s], ph ^ 1);
             unsigned char *dst = b_dst + s * STAGE_BYTES + bhalf * TNH * 16;
 #pragma unroll
             for (int q = 0; q < 4; q++)
-                if (!(CS_PAIR_DIAG & 1)) *reinterpret_cast<uint4 *>(dst + 2 * q * TNH * 16) = w[q];
+                *reinterpret_cast<uint4 *>(dst + 2 * q * TNH * 16) = w[q];
             publish(s);
             if (++s == NS) { s = 0; ph ^= 1; }
         };
@@ -601,14 +578,13 @@ k_interval_pair(const __grid_constant__ CUtensorMap mapU, const __grid_constant_
                 w[0 + h] = make_uint4(nib<0>(xs[4 * h]), nib<0>(xs[4 * h + 1]), nib<0>(xs[4 * h + 2]), nib<0>(xs[4 * h + 3]));
                 w[2 + h] = make_uint4(nib<1>(xs[4 * h]), nib<1>(xs[4 * h + 1]), nib<1>(xs[4 * h + 2]), nib<1>(xs[4 * h + 3]));
                 w[4 + h] = make_uint4(nib<2>(xs[4 * h]), nib<2>(xs[4 * h + 1]), nib<2>(xs[4 * h + 2]), nib<2>(xs[4 * h + 3]));
-                if (CS_PAIR_DIAG & 8) w[6 + h] = make_uint4(xs[4 * h], xs[4 * h + 1], xs[4 * h + 2], xs[4 * h + 3]);
-                else w[6 + h] = make_uint4(nib3(xs[4 * h]), nib3(xs[4 * h + 1]), nib3(xs[4 * h + 2]), nib3(xs[4 * h + 3]));
+                w[6 + h] = make_uint4(nib3(xs[4 * h]), nib3(xs[4 * h + 1]), nib3(xs[4 * h + 2]), nib3(xs[4 * h + 3]));
             }
             mbar_wait(&s_empty[s], ph ^ 1);
             unsigned char *dst = b_dst + s * STAGE_BYTES;
 #pragma unroll
             for (int q = 0; q < 8; q++)
-                if (!(CS_PAIR_DIAG & 1)) *reinterpret_cast<uint4 *>(dst + q * TNH * 16) = w[q];
+                *reinterpret_cast<uint4 *>(dst + q * TNH * 16) = w[q];
             publish(s);
             if (++s == NS) { s = 0; ph ^= 1; }
         };
@@ -670,6 +646,7 @@ k_interval_pair(const __grid_constant__ CUtensorMap mapU, const __grid_constant_
             const uint32_t a_tmem0 = tmem_base + A_COL;
             const uint32_t sf0 = tmem_base + sf_col(0), sf1 = tmem_base + sf_col(1), sf2 = tmem_base + sf_col(2);
             uint32_t s = 0, ph = 0, tile_seq = 0;
+            unsigned long long issued = 0;      // stages this pair executed (for cs_interval_hist_stats)
             for (Sched sc = sched_first(); sc.b < (uint32_t)B; sched_next(sc)) {
                 const Tile tc = get_tile(sc);
                 if (tc.skip) continue;
@@ -693,6 +670,7 @@ k_interval_pair(const __grid_constant__ CUtensorMap mapU, const __grid_constant_
                     }
                     __syncwarp();
                     accum = 1;
+                    issued++;
                     if (++s == NS) { s = 0; ph ^= 1; }
                 };
                 for_each_group(tc, [&](int, bool first, bool second) {
@@ -702,6 +680,14 @@ k_interval_pair(const __grid_constant__ CUtensorMap mapU, const __grid_constant_
                 if (elect_one()) mma_commit_pair(&s_tfull[acc]);          // accumulator complete, both CTAs
                 __syncwarp();
                 tile_seq++;
+            }
+            if (lane == 0) {
+                if (issued) atomicAdd(&stats->stages_executed, issued);
+                if (t0 == 0) {
+                    stats->stages_total = stages_total;
+                    stats->blocks_examined = blocks_examined;
+                    stats->blocks_empty = flagU ? (unsigned long long)__ldg(n_empty) : 0ull;
+                }
             }
         }
     } else {
@@ -770,7 +756,6 @@ k_interval_pair(const __grid_constant__ CUtensorMap mapU, const __grid_constant_
             __syncwarp();
             if (lane == 0) mbar_arrive_cluster(&s_tempty[acc], 0);   // one arrival per warp, in CTA 0
             tile_seq++;
-            if (CS_PAIR_DIAG & 4) continue;
             my_nrel += __popcll(rel[0]) + __popcll(rel[1]);
             // Tally over the 128 columns in registers; 32 columns at a time are skipped when no lane of
             // the warp has a related pair there.  SMALL is branch-free (a branch per related pair
@@ -901,27 +886,30 @@ size_t interval_pair_scratch_bytes(int64_t N)
 template <bool SMALL, int TN>
 static int launch_pair_t(const CUtensorMap &mapU, const CUtensorMap &mapL, const uint64_t *bits, const uint32_t *tab,
                          const uint8_t *flagU, const uint8_t *flagT, const unsigned int *n_empty, int nT, uint32_t tiles_per, int64_t clusters, int64_t B, int64_t N, int64_t stride, int64_t kmax, int hs,
-                         int64_t row_begin, int64_t row_end, int64_t *hist, int64_t *nrel, cudaStream_t st)
+                         int64_t row_begin, int64_t row_end, int64_t *hist, int64_t *nrel,
+                         IntervalStats *stats, unsigned long long stages_total, unsigned long long blocks_examined, cudaStream_t st)
 {
-    static bool attr_set = false;
-    if (!attr_set) {
+    static PerDeviceFlag attr_set;
+    const int dev = current_device();
+    if (!attr_set.get(dev)) {
         CS_CUDA(cudaFuncSetAttribute(k_interval_pair<SMALL, TN>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                      Shape<TN>::SMEM_FIXED + (SMALL ? 0 : HS_MAX * 4)));
-        attr_set = true;
+        attr_set.set(dev);
     }
     // whole causets per cluster only if the last round of causets leaves at most 5 % of the clusters idle
     const int64_t rounds = (B + clusters - 1) / clusters;
     const int causet_major = (B > 1 && rounds * clusters * 20 <= B * 21) ? 1 : 0;
     k_interval_pair<SMALL, TN><<<(unsigned)(2 * clusters), THREADS, Shape<TN>::SMEM_FIXED + hs * 4, st>>>(
         mapU, mapL, bits, tab, flagU, flagT, n_empty, nT, tiles_per, B, N, stride, kmax, hs, causet_major, row_begin, row_end,
-        reinterpret_cast<unsigned long long *>(hist), reinterpret_cast<unsigned long long *>(nrel));
+        reinterpret_cast<unsigned long long *>(hist), reinterpret_cast<unsigned long long *>(nrel),
+        stats, stages_total, blocks_examined);
     CS_LAUNCHED("k_interval_pair");
     return CS_OK;
 }
 
 int launch_interval_pair(const uint64_t *bits, const uint64_t *bitsT, int64_t B, int64_t N, int64_t kmax,
                          int64_t row_begin, int64_t row_end, int64_t *hist, int64_t *nrel,
-                         void *scratch, size_t scratch_bytes, cudaStream_t st)
+                         void *scratch, size_t scratch_bytes, IntervalStats *stats, cudaStream_t st)
 {
     if (N > ((int64_t)1 << 22)) return CS_ERR_ARG;   // counts must stay exact in fp32; tile ids are 16 bits
     constexpr int TN = PAIR_TN;
@@ -942,7 +930,9 @@ int launch_interval_pair(const uint64_t *bits, const uint64_t *bitsT, int64_t B,
     // empty-block flags: one causet, and large enough that the ~10 us of the flag pass cannot matter
     uint8_t *flagU = nullptr, *flagT = nullptr;
     unsigned int *n_empty = nullptr;
-    if (CS_PAIR_SKIP && B == 1 && nT >= SKIP_MIN_TILES) {
+    unsigned long long blocks_examined = 0;
+    if (B == 1 && nT >= SKIP_MIN_TILES) {
+        for (int m = 0; m < SKIPM && m < nT; m++) blocks_examined += (unsigned long long)(nT - m);
         flagU = static_cast<uint8_t *>(scratch) + align_up((size_t)tiles_per * sizeof(uint32_t), 256);
         flagT = flagU + align_up((size_t)nT * SKIPM, 256);
         n_empty = reinterpret_cast<unsigned int *>(flagT + align_up((size_t)nT * SKIPM, 256));
@@ -950,6 +940,11 @@ int launch_interval_pair(const uint64_t *bits, const uint64_t *bitsT, int64_t B,
         k_pair_block_flags<<<dim3(nT, SKIPM), 256, 0, st>>>(bits, N, stride, nT, flagU, flagT, n_empty);
         CS_LAUNCHED("k_pair_block_flags");
     }
+    // stages of the tiles whose rows intersect [row_begin, row_end), nothing skipped: tile (I, I+d) has d+1
+    unsigned long long stages_total = 0;
+    for (int64_t I = row_begin / TILE; I < (row_end + TILE - 1) / TILE && I < nT; I++)
+        stages_total += (unsigned long long)((nT - I) * (nT - I + 1) / 2);
+    stages_total *= (unsigned long long)B;
     const int64_t total = tiles_per * B;
     int64_t clusters = sm_count() / 2;
     if (clusters > total) clusters = total;
@@ -959,7 +954,7 @@ int launch_interval_pair(const uint64_t *bits, const uint64_t *bitsT, int64_t B,
     const int64_t hs_cap = B > 1 ? HS_BATCHED : HS_MAX;
     const int hs = small ? 0 : (int)(kmax + 1 < hs_cap ? kmax + 1 : hs_cap);
 #define CS_PAIR_LAUNCH(S, T) \
-    launch_pair_t<S, T>(mapU, mapL, bits, tab, flagU, flagT, n_empty, nT, (uint32_t)tiles_per, clusters, B, N, stride, kmax, hs, row_begin, row_end, hist, nrel, st)
+    launch_pair_t<S, T>(mapU, mapL, bits, tab, flagU, flagT, n_empty, nT, (uint32_t)tiles_per, clusters, B, N, stride, kmax, hs, row_begin, row_end, hist, nrel, stats, stages_total, blocks_examined, st)
     return small ? CS_PAIR_LAUNCH(true, PAIR_TN) : CS_PAIR_LAUNCH(false, PAIR_TN);
 #undef CS_PAIR_LAUNCH
 }

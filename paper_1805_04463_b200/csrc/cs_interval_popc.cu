@@ -237,13 +237,14 @@ int launch_interval_popc(const uint64_t *bits, const uint64_t *bitsT, int64_t B,
                          int64_t row_begin, int64_t row_end, int64_t *hist, int64_t *nrel,
                          void *scratch, cudaStream_t st)
 {
-    static bool attr_set = false;
-    if (!attr_set) {
+    static PerDeviceFlag attr_set;
+    const int dev = current_device();
+    if (!attr_set.get(dev)) {
         CS_CUDA(cudaFuncSetAttribute(k_interval_popc, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES));
-        attr_set = true;
+        attr_set.set(dev);
     }
     const int64_t stride = row_stride_words(N);
-    CS_CUDA(cudaMemsetAsync(scratch, 0, 256, st));
+    // scratch = the workspace's IntervalStats block, zeroed by the caller; sched[0] is the tile counter
     const int64_t nT = (N + TI - 1) / TI;
     const int64_t total = nT * (nT + 1) / 2 * B;
     int64_t grid = (int64_t)sm_count() * 2;

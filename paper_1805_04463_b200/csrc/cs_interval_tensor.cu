@@ -461,10 +461,11 @@ int launch_interval_tensor(const uint64_t *bits, const uint64_t *bitsT, int64_t 
                            void *, size_t, cudaStream_t st)
 {
     if (N > ((int64_t)1 << 17)) return CS_ERR_ARG;   // count * 2^14 must stay below 2^31
-    static bool attr_set = false;
-    if (!attr_set) {
+    static PerDeviceFlag attr_set;
+    const int dev = current_device();
+    if (!attr_set.get(dev)) {
         CS_CUDA(cudaFuncSetAttribute(k_interval_tensor, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES));
-        attr_set = true;
+        attr_set.set(dev);
     }
     const int64_t stride = row_stride_words(N);
     CUtensorMap mapU, mapL;

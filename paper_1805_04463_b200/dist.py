@@ -59,6 +59,34 @@ def reduce_sum(x: float) -> float:
     return float(t.item())
 
 
+def all_reduce_sum_(t: torch.Tensor) -> torch.Tensor:
+    """In-place sum over ranks of an integer tensor (the partial interval histograms of `shard_rows`): NCCL when
+    the tensor is on a GPU, gloo on the CPU; a no-op with one process."""
+    if dist.is_initialized() and dist.get_world_size() > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.SUM)
+    return t
+
+
+def shard_rows(N: int, world: int, tile: int = 256):
+    """Contiguous row ranges [(begin, end)] * world of the outer element i of a2, cut on tile borders so that every
+    rank gets about the same tensor work (NEXT-4; the paper splits row groups over MPI ranks).
+    Row tile I of nT pairs with the tiles J >= I, tile (I, J) costing J - I + 1 K stages, so tile I costs
+    (nT - I)(nT - I + 1) / 2: early rows are far more expensive than late ones.  Greedy prefix cut at k/world of
+    the total; ranks beyond the number of tiles get empty ranges.  Pure host arithmetic."""
+    nT = (N + tile - 1) // tile
+    cost = [(nT - I) * (nT - I + 1) // 2 for I in range(nT)]
+    total = sum(cost)
+    cuts, acc, I = [0], 0, 0
+    for r in range(1, world):
+        target = total * r / world
+        while I < nT and acc + cost[I] / 2 <= target:
+            acc += cost[I]
+            I += 1
+        cuts.append(I)
+    cuts.append(nT)
+    return [(min(N, cuts[r] * tile), min(N, cuts[r + 1] * tile)) for r in range(world)]
+
+
 def replica_seed(base_seed: int, rank: int) -> int:
     """Replica `rank` sprinkles with its own seed (rank 0 keeps the config's seed)."""
     return base_seed + 1000003 * rank

@@ -33,15 +33,24 @@ def api():
     return _api
 
 
+ALL_ROUTES = ("ROUTE_POPC", "ROUTE_TENSOR", "ROUTE_TENSOR_FP4", "ROUTE_TENSOR_PAIR")
+
+
 def routes(api):
-    r = [api.ROUTE_POPC]
-    for cand in (api.ROUTE_TENSOR, api.ROUTE_TENSOR_FP4, api.ROUTE_TENSOR_PAIR):
+    """Every concrete a2 route.  On a compute-capability 10.x device all four must launch: a tensor route that
+    stops working fails the test that asked for it instead of quietly leaving the list."""
+    major, _ = torch.cuda.get_device_capability()
+    if major != 10:
+        pytest.fail("the tensor routes need an sm_100 device (found compute capability %d.x)" % major)
+    r = []
+    for name in ALL_ROUTES:
+        cand = getattr(api, name)
+        x = torch.zeros((128, 2), dtype=torch.int64, device="cuda")
         try:
-            x = torch.zeros((128, 2), dtype=torch.int64, device="cuda")
             api.interval_hist(x, x, 128, route=cand)
-            r.append(cand)
-        except RuntimeError:
-            pass
+        except RuntimeError as e:
+            pytest.fail("a2 route %s does not launch on this device: %s" % (name, e))
+        r.append(cand)
     return r
 
 
@@ -410,9 +419,11 @@ def test_interval_hist_random_block_patterns(api, oracle):
 
 
 # ----------------------------------------------------------------------------- full sizes
-def _full_size_check(api, oracle, cfg, full_hist):
-    """Bits compared in full; histogram compared in full (tier-1) or on sampled row ranges plus
-    the two moment identities that hold at any size."""
+def _full_size_check(api, oracle, cfg):
+    """BASELINE.json's full size, in the launch configuration bench.py times (default route, whole row range):
+    bits, the WHOLE histogram and the action element by element against the oracle (tier-1 = Alg. 20,
+    PAPER.md:1851-1893; bracket and S of Eq. 4.10-4.12, from the ORACLE's histogram),
+    plus the two moment identities and three sampled row ranges."""
     N = cfg.N
     coords = inp.make_config_coords(cfg)
     o_bits = oracle.causal_matrix_bits(coords, cfg.geometry)
@@ -426,31 +437,55 @@ def _full_size_check(api, oracle, cfg, full_hist):
     assert int(nrel[0]) == R and int(h.sum()) == R
     outdeg, indeg = oracle.degrees(o_bits, N)
     assert int((np.arange(N - 1, dtype=np.int64) * h).sum()) == int((outdeg * indeg).sum())
-    if full_hist:
-        o_hist, _, _ = oracle.interval_hist_alg20(o_bits, N)
-        assert np.array_equal(h, o_hist)
-    else:
-        rng = np.random.default_rng(cfg.index)
-        for r0 in sorted(rng.integers(0, N - 64, 3).tolist()):
-            part = api.interval_hist(bits, bitsT, N, row_begin=r0, row_end=r0 + 40).cpu().numpy()
-            assert np.array_equal(part, oracle.interval_hist_alg20(o_bits, N, r0, r0 + 40)[0])
+    o_hist, _, _ = oracle.interval_hist_alg20(o_bits, N)
+    assert np.array_equal(h, o_hist)
+    rng = np.random.default_rng(cfg.index)
+    for r0 in sorted(rng.integers(0, N - 64, 3).tolist()):
+        part = api.interval_hist(bits, bitsT, N, row_begin=r0, row_end=r0 + 40).cpu().numpy()
+        assert np.array_equal(part, oracle.interval_hist_alg20(o_bits, N, r0, r0 + 40)[0])
     S, I = api.bd_action(hist, N, cfg.dim, return_bracket=True)
-    oS, oI = oracle.bd_action(h, N, cfg.dim)
+    oS, oI = oracle.bd_action(o_hist, N, cfg.dim)          # from the oracle's own histogram
     assert int(I[0]) == oI and float(S[0]) == oS
+    # the host-buffer entry point bench.py's e2e leg times
+    h_host, s_host = api.action_host(torch.from_numpy(coords).pin_memory(), cfg.geometry)
+    assert np.array_equal(h_host.numpy(), o_hist) and float(s_host[0]) == oS
+    return o_hist, oS
 
 
 def test_config2_full(api, oracle):
-    _full_size_check(api, oracle, inp.CONFIGS[2], full_hist=True)
+    _full_size_check(api, oracle, inp.CONFIGS[2])
 
 
 @pytest.mark.slow
 def test_config3_full_size(api, oracle):
-    _full_size_check(api, oracle, inp.CONFIGS[3], full_hist=False)
+    """The headline workload (N = 65536, 3+1): every bin of N_k and the action printed by bench.py."""
+    _full_size_check(api, oracle, inp.CONFIGS[3])
 
 
 @pytest.mark.slow
 def test_config4_full_size(api, oracle):
-    _full_size_check(api, oracle, inp.CONFIGS[4], full_hist=False)
+    _full_size_check(api, oracle, inp.CONFIGS[4])
+
+
+def test_headline_size_routes_agree_on_device(api):
+    """N = 65536 (empty-block skipping, 16896 shared bins + global-atomic tail all active) without the oracle, so it
+    runs in the default GPU suite: the complete pair-route histogram against the POPC route, kmax = 3, a row range."""
+    cfg = inp.CONFIGS[3]
+    bits, bitsT = gpu_bits(api, inp.make_config_coords(cfg), cfg.geometry)
+    N = cfg.N
+    ws = torch.empty(api.interval_hist_workspace(N, -1, True, api.ROUTE_TENSOR_PAIR), dtype=torch.uint8, device="cuda")
+    pair = api.interval_hist(bits, bitsT, N, route=api.ROUTE_TENSOR_PAIR, workspace=ws)
+    executed, total, empty, examined = api.interval_hist_stats(ws)
+    popc = api.interval_hist(bits, bitsT, N, route=api.ROUTE_POPC)
+    assert torch.equal(pair, popc)
+    assert torch.equal(api.interval_hist(bits, bitsT, N, kmax=3), popc[:4])
+    a = api.interval_hist(bits, bitsT, N, route=api.ROUTE_TENSOR_PAIR, row_begin=30000, row_end=31000)
+    b = api.interval_hist(bits, bitsT, N, route=api.ROUTE_POPC, row_begin=30000, row_end=31000)
+    assert torch.equal(a, b)
+    # the executed-stage counter: dense-triangular total in closed form, fewer executed (empty blocks), none lost
+    nT = N // 256
+    assert total == nT * (nT + 1) * (nT + 2) // 6
+    assert 0 < executed < total and 0 < empty <= examined
 
 
 @pytest.mark.slow
@@ -687,3 +722,53 @@ def test_longest_chain_config2_is_lis(api):
     assert int(longest[0]) == len(piles)
     hh = h.cpu().numpy()
     assert hh.min() == 1 and np.array_equal(np.unique(hh), np.arange(1, len(piles) + 1))
+
+
+# ----------------------------------------------------------------------------- NEXT-4: row sharding on one GPU
+def test_row_sharding_matches_single_launch(api):
+    """bench.py --shard on one device: the row ranges dist.shard_rows hands to 2, 3 and 8 ranks, run one after the
+    other through cs_interval_hist_ex and summed, give the single-launch histogram of config 2 bit for bit."""
+    from paper_1805_04463_b200 import dist as csd
+    cfg = inp.CONFIGS[2]
+    bits, bitsT = gpu_bits(api, inp.make_config_coords(cfg), cfg.geometry)
+    full = api.interval_hist(bits, bitsT, cfg.N)
+    for world in (2, 3, 8):
+        total = torch.zeros_like(full)
+        for r0, r1 in csd.shard_rows(cfg.N, world):
+            total += api.interval_hist(bits, bitsT, cfg.N, row_begin=r0, row_end=r1)
+        assert torch.equal(total, full), world
+
+
+# ----------------------------------------------------------------------------- sanitizer target
+def test_small_everything(api, oracle):
+    """Every kernel of the library once on a small input (all four a2 routes, the batched ensemble, the cooperative
+    poset kernels, the smeared action, the host entry points), checked against the oracle.  This is the command
+    compute-sanitizer runs (profiles/r2_sanitizer.md):
+        compute-sanitizer --tool memcheck python -m pytest tests/test_gpu_parity.py -q -k small_everything"""
+    cfg = inp.CONFIGS[3]
+    N = 700
+    coords = inp.make_config_coords(cfg, N=N)
+    o_bits, o_hist, o_S, o_I = oracle.action_pipeline(coords, cfg.geometry, tier=1)
+    bits, bitsT = gpu_bits(api, coords, cfg.geometry)
+    assert np.array_equal(to_u64(bits), o_bits)
+    for r in routes(api):
+        assert np.array_equal(api.interval_hist(bits, bitsT, N, route=r).cpu().numpy(), o_hist), r
+        assert np.array_equal(api.interval_hist(bits, None, N, kmax=3, route=r).cpu().numpy(), o_hist[:4]), r
+    S, I = api.bd_action(api.interval_hist(bits, bitsT, N), N, cfg.dim, return_bracket=True)
+    assert int(I[0]) == o_I and float(S[0]) == o_S
+    ens = inp.make_ensemble_coords(inp.CONFIGS[5], B=3, N=600)
+    actions, hist4 = api.bd_action_batched(torch.from_numpy(ens).cuda(), cfg.geometry, return_hist4=True)
+    a_host, _ = api.bd_action_batched_host(torch.from_numpy(ens).pin_memory(), cfg.geometry)
+    for b in range(3):
+        _, oh, oS, _ = oracle.action_pipeline(ens[b], cfg.geometry, tier=1)
+        assert np.array_equal(hist4[b].cpu().numpy(), oh[:4]) and float(actions[b]) == oS == float(a_host[b])
+    C = oracle.causal_matrix_bytes(coords, cfg.geometry)
+    h, longest = api.chain_heights(bits, bitsT, N)
+    assert np.array_equal(h.cpu().numpy(), oracle.chain_heights(C)[0])
+    m, size = api.greedy_antichain(bits, bitsT, N, 3)
+    assert np.array_equal(_unpack_member(m, N), oracle.greedy_antichain(C, 3))
+    d_hist = torch.from_numpy(o_hist).cuda()
+    assert abs(float(api.smeared_action(d_hist, N, 4, 0.25)[0]) - oracle.smeared_action(o_hist, N, 4, 0.25)) \
+        <= _smear_tolerance(o_hist, 4, 0.25, oracle.smeared_action(o_hist, N, 4, 0.25))
+    h_host, s_host = api.action_host(torch.from_numpy(coords).pin_memory(), cfg.geometry)
+    assert np.array_equal(h_host.numpy(), o_hist) and float(s_host[0]) == o_S
