@@ -10,6 +10,7 @@ from .oracle import (  # noqa: F401
     GEOM_MINK_CONE,
     GEOM_DS2_SLAB,
     GEOM_FLRW_POLAR,
+    GEOM_DS4_SPHERICAL,
     build,
     row_stride_words,
     relation,

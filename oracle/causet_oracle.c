@@ -22,7 +22,9 @@
  *   4. (NEXT-1) smeared action, Eq. 4.13-4.18.
  *   5. (NEXT-3) longest chains (Algorithm 11) and the greedy maximal antichain
  *      (Algorithm 13).
- *   6. (NEXT-4) the FLRW relation of Eq. 7.7 as a fourth predicate of stage 1.
+ *   6. (NEXT-4) the FLRW relation of Eq. 7.7 as a fourth predicate of stage 1; the flat cone
+ *      in 4+1 dimensions (the 4+1 diamond of App. A.1.2); the 3+1 de Sitter slab with
+ *      spherical foliation (App. A.1.3) as a fifth predicate.
  *
  * Floating point: every predicate is evaluated in fp64 exactly in the order
  * written below; compile with -ffp-contract=off (no FMA), no -ffast-math.
@@ -42,7 +44,8 @@
 #include <omp.h>
 #endif
 
-enum { ORC_GEOM_MINK2_LIGHTCONE = 0, ORC_GEOM_MINK_CONE = 1, ORC_GEOM_DS2_SLAB = 2, ORC_GEOM_FLRW_POLAR = 3 };
+enum { ORC_GEOM_MINK2_LIGHTCONE = 0, ORC_GEOM_MINK_CONE = 1, ORC_GEOM_DS2_SLAB = 2, ORC_GEOM_FLRW_POLAR = 3,
+       ORC_GEOM_DS4_SPHERICAL = 4 };
 
 /* 2*pi as the fp64 nearest to the real number (bit pattern 0x401921FB54442D18). */
 static const double ORC_TWO_PI = 6.283185307179586476925286766559;
@@ -64,6 +67,17 @@ static const double ORC_TWO_PI = 6.283185307179586476925286766559;
  *                   (taken once per point, not once per pair), and cos(ph_i - ph_j) is expanded as
  *                   cos ph_i cos ph_j + sin ph_i sin ph_j, so the predicate is additions and multiplications
  *                   only (reading A17).  j is in the future of i only if eta_j > eta_i.
+ *  DS4_SPHERICAL:   (NEXT-4) 3+1 de Sitter, spherical foliation: ds^2 = lambda^2 sec^2(eta) (-d eta^2 + d Omega_3^2)
+ *                   (PAPER.md:3829-3831), conformal to R x S^3.  In conformal time "timelike ... intervals
+ *                   correspond to d eta^2 > d Sigma^2"; on the unit 3-sphere d Sigma is the
+ *                   great-circle angle omega between the two points, cos omega = X_i . X_j with X the unit
+ *                   4-vector (cos psi, sin psi cos th, sin psi sin th cos ph, sin psi sin th sin ph).  For
+ *                   0 < d eta <= pi (a slab eta in [0, eta0], eta0 < pi/2) and omega in [0, pi] the cosine is
+ *                   decreasing, so  d eta > omega  <=>  cos(d eta) < cos omega.  A point is
+ *                   (eta, cos eta, sin eta, X0, X1, X2, X3) -- as for FLRW_POLAR the trigonometric values are
+ *                   inputs -- and cos(d eta) = cos eta_i cos eta_j + sin eta_i sin eta_j, so the predicate is
+ *                   additions and multiplications only, strict, eta_j > eta_i (reading A18).
+ *  MINK_CONE dim 5: the same squared form with a fourth spatial coordinate (4+1 diamond).
  */
 int orc_relation(const double *xi, const double *xj, int dim, int geom)
 {
@@ -81,6 +95,10 @@ int orc_relation(const double *xi, const double *xj, int dim, int geom)
             double dz = xj[3] - xi[3];
             s = s + dz * dz;
         }
+        if (dim >= 5) {
+            double dw = xj[4] - xi[4];
+            s = s + dw * dw;
+        }
         return (dt >= 0.0) && (dt * dt >= s);
     } else if (geom == ORC_GEOM_DS2_SLAB) {
         double deta = xj[0] - xi[0];
@@ -94,6 +112,11 @@ int orc_relation(const double *xi, const double *xj, int dim, int geom)
         double ang = (xi[2] * xj[2]) + ((xi[3] * xj[3]) * cphi);
         double d2 = ((xi[1] * xi[1]) + (xj[1] * xj[1])) - ((2.0 * (xi[1] * xj[1])) * ang);
         return (deta > 0.0) && (d2 < deta * deta);
+    } else if (geom == ORC_GEOM_DS4_SPHERICAL) {
+        double deta = xj[0] - xi[0];
+        double cd = (xi[1] * xj[1]) + (xi[2] * xj[2]);                                          /* cos(d eta) */
+        double co = ((xi[3] * xj[3]) + (xi[4] * xj[4])) + ((xi[5] * xj[5]) + (xi[6] * xj[6]));  /* cos(omega) */
+        return (deta > 0.0) && (cd < co);
     }
     return 0;
 }
@@ -101,9 +124,10 @@ int orc_relation(const double *xi, const double *xj, int dim, int geom)
 static int orc_geom_ok(int dim, int geom)
 {
     if (geom == ORC_GEOM_MINK2_LIGHTCONE) return dim == 2;
-    if (geom == ORC_GEOM_MINK_CONE) return dim >= 2 && dim <= 4;
+    if (geom == ORC_GEOM_MINK_CONE) return dim >= 2 && dim <= 5;
     if (geom == ORC_GEOM_DS2_SLAB) return dim == 2;
     if (geom == ORC_GEOM_FLRW_POLAR) return dim == 6;
+    if (geom == ORC_GEOM_DS4_SPHERICAL) return dim == 7;
     return 0;
 }
 

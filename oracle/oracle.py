@@ -18,6 +18,7 @@ GEOM_MINK2_LIGHTCONE = 0
 GEOM_MINK_CONE = 1
 GEOM_DS2_SLAB = 2
 GEOM_FLRW_POLAR = 3
+GEOM_DS4_SPHERICAL = 4
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "causet_oracle.c")
@@ -249,5 +250,10 @@ def action_pipeline(coords, geom: int, tier: int = 1):
     else:
         bits = causal_matrix_bits(c, geom)
         hist, _, _ = interval_hist_alg20(bits, N)
-    S, br = bd_action(hist, N, 4 if geom == GEOM_FLRW_POLAR else dim)    # six coordinates, 3+1 dimensions
+    # FLRW_POLAR (six numbers per point) and DS4_SPHERICAL (seven) describe 3+1 dimensional events; the paper
+    # prints no action for 4+1 dimensions (Eq. 4.10-4.12 stop at d = 4): the bracket and S are then None
+    sdim = 4 if geom in (GEOM_FLRW_POLAR, GEOM_DS4_SPHERICAL) else dim
+    if sdim > 4:
+        return bits, hist, None, None
+    S, br = bd_action(hist, N, sdim)
     return bits, hist, S, br

@@ -28,7 +28,8 @@ ROUTE_TENSOR_FP4 = 3
 ROUTE_TENSOR_PAIR = 4
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "libcausalset.so")
+# CAUSALSET_LIB selects another build of the same library (A/B timing of kernel variants); default: in-tree
+LIB_PATH = os.environ.get("CAUSALSET_LIB") or os.path.join(_HERE, "libcausalset.so")
 HEADER_PATH = os.path.join(os.path.dirname(_HERE), "include", "causalset.h")
 
 _i64 = ctypes.c_int64

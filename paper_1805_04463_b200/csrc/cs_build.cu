@@ -146,39 +146,112 @@ __device__ __forceinline__ uint32_t transpose32(uint32_t x, int lane) { return T
 
 constexpr int NJ = 2;            // future points per lane: a CTA covers 256 rows x 512 columns
 
+// Packed single precision (Blackwell FFMA2 / FADD2: two fp32 lanes per instruction, each rounded like the scalar
+// operation, so the error bound above is unchanged).  A 64-bit register holds the values of two consecutive rows.
+typedef unsigned long long f32x2;
+__device__ __forceinline__ f32x2 bcast2(float v)
+{
+    f32x2 d;
+    asm("mov.b64 %0, {%1, %1};" : "=l"(d) : "f"(v));     // ptxas folds this into the .F32 broadcast operand form
+    return d;
+}
+__device__ __forceinline__ f32x2 ffma2(f32x2 a, f32x2 b, f32x2 c)
+{
+    f32x2 d;
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c));
+    return d;
+}
+__device__ __forceinline__ f32x2 fadd2(f32x2 a, f32x2 b)
+{
+    f32x2 d;
+    asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+    return d;
+}
+// min(u, |a|, |b|), NaN if any operand is NaN (one FMNMX3.NAN)
+__device__ __forceinline__ float min3_abs_nan(float u, uint32_t a, uint32_t b)
+{
+    float d;
+    asm("{\n"
+        ".reg .f32 x, y;\n"
+        "abs.f32 x, %2;\n"
+        "abs.f32 y, %3;\n"
+        "min.NaN.f32 %0, %1, x, y;\n"
+        "}\n" : "=f"(d) : "f"(u), "f"(__uint_as_float(a)), "f"(__uint_as_float(b)));
+    return d;
+}
+
 // One 32 x 32 block per future point k < NK of this lane: bit ii of lw[k] = (row i0 + ii  -<  point k),
 // decided by the fp32 prefilter; unc[k] is set if any of the lane's 32 decisions is inside the error
-// band.  The row's (t, x, y, z) and h are loaded once (LDS.128 broadcasts) for all NK points.
+// band (or NaN).
+//
+// Flat cone: the past points sit in shared memory as five arrays (-t, x, y, z, h), so one LDS.128 brings a
+// coordinate of four consecutive rows and each 64-bit half feeds a packed operation on two rows; the future
+// point's coordinates are per-lane scalars that FFMA2 broadcasts.  Per four pairs: 8 FFMA2 + 2 FADD2 for the
+// values, then one SHF per pair shifts the value's sign bit into the lane's word and one FMNMX3 per two pairs
+// keeps the smallest |a| -- if that exceeds the margin m, no decision of the block is inside the band, and
+// "a > m" is simply "sign bit clear".  4 instructions per pair instead of 8 (4 FFMA, FADD, 2 FSETP, predicated add).
 template <int GEOM, int DIM, int NK>
-__device__ __forceinline__ void fast_block(const float4 *__restrict__ fi, const float *__restrict__ hi,
+__device__ __forceinline__ void fast_block(const float *__restrict__ sf, int i0,
                                            const float (*fj)[4], const float *hj, const float *m,
                                            uint32_t *lw, bool *unc)
 {
+    if (GEOM == CS_GEOM_DS2_SLAB) {
+        const float2 *fi = reinterpret_cast<const float2 *>(sf) + i0;     // (eta, theta) per past point
 #pragma unroll
-    for (int i4 = 0; i4 < 32; i4 += 4) {
-        const float4 h4 = *reinterpret_cast<const float4 *>(hi + i4);
-        const float hq[4] = {h4.x, h4.y, h4.z, h4.w};
-#pragma unroll
-        for (int q = 0; q < 4; q++) {
-            const float4 p = fi[i4 + q];
+        for (int ii = 0; ii < 32; ii++) {
+            const float2 p = fi[ii];
 #pragma unroll
             for (int k = 0; k < NK; k++) {
-                float a;
-                if (GEOM == CS_GEOM_DS2_SLAB) {
-                    const float de = fj[k][0] - p.x;
-                    const float ab = fabsf(fj[k][1] - p.y);
-                    a = de - fminf(ab, 6.2831853071795865f - ab);
-                } else {
-                    a = fmaf(-p.x, fj[k][0], hq[q]);
-                    if (DIM > 1) a = fmaf(p.y, fj[k][1], a);
-                    if (DIM > 2) a = fmaf(p.z, fj[k][2], a);
-                    if (DIM > 3) a = fmaf(p.w, fj[k][3], a);
-                    a = a + hj[k];
-                }
-                if (a > m[k]) lw[k] |= 1u << (i4 + q);
+                const float de = fj[k][0] - p.x;
+                const float ab = fabsf(fj[k][1] - p.y);
+                const float a = de - fminf(ab, 6.2831853071795865f - ab);
+                if (a > m[k]) lw[k] |= 1u << ii;
                 unc[k] = unc[k] || !(fabsf(a) > m[k]);
             }
         }
+        return;
+    }
+    uint32_t sg[NK];
+    float mn[NK];
+    f32x2 ft[NK], fx[NK], fy[NK], fz[NK], fh[NK];
+#pragma unroll
+    for (int k = 0; k < NK; k++) {
+        sg[k] = 0;
+        mn[k] = __int_as_float(0x7f800000);
+        ft[k] = bcast2(fj[k][0]);
+        fx[k] = bcast2(fj[k][1]);
+        fy[k] = bcast2(fj[k][2]);
+        fz[k] = bcast2(fj[k][3]);
+        fh[k] = bcast2(hj[k]);
+    }
+#pragma unroll
+    for (int i4 = 0; i4 < 32; i4 += 4) {
+        const ulonglong2 T = *reinterpret_cast<const ulonglong2 *>(sf + (0) * BT + i0 + i4);     // -t of rows (0,1), (2,3)
+        const ulonglong2 X = *reinterpret_cast<const ulonglong2 *>(sf + (1) * BT + i0 + i4);
+        const ulonglong2 Y = *reinterpret_cast<const ulonglong2 *>(sf + (DIM > 2 ? 2 : 0) * BT + i0 + i4);
+        const ulonglong2 Z = *reinterpret_cast<const ulonglong2 *>(sf + (DIM > 3 ? 3 : 0) * BT + i0 + i4);
+        const ulonglong2 H = *reinterpret_cast<const ulonglong2 *>(sf + (4) * BT + i0 + i4);
+#pragma unroll
+        for (int k = 0; k < NK; k++) {
+            f32x2 a01 = ffma2(T.x, ft[k], H.x), a23 = ffma2(T.y, ft[k], H.y);
+            a01 = ffma2(X.x, fx[k], a01); a23 = ffma2(X.y, fx[k], a23);
+            if (DIM > 2) { a01 = ffma2(Y.x, fy[k], a01); a23 = ffma2(Y.y, fy[k], a23); }
+            if (DIM > 3) { a01 = ffma2(Z.x, fz[k], a01); a23 = ffma2(Z.y, fz[k], a23); }
+            a01 = fadd2(a01, fh[k]);
+            a23 = fadd2(a23, fh[k]);
+            const uint32_t a0 = (uint32_t)a01, a1 = (uint32_t)(a01 >> 32), a2 = (uint32_t)a23, a3 = (uint32_t)(a23 >> 32);
+            sg[k] = __funnelshift_l(a0, sg[k], 1);      // row i0 + ii ends up at bit 31 - ii
+            sg[k] = __funnelshift_l(a1, sg[k], 1);
+            sg[k] = __funnelshift_l(a2, sg[k], 1);
+            sg[k] = __funnelshift_l(a3, sg[k], 1);
+            mn[k] = min3_abs_nan(mn[k], a0, a1);
+            mn[k] = min3_abs_nan(mn[k], a2, a3);
+        }
+    }
+#pragma unroll
+    for (int k = 0; k < NK; k++) {
+        lw[k] = ~__brev(sg[k]);              // related = sign bit clear (valid when no decision is inside the band)
+        unc[k] = !(mn[k] > m[k]);            // NaN compares false: uncertain
     }
 }
 
@@ -212,13 +285,13 @@ k_causal_matrix(const double *__restrict__ coords, int64_t N, int64_t stride,
     constexpr bool FAST = FastCone<GEOM, DIM>::ok;
     constexpr int NW = BUILD_THREADS / 32;
     __shared__ double s_xi[DIM][BT];
-    __shared__ __align__(16) float4 s_fi[FAST ? BT : 1];   // (t, x, y, z) of the past points in fp32
-    __shared__ __align__(16) float s_hi[FAST ? BT : 4];    // h of the past points in fp32
+    // fp32 copies of the past points: flat cone -t, x, y, z, h as five arrays; dS slab (eta, theta) pairs in the first two
+    __shared__ __align__(16) float s_f[FAST ? 5 : 1][FAST ? BT : 4];
     __shared__ __align__(16) uint32_t s_U[BT][NJ * 8 + 1]; // row i_local, 32-bit word = 32 columns j
     __shared__ uint32_t s_L[NJ * BT][9];                   // row j_local, 32-bit word = 32 rows i
     uint32_t (*s_red)[NW] = reinterpret_cast<uint32_t (*)[NW]>(&s_U[0][0]);   // [2 + 2 NJ][NW], dead before s_U is written
     // static shared memory stops at 48 KB; the flat cone in 3+1 dimensions sits exactly on it
-    static_assert(sizeof(s_xi) + sizeof(s_fi) + sizeof(s_hi) + sizeof(s_U) + sizeof(s_L) <= 48 * 1024,
+    static_assert(sizeof(s_xi) + sizeof(s_f) + sizeof(s_U) + sizeof(s_L) <= 48 * 1024,
                   "k_causal_matrix: static shared memory");
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -272,8 +345,14 @@ k_causal_matrix(const double *__restrict__ coords, int64_t N, int64_t stride,
             ci = fmaxf(ci, fabsf(fi[d]));
             if (d > 0) si += xi0[d] * xi0[d];
         }
-        s_fi[tid] = make_float4(fi[0], fi[1], fi[2], fi[3]);
-        s_hi[tid] = (float)(0.5 * (xi0[0] * xi0[0] - si));
+        if (GEOM == CS_GEOM_DS2_SLAB) {
+            reinterpret_cast<float2 *>(&s_f[0][0])[tid] = make_float2(fi[0], fi[1]);
+        } else {
+            s_f[0][tid] = -fi[0];
+#pragma unroll
+            for (int d = 1; d < DIM; d++) s_f[d][tid] = fi[d];
+            s_f[4][tid] = (float)(0.5 * (xi0[0] * xi0[0] - si));
+        }
         const uint32_t wci = __reduce_max_sync(0xffffffffu, __float_as_uint(ci));   // ci >= 0: bit order = value order
         const uint32_t wti = __reduce_max_sync(0xffffffffu, float_key(__double2float_ru(xi0[0])));
         if (lane == 0) { s_red[0][warp] = wci; s_red[1][warp] = wti; }
@@ -335,9 +414,9 @@ k_causal_matrix(const double *__restrict__ coords, int64_t N, int64_t stride,
         if (FAST) {
             bool unc[NJ] = {false, false};
             const bool f0 = need[0] && fast[0], f1 = need[1] && fast[1];
-            if (f0 && f1) fast_block<GEOM, DIM, 2>(s_fi + sb * 32, s_hi + sb * 32, fj, hj, m, lw, unc);
-            else if (f0) fast_block<GEOM, DIM, 1>(s_fi + sb * 32, s_hi + sb * 32, fj, hj, m, lw, unc);
-            else if (f1) fast_block<GEOM, DIM, 1>(s_fi + sb * 32, s_hi + sb * 32, fj + 1, hj + 1, m + 1, lw + 1, unc + 1);
+            if (f0 && f1) fast_block<GEOM, DIM, 2>(&s_f[0][0], sb * 32, fj, hj, m, lw, unc);
+            else if (f0) fast_block<GEOM, DIM, 1>(&s_f[0][0], sb * 32, fj, hj, m, lw, unc);
+            else if (f1) fast_block<GEOM, DIM, 1>(&s_f[0][0], sb * 32, fj + 1, hj + 1, m + 1, lw + 1, unc + 1);
 #pragma unroll
             for (int k = 0; k < NJ; k++) {
                 if (__any_sync(0xffffffffu, unc[k])) { slow[k] = true; lw[k] = 0; }

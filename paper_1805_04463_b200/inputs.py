@@ -29,6 +29,7 @@ GEOM_MINK2_LIGHTCONE = 0
 GEOM_MINK_CONE = 1
 GEOM_DS2_SLAB = 2
 GEOM_FLRW_POLAR = 3
+GEOM_DS4_SPHERICAL = 4
 
 _GAMMA = np.uint64(0x9E3779B97F4A7C15)
 _M1 = np.uint64(0xBF58476D1CE4E5B9)
@@ -111,6 +112,91 @@ def sprinkle_flrw_polar(N: int, seed: int, eta0: float = 1.0, r0: float = 0.7) -
     return _sort_rows(c, eta, rad)
 
 
+# ---- the other regions of the paper's Appendix A.1, each with the paper's own recipe ---------
+def _invert_monotone(f, u: np.ndarray, lo: float, hi: float, iters: int = 70) -> np.ndarray:
+    """x in [lo, hi] with f(x) = u for an increasing f, by bisection (the paper: "must be inverted numerically");
+    a fixed iteration count keeps the result a deterministic function of u."""
+    a = np.full(u.shape, lo, dtype=np.float64)
+    b = np.full(u.shape, hi, dtype=np.float64)
+    for _ in range(iters):
+        mid = 0.5 * (a + b)
+        below = f(mid) < u
+        a = np.where(below, mid, a)
+        b = np.where(below, b, mid)
+    return 0.5 * (a + b)
+
+
+def sprinkle_mink2_square(N: int, seed: int, t0: float = 1.0, x0: float = 1.0) -> np.ndarray:
+    """1+1 square: t* = (2u-1) t0, x* = (2u-1) x0; [N][2] = (t, x) for GEOM_MINK_CONE."""
+    r = uniform01(seed, 0, 2 * N).reshape(N, 2)
+    c = np.stack([(2.0 * r[:, 0] - 1.0) * t0, (2.0 * r[:, 1] - 1.0) * x0], axis=1)
+    return _sort_rows(c, c[:, 0], c[:, 1])
+
+
+def sprinkle_mink2_cylinder(N: int, seed: int, t0: float = 1.0) -> np.ndarray:
+    """1+1 cylinder, ds^2 = -dt^2 + d theta^2: t* = (2u-1) t0, theta* = 2 pi u; [N][2] = (t, theta).
+    Its relation is the periodic one of GEOM_DS2_SLAB (the de Sitter slab is conformal to this cylinder)."""
+    r = uniform01(seed, 0, 2 * N).reshape(N, 2)
+    c = np.stack([(2.0 * r[:, 0] - 1.0) * t0, (2.0 * np.pi) * r[:, 1]], axis=1)
+    return _sort_rows(c, c[:, 0], c[:, 1])
+
+
+def sprinkle_mink3_diamond_uv(N: int, seed: int, u0: float = 1.0) -> np.ndarray:
+    """2+1 diamond by the paper's inverse CDFs: u* = u^(1/3) u0, v* = u* (1 - sqrt(1 - u)),
+    theta* = 2 pi u, with t = (u+v)/sqrt 2, r = (u-v)/sqrt 2; [N][3] = (t, x, y) for GEOM_MINK_CONE."""
+    r = uniform01(seed, 0, 3 * N).reshape(N, 3)
+    u = np.cbrt(r[:, 0]) * u0
+    v = u * (1.0 - np.sqrt(1.0 - r[:, 1]))
+    th = (2.0 * np.pi) * r[:, 2]
+    t = (u + v) / np.sqrt(2.0)
+    rad = (u - v) / np.sqrt(2.0)
+    c = np.stack([t, rad * np.cos(th), rad * np.sin(th)], axis=1)
+    return _sort_rows(c, c[:, 0], c[:, 1])
+
+
+def sprinkle_mink5_diamond(N: int, seed: int) -> np.ndarray:
+    """4+1 flat diamond |t| + |x| <= 1 (the region of PAPER.md:3761-3777 up to shift and scale) by rejection from the
+    cube [-1,1)^5, as config 3 does in 3+1 (reading A11); [N][5] = (t, x, y, z, w) for GEOM_MINK_CONE."""
+    return _sprinkle_mink_low(N, 5, seed)
+
+
+def sprinkle_ds4_spherical(N: int, seed: int, eta0: float = 1.0) -> np.ndarray:
+    """3+1 de Sitter slab, spherical foliation: eta in [0, eta0] with density ~ sec^4 eta, psi with
+    density ~ sin^2 psi (u = (2 psi - sin 2 psi) / 2 pi "must be inverted numerically"), theta* = arccos(1 - 2u),
+    phi* = 2 pi u; draws per point in the order eta, psi, theta, phi.  The eta CDF is (tan eta + tan^3 eta / 3) /
+    (tan eta0 + tan^3 eta0 / 3) (the integral of sec^4), inverted numerically as well.
+    [N][7] = (eta, cos eta, sin eta, X0, X1, X2, X3), X the unit 4-vector of (psi, theta, phi): the trigonometric
+    values are part of the input (reading A18)."""
+    r = uniform01(seed, 0, 4 * N).reshape(N, 4)
+    t0 = np.tan(eta0)
+    norm = t0 + t0 ** 3 / 3.0
+    tan_eta = _invert_monotone(lambda t: (t + t ** 3 / 3.0) / norm, r[:, 0], 0.0, t0)
+    eta = np.arctan(tan_eta)
+    psi = _invert_monotone(lambda p: (2.0 * p - np.sin(2.0 * p)) / (2.0 * np.pi), r[:, 1], 0.0, np.pi)
+    ct = 1.0 - 2.0 * r[:, 2]
+    st = np.sqrt(np.maximum(0.0, 1.0 - ct * ct))
+    ph = (2.0 * np.pi) * r[:, 3]
+    sp = np.sin(psi)
+    c = np.stack([eta, np.cos(eta), np.sin(eta), np.cos(psi), sp * ct, sp * st * np.cos(ph), sp * st * np.sin(ph)], axis=1)
+    return _sort_rows(c, eta, c[:, 3])
+
+
+def sprinkle_dust_slab(N: int, seed: int, tau0: float = 1.0, r0: float = 0.5) -> np.ndarray:
+    """3+1 dust (Einstein-de Sitter) slab: tau* = tau0 u^(1/3), r* = r0 u^(1/3),
+    theta* = arccos(1 - 2u), phi* = 2 pi u.  The relation of a conformally flat FLRW spacetime is Eq. 7.7 in conformal
+    time: with a = (3 tau / 2)^(2/3) (alpha~ = 1), eta = int d tau / a = 2 (3 tau / 2)^(1/3).
+    [N][6] = (eta, r, cos th, sin th, cos ph, sin ph) for GEOM_FLRW_POLAR."""
+    r = uniform01(seed, 0, 4 * N).reshape(N, 4)
+    tau = tau0 * np.cbrt(r[:, 0])
+    eta = 2.0 * np.cbrt(1.5 * tau)
+    rad = r0 * np.cbrt(r[:, 1])
+    ct = 1.0 - 2.0 * r[:, 2]
+    st = np.sqrt(np.maximum(0.0, 1.0 - ct * ct))
+    ph = (2.0 * np.pi) * r[:, 3]
+    c = np.stack([eta, rad, ct, st, np.cos(ph), np.sin(ph)], axis=1)
+    return _sort_rows(c, eta, rad)
+
+
 def chain_lightcone(N: int) -> np.ndarray:
     """Total order: u_i = v_i = i/N (sorted already)."""
     u = np.arange(N, dtype=np.float64) / max(N, 1)
@@ -154,6 +240,10 @@ def sprinkle(geometry: int, dim: int, N: int, seed: int) -> np.ndarray:
         return sprinkle_mink2_lightcone(N, seed)
     if geometry == GEOM_MINK_CONE and dim == 4:
         return sprinkle_mink4_diamond(N, seed)
+    if geometry == GEOM_MINK_CONE and dim == 5:
+        return sprinkle_mink5_diamond(N, seed)
+    if geometry == GEOM_DS4_SPHERICAL and dim == 7:
+        return sprinkle_ds4_spherical(N, seed)
     if geometry == GEOM_MINK_CONE and dim in (2, 3):
         # lower-dimensional flat diamonds: take the first `dim` coordinates of a
         # cube rejection restricted to those coordinates
@@ -170,7 +260,7 @@ def _sprinkle_mink_low(N: int, dim: int, seed: int) -> np.ndarray:
     have = 0
     trial = 0
     while have < N:
-        batch = max(4096, int((N - have) * 4))
+        batch = max(4096, int((N - have) * (4 if dim < 5 else 18)))
         r = 2.0 * uniform01(seed, dim * trial, dim * batch).reshape(batch, dim) - 1.0
         ok = np.abs(r[:, 0]) + np.sqrt((r[:, 1:] ** 2).sum(axis=1)) <= 1.0
         acc = r[ok]

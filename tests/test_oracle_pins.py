@@ -452,3 +452,110 @@ def test_flrw_polar_relation(oracle):
     # the action pipeline treats it as 3+1 dimensional
     _, hist, S, I = oracle.action_pipeline(c, g)
     assert I == N - hist[0] + 9 * hist[1] - 16 * hist[2] + 8 * hist[3]
+
+
+# ----------------------------------------------------------------------------- NEXT-4: the other App. A regions
+def test_cone_in_five_dimensions(oracle):
+    """4+1 flat cone: hand cases incl. the null pair (related, reading A1) and the fourth spatial
+    coordinate really entering; numpy re-evaluation of the squared form on a 4+1 diamond; the ordering fraction of
+    the d-dimensional diamond falls with d (soft check that a coordinate was not dropped)."""
+    g = inp.GEOM_MINK_CONE
+    assert oracle.relation([0, 0, 0, 0, 0], [1.0, 0.5, 0.5, 0.5, 0.5], g)           # 1 >= 1: null
+    assert not oracle.relation([0, 0, 0, 0, 0], [1.0, 0.5, 0.5, 0.5, 0.51], g)
+    assert oracle.relation([0, 0, 0, 0, 0], [1.0, 0, 0, 0, 0.99], g)
+    assert not oracle.relation([0, 0, 0, 0, 0], [1.0, 0, 0, 0, 1.01], g)            # only w decides
+    assert not oracle.relation([1.0, 0, 0, 0, 0], [0, 0, 0, 0, 0], g)
+    N = 500
+    c = inp.sprinkle(g, 5, N, 31)
+    assert c.shape == (N, 5) and np.all(np.diff(c[:, 0]) >= 0)
+    assert np.all(np.abs(c[:, 0]) + np.sqrt((c[:, 1:] ** 2).sum(axis=1)) <= 1.0)
+    C = oracle.causal_matrix_bytes(c, g).astype(bool)
+    d = c[None, :, :] - c[:, None, :]
+    s = np.zeros((N, N))
+    for a in range(1, 5):
+        s = s + d[:, :, a] * d[:, :, a]
+    assert np.array_equal(C, np.triu((d[:, :, 0] >= 0) & (d[:, :, 0] ** 2 >= s), 1))
+    frac = {dim: oracle.causal_matrix_bytes(inp.sprinkle(g, dim, 600, 7), g).sum() / (600 * 599 / 2) for dim in (2, 3, 4, 5)}
+    assert frac[2] > frac[3] > frac[4] > frac[5] > 0.01
+    bits, hist, S, I = oracle.action_pipeline(c, g)                                  # no action printed for d = 5
+    assert S is None and hist.sum() == C.sum()
+
+
+def _ds4_point(eta, psi, th, ph):
+    sp = math.sin(psi)
+    return np.array([eta, math.cos(eta), math.sin(eta), math.cos(psi), sp * math.cos(th),
+                     sp * math.sin(th) * math.cos(ph), sp * math.sin(th) * math.sin(ph)])
+
+
+def test_ds4_spherical_relation(oracle):
+    """3+1 de Sitter, spherical foliation (d eta^2 > d Sigma^2).  Hand cases; the
+    arccos form of the great-circle distance away from the cone; on a great circle of the 3-sphere the relation is
+    the 1+1 slab's periodic one (GEOM_DS2_SLAB, strictness aside); transitivity; the sprinkler's marginals."""
+    g = inp.GEOM_DS4_SPHERICAL
+    assert oracle.relation(_ds4_point(0.1, 1.0, 1.0, 1.0), _ds4_point(0.2, 1.0, 1.0, 1.0), g)        # same place, later
+    assert not oracle.relation(_ds4_point(0.2, 1.0, 1.0, 1.0), _ds4_point(0.1, 1.0, 1.0, 1.0), g)    # time order
+    assert not oracle.relation(_ds4_point(0.2, 1.0, 1.0, 1.0), _ds4_point(0.2, 1.0, 1.0, 1.0), g)    # same event
+    assert oracle.relation(_ds4_point(0.0, 0.5, 1.0, 1.0), _ds4_point(0.31, 0.8, 1.0, 1.0), g)       # d psi = 0.3 < 0.31
+    assert not oracle.relation(_ds4_point(0.0, 0.5, 1.0, 1.0), _ds4_point(0.29, 0.8, 1.0, 1.0), g)
+    assert not oracle.relation(_ds4_point(0.0, 0.1, 0.0, 0.0), _ds4_point(1.4, math.pi - 0.1, 0.0, 0.0), g)  # nearly antipodal
+    rng = np.random.default_rng(3)
+    n = 0
+    for _ in range(3000):
+        e1, e2 = np.sort(rng.uniform(0.0, 1.3, 2))
+        a = (rng.uniform(0, np.pi), rng.uniform(0, np.pi), rng.uniform(0, 2 * np.pi))
+        b = (rng.uniform(0, np.pi), rng.uniform(0, np.pi), rng.uniform(0, 2 * np.pi))
+        p, q = _ds4_point(e1, *a), _ds4_point(e2, *b)
+        omega = math.acos(max(-1.0, min(1.0, float(p[3:] @ q[3:]))))
+        if abs(omega - (e2 - e1)) < 1e-9:
+            continue
+        n += 1
+        assert oracle.relation(p, q, g) == (e2 - e1 > omega)
+    assert n > 2900
+    # a great circle: psi = th = pi/2, phi free -> the relation of the 1+1 slab on (eta, phi)
+    for _ in range(2000):
+        e1, e2 = np.sort(rng.uniform(0.0, 1.3, 2))
+        f1, f2 = rng.uniform(0, 2 * np.pi, 2)
+        d = min(abs(f1 - f2), 2 * np.pi - abs(f1 - f2))
+        if abs(d - (e2 - e1)) < 1e-9:
+            continue
+        assert oracle.relation(_ds4_point(e1, np.pi / 2, np.pi / 2, f1), _ds4_point(e2, np.pi / 2, np.pi / 2, f2), g) == \
+            oracle.relation([e1, f1], [e2, f2], inp.GEOM_DS2_SLAB)
+    N = 600
+    c = inp.sprinkle(g, 7, N, 17)
+    assert np.all(np.diff(c[:, 0]) >= 0) and np.allclose((c[:, 3:] ** 2).sum(axis=1), 1) and np.allclose(c[:, 1] ** 2 + c[:, 2] ** 2, 1)
+    C = oracle.causal_matrix_bytes(c, g).astype(bool)
+    assert np.array_equal(C, np.triu(C, 1)) and 0.005 < C.sum() / (N * (N - 1) / 2) < 0.6
+    assert not (C.astype(np.int32) @ C.astype(np.int32) > 0)[~C & np.triu(np.ones_like(C), 1)].any()
+    _, hist, S, I = oracle.action_pipeline(c, g)                                     # a 3+1 dimensional spacetime
+    assert I == N - hist[0] + 9 * hist[1] - 16 * hist[2] + 8 * hist[3]
+    # marginals of the sprinkler (PAPER.md:3835-3841): E[sin^2 psi] = 3/4 under (2/pi) sin^2 psi, E[cos th] = 0
+    big = inp.sprinkle_ds4_spherical(20000, 5)
+    assert abs((1 - big[:, 3] ** 2).mean() - 0.75) < 0.01 and abs(big[:, 4].mean()) < 0.02
+    assert big[:, 0].min() >= 0 and big[:, 0].max() <= 1.0 and np.median(big[:, 0]) > 0.7     # sec^4: late times dominate
+
+
+def test_appendix_a_sprinklers(oracle):
+    """The remaining flat / FLRW regions are sprinklers over predicates already pinned: the 1+1 square and the paper's
+    own inverse-CDF 2+1 diamond feed the flat cone, the 1+1 cylinder the periodic relation, the dust slab Eq. 7.7 in
+    conformal time.  Checks: region bounds, time order, the 2+1 diamond's radial law, and that the dust slab's
+    relation agrees with the flat cone in Cartesian conformal coordinates."""
+    sq = inp.sprinkle_mink2_square(500, 3, t0=0.5, x0=2.0)
+    assert np.all(np.abs(sq[:, 0]) <= 0.5) and np.all(np.abs(sq[:, 1]) <= 2.0) and np.all(np.diff(sq[:, 0]) >= 0)
+    cy = inp.sprinkle_mink2_cylinder(500, 4)
+    assert np.all((cy[:, 1] >= 0) & (cy[:, 1] < 2 * np.pi)) and np.all(np.diff(cy[:, 0]) >= 0)
+    C = oracle.causal_matrix_bytes(cy, inp.GEOM_DS2_SLAB)
+    d = np.abs(cy[None, :, 1] - cy[:, None, 1]); d = np.minimum(d, 2 * np.pi - d)
+    assert np.array_equal(C.astype(bool), np.triu((cy[None, :, 0] - cy[:, None, 0]) >= d, 1))
+    di = inp.sprinkle_mink3_diamond_uv(20000, 5)
+    t, r = di[:, 0], np.hypot(di[:, 1], di[:, 2])
+    u, v = (t + r) / np.sqrt(2), (t - r) / np.sqrt(2)
+    assert np.all(u <= 1 + 1e-12) and np.all(v >= -1e-12) and np.all(v <= u + 1e-12)
+    assert abs((u ** 3).mean() - 0.5) < 0.01                  # u* = u^(1/3): u*^3 is uniform
+    du = inp.sprinkle_dust_slab(400, 6)
+    assert np.all(np.diff(du[:, 0]) >= 0) and np.all(du[:, 1] <= 0.5)
+    C = oracle.causal_matrix_bytes(du, inp.GEOM_FLRW_POLAR).astype(bool)
+    x = du[:, 1] * du[:, 3] * du[:, 4]; y = du[:, 1] * du[:, 3] * du[:, 5]; z = du[:, 1] * du[:, 2]
+    dt = du[None, :, 0] - du[:, None, 0]
+    q = dt ** 2 - ((x[None] - x[:, None]) ** 2 + (y[None] - y[:, None]) ** 2 + (z[None] - z[:, None]) ** 2)
+    clear = np.triu(np.abs(q) > 1e-12, 1)
+    assert np.array_equal(C[clear], np.triu((dt > 0) & (q > 0), 1)[clear]) and C.sum() > 1000
