@@ -43,8 +43,9 @@ enum cs_geometry {
     /* dim = 2, coords (u,v) light-cone coordinates, ds^2 = -2 du dv:
        i -< j  <=>  u_i < u_j && v_i < v_j. */
     CS_GEOM_MINK2_LIGHTCONE = 0,
-    /* dim = 2..4, coords (t,x[,y[,z]]) (squared form of Eq. 7.7):
-       dt = t_j - t_i, d_a = x^a_j - x^a_i, s = ((dx*dx) + (dy*dy)) + (dz*dz),
+    /* dim = 2..5, coords (t,x[,y[,z[,w]]]) (squared form of Eq. 7.7; dim 5 = the 4+1
+       diamond of App. A.1.2):
+       dt = t_j - t_i, d_a = x^a_j - x^a_i, s = (((dx*dx) + (dy*dy)) + (dz*dz)) + (dw*dw),
        i -< j  <=>  dt >= 0 && dt*dt >= s        (fp64, no FMA contraction). */
     CS_GEOM_MINK_CONE = 1,
     /* dim = 2, coords (eta,theta) of the 1+1 de Sitter slab (Eq. 4.19):
@@ -58,7 +59,16 @@ enum cs_geometry {
        d2 = ((r_i*r_i) + (r_j*r_j)) - ((2*(r_i*r_j))*ang), deta = eta_j - eta_i,
        i -< j  <=>  deta > 0 && d2 < deta*deta   (fp64, no FMA contraction).
        The spacetime dimension (for the action entry points that take coordinates) is 4. */
-    CS_GEOM_FLRW_POLAR = 3
+    CS_GEOM_FLRW_POLAR = 3,
+    /* dim = 7, a point is (eta, cos eta, sin eta, X0, X1, X2, X3): 3+1 de Sitter with spherical foliation,
+       ds^2 = lambda^2 sec^2(eta) (-d eta^2 + d Omega_3^2) (App. A.1.3), X = (cos psi,
+       sin psi cos th, sin psi sin th cos ph, sin psi sin th sin ph) the point's unit vector on the 3-sphere.
+       Timelike <=> d eta^2 > d Sigma^2 with d Sigma = omega the great-circle angle; for
+       0 < d eta <= pi that is cos(d eta) < cos(omega) (reading A18):
+       cd = (ce_i*ce_j) + (se_i*se_j), co = ((X0_i*X0_j) + (X1_i*X1_j)) + ((X2_i*X2_j) + (X3_i*X3_j)),
+       i -< j  <=>  eta_j - eta_i > 0 && cd < co   (fp64, no FMA contraction; strict like Eq. 7.7).
+       The spacetime dimension (for the action entry points that take coordinates) is 4. */
+    CS_GEOM_DS4_SPHERICAL = 4
 };
 
 enum cs_status {

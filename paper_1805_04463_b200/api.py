@@ -21,6 +21,7 @@ GEOM_MINK_CONE = 1
 GEOM_DS2_SLAB = 2
 
 GEOM_FLRW_POLAR = 3   # include/causalset.h
+GEOM_DS4_SPHERICAL = 4
 ROUTE_AUTO = 0
 ROUTE_POPC = 1
 ROUTE_TENSOR = 2

@@ -24,7 +24,10 @@ int sm_count()
 
 // spacetime dimension of a point set: the number of coordinates, except for the FLRW geometry whose six
 // numbers per point describe a 3+1 dimensional event
-static int spacetime_dim(int geometry, int dim) { return geometry == CS_GEOM_FLRW_POLAR ? 4 : dim; }
+static int spacetime_dim(int geometry, int dim)
+{
+    return (geometry == CS_GEOM_FLRW_POLAR || geometry == CS_GEOM_DS4_SPHERICAL) ? 4 : dim;
+}
 
 // rows are read with 128-bit loads, bulk copies and TMA: the matrices must start on a 16-byte boundary
 static bool misaligned16(const void *a, const void *b)
@@ -134,9 +137,9 @@ int cs_causal_matrix_batched(const double *coords, int64_t B, int64_t N, int dim
                              uint64_t *bits, uint64_t *bitsT, void *stream)
 {
     if (N < 0 || B < 0) return CS_ERR_ARG;
-    if (geometry < CS_GEOM_MINK2_LIGHTCONE || geometry > CS_GEOM_FLRW_POLAR) return CS_ERR_GEOM;
-    if (geometry == CS_GEOM_MINK_CONE ? (dim < 2 || dim > 4) : (dim != (geometry == CS_GEOM_FLRW_POLAR ? 6 : 2)))
-        return CS_ERR_DIM;
+    if (geometry < CS_GEOM_MINK2_LIGHTCONE || geometry > CS_GEOM_DS4_SPHERICAL) return CS_ERR_GEOM;
+    const int want = geometry == CS_GEOM_FLRW_POLAR ? 6 : geometry == CS_GEOM_DS4_SPHERICAL ? 7 : 2;
+    if (geometry == CS_GEOM_MINK_CONE ? (dim < 2 || dim > 5) : (dim != want)) return CS_ERR_DIM;
     if (N == 0 || B == 0) return CS_OK;
     if (!coords || !bits) return CS_ERR_ARG;
     return launch_causal_matrix(coords, B, N, dim, geometry, bits, bitsT, static_cast<cudaStream_t>(stream));
@@ -355,7 +358,7 @@ static int copy_pipe(CopyPipe **out)
 
 size_t cs_bd_action_batched_host_workspace(int64_t B, int64_t N, int dim)
 {
-    if (B < 0 || N < 0 || dim < 2 || dim > 6) return 0;
+    if (B < 0 || N < 0 || dim < 2 || dim > 7) return 0;
     const int64_t CB = ensemble_chunk(B);
     const size_t cbuf = align_up((size_t)CB * N * dim * 8, 256);
     const size_t mat = align_up((size_t)CB * N * row_stride_words(N) * 8, 256);
@@ -370,7 +373,7 @@ int cs_bd_action_batched_host(const double *coords_host, int64_t B, int64_t N, i
     if (B < 0 || N < 0) return CS_ERR_ARG;
     if (B == 0) return CS_OK;
     if (!coords_host || !actions_host) return CS_ERR_ARG;
-    if (dim < 2 || dim > 6) return CS_ERR_DIM;
+    if (dim < 2 || dim > 7) return CS_ERR_DIM;
     if (!workspace || workspace_bytes < cs_bd_action_batched_host_workspace(B, N, dim) || ((uintptr_t)workspace & 255))
         return CS_ERR_WORKSPACE;
     cudaStream_t st = static_cast<cudaStream_t>(stream);
@@ -432,7 +435,7 @@ size_t cs_action_host_workspace(int64_t N, int64_t kmax)
     if (N < 0) return 0;
     kmax = clamp_kmax(N, kmax);
     const size_t mat = align_up((size_t)N * row_stride_words(N) * 8, 256);
-    return align_up((size_t)N * 6 * 8, 256) + 2 * mat + align_up((size_t)(kmax + 1) * 8, 256) + 256 +
+    return align_up((size_t)N * 7 * 8, 256) + 2 * mat + align_up((size_t)(kmax + 1) * 8, 256) + 256 +
            interval_ws_bytes(1, N, 1, cs_default_route(N));
 }
 
@@ -441,7 +444,7 @@ int cs_action_host(const double *coords_host, int64_t N, int dim, int geometry, 
                    void *workspace, size_t workspace_bytes, void *stream)
 {
     if (N < 0 || !hist_host || !action_host || (N > 0 && !coords_host)) return CS_ERR_ARG;
-    if (dim < 2 || dim > 6) return CS_ERR_DIM;
+    if (dim < 2 || dim > 7) return CS_ERR_DIM;
     if (!workspace || workspace_bytes < cs_action_host_workspace(N, kmax) || ((uintptr_t)workspace & 255))
         return CS_ERR_WORKSPACE;
     cudaStream_t st = static_cast<cudaStream_t>(stream);
@@ -449,7 +452,7 @@ int cs_action_host(const double *coords_host, int64_t N, int dim, int geometry, 
     const size_t mat = align_up((size_t)N * row_stride_words(N) * 8, 256);
     unsigned char *ws = static_cast<unsigned char *>(workspace);
     double *coords = reinterpret_cast<double *>(ws);
-    ws += align_up((size_t)N * 6 * 8, 256);
+    ws += align_up((size_t)N * 7 * 8, 256);
     uint64_t *bits = reinterpret_cast<uint64_t *>(ws);
     ws += mat;
     uint64_t *bitsT = reinterpret_cast<uint64_t *>(ws);

@@ -45,6 +45,10 @@ struct Pred<CS_GEOM_MINK_CONE, DIM> {
             double dz = __dsub_rn(xj[3], xi[3]);
             s = __dadd_rn(s, __dmul_rn(dz, dz));
         }
+        if (DIM >= 5) {
+            double dw = __dsub_rn(xj[4], xi[4]);
+            s = __dadd_rn(s, __dmul_rn(dw, dw));
+        }
         return (dt >= 0.0) && (__dmul_rn(dt, dt) >= s);
     }
 };
@@ -75,6 +79,18 @@ struct Pred<CS_GEOM_FLRW_POLAR, 6> {
     }
 };
 
+template <>
+struct Pred<CS_GEOM_DS4_SPHERICAL, 7> {
+    __device__ static __forceinline__ bool rel(const double *xi, const double *xj)
+    {
+        const double deta = __dsub_rn(xj[0], xi[0]);
+        const double cd = __dadd_rn(__dmul_rn(xi[1], xj[1]), __dmul_rn(xi[2], xj[2]));
+        const double co = __dadd_rn(__dadd_rn(__dmul_rn(xi[3], xj[3]), __dmul_rn(xi[4], xj[4])),
+                                    __dadd_rn(__dmul_rn(xi[5], xj[5]), __dmul_rn(xi[6], xj[6])));
+        return (deta > 0.0) && (cd < co);
+    }
+};
+
 // ---- exact single-precision prefilter (flat cone) ----------------------------------------------
 // With h = (t^2 - |x|^2) / 2 the sign of the interval is the sign of
 //     T = ((t_j - t_i)^2 - |x_j - x_i|^2) / 2 = h_i + h_j - t_i t_j + x_i . x_j ,
@@ -95,12 +111,89 @@ struct Pred<CS_GEOM_FLRW_POLAR, 6> {
 // roundings and the subtraction), b = 2pi - a by <= 8 u C, the minimum by no more, d = deta - m by
 // <= 17 u C; margin m = 32 u C.  d > m => D > 15 u C => the fp64 expression (errors ~2^-50 C) says related,
 // d < -m => unrelated, else fp64.  No time-order condition: the header's expression has none.
+//
+// The same scheme covers every predicate that is the sign of a bilinear form  T = sum_c P_c(i) F_c(j) + h_i + h_j :
+//   flat cone, dim 2..5      P = (-t, x, ..), F = (t, x, ..), h = (t^2 - |x|^2) / 2
+//   FLRW, Eq. 7.7            the flat cone of the Cartesian conformal coordinates (eta, r st cp, r st sp, r ct), formed
+//                            per point in fp64.  The header's law-of-cosines value differs from |x_i - x_j|^2 by
+//                            r^2 (1 - (ct^2 + st^2 (cp^2 + sp^2))) per point, so a tile takes the fast path only if every
+//                            point has ct^2 + st^2 and cp^2 + sp^2 within 2^-30 of 1 (<= 2^-28 C^2 in all, against a
+//                            margin of 2^-18 C^2); anything else falls back to the header's fp64 expression.
+//   3+1 de Sitter, spherical P = (-cos eta, -sin eta, X0..X3), F = (cos eta, sin eta, X0..X3), no h:
+//                            T = cos(omega) - cos(d eta); 12 input roundings + partial sums 1..6 C^2 <= 33 u C^2.
+//                            Unit inputs only (see Fast<DS4_SPHERICAL>::convert: pairs of equal times).
+// With NP products the bound is (2.01 NP + (NP - 1) + sum of the partial sums) u C^2: 34 (NP = 4), 48 (NP = 5), so the
+// margin is 64 u C^2 up to four products (and for the h-free six of de Sitter) and 96 u C^2 for five.
+// The first NNEG components are stored negated for the past point.  convert() returns false for a point that may not
+// use the prefilter.
 template <int GEOM, int DIM>
-struct FastCone { static constexpr bool ok = false; };
+struct Fast {
+    static constexpr bool ok = false, H = false;
+    static constexpr int NP = 1, NNEG = 0, MARGIN = 64;
+    __device__ static __forceinline__ bool convert(const double *, float *, float &) { return false; }
+};
 template <int DIM>
-struct FastCone<CS_GEOM_MINK_CONE, DIM> { static constexpr bool ok = true; };
+struct Fast<CS_GEOM_MINK_CONE, DIM> {
+    static constexpr bool ok = true, H = true;
+    static constexpr int NP = DIM, NNEG = 1, MARGIN = DIM <= 4 ? 64 : 96;
+    __device__ static __forceinline__ bool convert(const double *x, float *v, float &h)
+    {
+        double sq = 0.0;
+#pragma unroll
+        for (int d = 0; d < DIM; d++) {
+            v[d] = (float)x[d];
+            if (d > 0) sq += x[d] * x[d];
+        }
+        h = (float)(0.5 * (x[0] * x[0] - sq));
+        return true;
+    }
+};
 template <>
-struct FastCone<CS_GEOM_DS2_SLAB, 2> { static constexpr bool ok = true; };
+struct Fast<CS_GEOM_DS2_SLAB, 2> {      // not a bilinear form: its own five-operation expression (above)
+    static constexpr bool ok = true, H = false;
+    static constexpr int NP = 2, NNEG = 0, MARGIN = 32;
+    __device__ static __forceinline__ bool convert(const double *x, float *v, float &h)
+    {
+        v[0] = (float)x[0];
+        v[1] = (float)x[1];
+        h = 0.f;
+        return true;
+    }
+};
+template <>
+struct Fast<CS_GEOM_DS4_SPHERICAL, 7> {
+    static constexpr bool ok = true, H = false;
+    static constexpr int NP = 6, NNEG = 2, MARGIN = 64;
+    __device__ static __forceinline__ bool convert(const double *x, float *v, float &h)
+    {
+#pragma unroll
+        for (int c = 0; c < 6; c++) v[c] = (float)x[1 + c];
+        h = 0.f;
+        // The header's expression also wants eta_j > eta_i; the tile-level time order only gives >=.  With unit
+        // inputs a pair of equal times has T = cos(omega) - 1 <= 2^-29, never above the margin, so it is decided
+        // "unrelated" or re-evaluated; inputs that are not unit vectors do not take the prefilter.
+        const double n1 = x[1] * x[1] + x[2] * x[2] - 1.0;
+        const double n2 = (x[3] * x[3] + x[4] * x[4]) + (x[5] * x[5] + x[6] * x[6]) - 1.0;
+        return fabs(n1) <= 0x1p-30 && fabs(n2) <= 0x1p-30;      // false for NaN
+    }
+};
+template <>
+struct Fast<CS_GEOM_FLRW_POLAR, 6> {
+    static constexpr bool ok = true, H = true;
+    static constexpr int NP = 4, NNEG = 1, MARGIN = 64;
+    __device__ static __forceinline__ bool convert(const double *x, float *v, float &h)
+    {
+        const double rs = x[1] * x[3];
+        const double cx = rs * x[4], cy = rs * x[5], cz = x[1] * x[2];
+        v[0] = (float)x[0];
+        v[1] = (float)cx;
+        v[2] = (float)cy;
+        v[3] = (float)cz;
+        h = (float)(0.5 * (x[0] * x[0] - (cx * cx + cy * cy + cz * cz)));
+        const double n1 = x[2] * x[2] + x[3] * x[3] - 1.0, n2 = x[4] * x[4] + x[5] * x[5] - 1.0;
+        return fabs(n1) <= 0x1p-30 && fabs(n2) <= 0x1p-30;      // false for NaN
+    }
+};
 
 // order-preserving map float -> uint32 (NaN with the sign bit clear sorts above +inf, set below -inf)
 __device__ __forceinline__ uint32_t float_key(float f)
@@ -161,6 +254,12 @@ __device__ __forceinline__ f32x2 ffma2(f32x2 a, f32x2 b, f32x2 c)
     asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c));
     return d;
 }
+__device__ __forceinline__ f32x2 fmul2(f32x2 a, f32x2 b)
+{
+    f32x2 d;
+    asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+    return d;
+}
 __device__ __forceinline__ f32x2 fadd2(f32x2 a, f32x2 b)
 {
     f32x2 d;
@@ -184,17 +283,19 @@ __device__ __forceinline__ float min3_abs_nan(float u, uint32_t a, uint32_t b)
 // decided by the fp32 prefilter; unc[k] is set if any of the lane's 32 decisions is inside the error
 // band (or NaN).
 //
-// Flat cone: the past points sit in shared memory as five arrays (-t, x, y, z, h), so one LDS.128 brings a
-// coordinate of four consecutive rows and each 64-bit half feeds a packed operation on two rows; the future
+// Bilinear forms (flat cone, FLRW, 3+1 de Sitter): the past points sit in shared memory as NP (+1) arrays
+// (-t, x, y, z, h for the 3+1 cone), so one LDS.128 brings a component of four consecutive rows and each 64-bit half feeds a packed operation on two rows; the future
 // point's coordinates are per-lane scalars that FFMA2 broadcasts.  Per four pairs: 8 FFMA2 + 2 FADD2 for the
 // values, then one SHF per pair shifts the value's sign bit into the lane's word and one FMNMX3 per two pairs
 // keeps the smallest |a| -- if that exceeds the margin m, no decision of the block is inside the band, and
 // "a > m" is simply "sign bit clear".  4 instructions per pair instead of 8 (4 FFMA, FADD, 2 FSETP, predicated add).
 template <int GEOM, int DIM, int NK>
 __device__ __forceinline__ void fast_block(const float *__restrict__ sf, int i0,
-                                           const float (*fj)[4], const float *hj, const float *m,
+                                           const float (*fj)[Fast<GEOM, DIM>::NP], const float *hj, const float *m,
                                            uint32_t *lw, bool *unc)
 {
+    constexpr int NP = Fast<GEOM, DIM>::NP;
+    constexpr bool H = Fast<GEOM, DIM>::H;
     if (GEOM == CS_GEOM_DS2_SLAB) {
         const float2 *fi = reinterpret_cast<const float2 *>(sf) + i0;     // (eta, theta) per past point
 #pragma unroll
@@ -213,32 +314,40 @@ __device__ __forceinline__ void fast_block(const float *__restrict__ sf, int i0,
     }
     uint32_t sg[NK];
     float mn[NK];
-    f32x2 ft[NK], fx[NK], fy[NK], fz[NK], fh[NK];
+    f32x2 fb[NK][NP], fh[NK];
 #pragma unroll
     for (int k = 0; k < NK; k++) {
         sg[k] = 0;
         mn[k] = __int_as_float(0x7f800000);
-        ft[k] = bcast2(fj[k][0]);
-        fx[k] = bcast2(fj[k][1]);
-        fy[k] = bcast2(fj[k][2]);
-        fz[k] = bcast2(fj[k][3]);
+#pragma unroll
+        for (int c = 0; c < NP; c++) fb[k][c] = bcast2(fj[k][c]);
         fh[k] = bcast2(hj[k]);
     }
 #pragma unroll
     for (int i4 = 0; i4 < 32; i4 += 4) {
-        const ulonglong2 T = *reinterpret_cast<const ulonglong2 *>(sf + (0) * BT + i0 + i4);     // -t of rows (0,1), (2,3)
-        const ulonglong2 X = *reinterpret_cast<const ulonglong2 *>(sf + (1) * BT + i0 + i4);
-        const ulonglong2 Y = *reinterpret_cast<const ulonglong2 *>(sf + (DIM > 2 ? 2 : 0) * BT + i0 + i4);
-        const ulonglong2 Z = *reinterpret_cast<const ulonglong2 *>(sf + (DIM > 3 ? 3 : 0) * BT + i0 + i4);
-        const ulonglong2 H = *reinterpret_cast<const ulonglong2 *>(sf + (4) * BT + i0 + i4);
+        ulonglong2 P[NP], Hh;                           // component c of rows (0,1), (2,3)
+#pragma unroll
+        for (int c = 0; c < NP; c++) P[c] = *reinterpret_cast<const ulonglong2 *>(sf + c * BT + i0 + i4);
+        if (H) Hh = *reinterpret_cast<const ulonglong2 *>(sf + NP * BT + i0 + i4);
 #pragma unroll
         for (int k = 0; k < NK; k++) {
-            f32x2 a01 = ffma2(T.x, ft[k], H.x), a23 = ffma2(T.y, ft[k], H.y);
-            a01 = ffma2(X.x, fx[k], a01); a23 = ffma2(X.y, fx[k], a23);
-            if (DIM > 2) { a01 = ffma2(Y.x, fy[k], a01); a23 = ffma2(Y.y, fy[k], a23); }
-            if (DIM > 3) { a01 = ffma2(Z.x, fz[k], a01); a23 = ffma2(Z.y, fz[k], a23); }
-            a01 = fadd2(a01, fh[k]);
-            a23 = fadd2(a23, fh[k]);
+            f32x2 a01, a23;
+            if (H) {
+                a01 = ffma2(P[0].x, fb[k][0], Hh.x);
+                a23 = ffma2(P[0].y, fb[k][0], Hh.y);
+            } else {
+                a01 = fmul2(P[0].x, fb[k][0]);
+                a23 = fmul2(P[0].y, fb[k][0]);
+            }
+#pragma unroll
+            for (int c = 1; c < NP; c++) {
+                a01 = ffma2(P[c].x, fb[k][c], a01);
+                a23 = ffma2(P[c].y, fb[k][c], a23);
+            }
+            if (H) {
+                a01 = fadd2(a01, fh[k]);
+                a23 = fadd2(a23, fh[k]);
+            }
             const uint32_t a0 = (uint32_t)a01, a1 = (uint32_t)(a01 >> 32), a2 = (uint32_t)a23, a3 = (uint32_t)(a23 >> 32);
             sg[k] = __funnelshift_l(a0, sg[k], 1);      // row i0 + ii ends up at bit 31 - ii
             sg[k] = __funnelshift_l(a1, sg[k], 1);
@@ -269,6 +378,19 @@ __device__ __forceinline__ void exact_block(const double (*xi_s)[BT], int i0, co
     }
 }
 
+// shared memory of one CTA (dynamic: the wider geometries pass the 48 KB static limit)
+template <int GEOM, int DIM>
+struct BuildSmem {
+    using F = Fast<GEOM, DIM>;
+    static constexpr int NF = F::ok ? F::NP + (F::H ? 1 : 0) : 0;          // fp32 arrays of the past points
+    static constexpr size_t XI = 0;                                         // double [DIM][BT]
+    static constexpr size_t SF = XI + (size_t)DIM * BT * 8;                 // float  [NF][BT]
+    static constexpr size_t SU = SF + (size_t)NF * BT * 4;                  // uint32 [BT][NJ * 8 + 1]
+    static constexpr size_t SL = SU + (size_t)BT * (NJ * 8 + 1) * 4;        // uint32 [NJ * BT][9]
+    static constexpr size_t BYTES = SL + (size_t)NJ * BT * 9 * 4;
+    static_assert(SF % 16 == 0 && SU % 16 == 0 && BYTES <= 56 * 1024, "k_causal_matrix: shared memory (four CTAs per SM)");
+};
+
 template <int GEOM, int DIM>
 __global__ void __launch_bounds__(BUILD_THREADS)
 k_causal_matrix(const double *__restrict__ coords, int64_t N, int64_t stride,
@@ -282,17 +404,18 @@ k_causal_matrix(const double *__restrict__ coords, int64_t N, int64_t stride,
     bits += b * N * stride;
     if (bitsT) bitsT += b * N * stride;
 
-    constexpr bool FAST = FastCone<GEOM, DIM>::ok;
+    using F = Fast<GEOM, DIM>;
+    using SM = BuildSmem<GEOM, DIM>;
+    constexpr bool FAST = F::ok;
+    constexpr int NP = F::NP;
     constexpr int NW = BUILD_THREADS / 32;
-    __shared__ double s_xi[DIM][BT];
-    // fp32 copies of the past points: flat cone -t, x, y, z, h as five arrays; dS slab (eta, theta) pairs in the first two
-    __shared__ __align__(16) float s_f[FAST ? 5 : 1][FAST ? BT : 4];
-    __shared__ __align__(16) uint32_t s_U[BT][NJ * 8 + 1]; // row i_local, 32-bit word = 32 columns j
-    __shared__ uint32_t s_L[NJ * BT][9];                   // row j_local, 32-bit word = 32 rows i
-    uint32_t (*s_red)[NW] = reinterpret_cast<uint32_t (*)[NW]>(&s_U[0][0]);   // [2 + 2 NJ][NW], dead before s_U is written
-    // static shared memory stops at 48 KB; the flat cone in 3+1 dimensions sits exactly on it
-    static_assert(sizeof(s_xi) + sizeof(s_f) + sizeof(s_U) + sizeof(s_L) <= 48 * 1024,
-                  "k_causal_matrix: static shared memory");
+    extern __shared__ __align__(16) unsigned char dsm[];
+    double (*s_xi)[BT] = reinterpret_cast<double (*)[BT]>(dsm + SM::XI);
+    // fp32 copies of the past points: NP component arrays (+ h); dS slab: (eta, theta) pairs
+    float *s_f = reinterpret_cast<float *>(dsm + SM::SF);
+    uint32_t (*s_U)[NJ * 8 + 1] = reinterpret_cast<uint32_t (*)[NJ * 8 + 1]>(dsm + SM::SU);   // row i_local, word = 32 columns j
+    uint32_t (*s_L)[9] = reinterpret_cast<uint32_t (*)[9]>(dsm + SM::SL);                     // row j_local, word = 32 rows i
+    uint32_t (*s_red)[NW] = reinterpret_cast<uint32_t (*)[NW]>(dsm + SM::SU);   // [2 + 2 NJ][NW], dead before s_U is written
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const double qnan = __longlong_as_double(0x7FF8000000000000LL);   // compares false: unrelated
@@ -327,46 +450,43 @@ k_causal_matrix(const double *__restrict__ coords, int64_t N, int64_t stride,
     }
 
     bool fast[NJ];
-    float fj[NJ][4], hj[NJ], m[NJ];
+    float fj[NJ][NP], hj[NJ], m[NJ];
 #pragma unroll
-    for (int k = 0; k < NJ; k++) { fast[k] = false; hj[k] = 0.f; m[k] = 0.f; fj[k][0] = fj[k][1] = fj[k][2] = fj[k][3] = 0.f; }
+    for (int k = 0; k < NJ; k++) {
+        fast[k] = false; hj[k] = 0.f; m[k] = 0.f;
+#pragma unroll
+        for (int c = 0; c < NP; c++) fj[k][c] = 0.f;
+    }
     if (FAST) {
         // Tile summaries, all as floats reduced with redux.sync on order-preserving integer keys:
-        //   C   >= largest |coordinate| of the past points and of each set of future points (the fp32
-        //          conversions, NaN ignored by fmaxf; rounding to nearest is covered by m's 1.001),
+        //   C   >= largest |component| of the past points and of each set of future points (the fp32
+        //          conversions, NaN ignored by fmaxf; rounding to nearest is covered by m's 1.001); a point that
+        //          may not use the prefilter (Fast::convert) reports +inf, which fails the range test below,
         //   max t_i rounded up and min t_j rounded down, so "max t_i <= min t_j" is only ever claimed when
         //   it holds for the doubles (a NaN time makes the claim fail or is ignored; either is safe).
         // Inside the diagonal tile i < j must imply t_i <= t_j instead: its points are in time order.
-        double si = 0.0;
-        float fi[4] = {0.f, 0.f, 0.f, 0.f}, ci = 0.f;
+        float fi[NP], hi0, ci = 0.f;
+        const bool oki = F::convert(xi0, fi, hi0);
 #pragma unroll
-        for (int d = 0; d < DIM; d++) {
-            fi[d] = (float)xi0[d];
-            ci = fmaxf(ci, fabsf(fi[d]));
-            if (d > 0) si += xi0[d] * xi0[d];
-        }
+        for (int c = 0; c < NP; c++) ci = fmaxf(ci, fabsf(fi[c]));
+        if (!oki && !(xi0[0] != xi0[0])) ci = __int_as_float(0x7f800000);     // (padding points are NaN: harmless)
         if (GEOM == CS_GEOM_DS2_SLAB) {
-            reinterpret_cast<float2 *>(&s_f[0][0])[tid] = make_float2(fi[0], fi[1]);
+            reinterpret_cast<float2 *>(s_f)[tid] = make_float2(fi[0], fi[1]);
         } else {
-            s_f[0][tid] = -fi[0];
 #pragma unroll
-            for (int d = 1; d < DIM; d++) s_f[d][tid] = fi[d];
-            s_f[4][tid] = (float)(0.5 * (xi0[0] * xi0[0] - si));
+            for (int c = 0; c < NP; c++) s_f[c * BT + tid] = c < F::NNEG ? -fi[c] : fi[c];
+            if (F::H) s_f[NP * BT + tid] = hi0;
         }
         const uint32_t wci = __reduce_max_sync(0xffffffffu, __float_as_uint(ci));   // ci >= 0: bit order = value order
         const uint32_t wti = __reduce_max_sync(0xffffffffu, float_key(__double2float_ru(xi0[0])));
         if (lane == 0) { s_red[0][warp] = wci; s_red[1][warp] = wti; }
 #pragma unroll
         for (int k = 0; k < NJ; k++) {
-            double sj = 0.0;
             float cj = 0.f;
+            const bool okj = F::convert(xj[k], fj[k], hj[k]);
 #pragma unroll
-            for (int d = 0; d < DIM; d++) {
-                fj[k][d] = (float)xj[k][d];
-                cj = fmaxf(cj, fabsf(fj[k][d]));
-                if (d > 0) sj += xj[k][d] * xj[k][d];
-            }
-            hj[k] = (float)(0.5 * (xj[k][0] * xj[k][0] - sj));
+            for (int c = 0; c < NP; c++) cj = fmaxf(cj, fabsf(fj[k][c]));
+            if (!okj && !(xj[k][0] != xj[k][0])) cj = __int_as_float(0x7f800000);
             const uint32_t wcj = __reduce_max_sync(0xffffffffu, __float_as_uint(cj));
             const uint32_t wtj = __reduce_max_sync(0xffffffffu, float_key(-__double2float_rd(xj[k][0])));   // -(min t_j)
             if (lane == 0) { s_red[2 + 2 * k][warp] = wcj; s_red[3 + 2 * k][warp] = wtj; }
@@ -395,11 +515,11 @@ k_causal_matrix(const double *__restrict__ coords, int64_t N, int64_t stride,
             } else {
                 const bool ordered = dg[k] ? tile_ordered : (tmaxI <= -key_float(r[3 + 2 * k]));
                 fast[k] = act[k] && ordered && (C >= 0x1p-40f) && (C <= 0x1p40f);
-                m[k] = __fmul_ru(__fmul_ru(C, C), 0x1p-18f * 1.001f);
+                m[k] = __fmul_ru(__fmul_ru(C, C), (float)F::MARGIN * 0x1p-24f * 1.001f);
             }
         }
     }
-    __syncthreads();    // s_xi / s_fi / s_hi visible; s_red (aliased on s_U) no longer read
+    __syncthreads();    // s_xi / s_f visible; s_red (aliased on s_U) no longer read
 
 #pragma unroll 1
     for (int sb = 0; sb < BT / 32; sb++) {
@@ -414,9 +534,9 @@ k_causal_matrix(const double *__restrict__ coords, int64_t N, int64_t stride,
         if (FAST) {
             bool unc[NJ] = {false, false};
             const bool f0 = need[0] && fast[0], f1 = need[1] && fast[1];
-            if (f0 && f1) fast_block<GEOM, DIM, 2>(&s_f[0][0], sb * 32, fj, hj, m, lw, unc);
-            else if (f0) fast_block<GEOM, DIM, 1>(&s_f[0][0], sb * 32, fj, hj, m, lw, unc);
-            else if (f1) fast_block<GEOM, DIM, 1>(&s_f[0][0], sb * 32, fj + 1, hj + 1, m + 1, lw + 1, unc + 1);
+            if (f0 && f1) fast_block<GEOM, DIM, 2>(s_f, sb * 32, fj, hj, m, lw, unc);
+            else if (f0) fast_block<GEOM, DIM, 1>(s_f, sb * 32, fj, hj, m, lw, unc);
+            else if (f1) fast_block<GEOM, DIM, 1>(s_f, sb * 32, fj + 1, hj + 1, m + 1, lw + 1, unc + 1);
 #pragma unroll
             for (int k = 0; k < NJ; k++) {
                 if (__any_sync(0xffffffffu, unc[k])) { slow[k] = true; lw[k] = 0; }
@@ -495,7 +615,16 @@ static int launch_build_t(const double *coords, int64_t B, int64_t N, int64_t st
 {
     const int nT = (int)((N + BT - 1) / BT);
     dim3 grid((nT + NJ - 1) / NJ, nT, (unsigned)B);   // x: groups of NJ column tiles, y: row tile
-    k_causal_matrix<GEOM, DIM><<<grid, BUILD_THREADS, 0, st>>>(coords, N, stride, bits, bitsT);
+    constexpr size_t smem = BuildSmem<GEOM, DIM>::BYTES;
+    if (smem > 48 * 1024) {
+        static PerDeviceFlag attr_set;
+        const int dev = current_device();
+        if (!attr_set.get(dev)) {
+            CS_CUDA(cudaFuncSetAttribute(k_causal_matrix<GEOM, DIM>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+            attr_set.set(dev);
+        }
+    }
+    k_causal_matrix<GEOM, DIM><<<grid, BUILD_THREADS, smem, st>>>(coords, N, stride, bits, bitsT);
     CS_LAUNCHED("k_causal_matrix");
     const int64_t covered = (int64_t)nT * (BT / 64);
     if (covered < stride) {
@@ -519,6 +648,7 @@ int launch_causal_matrix(const double *coords, int64_t B, int64_t N, int dim, in
         if (dim == 2) return launch_build_t<CS_GEOM_MINK_CONE, 2>(coords, B, N, stride, bits, bitsT, st);
         if (dim == 3) return launch_build_t<CS_GEOM_MINK_CONE, 3>(coords, B, N, stride, bits, bitsT, st);
         if (dim == 4) return launch_build_t<CS_GEOM_MINK_CONE, 4>(coords, B, N, stride, bits, bitsT, st);
+        if (dim == 5) return launch_build_t<CS_GEOM_MINK_CONE, 5>(coords, B, N, stride, bits, bitsT, st);
         return CS_ERR_DIM;
     case CS_GEOM_DS2_SLAB:
         if (dim != 2) return CS_ERR_DIM;
@@ -526,6 +656,9 @@ int launch_causal_matrix(const double *coords, int64_t B, int64_t N, int dim, in
     case CS_GEOM_FLRW_POLAR:
         if (dim != 6) return CS_ERR_DIM;
         return launch_build_t<CS_GEOM_FLRW_POLAR, 6>(coords, B, N, stride, bits, bitsT, st);
+    case CS_GEOM_DS4_SPHERICAL:
+        if (dim != 7) return CS_ERR_DIM;
+        return launch_build_t<CS_GEOM_DS4_SPHERICAL, 7>(coords, B, N, stride, bits, bitsT, st);
     default:
         return CS_ERR_GEOM;
     }

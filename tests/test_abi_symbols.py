@@ -42,7 +42,7 @@ def test_argument_errors_need_no_gpu(lib):
     assert lib.cs_causal_matrix(None, -1, 2, 0, None, None, None) == -1          # CS_ERR_ARG
     assert lib.cs_causal_matrix(None, 8, 2, 7, None, None, None) == -3           # CS_ERR_GEOM
     assert lib.cs_causal_matrix(None, 8, 3, 0, None, None, None) == -2           # CS_ERR_DIM
-    assert lib.cs_causal_matrix(None, 8, 5, 1, None, None, None) == -2
+    assert lib.cs_causal_matrix(None, 8, 6, 1, None, None, None) == -2           # the flat cone stops at 4+1
     assert lib.cs_causal_matrix(None, 8, 2, 0, None, None, None) == -1           # NULL buffers
     assert lib.cs_causal_matrix(None, 0, 2, 0, None, None, None) == 0            # N = 0 is a no-op
     assert lib.cs_bd_action(None, 3, 10, 4, None, None, None) == -1

@@ -20,6 +20,8 @@ GEOMS = [
     (inp.GEOM_MINK_CONE, 4),
     (inp.GEOM_DS2_SLAB, 2),
     (inp.GEOM_FLRW_POLAR, 6),          # NEXT-4: Eq. 7.7
+    (inp.GEOM_MINK_CONE, 5),           # NEXT-4: 4+1 diamond
+    (inp.GEOM_DS4_SPHERICAL, 7),       # NEXT-4: 3+1 de Sitter, spherical foliation
 ]
 
 
@@ -117,7 +119,7 @@ def _near_null_set(rng, n, dim):
     return np.ascontiguousarray(coords[np.lexsort((coords[:, 1], coords[:, 0]))])
 
 
-@pytest.mark.parametrize("dim", [2, 3, 4])
+@pytest.mark.parametrize("dim", [2, 3, 4, 5])
 @pytest.mark.parametrize("scale", [1.0, 2.0 ** 30, 2.0 ** -30, 2.0 ** 45, 2.0 ** -45, 2.0 ** 600, 2.0 ** -600])
 def test_causal_matrix_prefilter_bands(api, oracle, dim, scale):
     """The single-precision prefilter of the flat cone never decides a pair the fp64 expression would
@@ -182,6 +184,73 @@ def test_causal_matrix_prefilter_ds_slab(api, oracle):
     shuffled = np.ascontiguousarray(coords[rng.permutation(N)])     # not time-sorted: d_eta < 0 pairs
     assert np.array_equal(to_u64(gpu_bits(api, shuffled, inp.GEOM_DS2_SLAB)[0]),
                           oracle.causal_matrix_bits(shuffled, inp.GEOM_DS2_SLAB))
+
+
+def test_causal_matrix_prefilter_ds4_spherical(api, oracle):
+    """The bilinear prefilter of the 3+1 de Sitter predicate (cos omega - cos d eta): partners displaced along a great
+    circle by exactly d eta and one ulp either side of it, equal times, NaN / infinite / non-unit inputs, unsorted input."""
+    rng = np.random.default_rng(31)
+    n = 500
+
+    def pts(eta, psi, th, ph):
+        sp = np.sin(psi)
+        return np.stack([eta, np.cos(eta), np.sin(eta), np.cos(psi), sp * np.cos(th), sp * np.sin(th) * np.cos(ph),
+                         sp * np.sin(th) * np.sin(ph)], axis=1)
+    eta = rng.uniform(0.0, 0.9, n); psi = rng.uniform(0.2, 2.0, n); th = rng.uniform(0.2, 2.9, n); ph = rng.uniform(0, 6.28, n)
+    d = rng.uniform(0.01, 0.4, n)
+    sets = [pts(eta, psi, th, ph)]
+    for k in (0.0, 10.0, -10.0):
+        e2 = eta + d
+        if k:
+            e2 = np.nextafter(e2, k)
+        sets.append(pts(e2, psi + d, th, ph))               # same meridian: omega = d
+    sets.append(pts(eta, psi + 0.3, th, ph))                # equal times: never related
+    coords = np.concatenate(sets)
+    coords = np.ascontiguousarray(coords[np.lexsort((coords[:, 3], coords[:, 0]))])
+    N = coords.shape[0]
+    for variant in range(4):
+        c = coords.copy()
+        if variant == 1:
+            c[5, 3] = np.nan; c[300, 0] = np.inf; c[900, 4] = -np.inf; c[1200:1500] = c[1200]
+        if variant == 2:
+            c[:, 3:] *= 3.0                                 # not unit vectors: still the header's expression
+        if variant == 3:
+            c = np.ascontiguousarray(c[rng.permutation(N)])
+        o_bits = oracle.causal_matrix_bits(c, inp.GEOM_DS4_SPHERICAL)
+        bits, bitsT = gpu_bits(api, c, inp.GEOM_DS4_SPHERICAL)
+        assert np.array_equal(to_u64(bits), o_bits), variant
+        assert np.array_equal(to_u64(bitsT), oracle.transpose_bits(o_bits, N)), variant
+
+
+def test_causal_matrix_prefilter_flrw(api, oracle):
+    """Eq. 7.7's prefilter runs on Cartesian conformal coordinates formed per point; it may only be used when the
+    trigonometric inputs are unit vectors.  Near-null pairs along rays and across them, inputs whose (cos, sin) pairs
+    are NOT normalised (the law-of-cosines value then differs from the Cartesian distance), NaN, unsorted."""
+    rng = np.random.default_rng(41)
+    base = inp.sprinkle_flrw_polar(900, 9)
+    extra = base[:300].copy()
+    extra[:, 0] = base[:300, 0] + 0.0625
+    extra[:, 1] = base[:300, 1] + 0.0625                    # same ray, null separated
+    e2 = extra.copy(); e2[:, 0] = np.nextafter(extra[:, 0], 10.0)
+    e3 = extra.copy(); e3[:, 0] = np.nextafter(extra[:, 0], -10.0)
+    coords = np.concatenate([base, extra, e2, e3])
+    coords = np.ascontiguousarray(coords[np.lexsort((coords[:, 1], coords[:, 0]))])
+    N = coords.shape[0]
+    for variant in range(4):
+        c = coords.copy()
+        if variant == 1:
+            c[::7, 2:4] *= 1.0 + 1e-6                       # cos^2 + sin^2 != 1 on every 7th point
+        if variant == 2:
+            c[:, 4:6] *= 0.5; c[11, 1] = np.nan; c[700, 0] = np.inf
+        if variant == 3:
+            c = np.ascontiguousarray(c[rng.permutation(N)])
+        o_bits = oracle.causal_matrix_bits(c, inp.GEOM_FLRW_POLAR)
+        bits, bitsT = gpu_bits(api, c, inp.GEOM_FLRW_POLAR)
+        assert np.array_equal(to_u64(bits), o_bits), variant
+        assert np.array_equal(to_u64(bitsT), oracle.transpose_bits(o_bits, N)), variant
+    dust = inp.sprinkle_dust_slab(2500, 3)                  # App. A.1.4 through the same predicate
+    assert np.array_equal(to_u64(gpu_bits(api, dust, inp.GEOM_FLRW_POLAR)[0]),
+                          oracle.causal_matrix_bits(dust, inp.GEOM_FLRW_POLAR))
 
 
 def test_causal_matrix_lightcone_ties(api, oracle):
@@ -772,3 +841,28 @@ def test_small_everything(api, oracle):
         <= _smear_tolerance(o_hist, 4, 0.25, oracle.smeared_action(o_hist, N, 4, 0.25))
     h_host, s_host = api.action_host(torch.from_numpy(coords).pin_memory(), cfg.geometry)
     assert np.array_equal(h_host.numpy(), o_hist) and float(s_host[0]) == o_S
+
+
+def test_ds4_spherical_and_cone5_pipelines(api, oracle):
+    """NEXT-4: the 3+1 de Sitter slab (spherical foliation) through the whole path incl. the host entry point (a 3+1
+    dimensional action), and the 4+1 flat diamond up to its histogram (the paper prints no action for d = 5)."""
+    N = 2100
+    c = inp.sprinkle(inp.GEOM_DS4_SPHERICAL, 7, N, 8)
+    o_bits, o_hist, o_S, o_I = oracle.action_pipeline(c, inp.GEOM_DS4_SPHERICAL, tier=1)
+    bits, bitsT = gpu_bits(api, c, inp.GEOM_DS4_SPHERICAL)
+    assert np.array_equal(to_u64(bits), o_bits)
+    hist = api.interval_hist(bits, bitsT, N)
+    assert np.array_equal(hist.cpu().numpy(), o_hist)
+    S, I = api.bd_action(hist, N, 4, return_bracket=True)
+    assert int(I[0]) == o_I and float(S[0]) == o_S
+    h_host, s_host = api.action_host(torch.from_numpy(c).pin_memory(), inp.GEOM_DS4_SPHERICAL)
+    assert np.array_equal(h_host.numpy(), o_hist) and float(s_host[0]) == o_S
+    c5 = inp.sprinkle(inp.GEOM_MINK_CONE, 5, N, 9)
+    o_bits, o_hist, _, _ = oracle.action_pipeline(c5, inp.GEOM_MINK_CONE, tier=1)
+    bits, bitsT = gpu_bits(api, c5, inp.GEOM_MINK_CONE)
+    assert np.array_equal(to_u64(bits), o_bits)
+    assert np.array_equal(api.interval_hist(bits, bitsT, N).cpu().numpy(), o_hist)
+    with pytest.raises(RuntimeError):
+        api.bd_action(hist, N, 5)
+    with pytest.raises(RuntimeError):
+        api.causal_matrix(torch.zeros((10, 6), dtype=torch.float64, device="cuda"), inp.GEOM_DS4_SPHERICAL)
