@@ -223,7 +223,9 @@ int cs_smeared_action(const int64_t *hist, int64_t kmax, int64_t N, int dim, dou
                       double *action, void *stream);
 
 /* Batched ensemble (Monte-Carlo use): B independent causets of N points each,
- * one action per causet.
+ * one action per causet.  The ensemble is built and reduced chunk by chunk (a whole number of causets per CTA
+ * pair of a2's grid, at most 448 MiB of bit matrices at a time), so the workspace does not grow with B beyond
+ * 32 bytes per causet.
  *   coords   device, [B][N][dim] fp64, each causet sorted by time.
  *   actions  device, double[B], overwritten.
  *   hist4    device int64[B][4] or NULL: N_0..N_3 of every causet.
@@ -245,7 +247,7 @@ int cs_action_host(const double *coords_host, int64_t N, int dim, int geometry, 
                    void *workspace, size_t workspace_bytes, void *stream);
 
 /* The ensemble end to end with HOST buffers (the Monte-Carlo use): B causets of N points each,
- * processed in chunks of up to 512 causets; the coordinates of the next chunk are copied on a library-owned
+ * processed in the same chunks as cs_bd_action_batched; the coordinates of the next chunk are copied on a library-owned
  * stream while `stream` builds and reduces the current one, so the PCIe time hides behind the kernels.  Copies the
  * actions (and N_0..N_3 per causet) back and synchronises `stream` before returning.
  *   coords_host   host, [B][N][dim] fp64; pinned memory is needed for the copies to overlap.

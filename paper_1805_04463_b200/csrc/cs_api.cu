@@ -276,13 +276,30 @@ int cs_greedy_antichain(const uint64_t *bits, const uint64_t *bitsT, int64_t N, 
 }
 
 // ---- batched ensemble ----------------------------------------------------------------------
-// workspace: [bits B*N*stride][bitsT B*N*stride][hist B*4 int64][interval scratch]
+// The ensemble is processed in chunks of CB causets: a1 writes the chunk's bit matrices, a2 reduces them to
+// N_0..N_3, and the same buffers take the next chunk, so the workspace holds the matrices of one chunk (at most
+// ENSEMBLE_MAT_BYTES), not of the ensemble (4 GiB for 4096 x 2048).  CB is a whole number of causets per CTA pair
+// of a2's persistent grid (causet-major schedule: every pair then gets the same number of causets).
+// workspace: [bits CB*N*stride][bitsT CB*N*stride][hist B*4 int64][interval scratch]
+constexpr size_t ENSEMBLE_MAT_BYTES = (size_t)448 << 20;     // both matrices of a chunk
+
+static int64_t ensemble_chunk(int64_t B, int64_t N)
+{
+    const size_t per = 2 * (size_t)N * row_stride_words(N) * 8;
+    int64_t cb = per ? (int64_t)(ENSEMBLE_MAT_BYTES / per) : B;
+    const int64_t pairs = sm_count() / 2;
+    if (cb > pairs) cb -= cb % pairs;
+    if (cb < 1) cb = 1;
+    return cb < B ? cb : B;
+}
+
 size_t cs_bd_action_batched_workspace(int64_t B, int64_t N)
 {
     if (B < 0 || N < 0) return 0;
-    const size_t mat = align_up((size_t)B * N * row_stride_words(N) * 8, 256);
+    const int64_t CB = ensemble_chunk(B, N);
+    const size_t mat = align_up((size_t)CB * N * row_stride_words(N) * 8, 256);
     int r = cs_default_route(N);
-    return 2 * mat + align_up((size_t)B * 4 * 8, 256) + interval_ws_bytes(B, N, 1, r);
+    return 2 * mat + align_up((size_t)B * 4 * 8, 256) + interval_ws_bytes(CB, N, 1, r);
 }
 
 int cs_bd_action_batched(const double *coords, int64_t B, int64_t N, int dim, int geometry,
@@ -295,31 +312,32 @@ int cs_bd_action_batched(const double *coords, int64_t B, int64_t N, int dim, in
     if (!workspace || workspace_bytes < cs_bd_action_batched_workspace(B, N) || ((uintptr_t)workspace & 255))
         return CS_ERR_WORKSPACE;
     cudaStream_t st = static_cast<cudaStream_t>(stream);
-    const size_t mat = align_up((size_t)B * N * row_stride_words(N) * 8, 256);
+    const int64_t CB = ensemble_chunk(B, N);
+    const size_t mat = align_up((size_t)CB * N * row_stride_words(N) * 8, 256);
     unsigned char *ws = static_cast<unsigned char *>(workspace);
     uint64_t *bits = reinterpret_cast<uint64_t *>(ws);
     uint64_t *bitsT = reinterpret_cast<uint64_t *>(ws + mat);
     int64_t *hist = reinterpret_cast<int64_t *>(ws + 2 * mat);
     unsigned char *iws = ws + 2 * mat + align_up((size_t)B * 4 * 8, 256);
-    int rc = cs_causal_matrix_batched(coords, B, N, dim, geometry, bits, bitsT, stream);
-    if (rc) return rc;
     const int64_t kmax = clamp_kmax(N, 3);
-    if (kmax < 3) CS_CUDA(cudaMemsetAsync(hist, 0, (size_t)B * 4 * 8, st));
     // hist rows are kmax+1 long; with kmax = 3 that is the [B][4] layout asked for
-    int64_t *hist_k = hist;
-    rc = interval_hist_impl(bits, bitsT, B, N, kmax, 0, N, CS_ROUTE_AUTO, hist_k, nullptr, iws,
-                            workspace_bytes - (size_t)(iws - ws), st);
-    if (rc) return rc;
-    return launch_bd_action(hist_k, kmax + 1, B, kmax, N, spacetime_dim(geometry, dim), actions, nullptr, hist4, st);
+    if (kmax < 3) CS_CUDA(cudaMemsetAsync(hist, 0, (size_t)B * 4 * 8, st));
+    for (int64_t b0 = 0; b0 < B; b0 += CB) {
+        const int64_t nb = B - b0 < CB ? B - b0 : CB;
+        int rc = cs_causal_matrix_batched(coords + b0 * N * dim, nb, N, dim, geometry, bits, bitsT, stream);
+        if (rc) return rc;
+        rc = interval_hist_impl(bits, bitsT, nb, N, kmax, 0, N, CS_ROUTE_AUTO, hist + b0 * (kmax + 1), nullptr, iws,
+                                workspace_bytes - (size_t)(iws - ws), st);
+        if (rc) return rc;
+    }
+    return launch_bd_action(hist, kmax + 1, B, kmax, N, spacetime_dim(geometry, dim), actions, nullptr, hist4, st);
 }
 
 // ---- ensemble end to end with host buffers: chunked, copies overlapped with compute -------------
-// The coordinates of the next chunk of causets travel over PCIe on a library-owned copy stream while the
-// caller's stream builds and reduces the current chunk; two coordinate buffers alternate, the bit matrices
-// exist for one chunk only.
+// The coordinates of the next chunk of causets (ensemble_chunk above) travel over PCIe on a library-owned copy
+// stream while the caller's stream builds and reduces the current chunk; two coordinate buffers alternate, the
+// bit matrices exist for one chunk only.
 // workspace: [coords chunk x2][bits chunk][bitsT chunk][hist CB*4][actions B][hist4 B*4][interval scratch]
-static int64_t ensemble_chunk(int64_t B) { return B < 512 ? B : 512; }
-
 // copy stream and events of the host pipeline, one set per device, created under a lock on first use;
 // a partial failure destroys what was created so that the next call starts over
 struct CopyPipe {
@@ -359,7 +377,7 @@ static int copy_pipe(CopyPipe **out)
 size_t cs_bd_action_batched_host_workspace(int64_t B, int64_t N, int dim)
 {
     if (B < 0 || N < 0 || dim < 2 || dim > 7) return 0;
-    const int64_t CB = ensemble_chunk(B);
+    const int64_t CB = ensemble_chunk(B, N);
     const size_t cbuf = align_up((size_t)CB * N * dim * 8, 256);
     const size_t mat = align_up((size_t)CB * N * row_stride_words(N) * 8, 256);
     return 2 * cbuf + 2 * mat + align_up((size_t)CB * 4 * 8, 256) + align_up((size_t)B * 8, 256) +
@@ -382,7 +400,7 @@ int cs_bd_action_batched_host(const double *coords_host, int64_t B, int64_t N, i
     if (prc) return prc;
     cudaStream_t copy_stream = pipe->stream;
     cudaEvent_t *copied = pipe->copied, *consumed = pipe->consumed, start = pipe->start;
-    const int64_t CB = ensemble_chunk(B);
+    const int64_t CB = ensemble_chunk(B, N);
     const size_t cbuf = align_up((size_t)CB * N * dim * 8, 256);
     const size_t mat = align_up((size_t)CB * N * row_stride_words(N) * 8, 256);
     unsigned char *ws = static_cast<unsigned char *>(workspace);

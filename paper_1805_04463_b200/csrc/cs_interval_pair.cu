@@ -12,13 +12,19 @@
 //  * expansion without shifts: with x a 32-bit slice of a bit row, x & 0x11111111, x & 0x22222222 and
 //    x & 0x44444444 are already E2M1 nibbles (0.5, 1.0, 2.0 where the bit is set); only bit 3 of
 //    every nibble needs a shift ((x >> 3) & 0x11111111).  Each K=64 MMA takes one nibble position
-//    of eight slices, so its products are all 0.25, 1 or 4 -- undone exactly by constant UE8M0
-//    block scales 2^1, 2^0, 2^-1 kept in three TMEM regions.  k is permuted inside a 256-k stage,
+//    of eight slices, so its products are all 0.25, 1 or 4 -- levelled exactly by constant UE8M0
+//    block scales kept in three TMEM regions.  k is permuted inside a 256-k stage,
 //    identically for both operands, which leaves the contraction unchanged.
+//  * the scales are 2^-72, 2^-73, 2^-74 (not 2^1, 2^0, 2^-1): every product is then 2^-146 = eight
+//    units in the last place of a SUBNORMAL fp32, and subnormals add like integers, so the bit pattern of
+//    the accumulator is the integer 8 * count -- no float-to-integer step in the epilogue (the tally of the
+//    ensemble case shifts by it directly: 2 instead of 4 instructions per pair).  Exact while
+//    8 * count < 2^24 (the fp32 grid stays 2^-149 up to there): count < 2^21.  Measured: the tensor cores
+//    accumulate subnormals without flushing; every a2 parity test runs on this path.
 //  * tiles are visited in a table order (longest K first in bands of 8 diagonals, I-major inside
 //    a band) so that the ~74 tiles in flight share a few row panels in L2.
 //
-// Products are 0 or 1 and the fp32 accumulators are exact for counts < 2^24.
+// Products are 0 or 2^-146 and the fp32 accumulators are exact for counts < 2^21.
 #include <cuda.h>
 
 #include <type_traits>
@@ -247,7 +253,7 @@ __device__ __forceinline__ uint32_t nib(uint32_t x)
     if (Q == 1) return x & 0x22222222u;
     return x & 0x44444444u;
 }
-// UE8M0 block scale that turns the products of nibble position q into exactly 1: 2^1, 2^0, 2^-1, 2^1
+// TMEM region of the UE8M0 block scale that levels the products of nibble position q (0.25, 1, 4, 0.25)
 __device__ __forceinline__ uint32_t sf_col(int q) { return SF_COL + (q == 1 ? 16u : q == 2 ? 32u : 0u); }
 
 // ---- tile order ---------------------------------------------------------------------------------
@@ -485,9 +491,9 @@ k_interval_pair(const __grid_constant__ CUtensorMap mapU, const __grid_constant_
     const uint32_t tmem_base = *s_tmem;
     if (warp < 4) {           // constant UE8M0 block scales: 2^1, 2^0, 2^-1 in every byte of their region
         const uint32_t sf = tmem_base + ((uint32_t)(warp * 32) << 16) + SF_COL;
-        tmem_st16_const(sf, 0x80808080u);
-        tmem_st16_const(sf + 16, 0x7F7F7F7Fu);
-        tmem_st16_const(sf + 32, 0x7E7E7E7Eu);
+        tmem_st16_const(sf, 0x37373737u);          // 2^-72, 2^-73, 2^-74 on both operands
+        tmem_st16_const(sf + 16, 0x36363636u);
+        tmem_st16_const(sf + 32, 0x35353535u);
     }
     tc_fence_before();
     __syncthreads();
@@ -701,8 +707,7 @@ k_interval_pair(const __grid_constant__ CUtensorMap mapU, const __grid_constant_
         int cur_batch = -1;
         const int quarter = warp & 3, colhalf = warp >> 2;   // TMEM lane quarter; which CW = TN/2 columns
         const uint32_t taddr0 = tmem_base + ((uint32_t)(quarter * 32) << 16) + colhalf * CW;
-        // Counts are exact small integers held as fp32: adding 2^23 leaves the count in the low mantissa
-        // bits (one FADD, no F2I), and comparisons are taken on the float itself.
+        // The accumulator's bit pattern is 8 * count (subnormal fp32, see the header).
         const uint32_t kmax32 = (uint32_t)kmax;
         uint32_t small[4] = {0, 0, 0, 0};                    // SMALL: this thread's tallies of counts 0..3
         auto flush_small = [&](int batch) {                  // one warp reduction, <= 4 global atomics per warp
@@ -772,11 +777,10 @@ k_interval_pair(const __grid_constant__ CUtensorMap mapU, const __grid_constant_
                     if (!__any_sync(0xffffffffu, relw != 0)) continue;
 #pragma unroll
                     for (int c = 0; c < 32; c++) {
-                        const float f = __uint_as_float(v[w * 32 + c]);
-                        const uint32_t ub = __float_as_uint(f + 8388608.0f);        // 0x4B000000 + count
+                        const uint32_t raw = v[w * 32 + c];                         // 8 count (see the block scales)
                         if (SMALL) {
                             // inc = 1 << 8 count; shl.b32 clamps the shift amount, so counts >= 4 give 0.
-                            // FADD, LEA, SHF, R2P (7 columns at once), SEL, 1/2 IADD3 per column.
+                            // SHF, predicated IADD, and one R2P per 7 columns.
                             uint32_t &acc = (c & 1) ? acc1 : acc0;
                             asm("{\n"
                                 ".reg .pred r;\n"
@@ -785,9 +789,9 @@ k_interval_pair(const __grid_constant__ CUtensorMap mapU, const __grid_constant_
                                 "setp.ne.u32 r, t, 0;\n"
                                 "shl.b32 i, 1, %3;\n"
                                 "@r add.u32 %0, %0, i;\n"
-                                "}\n" : "+r"(acc) : "r"(relw), "r"(1u << c), "r"((ub - 0x4B000000u) * 8u));
+                                "}\n" : "+r"(acc) : "r"(relw), "r"(1u << c), "r"(raw));
                         } else if (relw & (1u << c)) {
-                            const uint32_t cnt = ub - 0x4B000000u;
+                            const uint32_t cnt = raw >> 3;
                             if (!BIG || cnt < (uint32_t)hs) atomicAdd(&s_hist[cnt], 1u);
                             else if (cnt <= kmax32) atomicAdd(&ghist[cnt], 1ULL);
                         }
@@ -911,7 +915,7 @@ int launch_interval_pair(const uint64_t *bits, const uint64_t *bitsT, int64_t B,
                          int64_t row_begin, int64_t row_end, int64_t *hist, int64_t *nrel,
                          void *scratch, size_t scratch_bytes, IntervalStats *stats, cudaStream_t st)
 {
-    if (N > ((int64_t)1 << 22)) return CS_ERR_ARG;   // counts must stay exact in fp32; tile ids are 16 bits
+    if (N > ((int64_t)1 << 21)) return CS_ERR_ARG;   // 8 * count must stay below 2^24; tile ids are 16 bits
     constexpr int TN = PAIR_TN;
     static_assert(PAIR_TN == TILE, "the tile table lists square tiles");
     const int64_t tiles_per = pair_tiles_per_causet(N);
