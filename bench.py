@@ -235,7 +235,7 @@ def run_peaks(args, local_rank):
     api.load()
     ws = torch.empty((1 << 30) + 65536, dtype=torch.uint8, device="cuda")
     iters = {"mxf4_pair": 1 << 16, "i8": 1 << 16, "popc": 2048, "dfma": 2048, "ffma": 8192, "ffma2": 8192,
-             "hbm_write": 4, "hbm_copy": 4, "tmem_ld4": 1 << 14, "tmem_ld8": 1 << 14}
+             "hbm_write": 4, "hbm_copy": 4, "tmem_ld4": 1 << 14, "tmem_ld8": 1 << 14, "mxf4_pair_n128": 1 << 16, "mxf4_pair_n128_dep": 1 << 16}
     out = {}
     sampler = ClockSampler(local_rank); sampler.start()
     t0 = time.perf_counter()

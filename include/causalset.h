@@ -280,7 +280,9 @@ enum cs_peak_kind {
     CS_PEAK_HBM_WRITE = 6,  /* 128-bit stores */
     CS_PEAK_HBM_COPY = 7,   /* 128-bit loads + stores */
     CS_PEAK_TMEM_LD4 = 8,   /* tcgen05.ld 32x32b.x32, one warp per TMEM lane quarter */
-    CS_PEAK_TMEM_LD8 = 9    /* the same from two warps per lane quarter */
+    CS_PEAK_TMEM_LD8 = 9,   /* the same from two warps per lane quarter */
+    CS_PEAK_MXF4_PAIR_N128 = 10, /* MXF4_PAIR with N = 128, alternating between two 128-column accumulator halves */
+    CS_PEAK_MXF4_PAIR_N128_DEP = 11 /* MXF4_PAIR with N = 128, all into one half: a chain of dependent accumulations */
 };
 int cs_peak_probe(int kind, int64_t iters, void *workspace, size_t workspace_bytes, double *out_host, void *stream);
 

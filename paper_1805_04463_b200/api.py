@@ -128,7 +128,7 @@ def default_route(N: int) -> int:
 
 
 PEAK_KINDS = {"mxf4_pair": 0, "i8": 1, "popc": 2, "dfma": 3, "ffma": 4, "ffma2": 5, "hbm_write": 6, "hbm_copy": 7,
-              "tmem_ld4": 8, "tmem_ld8": 9}
+              "tmem_ld4": 8, "tmem_ld8": 9, "mxf4_pair_n128": 10, "mxf4_pair_n128_dep": 11}
 
 
 def peak_probe(kind: str, iters: int, workspace: torch.Tensor):

@@ -11,6 +11,8 @@
 //   FFMA       fp32 FFMA                            FFMA2  fma.rn.f32x2 (the packed prefilter of a1)
 //   HBM_WRITE  128-bit stores over the workspace    HBM_COPY  128-bit loads + stores
 //   TMEM_LD    tcgen05.ld 32x32b.x32 from 4 or 8 warps of a CTA (the epilogue's accumulator drain)
+//   MXF4_PAIR_N128  the MXF4_PAIR instruction with N = 128, alternating between two accumulator halves
+//   MXF4_PAIR_N128_DEP  the same, every MMA accumulating into the same half (a dependent chain)
 #include <vector>
 
 #include "cs_common.cuh"
@@ -87,11 +89,18 @@ __device__ __forceinline__ void tmem_st16_const(uint32_t taddr, uint32_t val)
 constexpr int MMA_GROUP = 32;          // MMAs between two commits; two groups are in flight at most
 
 // ---- kind::mxf4 on CTA pairs ----------------------------------------------------------------------
-constexpr uint32_t MXF4_IDESC = (1u << 7) | (1u << 10) | ((uint32_t)(256 >> 3) << 17) | (1u << 23) | ((uint32_t)(256 >> 4) << 24);
+__host__ __device__ constexpr uint32_t mxf4_idesc(int n)
+{
+    return (1u << 7) | (1u << 10) | ((uint32_t)(n >> 3) << 17) | (1u << 23) | ((uint32_t)(256 >> 4) << 24);
+}
 
+// NCOLS = 256: the MMA of k_interval_pair.  NCOLS = 128: the same with half the columns, alternating between two
+// accumulator halves (independent chains) -- the shape a split accumulator would need.
+template <int NCOLS, bool ALTERNATE>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(128, 1)
 k_probe_mxf4_pair(int groups, unsigned long long *__restrict__ clk)
 {
+    constexpr uint32_t MXF4_IDESC = mxf4_idesc(NCOLS);
     __shared__ __align__(1024) unsigned char s_b[4096];   // this CTA's half of B: 128 rows x K = 64 E2M1
     __shared__ uint64_t s_bar[2];
     __shared__ uint32_t s_tmem;
@@ -121,7 +130,7 @@ k_probe_mxf4_pair(int groups, unsigned long long *__restrict__ clk)
     cluster_sync();
     tc_fence_after();
     if (warp == 0 && rank == 0) {
-        const uint64_t bd = make_desc(smem_u32(s_b), 128 * 16, 128);
+        const uint64_t bd = make_desc(smem_u32(s_b), (NCOLS / 2) * 16, 128);
         unsigned long long t0 = 0;
         for (int g = 0; g < groups; g++) {
             if (g >= 2) mbar_wait(&s_bar[g & 1], ((g >> 1) - 1) & 1);     // group g-2 has retired
@@ -129,13 +138,14 @@ k_probe_mxf4_pair(int groups, unsigned long long *__restrict__ clk)
             if (elect_one()) {
 #pragma unroll 4
                 for (int i = 0; i < MMA_GROUP; i++) {
+                    const uint32_t d = tmem + (ALTERNATE ? (uint32_t)(i & 1) * 128u : 0u);
                     asm volatile(
                         "{\n"
                         ".reg .pred p;\n"
                         "setp.ne.b32 p, %4, 0;\n"
                         "tcgen05.mma.cta_group::2.kind::mxf4.block_scale.block32 [%0], [%1], %2, %3, [%5], [%5], p;\n"
-                        "}\n" ::"r"(tmem),
-                        "r"(tmem + 320), "l"(bd), "r"(MXF4_IDESC), "r"((uint32_t)((g | i) != 0)), "r"(tmem + 256)
+                        "}\n" ::"r"(d),
+                        "r"(tmem + 320), "l"(bd), "r"(MXF4_IDESC), "r"((uint32_t)((g | (i >> 1)) != 0)), "r"(tmem + 256)
                         : "memory");
                 }
                 asm volatile(
@@ -384,11 +394,16 @@ int launch_peak_probe(int kind, int64_t iters, void *workspace, size_t workspace
     int rc = CS_OK;
     auto launch = [&]() -> int {
         switch (kind) {
-        case CS_PEAK_MXF4_PAIR: {
+        case CS_PEAK_MXF4_PAIR:
+        case CS_PEAK_MXF4_PAIR_N128:
+        case CS_PEAK_MXF4_PAIR_N128_DEP: {
             const int groups = (int)((iters + MMA_GROUP - 1) / MMA_GROUP) + 2;
-            k_probe_mxf4_pair<<<sms / 2 * 2, 128, 0, st>>>(groups, clk);
-            units = 2.0 * 256 * 256 * 64 * MMA_GROUP * (double)groups * (sms / 2);
-            per_clk_units = 2.0 * 256 * 256 * 64 * MMA_GROUP * (double)(groups - 2);
+            const double ncols = kind == CS_PEAK_MXF4_PAIR ? 256.0 : 128.0;
+            if (kind == CS_PEAK_MXF4_PAIR) k_probe_mxf4_pair<256, false><<<sms / 2 * 2, 128, 0, st>>>(groups, clk);
+            else if (kind == CS_PEAK_MXF4_PAIR_N128) k_probe_mxf4_pair<128, true><<<sms / 2 * 2, 128, 0, st>>>(groups, clk);
+            else k_probe_mxf4_pair<128, false><<<sms / 2 * 2, 128, 0, st>>>(groups, clk);
+            units = 2.0 * 256 * ncols * 64 * MMA_GROUP * (double)groups * (sms / 2);
+            per_clk_units = 2.0 * 256 * ncols * 64 * MMA_GROUP * (double)(groups - 2);
             nclk = sms / 2; sms_per_clk = 2;
             break;
         }
