@@ -42,23 +42,15 @@ constexpr int NS = 6;                   // operand stages (B in shared memory, A
 constexpr int GK = 2;                   // stages per staged group of bit rows
 constexpr int BROW = GK * 32;           // bytes per staged bit row (TMA box inner extent, 64B swizzle)
 constexpr int NB = 4;                   // bit-row buffers
-// Tile width TN (columns j of a tile): 256, one accumulator, or 128, two accumulators that ping-pong
-// so that the epilogue drains one (TMEM reads run at 64 B/clk: 2048 clk for 128 lanes x 256 columns)
-// while the MMAs of the next tile fill the other.  TN = 128 expands every A stage for half the MMA work,
-// which only pays when tiles are short (small N, batched ensembles).
-template <int TN>
-struct Shape {
-    static constexpr int TNH = TN / 2;                          // B rows (j) per CTA
-    static constexpr int NACC = 256 / TN;                       // accumulators of TN columns
-    static constexpr int CW = TN / 2;                           // columns drained per epilogue warp
-    static constexpr int BITS_BYTES = (TM + TNH) * BROW;        // staged bit rows per buffer
-    static constexpr int STAGE_BYTES = TNH * (KSTEP / 2);       // this CTA's half of B, one stage
-    static constexpr int SMEM_FIXED = NS * STAGE_BYTES + NB * BITS_BYTES + 512;      // + 4 bytes per histogram bin
-    // block-scaled instruction descriptor, kind::mxf4: A = B = E2M1 (1 at bits 7 and 10), both K-major,
-    // N >> 3 at bit 17, scale format UE8M0 (bit 23), M >> 4 at bit 24 (M = 256 over the pair), K = 64
-    static constexpr uint32_t IDESC =
-        (1u << 7) | (1u << 10) | ((uint32_t)(TN >> 3) << 17) | (1u << 23) | ((uint32_t)(256 >> 4) << 24);
-};
+constexpr int TN = 256;                 // columns (j) of a tile: one 256-column fp32 accumulator
+constexpr int TNH = TN / 2;             // B rows (j) per CTA (cta_group::2 splits N over the pair)
+constexpr int CW = TN / 2;              // columns drained per epilogue warp
+constexpr int BITS_BYTES = (TM + TNH) * BROW;        // staged bit rows per buffer
+constexpr int STAGE_BYTES = TNH * (KSTEP / 2);       // this CTA's half of B, one stage
+constexpr int SMEM_FIXED = NS * STAGE_BYTES + NB * BITS_BYTES + 512;      // + 4 bytes per histogram bin
+// block-scaled instruction descriptor, kind::mxf4: A = B = E2M1 (1 at bits 7 and 10), both K-major,
+// N >> 3 at bit 17, scale format UE8M0 (bit 23), M >> 4 at bit 24 (M = 256 over the pair), K = 64
+constexpr uint32_t IDESC = (1u << 7) | (1u << 10) | ((uint32_t)(TN >> 3) << 17) | (1u << 23) | ((uint32_t)(256 >> 4) << 24);
 constexpr int HS_MAX = 16896;           // shared-memory histogram bins that fit beside the operand rings
 constexpr int HS_BATCHED = 2048;        // bins when several causets share a CTA (flushed at every switch)
 constexpr int BANDW = 8;                // diagonals (in 256-column units) per band of the tile order
@@ -68,7 +60,7 @@ constexpr int BANDW = 8;                // diagonals (in 256-column units) per b
 // row slice (128 columns) in registers, so registers are re-split by warpgroup with setmaxnreg.
 constexpr int EPI_WARPS = 8, EXPA_WARP0 = 8, EXPB_WARP0 = 12, EXP_WARPS = 8, MMA_WARP = 16, LOAD_WARP = 17;
 constexpr int THREADS = 20 * 32;
-constexpr int SMEM_BYTES = Shape<256>::SMEM_FIXED + HS_MAX * 4;
+constexpr int SMEM_BYTES = SMEM_FIXED + HS_MAX * 4;
 constexpr uint32_t SF_COL = 256;        // three 16-column regions of constant scale factors: 2^1, 2^0, 2^-1
 constexpr uint32_t A_COL = 320;         // TMEM ring of the A operand: NS x 32 columns
 static_assert(A_COL + NS * 32 <= 512, "TMEM columns");
@@ -390,7 +382,7 @@ __device__ __forceinline__ void for_each_group(const Tile &tc, F f)
 
 // SMALL: kmax <= 3 (the Monte-Carlo case, only N_0..N_3 enter Eq. 4.10-4.12): the tally keeps packed
 // counters in registers and never touches the shared histogram (hs = 0).
-template <bool SMALL, int TN>
+template <bool SMALL>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(THREADS, 1)
 k_interval_pair(const __grid_constant__ CUtensorMap mapU, const __grid_constant__ CUtensorMap mapL,
                 const uint64_t *__restrict__ bits, const uint32_t *__restrict__ tile_tab,
@@ -403,14 +395,11 @@ k_interval_pair(const __grid_constant__ CUtensorMap mapU, const __grid_constant_
 {
     extern __shared__ __align__(1024) unsigned char smem[];
     unsigned char *s_stage = smem;
-    using SH = Shape<TN>;
-    constexpr int TNH = SH::TNH, NACC = SH::NACC, CW = SH::CW;
-    constexpr int BITS_BYTES = SH::BITS_BYTES, STAGE_BYTES = SH::STAGE_BYTES, SMEM_FIXED = SH::SMEM_FIXED;
     unsigned char *s_bits = smem + NS * STAGE_BYTES;
     uint64_t *s_full = reinterpret_cast<uint64_t *>(smem + NS * STAGE_BYTES + NB * BITS_BYTES);
     uint64_t *s_empty = s_full + NS;      // [NS] stage free again (multicast commit from CTA 0)
-    uint64_t *s_tfull = s_empty + NS;     // [2] accumulator complete (multicast commit)
-    uint64_t *s_tempty = s_tfull + 2;     // [2] accumulator drained (used in CTA 0 only)
+    uint64_t *s_tfull = s_empty + NS;     // [1 of 2 slots] accumulator complete (multicast commit)
+    uint64_t *s_tempty = s_tfull + 2;     // [1 of 2 slots] accumulator drained (used in CTA 0 only)
     uint64_t *s_bfull = s_tempty + 2;     // [NB] staged bit rows have landed
     uint64_t *s_bempty = s_bfull + NB;    // [NB] every expander warp is done with the buffer
     uint32_t *s_tmem = reinterpret_cast<uint32_t *>(s_bempty + NB);
@@ -509,12 +498,8 @@ k_interval_pair(const __grid_constant__ CUtensorMap mapU, const __grid_constant_
         // ===================================== expanders =====================================
         // warpgroup 2 owns this CTA's 128 A rows (row = TMEM lane: warp w may only touch lanes
         // 32 (w % 4) ..), warpgroup 3 its 128 B rows.  One thread per row.
-        // With TN = 128 a CTA has only 64 B rows: two threads share a row, thread half h expanding the
-        // 16-byte chunks h (first stage of a group) and 2 + h (second stage).
         const bool isA = warp < EXPB_WARP0;
-        const int r128 = (warp & 3) * 32 + lane;
-        const int r = isA ? r128 : (r128 & (TNH - 1));
-        const int bhalf = r128 / TNH;                     // 0 unless TNH = 64
+        const int r = (warp & 3) * 32 + lane;
         // TMA 64B swizzle: 16-byte chunk c of row e sits at chunk c ^ ((e >> 1) & 3)
         const unsigned char *my_bits = s_bits + (isA ? 0 : TM * BROW) + r * BROW;
         const int swz = (r >> 1) & 3;
@@ -560,22 +545,6 @@ k_interval_pair(const __grid_constant__ CUtensorMap mapU, const __grid_constant_
             publish(s);
             if (++s == NS) { s = 0; ph ^= 1; }
         };
-        // one thread, half a row: chunk c = slices 4 h .. 4 h + 3 of the stage -> 16-byte chunks 2 q + h
-        auto stage_B_half = [&](const uint4 &c) {
-            const uint32_t xs[4] = {c.x, c.y, c.z, c.w};
-            uint4 w[4];
-            w[0] = make_uint4(nib<0>(xs[0]), nib<0>(xs[1]), nib<0>(xs[2]), nib<0>(xs[3]));
-            w[1] = make_uint4(nib<1>(xs[0]), nib<1>(xs[1]), nib<1>(xs[2]), nib<1>(xs[3]));
-            w[2] = make_uint4(nib<2>(xs[0]), nib<2>(xs[1]), nib<2>(xs[2]), nib<2>(xs[3]));
-            w[3] = make_uint4(nib3(xs[0]), nib3(xs[1]), nib3(xs[2]), nib3(xs[3]));
-            mbar_wait(&s_empty[s], ph ^ 1);
-            unsigned char *dst = b_dst + s * STAGE_BYTES + bhalf * TNH * 16;
-#pragma unroll
-            for (int q = 0; q < 4; q++)
-                *reinterpret_cast<uint4 *>(dst + 2 * q * TNH * 16) = w[q];
-            publish(s);
-            if (++s == NS) { s = 0; ph ^= 1; }
-        };
         auto stage_B = [&](const uint4 &c0, const uint4 &c1) {
             const uint32_t xs[8] = {c0.x, c0.y, c0.z, c0.w, c1.x, c1.y, c1.z, c1.w};
             uint4 w[8];       // 16-byte chunk 2 q + h of this row = nibble position q of slices 4 h .. 4 h + 3
@@ -604,9 +573,6 @@ k_interval_pair(const __grid_constant__ CUtensorMap mapU, const __grid_constant_
                 if (isA) {
                     if (first) stage_A(*reinterpret_cast<const uint4 *>(src + off0), *reinterpret_cast<const uint4 *>(src + off1));
                     if (second) stage_A(*reinterpret_cast<const uint4 *>(src + off2), *reinterpret_cast<const uint4 *>(src + off3));
-                } else if (TNH == 64) {
-                    if (first) stage_B_half(*reinterpret_cast<const uint4 *>(src + (bhalf ? off1 : off0)));
-                    if (second) stage_B_half(*reinterpret_cast<const uint4 *>(src + (bhalf ? off3 : off2)));
                 } else {
                     if (first) stage_B(*reinterpret_cast<const uint4 *>(src + off0), *reinterpret_cast<const uint4 *>(src + off1));
                     if (second) stage_B(*reinterpret_cast<const uint4 *>(src + off2), *reinterpret_cast<const uint4 *>(src + off3));
@@ -656,10 +622,9 @@ k_interval_pair(const __grid_constant__ CUtensorMap mapU, const __grid_constant_
             for (Sched sc = sched_first(); sc.b < (uint32_t)B; sched_next(sc)) {
                 const Tile tc = get_tile(sc);
                 if (tc.skip) continue;
-                const uint32_t acc = tile_seq % NACC, use = tile_seq / NACC;     // accumulator and how often it was used
-                mbar_wait_cluster(&s_tempty[acc], (use & 1) ^ 1);         // both epilogues have drained this accumulator
+                mbar_wait_cluster(&s_tempty[0], (tile_seq & 1) ^ 1);      // both epilogues have drained the accumulator
                 tc_fence_after();
-                const uint32_t d_tmem = tmem_base + acc * TN;
+                const uint32_t d_tmem = tmem_base;
                 uint32_t accum = 0;                                       // the first stage that runs overwrites
                 auto issue_stage = [&]() {
                     mbar_wait_cluster(&s_full[s], ph);
@@ -668,10 +633,10 @@ k_interval_pair(const __grid_constant__ CUtensorMap mapU, const __grid_constant_
                         const uint64_t bd = bdesc0 + (uint64_t)((s * STAGE_BYTES) >> 4);
                         const uint32_t at = a_tmem0 + s * 32;
                         // K = 64 per MMA: 8 TMEM columns of A, 2 chunks of B
-                        mma_mxf4_pair(d_tmem, at, bd, SH::IDESC, accum, sf0, sf0);
-                        mma_mxf4_pair(d_tmem, at + 8, bd + ((2 * TNH * 16) >> 4), SH::IDESC, 1u, sf1, sf1);
-                        mma_mxf4_pair(d_tmem, at + 16, bd + ((4 * TNH * 16) >> 4), SH::IDESC, 1u, sf2, sf2);
-                        mma_mxf4_pair(d_tmem, at + 24, bd + ((6 * TNH * 16) >> 4), SH::IDESC, 1u, sf0, sf0);
+                        mma_mxf4_pair(d_tmem, at, bd, IDESC, accum, sf0, sf0);
+                        mma_mxf4_pair(d_tmem, at + 8, bd + ((2 * TNH * 16) >> 4), IDESC, 1u, sf1, sf1);
+                        mma_mxf4_pair(d_tmem, at + 16, bd + ((4 * TNH * 16) >> 4), IDESC, 1u, sf2, sf2);
+                        mma_mxf4_pair(d_tmem, at + 24, bd + ((6 * TNH * 16) >> 4), IDESC, 1u, sf0, sf0);
                         mma_commit_pair(&s_empty[s]);                     // stage s free in both CTAs once these MMAs retire
                     }
                     __syncwarp();
@@ -683,7 +648,7 @@ k_interval_pair(const __grid_constant__ CUtensorMap mapU, const __grid_constant_
                     if (first) issue_stage();
                     if (second) issue_stage();
                 });
-                if (elect_one()) mma_commit_pair(&s_tfull[acc]);          // accumulator complete, both CTAs
+                if (elect_one()) mma_commit_pair(&s_tfull[0]);            // accumulator complete, both CTAs
                 __syncwarp();
                 tile_seq++;
             }
@@ -750,16 +715,15 @@ k_interval_pair(const __grid_constant__ CUtensorMap mapU, const __grid_constant_
             }
             unsigned long long *ghist = hist + (int64_t)cur_batch * hist_len;
             uint32_t v[CW];
-            const uint32_t acc = tile_seq % NACC, use = tile_seq / NACC;
-            const uint32_t taddr = taddr0 + acc * TN;
-            mbar_wait(&s_tfull[acc], use & 1);
+            const uint32_t taddr = taddr0;
+            mbar_wait(&s_tfull[0], tile_seq & 1);
             tc_fence_after();
 #pragma unroll
             for (int c = 0; c < CW / 32; c++) tmem_ld32(taddr + c * 32, &v[c * 32]);
             asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
             tc_fence_before();
             __syncwarp();
-            if (lane == 0) mbar_arrive_cluster(&s_tempty[acc], 0);   // one arrival per warp, in CTA 0
+            if (lane == 0) mbar_arrive_cluster(&s_tempty[0], 0);     // one arrival per warp, in CTA 0
             tile_seq++;
             my_nrel += __popcll(rel[0]) + __popcll(rel[1]);
             // Tally over the 128 columns in registers; 32 columns at a time are skipped when no lane of
@@ -875,19 +839,20 @@ static int pair_bits_map(CUtensorMap *map, const uint64_t *base, int64_t B, int6
     return CS_OK;
 }
 
-// Only TN = 256 is instantiated.  TN = 128 (two ping-pong accumulators, so that the 2048-clk drain of one
-// overlaps the MMAs into the other) was built and measured: bit-exact, but slower at every size (N = 32768:
-// 2.80 vs 1.48 ms; 1024 x N = 2048: 1.69 vs 1.11 ms) -- it expands every A stage for half the MMA work, and
-// the A stores into TMEM and the B stores into shared memory are what the tensor pipe waits for.
-constexpr int PAIR_TN = 256;
-
+// One 256-column accumulator per tile.  Measured alternatives that were dropped: 128-column
+// tiles with two ping-pong accumulators (round 1: every A stage expanded for half the MMA work, slower at every
+// size); the 256-column tile issued as two independently committed 128-column halves, the right half trailing the
+// left by 1-4 stages so that one half drains while the other's MMAs run (round 2, three issuer designs, all bit-exact:
+// N = 128 MMAs do run at the pipe's full rate, but holding every operand stage for the trailing half shortens the
+// expanders' run-ahead and the tile is not bound by the hand-over chain but by the expanders: 10.3-10.7 ms against
+// 9.8 ms at N = 65536, 0.83 against 0.80 ms per 1024 causets of N = 2048).
 size_t interval_pair_scratch_bytes(int64_t N)
 {
     const int64_t nT = (N + TILE - 1) / TILE;
     return align_up((size_t)pair_tiles_per_causet(N) * sizeof(uint32_t), 256) + 2 * align_up((size_t)nT * SKIPM, 256) + 256;
 }
 
-template <bool SMALL, int TN>
+template <bool SMALL>
 static int launch_pair_t(const CUtensorMap &mapU, const CUtensorMap &mapL, const uint64_t *bits, const uint32_t *tab,
                          const uint8_t *flagU, const uint8_t *flagT, const unsigned int *n_empty, int nT, uint32_t tiles_per, int64_t clusters, int64_t B, int64_t N, int64_t stride, int64_t kmax, int hs,
                          int64_t row_begin, int64_t row_end, int64_t *hist, int64_t *nrel,
@@ -896,14 +861,14 @@ static int launch_pair_t(const CUtensorMap &mapU, const CUtensorMap &mapL, const
     static PerDeviceFlag attr_set;
     const int dev = current_device();
     if (!attr_set.get(dev)) {
-        CS_CUDA(cudaFuncSetAttribute(k_interval_pair<SMALL, TN>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                     Shape<TN>::SMEM_FIXED + (SMALL ? 0 : HS_MAX * 4)));
+        CS_CUDA(cudaFuncSetAttribute(k_interval_pair<SMALL>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                     SMEM_FIXED + (SMALL ? 0 : HS_MAX * 4)));
         attr_set.set(dev);
     }
     // whole causets per cluster only if the last round of causets leaves at most 5 % of the clusters idle
     const int64_t rounds = (B + clusters - 1) / clusters;
     const int causet_major = (B > 1 && rounds * clusters * 20 <= B * 21) ? 1 : 0;
-    k_interval_pair<SMALL, TN><<<(unsigned)(2 * clusters), THREADS, Shape<TN>::SMEM_FIXED + hs * 4, st>>>(
+    k_interval_pair<SMALL><<<(unsigned)(2 * clusters), THREADS, SMEM_FIXED + hs * 4, st>>>(
         mapU, mapL, bits, tab, flagU, flagT, n_empty, nT, tiles_per, B, N, stride, kmax, hs, causet_major, row_begin, row_end,
         reinterpret_cast<unsigned long long *>(hist), reinterpret_cast<unsigned long long *>(nrel),
         stats, stages_total, blocks_examined);
@@ -916,8 +881,7 @@ int launch_interval_pair(const uint64_t *bits, const uint64_t *bitsT, int64_t B,
                          void *scratch, size_t scratch_bytes, IntervalStats *stats, cudaStream_t st)
 {
     if (N > ((int64_t)1 << 21)) return CS_ERR_ARG;   // 8 * count must stay below 2^24; tile ids are 16 bits
-    constexpr int TN = PAIR_TN;
-    static_assert(PAIR_TN == TILE, "the tile table lists square tiles");
+    static_assert(TN == TILE, "the tile table lists square tiles");
     const int64_t tiles_per = pair_tiles_per_causet(N);
     if (B > 0 && tiles_per > (((int64_t)1 << 31) - 1) / B) return CS_ERR_ARG;   // 32-bit tile schedule
     if (!scratch || scratch_bytes < interval_pair_scratch_bytes(N)) return CS_ERR_WORKSPACE;
@@ -957,9 +921,9 @@ int launch_interval_pair(const uint64_t *bits, const uint64_t *bitsT, int64_t B,
     const bool small = kmax <= 3;
     const int64_t hs_cap = B > 1 ? HS_BATCHED : HS_MAX;
     const int hs = small ? 0 : (int)(kmax + 1 < hs_cap ? kmax + 1 : hs_cap);
-#define CS_PAIR_LAUNCH(S, T) \
-    launch_pair_t<S, T>(mapU, mapL, bits, tab, flagU, flagT, n_empty, nT, (uint32_t)tiles_per, clusters, B, N, stride, kmax, hs, row_begin, row_end, hist, nrel, stats, stages_total, blocks_examined, st)
-    return small ? CS_PAIR_LAUNCH(true, PAIR_TN) : CS_PAIR_LAUNCH(false, PAIR_TN);
+#define CS_PAIR_LAUNCH(S) \
+    launch_pair_t<S>(mapU, mapL, bits, tab, flagU, flagT, n_empty, nT, (uint32_t)tiles_per, clusters, B, N, stride, kmax, hs, row_begin, row_end, hist, nrel, stats, stages_total, blocks_examined, st)
+    return small ? CS_PAIR_LAUNCH(true) : CS_PAIR_LAUNCH(false);
 #undef CS_PAIR_LAUNCH
 }
 
