@@ -197,6 +197,70 @@ def sprinkle_dust_slab(N: int, seed: int, tau0: float = 1.0, r0: float = 0.5) ->
     return _sort_rows(c, eta, rad)
 
 
+def sprinkle_ds4_flat_slab(N: int, seed: int, eta0: float = -0.25, r0: float = 0.6) -> np.ndarray:
+    """3+1 de Sitter slab, flat foliation ("3+1 Dimensional Slab (Flat Foliation)"), conformal time
+    eta in [-1, eta0]: eta* = [u (1 + eta0^-3) - 1]^(-1/3), r* = u^(1/3) r0, theta* = arccos(1 - 2u), phi* = 2 pi u.
+    Conformally flat, so the relation is Eq. 7.7: [N][6] = (eta, r, cos th, sin th, cos ph, sin ph) for GEOM_FLRW_POLAR."""
+    r = uniform01(seed, 0, 4 * N).reshape(N, 4)
+    eta = 1.0 / np.cbrt(r[:, 0] * (1.0 + eta0 ** -3) - 1.0)
+    rad = r0 * np.cbrt(r[:, 1])
+    ct = 1.0 - 2.0 * r[:, 2]
+    st = np.sqrt(np.maximum(0.0, 1.0 - ct * ct))
+    ph = (2.0 * np.pi) * r[:, 3]
+    c = np.stack([eta, rad, ct, st, np.cos(ph), np.sin(ph)], axis=1)
+    return _sort_rows(c, eta, rad)
+
+
+def sprinkle_dust_lambda_slab(N: int, seed: int, tau0: float = 1.0, r0: float = 0.5) -> np.ndarray:
+    """3+1 dust + dark energy slab: tau from u = (sinh 3 tau - 3 tau) / (sinh 3 tau0 - 3 tau0)
+    ("must be inverted numerically"), r* = r0 u^(1/3), theta*, phi* as above; conformal time by Eq. 7.5
+    (PAPER.md:3167), eta_M = 2 sinh^(1/3)(3 tau / 2) 2F1(1/6, 1/2; 7/6; -sinh^2(3 tau / 2)) with alpha~ = 1.
+    [N][6] for GEOM_FLRW_POLAR."""
+    from scipy.special import hyp2f1
+    r = uniform01(seed, 0, 4 * N).reshape(N, 4)
+    norm = np.sinh(3.0 * tau0) - 3.0 * tau0
+    tau = _invert_monotone(lambda t: (np.sinh(3.0 * t) - 3.0 * t) / norm, r[:, 0], 0.0, tau0)
+    sh = np.sinh(1.5 * tau)
+    eta = 2.0 * np.cbrt(sh) * hyp2f1(1.0 / 6.0, 0.5, 7.0 / 6.0, -sh * sh)
+    rad = r0 * np.cbrt(r[:, 1])
+    ct = 1.0 - 2.0 * r[:, 2]
+    st = np.sqrt(np.maximum(0.0, 1.0 - ct * ct))
+    ph = (2.0 * np.pi) * r[:, 3]
+    c = np.stack([eta, rad, ct, st, np.cos(ph), np.sin(ph)], axis=1)
+    return _sort_rows(c, eta, rad)
+
+
+def sprinkle_ds2_diamond_flat(N: int, seed: int, w: float = 0.5) -> np.ndarray:
+    """1+1 de Sitter diamond, flat foliation, ds^2 = -4 lambda^2 du dv / (u + v)^2 on [u0, u0 + w]^2 with
+    u0 = v0 = -1/sqrt 2: mu = (u0+v0+w)^2 / ((u0+v0)(u0+v0+2w)), beta = (u0+v0)/(u0+v0+w) mu^u,
+    u* = (beta (v0+w) - v0) / (1 - beta), gamma = w u / (u* + v0 + w), v* = (gamma u* + v0) / (1 - gamma).
+    Conformal to the flat light-cone diamond: [N][2] = (u, v) for GEOM_MINK2_LIGHTCONE."""
+    r = uniform01(seed, 0, 2 * N).reshape(N, 2)
+    u0 = v0 = -1.0 / np.sqrt(2.0)
+    mu = (u0 + v0 + w) ** 2 / ((u0 + v0) * (u0 + v0 + 2.0 * w))
+    beta = (u0 + v0) / (u0 + v0 + w) * mu ** r[:, 0]
+    u = (beta * (v0 + w) - v0) / (1.0 - beta)
+    gamma = w * r[:, 1] / (u + v0 + w)
+    v = (gamma * u + v0) / (1.0 - gamma)
+    c = np.stack([u, v], axis=1)
+    return _sort_rows(c, (u + v) / 2.0, u)
+
+
+def sprinkle_ds2_diamond_spherical(N: int, seed: int, w0: float = 0.8) -> np.ndarray:
+    """1+1 de Sitter diamond, spherical foliation, density ~ sec^2((u + v)/sqrt 2) on [0, w0]^2:
+    mu = (1 + sec(sqrt 2 w0)) / 2, u* = sqrt 2 arctan[(1 - mu^-u) cot(w0 / sqrt 2)],
+    v* = sqrt 2 arctan[u tan((u* + w0)/sqrt 2) + (1 - u) tan(u* / sqrt 2)] - u*.
+    (The extracted text prints the first tangent without its factor u; with it the expression is the inverse of the
+    conditional CDF of the stated density, reading A20.)  [N][2] = (u, v) for GEOM_MINK2_LIGHTCONE."""
+    r = uniform01(seed, 0, 2 * N).reshape(N, 2)
+    s2 = np.sqrt(2.0)
+    mu = (1.0 + 1.0 / np.cos(s2 * w0)) / 2.0
+    u = s2 * np.arctan((1.0 - mu ** (-r[:, 0])) / np.tan(w0 / s2))
+    v = s2 * np.arctan(r[:, 1] * np.tan((u + w0) / s2) + (1.0 - r[:, 1]) * np.tan(u / s2)) - u
+    c = np.stack([u, v], axis=1)
+    return _sort_rows(c, (u + v) / 2.0, u)
+
+
 def chain_lightcone(N: int) -> np.ndarray:
     """Total order: u_i = v_i = i/N (sorted already)."""
     u = np.arange(N, dtype=np.float64) / max(N, 1)

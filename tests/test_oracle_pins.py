@@ -559,3 +559,54 @@ def test_appendix_a_sprinklers(oracle):
     q = dt ** 2 - ((x[None] - x[:, None]) ** 2 + (y[None] - y[:, None]) ** 2 + (z[None] - z[:, None]) ** 2)
     clear = np.triu(np.abs(q) > 1e-12, 1)
     assert np.array_equal(C[clear], np.triu((dt > 0) & (q > 0), 1)[clear]) and C.sum() > 1000
+
+
+def _cdf_close(sample, cdf, lo, hi, tol):
+    qs = np.linspace(lo, hi, 12)[1:-1]
+    emp = np.array([(sample < q).mean() for q in qs])
+    assert np.max(np.abs(emp - cdf(qs))) < tol, (emp, cdf(qs))
+
+
+def test_appendix_a_de_sitter_and_dust_lambda_sprinklers(oracle):
+    """The de Sitter diamonds / flat slab and the dust + dark energy slab: every
+    recipe is checked against the density the paper states for it (marginal and conditional CDFs in closed form),
+    and the conformal time of Eq. 7.5 against a direct quadrature of d tau / a."""
+    n = 60000
+    # 1+1 dS diamond, flat foliation: rho(u, v) ~ 1 / (u + v)^2 on [u0, u0 + w]^2
+    w = 0.5; u0 = v0 = -1 / np.sqrt(2)
+    c = inp.sprinkle_ds2_diamond_flat(n, 3, w)
+    assert c[:, 0].min() >= u0 - 1e-12 and c[:, 0].max() <= u0 + w + 1e-12 and c[:, 1].min() >= v0 - 1e-12 and c[:, 1].max() <= v0 + w + 1e-12
+    g = lambda x: np.log(np.abs(x + v0)) - np.log(np.abs(x + v0 + w))
+    _cdf_close(c[:, 0], lambda q: (g(q) - g(u0)) / (g(u0 + w) - g(u0)), u0, u0 + w, 0.01)
+    band = (c[:, 0] > u0 + 0.2) & (c[:, 0] < u0 + 0.25); um = c[band, 0].mean()
+    _cdf_close(c[band, 1], lambda q: (1 / (um + v0) - 1 / (um + q)) / (1 / (um + v0) - 1 / (um + v0 + w)), v0, v0 + w, 0.03)
+    # 1+1 dS diamond, spherical foliation: rho ~ sec^2((u + v) / sqrt 2) on [0, w0]^2 (reading A20)
+    w0 = 0.8; s2 = np.sqrt(2)
+    c = inp.sprinkle_ds2_diamond_spherical(n, 4, w0)
+    assert c.min() >= -1e-12 and c.max() <= w0 + 1e-12
+    G = lambda x: -np.log(np.cos((x + w0) / s2)) + np.log(np.cos(x / s2))
+    _cdf_close(c[:, 0], lambda q: (G(q) - G(0)) / (G(w0) - G(0)), 0, w0, 0.01)
+    band = (c[:, 0] > 0.3) & (c[:, 0] < 0.33); um = c[band, 0].mean()
+    _cdf_close(c[band, 1], lambda q: (np.tan((um + q) / s2) - np.tan(um / s2)) / (np.tan((um + w0) / s2) - np.tan(um / s2)), 0, w0, 0.03)
+    # both feed the light-cone relation: sorted by time, transitive
+    C = oracle.causal_matrix_bytes(c[:400], inp.GEOM_MINK2_LIGHTCONE).astype(bool)
+    assert not (C.astype(np.int32) @ C.astype(np.int32) > 0)[~C & np.triu(np.ones_like(C), 1)].any()
+    # 3+1 dS slab, flat foliation: rho(eta) ~ eta^-4 on [-1, eta0]
+    e0 = -0.25
+    c = inp.sprinkle_ds4_flat_slab(n, 5, e0, 0.6)
+    assert c[:, 0].min() >= -1 - 1e-12 and c[:, 0].max() <= e0 + 1e-12 and np.all(np.diff(c[:, 0]) >= 0)
+    _cdf_close(c[:, 0], lambda q: (-q ** -3 - 1) / (-e0 ** -3 - 1), -1, e0, 0.01)
+    _cdf_close(c[:, 1] ** 3, lambda q: q / 0.6 ** 3, 0, 0.6 ** 3, 0.01)
+    # dust + dark energy: tau from (sinh 3 tau - 3 tau), eta by Eq. 7.5 = integral of d tau / sinh^(2/3)(3 tau / 2)
+    from scipy.integrate import quad
+    c = inp.sprinkle_dust_lambda_slab(4000, 6, 1.0, 0.5)
+    assert np.all(np.diff(c[:, 0]) >= 0) and c[:, 1].max() <= 0.5
+    for tau in (0.2, 0.7, 1.0):
+        sh = np.sinh(1.5 * tau)
+        from scipy.special import hyp2f1
+        eta = 2 * np.cbrt(sh) * hyp2f1(1 / 6, 0.5, 7 / 6, -sh * sh)
+        assert eta == pytest.approx(quad(lambda t: np.sinh(1.5 * t) ** (-2 / 3), 0, tau)[0], rel=1e-6)
+    eta_max = 2 * np.cbrt(np.sinh(1.5)) * hyp2f1(1 / 6, 0.5, 7 / 6, -np.sinh(1.5) ** 2)
+    assert 0 < c[:, 0].min() and c[:, 0].max() <= eta_max + 1e-12
+    C = oracle.causal_matrix_bytes(c[:500], inp.GEOM_FLRW_POLAR)
+    assert C.sum() > 0
