@@ -866,3 +866,34 @@ def test_ds4_spherical_and_cone5_pipelines(api, oracle):
         api.bd_action(hist, N, 5)
     with pytest.raises(RuntimeError):
         api.causal_matrix(torch.zeros((10, 6), dtype=torch.float64, device="cuda"), inp.GEOM_DS4_SPHERICAL)
+
+
+@pytest.mark.slow
+def test_larger_N_properties(api, oracle):
+    """NEXT-4 'larger N': N = 262144 (8 GiB per bit matrix, 1024 x 1024 tiles) in the 1+1 de Sitter slab.  The oracle's
+    tier-1 would need ~10 minutes here, so the checks are the ones that hold at any size: sum_k N_k = R,
+    sum_k k N_k = sum_m indeg(m) outdeg(m), additivity of row ranges (the --shard split of 4 ranks), and six sampled
+    rows whose per-pair interval sizes are recounted on the host from the definition, popcount(bits[i] & bitsT[j])."""
+    from paper_1805_04463_b200 import dist as csd
+    N = 1 << 18
+    coords = inp.sprinkle_ds2_slab(N, 2718)
+    bits, bitsT = gpu_bits(api, coords, inp.GEOM_DS2_SLAB)
+    stats = api.relation_stats(bits, N).cpu().numpy()
+    hist, nrel = api.interval_hist(bits, bitsT, N, return_relations=True)
+    assert int(nrel[0]) == int(stats[0]) == int(hist.sum())
+    outdeg, indeg = api.degrees(bits, bitsT, N)
+    k = torch.arange(hist.numel(), device="cuda", dtype=torch.int64)
+    assert int((k * hist).sum()) == int((outdeg * indeg).sum())
+    total = torch.zeros_like(hist)
+    for r0, r1 in csd.shard_rows(N, 4):
+        total += api.interval_hist(bits, bitsT, N, row_begin=r0, row_end=r1)
+    assert torch.equal(total, hist)
+    # sampled rows i: count(i, j) = popcount(bits[i] & bitsT[j]) over the related j, histogrammed with numpy
+    hb = bits.cpu().numpy().view(np.uint64); hbT = bitsT.cpu().numpy().view(np.uint64)
+    rng = np.random.default_rng(5)
+    for i in rng.integers(0, N - 1000, 6).tolist():
+        part = api.interval_hist(bits, bitsT, N, row_begin=i, row_end=i + 1).cpu().numpy()
+        js = np.flatnonzero(np.unpackbits(hb[i].view(np.uint8), bitorder="little")[:N])
+        cnt = np.array([int(np.unpackbits((hb[i] & hbT[j]).view(np.uint8)).sum()) for j in js], dtype=np.int64)
+        want = np.bincount(cnt, minlength=part.shape[0])[:part.shape[0]]
+        assert np.array_equal(part, want), i
