@@ -521,8 +521,29 @@ k_causal_matrix(const double *__restrict__ coords, int64_t N, int64_t stride,
     }
     __syncthreads();    // s_xi / s_f visible; s_red (aliased on s_U) no longer read
 
+    // The common CTA -- both column tiles above the diagonal and on the prefilter -- runs a loop with nothing in it
+    // but the blocks, the (rare) fp64 fallback, the two transposes and four shared-memory stores; everything that
+    // depends on diagonal tiles, inactive tiles or tiles off the prefilter stays in the general loop below.
+    const bool plain = FAST && !any_diag && act[0] && act[1] && fast[0] && fast[1];
+    if (plain) {
+        uint32_t *pL0 = &s_L[jl][0], *pL1 = &s_L[BT + jl][0], *pU = &s_U[lane][warp];
 #pragma unroll 1
-    for (int sb = 0; sb < BT / 32; sb++) {
+        for (int sb = 0; sb < BT / 32; sb++) {
+            uint32_t lw[NJ] = {0, 0};
+            bool unc[NJ] = {false, false};
+            fast_block<GEOM, DIM, 2>(s_f, sb * 32, fj, hj, m, lw, unc);
+            if (__any_sync(0xffffffffu, unc[0] || unc[1])) {
+                lw[0] = lw[1] = 0;
+                exact_block<GEOM, DIM, 2>(s_xi, sb * 32, xj, lw);
+            }
+            pL0[sb] = lw[0];
+            pL1[sb] = lw[1];
+            pU[sb * 32 * (NJ * 8 + 1)] = transpose(lw[0]);
+            pU[sb * 32 * (NJ * 8 + 1) + 8] = transpose(lw[1]);
+        }
+    }
+#pragma unroll 1
+    for (int sb = plain ? BT / 32 : 0; sb < BT / 32; sb++) {
         uint32_t lw[NJ];
         bool need[NJ], slow[NJ];
 #pragma unroll
