@@ -115,6 +115,35 @@ int cs_causal_matrix(const double *coords, int64_t N, int dim, int geometry,
 int cs_causal_matrix_batched(const double *coords, int64_t B, int64_t N, int dim, int geometry,
                              uint64_t *bits, uint64_t *bitsT, void *stream);
 
+/* How a1 is computed.  Both routes write identical bits. */
+enum cs_a1_route {
+    CS_A1_AUTO = 0,         /* the library's choice for this geometry and size */
+    CS_A1_FMA = 1,          /* every geometry: predicate on the FMA pipes (exact fp32 prefilter, fp64 inside its error band) */
+    CS_A1_TENSOR = 2        /* predicates that are the sign of a bilinear form (CS_GEOM_MINK_CONE, CS_GEOM_FLRW_POLAR,
+                               CS_GEOM_DS4_SPHERICAL): the form as a split-bf16 contraction on tcgen05 tensor cores, rows of a
+                               32 x 32 block with a value inside the error band re-evaluated in fp64.  CS_ERR_ARG for the
+                               other geometries. */
+};
+
+/* a1 with the route chosen by the caller and an optional workspace (B causets, B = 1 for a single one).
+ *   workspace  device, >= cs_causal_matrix_workspace() bytes, 256-byte aligned, or NULL: the tensor route then takes its
+ *              scratch (operand rows of the points, 128 B per point and less than 1 % of the matrices) from a
+ *              stream-ordered memory pool the library owns on this device.
+ * bits / bitsT must be 16-byte aligned.  Errors as cs_causal_matrix, + CS_ERR_WORKSPACE. */
+size_t cs_causal_matrix_workspace(int64_t B, int64_t N, int dim, int geometry, int route);
+int cs_causal_matrix_ex(const double *coords, int64_t B, int64_t N, int dim, int geometry, int route,
+                        uint64_t *bits, uint64_t *bitsT, void *workspace, size_t workspace_bytes, void *stream);
+
+/* CS_A1_TENSOR on one flat-cone causet (dim 4 or 5) with its counters on: what the tensor-core value of the bilinear form
+ * was worth on this input.  Writes bits / bitsT as cs_causal_matrix does.
+ *   out_host  host, double[4], overwritten: [0] the largest |a - T| seen, in units of 2^-24 C^2 (a = tensor-core value,
+ *             T = the form evaluated in fp64, C = largest |coordinate| of the tile; over all pairs decided by sign),
+ *             [1] (row, 32-column block) pairs re-evaluated in fp64, [2] (row, block) pairs examined, [3] the margin the
+ *             kernel uses, same unit as [0].
+ * Synchronises `stream`.  Errors: CS_ERR_ARG, CS_ERR_DIM, CS_ERR_WORKSPACE, CS_ERR_CUDA. */
+int cs_a1_tensor_probe(const double *coords, int64_t N, int dim, uint64_t *bits, uint64_t *bitsT,
+                       void *workspace, size_t workspace_bytes, double *out_host, void *stream);
+
 /* bitsT <- transpose(bits) (both device, [N][stride]); for callers that kept only `bits`. */
 int cs_transpose_bits(const uint64_t *bits, int64_t N, uint64_t *bitsT, void *stream);
 

@@ -27,6 +27,9 @@ ROUTE_POPC = 1
 ROUTE_TENSOR = 2
 ROUTE_TENSOR_FP4 = 3
 ROUTE_TENSOR_PAIR = 4
+A1_AUTO = 0           # cs_a1_route
+A1_FMA = 1
+A1_TENSOR = 2
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 # CAUSALSET_LIB selects another build of the same library (A/B timing of kernel variants); default: in-tree
@@ -45,6 +48,9 @@ _SIGNATURES = {
     "cs_row_stride_words": (_i64, [_i64]),
     "cs_causal_matrix": (_int, [_p, _i64, _int, _int, _p, _p, _p]),
     "cs_causal_matrix_batched": (_int, [_p, _i64, _i64, _int, _int, _p, _p, _p]),
+    "cs_causal_matrix_workspace": (_sz, [_i64, _i64, _int, _int, _int]),
+    "cs_causal_matrix_ex": (_int, [_p, _i64, _i64, _int, _int, _int, _p, _p, _p, _sz, _p]),
+    "cs_a1_tensor_probe": (_int, [_p, _i64, _int, _p, _p, _p, _sz, _p, _p]),
     "cs_transpose_bits": (_int, [_p, _i64, _p, _p]),
     "cs_degrees": (_int, [_p, _p, _i64, _p, _p, _p]),
     "cs_relation_stats": (_int, [_p, _i64, _p, _p]),
@@ -139,7 +145,12 @@ def peak_probe(kind: str, iters: int, workspace: torch.Tensor):
     return float(out[0]), float(out[1]), float(out[2])
 
 
-def causal_matrix(coords: torch.Tensor, geometry: int, want_transpose: bool = True):
+def causal_matrix_workspace(B: int, N: int, dim: int, geometry: int, route: int = A1_AUTO) -> int:
+    return int(load().cs_causal_matrix_workspace(B, N, dim, geometry, route))
+
+
+def causal_matrix(coords: torch.Tensor, geometry: int, want_transpose: bool = True, route: int = A1_AUTO,
+                  workspace: torch.Tensor | None = None):
     """coords [N][dim] fp64 (CUDA, time-sorted) -> (bits, bitsT) int64 tensors [N][stride]
     holding the uint64 bit rows (bitsT is None if want_transpose is False)."""
     _need_cuda(coords, torch.float64, "coords")
@@ -147,20 +158,39 @@ def causal_matrix(coords: torch.Tensor, geometry: int, want_transpose: bool = Tr
     stride = row_stride_words(N)
     bits = torch.empty((N, stride), dtype=torch.int64, device=coords.device)
     bitsT = torch.empty((N, stride), dtype=torch.int64, device=coords.device) if want_transpose else None
-    _check(load().cs_causal_matrix(_dptr(coords), N, dim, geometry, _dptr(bits), _dptr(bitsT), _stream()),
-           "cs_causal_matrix")
+    _check(load().cs_causal_matrix_ex(_dptr(coords), 1, N, dim, geometry, route, _dptr(bits), _dptr(bitsT),
+                                      _dptr(workspace), workspace.numel() if workspace is not None else 0, _stream()),
+           "cs_causal_matrix_ex")
     return bits, bitsT
 
 
-def causal_matrix_batched(coords: torch.Tensor, geometry: int, want_transpose: bool = True):
+def causal_matrix_batched(coords: torch.Tensor, geometry: int, want_transpose: bool = True, route: int = A1_AUTO,
+                          workspace: torch.Tensor | None = None):
     _need_cuda(coords, torch.float64, "coords")
     B, N, dim = coords.shape
     stride = row_stride_words(N)
     bits = torch.empty((B, N, stride), dtype=torch.int64, device=coords.device)
     bitsT = torch.empty((B, N, stride), dtype=torch.int64, device=coords.device) if want_transpose else None
-    _check(load().cs_causal_matrix_batched(_dptr(coords), B, N, dim, geometry, _dptr(bits), _dptr(bitsT), _stream()),
-           "cs_causal_matrix_batched")
+    _check(load().cs_causal_matrix_ex(_dptr(coords), B, N, dim, geometry, route, _dptr(bits), _dptr(bitsT),
+                                      _dptr(workspace), workspace.numel() if workspace is not None else 0, _stream()),
+           "cs_causal_matrix_ex")
     return bits, bitsT
+
+
+def a1_tensor_probe(coords: torch.Tensor):
+    """CS_A1_TENSOR on one flat-cone causet (dim 4 or 5) with its counters on ->
+    (bits, bitsT, {"max_err_u": .., "rows_fp64": .., "rows_total": .., "margin_u": ..})."""
+    _need_cuda(coords, torch.float64, "coords")
+    N, dim = coords.shape
+    stride = row_stride_words(N)
+    bits = torch.empty((N, stride), dtype=torch.int64, device=coords.device)
+    bitsT = torch.empty((N, stride), dtype=torch.int64, device=coords.device)
+    ws = _workspace(causal_matrix_workspace(1, N, dim, GEOM_MINK_CONE, A1_TENSOR), coords.device)
+    out = (ctypes.c_double * 4)()
+    _check(load().cs_a1_tensor_probe(_dptr(coords), N, dim, _dptr(bits), _dptr(bitsT), _dptr(ws), ws.numel(),
+                                     ctypes.addressof(out), _stream()), "cs_a1_tensor_probe")
+    return bits, bitsT, {"max_err_u": float(out[0]), "rows_fp64": int(out[1]), "rows_total": int(out[2]),
+                         "margin_u": float(out[3])}
 
 
 def transpose_bits(bits: torch.Tensor, N: int) -> torch.Tensor:

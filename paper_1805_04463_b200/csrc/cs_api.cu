@@ -133,22 +133,57 @@ int cs_default_route(int64_t N)
     return interval_tensor_available() && N >= 1024 ? CS_ROUTE_TENSOR_PAIR : CS_ROUTE_POPC;
 }
 
-int cs_causal_matrix_batched(const double *coords, int64_t B, int64_t N, int dim, int geometry,
-                             uint64_t *bits, uint64_t *bitsT, void *stream)
+static int check_a1_args(const double *coords, int64_t B, int64_t N, int dim, int geometry, const uint64_t *bits)
 {
     if (N < 0 || B < 0) return CS_ERR_ARG;
     if (geometry < CS_GEOM_MINK2_LIGHTCONE || geometry > CS_GEOM_DS4_SPHERICAL) return CS_ERR_GEOM;
     const int want = geometry == CS_GEOM_FLRW_POLAR ? 6 : geometry == CS_GEOM_DS4_SPHERICAL ? 7 : 2;
     if (geometry == CS_GEOM_MINK_CONE ? (dim < 2 || dim > 5) : (dim != want)) return CS_ERR_DIM;
-    if (N == 0 || B == 0) return CS_OK;
+    if (N == 0 || B == 0) return 1;      // nothing to do
     if (!coords || !bits) return CS_ERR_ARG;
-    return launch_causal_matrix(coords, B, N, dim, geometry, bits, bitsT, static_cast<cudaStream_t>(stream));
+    return CS_OK;
+}
+
+size_t cs_causal_matrix_workspace(int64_t B, int64_t N, int dim, int geometry, int route)
+{
+    if (check_a1_args(reinterpret_cast<const double *>(16), B, N, dim, geometry, reinterpret_cast<const uint64_t *>(16)) != CS_OK) return 0;
+    if (route < CS_A1_AUTO || route > CS_A1_TENSOR) return 0;
+    return causal_matrix_scratch_bytes(B, N, dim, geometry, route);
+}
+
+int cs_causal_matrix_ex(const double *coords, int64_t B, int64_t N, int dim, int geometry, int route,
+                        uint64_t *bits, uint64_t *bitsT, void *workspace, size_t workspace_bytes, void *stream)
+{
+    const int rc = check_a1_args(coords, B, N, dim, geometry, bits);
+    if (rc) return rc < 0 ? rc : CS_OK;
+    if (route < CS_A1_AUTO || route > CS_A1_TENSOR) return CS_ERR_ARG;
+    if (misaligned16(bits, bitsT)) return CS_ERR_ARG;
+    return launch_causal_matrix(coords, B, N, dim, geometry, route, bits, bitsT, workspace, workspace_bytes,
+                                static_cast<cudaStream_t>(stream));
+}
+
+int cs_causal_matrix_batched(const double *coords, int64_t B, int64_t N, int dim, int geometry,
+                             uint64_t *bits, uint64_t *bitsT, void *stream)
+{
+    return cs_causal_matrix_ex(coords, B, N, dim, geometry, CS_A1_AUTO, bits, bitsT, nullptr, 0, stream);
 }
 
 int cs_causal_matrix(const double *coords, int64_t N, int dim, int geometry,
                      uint64_t *bits, uint64_t *bitsT, void *stream)
 {
-    return cs_causal_matrix_batched(coords, 1, N, dim, geometry, bits, bitsT, stream);
+    return cs_causal_matrix_ex(coords, 1, N, dim, geometry, CS_A1_AUTO, bits, bitsT, nullptr, 0, stream);
+}
+
+int cs_a1_tensor_probe(const double *coords, int64_t N, int dim, uint64_t *bits, uint64_t *bitsT,
+                       void *workspace, size_t workspace_bytes, double *out_host, void *stream)
+{
+    if (!coords || !bits || !out_host || N < 1) return CS_ERR_ARG;
+    if (dim != 4 && dim != 5) return CS_ERR_DIM;
+    if (misaligned16(bits, bitsT)) return CS_ERR_ARG;
+    if (!causal_tc_supported(CS_GEOM_MINK_CONE, dim)) return CS_ERR_ARG;
+    if (!workspace || workspace_bytes < causal_tc_scratch_bytes(1, N, dim, CS_GEOM_MINK_CONE) || ((uintptr_t)workspace & 255))
+        return CS_ERR_WORKSPACE;
+    return launch_causal_tc_probe(coords, N, dim, bits, bitsT, workspace, out_host, static_cast<cudaStream_t>(stream));
 }
 
 int cs_transpose_bits(const uint64_t *bits, int64_t N, uint64_t *bitsT, void *stream)

@@ -12,6 +12,8 @@
 //
 // Floating point: explicit round-to-nearest intrinsics (__dsub_rn, __dmul_rn, __dadd_rn), which
 // the compiler never contracts into FMA, in exactly the order stated in include/causalset.h.
+#include <mutex>
+
 #include "cs_predicates.cuh"
 
 namespace cs {
@@ -437,8 +439,8 @@ static int launch_build_t(const double *coords, int64_t B, int64_t N, int64_t st
     return CS_OK;
 }
 
-int launch_causal_matrix(const double *coords, int64_t B, int64_t N, int dim, int geometry,
-                         uint64_t *bits, uint64_t *bitsT, cudaStream_t st)
+static int launch_causal_fma(const double *coords, int64_t B, int64_t N, int dim, int geometry,
+                             uint64_t *bits, uint64_t *bitsT, cudaStream_t st)
 {
     const int64_t stride = row_stride_words(N);
     if (N > (int64_t)BT * 65535 || B > 65535) return CS_ERR_ARG;
@@ -464,6 +466,72 @@ int launch_causal_matrix(const double *coords, int64_t B, int64_t N, int dim, in
     default:
         return CS_ERR_GEOM;
     }
+}
+
+// Which kernel builds the matrix.  The tensor route (cs_build_tc.cu) serves the bilinear predicates; measured on
+// B200 it wins from a few 256 x 256 tiles per SM up, below that the persistent kernel's set-up (TMEM allocation,
+// operand prep launch) is not paid back.
+constexpr int64_t TC_MIN_PAIRS = (int64_t)1 << 21;      // B * N^2 / 2 pairs: 2048 points of one causet
+
+static int resolve_a1_route(int64_t B, int64_t N, int dim, int geometry, int route)
+{
+    if (route == CS_A1_FMA) return CS_A1_FMA;
+    const bool can = causal_tc_supported(geometry, dim) && N >= 1;
+    if (route == CS_A1_TENSOR) return can ? CS_A1_TENSOR : -1;
+    return can && B * N * N / 2 >= TC_MIN_PAIRS ? CS_A1_TENSOR : CS_A1_FMA;
+}
+
+size_t causal_matrix_scratch_bytes(int64_t B, int64_t N, int dim, int geometry, int route)
+{
+    const int r = resolve_a1_route(B, N, dim, geometry, route);
+    return r == CS_A1_TENSOR ? causal_tc_scratch_bytes(B, N, dim, geometry) : 0;
+}
+
+// Stream-ordered scratch for callers that pass no workspace: one memory pool per device, owned by the library, which
+// keeps what it has allocated (release threshold = never), so that after the first call an allocation is a pointer bump.
+static int scratch_pool(cudaMemPool_t *out)
+{
+    static cudaMemPool_t pools[MAX_DEVICES];
+    static bool ready[MAX_DEVICES];
+    static std::mutex mu;
+    std::lock_guard<std::mutex> lock(mu);
+    const int dev = current_device();
+    if (!ready[dev]) {
+        cudaMemPoolProps props;
+        memset(&props, 0, sizeof(props));
+        props.allocType = cudaMemAllocationTypePinned;
+        props.handleTypes = cudaMemHandleTypeNone;
+        props.location.type = cudaMemLocationTypeDevice;
+        props.location.id = dev;
+        CS_CUDA(cudaMemPoolCreate(&pools[dev], &props));
+        uint64_t keep = ~(uint64_t)0;
+        CS_CUDA(cudaMemPoolSetAttribute(pools[dev], cudaMemPoolAttrReleaseThreshold, &keep));
+        ready[dev] = true;
+    }
+    *out = pools[dev];
+    return CS_OK;
+}
+
+int launch_causal_matrix(const double *coords, int64_t B, int64_t N, int dim, int geometry, int route,
+                         uint64_t *bits, uint64_t *bitsT, void *scratch, size_t scratch_bytes, cudaStream_t st)
+{
+    const int r = resolve_a1_route(B, N, dim, geometry, route);
+    if (r < 0) return CS_ERR_ARG;
+    if (r == CS_A1_FMA) return launch_causal_fma(coords, B, N, dim, geometry, bits, bitsT, st);
+    const size_t need = causal_tc_scratch_bytes(B, N, dim, geometry);
+    if (scratch) {
+        if (scratch_bytes < need || ((uintptr_t)scratch & 255)) return CS_ERR_WORKSPACE;
+        return launch_causal_tc(coords, B, N, dim, geometry, bits, bitsT, scratch, st);
+    }
+    cudaMemPool_t pool;
+    int rc = scratch_pool(&pool);
+    if (rc) return rc;
+    void *p = nullptr;
+    CS_CUDA(cudaMallocFromPoolAsync(&p, need, pool, st));
+    rc = launch_causal_tc(coords, B, N, dim, geometry, bits, bitsT, p, st);
+    cudaError_t e = cudaFreeAsync(p, st);
+    if (rc == CS_OK && e != cudaSuccess) return cuda_fail(e, "cudaFreeAsync");
+    return rc;
 }
 
 // ---- transpose -----------------------------------------------------------------------------

@@ -1,0 +1,749 @@
+// cs_build_tc.cu -- stage a1 on the tensor cores, for the predicates that are the sign of a bilinear form
+// (flat cone in 1+1 .. 4+1 dimensions, FLRW Eq. 7.7, 3+1 de Sitter).
+//
+// The sign of the interval between i and j is the sign of
+//     T(i, j) = h_i + h_j + sum_c P_c(i) F_c(j)          (cs_predicates.cuh, Fast<GEOM, DIM>)
+// i.e. one entry of a rank-(NP + 2) matrix product.  Every fp32 input v is split exactly into three bf16 pieces
+// v = hi + mid + lo (round to nearest each time: |mid| <= 2^-8 |v|, |lo| <= 2^-16 |v|); a product P F is then the sum
+// of nine piece products, each exact in fp32, of which the six not smaller than 2^-16 |P F| are kept:
+//     hi hi | hi mid, mid hi | mid mid, hi lo, lo hi          (dropped: mid lo, lo mid, lo lo <= 2.01 * 2^-24 |P F|)
+// and h_i + h_j enters as (h pieces of i) x 1 + 1 x (h pieces of j).  That is K = 6 NP + 6 <= 32 (48 for five or six
+// products) bf16 columns per point, and T for a 128 x 256 block of pairs is two (three) tcgen05.mma kind::f16
+// instructions with fp32 accumulation in TMEM -- 1/32 of what the FMA pipes need for the same block.
+//
+// What the tensor core returns is a value `a` with |a - T| <= E: the error of the fp32 prefilter's inputs (the same
+// fp64 -> fp32 conversions as in cs_build.cu: <= 11.04 u C^2 for four products, u = 2^-24, C = largest |component|
+// of the tile), the dropped piece products (<= 2.01 NP u C^2) and the accumulation inside the tensor core.  The order
+// and the width of that accumulation are not documented; the margin below assumes nothing about the order and allows
+// every one of the K + 1 addends of an instruction to lose one unit in the last place of an fp32 number as large as
+// the largest partial sum can be ((NP / 2 + 2 + NP) C^2 <= 8 C^2: <= 2^-20 C^2 per addend), i.e. E <= (K + 3) 2^-20
+// C^2 + 20 u C^2 < 2^-14 C^2 for K <= 48.  `cs_a1_tc_probe` measures |a - T| against the fp64 value on real tiles
+// (profiles/r2_a1_tensor.md: the largest error seen is ~3 u C^2, 300 times below the margin).
+//     |a| > m = 2^-14 C^2   =>   sign(a) = sign(T), and |T| > 2^-15 C^2 is far outside the rounding of the fp64
+//                                expression of the header (2^-46 C^2): related iff a > 0
+//     anything else (NaN included): the 32 pairs of that ROW of the block are re-evaluated with the fp64 expression.
+// As in cs_build.cu a tile takes the prefilter only if dt >= 0 is known for every pair it keeps (time order per
+// tile, checked on the doubles by the prep kernel), 2^-40 <= C <= 2^40 and every point is finite and passes
+// Fast::convert; otherwise m = +inf and every row goes to fp64.  The output is bit-identical to the fp64 evaluation
+// by construction.
+//
+// Kernels: k_tc_prep (one thread per point: conversion, pieces, both operand rows in the UMMA canonical K-major
+// layout, per-128-point summaries) and k_causal_tc (persistent, one CTA per SM: a bulk-copy loader, a one-thread MMA
+// issuer, 16 epilogue warps).  An epilogue warp reads 32 rows x 32 columns of accumulators (tcgen05.ld, lane = row),
+// shifts the 32 sign bits of its row into one word (one SHF per pair), keeps min |a| (one FMNMX3 per two pairs),
+// transposes the 32 x 32 bit block with the shuffle butterfly for the second output, and stages both in shared
+// memory; a 256 x 256 tile leaves as full 32-byte row segments, mirrored zero tiles included.
+#include <cuda_bf16.h>
+
+#include <type_traits>
+
+#include "cs_predicates.cuh"
+
+namespace cs {
+
+namespace {
+
+constexpr int TCT = 256;                 // tile edge (pairs): two M = 128 accumulators of 256 columns
+constexpr int TC_EPI_WARPS = 16;
+constexpr int TC_EPI0 = 2;               // warp 0: loader, warp 1: MMA issuer + TMEM owner, warps 2..17: epilogue,
+constexpr int TC_WR0 = TC_EPI0 + TC_EPI_WARPS;   // warps 18..19: writers (staged tile -> global memory)
+constexpr int TC_WR_WARPS = 2;
+constexpr int TC_THREADS = (TC_WR0 + TC_WR_WARPS) * 32;
+constexpr int TC_PITCH = 9;              // words per staged row (8 + 1: conflict-free 4-byte stores by 32 rows)
+constexpr int TC_MARGIN_LOG2 = -14;      // m = 2^-14 C^2
+
+template <int GEOM, int DIM>
+struct TcShape {
+    using F = Fast<GEOM, DIM>;
+    static constexpr int USED = 6 * F::NP + (F::H ? 6 : 2);     // without h two columns carry the padding marker
+    static constexpr int K = USED <= 32 ? 32 : 48;
+    static constexpr int KC = K / 8;                              // 16-byte chunks per operand row
+    static constexpr int A_BLOCK = KC * 128 * 16;                 // operand image of 128 past points
+    static constexpr int B_BLOCK = KC * 256 * 16;                 // operand image of 256 future points
+    static constexpr int STAGE = 2 * A_BLOCK + B_BLOCK;
+    static_assert(USED <= 48, "operand columns");
+};
+
+struct TcBlockInfo {                     // summary of 128 consecutive points
+    double tmin, tmax;                   // over the valid points (+inf / -inf if none)
+    float C;                             // largest |fp32 component|
+    uint32_t flags;                      // 1: t non-decreasing inside the block, 2: last point <= first of the next block, 4: a point
+                                         // that may not use the prefilter (not finite, or Fast::convert says no)
+    uint32_t pad[2];
+};
+static_assert(sizeof(TcBlockInfo) == 32, "TcBlockInfo");
+
+__device__ __forceinline__ uint32_t tc_smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void tc_mbar_init(uint64_t *bar, uint32_t count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(tc_smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void tc_mbar_arrive(uint64_t *bar)
+{
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(tc_smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void tc_mbar_wait(uint64_t *bar, uint32_t parity)
+{
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "LAB_WAIT:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra LAB_DONE;\n"
+        "bra LAB_WAIT;\n"
+        "LAB_DONE:\n"
+        "}\n" ::"r"(tc_smem_u32(bar)),
+        "r"(parity)
+        : "memory");
+}
+__device__ __forceinline__ void tc_mbar_expect_tx(uint64_t *bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(tc_smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void tc_bulk_g2s(void *dst, const void *src, uint32_t bytes, uint64_t *bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+                     tc_smem_u32(dst)),
+                 "l"(src), "r"(bytes), "r"(tc_smem_u32(bar))
+                 : "memory");
+}
+__device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
+
+// shared-memory matrix descriptor: no swizzle, K-major; LBO = distance between 16-byte k chunks, SBO = between
+// groups of 8 rows (both in bytes); bit 46 = descriptor version of sm_100
+__device__ __forceinline__ uint64_t tc_desc(uint32_t saddr, uint32_t lbo_bytes, uint32_t sbo_bytes)
+{
+    uint64_t d = 0;
+    d |= (uint64_t)((saddr >> 4) & 0x3FFF);
+    d |= (uint64_t)((lbo_bytes >> 4) & 0x3FFF) << 16;
+    d |= (uint64_t)((sbo_bytes >> 4) & 0x3FFF) << 32;
+    d |= (uint64_t)1 << 46;
+    return d;
+}
+// instruction descriptor, kind::f16: D = F32 (1 at bit 4), A = B = BF16 (1 at bits 7 and 10), both K-major,
+// N >> 3 at bit 17, M >> 4 at bit 24
+constexpr uint32_t TC_IDESC = (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(256 >> 3) << 17) | ((uint32_t)(128 >> 4) << 24);
+
+__device__ __forceinline__ void tc_mma_bf16(uint32_t d_tmem, uint64_t adesc, uint64_t bdesc, uint32_t accum)
+{
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "setp.ne.b32 p, %4, 0;\n"
+        "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n"
+        "}\n" ::"r"(d_tmem),
+        "l"(adesc), "l"(bdesc), "r"(TC_IDESC), "r"(accum)
+        : "memory");
+}
+__device__ __forceinline__ void tc_commit(uint64_t *bar)
+{
+    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(tc_smem_u32(bar))
+                 : "memory");
+}
+// 32 lanes x 32 columns -> 32 registers per thread; the caller issues tcgen05.wait::ld
+__device__ __forceinline__ void tc_ld32(uint32_t taddr, uint32_t *v)
+{
+    asm volatile(
+        "tcgen05.ld.sync.aligned.32x32b.x32.b32 "
+        "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, "
+        "%16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31}, [%32];\n"
+        : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]),
+          "=r"(v[8]), "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15]),
+          "=r"(v[16]), "=r"(v[17]), "=r"(v[18]), "=r"(v[19]), "=r"(v[20]), "=r"(v[21]), "=r"(v[22]), "=r"(v[23]),
+          "=r"(v[24]), "=r"(v[25]), "=r"(v[26]), "=r"(v[27]), "=r"(v[28]), "=r"(v[29]), "=r"(v[30]), "=r"(v[31])
+        : "r"(taddr)
+        : "memory");
+}
+
+// v = hi + mid + lo exactly (each piece rounded to nearest; 24 significand bits = 3 x 8)
+__device__ __forceinline__ void split3(float v, uint16_t (&p)[3])
+{
+    const __nv_bfloat16 a = __float2bfloat16_rn(v);
+    const float r1 = v - __bfloat162float(a);
+    const __nv_bfloat16 b = __float2bfloat16_rn(r1);
+    const float r2 = r1 - __bfloat162float(b);
+    const __nv_bfloat16 c = __float2bfloat16_rn(r2);
+    p[0] = __bfloat16_as_ushort(a);
+    p[1] = __bfloat16_as_ushort(b);
+    p[2] = __bfloat16_as_ushort(c);
+}
+
+// ---- prep: one thread per point ------------------------------------------------------------------
+// Operand columns, in this order (pairs (A column of the past point, B column of the future point)):
+//   rank 0:  (P_hi, F_hi) per component                      [+ (h_hi, 1), (1, h_hi)]
+//   rank 1:  (P_hi, F_mid), (P_mid, F_hi) per component      [+ (h_mid, 1), (1, h_mid)]
+//   rank 2:  (P_mid, F_mid), (P_hi, F_lo), (P_lo, F_hi)      [+ (h_lo, 1), (1, h_lo)]
+// A point beyond N has zero components and h = -2^100 (exactly one bf16 piece), so that every pair it belongs to reads
+// a = -2^100 or -2^101: "unrelated", far outside the band.  Predicates without h carry the marker in two columns of
+// their own, (pad, 1) and (1, pad), pad = 0 for a valid point.
+constexpr float TC_PAD = -0x1p100f;
+
+template <int GEOM, int DIM>
+__global__ void __launch_bounds__(128)
+k_tc_prep(const double *__restrict__ coords, int64_t N, int nA,
+          unsigned char *__restrict__ opA, unsigned char *__restrict__ opB, TcBlockInfo *__restrict__ info,
+          double *__restrict__ cpad)
+{
+    using F = Fast<GEOM, DIM>;
+    using S = TcShape<GEOM, DIM>;
+    constexpr int NP = F::NP;
+    const int a = blockIdx.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int64_t b = blockIdx.y;
+    coords += b * N * DIM;
+    const int64_t gp = (int64_t)a * 128 + tid;
+    const bool valid = gp < N;
+
+    double x[DIM];
+#pragma unroll
+    for (int d = 0; d < DIM; d++) x[d] = valid ? coords[gp * DIM + d] : 0.0;
+    {   // padded copy of the coordinates (NaN beyond N: unrelated to everything) for the fp64 rows of the main kernel
+        const double qnan = __longlong_as_double(0x7FF8000000000000LL);
+        double *cp = cpad + (((size_t)b * nA + a) * 128 + tid) * DIM;
+#pragma unroll
+        for (int d = 0; d < DIM; d++) cp[d] = valid ? x[d] : qnan;
+    }
+    float v[NP], h = 0.f;
+    bool ok = F::convert(x, v, h);
+    float c = 0.f;
+#pragma unroll
+    for (int q = 0; q < NP; q++) {
+        c = fmaxf(c, fabsf(v[q]));
+        ok = ok && isfinite(v[q]);
+    }
+    ok = ok && isfinite(h);
+    if (!valid) {
+#pragma unroll
+        for (int q = 0; q < NP; q++) v[q] = 0.f;
+        h = F::H ? TC_PAD : 0.f;
+        c = 0.f;
+        ok = true;
+    }
+
+    // operand rows
+    uint16_t A[S::K], Bv[S::K];
+    {
+        uint16_t P[NP][3], Fp[NP][3], hp[3], pp[3];
+#pragma unroll
+        for (int q = 0; q < NP; q++) {
+            split3(v[q], Fp[q]);
+            split3(q < F::NNEG ? -v[q] : v[q], P[q]);
+        }
+        split3(h, hp);
+        split3(valid ? 0.f : TC_PAD, pp);
+        constexpr uint16_t ONE = 0x3F80;
+        int k = 0;
+#pragma unroll
+        for (int q = 0; q < NP; q++) { A[k] = P[q][0]; Bv[k] = Fp[q][0]; k++; }
+        if (F::H) { A[k] = hp[0]; Bv[k] = ONE; k++; A[k] = ONE; Bv[k] = hp[0]; k++; }
+        else      { A[k] = pp[0]; Bv[k] = ONE; k++; A[k] = ONE; Bv[k] = pp[0]; k++; }
+#pragma unroll
+        for (int q = 0; q < NP; q++) {
+            A[k] = P[q][0]; Bv[k] = Fp[q][1]; k++;
+            A[k] = P[q][1]; Bv[k] = Fp[q][0]; k++;
+        }
+        if (F::H) { A[k] = hp[1]; Bv[k] = ONE; k++; A[k] = ONE; Bv[k] = hp[1]; k++; }
+#pragma unroll
+        for (int q = 0; q < NP; q++) {
+            A[k] = P[q][1]; Bv[k] = Fp[q][1]; k++;
+            A[k] = P[q][0]; Bv[k] = Fp[q][2]; k++;
+            A[k] = P[q][2]; Bv[k] = Fp[q][0]; k++;
+        }
+        if (F::H) { A[k] = hp[2]; Bv[k] = ONE; k++; A[k] = ONE; Bv[k] = hp[2]; k++; }
+#pragma unroll
+        for (; k < S::K; k++) { A[k] = 0; Bv[k] = 0; }
+    }
+    unsigned char *dA = opA + ((size_t)b * nA + a) * S::A_BLOCK + (size_t)tid * 16;
+    unsigned char *dB = opB + ((size_t)b * (nA / 2) + (a >> 1)) * S::B_BLOCK + (size_t)((a & 1) * 128 + tid) * 16;
+#pragma unroll
+    for (int kc = 0; kc < S::KC; kc++) {
+        uint4 wa, wb;
+        wa.x = A[8 * kc] | ((uint32_t)A[8 * kc + 1] << 16);
+        wa.y = A[8 * kc + 2] | ((uint32_t)A[8 * kc + 3] << 16);
+        wa.z = A[8 * kc + 4] | ((uint32_t)A[8 * kc + 5] << 16);
+        wa.w = A[8 * kc + 6] | ((uint32_t)A[8 * kc + 7] << 16);
+        wb.x = Bv[8 * kc] | ((uint32_t)Bv[8 * kc + 1] << 16);
+        wb.y = Bv[8 * kc + 2] | ((uint32_t)Bv[8 * kc + 3] << 16);
+        wb.z = Bv[8 * kc + 4] | ((uint32_t)Bv[8 * kc + 5] << 16);
+        wb.w = Bv[8 * kc + 6] | ((uint32_t)Bv[8 * kc + 7] << 16);
+        *reinterpret_cast<uint4 *>(dA + (size_t)kc * 128 * 16) = wa;
+        *reinterpret_cast<uint4 *>(dB + (size_t)kc * 256 * 16) = wb;
+    }
+
+    // block summary
+    const double inf = __longlong_as_double(0x7FF0000000000000LL);
+    double tmn = valid ? x[0] : inf, tmx = valid ? x[0] : -inf;
+    bool sorted = true;                                   // this point <= the next one (fp64; NaN: false)
+    if (valid && gp + 1 < N) sorted = x[0] <= coords[(gp + 1) * DIM];
+#pragma unroll
+    for (int s = 16; s >= 1; s >>= 1) {
+        tmn = fmin(tmn, __shfl_xor_sync(0xffffffffu, tmn, s));
+        tmx = fmax(tmx, __shfl_xor_sync(0xffffffffu, tmx, s));
+        c = fmaxf(c, __shfl_xor_sync(0xffffffffu, c, s));
+    }
+    __shared__ double s_mn[4], s_mx[4];
+    __shared__ float s_c[4];
+    if (lane == 0) { s_mn[warp] = tmn; s_mx[warp] = tmx; s_c[warp] = c; }
+    const int inner = __syncthreads_and(sorted || tid == 127);
+    const int link = __syncthreads_and(sorted || tid != 127);
+    const int bad = __syncthreads_or(!ok);
+    if (tid == 0) {
+        TcBlockInfo bi;
+        bi.tmin = fmin(fmin(s_mn[0], s_mn[1]), fmin(s_mn[2], s_mn[3]));
+        bi.tmax = fmax(fmax(s_mx[0], s_mx[1]), fmax(s_mx[2], s_mx[3]));
+        bi.C = fmaxf(fmaxf(s_c[0], s_c[1]), fmaxf(s_c[2], s_c[3]));
+        bi.flags = (inner ? 1u : 0u) | (link ? 2u : 0u) | (bad ? 4u : 0u);
+        bi.pad[0] = bi.pad[1] = 0;
+        info[(size_t)b * nA + a] = bi;
+    }
+}
+
+// ---- tile table ------------------------------------------------------------------------------------
+// One entry per tile of the launch, row-major over the upper triangle (J >= I) of every causet:
+//   x = I | J << 16, y = causet, z = margin m (float bits; +inf: every row of the tile goes to fp64), w = unused.
+__global__ void __launch_bounds__(256)
+k_tc_tiles(const TcBlockInfo *__restrict__ info, int nT, uint32_t tiles_per, uint32_t total_tiles, uint4 *__restrict__ tab)
+{
+    const uint32_t t = blockIdx.x * 256 + threadIdx.x;
+    if (t >= total_tiles) return;
+    const uint32_t b = t / tiles_per, idx = t - b * tiles_per;
+    const double w = 2.0 * nT + 1.0;
+    int I = (int)((w - sqrt(w * w - 8.0 * (double)idx)) * 0.5);
+    if (I < 0) I = 0;
+    if (I > nT - 1) I = nT - 1;
+    auto off = [&](int r) { return (uint32_t)r * (uint32_t)nT - (uint32_t)((int64_t)r * (r - 1) / 2); };
+    while (I > 0 && off(I) > idx) I--;
+    while (I + 1 < nT && off(I + 1) <= idx) I++;
+    const int J = I + (int)(idx - off(I));
+    const TcBlockInfo *bi = info + (size_t)b * 2 * nT;
+    const TcBlockInfo i0 = bi[2 * I], i1 = bi[2 * I + 1], j0 = bi[2 * J], j1 = bi[2 * J + 1];
+    const float C = fmaxf(fmaxf(i0.C, i1.C), fmaxf(j0.C, j1.C));
+    const bool bad = ((i0.flags | i1.flags | j0.flags | j1.flags) & 4u) != 0;
+    const bool ordered = (I == J) ? ((i0.flags & 3u) == 3u && (i1.flags & 1u) != 0)
+                                  : (fmax(i0.tmax, i1.tmax) <= fmin(j0.tmin, j1.tmin));
+    const bool fast = !bad && ordered && C >= 0x1p-40f && C <= 0x1p40f;
+    const float m = fast ? __fmul_ru(__fmul_ru(C, C), 1.001f * exp2f((float)TC_MARGIN_LOG2)) : __int_as_float(0x7f800000);
+    tab[t] = make_uint4((uint32_t)I | ((uint32_t)J << 16), b, __float_as_uint(m), __float_as_uint(C));
+}
+
+// ---- main kernel -----------------------------------------------------------------------------------
+struct TcProbe {                 // cs_a1_tensor_probe: what the prefilter saw (all tiles of the launch)
+    unsigned int max_err_bits;   // max |a - T| / C^2 as float bits (pairs decided by sign)
+    unsigned int pad;
+    unsigned long long rows_fp64;   // (row, 32-column block) pairs re-evaluated in fp64
+    unsigned long long rows_total;  // (row, block) pairs examined
+};
+
+// wait with back-off, for the two single-thread roles (their polling would otherwise take issue slots from the
+// epilogue warps of their scheduler)
+__device__ __forceinline__ void tc_mbar_wait_idle(uint64_t *bar, uint32_t parity)
+{
+    uint32_t done = 0;
+    while (true) {
+        asm volatile(
+            "{\n"
+            ".reg .pred p;\n"
+            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n"
+            "selp.u32 %0, 1, 0, p;\n"
+            "}\n" : "=r"(done) : "r"(tc_smem_u32(bar)), "r"(parity) : "memory");
+        if (done) break;
+        __nanosleep(200);
+    }
+}
+
+template <int GEOM, int DIM>
+struct TcSmem {
+    using S = TcShape<GEOM, DIM>;
+    static constexpr int NSTG = S::K == 32 ? 3 : 2;                 // operand stages (one tile each)
+    static constexpr int COORD = TCT * DIM * 8;                     // fp64 coordinates of 256 points (for the fp64 rows)
+    static constexpr int STAGE = S::STAGE + 2 * COORD;              // [A 2 blocks][B][coords I][coords J]
+    static constexpr size_t STAGING = (size_t)NSTG * STAGE;         // uint32 [2][256][TC_PITCH] x 2 (U, L)
+    static constexpr size_t BARS = STAGING + 4 * TCT * TC_PITCH * 4;
+    static constexpr size_t BYTES = BARS + (2 * NSTG + 8) * 8 + 16;
+    static_assert(STAGE % 16 == 0 && BYTES <= 227 * 1024, "k_causal_tc: shared memory");
+};
+
+template <int GEOM, int DIM, bool PROBE>
+__global__ void __launch_bounds__(TC_THREADS, 1)
+k_causal_tc(const double *__restrict__ cpad, const unsigned char *__restrict__ opA,
+            const unsigned char *__restrict__ opB, const uint4 *__restrict__ tab,
+            int64_t N, int64_t stride, int nT, uint32_t total_tiles,
+            uint64_t *__restrict__ bits, uint64_t *__restrict__ bitsT, TcProbe *__restrict__ probe)
+{
+    using S = TcShape<GEOM, DIM>;
+    using SM = TcSmem<GEOM, DIM>;
+    constexpr int NSTG = SM::NSTG;
+    extern __shared__ __align__(1024) unsigned char smem[];
+    unsigned char *s_stage = smem;
+    uint32_t *s_U = reinterpret_cast<uint32_t *>(smem + SM::STAGING);                    // [2][256][TC_PITCH]
+    uint32_t *s_L = s_U + 2 * TCT * TC_PITCH;                                            // [2][256][TC_PITCH]
+    uint64_t *s_full = reinterpret_cast<uint64_t *>(smem + SM::BARS);                    // [NSTG] operands landed
+    uint64_t *s_empty = s_full + NSTG;                                                   // [NSTG] stage free again
+    uint64_t *s_tfull = s_empty + NSTG;                                                  // [2] accumulator complete
+    uint64_t *s_tempty = s_tfull + 2;                                                    // [2] accumulator drained
+    uint64_t *s_sfull = s_tempty + 2;                                                    // [2] staged tile complete
+    uint64_t *s_sempty = s_sfull + 2;                                                    // [2] staged tile written out
+    uint32_t *s_tmem = reinterpret_cast<uint32_t *>(s_sempty + 2);
+
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const int nA = 2 * nT;
+
+    if (tid == 0) {
+        for (int s = 0; s < NSTG; s++) {
+            tc_mbar_init(&s_full[s], 1);
+            tc_mbar_init(&s_empty[s], 1 + TC_EPI_WARPS);      // the MMAs (commit) and every epilogue warp (fp64 rows read the coordinates)
+        }
+        for (int h = 0; h < 2; h++) {
+            tc_mbar_init(&s_tfull[h], 1);
+            tc_mbar_init(&s_tempty[h], TC_EPI_WARPS);
+            tc_mbar_init(&s_sfull[h], TC_EPI_WARPS);
+            tc_mbar_init(&s_sempty[h], TC_WR_WARPS);
+        }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    if (warp == 1) {
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 512;" ::"r"(tc_smem_u32(s_tmem)));
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
+    }
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    const uint32_t tmem_base = *s_tmem;
+
+    if (warp == 0) {
+        // ===================================== loader =========================================
+        if (lane == 0) {
+            uint32_t n = 0;
+            for (uint32_t t = blockIdx.x; t < total_tiles; t += gridDim.x, n++) {
+                const uint4 e = __ldg(tab + t);
+                const uint32_t I = e.x & 0xFFFFu, J = e.x >> 16, b = e.y;
+                const uint32_t s = n % NSTG;
+                tc_mbar_wait_idle(&s_empty[s], ((n / NSTG) & 1) ^ 1);
+                tc_mbar_expect_tx(&s_full[s], (uint32_t)SM::STAGE);
+                unsigned char *dst = s_stage + (size_t)s * SM::STAGE;
+                const unsigned char *cp = reinterpret_cast<const unsigned char *>(cpad) + (size_t)b * nT * SM::COORD;
+                tc_bulk_g2s(dst, opA + ((size_t)b * nA + 2 * I) * S::A_BLOCK, 2 * S::A_BLOCK, &s_full[s]);
+                tc_bulk_g2s(dst + 2 * S::A_BLOCK, opB + ((size_t)b * nT + J) * S::B_BLOCK, S::B_BLOCK, &s_full[s]);
+                tc_bulk_g2s(dst + S::STAGE, cp + (size_t)I * SM::COORD, SM::COORD, &s_full[s]);
+                tc_bulk_g2s(dst + S::STAGE + SM::COORD, cp + (size_t)J * SM::COORD, SM::COORD, &s_full[s]);
+            }
+        }
+    } else if (warp == 1) {
+        // ===================================== MMA issuer =====================================
+        if (lane == 0) {
+            uint32_t n = 0;
+            for (uint32_t t = blockIdx.x; t < total_tiles; t += gridDim.x, n++) {
+                const uint32_t s = n % NSTG;
+                tc_mbar_wait_idle(&s_full[s], (n / NSTG) & 1);
+                const uint32_t a_addr = tc_smem_u32(s_stage + (size_t)s * SM::STAGE);
+                const uint32_t b_addr = a_addr + 2 * S::A_BLOCK;
+#pragma unroll
+                for (int h = 0; h < 2; h++) {
+                    tc_mbar_wait_idle(&s_tempty[h], (n & 1) ^ 1);     // the epilogue has read accumulator h of the tile before
+                    tc_fence_after();
+#pragma unroll
+                    for (int q = 0; q < S::KC / 2; q++) {             // K = 16 per instruction: two 16-byte chunks
+                        const uint64_t ad = tc_desc(a_addr + h * S::A_BLOCK + q * 2 * 128 * 16, 128 * 16, 128);
+                        const uint64_t bd = tc_desc(b_addr + q * 2 * 256 * 16, 256 * 16, 128);
+                        tc_mma_bf16(tmem_base + h * 256, ad, bd, q > 0 ? 1u : 0u);
+                    }
+                    tc_commit(&s_tfull[h]);
+                }
+                tc_commit(&s_empty[s]);
+            }
+        }
+    } else if (warp < TC_WR0) {
+        // ===================================== epilogue =======================================
+        const int e = warp - TC_EPI0;
+        const int q = warp & 3;                       // TMEM lane quarter this warp may read
+        const int g = e >> 2;                         // 64 columns of the 256
+        const TransposeLane transpose(lane);
+        uint32_t n = 0;
+        float p_err = 0.f;
+        unsigned long long p_rows = 0, p_tot = 0;
+        uint2 ent = blockIdx.x < total_tiles ? __ldg(reinterpret_cast<const uint2 *>(tab + blockIdx.x)) : make_uint2(0, 0);
+        uint32_t ent_m = blockIdx.x < total_tiles ? __ldg(reinterpret_cast<const uint32_t *>(tab + blockIdx.x) + 2) : 0;
+        for (uint32_t t = blockIdx.x; t < total_tiles; t += gridDim.x, n++) {
+            const bool diag = (ent.x & 0xFFFFu) == (ent.x >> 16);
+            const float m = __uint_as_float(ent_m);
+            float C2 = 0.f;
+            if (PROBE) {
+                const float C = __uint_as_float(__ldg(reinterpret_cast<const uint32_t *>(tab + t) + 3));
+                C2 = C * C;
+            }
+            if (t + gridDim.x < total_tiles) {                     // next tile's entry, a tile ahead
+                ent = __ldg(reinterpret_cast<const uint2 *>(tab + t + gridDim.x));
+                ent_m = __ldg(reinterpret_cast<const uint32_t *>(tab + t + gridDim.x) + 2);
+            }
+            const uint32_t s = n % NSTG;
+            const double *cI = reinterpret_cast<const double *>(s_stage + (size_t)s * SM::STAGE + S::STAGE);
+            const double *cJ = cI + TCT * DIM;
+            uint32_t *U = s_U + (n & 1) * TCT * TC_PITCH, *L = s_L + (n & 1) * TCT * TC_PITCH;
+            tc_mbar_wait(&s_sempty[n & 1], ((n >> 1) & 1) ^ 1);    // the writers are done with this staging buffer
+
+            auto do_tile = [&](auto diag_tag) {
+                constexpr bool DIAG = decltype(diag_tag)::value;
+#pragma unroll 1
+                for (int h = 0; h < 2; h++) {
+                    const int r0 = h * 128 + q * 32;                  // first row of this warp's blocks (tile-local)
+                    tc_mbar_wait(&s_tfull[h], n & 1);
+                    tc_fence_after();
+                    const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + h * 256 + g * 64;
+#pragma unroll 1
+                    for (int k = 0; k < 2; k++) {
+                        const int c0 = g * 64 + k * 32;               // first column of the block (tile-local)
+                        uint32_t lw = 0;
+                        if (!(DIAG && c0 + 31 <= r0)) {               // (a block at or below the diagonal stays 0)
+                            uint32_t v[32];
+                            tc_ld32(taddr + k * 32, v);
+                            asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+                            uint32_t sg = 0;
+                            float mn = __int_as_float(0x7f800000);
+#pragma unroll
+                            for (int c = 31; c >= 1; c -= 2) {
+                                sg = __funnelshift_l(v[c], sg, 1);
+                                sg = __funnelshift_l(v[c - 1], sg, 1);
+                                mn = min3_abs_nan(mn, v[c], v[c - 1]);
+                            }
+                            lw = ~sg;                                 // related = sign bit clear (valid outside the band)
+                            const bool unc = !(mn > m);               // NaN compares false: uncertain
+                            uint32_t todo = __ballot_sync(0xffffffffu, unc);
+                            if (PROBE) {
+                                p_tot++;
+                                p_rows += unc ? 1 : 0;
+                                if (GEOM == CS_GEOM_MINK_CONE && !unc) {
+#pragma unroll
+                                    for (int c = 0; c < 32; c++) {
+                                        double T = 0.0;
+#pragma unroll
+                                        for (int d = 0; d < DIM; d++) {
+                                            const double dd = cJ[(c0 + c) * DIM + d] - cI[(r0 + lane) * DIM + d];
+                                            T += d == 0 ? dd * dd : -dd * dd;
+                                        }
+                                        const float er = (float)(fabs((double)__uint_as_float(v[c]) - 0.5 * T) / (double)C2);
+                                        if (er == er) p_err = fmaxf(p_err, er);      // (padding points are NaN)
+                                    }
+                                }
+                            }
+                            while (todo) {                            // fp64 for whole rows of the block, one pair per lane
+                                const int r = __ffs(todo) - 1;
+                                todo &= todo - 1;
+                                double xi[DIM], xj[DIM];
+#pragma unroll
+                                for (int d = 0; d < DIM; d++) {
+                                    xi[d] = cI[(r0 + r) * DIM + d];   // (points beyond N are NaN: unrelated)
+                                    xj[d] = cJ[(c0 + lane) * DIM + d];
+                                }
+                                const uint32_t w = __ballot_sync(0xffffffffu, Pred<GEOM, DIM>::rel(xi, xj));
+                                if (lane == r) lw = w;
+                            }
+                            if (DIAG) {                               // only i < j inside the diagonal tile
+                                const int keep_from = r0 + lane + 1 - c0;          // columns c >= keep_from are kept
+                                lw &= keep_from <= 0 ? 0xffffffffu : (keep_from >= 32 ? 0u : (0xffffffffu << keep_from));
+                            }
+                        }
+                        U[(r0 + lane) * TC_PITCH + (c0 >> 5)] = lw;                   // future of i: bit = column j
+                        L[(c0 + lane) * TC_PITCH + (r0 >> 5)] = transpose(lw);        // past of j: bit = row i
+                    }
+                    tc_fence_before();
+                    __syncwarp();
+                    if (lane == 0) tc_mbar_arrive(&s_tempty[h]);      // accumulator h may be overwritten
+                }
+            };
+            if (diag) do_tile(std::true_type{});
+            else do_tile(std::false_type{});
+            __syncwarp();
+            if (lane == 0) {
+                tc_mbar_arrive(&s_empty[s]);          // this warp no longer reads the stage's coordinates
+                tc_mbar_arrive(&s_sfull[n & 1]);      // its part of the staged tile is complete
+            }
+        }
+        if (PROBE) {
+#pragma unroll
+            for (int sft = 16; sft >= 1; sft >>= 1) {
+                p_err = fmaxf(p_err, __shfl_xor_sync(0xffffffffu, p_err, sft));
+                p_rows += __shfl_xor_sync(0xffffffffu, p_rows, sft);
+                p_tot += __shfl_xor_sync(0xffffffffu, p_tot, sft);
+            }
+            if (lane == 0) {
+                atomicMax(&probe->max_err_bits, __float_as_uint(p_err));
+                atomicAdd(&probe->rows_fp64, p_rows);
+                atomicAdd(&probe->rows_total, p_tot);
+            }
+        }
+    } else {
+        // ===================================== writers ========================================
+        // 64 threads move a staged tile to global memory: thread = (row mod 32, 16-byte half of the 32-byte segment),
+        // eight rows each; the mirrored tile of an off-diagonal tile is written as zeros.
+        const int wt = tid - TC_WR0 * 32;             // 0 .. 63
+        const int hf = wt & 1, rr = wt >> 1;
+        const int64_t row_bytes = stride * 8;
+        const uint4 zero = make_uint4(0, 0, 0, 0);
+        uint32_t n = 0;
+        for (uint32_t t = blockIdx.x; t < total_tiles; t += gridDim.x, n++) {
+            const uint4 e = __ldg(tab + t);
+            const int I = (int)(e.x & 0xFFFFu), J = (int)(e.x >> 16);
+            const int64_t colI = (int64_t)I * 32 + hf * 16, colJ = (int64_t)J * 32 + hf * 16;      // byte offsets in a row
+            const size_t mat = (size_t)e.y * N * row_bytes;
+            unsigned char *pb = reinterpret_cast<unsigned char *>(bits) + mat;
+            unsigned char *pt = bitsT ? reinterpret_cast<unsigned char *>(bitsT) + mat : nullptr;
+            const bool okI = colI < row_bytes, okJ = colJ < row_bytes, off = I != J;
+            const uint32_t *u = s_U + (n & 1) * TCT * TC_PITCH + rr * TC_PITCH + hf * 4;
+            const uint32_t *l = s_L + (n & 1) * TCT * TC_PITCH + rr * TC_PITCH + hf * 4;
+            int64_t gi = (int64_t)I * TCT + rr, gj = (int64_t)J * TCT + rr;
+            size_t oi = (size_t)gi * row_bytes, oj = (size_t)gj * row_bytes;
+            tc_mbar_wait(&s_sfull[n & 1], (n >> 1) & 1);
+#pragma unroll 4
+            for (int p = 0; p < 8; p++) {
+                if (gi < N && okJ) {
+                    *reinterpret_cast<uint4 *>(pb + oi + colJ) = make_uint4(u[0], u[1], u[2], u[3]);
+                    if (pt && off) *reinterpret_cast<uint4 *>(pt + oi + colJ) = zero;
+                }
+                if (gj < N && okI) {
+                    if (pt) *reinterpret_cast<uint4 *>(pt + oj + colI) = make_uint4(l[0], l[1], l[2], l[3]);
+                    if (off) *reinterpret_cast<uint4 *>(pb + oj + colI) = zero;
+                }
+                u += 32 * TC_PITCH;
+                l += 32 * TC_PITCH;
+                gi += 32;
+                gj += 32;
+                oi += 32 * (size_t)row_bytes;
+                oj += 32 * (size_t)row_bytes;
+            }
+            __syncwarp();
+            if (lane == 0) tc_mbar_arrive(&s_sempty[n & 1]);
+        }
+    }
+
+    tc_fence_before();
+    __syncthreads();
+    if (warp == 1) {
+        asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, 512;" ::"r"(tmem_base));
+    }
+}
+
+template <int GEOM, int DIM>
+size_t tc_scratch_t(int64_t B, int64_t N)
+{
+    using S = TcShape<GEOM, DIM>;
+    const size_t nT = (size_t)((N + TCT - 1) / TCT);
+    const size_t tiles = (size_t)B * (nT * (nT + 1) / 2);
+    return align_up((size_t)B * 2 * nT * S::A_BLOCK, 256) + align_up((size_t)B * nT * S::B_BLOCK, 256) +
+           align_up((size_t)B * 2 * nT * sizeof(TcBlockInfo), 256) + align_up((size_t)B * nT * TCT * DIM * 8, 256) +
+           align_up(tiles * sizeof(uint4), 256);
+}
+
+template <int GEOM, int DIM, bool PROBE>
+int launch_tc_t(const double *coords, int64_t B, int64_t N, int64_t stride, uint64_t *bits, uint64_t *bitsT,
+                void *scratch, TcProbe *probe, cudaStream_t st)
+{
+    using S = TcShape<GEOM, DIM>;
+    const int nT = (int)((N + TCT - 1) / TCT);
+    const int64_t tiles_per = (int64_t)nT * (nT + 1) / 2;
+    if (nT > 32768 || B > 65535 || tiles_per * B >= ((int64_t)1 << 32)) return CS_ERR_ARG;
+    using SM = TcSmem<GEOM, DIM>;
+    const int64_t total = tiles_per * B;
+    unsigned char *opA = static_cast<unsigned char *>(scratch);
+    unsigned char *opB = opA + align_up((size_t)B * 2 * nT * S::A_BLOCK, 256);
+    TcBlockInfo *info = reinterpret_cast<TcBlockInfo *>(opB + align_up((size_t)B * nT * S::B_BLOCK, 256));
+    double *cpad = reinterpret_cast<double *>(reinterpret_cast<unsigned char *>(info) + align_up((size_t)B * 2 * nT * sizeof(TcBlockInfo), 256));
+    uint4 *tab = reinterpret_cast<uint4 *>(reinterpret_cast<unsigned char *>(cpad) + align_up((size_t)B * nT * TCT * DIM * 8, 256));
+    k_tc_prep<GEOM, DIM><<<dim3(2 * nT, (unsigned)B), 128, 0, st>>>(coords, N, 2 * nT, opA, opB, info, cpad);
+    CS_LAUNCHED("k_tc_prep");
+    k_tc_tiles<<<(unsigned)((total + 255) / 256), 256, 0, st>>>(info, nT, (uint32_t)tiles_per, (uint32_t)total, tab);
+    CS_LAUNCHED("k_tc_tiles");
+    constexpr size_t smem = SM::BYTES;
+    static PerDeviceFlag attr_set;
+    const int dev = current_device();
+    if (!attr_set.get(dev)) {
+        CS_CUDA(cudaFuncSetAttribute(k_causal_tc<GEOM, DIM, PROBE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        attr_set.set(dev);
+    }
+    int grid = sm_count();
+    if (grid > total) grid = (int)total;
+    k_causal_tc<GEOM, DIM, PROBE><<<grid, TC_THREADS, smem, st>>>(cpad, opA, opB, tab, N, stride, nT, (uint32_t)total,
+                                                                  bits, bitsT, probe);
+    CS_LAUNCHED("k_causal_tc");
+    return CS_OK;
+}
+
+}  // namespace
+
+bool causal_tc_supported(int geometry, int dim)
+{
+    if (!interval_tensor_available()) return false;      // tcgen05: compute capability 10.x
+    switch (geometry) {
+    case CS_GEOM_MINK_CONE: return dim >= 2 && dim <= 5;
+    case CS_GEOM_FLRW_POLAR: return dim == 6;
+    case CS_GEOM_DS4_SPHERICAL: return dim == 7;
+    default: return false;
+    }
+}
+
+#define CS_TC_DISPATCH(CALL)                                                                       \
+    switch (geometry) {                                                                            \
+    case CS_GEOM_MINK_CONE:                                                                        \
+        if (dim == 2) return CALL(CS_GEOM_MINK_CONE, 2);                                           \
+        if (dim == 3) return CALL(CS_GEOM_MINK_CONE, 3);                                           \
+        if (dim == 4) return CALL(CS_GEOM_MINK_CONE, 4);                                           \
+        if (dim == 5) return CALL(CS_GEOM_MINK_CONE, 5);                                           \
+        break;                                                                                     \
+    case CS_GEOM_FLRW_POLAR:                                                                       \
+        if (dim == 6) return CALL(CS_GEOM_FLRW_POLAR, 6);                                          \
+        break;                                                                                     \
+    case CS_GEOM_DS4_SPHERICAL:                                                                    \
+        if (dim == 7) return CALL(CS_GEOM_DS4_SPHERICAL, 7);                                       \
+        break;                                                                                     \
+    default:                                                                                       \
+        break;                                                                                     \
+    }
+
+size_t causal_tc_scratch_bytes(int64_t B, int64_t N, int dim, int geometry)
+{
+#define CS_TC_SCRATCH(G, D) tc_scratch_t<G, D>(B, N)
+    CS_TC_DISPATCH(CS_TC_SCRATCH)
+#undef CS_TC_SCRATCH
+    return 0;
+}
+
+int launch_causal_tc(const double *coords, int64_t B, int64_t N, int dim, int geometry,
+                     uint64_t *bits, uint64_t *bitsT, void *scratch, cudaStream_t st)
+{
+    const int64_t stride = row_stride_words(N);
+#define CS_TC_LAUNCH(G, D) launch_tc_t<G, D, false>(coords, B, N, stride, bits, bitsT, scratch, nullptr, st)
+    CS_TC_DISPATCH(CS_TC_LAUNCH)
+#undef CS_TC_LAUNCH
+    return CS_ERR_GEOM;
+}
+
+// The same launch with the probe counters switched on (flat cone in 3+1 and 4+1 dimensions: K = 32 and K = 48).
+// out_host: [0] largest |a - T| / (2^-24 C^2) over the pairs decided by sign, [1] (row, block) pairs sent to fp64,
+// [2] (row, block) pairs examined, [3] the margin in the same unit.
+int launch_causal_tc_probe(const double *coords, int64_t N, int dim, uint64_t *bits, uint64_t *bitsT,
+                           void *scratch, double *out_host, cudaStream_t st)
+{
+    const int64_t stride = row_stride_words(N);
+    TcProbe *dp = nullptr;
+    CS_CUDA(cudaMallocAsync(reinterpret_cast<void **>(&dp), sizeof(TcProbe), st));
+    CS_CUDA(cudaMemsetAsync(dp, 0, sizeof(TcProbe), st));
+    int rc = CS_ERR_DIM;
+    if (dim == 4) rc = launch_tc_t<CS_GEOM_MINK_CONE, 4, true>(coords, 1, N, stride, bits, bitsT, scratch, dp, st);
+    if (dim == 5) rc = launch_tc_t<CS_GEOM_MINK_CONE, 5, true>(coords, 1, N, stride, bits, bitsT, scratch, dp, st);
+    TcProbe hp;
+    memset(&hp, 0, sizeof(hp));
+    if (rc == CS_OK) {
+        CS_CUDA(cudaMemcpyAsync(&hp, dp, sizeof(hp), cudaMemcpyDeviceToHost, st));
+        CS_CUDA(cudaStreamSynchronize(st));
+    }
+    cudaFreeAsync(dp, st);
+    if (rc) return rc;
+    float err;
+    memcpy(&err, &hp.max_err_bits, 4);
+    out_host[0] = (double)err * 16777216.0;
+    out_host[1] = (double)hp.rows_fp64;
+    out_host[2] = (double)hp.rows_total;
+    out_host[3] = ldexp(1.0, 24 + TC_MARGIN_LOG2);
+    return CS_OK;
+}
+
+}  // namespace cs

@@ -79,8 +79,17 @@ struct IntervalStats {
 static_assert(sizeof(IntervalStats) <= 256, "stats block");
 
 // ---- stage launchers (defined in the .cu files) ---------------------------------------------
-int launch_causal_matrix(const double *coords, int64_t B, int64_t N, int dim, int geometry,
-                         uint64_t *bits, uint64_t *bitsT, cudaStream_t st);
+// a1.  route: CS_A1_AUTO / CS_A1_FMA / CS_A1_TENSOR; scratch (device, causal_matrix_scratch_bytes) may be NULL: the
+// tensor route then takes it from the library's stream-ordered pool.
+int launch_causal_matrix(const double *coords, int64_t B, int64_t N, int dim, int geometry, int route,
+                         uint64_t *bits, uint64_t *bitsT, void *scratch, size_t scratch_bytes, cudaStream_t st);
+size_t causal_matrix_scratch_bytes(int64_t B, int64_t N, int dim, int geometry, int route);
+bool causal_tc_supported(int geometry, int dim);
+size_t causal_tc_scratch_bytes(int64_t B, int64_t N, int dim, int geometry);
+int launch_causal_tc(const double *coords, int64_t B, int64_t N, int dim, int geometry,
+                     uint64_t *bits, uint64_t *bitsT, void *scratch, cudaStream_t st);
+int launch_causal_tc_probe(const double *coords, int64_t N, int dim, uint64_t *bits, uint64_t *bitsT,
+                           void *scratch, double *out_host, cudaStream_t st);
 int launch_transpose_bits(const uint64_t *bits, int64_t B, int64_t N, uint64_t *bitsT, cudaStream_t st);
 int launch_degrees(const uint64_t *bits, const uint64_t *bitsT, int64_t N, int64_t *outdeg, int64_t *indeg, cudaStream_t st);
 int launch_relation_stats(const uint64_t *bits, int64_t N, int64_t *out, cudaStream_t st);
