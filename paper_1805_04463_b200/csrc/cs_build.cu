@@ -476,7 +476,7 @@ constexpr int64_t TC_MIN_PAIRS = (int64_t)1 << 21;      // B * N^2 / 2 pairs: 20
 static int resolve_a1_route(int64_t B, int64_t N, int dim, int geometry, int route)
 {
     if (route == CS_A1_FMA) return CS_A1_FMA;
-    const bool can = causal_tc_supported(geometry, dim) && N >= 1;
+    const bool can = causal_tc_supported(geometry, dim) && N >= 256;      // (rows of at least 32 bytes: TMA boxes)
     if (route == CS_A1_TENSOR) return can ? CS_A1_TENSOR : -1;
     return can && B * N * N / 2 >= TC_MIN_PAIRS ? CS_A1_TENSOR : CS_A1_FMA;
 }

@@ -33,6 +33,7 @@
 // shifts the 32 sign bits of its row into one word (one SHF per pair), keeps min |a| (one FMNMX3 per two pairs),
 // transposes the 32 x 32 bit block with the shuffle butterfly for the second output, and stages both in shared
 // memory; a 256 x 256 tile leaves as full 32-byte row segments, mirrored zero tiles included.
+#include <cuda.h>
 #include <cuda_bf16.h>
 
 #include <type_traits>
@@ -40,6 +41,9 @@
 #include "cs_predicates.cuh"
 
 namespace cs {
+
+int bits_tensor_map(CUtensorMap *map, const uint64_t *base, int64_t B, int64_t N, int64_t stride, int box_bytes, int rows,
+                    bool swizzle64);      // cs_interval_pair.cu
 
 namespace {
 
@@ -51,6 +55,9 @@ constexpr int TC_WR_WARPS = 2;
 constexpr int TC_THREADS = (TC_WR0 + TC_WR_WARPS) * 32;
 constexpr int TC_PITCH = 9;              // words per staged row (8 + 1: conflict-free 4-byte stores by 32 rows)
 constexpr int TC_MARGIN_LOG2 = -14;      // m = 2^-14 C^2
+#ifndef TC_NF
+#define TC_NF 12                         // columns of a 32 x 32 block whose sign bit goes through the FMA pipe (0 .. 23)
+#endif
 
 template <int GEOM, int DIM>
 struct TcShape {
@@ -82,18 +89,20 @@ __device__ __forceinline__ void tc_mbar_arrive(uint64_t *bar)
 {
     asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(tc_smem_u32(bar)) : "memory");
 }
+// try_wait with a suspend-time hint: the thread sleeps in hardware until the phase completes (or the hint expires)
+// instead of spinning through issue slots the epilogue warps need
 __device__ __forceinline__ void tc_mbar_wait(uint64_t *bar, uint32_t parity)
 {
     asm volatile(
         "{\n"
         ".reg .pred p;\n"
         "LAB_WAIT:\n"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1, %2;\n"
         "@p bra LAB_DONE;\n"
         "bra LAB_WAIT;\n"
         "LAB_DONE:\n"
         "}\n" ::"r"(tc_smem_u32(bar)),
-        "r"(parity)
+        "r"(parity), "r"(0x989680u)
         : "memory");
 }
 __device__ __forceinline__ void tc_mbar_expect_tx(uint64_t *bar, uint32_t bytes)
@@ -334,23 +343,6 @@ struct TcProbe {                 // cs_a1_tensor_probe: what the prefilter saw (
     unsigned long long rows_total;  // (row, block) pairs examined
 };
 
-// wait with back-off, for the two single-thread roles (their polling would otherwise take issue slots from the
-// epilogue warps of their scheduler)
-__device__ __forceinline__ void tc_mbar_wait_idle(uint64_t *bar, uint32_t parity)
-{
-    uint32_t done = 0;
-    while (true) {
-        asm volatile(
-            "{\n"
-            ".reg .pred p;\n"
-            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n"
-            "selp.u32 %0, 1, 0, p;\n"
-            "}\n" : "=r"(done) : "r"(tc_smem_u32(bar)), "r"(parity) : "memory");
-        if (done) break;
-        __nanosleep(200);
-    }
-}
-
 template <int GEOM, int DIM>
 struct TcSmem {
     using S = TcShape<GEOM, DIM>;
@@ -358,14 +350,16 @@ struct TcSmem {
     static constexpr int COORD = TCT * DIM * 8;                     // fp64 coordinates of 256 points (for the fp64 rows)
     static constexpr int STAGE = S::STAGE + 2 * COORD;              // [A 2 blocks][B][coords I][coords J]
     static constexpr size_t STAGING = (size_t)NSTG * STAGE;         // uint32 [2][256][TC_PITCH] x 2 (U, L)
-    static constexpr size_t BARS = STAGING + 4 * TCT * TC_PITCH * 4;
+    static constexpr size_t ZERO = STAGING + 4 * TCT * TC_PITCH * 4;   // 256 x 32 bytes of zeros (source of the mirrored tiles)
+    static constexpr size_t BARS = ZERO + TCT * 32;
     static constexpr size_t BYTES = BARS + (2 * NSTG + 8) * 8 + 16;
     static_assert(STAGE % 16 == 0 && BYTES <= 227 * 1024, "k_causal_tc: shared memory");
 };
 
 template <int GEOM, int DIM, bool PROBE>
 __global__ void __launch_bounds__(TC_THREADS, 1)
-k_causal_tc(const double *__restrict__ cpad, const unsigned char *__restrict__ opA,
+k_causal_tc(const __grid_constant__ CUtensorMap mapB, const __grid_constant__ CUtensorMap mapT,
+            const double *__restrict__ cpad, const unsigned char *__restrict__ opA,
             const unsigned char *__restrict__ opB, const uint4 *__restrict__ tab,
             int64_t N, int64_t stride, int nT, uint32_t total_tiles,
             uint64_t *__restrict__ bits, uint64_t *__restrict__ bitsT, TcProbe *__restrict__ probe)
@@ -401,6 +395,8 @@ k_causal_tc(const double *__restrict__ cpad, const unsigned char *__restrict__ o
         }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
+    for (int i = tid; i < TCT * 32 / 16; i += TC_THREADS) reinterpret_cast<uint4 *>(smem + SM::ZERO)[i] = make_uint4(0, 0, 0, 0);
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");      // read by TMA stores
     if (warp == 1) {
         asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], 512;" ::"r"(tc_smem_u32(s_tmem)));
         asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
@@ -418,7 +414,7 @@ k_causal_tc(const double *__restrict__ cpad, const unsigned char *__restrict__ o
                 const uint4 e = __ldg(tab + t);
                 const uint32_t I = e.x & 0xFFFFu, J = e.x >> 16, b = e.y;
                 const uint32_t s = n % NSTG;
-                tc_mbar_wait_idle(&s_empty[s], ((n / NSTG) & 1) ^ 1);
+                tc_mbar_wait(&s_empty[s], ((n / NSTG) & 1) ^ 1);
                 tc_mbar_expect_tx(&s_full[s], (uint32_t)SM::STAGE);
                 unsigned char *dst = s_stage + (size_t)s * SM::STAGE;
                 const unsigned char *cp = reinterpret_cast<const unsigned char *>(cpad) + (size_t)b * nT * SM::COORD;
@@ -434,12 +430,12 @@ k_causal_tc(const double *__restrict__ cpad, const unsigned char *__restrict__ o
             uint32_t n = 0;
             for (uint32_t t = blockIdx.x; t < total_tiles; t += gridDim.x, n++) {
                 const uint32_t s = n % NSTG;
-                tc_mbar_wait_idle(&s_full[s], (n / NSTG) & 1);
+                tc_mbar_wait(&s_full[s], (n / NSTG) & 1);
                 const uint32_t a_addr = tc_smem_u32(s_stage + (size_t)s * SM::STAGE);
                 const uint32_t b_addr = a_addr + 2 * S::A_BLOCK;
 #pragma unroll
                 for (int h = 0; h < 2; h++) {
-                    tc_mbar_wait_idle(&s_tempty[h], (n & 1) ^ 1);     // the epilogue has read accumulator h of the tile before
+                    tc_mbar_wait(&s_tempty[h], (n & 1) ^ 1);     // the epilogue has read accumulator h of the tile before
                     tc_fence_after();
 #pragma unroll
                     for (int q = 0; q < S::KC / 2; q++) {             // K = 16 per instruction: two 16-byte chunks
@@ -481,74 +477,131 @@ k_causal_tc(const double *__restrict__ cpad, const unsigned char *__restrict__ o
             uint32_t *U = s_U + (n & 1) * TCT * TC_PITCH, *L = s_L + (n & 1) * TCT * TC_PITCH;
             tc_mbar_wait(&s_sempty[n & 1], ((n >> 1) & 1) ^ 1);    // the writers are done with this staging buffer
 
+            // The blocks of a tile are software-pipelined: the shuffle butterfly of the block before (five dependent
+            // shuffles, ~150 clk of latency) is interleaved with the sign extraction of the current one.
             auto do_tile = [&](auto diag_tag) {
                 constexpr bool DIAG = decltype(diag_tag)::value;
-#pragma unroll 1
+                uint32_t pend = 0;                    // word of the block before, not yet transposed
+                uint32_t *pendL = L + lane * TC_PITCH;   // where its transpose goes (first use: a dummy store of 0, overwritten)
+                bool have = false;
+#pragma unroll
                 for (int h = 0; h < 2; h++) {
                     const int r0 = h * 128 + q * 32;                  // first row of this warp's blocks (tile-local)
                     tc_mbar_wait(&s_tfull[h], n & 1);
                     tc_fence_after();
                     const uint32_t taddr = tmem_base + ((uint32_t)(q * 32) << 16) + h * 256 + g * 64;
-#pragma unroll 1
+#pragma unroll
                     for (int k = 0; k < 2; k++) {
                         const int c0 = g * 64 + k * 32;               // first column of the block (tile-local)
                         uint32_t lw = 0;
-                        if (!(DIAG && c0 + 31 <= r0)) {               // (a block at or below the diagonal stays 0)
-                            uint32_t v[32];
-                            tc_ld32(taddr + k * 32, v);
-                            asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
-                            uint32_t sg = 0;
-                            float mn = __int_as_float(0x7f800000);
+                        if (DIAG && c0 + 31 <= r0) {                  // a block at or below the diagonal: all zero
+                            if (have) *pendL = transpose(pend);
+                            U[(r0 + lane) * TC_PITCH + (c0 >> 5)] = 0;
+                            pend = 0;
+                            pendL = L + (c0 + lane) * TC_PITCH + (r0 >> 5);
+                            have = true;
+                            continue;
+                        }
+                        uint32_t v[32];
+                        tc_ld32(taddr + k * 32, v);
+                        asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+                        // Sign bits.  The kernel is bound by instruction issue and by the ALU pipe (SHF, FMNMX3, LOP3: one warp
+                        // instruction per two clocks) while the FMA pipe is idle: TC_NF columns take their bit through it,
+                        //     t = fma.sat(a, 2^100, 0.5)      1.0 if a > 0, 0.0 if a < 0 (|a| > m >= 2^-94; in-band rows are redone)
+                        //     acc = fma(t, 2^c, acc)           acc = 2^23 + sum: the bits sit in the significand
+                        // (two FMA-pipe instructions per pair) and the others through the funnel shift (one ALU instruction per
+                        // pair); TC_NF balances the two pipes against the issue slots.  min |a| over all 32 columns stays on the
+                        // ALU pipe (one FMNMX3 per two pairs, two independent chains).  The five butterfly steps of the block
+                        // before are spread between them by hand (ptxas keeps the shuffles together otherwise).
+                        uint32_t sg = 0;
+                        float acc = 0x1p23f;
+                        float mn0 = __int_as_float(0x7f800000), mn1 = mn0;
+                        uint32_t px = pend, po;
+#define TC_BIT(c)                                                                                           \
+    if ((c) < TC_NF) {                                                                                      \
+        float t_;                                                                                           \
+        asm("fma.rn.sat.f32 %0, %1, 0f71800000, 0f3F000000;" : "=f"(t_) : "f"(__uint_as_float(v[c])));      \
+        acc = __fmaf_rn(t_, (float)(1u << ((c) < TC_NF ? (c) : 0)), acc);                                   \
+    } else {                                                                                                \
+        sg = __funnelshift_l(v[c], sg, 1);                                                                  \
+    }
+#define TC_MIN(c)                                                      \
+    mn0 = min3_abs_nan(mn0, v[c], v[c - 1]);                           \
+    mn1 = min3_abs_nan(mn1, v[16 + c], v[16 + c - 1]);
+#define TC_BFLY_SEND(t) po = __shfl_xor_sync(0xffffffffu, px, 16 >> t);
+#define TC_BFLY_TAKE(t)                                                \
+    po = __funnelshift_l(po, po, transpose.rot[t]);                    \
+    px = (px & transpose.keep[t]) | (po & ~transpose.keep[t]);
+                        TC_BFLY_SEND(0)
+                        TC_BIT(31) TC_BIT(30) TC_BIT(0) TC_BIT(29) TC_BIT(28) TC_BIT(1) TC_BIT(27)
+                        TC_MIN(15) TC_MIN(13)
+                        TC_BFLY_TAKE(0) TC_BFLY_SEND(1)
+                        TC_BIT(26) TC_BIT(2) TC_BIT(25) TC_BIT(24) TC_BIT(3) TC_BIT(23) TC_BIT(22)
+                        TC_MIN(11) TC_MIN(9)
+                        TC_BFLY_TAKE(1) TC_BFLY_SEND(2)
+                        TC_BIT(4) TC_BIT(21) TC_BIT(20) TC_BIT(5) TC_BIT(19) TC_BIT(18) TC_BIT(6)
+                        TC_MIN(7) TC_MIN(5)
+                        TC_BFLY_TAKE(2) TC_BFLY_SEND(3)
+                        TC_BIT(17) TC_BIT(16) TC_BIT(7) TC_BIT(15) TC_BIT(14) TC_BIT(13)
+                        TC_MIN(3)
+                        TC_BFLY_TAKE(3) TC_BFLY_SEND(4)
+                        TC_BIT(12) TC_BIT(11) TC_BIT(10) TC_BIT(9) TC_BIT(8)
+                        TC_MIN(1)
+                        TC_BFLY_TAKE(4)
+#undef TC_BIT
+#undef TC_MIN
+#undef TC_BFLY_SEND
+#undef TC_BFLY_TAKE
+                        const uint32_t pendT = px;
+                        // bits 0..NF-1: related = 1, from the significand of acc (0x4B000000 | bits); the other columns: related =
+                        // sign clear, sg holds their signs (column 31 highest):  lw = bits + ((2^(32-NF) - 1 - sg) << NF)
+                        lw = (__float_as_uint(acc) - 0x4B000000u + (0xFFFFFFFFu << TC_NF)) - (sg << TC_NF);
+                        const bool unc = !(mn0 > m && mn1 > m);       // NaN compares false: uncertain
+                        uint32_t todo = __ballot_sync(0xffffffffu, unc);
+                        if (have) *pendL = pendT;                     // past of j: bit = row i
+                        if (PROBE) {
+                            p_tot++;
+                            p_rows += unc ? 1 : 0;
+                            if (GEOM == CS_GEOM_MINK_CONE && !unc) {
 #pragma unroll
-                            for (int c = 31; c >= 1; c -= 2) {
-                                sg = __funnelshift_l(v[c], sg, 1);
-                                sg = __funnelshift_l(v[c - 1], sg, 1);
-                                mn = min3_abs_nan(mn, v[c], v[c - 1]);
-                            }
-                            lw = ~sg;                                 // related = sign bit clear (valid outside the band)
-                            const bool unc = !(mn > m);               // NaN compares false: uncertain
-                            uint32_t todo = __ballot_sync(0xffffffffu, unc);
-                            if (PROBE) {
-                                p_tot++;
-                                p_rows += unc ? 1 : 0;
-                                if (GEOM == CS_GEOM_MINK_CONE && !unc) {
+                                for (int c = 0; c < 32; c++) {
+                                    double T = 0.0;
 #pragma unroll
-                                    for (int c = 0; c < 32; c++) {
-                                        double T = 0.0;
-#pragma unroll
-                                        for (int d = 0; d < DIM; d++) {
-                                            const double dd = cJ[(c0 + c) * DIM + d] - cI[(r0 + lane) * DIM + d];
-                                            T += d == 0 ? dd * dd : -dd * dd;
-                                        }
-                                        const float er = (float)(fabs((double)__uint_as_float(v[c]) - 0.5 * T) / (double)C2);
-                                        if (er == er) p_err = fmaxf(p_err, er);      // (padding points are NaN)
+                                    for (int d = 0; d < DIM; d++) {
+                                        const double dd = cJ[(c0 + c) * DIM + d] - cI[(r0 + lane) * DIM + d];
+                                        T += d == 0 ? dd * dd : -dd * dd;
                                     }
+                                    const float er = (float)(fabs((double)__uint_as_float(v[c]) - 0.5 * T) / (double)C2);
+                                    if (er == er) p_err = fmaxf(p_err, er);      // (padding points are NaN)
                                 }
-                            }
-                            while (todo) {                            // fp64 for whole rows of the block, one pair per lane
-                                const int r = __ffs(todo) - 1;
-                                todo &= todo - 1;
-                                double xi[DIM], xj[DIM];
-#pragma unroll
-                                for (int d = 0; d < DIM; d++) {
-                                    xi[d] = cI[(r0 + r) * DIM + d];   // (points beyond N are NaN: unrelated)
-                                    xj[d] = cJ[(c0 + lane) * DIM + d];
-                                }
-                                const uint32_t w = __ballot_sync(0xffffffffu, Pred<GEOM, DIM>::rel(xi, xj));
-                                if (lane == r) lw = w;
-                            }
-                            if (DIAG) {                               // only i < j inside the diagonal tile
-                                const int keep_from = r0 + lane + 1 - c0;          // columns c >= keep_from are kept
-                                lw &= keep_from <= 0 ? 0xffffffffu : (keep_from >= 32 ? 0u : (0xffffffffu << keep_from));
                             }
                         }
+                        while (todo) {                                // fp64 for whole rows of the block, one pair per lane
+                            const int r = __ffs(todo) - 1;
+                            todo &= todo - 1;
+                            double xi[DIM], xj[DIM];
+#pragma unroll
+                            for (int d = 0; d < DIM; d++) {
+                                xi[d] = cI[(r0 + r) * DIM + d];       // (points beyond N are NaN: unrelated)
+                                xj[d] = cJ[(c0 + lane) * DIM + d];
+                            }
+                            const uint32_t w = __ballot_sync(0xffffffffu, Pred<GEOM, DIM>::rel(xi, xj));
+                            if (lane == r) lw = w;
+                        }
+                        if (DIAG) {                                   // only i < j inside the diagonal tile
+                            const int keep_from = r0 + lane + 1 - c0;              // columns c >= keep_from are kept
+                            lw &= keep_from <= 0 ? 0xffffffffu : (keep_from >= 32 ? 0u : (0xffffffffu << keep_from));
+                        }
                         U[(r0 + lane) * TC_PITCH + (c0 >> 5)] = lw;                   // future of i: bit = column j
-                        L[(c0 + lane) * TC_PITCH + (r0 >> 5)] = transpose(lw);        // past of j: bit = row i
+                        pend = lw;
+                        pendL = L + (c0 + lane) * TC_PITCH + (r0 >> 5);
+                        have = true;
                     }
                     tc_fence_before();
                     __syncwarp();
                     if (lane == 0) tc_mbar_arrive(&s_tempty[h]);      // accumulator h may be overwritten
                 }
+                *pendL = transpose(pend);
             };
             if (diag) do_tile(std::true_type{});
             else do_tile(std::false_type{});
@@ -574,45 +627,46 @@ k_causal_tc(const double *__restrict__ cpad, const unsigned char *__restrict__ o
     } else {
         // ===================================== writers ========================================
         // 64 threads move a staged tile to global memory: thread = (row mod 32, 16-byte half of the 32-byte segment),
-        // eight rows each; the mirrored tile of an off-diagonal tile is written as zeros.
+        // eight rows each.  The mirrored tile of an off-diagonal tile is zeros: two TMA tile stores from a constant zero
+        // tile (rows beyond N and bytes beyond the row are clipped by the tensor map).
         const int wt = tid - TC_WR0 * 32;             // 0 .. 63
         const int hf = wt & 1, rr = wt >> 1;
         const int64_t row_bytes = stride * 8;
-        const uint4 zero = make_uint4(0, 0, 0, 0);
         uint32_t n = 0;
         for (uint32_t t = blockIdx.x; t < total_tiles; t += gridDim.x, n++) {
             const uint4 e = __ldg(tab + t);
             const int I = (int)(e.x & 0xFFFFu), J = (int)(e.x >> 16);
+            if (wt == 0 && I != J) {
+                const uint32_t zsrc = tc_smem_u32(smem + SM::ZERO);
+                asm volatile("cp.async.bulk.tensor.3d.global.shared::cta.bulk_group [%0, {%1, %2, %3}], [%4];" ::"l"(&mapB),
+                             "r"(I * 32), "r"(J * TCT), "r"((int)e.y), "r"(zsrc) : "memory");
+                if (bitsT)
+                    asm volatile("cp.async.bulk.tensor.3d.global.shared::cta.bulk_group [%0, {%1, %2, %3}], [%4];" ::"l"(&mapT),
+                                 "r"(J * 32), "r"(I * TCT), "r"((int)e.y), "r"(zsrc) : "memory");
+                asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+            }
             const int64_t colI = (int64_t)I * 32 + hf * 16, colJ = (int64_t)J * 32 + hf * 16;      // byte offsets in a row
             const size_t mat = (size_t)e.y * N * row_bytes;
-            unsigned char *pb = reinterpret_cast<unsigned char *>(bits) + mat;
-            unsigned char *pt = bitsT ? reinterpret_cast<unsigned char *>(bitsT) + mat : nullptr;
-            const bool okI = colI < row_bytes, okJ = colJ < row_bytes, off = I != J;
+            unsigned char *pb = reinterpret_cast<unsigned char *>(bits) + mat + colJ;
+            unsigned char *pt = reinterpret_cast<unsigned char *>(bitsT) + mat + colI;
+            const bool okI = colI < row_bytes && bitsT != nullptr, okJ = colJ < row_bytes;
             const uint32_t *u = s_U + (n & 1) * TCT * TC_PITCH + rr * TC_PITCH + hf * 4;
             const uint32_t *l = s_L + (n & 1) * TCT * TC_PITCH + rr * TC_PITCH + hf * 4;
             int64_t gi = (int64_t)I * TCT + rr, gj = (int64_t)J * TCT + rr;
-            size_t oi = (size_t)gi * row_bytes, oj = (size_t)gj * row_bytes;
             tc_mbar_wait(&s_sfull[n & 1], (n >> 1) & 1);
-#pragma unroll 4
+#pragma unroll
             for (int p = 0; p < 8; p++) {
-                if (gi < N && okJ) {
-                    *reinterpret_cast<uint4 *>(pb + oi + colJ) = make_uint4(u[0], u[1], u[2], u[3]);
-                    if (pt && off) *reinterpret_cast<uint4 *>(pt + oi + colJ) = zero;
-                }
-                if (gj < N && okI) {
-                    if (pt) *reinterpret_cast<uint4 *>(pt + oj + colI) = make_uint4(l[0], l[1], l[2], l[3]);
-                    if (off) *reinterpret_cast<uint4 *>(pb + oj + colI) = zero;
-                }
+                if (gi < N && okJ) *reinterpret_cast<uint4 *>(pb + (size_t)gi * row_bytes) = make_uint4(u[0], u[1], u[2], u[3]);
+                if (gj < N && okI) *reinterpret_cast<uint4 *>(pt + (size_t)gj * row_bytes) = make_uint4(l[0], l[1], l[2], l[3]);
                 u += 32 * TC_PITCH;
                 l += 32 * TC_PITCH;
                 gi += 32;
                 gj += 32;
-                oi += 32 * (size_t)row_bytes;
-                oj += 32 * (size_t)row_bytes;
             }
             __syncwarp();
             if (lane == 0) tc_mbar_arrive(&s_sempty[n & 1]);
         }
+        if (wt == 0) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
     }
 
     tc_fence_before();
@@ -659,9 +713,14 @@ int launch_tc_t(const double *coords, int64_t B, int64_t N, int64_t stride, uint
         CS_CUDA(cudaFuncSetAttribute(k_causal_tc<GEOM, DIM, PROBE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         attr_set.set(dev);
     }
+    CUtensorMap mapB, mapT;
+    int rc = bits_tensor_map(&mapB, bits, B, N, stride, 32, TCT, false);
+    if (rc) return rc;
+    rc = bits_tensor_map(&mapT, bitsT ? bitsT : bits, B, N, stride, 32, TCT, false);
+    if (rc) return rc;
     int grid = sm_count();
     if (grid > total) grid = (int)total;
-    k_causal_tc<GEOM, DIM, PROBE><<<grid, TC_THREADS, smem, st>>>(cpad, opA, opB, tab, N, stride, nT, (uint32_t)total,
+    k_causal_tc<GEOM, DIM, PROBE><<<grid, TC_THREADS, smem, st>>>(mapB, mapT, cpad, opA, opB, tab, N, stride, nT, (uint32_t)total,
                                                                   bits, bitsT, probe);
     CS_LAUNCHED("k_causal_tc");
     return CS_OK;

@@ -817,8 +817,10 @@ static EncodeTiledFn pair_encode_fn()
     return fn;
 }
 
-// bit matrix [B][N][stride uint64] seen as bytes: dims {stride*8, N, B}; box {BROW bytes, rows, 1}
-static int pair_bits_map(CUtensorMap *map, const uint64_t *base, int64_t B, int64_t N, int64_t stride, int rows)
+// bit matrix [B][N][stride uint64] seen as bytes: dims {stride*8, N, B}; box {box_bytes, rows, 1}; 64-byte swizzle (the
+// staged rows of this kernel) or none (the zero tiles cs_build_tc.cu stores)
+int bits_tensor_map(CUtensorMap *map, const uint64_t *base, int64_t B, int64_t N, int64_t stride, int box_bytes, int rows,
+                    bool swizzle64)
 {
     EncodeTiledFn fn = pair_encode_fn();
     if (!fn) {
@@ -827,16 +829,20 @@ static int pair_bits_map(CUtensorMap *map, const uint64_t *base, int64_t B, int6
     }
     cuuint64_t gdim[3] = {(cuuint64_t)(stride * 8), (cuuint64_t)N, (cuuint64_t)B};
     cuuint64_t gstr[2] = {(cuuint64_t)(stride * 8), (cuuint64_t)(N * stride * 8)};
-    cuuint32_t box[3] = {(cuuint32_t)BROW, (cuuint32_t)rows, 1};
+    cuuint32_t box[3] = {(cuuint32_t)box_bytes, (cuuint32_t)rows, 1};
     cuuint32_t estr[3] = {1, 1, 1};
     CUresult r = fn(map, CU_TENSOR_MAP_DATA_TYPE_UINT8, 3, const_cast<uint64_t *>(base), gdim, gstr, box, estr,
-                    CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_64B, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
-                    CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+                    CU_TENSOR_MAP_INTERLEAVE_NONE, swizzle64 ? CU_TENSOR_MAP_SWIZZLE_64B : CU_TENSOR_MAP_SWIZZLE_NONE,
+                    CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (r != CUDA_SUCCESS) {
         snprintf(g_cuda_err, sizeof(g_cuda_err), "cuTensorMapEncodeTiled failed (%d)", (int)r);
         return CS_ERR_CUDA;
     }
     return CS_OK;
+}
+static int pair_bits_map(CUtensorMap *map, const uint64_t *base, int64_t B, int64_t N, int64_t stride, int rows)
+{
+    return bits_tensor_map(map, base, B, N, stride, BROW, rows, true);
 }
 
 // One 256-column accumulator per tile.  Measured alternatives that were dropped: 128-column
