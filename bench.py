@@ -252,7 +252,10 @@ def run_peaks(args, local_rank):
                                "multiply-adds; hbm: bytes; tmem_ld: bytes"}))
 
 
-def time_single(api, cfg, N, route, steps, warmup, seed, local_rank, csd, e2e=True):
+A1_ROUTES = {"auto": 0, "fma": 1, "tensor": 2}
+
+
+def time_single(api, cfg, N, route, steps, warmup, seed, local_rank, csd, e2e=True, a1_route=0):
     """K timed steps of a1 -> a2 -> a3 on one seeded sprinkling (inputs resident in HBM), device time per stage,
     then (optionally) the same through cs_action_host with pinned host buffers."""
     import torch
@@ -263,6 +266,7 @@ def time_single(api, cfg, N, route, steps, warmup, seed, local_rank, csd, e2e=Tr
     kmax = api.clamp_kmax(N, cfg.kmax)
     # persistent device buffers (the library never allocates)
     ws = torch.empty(max(api.interval_hist_workspace(N, kmax, True, route), 256), dtype=torch.uint8, device="cuda")
+    ws1 = torch.empty(max(api.causal_matrix_workspace(1, N, cfg.dim, cfg.geometry, a1_route), 256), dtype=torch.uint8, device="cuda")
     bits = torch.empty((N, stride), dtype=torch.int64, device="cuda")
     bitsT = torch.empty((N, stride), dtype=torch.int64, device="cuda")
     hist = torch.empty(kmax + 1, dtype=torch.int64, device="cuda")
@@ -272,8 +276,8 @@ def time_single(api, cfg, N, route, steps, warmup, seed, local_rank, csd, e2e=Tr
 
     def step(events=None):
         if events is not None: events[0].record()
-        api._check(lib.cs_causal_matrix(d_coords.data_ptr(), N, cfg.dim, cfg.geometry, bits.data_ptr(),
-                                        bitsT.data_ptr(), st), "cs_causal_matrix")
+        api._check(lib.cs_causal_matrix_ex(d_coords.data_ptr(), 1, N, cfg.dim, cfg.geometry, a1_route, bits.data_ptr(),
+                                           bitsT.data_ptr(), ws1.data_ptr(), ws1.numel(), st), "cs_causal_matrix_ex")
         if events is not None: events[1].record()
         api._check(lib.cs_interval_hist_ex(bits.data_ptr(), bitsT.data_ptr(), N, kmax, 0, N, route, hist.data_ptr(),
                                            None, ws.data_ptr(), ws.numel(), st), "cs_interval_hist_ex")
@@ -298,7 +302,9 @@ def time_single(api, cfg, N, route, steps, warmup, seed, local_rank, csd, e2e=Tr
         step(ev[k])
     torch.cuda.synchronize(); csd.barrier()
     t1 = time.perf_counter()
+    a1_used = a1_route if a1_route else api.default_a1_route(1, N, cfg.dim, cfg.geometry)
     m = {"coords": coords, "N": N, "kmax": kmax, "stride": stride, "R": R, "W_alg": W_alg, "route": route,
+         "a1_route": {1: "fma", 2: "tensor"}[a1_used],
          "launches": api.launch_count() - launches0, "clocks": sampler.stop(t0, t1),
          "total_ms": ev[0][0].elapsed_time(ev[-1][3]),
          "build_ms": [e[0].elapsed_time(e[1]) for e in ev], "hist_ms": [e[1].elapsed_time(e[2]) for e in ev],
@@ -469,6 +475,7 @@ def main():
     ap.add_argument("--N", type=int, default=0, help="override N (debug only; the line then names it)")
     ap.add_argument("--B", type=int, default=0, help="config 5 only: number of causets per step (default 4096)")
     ap.add_argument("--route", type=int, default=0, help="0 auto, 1 popc, 2 tensor int8, 3 tensor fp4, 4 tensor fp4 on CTA pairs")
+    ap.add_argument("--a1-route", default="auto", choices=sorted(A1_ROUTES), help="a1: auto, FMA pipes, or tensor cores (bilinear predicates)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-other-configs", action="store_true", help="skip the short passes over configs 2, 4 and 5")
     ap.add_argument("--peaks", action="store_true", help="run the peak probes only")
@@ -506,7 +513,8 @@ def main():
 
     N = args.N or cfg.N
     route = args.route or api.default_route(N)
-    m = time_single(api, cfg, N, route, args.steps, args.warmup, csd.replica_seed(cfg.seed, rank), local_rank, csd)
+    m = time_single(api, cfg, N, route, args.steps, args.warmup, csd.replica_seed(cfg.seed, rank), local_rank, csd,
+                    a1_route=A1_ROUTES[args.a1_route])
     R, W_alg, kmax, stride = m["R"], m["W_alg"], m["kmax"], m["stride"]
     units, secs, value = csd.aggregate(float(W_alg) * args.steps, m["total_ms"] / 1e3)
     ms_per_step = 1e3 * secs / args.steps
@@ -562,7 +570,7 @@ def main():
     stages = {"build_ms": statistics.mean(m["build_ms"]), "interval_ms": statistics.mean(m["hist_ms"]),
               "action_ms": statistics.mean(m["act_ms"]), "interval_ms_min": min(m["hist_ms"]),
               "build_hbm_gbs": build_bytes / build_s / 1e9,
-              "build_hbm_frac": build_bytes / build_s / 1e9 / peaks["hbm_gbs"],
+              "build_hbm_frac": build_bytes / build_s / 1e9 / peaks["hbm_gbs"], "build_route": m["a1_route"],
               "interval_share_of_step": statistics.mean(m["hist_ms"]) / (m["total_ms"] / args.steps)}
 
     line = {

@@ -49,6 +49,7 @@ _SIGNATURES = {
     "cs_causal_matrix": (_int, [_p, _i64, _int, _int, _p, _p, _p]),
     "cs_causal_matrix_batched": (_int, [_p, _i64, _i64, _int, _int, _p, _p, _p]),
     "cs_causal_matrix_workspace": (_sz, [_i64, _i64, _int, _int, _int]),
+    "cs_default_a1_route": (_int, [_i64, _i64, _int, _int]),
     "cs_causal_matrix_ex": (_int, [_p, _i64, _i64, _int, _int, _int, _p, _p, _p, _sz, _p]),
     "cs_a1_tensor_probe": (_int, [_p, _i64, _int, _p, _p, _p, _sz, _p, _p]),
     "cs_transpose_bits": (_int, [_p, _i64, _p, _p]),
@@ -147,6 +148,10 @@ def peak_probe(kind: str, iters: int, workspace: torch.Tensor):
 
 def causal_matrix_workspace(B: int, N: int, dim: int, geometry: int, route: int = A1_AUTO) -> int:
     return int(load().cs_causal_matrix_workspace(B, N, dim, geometry, route))
+
+
+def default_a1_route(B: int, N: int, dim: int, geometry: int) -> int:
+    return int(load().cs_default_a1_route(B, N, dim, geometry))
 
 
 def causal_matrix(coords: torch.Tensor, geometry: int, want_transpose: bool = True, route: int = A1_AUTO,

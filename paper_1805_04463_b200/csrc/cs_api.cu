@@ -151,6 +151,12 @@ size_t cs_causal_matrix_workspace(int64_t B, int64_t N, int dim, int geometry, i
     return causal_matrix_scratch_bytes(B, N, dim, geometry, route);
 }
 
+int cs_default_a1_route(int64_t B, int64_t N, int dim, int geometry)
+{
+    if (B < 1 || N < 1) return CS_A1_FMA;
+    return causal_matrix_scratch_bytes(B, N, dim, geometry, CS_A1_AUTO) ? CS_A1_TENSOR : CS_A1_FMA;
+}
+
 int cs_causal_matrix_ex(const double *coords, int64_t B, int64_t N, int dim, int geometry, int route,
                         uint64_t *bits, uint64_t *bitsT, void *workspace, size_t workspace_bytes, void *stream)
 {
@@ -316,11 +322,17 @@ int cs_greedy_antichain(const uint64_t *bits, const uint64_t *bitsT, int64_t N, 
 // ENSEMBLE_MAT_BYTES), not of the ensemble (4 GiB for 4096 x 2048).  CB is a whole number of causets per CTA pair
 // of a2's persistent grid (causet-major schedule: every pair then gets the same number of causets).
 // workspace: [bits CB*N*stride][bitsT CB*N*stride][hist B*4 int64][interval scratch]
-constexpr size_t ENSEMBLE_MAT_BYTES = (size_t)448 << 20;     // both matrices of a chunk
+constexpr size_t ENSEMBLE_MAT_BYTES = (size_t)448 << 20;     // both matrices of a chunk + the scratch of its a1
+
+// a1 scratch of cb causets, whatever the geometry (the workspace queries do not know it): the widest operand rows
+static size_t ensemble_a1_scratch(int64_t cb, int64_t N)
+{
+    return align_up(causal_tc_scratch_bytes(cb, N, 7, CS_GEOM_DS4_SPHERICAL), 256);
+}
 
 static int64_t ensemble_chunk(int64_t B, int64_t N)
 {
-    const size_t per = 2 * (size_t)N * row_stride_words(N) * 8;
+    const size_t per = 2 * (size_t)N * row_stride_words(N) * 8 + ensemble_a1_scratch(1, N);
     int64_t cb = per ? (int64_t)(ENSEMBLE_MAT_BYTES / per) : B;
     const int64_t pairs = sm_count() / 2;
     if (cb > pairs) cb -= cb % pairs;
@@ -334,7 +346,7 @@ size_t cs_bd_action_batched_workspace(int64_t B, int64_t N)
     const int64_t CB = ensemble_chunk(B, N);
     const size_t mat = align_up((size_t)CB * N * row_stride_words(N) * 8, 256);
     int r = cs_default_route(N);
-    return 2 * mat + align_up((size_t)B * 4 * 8, 256) + interval_ws_bytes(CB, N, 1, r);
+    return 2 * mat + align_up((size_t)B * 4 * 8, 256) + interval_ws_bytes(CB, N, 1, r) + ensemble_a1_scratch(CB, N);
 }
 
 int cs_bd_action_batched(const double *coords, int64_t B, int64_t N, int dim, int geometry,
@@ -354,15 +366,17 @@ int cs_bd_action_batched(const double *coords, int64_t B, int64_t N, int dim, in
     uint64_t *bitsT = reinterpret_cast<uint64_t *>(ws + mat);
     int64_t *hist = reinterpret_cast<int64_t *>(ws + 2 * mat);
     unsigned char *iws = ws + 2 * mat + align_up((size_t)B * 4 * 8, 256);
+    const size_t a1_bytes = ensemble_a1_scratch(CB, N);
+    unsigned char *a1ws = ws + cs_bd_action_batched_workspace(B, N) - a1_bytes;
     const int64_t kmax = clamp_kmax(N, 3);
     // hist rows are kmax+1 long; with kmax = 3 that is the [B][4] layout asked for
     if (kmax < 3) CS_CUDA(cudaMemsetAsync(hist, 0, (size_t)B * 4 * 8, st));
     for (int64_t b0 = 0; b0 < B; b0 += CB) {
         const int64_t nb = B - b0 < CB ? B - b0 : CB;
-        int rc = cs_causal_matrix_batched(coords + b0 * N * dim, nb, N, dim, geometry, bits, bitsT, stream);
+        int rc = cs_causal_matrix_ex(coords + b0 * N * dim, nb, N, dim, geometry, CS_A1_AUTO, bits, bitsT, a1ws, a1_bytes, stream);
         if (rc) return rc;
         rc = interval_hist_impl(bits, bitsT, nb, N, kmax, 0, N, CS_ROUTE_AUTO, hist + b0 * (kmax + 1), nullptr, iws,
-                                workspace_bytes - (size_t)(iws - ws), st);
+                                (size_t)(a1ws - iws), st);
         if (rc) return rc;
     }
     return launch_bd_action(hist, kmax + 1, B, kmax, N, spacetime_dim(geometry, dim), actions, nullptr, hist4, st);
@@ -416,7 +430,7 @@ size_t cs_bd_action_batched_host_workspace(int64_t B, int64_t N, int dim)
     const size_t cbuf = align_up((size_t)CB * N * dim * 8, 256);
     const size_t mat = align_up((size_t)CB * N * row_stride_words(N) * 8, 256);
     return 2 * cbuf + 2 * mat + align_up((size_t)CB * 4 * 8, 256) + align_up((size_t)B * 8, 256) +
-           align_up((size_t)B * 4 * 8, 256) + interval_ws_bytes(CB, N, 1, cs_default_route(N));
+           align_up((size_t)B * 4 * 8, 256) + interval_ws_bytes(CB, N, 1, cs_default_route(N)) + ensemble_a1_scratch(CB, N);
 }
 
 int cs_bd_action_batched_host(const double *coords_host, int64_t B, int64_t N, int dim, int geometry,
@@ -450,7 +464,9 @@ int cs_bd_action_batched_host(const double *coords_host, int64_t B, int64_t N, i
     ws += align_up((size_t)B * 8, 256);
     int64_t *hist4 = reinterpret_cast<int64_t *>(ws);
     ws += align_up((size_t)B * 4 * 8, 256);
-    const size_t left = workspace_bytes - (size_t)(ws - static_cast<unsigned char *>(workspace));
+    const size_t a1_bytes = ensemble_a1_scratch(CB, N);
+    unsigned char *a1ws = static_cast<unsigned char *>(workspace) + cs_bd_action_batched_host_workspace(B, N, dim) - a1_bytes;
+    const size_t left = (size_t)(a1ws - ws);
     const int64_t kmax = clamp_kmax(N, 3);
 
     // the copy stream may not touch the workspace before the caller's stream is done with earlier work on it
@@ -465,7 +481,7 @@ int cs_bd_action_batched_host(const double *coords_host, int64_t B, int64_t N, i
                                 cudaMemcpyHostToDevice, copy_stream));
         CS_CUDA(cudaEventRecord(copied[buf], copy_stream));
         CS_CUDA(cudaStreamWaitEvent(st, copied[buf], 0));
-        int rc = cs_causal_matrix_batched(cdev[buf], nb, N, dim, geometry, bits, bitsT, stream);
+        int rc = cs_causal_matrix_ex(cdev[buf], nb, N, dim, geometry, CS_A1_AUTO, bits, bitsT, a1ws, a1_bytes, stream);
         if (rc) return rc;
         CS_CUDA(cudaEventRecord(consumed[buf], st));
         if (kmax < 3) CS_CUDA(cudaMemsetAsync(hist, 0, (size_t)nb * 4 * 8, st));
@@ -489,7 +505,7 @@ size_t cs_action_host_workspace(int64_t N, int64_t kmax)
     kmax = clamp_kmax(N, kmax);
     const size_t mat = align_up((size_t)N * row_stride_words(N) * 8, 256);
     return align_up((size_t)N * 7 * 8, 256) + 2 * mat + align_up((size_t)(kmax + 1) * 8, 256) + 256 +
-           interval_ws_bytes(1, N, 1, cs_default_route(N));
+           interval_ws_bytes(1, N, 1, cs_default_route(N)) + ensemble_a1_scratch(1, N);
 }
 
 int cs_action_host(const double *coords_host, int64_t N, int dim, int geometry, int64_t kmax,
@@ -514,10 +530,12 @@ int cs_action_host(const double *coords_host, int64_t N, int dim, int geometry, 
     ws += align_up((size_t)(kmax + 1) * 8, 256);
     double *action = reinterpret_cast<double *>(ws);
     ws += 256;
-    const size_t left = workspace_bytes - (size_t)(ws - static_cast<unsigned char *>(workspace));
+    const size_t a1_bytes = ensemble_a1_scratch(1, N);
+    unsigned char *a1ws = static_cast<unsigned char *>(workspace) + cs_action_host_workspace(N, kmax) - a1_bytes;
+    const size_t left = (size_t)(a1ws - ws);
 
     if (N > 0) CS_CUDA(cudaMemcpyAsync(coords, coords_host, (size_t)N * dim * 8, cudaMemcpyHostToDevice, st));
-    int rc = cs_causal_matrix(coords, N, dim, geometry, bits, bitsT, stream);
+    int rc = cs_causal_matrix_ex(coords, 1, N, dim, geometry, CS_A1_AUTO, bits, bitsT, a1ws, a1_bytes, stream);
     if (rc) return rc;
     rc = cs_interval_hist(bits, bitsT, N, kmax, hist, nullptr, ws, left, stream);
     if (rc) return rc;

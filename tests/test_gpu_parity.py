@@ -60,9 +60,25 @@ def to_u64(t):
     return t.cpu().numpy().view(np.uint64)
 
 
+TENSOR_A1_GEOMS = (inp.GEOM_MINK_CONE, inp.GEOM_FLRW_POLAR, inp.GEOM_DS4_SPHERICAL)    # bilinear predicates
+
+
+def a1_routes(api, geom, N):
+    """Every concrete a1 route that serves this geometry and size (the tensor route wants rows of >= 32 bytes)."""
+    r = [api.A1_FMA]
+    if geom in TENSOR_A1_GEOMS and N >= 256:
+        r.append(api.A1_TENSOR)
+    return r
+
+
 def gpu_bits(api, coords, geom):
+    """The library's default a1 route -- and, asserted bit-identical to it, every other route that serves the geometry,
+    so that each a1 test compares all of them with the oracle."""
     d = torch.from_numpy(np.ascontiguousarray(coords)).cuda()
     bits, bitsT = api.causal_matrix(d, geom)
+    for route in a1_routes(api, geom, coords.shape[0]):
+        b, t = api.causal_matrix(d, geom, route=route)
+        assert torch.equal(b, bits) and torch.equal(t, bitsT), "a1 route %d differs from the default route" % route
     torch.cuda.synchronize()
     return bits, bitsT
 
@@ -251,6 +267,72 @@ def test_causal_matrix_prefilter_flrw(api, oracle):
     dust = inp.sprinkle_dust_slab(2500, 3)                  # App. A.1.4 through the same predicate
     assert np.array_equal(to_u64(gpu_bits(api, dust, inp.GEOM_FLRW_POLAR)[0]),
                           oracle.causal_matrix_bits(dust, inp.GEOM_FLRW_POLAR))
+
+
+@pytest.mark.parametrize("geom,dim", [(g, d) for g, d in GEOMS if g in TENSOR_A1_GEOMS])
+@pytest.mark.parametrize("N", [256, 257, 511, 1025, 2304, 3001])
+def test_causal_matrix_tensor_route(api, oracle, geom, dim, N):
+    """a1 on the tensor cores (CS_A1_TENSOR) against the oracle at sizes from one tile up: with the library's pool and with
+    a caller's workspace, with and without the transposed output, and as a batch of ragged causets."""
+    coords = inp.sprinkle(geom, dim, N, 300 + N + dim)
+    o_bits = oracle.causal_matrix_bits(coords, geom)
+    d = torch.from_numpy(coords).cuda()
+    bits, bitsT = api.causal_matrix(d, geom, route=api.A1_TENSOR)
+    assert np.array_equal(to_u64(bits), o_bits)
+    assert np.array_equal(to_u64(bitsT), oracle.transpose_bits(o_bits, N))
+    nbytes = api.causal_matrix_workspace(1, N, dim, geom, api.A1_TENSOR)
+    assert nbytes > 0 and api.causal_matrix_workspace(1, N, dim, geom, api.A1_FMA) == 0
+    ws = torch.empty(nbytes, dtype=torch.uint8, device="cuda")
+    b2, t2 = api.causal_matrix(d, geom, route=api.A1_TENSOR, workspace=ws)
+    assert torch.equal(b2, bits) and torch.equal(t2, bitsT)
+    b3, none = api.causal_matrix(d, geom, want_transpose=False, route=api.A1_TENSOR)
+    assert none is None and torch.equal(b3, bits)
+    with pytest.raises(RuntimeError):      # a workspace that is too small is refused, not overrun
+        api.causal_matrix(d, geom, route=api.A1_TENSOR, workspace=ws[:256])
+    if N <= 1025:
+        ens = np.stack([inp.sprinkle(geom, dim, N, 900 + b) for b in range(3)])
+        eb, et = api.causal_matrix_batched(torch.from_numpy(ens).cuda(), geom, route=api.A1_TENSOR)
+        for b in range(3):
+            ob = oracle.causal_matrix_bits(ens[b], geom)
+            assert np.array_equal(to_u64(eb[b]), ob) and np.array_equal(to_u64(et[b]), oracle.transpose_bits(ob, N))
+
+
+def test_causal_matrix_tensor_route_arguments_and_probe(api, oracle):
+    """The tensor route refuses what it does not serve; its probe reports an error of the tensor-core value far inside
+    the margin, and rows re-evaluated in fp64 exactly where the input forces them (unsorted input: every row)."""
+    lc = torch.from_numpy(inp.sprinkle(inp.GEOM_MINK2_LIGHTCONE, 2, 512, 1)).cuda()
+    with pytest.raises(RuntimeError):
+        api.causal_matrix(lc, inp.GEOM_MINK2_LIGHTCONE, route=api.A1_TENSOR)
+    small = torch.from_numpy(inp.sprinkle(inp.GEOM_MINK_CONE, 4, 100, 1)).cuda()
+    with pytest.raises(RuntimeError):
+        api.causal_matrix(small, inp.GEOM_MINK_CONE, route=api.A1_TENSOR)
+    assert api.causal_matrix_workspace(1, 512, 2, inp.GEOM_MINK2_LIGHTCONE, api.A1_TENSOR) == 0
+    for dim in (4, 5):
+        coords = inp.sprinkle(inp.GEOM_MINK_CONE, dim, 3000, 17)
+        o_bits = oracle.causal_matrix_bits(coords, inp.GEOM_MINK_CONE)
+        bits, bitsT, st = api.a1_tensor_probe(torch.from_numpy(coords).cuda())
+        assert np.array_equal(to_u64(bits), o_bits)
+        assert np.array_equal(to_u64(bitsT), oracle.transpose_bits(o_bits, 3000))
+        assert 0.0 < st["max_err_u"] < st["margin_u"] / 8, st
+        assert 0 < st["rows_fp64"] < st["rows_total"] / 10, st
+        rng = np.random.default_rng(3)
+        shuffled = np.ascontiguousarray(coords[rng.permutation(3000)])
+        b2, _, st2 = api.a1_tensor_probe(torch.from_numpy(shuffled).cuda())
+        assert np.array_equal(to_u64(b2), oracle.causal_matrix_bits(shuffled, inp.GEOM_MINK_CONE))
+        assert st2["rows_fp64"] > 0.9 * st2["rows_total"], st2       # (only the tiles whose points happen to be ordered escape)
+
+
+def test_causal_matrix_tensor_route_degenerate(api, oracle):
+    """Identical points (T = 0 for every pair: every row inside the band), NaN rows, huge and tiny scales mixed in one
+    causet (the tile range test), all through CS_A1_TENSOR (gpu_bits checks every route)."""
+    coords = np.zeros((600, 4)); coords[10:20, 1] = np.nan; coords[300:, 0] = 1.0
+    assert np.array_equal(to_u64(gpu_bits(api, coords, inp.GEOM_MINK_CONE)[0]),
+                          oracle.causal_matrix_bits(coords, inp.GEOM_MINK_CONE))
+    mixed = inp.sprinkle(inp.GEOM_MINK_CONE, 4, 1200, 4)
+    mixed[400:800] *= 2.0 ** 50; mixed[800:] *= 2.0 ** -50
+    mixed = np.ascontiguousarray(mixed[np.lexsort((mixed[:, 1], mixed[:, 0]))])
+    assert np.array_equal(to_u64(gpu_bits(api, mixed, inp.GEOM_MINK_CONE)[0]),
+                          oracle.causal_matrix_bits(mixed, inp.GEOM_MINK_CONE))
 
 
 def test_causal_matrix_lightcone_ties(api, oracle):
