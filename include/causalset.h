@@ -139,10 +139,12 @@ int cs_causal_matrix_ex(const double *coords, int64_t B, int64_t N, int dim, int
 
 /* CS_A1_TENSOR on one flat-cone causet (dim 4 or 5) with its counters on: what the tensor-core value of the bilinear form
  * was worth on this input.  Writes bits / bitsT as cs_causal_matrix does.
- *   out_host  host, double[4], overwritten: [0] the largest |a - T| seen, in units of 2^-24 C^2 (a = tensor-core value,
+ *   out_host  host, double[5], overwritten: [0] the largest |a - T| seen, in units of 2^-24 C^2 (a = tensor-core value,
  *             T = the form evaluated in fp64, C = largest |coordinate| of the tile; over all pairs decided by sign),
- *             [1] (row, 32-column block) pairs re-evaluated in fp64, [2] (row, block) pairs examined, [3] the margin the
- *             kernel uses, same unit as [0].
+ *             [1] (row, 32-column block) pairs re-evaluated in fp64, [2] (row, block) pairs examined, [3] the largest
+ *             |a - T| / m, m = the margin of the pair's tile (a decision by sign can only be wrong if this reaches 1),
+ *             [4] the largest |a - S| in the unit of [0], S = the exact sum of the products of the bf16 operand pieces
+ *             the tensor core was given (its accumulation error alone).
  * Synchronises `stream`.  Errors: CS_ERR_ARG, CS_ERR_DIM, CS_ERR_WORKSPACE, CS_ERR_CUDA. */
 int cs_a1_tensor_probe(const double *coords, int64_t N, int dim, uint64_t *bits, uint64_t *bitsT,
                        void *workspace, size_t workspace_bytes, double *out_host, void *stream);

@@ -184,18 +184,18 @@ def causal_matrix_batched(coords: torch.Tensor, geometry: int, want_transpose: b
 
 def a1_tensor_probe(coords: torch.Tensor):
     """CS_A1_TENSOR on one flat-cone causet (dim 4 or 5) with its counters on ->
-    (bits, bitsT, {"max_err_u": .., "rows_fp64": .., "rows_total": .., "margin_u": ..})."""
+    (bits, bitsT, {"max_err_u", "max_acc_err_u", "max_err_over_margin", "rows_fp64", "rows_total"})."""
     _need_cuda(coords, torch.float64, "coords")
     N, dim = coords.shape
     stride = row_stride_words(N)
     bits = torch.empty((N, stride), dtype=torch.int64, device=coords.device)
     bitsT = torch.empty((N, stride), dtype=torch.int64, device=coords.device)
     ws = _workspace(causal_matrix_workspace(1, N, dim, GEOM_MINK_CONE, A1_TENSOR), coords.device)
-    out = (ctypes.c_double * 4)()
+    out = (ctypes.c_double * 5)()
     _check(load().cs_a1_tensor_probe(_dptr(coords), N, dim, _dptr(bits), _dptr(bitsT), _dptr(ws), ws.numel(),
                                      ctypes.addressof(out), _stream()), "cs_a1_tensor_probe")
     return bits, bitsT, {"max_err_u": float(out[0]), "rows_fp64": int(out[1]), "rows_total": int(out[2]),
-                         "margin_u": float(out[3])}
+                         "max_err_over_margin": float(out[3]), "max_acc_err_u": float(out[4])}
 
 
 def transpose_bits(bits: torch.Tensor, N: int) -> torch.Tensor:

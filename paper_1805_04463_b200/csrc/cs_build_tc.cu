@@ -11,28 +11,43 @@
 // products) bf16 columns per point, and T for a 128 x 256 block of pairs is two (three) tcgen05.mma kind::f16
 // instructions with fp32 accumulation in TMEM -- 1/32 of what the FMA pipes need for the same block.
 //
-// What the tensor core returns is a value `a` with |a - T| <= E: the error of the fp32 prefilter's inputs (the same
-// fp64 -> fp32 conversions as in cs_build.cu: <= 11.04 u C^2 for four products, u = 2^-24, C = largest |component|
-// of the tile), the dropped piece products (<= 2.01 NP u C^2) and the accumulation inside the tensor core.  The order
-// and the width of that accumulation are not documented; the margin below assumes nothing about the order and allows
-// every one of the K + 1 addends of an instruction to lose one unit in the last place of an fp32 number as large as
-// the largest partial sum can be ((NP / 2 + 2 + NP) C^2 <= 8 C^2: <= 2^-20 C^2 per addend), i.e. E <= (K + 3) 2^-20
-// C^2 + 20 u C^2 < 2^-14 C^2 for K <= 48.  `cs_a1_tc_probe` measures |a - T| against the fp64 value on real tiles
-// (profiles/r2_a1_tensor.md: the largest error seen is ~3 u C^2, 300 times below the margin).
-//     |a| > m = 2^-14 C^2   =>   sign(a) = sign(T), and |T| > 2^-15 C^2 is far outside the rounding of the fp64
-//                                expression of the header (2^-46 C^2): related iff a > 0
+// What the tensor core returns is a value `a` with |a - T| <= E = E_in + E_acc (u = 2^-24, C = largest |component| of
+// the tile):
+//   E_in   the inputs of the fp32 prefilter (the same fp64 -> fp32 conversions as in cs_build.cu; Fast::MARGIN / 2 u C^2
+//          covers them with room) and the dropped piece products (<= 2.01 NP u C^2): (MARGIN / 2 + 3 NP) u C^2.
+//   E_acc  the accumulation inside the tensor core, whose width and order are not documented.  Model taken (the one
+//          published analyses of earlier generations found, and what the probe below measures here): an instruction
+//          aligns its 16 products and the accumulator to the largest exponent among them, keeps at least 24 bits, adds
+//          exactly and rounds once -- every addend loses less than 2^-23 of the largest one.  For a pair near the cone
+//          (|T| small, the only pairs whose sign an error can change) the largest addend is at most
+//          M = max(|h_i|, |h_j|, |P_c(i) F_c(j)|), bounded per tile from per-128-point maxima, so
+//          E_acc <= (K + 2) 2 u M over the K / 16 instructions; for a pair with |T| >= M the same model gives a relative
+//          error of (K + 2) 2 u, which cannot change a sign either.
+// The margin is m = (4 (K + 2) M + (MARGIN / 2 + 3 NP) C^2) u, i.e. TWICE the modelled accumulation loss.
+// `cs_a1_tensor_probe` measures on real tiles |a - T| against the fp64 value, |a - S| against the exact sum S of the
+// operand products, and the largest |a - T| / m (profiles/r2_a1_tensor.md: the accumulation alone loses up to 14 u C^2
+// -- the tensor core does truncate --, |a - T| / m stays below 0.08).
+//     |a| > m   =>   sign(a) = sign(T), and |T| is far outside the rounding of the fp64 expression of the header
+//                    (2^-46 C^2): related iff a > 0
 //     anything else (NaN included): the 32 pairs of that ROW of the block are re-evaluated with the fp64 expression.
 // As in cs_build.cu a tile takes the prefilter only if dt >= 0 is known for every pair it keeps (time order per
 // tile, checked on the doubles by the prep kernel), 2^-40 <= C <= 2^40 and every point is finite and passes
 // Fast::convert; otherwise m = +inf and every row goes to fp64.  The output is bit-identical to the fp64 evaluation
-// by construction.
+// as long as the model above holds; the parity tests compare every bit with the oracle.
 //
 // Kernels: k_tc_prep (one thread per point: conversion, pieces, both operand rows in the UMMA canonical K-major
-// layout, per-128-point summaries) and k_causal_tc (persistent, one CTA per SM: a bulk-copy loader, a one-thread MMA
-// issuer, 16 epilogue warps).  An epilogue warp reads 32 rows x 32 columns of accumulators (tcgen05.ld, lane = row),
-// shifts the 32 sign bits of its row into one word (one SHF per pair), keeps min |a| (one FMNMX3 per two pairs),
-// transposes the 32 x 32 bit block with the shuffle butterfly for the second output, and stages both in shared
-// memory; a 256 x 256 tile leaves as full 32-byte row segments, mirrored zero tiles included.
+// layout, a padded copy of the coordinates, per-128-point summaries), k_tc_tiles (one thread per tile: its (I, J), causet
+// and margin) and k_causal_tc (persistent, one CTA per SM):
+//   loader (1 thread)    bulk copies of the tile's operand rows and coordinates into a 3-deep ring
+//   MMA issuer (1 thread) K / 16 tcgen05.mma (M = 128, N = 256) per half tile into two TMEM accumulators
+//   16 epilogue warps    each 32 rows x 64 columns of a half: tcgen05.ld (lane = row), the 32 sign bits of the row into
+//                        one word (funnel shift on the ALU pipe; TC_NF of them through fma.sat on the idle FMA pipe),
+//                        min |a| (one FMNMX3 per two pairs), fp64 rows if the minimum is inside the band, the shuffle
+//                        butterfly for the transposed output (interleaved with the next block's extraction), both
+//                        words staged in shared memory
+//   2 writer warps       the staged 256 x 256 tile to global memory as 32-byte row segments; the mirrored tile of an
+//                        off-diagonal tile as two TMA tile stores from a constant zero tile.
+// The kernel is bound by instruction issue / the ALU pipe: 1.5 instructions per pair are the floor of this scheme.
 #include <cuda.h>
 #include <cuda_bf16.h>
 
@@ -54,7 +69,6 @@ constexpr int TC_WR0 = TC_EPI0 + TC_EPI_WARPS;   // warps 18..19: writers (stage
 constexpr int TC_WR_WARPS = 2;
 constexpr int TC_THREADS = (TC_WR0 + TC_WR_WARPS) * 32;
 constexpr int TC_PITCH = 9;              // words per staged row (8 + 1: conflict-free 4-byte stores by 32 rows)
-constexpr int TC_MARGIN_LOG2 = -14;      // m = 2^-14 C^2
 #ifndef TC_NF
 #define TC_NF 12                         // columns of a 32 x 32 block whose sign bit goes through the FMA pipe (0 .. 23)
 #endif
@@ -76,9 +90,11 @@ struct TcBlockInfo {                     // summary of 128 consecutive points
     float C;                             // largest |fp32 component|
     uint32_t flags;                      // 1: t non-decreasing inside the block, 2: last point <= first of the next block, 4: a point
                                          // that may not use the prefilter (not finite, or Fast::convert says no)
-    uint32_t pad[2];
+    float cmax[6];                       // largest |fp32 component| per component (0 beyond NP)
+    float hmax;                          // largest |h|
+    uint32_t pad[3];
 };
-static_assert(sizeof(TcBlockInfo) == 32, "TcBlockInfo");
+static_assert(sizeof(TcBlockInfo) == 64, "TcBlockInfo");
 
 __device__ __forceinline__ uint32_t tc_smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
 __device__ __forceinline__ void tc_mbar_init(uint64_t *bar, uint32_t count)
@@ -292,7 +308,16 @@ k_tc_prep(const double *__restrict__ coords, int64_t N, int nA,
     }
     __shared__ double s_mn[4], s_mx[4];
     __shared__ float s_c[4];
-    if (lane == 0) { s_mn[warp] = tmn; s_mx[warp] = tmx; s_c[warp] = c; }
+    __shared__ uint32_t s_cm[4][7];
+    uint32_t cm[7];                                       // |component| and |h| maxima: non-negative floats order like their bits
+#pragma unroll
+    for (int q = 0; q < 6; q++) cm[q] = __reduce_max_sync(0xffffffffu, (q < NP && valid) ? (__float_as_uint(v[q]) & 0x7fffffffu) : 0u);
+    cm[6] = __reduce_max_sync(0xffffffffu, (F::H && valid) ? (__float_as_uint(h) & 0x7fffffffu) : 0u);
+    if (lane == 0) {
+        s_mn[warp] = tmn; s_mx[warp] = tmx; s_c[warp] = c;
+#pragma unroll
+        for (int q = 0; q < 7; q++) s_cm[warp][q] = cm[q];
+    }
     const int inner = __syncthreads_and(sorted || tid == 127);
     const int link = __syncthreads_and(sorted || tid != 127);
     const int bad = __syncthreads_or(!ok);
@@ -302,7 +327,10 @@ k_tc_prep(const double *__restrict__ coords, int64_t N, int nA,
         bi.tmax = fmax(fmax(s_mx[0], s_mx[1]), fmax(s_mx[2], s_mx[3]));
         bi.C = fmaxf(fmaxf(s_c[0], s_c[1]), fmaxf(s_c[2], s_c[3]));
         bi.flags = (inner ? 1u : 0u) | (link ? 2u : 0u) | (bad ? 4u : 0u);
-        bi.pad[0] = bi.pad[1] = 0;
+#pragma unroll
+        for (int q = 0; q < 6; q++) bi.cmax[q] = __uint_as_float(max(max(s_cm[0][q], s_cm[1][q]), max(s_cm[2][q], s_cm[3][q])));
+        bi.hmax = __uint_as_float(max(max(s_cm[0][6], s_cm[1][6]), max(s_cm[2][6], s_cm[3][6])));
+        bi.pad[0] = bi.pad[1] = bi.pad[2] = 0;
         info[(size_t)b * nA + a] = bi;
     }
 }
@@ -311,7 +339,8 @@ k_tc_prep(const double *__restrict__ coords, int64_t N, int nA,
 // One entry per tile of the launch, row-major over the upper triangle (J >= I) of every causet:
 //   x = I | J << 16, y = causet, z = margin m (float bits; +inf: every row of the tile goes to fp64), w = unused.
 __global__ void __launch_bounds__(256)
-k_tc_tiles(const TcBlockInfo *__restrict__ info, int nT, uint32_t tiles_per, uint32_t total_tiles, uint4 *__restrict__ tab)
+k_tc_tiles(const TcBlockInfo *__restrict__ info, int nT, uint32_t tiles_per, uint32_t total_tiles, float acc_units,
+           float in_units, uint4 *__restrict__ tab)
 {
     const uint32_t t = blockIdx.x * 256 + threadIdx.x;
     if (t >= total_tiles) return;
@@ -331,13 +360,20 @@ k_tc_tiles(const TcBlockInfo *__restrict__ info, int nT, uint32_t tiles_per, uin
     const bool ordered = (I == J) ? ((i0.flags & 3u) == 3u && (i1.flags & 1u) != 0)
                                   : (fmax(i0.tmax, i1.tmax) <= fmin(j0.tmin, j1.tmin));
     const bool fast = !bad && ordered && C >= 0x1p-40f && C <= 0x1p40f;
-    const float m = fast ? __fmul_ru(__fmul_ru(C, C), 1.001f * exp2f((float)TC_MARGIN_LOG2)) : __int_as_float(0x7f800000);
+    // largest single addend a pair of this tile can hand to the tensor core: |h_i|, |h_j|, |P_c(i) F_c(j)|
+    float M = fmaxf(fmaxf(i0.hmax, i1.hmax), fmaxf(j0.hmax, j1.hmax));
+#pragma unroll
+    for (int q = 0; q < 6; q++) M = fmaxf(M, __fmul_ru(fmaxf(i0.cmax[q], i1.cmax[q]), fmaxf(j0.cmax[q], j1.cmax[q])));
+    const float m = fast ? __fmul_ru(1.001f * 0x1p-24f, __fmaf_ru(acc_units, M, __fmul_ru(in_units, __fmul_ru(C, C))))
+                         : __int_as_float(0x7f800000);
     tab[t] = make_uint4((uint32_t)I | ((uint32_t)J << 16), b, __float_as_uint(m), __float_as_uint(C));
 }
 
 // ---- main kernel -----------------------------------------------------------------------------------
 struct TcProbe {                 // cs_a1_tensor_probe: what the prefilter saw (all tiles of the launch)
     unsigned int max_err_bits;   // max |a - T| / C^2 as float bits (pairs decided by sign)
+    unsigned int max_acc_bits;   // max |a - exact sum of the operand products| / C^2: the tensor core's own accumulation error
+    unsigned int max_ratio_bits; // max |a - T| / m, m = the margin of the pair's tile: must stay below 1
     unsigned int pad;
     unsigned long long rows_fp64;   // (row, 32-column block) pairs re-evaluated in fp64
     unsigned long long rows_total;  // (row, block) pairs examined
@@ -455,7 +491,7 @@ k_causal_tc(const __grid_constant__ CUtensorMap mapB, const __grid_constant__ CU
         const int g = e >> 2;                         // 64 columns of the 256
         const TransposeLane transpose(lane);
         uint32_t n = 0;
-        float p_err = 0.f;
+        float p_err = 0.f, p_acc = 0.f, p_ratio = 0.f;
         unsigned long long p_rows = 0, p_tot = 0;
         uint2 ent = blockIdx.x < total_tiles ? __ldg(reinterpret_cast<const uint2 *>(tab + blockIdx.x)) : make_uint2(0, 0);
         uint32_t ent_m = blockIdx.x < total_tiles ? __ldg(reinterpret_cast<const uint32_t *>(tab + blockIdx.x) + 2) : 0;
@@ -505,6 +541,11 @@ k_causal_tc(const __grid_constant__ CUtensorMap mapB, const __grid_constant__ CU
                         uint32_t v[32];
                         tc_ld32(taddr + k * 32, v);
                         asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+                        if (DIAG && c0 == r0) {                       // the block on the diagonal: T(i, i) = 0 would send every row
+#pragma unroll
+                            for (int c = 0; c < 32; c++)              // to fp64; pairs with j <= i read -inf (unrelated, outside the band)
+                                if (c <= lane) v[c] = 0xff800000u;
+                        }
                         // Sign bits.  The kernel is bound by instruction issue and by the ALU pipe (SHF, FMNMX3, LOP3: one warp
                         // instruction per two clocks) while the FMA pipe is idle: TC_NF columns take their bit through it,
                         //     t = fma.sat(a, 2^100, 0.5)      1.0 if a > 0, 0.0 if a < 0 (|a| > m >= 2^-94; in-band rows are redone)
@@ -572,7 +613,24 @@ k_causal_tc(const __grid_constant__ CUtensorMap mapB, const __grid_constant__ CU
                                         T += d == 0 ? dd * dd : -dd * dd;
                                     }
                                     const float er = (float)(fabs((double)__uint_as_float(v[c]) - 0.5 * T) / (double)C2);
-                                    if (er == er) p_err = fmaxf(p_err, er);      // (padding points are NaN)
+                                    if (er == er && isfinite(__uint_as_float(v[c]))) {      // (padding points are NaN, masked pairs -inf)
+                                        p_err = fmaxf(p_err, er);
+                                        p_ratio = fmaxf(p_ratio, er * C2 / m);
+                                    }
+                                    // the same pair from the operand rows the tensor core read (every product of two bf16
+                                    // pieces is exact in fp64, and so is their sum to 2^-50)
+                                    const unsigned char *st_ = s_stage + (size_t)s * SM::STAGE;
+                                    const int ra = (r0 + lane) & 127, hb = (r0 + lane) >> 7;
+                                    double ex = 0.0;
+                                    for (int kk = 0; kk < S::K; kk++) {
+                                        const uint16_t ua = *reinterpret_cast<const uint16_t *>(
+                                            st_ + hb * S::A_BLOCK + ((kk >> 3) * 128 + ra) * 16 + (kk & 7) * 2);
+                                        const uint16_t ub = *reinterpret_cast<const uint16_t *>(
+                                            st_ + 2 * S::A_BLOCK + ((kk >> 3) * 256 + c0 + c) * 16 + (kk & 7) * 2);
+                                        ex += (double)__uint_as_float((uint32_t)ua << 16) * (double)__uint_as_float((uint32_t)ub << 16);
+                                    }
+                                    const float ea = (float)(fabs((double)__uint_as_float(v[c]) - ex) / (double)C2);
+                                    if (er == er && fabs(ex) < 1e30 && isfinite(__uint_as_float(v[c]))) p_acc = fmaxf(p_acc, ea);
                                 }
                             }
                         }
@@ -615,11 +673,15 @@ k_causal_tc(const __grid_constant__ CUtensorMap mapB, const __grid_constant__ CU
 #pragma unroll
             for (int sft = 16; sft >= 1; sft >>= 1) {
                 p_err = fmaxf(p_err, __shfl_xor_sync(0xffffffffu, p_err, sft));
+                p_acc = fmaxf(p_acc, __shfl_xor_sync(0xffffffffu, p_acc, sft));
+                p_ratio = fmaxf(p_ratio, __shfl_xor_sync(0xffffffffu, p_ratio, sft));
                 p_rows += __shfl_xor_sync(0xffffffffu, p_rows, sft);
                 p_tot += __shfl_xor_sync(0xffffffffu, p_tot, sft);
             }
             if (lane == 0) {
                 atomicMax(&probe->max_err_bits, __float_as_uint(p_err));
+                atomicMax(&probe->max_acc_bits, __float_as_uint(p_acc));
+                atomicMax(&probe->max_ratio_bits, __float_as_uint(p_ratio));
                 atomicAdd(&probe->rows_fp64, p_rows);
                 atomicAdd(&probe->rows_total, p_tot);
             }
@@ -704,7 +766,10 @@ int launch_tc_t(const double *coords, int64_t B, int64_t N, int64_t stride, uint
     uint4 *tab = reinterpret_cast<uint4 *>(reinterpret_cast<unsigned char *>(cpad) + align_up((size_t)B * nT * TCT * DIM * 8, 256));
     k_tc_prep<GEOM, DIM><<<dim3(2 * nT, (unsigned)B), 128, 0, st>>>(coords, N, 2 * nT, opA, opB, info, cpad);
     CS_LAUNCHED("k_tc_prep");
-    k_tc_tiles<<<(unsigned)((total + 255) / 256), 256, 0, st>>>(info, nT, (uint32_t)tiles_per, (uint32_t)total, tab);
+    // margin m = (ACC M + IN C^2) 2^-24, see the header: ACC = 4 (K + 2) (twice the alignment loss of K + 2 addends),
+    // IN = the fp32 prefilter's own bound (Fast::MARGIN / 2, conversions included) + the dropped piece products
+    k_tc_tiles<<<(unsigned)((total + 255) / 256), 256, 0, st>>>(info, nT, (uint32_t)tiles_per, (uint32_t)total,
+                                                                 4.f * (S::K + 2), (float)(Fast<GEOM, DIM>::MARGIN / 2 + 3 * Fast<GEOM, DIM>::NP), tab);
     CS_LAUNCHED("k_tc_tiles");
     constexpr size_t smem = SM::BYTES;
     static PerDeviceFlag attr_set;
@@ -777,7 +842,9 @@ int launch_causal_tc(const double *coords, int64_t B, int64_t N, int dim, int ge
 
 // The same launch with the probe counters switched on (flat cone in 3+1 and 4+1 dimensions: K = 32 and K = 48).
 // out_host: [0] largest |a - T| / (2^-24 C^2) over the pairs decided by sign, [1] (row, block) pairs sent to fp64,
-// [2] (row, block) pairs examined, [3] the margin in the same unit.
+// [2] (row, block) pairs examined, [3] largest |a - T| / m with m the margin of the pair's tile (< 1 or a decision by sign
+// could be wrong), [4] largest |a - exact sum of the operand products|
+// in the same unit (what the tensor core's accumulation alone lost).
 int launch_causal_tc_probe(const double *coords, int64_t N, int dim, uint64_t *bits, uint64_t *bitsT,
                            void *scratch, double *out_host, cudaStream_t st)
 {
@@ -801,7 +868,10 @@ int launch_causal_tc_probe(const double *coords, int64_t N, int dim, uint64_t *b
     out_host[0] = (double)err * 16777216.0;
     out_host[1] = (double)hp.rows_fp64;
     out_host[2] = (double)hp.rows_total;
-    out_host[3] = ldexp(1.0, 24 + TC_MARGIN_LOG2);
+    memcpy(&err, &hp.max_ratio_bits, 4);
+    out_host[3] = (double)err;
+    memcpy(&err, &hp.max_acc_bits, 4);
+    out_host[4] = (double)err * 16777216.0;
     return CS_OK;
 }
 

@@ -313,7 +313,7 @@ def test_causal_matrix_tensor_route_arguments_and_probe(api, oracle):
         bits, bitsT, st = api.a1_tensor_probe(torch.from_numpy(coords).cuda())
         assert np.array_equal(to_u64(bits), o_bits)
         assert np.array_equal(to_u64(bitsT), oracle.transpose_bits(o_bits, 3000))
-        assert 0.0 < st["max_err_u"] < st["margin_u"] / 8, st
+        assert 0.0 < st["max_err_over_margin"] < 0.25 and 0.0 < st["max_acc_err_u"] < 64.0, st
         assert 0 < st["rows_fp64"] < st["rows_total"] / 10, st
         rng = np.random.default_rng(3)
         shuffled = np.ascontiguousarray(coords[rng.permutation(3000)])
