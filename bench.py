@@ -255,6 +255,35 @@ def run_peaks(args, local_rank):
 A1_ROUTES = {"auto": 0, "fma": 1, "tensor": 2}
 
 
+def run_a1_probe(args, local_rank):
+    """cs_a1_tensor_probe on seeded sprinklings: what the tensor-core value of the bilinear form is worth (error against the
+    fp64 value, the accumulation error alone, error over margin, rows sent to fp64), and the two a1 routes timed side by side."""
+    import torch
+    from paper_1805_04463_b200 import api, inputs as inp
+    torch.cuda.set_device(local_rank)
+    api.load()
+    out = {}
+    cases = [("mink4_N65536", inp.GEOM_MINK_CONE, 4, 65536, inp.CONFIGS[3].seed), ("mink4_N2048", inp.GEOM_MINK_CONE, 4, 2048, 7),
+             ("mink5_N16384", inp.GEOM_MINK_CONE, 5, 16384, 7)]
+    for name, geom, dim, N, seed in cases:
+        d = torch.from_numpy(inp.sprinkle(geom, dim, N, seed)).cuda()
+        bits, bitsT, st = api.a1_tensor_probe(d)
+        ref, refT = api.causal_matrix(d, geom, route=api.A1_FMA)
+        st["equal_to_fma_route"] = bool(torch.equal(bits, ref) and torch.equal(bitsT, refT))
+        for rname, route in (("fma", api.A1_FMA), ("tensor", api.A1_TENSOR)):
+            ws = torch.empty(max(api.causal_matrix_workspace(1, N, dim, geom, route), 256), dtype=torch.uint8, device="cuda")
+            for _ in range(3):
+                api.causal_matrix(d, geom, route=route, workspace=ws)
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            torch.cuda.synchronize(); e0.record()
+            for _ in range(10):
+                api.causal_matrix(d, geom, route=route, workspace=ws)
+            e1.record(); torch.cuda.synchronize()
+            st["ms_" + rname] = e0.elapsed_time(e1) / 10      # (includes torch.empty of the two outputs: ~10 us)
+        out[name] = st
+    print(json.dumps({"a1_tensor_probe": out, "units": "max_err_u, max_acc_err_u: 2^-24 C^2; max_err_over_margin: must stay below 1"}))
+
+
 def time_single(api, cfg, N, route, steps, warmup, seed, local_rank, csd, e2e=True, a1_route=0):
     """K timed steps of a1 -> a2 -> a3 on one seeded sprinkling (inputs resident in HBM), device time per stage,
     then (optionally) the same through cs_action_host with pinned host buffers."""
@@ -479,6 +508,7 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-other-configs", action="store_true", help="skip the short passes over configs 2, 4 and 5")
     ap.add_argument("--peaks", action="store_true", help="run the peak probes only")
+    ap.add_argument("--a1-probe", action="store_true", help="run cs_a1_tensor_probe and time the two a1 routes only")
     ap.add_argument("--shard", action="store_true", help="split the rows of one causet over the ranks (NEXT-4)")
     ap.add_argument("--cpu-seconds", type=float, default=12.0)
     ap.add_argument("--ref-seconds", type=float, default=6.0)
@@ -499,6 +529,10 @@ def main():
     if args.peaks:
         if rank == 0:
             run_peaks(args, local_rank)
+        return
+    if args.a1_probe:
+        if rank == 0:
+            run_a1_probe(args, local_rank)
         return
     if args.shard:
         run_shard(args, cfg, rank, local_rank, world)

@@ -131,8 +131,8 @@ enum cs_a1_route {
  *              stream-ordered memory pool the library owns on this device.
  * bits / bitsT must be 16-byte aligned.  Errors as cs_causal_matrix, + CS_ERR_WORKSPACE. */
 size_t cs_causal_matrix_workspace(int64_t B, int64_t N, int dim, int geometry, int route);
-/* What CS_A1_AUTO resolves to for B causets of N points: CS_A1_TENSOR for the bilinear predicates from about 2^21 pairs
- * up (N >= 256), else CS_A1_FMA. */
+/* What CS_A1_AUTO resolves to for B causets of N points: CS_A1_TENSOR for the bilinear predicates once the launch has
+ * at least 128 tiles of 256 x 256 pairs (one causet: N >= 3841; ensembles earlier; always N >= 256), else CS_A1_FMA. */
 int cs_default_a1_route(int64_t B, int64_t N, int dim, int geometry);
 int cs_causal_matrix_ex(const double *coords, int64_t B, int64_t N, int dim, int geometry, int route,
                         uint64_t *bits, uint64_t *bitsT, void *workspace, size_t workspace_bytes, void *stream);

@@ -322,12 +322,14 @@ int cs_greedy_antichain(const uint64_t *bits, const uint64_t *bitsT, int64_t N, 
 // ENSEMBLE_MAT_BYTES), not of the ensemble (4 GiB for 4096 x 2048).  CB is a whole number of causets per CTA pair
 // of a2's persistent grid (causet-major schedule: every pair then gets the same number of causets).
 // workspace: [bits CB*N*stride][bitsT CB*N*stride][hist B*4 int64][interval scratch]
-constexpr size_t ENSEMBLE_MAT_BYTES = (size_t)448 << 20;     // both matrices of a chunk + the scratch of its a1
+constexpr size_t ENSEMBLE_MAT_BYTES = (size_t)500 << 20;     // both matrices of a chunk + the scratch of its a1
 
-// a1 scratch of cb causets, whatever the geometry (the workspace queries do not know it): the widest operand rows
+// a1 scratch of cb causets carved from the workspace.  The workspace queries do not know the geometry: the carve is sized
+// for the K = 32 operand rows with the widest coordinates (Eq. 7.7: six doubles per point), which covers the flat cone up
+// to 3+1 dimensions; the two geometries with K = 48 rows take their scratch from the library's pool instead.
 static size_t ensemble_a1_scratch(int64_t cb, int64_t N)
 {
-    return align_up(causal_tc_scratch_bytes(cb, N, 7, CS_GEOM_DS4_SPHERICAL), 256);
+    return align_up(causal_tc_scratch_bytes(cb, N, 6, CS_GEOM_FLRW_POLAR), 256);
 }
 
 static int64_t ensemble_chunk(int64_t B, int64_t N)
@@ -373,7 +375,9 @@ int cs_bd_action_batched(const double *coords, int64_t B, int64_t N, int dim, in
     if (kmax < 3) CS_CUDA(cudaMemsetAsync(hist, 0, (size_t)B * 4 * 8, st));
     for (int64_t b0 = 0; b0 < B; b0 += CB) {
         const int64_t nb = B - b0 < CB ? B - b0 : CB;
-        int rc = cs_causal_matrix_ex(coords + b0 * N * dim, nb, N, dim, geometry, CS_A1_AUTO, bits, bitsT, a1ws, a1_bytes, stream);
+        const bool fits = cs_causal_matrix_workspace(nb, N, dim, geometry, CS_A1_AUTO) <= a1_bytes;
+        int rc = cs_causal_matrix_ex(coords + b0 * N * dim, nb, N, dim, geometry, CS_A1_AUTO, bits, bitsT, fits ? a1ws : nullptr,
+                                     fits ? a1_bytes : 0, stream);
         if (rc) return rc;
         rc = interval_hist_impl(bits, bitsT, nb, N, kmax, 0, N, CS_ROUTE_AUTO, hist + b0 * (kmax + 1), nullptr, iws,
                                 (size_t)(a1ws - iws), st);
@@ -481,7 +485,9 @@ int cs_bd_action_batched_host(const double *coords_host, int64_t B, int64_t N, i
                                 cudaMemcpyHostToDevice, copy_stream));
         CS_CUDA(cudaEventRecord(copied[buf], copy_stream));
         CS_CUDA(cudaStreamWaitEvent(st, copied[buf], 0));
-        int rc = cs_causal_matrix_ex(cdev[buf], nb, N, dim, geometry, CS_A1_AUTO, bits, bitsT, a1ws, a1_bytes, stream);
+        const bool fits = cs_causal_matrix_workspace(nb, N, dim, geometry, CS_A1_AUTO) <= a1_bytes;
+        int rc = cs_causal_matrix_ex(cdev[buf], nb, N, dim, geometry, CS_A1_AUTO, bits, bitsT, fits ? a1ws : nullptr,
+                                     fits ? a1_bytes : 0, stream);
         if (rc) return rc;
         CS_CUDA(cudaEventRecord(consumed[buf], st));
         if (kmax < 3) CS_CUDA(cudaMemsetAsync(hist, 0, (size_t)nb * 4 * 8, st));
@@ -535,7 +541,8 @@ int cs_action_host(const double *coords_host, int64_t N, int dim, int geometry, 
     const size_t left = (size_t)(a1ws - ws);
 
     if (N > 0) CS_CUDA(cudaMemcpyAsync(coords, coords_host, (size_t)N * dim * 8, cudaMemcpyHostToDevice, st));
-    int rc = cs_causal_matrix_ex(coords, 1, N, dim, geometry, CS_A1_AUTO, bits, bitsT, a1ws, a1_bytes, stream);
+    const bool fits = cs_causal_matrix_workspace(1, N, dim, geometry, CS_A1_AUTO) <= a1_bytes;
+    int rc = cs_causal_matrix_ex(coords, 1, N, dim, geometry, CS_A1_AUTO, bits, bitsT, fits ? a1ws : nullptr, fits ? a1_bytes : 0, stream);
     if (rc) return rc;
     rc = cs_interval_hist(bits, bitsT, N, kmax, hist, nullptr, ws, left, stream);
     if (rc) return rc;

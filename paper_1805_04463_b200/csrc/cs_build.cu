@@ -468,17 +468,19 @@ static int launch_causal_fma(const double *coords, int64_t B, int64_t N, int dim
     }
 }
 
-// Which kernel builds the matrix.  The tensor route (cs_build_tc.cu) serves the bilinear predicates; measured on
-// B200 it wins from a few 256 x 256 tiles per SM up, below that the persistent kernel's set-up (TMEM allocation,
-// operand prep launch) is not paid back.
-constexpr int64_t TC_MIN_PAIRS = (int64_t)1 << 21;      // B * N^2 / 2 pairs: 2048 points of one causet
+// Which kernel builds the matrix.  The tensor route (cs_build_tc.cu) serves the bilinear predicates; it is a persistent
+// kernel over 256 x 256 tiles, one CTA per SM, and wins once there are about as many tiles as SMs (measured on B200,
+// flat cone in 3+1: 0.38 against 0.75 ms at N = 65536, 0.043 against 0.071 ms at N = 16384; a single causet of N = 2048 --
+// 36 tiles -- takes 0.034 against 0.023 ms, while 296 of them take 0.13 against 0.27 ms).
+constexpr int64_t TC_MIN_TILES = 128;
 
 static int resolve_a1_route(int64_t B, int64_t N, int dim, int geometry, int route)
 {
     if (route == CS_A1_FMA) return CS_A1_FMA;
     const bool can = causal_tc_supported(geometry, dim) && N >= 256;      // (rows of at least 32 bytes: TMA boxes)
     if (route == CS_A1_TENSOR) return can ? CS_A1_TENSOR : -1;
-    return can && B * N * N / 2 >= TC_MIN_PAIRS ? CS_A1_TENSOR : CS_A1_FMA;
+    const int64_t nT = (N + 255) / 256;
+    return can && B * (nT * (nT + 1) / 2) >= TC_MIN_TILES ? CS_A1_TENSOR : CS_A1_FMA;
 }
 
 size_t causal_matrix_scratch_bytes(int64_t B, int64_t N, int dim, int geometry, int route)
