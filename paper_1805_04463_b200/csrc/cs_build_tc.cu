@@ -121,6 +121,22 @@ __device__ __forceinline__ void tc_mbar_wait(uint64_t *bar, uint32_t parity)
         "r"(parity), "r"(0x989680u)
         : "memory");
 }
+// the same for the roles that mostly wait (loader, MMA issuer, writers): between two tries the warp sleeps, so that its
+// polling does not take issue slots from the epilogue warps of its scheduler (12 % of all instructions without it)
+__device__ __forceinline__ void tc_mbar_wait_sleep(uint64_t *bar, uint32_t parity, uint32_t ns)
+{
+    uint32_t done;
+    while (true) {
+        asm volatile(
+            "{\n"
+            ".reg .pred p;\n"
+            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2, %3;\n"
+            "selp.u32 %0, 1, 0, p;\n"
+            "}\n" : "=r"(done) : "r"(tc_smem_u32(bar)), "r"(parity), "r"(0x989680u) : "memory");
+        if (done) break;
+        __nanosleep(ns);
+    }
+}
 __device__ __forceinline__ void tc_mbar_expect_tx(uint64_t *bar, uint32_t bytes)
 {
     asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(tc_smem_u32(bar)), "r"(bytes) : "memory");
@@ -450,7 +466,7 @@ k_causal_tc(const __grid_constant__ CUtensorMap mapB, const __grid_constant__ CU
                 const uint4 e = __ldg(tab + t);
                 const uint32_t I = e.x & 0xFFFFu, J = e.x >> 16, b = e.y;
                 const uint32_t s = n % NSTG;
-                tc_mbar_wait(&s_empty[s], ((n / NSTG) & 1) ^ 1);
+                tc_mbar_wait_sleep(&s_empty[s], ((n / NSTG) & 1) ^ 1, 800);
                 tc_mbar_expect_tx(&s_full[s], (uint32_t)SM::STAGE);
                 unsigned char *dst = s_stage + (size_t)s * SM::STAGE;
                 const unsigned char *cp = reinterpret_cast<const unsigned char *>(cpad) + (size_t)b * nT * SM::COORD;
@@ -466,12 +482,12 @@ k_causal_tc(const __grid_constant__ CUtensorMap mapB, const __grid_constant__ CU
             uint32_t n = 0;
             for (uint32_t t = blockIdx.x; t < total_tiles; t += gridDim.x, n++) {
                 const uint32_t s = n % NSTG;
-                tc_mbar_wait(&s_full[s], (n / NSTG) & 1);
+                tc_mbar_wait_sleep(&s_full[s], (n / NSTG) & 1, 100);
                 const uint32_t a_addr = tc_smem_u32(s_stage + (size_t)s * SM::STAGE);
                 const uint32_t b_addr = a_addr + 2 * S::A_BLOCK;
 #pragma unroll
                 for (int h = 0; h < 2; h++) {
-                    tc_mbar_wait(&s_tempty[h], (n & 1) ^ 1);     // the epilogue has read accumulator h of the tile before
+                    tc_mbar_wait_sleep(&s_tempty[h], (n & 1) ^ 1, 100);     // the epilogue has read accumulator h of the tile before
                     tc_fence_after();
 #pragma unroll
                     for (int q = 0; q < S::KC / 2; q++) {             // K = 16 per instruction: two 16-byte chunks
@@ -715,7 +731,7 @@ k_causal_tc(const __grid_constant__ CUtensorMap mapB, const __grid_constant__ CU
             const uint32_t *u = s_U + (n & 1) * TCT * TC_PITCH + rr * TC_PITCH + hf * 4;
             const uint32_t *l = s_L + (n & 1) * TCT * TC_PITCH + rr * TC_PITCH + hf * 4;
             int64_t gi = (int64_t)I * TCT + rr, gj = (int64_t)J * TCT + rr;
-            tc_mbar_wait(&s_sfull[n & 1], (n >> 1) & 1);
+            tc_mbar_wait_sleep(&s_sfull[n & 1], (n >> 1) & 1, 400);
 #pragma unroll
             for (int p = 0; p < 8; p++) {
                 if (gi < N && okJ) *reinterpret_cast<uint4 *>(pb + (size_t)gi * row_bytes) = make_uint4(u[0], u[1], u[2], u[3]);
