@@ -25,7 +25,7 @@
 //          error of (K + 2) 2 u, which cannot change a sign either.
 // The margin is m = (4 (K + 2) M + (MARGIN / 2 + 3 NP) C^2) u, i.e. TWICE the modelled accumulation loss.
 // `cs_a1_tensor_probe` measures on real tiles |a - T| against the fp64 value, |a - S| against the exact sum S of the
-// operand products, and the largest |a - T| / m (profiles/r2_a1_tensor.md: the accumulation alone loses up to 14 u C^2
+// operand products, and the largest |a - T| / m (profiles/r2b_a1_tensor.md: the accumulation alone loses up to 14 u C^2
 // -- the tensor core does truncate --, |a - T| / m stays below 0.08).
 //     |a| > m   =>   sign(a) = sign(T), and |T| is far outside the rounding of the fp64 expression of the header
 //                    (2^-46 C^2): related iff a > 0
