@@ -119,10 +119,11 @@ int cs_causal_matrix_batched(const double *coords, int64_t B, int64_t N, int dim
 enum cs_a1_route {
     CS_A1_AUTO = 0,         /* the library's choice for this geometry and size */
     CS_A1_FMA = 1,          /* every geometry: predicate on the FMA pipes (exact fp32 prefilter, fp64 inside its error band) */
-    CS_A1_TENSOR = 2        /* predicates that are the sign of a bilinear form (CS_GEOM_MINK_CONE, CS_GEOM_FLRW_POLAR,
-                               CS_GEOM_DS4_SPHERICAL): the form as a split-bf16 contraction on tcgen05 tensor cores, rows of a
-                               32 x 32 block with a value inside the error band re-evaluated in fp64.  CS_ERR_ARG for the
-                               other geometries. */
+    CS_A1_TENSOR = 2        /* the predicate as the sign of a bilinear form (every geometry has one: the 1+1 light cone as
+                               du dv, the 1+1 dS slab as cos dtheta - cos d eta, the others as in CS_A1_FMA's prefilter),
+                               evaluated as a split-bf16 contraction on tcgen05 tensor cores; rows of a 32 x 32 block with a
+                               value inside the error band are re-evaluated with the fp64 expression.  N >= 256 (CS_ERR_ARG
+                               below that). */
 };
 
 /* a1 with the route chosen by the caller and an optional workspace (B causets, B = 1 for a single one).
@@ -131,7 +132,7 @@ enum cs_a1_route {
  *              stream-ordered memory pool the library owns on this device.
  * bits / bitsT must be 16-byte aligned.  Errors as cs_causal_matrix, + CS_ERR_WORKSPACE. */
 size_t cs_causal_matrix_workspace(int64_t B, int64_t N, int dim, int geometry, int route);
-/* What CS_A1_AUTO resolves to for B causets of N points: CS_A1_TENSOR for the bilinear predicates once the launch has
+/* What CS_A1_AUTO resolves to for B causets of N points: CS_A1_TENSOR once the launch has
  * at least 128 tiles of 256 x 256 pairs (one causet: N >= 3841; ensembles earlier; always N >= 256), else CS_A1_FMA. */
 int cs_default_a1_route(int64_t B, int64_t N, int dim, int geometry);
 int cs_causal_matrix_ex(const double *coords, int64_t B, int64_t N, int dim, int geometry, int route,

@@ -73,9 +73,56 @@ constexpr int TC_PITCH = 9;              // words per staged row (8 + 1: conflic
 #define TC_NF 12                         // columns of a 32 x 32 block whose sign bit goes through the FMA pipe (0 .. 23)
 #endif
 
+// Per-point data of the tensor route: Fast<> of cs_predicates.cuh for the predicates cs_build.cu already treats as
+// bilinear forms, and two more that are bilinear in derived coordinates only.  F_c is component fcomp(c) of the point's
+// vector (P_c is component c, negated for c < NNEG); time() is what the tiles must be ordered by.
+template <int GEOM, int DIM>
+struct TcFast : Fast<GEOM, DIM> {
+    static constexpr bool RANGE2 = false;        // the tile also needs a bounded range of the second coordinate
+    __device__ static __forceinline__ double time(const double *x) { return x[0]; }
+    __device__ static __forceinline__ constexpr int fcomp(int c) { return c; }
+};
+// 1+1 light cone: (u_i < u_j) && (v_i < v_j)  <=>  T = du dv > 0 and du + dv > 0;  T = h_i + h_j - u_i v_j - v_i u_j with
+// h = u v.  Tiles ordered by t = (u + v) / 2: a pair decided "related" has |du dv| > m, far more than the rounding of t, so
+// du + dv > 0 follows from t_j >= t_i and both differences are positive.
+template <>
+struct TcFast<CS_GEOM_MINK2_LIGHTCONE, 2> {
+    static constexpr bool ok = true, H = true, RANGE2 = false;
+    static constexpr int NP = 2, NNEG = 2, MARGIN = 64;
+    __device__ static __forceinline__ double time(const double *x) { return (x[0] + x[1]) * 0.5; }
+    __device__ static __forceinline__ constexpr int fcomp(int c) { return 1 - c; }
+    __device__ static __forceinline__ bool convert(const double *x, float *v, float &h)
+    {
+        v[0] = (float)x[0];
+        v[1] = (float)x[1];
+        h = (float)(x[0] * x[1]);
+        return true;
+    }
+};
+// 1+1 de Sitter slab: with omega = min(|dtheta|, 2 pi - |dtheta|) the arc between the two angles and 0 <= d eta <= pi,
+// d eta >= omega  <=>  T = cos(dtheta) - cos(d eta) >= 0, bilinear in (cos eta, sin eta, cos theta, sin theta) formed per
+// point in fp64.  The header's expression is that arc only while |dtheta| <= 2 pi: a tile takes the band only if its angles
+// span at most 2 pi and its times at most pi (RANGE2); the fp64 rows use the header's expression as everywhere.
+template <>
+struct TcFast<CS_GEOM_DS2_SLAB, 2> {
+    static constexpr bool ok = true, H = false, RANGE2 = true;
+    static constexpr int NP = 4, NNEG = 2, MARGIN = 64;
+    __device__ static __forceinline__ double time(const double *x) { return x[0]; }
+    __device__ static __forceinline__ constexpr int fcomp(int c) { return c; }
+    __device__ static __forceinline__ bool convert(const double *x, float *v, float &h)
+    {
+        double s0, c0, s1, c1;
+        sincos(x[0], &s0, &c0);
+        sincos(x[1], &s1, &c1);
+        v[0] = (float)c0; v[1] = (float)s0; v[2] = (float)c1; v[3] = (float)s1;
+        h = 0.f;
+        return isfinite(x[0]) && isfinite(x[1]);
+    }
+};
+
 template <int GEOM, int DIM>
 struct TcShape {
-    using F = Fast<GEOM, DIM>;
+    using F = TcFast<GEOM, DIM>;
     static constexpr int USED = 6 * F::NP + (F::H ? 6 : 2);     // without h two columns carry the padding marker
     static constexpr int K = USED <= 32 ? 32 : 48;
     static constexpr int KC = K / 8;                              // 16-byte chunks per operand row
@@ -92,7 +139,8 @@ struct TcBlockInfo {                     // summary of 128 consecutive points
                                          // that may not use the prefilter (not finite, or Fast::convert says no)
     float cmax[6];                       // largest |fp32 component| per component (0 beyond NP)
     float hmax;                          // largest |h|
-    uint32_t pad[3];
+    float x1min, x1max;                  // range of the second coordinate, rounded outwards (RANGE2 geometries only)
+    uint32_t pad;
 };
 static_assert(sizeof(TcBlockInfo) == 64, "TcBlockInfo");
 
@@ -226,7 +274,7 @@ k_tc_prep(const double *__restrict__ coords, int64_t N, int nA,
           unsigned char *__restrict__ opA, unsigned char *__restrict__ opB, TcBlockInfo *__restrict__ info,
           double *__restrict__ cpad)
 {
-    using F = Fast<GEOM, DIM>;
+    using F = TcFast<GEOM, DIM>;
     using S = TcShape<GEOM, DIM>;
     constexpr int NP = F::NP;
     const int a = blockIdx.x, tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -267,7 +315,7 @@ k_tc_prep(const double *__restrict__ coords, int64_t N, int nA,
         uint16_t P[NP][3], Fp[NP][3], hp[3], pp[3];
 #pragma unroll
         for (int q = 0; q < NP; q++) {
-            split3(v[q], Fp[q]);
+            split3(v[F::fcomp(q)], Fp[q]);
             split3(q < F::NNEG ? -v[q] : v[q], P[q]);
         }
         split3(h, hp);
@@ -313,17 +361,24 @@ k_tc_prep(const double *__restrict__ coords, int64_t N, int nA,
 
     // block summary
     const double inf = __longlong_as_double(0x7FF0000000000000LL);
-    double tmn = valid ? x[0] : inf, tmx = valid ? x[0] : -inf;
+    const double tp = F::time(x);
+    double tmn = valid ? tp : inf, tmx = valid ? tp : -inf;
     bool sorted = true;                                   // this point <= the next one (fp64; NaN: false)
-    if (valid && gp + 1 < N) sorted = x[0] <= coords[(gp + 1) * DIM];
+    if (valid && gp + 1 < N) sorted = tp <= F::time(coords + (gp + 1) * DIM);
+    float x1lo = __int_as_float(0x7f800000), x1hi = __int_as_float(0xff800000);
+    if (F::RANGE2 && valid) { x1lo = __double2float_rd(x[1]); x1hi = __double2float_ru(x[1]); }
 #pragma unroll
     for (int s = 16; s >= 1; s >>= 1) {
         tmn = fmin(tmn, __shfl_xor_sync(0xffffffffu, tmn, s));
         tmx = fmax(tmx, __shfl_xor_sync(0xffffffffu, tmx, s));
         c = fmaxf(c, __shfl_xor_sync(0xffffffffu, c, s));
+        if (F::RANGE2) {
+            x1lo = fminf(x1lo, __shfl_xor_sync(0xffffffffu, x1lo, s));
+            x1hi = fmaxf(x1hi, __shfl_xor_sync(0xffffffffu, x1hi, s));
+        }
     }
     __shared__ double s_mn[4], s_mx[4];
-    __shared__ float s_c[4];
+    __shared__ float s_c[4], s_x1[4][2];
     __shared__ uint32_t s_cm[4][7];
     uint32_t cm[7];                                       // |component| and |h| maxima: non-negative floats order like their bits
 #pragma unroll
@@ -331,6 +386,7 @@ k_tc_prep(const double *__restrict__ coords, int64_t N, int nA,
     cm[6] = __reduce_max_sync(0xffffffffu, (F::H && valid) ? (__float_as_uint(h) & 0x7fffffffu) : 0u);
     if (lane == 0) {
         s_mn[warp] = tmn; s_mx[warp] = tmx; s_c[warp] = c;
+        s_x1[warp][0] = x1lo; s_x1[warp][1] = x1hi;
 #pragma unroll
         for (int q = 0; q < 7; q++) s_cm[warp][q] = cm[q];
     }
@@ -346,7 +402,13 @@ k_tc_prep(const double *__restrict__ coords, int64_t N, int nA,
 #pragma unroll
         for (int q = 0; q < 6; q++) bi.cmax[q] = __uint_as_float(max(max(s_cm[0][q], s_cm[1][q]), max(s_cm[2][q], s_cm[3][q])));
         bi.hmax = __uint_as_float(max(max(s_cm[0][6], s_cm[1][6]), max(s_cm[2][6], s_cm[3][6])));
-        bi.pad[0] = bi.pad[1] = bi.pad[2] = 0;
+        if (F::fcomp(0) != 0) {                       // P_c and F_c are different components: one bound for all products
+#pragma unroll
+            for (int q = 0; q < 6; q++) bi.cmax[q] = q < NP ? bi.C : 0.f;
+        }
+        bi.x1min = fminf(fminf(s_x1[0][0], s_x1[1][0]), fminf(s_x1[2][0], s_x1[3][0]));
+        bi.x1max = fmaxf(fmaxf(s_x1[0][1], s_x1[1][1]), fmaxf(s_x1[2][1], s_x1[3][1]));
+        bi.pad = 0;
         info[(size_t)b * nA + a] = bi;
     }
 }
@@ -356,7 +418,7 @@ k_tc_prep(const double *__restrict__ coords, int64_t N, int nA,
 //   x = I | J << 16, y = causet, z = margin m (float bits; +inf: every row of the tile goes to fp64), w = unused.
 __global__ void __launch_bounds__(256)
 k_tc_tiles(const TcBlockInfo *__restrict__ info, int nT, uint32_t tiles_per, uint32_t total_tiles, float acc_units,
-           float in_units, uint4 *__restrict__ tab)
+           float in_units, int range2, uint4 *__restrict__ tab)
 {
     const uint32_t t = blockIdx.x * 256 + threadIdx.x;
     if (t >= total_tiles) return;
@@ -375,7 +437,13 @@ k_tc_tiles(const TcBlockInfo *__restrict__ info, int nT, uint32_t tiles_per, uin
     const bool bad = ((i0.flags | i1.flags | j0.flags | j1.flags) & 4u) != 0;
     const bool ordered = (I == J) ? ((i0.flags & 3u) == 3u && (i1.flags & 1u) != 0)
                                   : (fmax(i0.tmax, i1.tmax) <= fmin(j0.tmin, j1.tmin));
-    const bool fast = !bad && ordered && C >= 0x1p-40f && C <= 0x1p40f;
+    bool fast = !bad && ordered && C >= 0x1p-40f && C <= 0x1p40f;
+    if (range2) {       // 1+1 dS slab: times within pi and angles within 2 pi over the whole tile (both tested a little short)
+        const double tspan = fmax(j0.tmax, j1.tmax) - fmin(i0.tmin, i1.tmin);
+        const float aspan = __fsub_ru(fmaxf(fmaxf(i0.x1max, i1.x1max), fmaxf(j0.x1max, j1.x1max)),
+                                      fminf(fminf(i0.x1min, i1.x1min), fminf(j0.x1min, j1.x1min)));
+        fast = fast && tspan <= 3.1415926 && aspan <= 6.2831845f;
+    }
     // largest single addend a pair of this tile can hand to the tensor core: |h_i|, |h_j|, |P_c(i) F_c(j)|
     float M = fmaxf(fmaxf(i0.hmax, i1.hmax), fmaxf(j0.hmax, j1.hmax));
 #pragma unroll
@@ -785,7 +853,8 @@ int launch_tc_t(const double *coords, int64_t B, int64_t N, int64_t stride, uint
     // margin m = (ACC M + IN C^2) 2^-24, see the header: ACC = 4 (K + 2) (twice the alignment loss of K + 2 addends),
     // IN = the fp32 prefilter's own bound (Fast::MARGIN / 2, conversions included) + the dropped piece products
     k_tc_tiles<<<(unsigned)((total + 255) / 256), 256, 0, st>>>(info, nT, (uint32_t)tiles_per, (uint32_t)total,
-                                                                 4.f * (S::K + 2), (float)(Fast<GEOM, DIM>::MARGIN / 2 + 3 * Fast<GEOM, DIM>::NP), tab);
+                                                                 4.f * (S::K + 2), (float)(TcFast<GEOM, DIM>::MARGIN / 2 + 3 * TcFast<GEOM, DIM>::NP),
+                                                                 TcFast<GEOM, DIM>::RANGE2 ? 1 : 0, tab);
     CS_LAUNCHED("k_tc_tiles");
     constexpr size_t smem = SM::BYTES;
     static PerDeviceFlag attr_set;
@@ -813,6 +882,8 @@ bool causal_tc_supported(int geometry, int dim)
 {
     if (!interval_tensor_available()) return false;      // tcgen05: compute capability 10.x
     switch (geometry) {
+    case CS_GEOM_MINK2_LIGHTCONE: return dim == 2;
+    case CS_GEOM_DS2_SLAB: return dim == 2;
     case CS_GEOM_MINK_CONE: return dim >= 2 && dim <= 5;
     case CS_GEOM_FLRW_POLAR: return dim == 6;
     case CS_GEOM_DS4_SPHERICAL: return dim == 7;
@@ -822,6 +893,12 @@ bool causal_tc_supported(int geometry, int dim)
 
 #define CS_TC_DISPATCH(CALL)                                                                       \
     switch (geometry) {                                                                            \
+    case CS_GEOM_MINK2_LIGHTCONE:                                                                  \
+        if (dim == 2) return CALL(CS_GEOM_MINK2_LIGHTCONE, 2);                                     \
+        break;                                                                                     \
+    case CS_GEOM_DS2_SLAB:                                                                         \
+        if (dim == 2) return CALL(CS_GEOM_DS2_SLAB, 2);                                            \
+        break;                                                                                     \
     case CS_GEOM_MINK_CONE:                                                                        \
         if (dim == 2) return CALL(CS_GEOM_MINK_CONE, 2);                                           \
         if (dim == 3) return CALL(CS_GEOM_MINK_CONE, 3);                                           \

@@ -48,7 +48,7 @@ def test_argument_errors_need_no_gpu(lib):
     assert lib.cs_causal_matrix_ex(None, 1, 8, 2, 0, 7, None, None, None, 0, None) == -1     # unknown a1 route
     assert lib.cs_causal_matrix_ex(None, 1, 8, 2, 0, 0, None, None, None, 0, None) == -1     # NULL buffers
     assert lib.cs_causal_matrix_ex(None, 0, 8, 2, 0, 0, None, None, None, 0, None) == 0      # B = 0 is a no-op
-    assert lib.cs_causal_matrix_workspace(1, 4096, 2, 0, 2) == 0                             # 1+1 light cone: no tensor route
+    assert lib.cs_causal_matrix_workspace(1, 200, 4, 1, 2) == 0                              # N < 256: no tensor route
     assert lib.cs_causal_matrix_workspace(1, 4096, 4, 1, 1) == 0                             # FMA route: no scratch
     assert lib.cs_causal_matrix_workspace(1, 4096, 4, 1, 2) >= 4096 * (128 + 32)             # operand rows + coordinates
     assert lib.cs_a1_tensor_probe(None, 8, 4, None, None, None, 0, None, None) == -1

@@ -60,7 +60,8 @@ def to_u64(t):
     return t.cpu().numpy().view(np.uint64)
 
 
-TENSOR_A1_GEOMS = (inp.GEOM_MINK_CONE, inp.GEOM_FLRW_POLAR, inp.GEOM_DS4_SPHERICAL)    # bilinear predicates
+# every predicate is the sign of a bilinear form, some in derived coordinates (cs_build_tc.cu)
+TENSOR_A1_GEOMS = (inp.GEOM_MINK2_LIGHTCONE, inp.GEOM_MINK_CONE, inp.GEOM_DS2_SLAB, inp.GEOM_FLRW_POLAR, inp.GEOM_DS4_SPHERICAL)
 
 
 def a1_routes(api, geom, N):
@@ -300,13 +301,15 @@ def test_causal_matrix_tensor_route(api, oracle, geom, dim, N):
 def test_causal_matrix_tensor_route_arguments_and_probe(api, oracle):
     """The tensor route refuses what it does not serve; its probe reports an error of the tensor-core value far inside
     the margin, and rows re-evaluated in fp64 exactly where the input forces them (unsorted input: every row)."""
-    lc = torch.from_numpy(inp.sprinkle(inp.GEOM_MINK2_LIGHTCONE, 2, 512, 1)).cuda()
-    with pytest.raises(RuntimeError):
-        api.causal_matrix(lc, inp.GEOM_MINK2_LIGHTCONE, route=api.A1_TENSOR)
     small = torch.from_numpy(inp.sprinkle(inp.GEOM_MINK_CONE, 4, 100, 1)).cuda()
-    with pytest.raises(RuntimeError):
+    with pytest.raises(RuntimeError):      # rows shorter than a TMA box
         api.causal_matrix(small, inp.GEOM_MINK_CONE, route=api.A1_TENSOR)
-    assert api.causal_matrix_workspace(1, 512, 2, inp.GEOM_MINK2_LIGHTCONE, api.A1_TENSOR) == 0
+    with pytest.raises(RuntimeError):      # no such route
+        api.causal_matrix(small, inp.GEOM_MINK_CONE, route=3)
+    assert api.causal_matrix_workspace(1, 100, 4, inp.GEOM_MINK_CONE, api.A1_TENSOR) == 0
+    assert api.default_a1_route(1, 1024, 2, inp.GEOM_MINK2_LIGHTCONE) == api.A1_FMA          # 10 tiles
+    assert api.default_a1_route(1, 16384, 2, inp.GEOM_MINK2_LIGHTCONE) == api.A1_TENSOR
+    assert api.default_a1_route(4096, 2048, 4, inp.GEOM_MINK_CONE) == api.A1_TENSOR
     for dim in (4, 5):
         coords = inp.sprinkle(inp.GEOM_MINK_CONE, dim, 3000, 17)
         o_bits = oracle.causal_matrix_bits(coords, inp.GEOM_MINK_CONE)
@@ -320,6 +323,21 @@ def test_causal_matrix_tensor_route_arguments_and_probe(api, oracle):
         b2, _, st2 = api.a1_tensor_probe(torch.from_numpy(shuffled).cuda())
         assert np.array_equal(to_u64(b2), oracle.causal_matrix_bits(shuffled, inp.GEOM_MINK_CONE))
         assert st2["rows_fp64"] > 0.9 * st2["rows_total"], st2       # (only the tiles whose points happen to be ordered escape)
+
+
+def test_causal_matrix_tensor_route_ds_slab_ranges(api, oracle):
+    """The bilinear form of the 1+1 dS slab (cos dtheta - cos d eta) is the header's expression only while the angles of a
+    tile span at most 2 pi and its times at most pi: slabs far wider than that, angles spread over many turns, and a
+    sprinkling inside the valid range, all through every a1 route (gpu_bits)."""
+    rng = np.random.default_rng(8)
+    n = 1500
+    for tspan, aspan in ((1.0, 2 * np.pi), (8.0, 2 * np.pi), (1.0, 40.0), (8.0, 40.0), (3.2, 6.4)):
+        c = np.stack([rng.uniform(-1.2, -1.2 + tspan, n), rng.uniform(0.0, aspan, n)], axis=1)
+        c = np.ascontiguousarray(c[np.lexsort((c[:, 1], c[:, 0]))])
+        bits, bitsT = gpu_bits(api, c, inp.GEOM_DS2_SLAB)
+        o_bits = oracle.causal_matrix_bits(c, inp.GEOM_DS2_SLAB)
+        assert np.array_equal(to_u64(bits), o_bits), (tspan, aspan)
+        assert np.array_equal(to_u64(bitsT), oracle.transpose_bits(o_bits, n)), (tspan, aspan)
 
 
 def test_causal_matrix_tensor_route_degenerate(api, oracle):
