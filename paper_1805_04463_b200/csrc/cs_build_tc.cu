@@ -1,5 +1,6 @@
-// cs_build_tc.cu -- stage a1 on the tensor cores, for the predicates that are the sign of a bilinear form
-// (flat cone in 1+1 .. 4+1 dimensions, FLRW Eq. 7.7, 3+1 de Sitter).
+// cs_build_tc.cu -- stage a1 on the tensor cores: every predicate of the library as the sign of a bilinear form
+// (flat cone in 1+1 .. 4+1 dimensions, FLRW Eq. 7.7, 3+1 de Sitter as in cs_predicates.cuh; the 1+1 light cone and the
+// 1+1 de Sitter slab in derived coordinates, TcFast below).
 //
 // The sign of the interval between i and j is the sign of
 //     T(i, j) = h_i + h_j + sum_c P_c(i) F_c(j)          (cs_predicates.cuh, Fast<GEOM, DIM>)
