@@ -314,6 +314,8 @@ def time_single(api, cfg, N, route, steps, warmup, seed, local_rank, csd, e2e=Tr
         api._check(lib.cs_bd_action(hist.data_ptr(), kmax, N, cfg.dim, action.data_ptr(), None, st), "cs_bd_action")
         if events is not None: events[3].record()
 
+    sampler = ClockSampler(local_rank)          # started before the warm-up: nvidia-smi needs ~0.1 s to its first line
+    sampler.start()
     for _ in range(warmup):
         step()
     torch.cuda.synchronize()
@@ -322,8 +324,6 @@ def time_single(api, cfg, N, route, steps, warmup, seed, local_rank, csd, e2e=Tr
 
     # ---- timed region: exactly K steps, device time, max over ranks -------------------------
     ev = [[torch.cuda.Event(enable_timing=True) for _ in range(4)] for _ in range(steps)]
-    sampler = ClockSampler(local_rank)
-    sampler.start()
     csd.barrier(); torch.cuda.synchronize()
     launches0 = api.launch_count()
     t0 = time.perf_counter()
@@ -368,9 +368,9 @@ def time_ensemble(api, cfg, B, N, steps, warmup, rank, local_rank, csd, e2e=True
         [inp.sprinkle(cfg.geometry, cfg.dim, N, cfg.seed * 4096 + b + 1000003 * rank) for b in range(B)]))
     d_coords = torch.from_numpy(coords).cuda()
     ws = torch.empty(api.bd_action_batched_workspace(B, N), dtype=torch.uint8, device="cuda")
+    sampler = ClockSampler(local_rank); sampler.start()      # started before the warm-up: nvidia-smi needs ~0.1 s to its first line
     for _ in range(warmup):
         actions = api.bd_action_batched(d_coords, cfg.geometry, workspace=ws)
-    sampler = ClockSampler(local_rank); sampler.start()
     csd.barrier(); torch.cuda.synchronize()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     l0 = api.launch_count(); t0 = time.perf_counter()
