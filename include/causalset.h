@@ -11,7 +11,12 @@
  * Conventions common to every entry point
  *   - "device" pointers are caller-owned CUDA device memory (e.g. from torch);
  *     "host" pointers are ordinary host memory.  The library never allocates
- *     or frees an output and keeps no pointer after the call returns.
+ *     or frees an output and keeps no pointer after the call returns.  One call
+ *     takes scratch of its own when it is given none: cs_causal_matrix /
+ *     cs_causal_matrix_batched / cs_causal_matrix_ex with workspace = NULL on the
+ *     tensor route, from a stream-ordered memory pool the library owns per device
+ *     (allocated and freed in stream order inside the call; the pool keeps the
+ *     memory for the next call).  Pass a workspace to avoid it.
  *   - `stream` is a cudaStream_t passed as void* (NULL = legacy default
  *     stream).  Device-pointer calls only enqueue work and return; results are
  *     valid after the stream is synchronised.  *_host calls synchronise.
