@@ -52,6 +52,14 @@ def test_argument_errors_need_no_gpu(lib):
     assert lib.cs_causal_matrix_workspace(1, 4096, 4, 1, 1) == 0                             # FMA route: no scratch
     assert lib.cs_causal_matrix_workspace(1, 4096, 4, 1, 2) >= 4096 * (128 + 32)             # operand rows + coordinates
     assert lib.cs_a1_tensor_probe(None, 8, 4, None, None, None, 0, None, None) == -1
+    # CS_A1_AUTO: the tensor route from 128 tiles of 256 x 256 pairs up, never below N = 256 (host logic only)
+    assert lib.cs_default_a1_route(1, 65536, 4, 1) == 2 and lib.cs_default_a1_route(1, 131072, 2, 2) == 2
+    assert lib.cs_default_a1_route(1, 3840, 4, 1) == 1 and lib.cs_default_a1_route(1, 3841, 4, 1) == 2
+    assert lib.cs_default_a1_route(1, 1024, 2, 0) == 1 and lib.cs_default_a1_route(4096, 2048, 4, 1) == 2
+    assert lib.cs_default_a1_route(100000, 200, 4, 1) == 1
+    w1, w2 = lib.cs_causal_matrix_workspace(1, 4096, 4, 1, 2), lib.cs_causal_matrix_workspace(2, 4096, 4, 1, 2)
+    assert 0 < w1 < w2 <= 2 * w1 and w1 % 256 == 0
+    assert lib.cs_bd_action_batched_workspace(4096, 2048) <= 512 << 20                       # the ensemble chunk keeps it there
     assert lib.cs_bd_action(None, 3, 10, 4, None, None, None) == -1
     assert lib.cs_interval_hist(None, None, 10, -1, None, None, None, 0, None) == -1
     assert lib.cs_interval_hist_workspace(65536, -1, 1, 1) >= 256
