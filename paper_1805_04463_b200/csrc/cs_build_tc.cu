@@ -88,7 +88,7 @@ struct TcFast : Fast<GEOM, DIM> {
 // du + dv > 0 follows from t_j >= t_i and both differences are positive.
 template <>
 struct TcFast<CS_GEOM_MINK2_LIGHTCONE, 2> {
-    static constexpr bool ok = true, H = true, RANGE2 = false;
+    static constexpr bool H = true, RANGE2 = false;
     static constexpr int NP = 2, NNEG = 2, MARGIN = 64;
     __device__ static __forceinline__ double time(const double *x) { return (x[0] + x[1]) * 0.5; }
     __device__ static __forceinline__ constexpr int fcomp(int c) { return 1 - c; }
@@ -106,7 +106,7 @@ struct TcFast<CS_GEOM_MINK2_LIGHTCONE, 2> {
 // span at most 2 pi and its times at most pi (RANGE2); the fp64 rows use the header's expression as everywhere.
 template <>
 struct TcFast<CS_GEOM_DS2_SLAB, 2> {
-    static constexpr bool ok = true, H = false, RANGE2 = true;
+    static constexpr bool H = false, RANGE2 = true;
     static constexpr int NP = 4, NNEG = 2, MARGIN = 64;
     __device__ static __forceinline__ double time(const double *x) { return x[0]; }
     __device__ static __forceinline__ constexpr int fcomp(int c) { return c; }
