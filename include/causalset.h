@@ -264,7 +264,7 @@ int cs_smeared_action(const int64_t *hist, int64_t kmax, int64_t N, int dim, dou
 
 /* Batched ensemble (Monte-Carlo use): B independent causets of N points each,
  * one action per causet.  The ensemble is built and reduced chunk by chunk (a whole number of causets per CTA
- * pair of a2's grid, at most 448 MiB of bit matrices at a time), so the workspace does not grow with B beyond
+ * pair of a2's grid, at most 500 MiB of bit matrices and a1 scratch at a time), so the workspace does not grow with B beyond
  * 32 bytes per causet.
  *   coords   device, [B][N][dim] fp64, each causet sorted by time.
  *   actions  device, double[B], overwritten.
