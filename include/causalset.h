@@ -155,6 +155,14 @@ int cs_causal_matrix_ex(const double *coords, int64_t B, int64_t N, int dim, int
 int cs_a1_tensor_probe(const double *coords, int64_t N, int dim, uint64_t *bits, uint64_t *bitsT,
                        void *workspace, size_t workspace_bytes, double *out_host, void *stream);
 
+/* The self-check behind CS_A1_AUTO.  The tensor route's error band rests on a model of the tensor core's accumulation
+ * (reading A21); the first time AUTO would take that route on a device the library runs the probe above on a
+ * seeded causet of 2048 points in 3+1 and in 4+1 dimensions and keeps the FMA route on that device if the largest
+ * |a - T| / m reaches 0.25.  This call runs the check if it has not run yet and reports it: 1 the device behaves like the
+ * model, 0 it does not (AUTO = FMA route there; CS_A1_TENSOR by name still runs), < 0 a cs_status.  Synchronises `stream`
+ * the first time (about 1 ms), then returns the cached answer. */
+int cs_a1_tensor_selfcheck(void *stream);
+
 /* bitsT <- transpose(bits) (both device, [N][stride]); for callers that kept only `bits`. */
 int cs_transpose_bits(const uint64_t *bits, int64_t N, uint64_t *bitsT, void *stream);
 

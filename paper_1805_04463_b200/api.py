@@ -51,6 +51,7 @@ _SIGNATURES = {
     "cs_causal_matrix_workspace": (_sz, [_i64, _i64, _int, _int, _int]),
     "cs_default_a1_route": (_int, [_i64, _i64, _int, _int]),
     "cs_causal_matrix_ex": (_int, [_p, _i64, _i64, _int, _int, _int, _p, _p, _p, _sz, _p]),
+    "cs_a1_tensor_selfcheck": (_int, [_p]),
     "cs_a1_tensor_probe": (_int, [_p, _i64, _int, _p, _p, _p, _sz, _p, _p]),
     "cs_transpose_bits": (_int, [_p, _i64, _p, _p]),
     "cs_degrees": (_int, [_p, _p, _i64, _p, _p, _p]),
@@ -180,6 +181,14 @@ def causal_matrix_batched(coords: torch.Tensor, geometry: int, want_transpose: b
                                       _dptr(workspace), workspace.numel() if workspace is not None else 0, _stream()),
            "cs_causal_matrix_ex")
     return bits, bitsT
+
+
+def a1_tensor_selfcheck() -> bool:
+    """True if this device's tensor cores accumulate like the model the tensor a1 route's error band assumes."""
+    rc = load().cs_a1_tensor_selfcheck(_stream())
+    if rc < 0:
+        _check(rc, "cs_a1_tensor_selfcheck")
+    return rc == 1
 
 
 def a1_tensor_probe(coords: torch.Tensor):

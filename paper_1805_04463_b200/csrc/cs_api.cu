@@ -180,6 +180,13 @@ int cs_causal_matrix(const double *coords, int64_t N, int dim, int geometry,
     return cs_causal_matrix_ex(coords, 1, N, dim, geometry, CS_A1_AUTO, bits, bitsT, nullptr, 0, stream);
 }
 
+int cs_a1_tensor_selfcheck(void *stream)
+{
+    bool trusted = false;
+    const int rc = tensor_route_trusted(static_cast<cudaStream_t>(stream), &trusted);
+    return rc ? rc : (trusted ? 1 : 0);
+}
+
 int cs_a1_tensor_probe(const double *coords, int64_t N, int dim, uint64_t *bits, uint64_t *bitsT,
                        void *workspace, size_t workspace_bytes, double *out_host, void *stream)
 {

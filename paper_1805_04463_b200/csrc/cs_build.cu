@@ -12,6 +12,7 @@
 //
 // Floating point: explicit round-to-nearest intrinsics (__dsub_rn, __dmul_rn, __dadd_rn), which
 // the compiler never contracts into FMA, in exactly the order stated in include/causalset.h.
+#include <atomic>
 #include <mutex>
 
 #include "cs_predicates.cuh"
@@ -514,11 +515,77 @@ static int scratch_pool(cudaMemPool_t *out)
     return CS_OK;
 }
 
+// ---- self-check of the tensor route ---------------------------------------------------------------
+// The error band of cs_build_tc.cu rests on a model of how the tensor core accumulates (reading A21).  The
+// first time CS_A1_AUTO would take the tensor route on a device, the library measures that on the device itself:
+// cs_a1_tensor_probe's counters on a seeded causet of 2048 points in 3+1 and in 4+1 dimensions (K = 32 and K = 48 operand
+// columns).  If the largest |a - T| reaches a quarter of the margin the device does not behave like the model and AUTO
+// keeps the FMA route on it (CS_A1_TENSOR still runs when asked for by name).  Costs ~1 ms and one stream synchronisation, once.
+__global__ void k_selfcheck_coords(double *coords, int N, int dim)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    coords[(size_t)i * dim] = -0.9 + 1.8 * (i + 0.5) / N;                    // time: increasing
+    uint64_t z = 0x9E3779B97F4A7C15ull * (uint64_t)(i + 1);
+    for (int d = 1; d < dim; d++) {                                          // space: SplitMix64 draws in (-0.45, 0.45)
+        z += 0x9E3779B97F4A7C15ull;
+        uint64_t x = z;
+        x = (x ^ (x >> 30)) * 0xBF58476D1CE4E5B9ull;
+        x = (x ^ (x >> 27)) * 0x94D049BB133111EBull;
+        x ^= x >> 31;
+        coords[(size_t)i * dim + d] = ((double)(x >> 11) * 0x1p-53 - 0.5) * 0.9;
+    }
+}
+
+int tensor_route_trusted(cudaStream_t st, bool *trusted)
+{
+    static std::atomic<int> state[MAX_DEVICES];       // 0 not measured, 1 behaves like the model, 2 does not
+    static std::mutex mu;
+    const int dev = current_device();
+    int s0 = state[dev].load(std::memory_order_acquire);
+    if (s0 == 0) {
+        std::lock_guard<std::mutex> lock(mu);
+        s0 = state[dev].load(std::memory_order_acquire);
+        if (s0 == 0) {
+            cudaMemPool_t pool;
+            int rc = scratch_pool(&pool);
+            if (rc) return rc;
+            const int64_t N = 2048, stride = row_stride_words(N);
+            bool ok = true;
+            for (int dim = 4; dim <= 5 && ok; dim++) {
+                const size_t cb = align_up((size_t)N * dim * 8, 256), mb = align_up((size_t)N * stride * 8, 256);
+                const size_t sb = causal_tc_scratch_bytes(1, N, dim, CS_GEOM_MINK_CONE);
+                unsigned char *p = nullptr;
+                CS_CUDA(cudaMallocFromPoolAsync(reinterpret_cast<void **>(&p), cb + 2 * mb + sb, pool, st));
+                double *coords = reinterpret_cast<double *>(p);
+                k_selfcheck_coords<<<(unsigned)((N + 255) / 256), 256, 0, st>>>(coords, (int)N, dim);
+                CS_LAUNCHED("k_selfcheck_coords");
+                double out[5] = {0, 0, 0, 0, 0};
+                rc = launch_causal_tc_probe(coords, N, dim, reinterpret_cast<uint64_t *>(p + cb),
+                                            reinterpret_cast<uint64_t *>(p + cb + mb), p + cb + 2 * mb, out, st);   // synchronises
+                cudaFreeAsync(p, st);
+                if (rc) return rc;
+                ok = out[3] > 0.0 && out[3] < 0.25;
+            }
+            s0 = ok ? 1 : 2;
+            state[dev].store(s0, std::memory_order_release);
+        }
+    }
+    *trusted = s0 == 1;
+    return CS_OK;
+}
+
 int launch_causal_matrix(const double *coords, int64_t B, int64_t N, int dim, int geometry, int route,
                          uint64_t *bits, uint64_t *bitsT, void *scratch, size_t scratch_bytes, cudaStream_t st)
 {
-    const int r = resolve_a1_route(B, N, dim, geometry, route);
+    int r = resolve_a1_route(B, N, dim, geometry, route);
     if (r < 0) return CS_ERR_ARG;
+    if (r == CS_A1_TENSOR && route == CS_A1_AUTO) {
+        bool trusted = false;
+        const int rc = tensor_route_trusted(st, &trusted);
+        if (rc) return rc;
+        if (!trusted) r = CS_A1_FMA;
+    }
     if (r == CS_A1_FMA) return launch_causal_fma(coords, B, N, dim, geometry, bits, bitsT, st);
     const size_t need = causal_tc_scratch_bytes(B, N, dim, geometry);
     if (scratch) {

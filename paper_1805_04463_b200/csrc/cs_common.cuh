@@ -84,6 +84,7 @@ static_assert(sizeof(IntervalStats) <= 256, "stats block");
 int launch_causal_matrix(const double *coords, int64_t B, int64_t N, int dim, int geometry, int route,
                          uint64_t *bits, uint64_t *bitsT, void *scratch, size_t scratch_bytes, cudaStream_t st);
 size_t causal_matrix_scratch_bytes(int64_t B, int64_t N, int dim, int geometry, int route);
+int tensor_route_trusted(cudaStream_t st, bool *trusted);   // one-time self-check of the tensor a1 route on this device
 bool causal_tc_supported(int geometry, int dim);
 size_t causal_tc_scratch_bytes(int64_t B, int64_t N, int dim, int geometry);
 int launch_causal_tc(const double *coords, int64_t B, int64_t N, int dim, int geometry,

@@ -301,6 +301,7 @@ def test_causal_matrix_tensor_route(api, oracle, geom, dim, N):
 def test_causal_matrix_tensor_route_arguments_and_probe(api, oracle):
     """The tensor route refuses what it does not serve; its probe reports an error of the tensor-core value far inside
     the margin, and rows re-evaluated in fp64 exactly where the input forces them (unsorted input: every row)."""
+    assert api.a1_tensor_selfcheck() is True        # the device accumulates like the model: AUTO may take the tensor route
     small = torch.from_numpy(inp.sprinkle(inp.GEOM_MINK_CONE, 4, 100, 1)).cuda()
     with pytest.raises(RuntimeError):      # rows shorter than a TMA box
         api.causal_matrix(small, inp.GEOM_MINK_CONE, route=api.A1_TENSOR)
