@@ -53,7 +53,6 @@ constexpr int SMEM_FIXED = NS * STAGE_BYTES + NB * BITS_BYTES + 512;      // + 4
 constexpr uint32_t IDESC = (1u << 7) | (1u << 10) | ((uint32_t)(TN >> 3) << 17) | (1u << 23) | ((uint32_t)(256 >> 4) << 24);
 constexpr int HS_MAX = 16896;           // shared-memory histogram bins that fit beside the operand rings
 constexpr int HS_BATCHED = 2048;        // bins when several causets share a CTA (flushed at every switch)
-constexpr int BANDW = 8;                // diagonals (in 256-column units) per band of the tile order
 
 // five warpgroups: 0-1 epilogue (warp & 3 = TMEM lane quarter, warp >> 2 = column half), 2 A expanders,
 // 3 B expanders, 4 = MMA issuer, TMA loader and two idle warps.  The epilogue keeps a whole accumulator
@@ -263,7 +262,7 @@ inline int64_t pair_tiles_per_causet(int64_t N)
     return nT * (nT + 1) / 2;
 }
 
-__global__ void k_pair_tile_order(int nT, uint32_t *__restrict__ tab)
+__global__ void k_pair_tile_order(int nT, int BANDW, uint32_t *__restrict__ tab)
 {
     const int b = blockIdx.x;
     const int dhi = nT - 1 - b * BANDW;
@@ -899,7 +898,12 @@ int launch_interval_pair(const uint64_t *bits, const uint64_t *bitsT, int64_t B,
     if (rc) return rc;
     const int nT = (int)((N + TILE - 1) / TILE);
     uint32_t *tab = static_cast<uint32_t *>(scratch);
-    k_pair_tile_order<<<(nT + BANDW - 1) / BANDW, 128, 0, st>>>(nT, tab);
+    // Band width of the tile order, measured on B200 (a2 time, flat cone / dS slab): N = 32768: 1.369 ms at 2 against 1.383 at
+    // 8; N = 65536: 9.745 at 2-3, 9.81 at 8, 9.83 at 16; N = 98304: 33.1 / 38.7 at 2, 32.5 / 36.5 at 8-32; N = 131072 (dS slab,
+    // 2 x 2 GiB, power-capped): 96.4 at 2, 90-92 at 8, 85.8 at 16-32, 87.7 at 64 -- wide bands cut the DRAM traffic of the long
+    // panels, and with it the power that caps the clock there.
+    const int bandw = nT <= 288 ? 2 : 16;
+    k_pair_tile_order<<<(nT + bandw - 1) / bandw, 128, 0, st>>>(nT, bandw, tab);
     CS_LAUNCHED("k_pair_tile_order");
     // empty-block flags: one causet, and large enough that the ~10 us of the flag pass cannot matter
     uint8_t *flagU = nullptr, *flagT = nullptr;
