@@ -898,11 +898,14 @@ int launch_interval_pair(const uint64_t *bits, const uint64_t *bitsT, int64_t B,
     if (rc) return rc;
     const int nT = (int)((N + TILE - 1) / TILE);
     uint32_t *tab = static_cast<uint32_t *>(scratch);
-    // Band width of the tile order, measured on B200 (a2 time, flat cone / dS slab): N = 32768: 1.369 ms at 2 against 1.383 at
-    // 8; N = 65536: 9.745 at 2-3, 9.81 at 8, 9.83 at 16; N = 98304: 33.1 / 38.7 at 2, 32.5 / 36.5 at 8-32; N = 131072 (dS slab,
-    // 2 x 2 GiB, power-capped): 96.4 at 2, 90-92 at 8, 85.8 at 16-32, 87.7 at 64 -- wide bands cut the DRAM traffic of the long
-    // panels, and with it the power that caps the clock there.
-    const int bandw = nT <= 288 ? 2 : 16;
+    // Band width of the tile order, from a measured sweep on B200 (a2 time / DRAM bytes read per launch).  Wide bands let the
+    // ~74 tiles in flight share their row panels in L2:
+    //   N = 65536 (2 x 512 MiB):  2: 9.74 ms / 23.3 GB   8: 9.81 / 9.7   16: 9.83 / 4.0   32: 9.85 / 2.3   64: 9.85 / 4.1   96: 9.91 / 7.6
+    //   N = 131072 (2 x 2 GiB, power-capped at narrow bands):  2: 96.4 ms   8: 90-92 / 185 GB   16: 85.8 / 102   32: 85.8 / 84   64: 87.7 / 111
+    //   N = 32768 (2 x 128 MiB): 0.3 GB at any width, 1.368 ms at 2 against 1.386 at 32
+    // 32 diagonals once the matrices are well beyond L2 (1 % slower than 2 at N = 65536, but a tenth of the DRAM traffic:
+    // 2.1 x the two matrices), 2 below.
+    const int bandw = nT <= 160 ? 2 : 32;
     k_pair_tile_order<<<(nT + bandw - 1) / bandw, 128, 0, st>>>(nT, bandw, tab);
     CS_LAUNCHED("k_pair_tile_order");
     // empty-block flags: one causet, and large enough that the ~10 us of the flag pass cannot matter
