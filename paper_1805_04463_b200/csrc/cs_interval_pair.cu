@@ -282,7 +282,11 @@ __global__ void k_pair_tile_order(int nT, int BANDW, uint32_t *__restrict__ tab)
             const int64_t m = I - full;   // rows full .. I-1 hold nT - dlo - I' entries each
             pos = (int64_t)full * w + m * (nT - dlo) - (int64_t)(full + I - 1) * m / 2;
         }
-        for (int d = dlo; d <= dhi && I + d < nT; d++) tab[off + pos + (d - dlo)] = ((uint32_t)I << 16) | (uint32_t)(I + d);
+        // d ascending in even rows, descending in odd ones: the clusters take tiles round-robin, and a snake keeps the
+        // K lengths one cluster collects from a wide band even
+        const int last = (dhi < nT - 1 - I ? dhi : nT - 1 - I) - dlo;      // entries of this row - 1
+        for (int d = dlo; d <= dhi && I + d < nT; d++)
+            tab[off + pos + ((I & 1) ? last - (d - dlo) : (d - dlo))] = ((uint32_t)I << 16) | (uint32_t)(I + d);
     }
 }
 
