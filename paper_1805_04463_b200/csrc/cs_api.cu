@@ -54,7 +54,7 @@ static size_t interval_ws_bytes(int64_t B, int64_t N, int have_bitsT, int route)
 // hist: int64[B][kmax+1]; shared by the single and the batched entry points
 static int interval_hist_impl(const uint64_t *bits, const uint64_t *bitsT, int64_t B, int64_t N, int64_t kmax,
                               int64_t row_begin, int64_t row_end, int route, int64_t *hist, int64_t *nrel,
-                              void *workspace, size_t workspace_bytes, cudaStream_t st)
+                              void *workspace, size_t workspace_bytes, cudaStream_t st, bool keep_table = false)
 {
     kmax = clamp_kmax(N, kmax);
     CS_CUDA(cudaMemsetAsync(hist, 0, (size_t)B * (kmax + 1) * sizeof(int64_t), st));
@@ -81,7 +81,7 @@ static int interval_hist_impl(const uint64_t *bits, const uint64_t *bitsT, int64
     if (route == CS_ROUTE_TENSOR_PAIR)
         return launch_interval_pair(bits, bitsT, B, N, kmax, row_begin, row_end, hist, nrel, ws,
                                     workspace_bytes - (size_t)(ws - static_cast<unsigned char *>(workspace)),
-                                    static_cast<IntervalStats *>(scratch), st);
+                                    static_cast<IntervalStats *>(scratch), keep_table, st);
     if (route == CS_ROUTE_TENSOR_FP4)
         return launch_interval_fp4(bits, bitsT, B, N, kmax, row_begin, row_end, hist, nrel, ws,
                                    workspace_bytes - (size_t)(ws - static_cast<unsigned char *>(workspace)), st);
@@ -387,7 +387,7 @@ int cs_bd_action_batched(const double *coords, int64_t B, int64_t N, int dim, in
                                      fits ? a1_bytes : 0, stream);
         if (rc) return rc;
         rc = interval_hist_impl(bits, bitsT, nb, N, kmax, 0, N, CS_ROUTE_AUTO, hist + b0 * (kmax + 1), nullptr, iws,
-                                (size_t)(a1ws - iws), st);
+                                (size_t)(a1ws - iws), st, b0 > 0);      // the tile table of the first chunk serves them all
         if (rc) return rc;
     }
     return launch_bd_action(hist, kmax + 1, B, kmax, N, spacetime_dim(geometry, dim), actions, nullptr, hist4, st);
@@ -498,7 +498,7 @@ int cs_bd_action_batched_host(const double *coords_host, int64_t B, int64_t N, i
         if (rc) return rc;
         CS_CUDA(cudaEventRecord(consumed[buf], st));
         if (kmax < 3) CS_CUDA(cudaMemsetAsync(hist, 0, (size_t)nb * 4 * 8, st));
-        rc = interval_hist_impl(bits, bitsT, nb, N, kmax, 0, N, CS_ROUTE_AUTO, hist, nullptr, ws, left, st);
+        rc = interval_hist_impl(bits, bitsT, nb, N, kmax, 0, N, CS_ROUTE_AUTO, hist, nullptr, ws, left, st, b0 > 0);
         if (rc) return rc;
         rc = launch_bd_action(hist, kmax + 1, nb, kmax, N, spacetime_dim(geometry, dim), actions + b0, nullptr,
                               hist4 + b0 * 4, st);

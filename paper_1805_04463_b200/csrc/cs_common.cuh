@@ -108,9 +108,11 @@ size_t interval_tensor_scratch_bytes(int64_t B, int64_t N);
 int launch_interval_fp4(const uint64_t *bits, const uint64_t *bitsT, int64_t B, int64_t N, int64_t kmax,
                         int64_t row_begin, int64_t row_end, int64_t *hist, int64_t *nrel,
                         void *scratch, size_t scratch_bytes, cudaStream_t st);
+// keep_table: the tile table in `scratch` was written by an earlier call with the same N on this stream (the chunks of an
+// ensemble): it is not rebuilt.
 int launch_interval_pair(const uint64_t *bits, const uint64_t *bitsT, int64_t B, int64_t N, int64_t kmax,
                          int64_t row_begin, int64_t row_end, int64_t *hist, int64_t *nrel,
-                         void *scratch, size_t scratch_bytes, IntervalStats *stats, cudaStream_t st);
+                         void *scratch, size_t scratch_bytes, IntervalStats *stats, bool keep_table, cudaStream_t st);
 size_t interval_pair_scratch_bytes(int64_t N);
 bool interval_tensor_available();
 

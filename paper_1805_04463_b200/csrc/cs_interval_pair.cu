@@ -896,7 +896,7 @@ static int launch_pair_t(const CUtensorMap &mapU, const CUtensorMap &mapL, const
 
 int launch_interval_pair(const uint64_t *bits, const uint64_t *bitsT, int64_t B, int64_t N, int64_t kmax,
                          int64_t row_begin, int64_t row_end, int64_t *hist, int64_t *nrel,
-                         void *scratch, size_t scratch_bytes, IntervalStats *stats, cudaStream_t st)
+                         void *scratch, size_t scratch_bytes, IntervalStats *stats, bool keep_table, cudaStream_t st)
 {
     if (N > ((int64_t)1 << 21)) return CS_ERR_ARG;   // 8 * count must stay below 2^24; tile ids are 16 bits
     static_assert(TN == TILE, "the tile table lists square tiles");
@@ -921,8 +921,10 @@ int launch_interval_pair(const uint64_t *bits, const uint64_t *bitsT, int64_t B,
     const int bandw = nT <= 160 ? 1 : 32;
     int deal_clusters = sm_count() / 2;       // as the grid below, unless there are fewer tiles than clusters
     if (deal_clusters < 1) deal_clusters = 1;
-    k_pair_tile_order<<<(nT + bandw - 1) / bandw, 128, 0, st>>>(nT, bandw, deal_clusters, tiles_per, tab);
-    CS_LAUNCHED("k_pair_tile_order");
+    if (!keep_table) {
+        k_pair_tile_order<<<(nT + bandw - 1) / bandw, 128, 0, st>>>(nT, bandw, deal_clusters, tiles_per, tab);
+        CS_LAUNCHED("k_pair_tile_order");
+    }
     // empty-block flags: one causet, and large enough that the ~10 us of the flag pass cannot matter
     uint8_t *flagU = nullptr, *flagT = nullptr;
     unsigned int *n_empty = nullptr;
