@@ -597,6 +597,8 @@ k_causal_tc(const __grid_constant__ CUtensorMap mapB, const __grid_constant__ CU
             const double *cJ = cI + TCT * DIM;
             uint32_t *U = s_U + (n & 1) * TCT * TC_PITCH, *L = s_L + (n & 1) * TCT * TC_PITCH;
             tc_mbar_wait(&s_sempty[n & 1], ((n >> 1) & 1) ^ 1);    // the writers are done with this staging buffer
+            tc_mbar_wait(&s_full[s], (n / NSTG) & 1);              // the stage's coordinates (read by the fp64 rows) have landed:
+                                                                   // complete long before, but this is the wait that orders the reads
 
             // The blocks of a tile are software-pipelined: the shuffle butterfly of the block before (five dependent
             // shuffles, ~150 clk of latency) is interleaved with the sign extraction of the current one.
