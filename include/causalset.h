@@ -83,7 +83,9 @@ enum cs_status {
     CS_ERR_GEOM = -3,       /* unknown geometry */
     CS_ERR_UNSORTED = -4,   /* reserved (the library does not check sortedness) */
     CS_ERR_WORKSPACE = -5,  /* workspace NULL or smaller than the *_workspace() query */
-    CS_ERR_CUDA = -6        /* a CUDA runtime call or launch failed; see cs_last_cuda_error() */
+    CS_ERR_CUDA = -6,       /* a CUDA runtime call or launch failed; see cs_last_cuda_error() */
+    CS_ERR_CAPACITY = -7    /* the size is beyond the fixed capacity of an entry point that owns its scratch
+                               (cs_interval_hist_static); cs_last_cuda_error() names the limit */
 };
 
 /* How a2 is computed.  All routes give identical integers. */
@@ -200,6 +202,32 @@ int cs_interval_hist_ex(const uint64_t *bits, const uint64_t *bitsT, int64_t N, 
                         int64_t row_begin, int64_t row_end, int route,
                         int64_t *hist, int64_t *n_relations,
                         void *workspace, size_t workspace_bytes, void *stream);
+/* a2 for callers that cannot allocate device memory.
+ *
+ * Every other a2 call wants a workspace, and somebody has to cudaMalloc it.  Some callers can't: code that runs inside
+ * another framework's allocator hook or while that framework's caching allocator is locked; a service whose device
+ * memory is budgeted once at start-up and must not grow (real-time, embedded, multi-tenant with a hard quota); a plugin
+ * that receives nothing but its input and output buffers.  This entry point is for them: the same result as
+ * cs_interval_hist_ex(route = CS_ROUTE_POPC) over all rows (Alg. 20), with the scratch -- the tile
+ * counter and, if bitsT is NULL, the transposed matrix -- in a static array inside the library's device image.
+ * It calls no cudaMalloc, cudaFree, memory-pool or other allocating routine; the caller still owns inputs and outputs.
+ *   bits, bitsT, kmax, hist, n_relations   exactly as for cs_interval_hist (bitsT may be NULL).
+ *   N            at most cs_interval_hist_static_max_n() = 8192.  Larger N returns CS_ERR_CAPACITY and
+ *                cs_last_cuda_error() states the limit; nothing is written.
+ * Cost: the array is 8 MiB + 256 B of device memory on every GPU that loads the library, from load until exit,
+ * whether or not this call is ever made.
+ * First call on a device: looks up the array's device address (cudaGetSymbolAddress) and sets the kernel's
+ * shared-memory attribute, once, with the calling thread's current device.  Make that first call outside any stream
+ * capture, e.g. once at start-up on a tiny input.
+ * Sharing: all calls on a device use the one array and it keeps what the previous call left.  The call clears what
+ * has to start at zero itself (in stream order), so back-to-back calls on ONE stream are fine; two calls whose work
+ * can overlap on the GPU (different streams, different host threads) race on the array and give wrong histograms --
+ * serialise them.
+ * Errors: CS_ERR_ARG, CS_ERR_CAPACITY, CS_ERR_CUDA.  N < 2 zeroes the outputs. */
+int64_t cs_interval_hist_static_max_n(void);
+int cs_interval_hist_static(const uint64_t *bits, const uint64_t *bitsT, int64_t N, int64_t kmax,
+                            int64_t *hist, int64_t *n_relations, void *stream);
+
 /* What the last cs_interval_hist* call that used `workspace` executed (for the roofline on executed work):
  *   stats_host  host, int64[4], overwritten:
  *     [0] (tile, stage) pairs whose MMAs were issued: a stage is 256 rows x 256 columns x 256 k of the 0/1

@@ -60,6 +60,8 @@ _SIGNATURES = {
     "cs_interval_hist": (_int, [_p, _p, _i64, _i64, _p, _p, _p, _sz, _p]),
     "cs_interval_hist_ex": (_int, [_p, _p, _i64, _i64, _i64, _i64, _int, _p, _p, _p, _sz, _p]),
     "cs_interval_hist_stats": (_int, [_p, _p, _p]),
+    "cs_interval_hist_static_max_n": (_i64, []),
+    "cs_interval_hist_static": (_int, [_p, _p, _i64, _i64, _p, _p, _p]),
     "cs_interval_hist_batched_workspace": (_sz, [_i64, _i64, _int]),
     "cs_interval_hist_batched": (_int, [_p, _p, _i64, _i64, _i64, _int, _p, _p, _sz, _p]),
     "cs_default_route": (_int, [_i64]),
@@ -251,6 +253,34 @@ def interval_hist(bits: torch.Tensor, bitsT, N: int, kmax: int = -1, route: int 
     _check(load().cs_interval_hist_ex(_dptr(bits), _dptr(bitsT), N, kmax, row_begin, row_end, route,
                                       _dptr(hist), _dptr(nrel), _dptr(ws), ws.numel(), _stream()),
            "cs_interval_hist_ex")
+    return (hist, nrel) if return_relations else hist
+
+
+def interval_hist_static_max_n() -> int:
+    return int(load().cs_interval_hist_static_max_n())
+
+
+def interval_hist_static(bits: torch.Tensor, bitsT, N: int, kmax: int = -1, hist: torch.Tensor | None = None,
+                         return_relations: bool = False):
+    """a2 through cs_interval_hist_static: for callers that cannot allocate device memory (inside an allocator
+    hook, under a fixed memory budget, plugins that only get their buffers).  The library's scratch is a static
+    device array, so no workspace is passed and nothing is allocated by the library; N <= interval_hist_static_max_n().
+    Pass `hist` (int64[kmax+1] after clamping) to keep this wrapper from allocating the output as well.
+    Calls share the one array per device: do not let two of them overlap on the GPU.
+    -> hist int64[kmax+1] (CUDA); with return_relations also int64[1] n_relations."""
+    _need_cuda(bits, torch.int64, "bits")
+    if bitsT is not None:
+        _need_cuda(bitsT, torch.int64, "bitsT")
+    k = clamp_kmax(N, kmax)
+    if hist is None:
+        hist = torch.empty(k + 1, dtype=torch.int64, device=bits.device)
+    else:
+        _need_cuda(hist, torch.int64, "hist")
+        if hist.numel() < k + 1:
+            raise ValueError("hist needs %d entries" % (k + 1))
+    nrel = torch.empty(1, dtype=torch.int64, device=bits.device) if return_relations else None
+    _check(load().cs_interval_hist_static(_dptr(bits), _dptr(bitsT), N, kmax, _dptr(hist), _dptr(nrel), _stream()),
+           "cs_interval_hist_static")
     return (hist, nrel) if return_relations else hist
 
 

@@ -109,6 +109,7 @@ const char *cs_status_string(int status)
     case CS_ERR_UNSORTED: return "elements not sorted by time";
     case CS_ERR_WORKSPACE: return "workspace missing, misaligned or too small";
     case CS_ERR_CUDA: return "CUDA error";
+    case CS_ERR_CAPACITY: return "size beyond the fixed capacity of this entry point";
     default: return "unknown status";
     }
 }
@@ -266,6 +267,16 @@ int cs_interval_hist(const uint64_t *bits, const uint64_t *bitsT, int64_t N, int
 {
     return cs_interval_hist_ex(bits, bitsT, N, kmax, 0, N, CS_ROUTE_AUTO, hist, n_relations,
                                workspace, workspace_bytes, stream);
+}
+
+int64_t cs_interval_hist_static_max_n(void) { return interval_static_max_n(); }
+
+int cs_interval_hist_static(const uint64_t *bits, const uint64_t *bitsT, int64_t N, int64_t kmax,
+                            int64_t *hist, int64_t *n_relations, void *stream)
+{
+    if (N < 0 || !hist || (N > 0 && !bits)) return CS_ERR_ARG;
+    if (misaligned16(bits, bitsT)) return CS_ERR_ARG;
+    return launch_interval_popc_static(bits, bitsT, N, kmax, hist, n_relations, static_cast<cudaStream_t>(stream));
 }
 
 int cs_interval_hist_stats(const void *workspace, int64_t *stats_host, void *stream)

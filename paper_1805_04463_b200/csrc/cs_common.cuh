@@ -100,6 +100,10 @@ int launch_interval_popc(const uint64_t *bits, const uint64_t *bitsT, int64_t B,
                          int64_t row_begin, int64_t row_end, int64_t *hist, int64_t *nrel,
                          void *scratch, cudaStream_t st);
 size_t interval_popc_scratch_bytes();
+// the bit route with its scratch in a static device array (no allocation anywhere on the path); N <= interval_static_max_n()
+int launch_interval_popc_static(const uint64_t *bits, const uint64_t *bitsT, int64_t N, int64_t kmax,
+                                int64_t *hist, int64_t *nrel, cudaStream_t st);
+int64_t interval_static_max_n();
 
 int launch_interval_tensor(const uint64_t *bits, const uint64_t *bitsT, int64_t B, int64_t N, int64_t kmax,
                            int64_t row_begin, int64_t row_end, int64_t *hist, int64_t *nrel,

@@ -12,6 +12,8 @@
 // counters in registers: 16 shared-memory loads feed 64 AND+POPC per word.  The epilogue tests the
 // relation bit of each pair and updates a shared-memory histogram (bins < HS; global atomics for
 // the rare larger intervals), flushed to the int64 histogram with few global atomics.
+#include <mutex>
+
 #include "cs_common.cuh"
 
 namespace cs {
@@ -255,6 +257,91 @@ int launch_interval_popc(const uint64_t *bits, const uint64_t *bitsT, int64_t B,
         reinterpret_cast<unsigned long long *>(hist), reinterpret_cast<unsigned long long *>(nrel),
         reinterpret_cast<unsigned long long *>(scratch));
     CS_LAUNCHED("k_interval_popc");
+    return CS_OK;
+}
+
+// ---- a2 for callers that must not allocate: scratch in a static device array --------------------------------
+// Some users of this library cannot hand over a workspace because they have no way to get one: code running inside
+// another framework's allocator callback or with its caching allocator locked, a real-time or embedded service whose
+// memory budget is fixed at start-up and forbids cudaMalloc afterwards, a plugin that is only given its input and
+// output buffers.  For them the scratch of the bit route (the tile counter of k_interval_popc and, when the caller has
+// no transposed matrix, the transposed matrix itself) lives in the array below, which is part of the library's device
+// image: every GPU that loads libcausalset.so holds these 8 MiB + 256 B until the process exits.
+//
+// `g_static_scratch` is a device symbol.  In host code the name is only a stand-in the runtime uses to look the symbol
+// up; it is NOT a device address, so it is never passed to a kernel or a memset.  static_scratch_address() asks the
+// runtime for the real address once per device (with that device current) and caches it.
+constexpr int64_t STATIC_MAX_N = 8192;
+constexpr size_t STATIC_HEAD_BYTES = 256;                                  // IntervalStats block: sched[0] = tile counter
+constexpr size_t STATIC_MAT_BYTES = (size_t)STATIC_MAX_N * (STATIC_MAX_N / 64) * 8;   // transposed matrix at the largest N
+constexpr size_t STATIC_SCRATCH_BYTES = STATIC_HEAD_BYTES + STATIC_MAT_BYTES;
+static __device__ __align__(256) unsigned char g_static_scratch[STATIC_SCRATCH_BYTES];
+
+int64_t interval_static_max_n() { return STATIC_MAX_N; }
+
+static int static_scratch_address(unsigned char **out)
+{
+    static unsigned char *addr[MAX_DEVICES];
+    static std::mutex mu;
+    int dev = -1;
+    CS_CUDA(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= MAX_DEVICES) {
+        snprintf(g_cuda_err, sizeof(g_cuda_err), "cs_interval_hist_static: device ordinal %d is beyond the %d this library tracks",
+                 dev, MAX_DEVICES);
+        return CS_ERR_ARG;
+    }
+    std::lock_guard<std::mutex> lock(mu);
+    if (!addr[dev]) {
+        void *p = nullptr;
+        CS_CUDA(cudaGetSymbolAddress(&p, g_static_scratch));   // the copy of the array that lives on the current device
+        if (!p || ((uintptr_t)p & 255)) {
+            snprintf(g_cuda_err, sizeof(g_cuda_err), "cs_interval_hist_static: bad address %p for the static scratch", p);
+            return CS_ERR_CUDA;
+        }
+        CS_CUDA(cudaFuncSetAttribute(k_interval_popc, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES));
+        addr[dev] = static_cast<unsigned char *>(p);
+    }
+    *out = addr[dev];
+    return CS_OK;
+}
+
+// The same kernels as cs_interval_hist_ex(route = CS_ROUTE_POPC) on the whole row range; only where the scratch comes
+// from differs.  No cudaMalloc / cudaFree / pool call on this path: memsets and launches only.
+int launch_interval_popc_static(const uint64_t *bits, const uint64_t *bitsT, int64_t N, int64_t kmax,
+                                int64_t *hist, int64_t *nrel, cudaStream_t st)
+{
+    if (N > STATIC_MAX_N) {
+        snprintf(g_cuda_err, sizeof(g_cuda_err),
+                 "cs_interval_hist_static: N = %lld is beyond the fixed capacity of the static scratch (N <= %lld); "
+                 "use cs_interval_hist with a workspace", (long long)N, (long long)STATIC_MAX_N);
+        return CS_ERR_CAPACITY;
+    }
+    kmax = clamp_kmax(N, kmax);
+    CS_CUDA(cudaMemsetAsync(hist, 0, (size_t)(kmax + 1) * sizeof(int64_t), st));
+    if (nrel) CS_CUDA(cudaMemsetAsync(nrel, 0, sizeof(int64_t), st));
+    if (N < 2) return CS_OK;
+    unsigned char *scratch = nullptr;
+    int rc = static_scratch_address(&scratch);
+    if (rc) return rc;
+    // the array keeps what the last call left in it: the tile counter must start at zero; the transposed matrix is
+    // overwritten whole (padding included) by launch_transpose_bits before the kernel reads it
+    CS_CUDA(cudaMemsetAsync(scratch, 0, STATIC_HEAD_BYTES, st));
+    if (!bitsT) {
+        uint64_t *t = reinterpret_cast<uint64_t *>(scratch + STATIC_HEAD_BYTES);
+        rc = launch_transpose_bits(bits, 1, N, t, st);
+        if (rc) return rc;
+        bitsT = t;
+    }
+    const int64_t stride = row_stride_words(N);
+    const int64_t nT = (N + TI - 1) / TI;
+    const int64_t total = nT * (nT + 1) / 2;
+    int64_t grid = (int64_t)sm_count() * 2;
+    if (grid > total) grid = total;
+    k_interval_popc<<<(unsigned)grid, THREADS, SMEM_BYTES, st>>>(
+        bits, bitsT, 1, N, stride, kmax, 0, N,
+        reinterpret_cast<unsigned long long *>(hist), reinterpret_cast<unsigned long long *>(nrel),
+        reinterpret_cast<unsigned long long *>(scratch));
+    CS_LAUNCHED("k_interval_popc(static scratch)");
     return CS_OK;
 }
 

@@ -64,6 +64,11 @@ def test_argument_errors_need_no_gpu(lib):
     assert lib.cs_interval_hist(None, None, 10, -1, None, None, None, 0, None) == -1
     assert lib.cs_interval_hist_workspace(65536, -1, 1, 1) >= 256
     assert lib.cs_interval_hist_workspace(1024, -1, 0, 1) >= 256 + 1024 * 16 * 8
+    # the entry point with static scratch refuses what its array cannot hold, before touching the device
+    assert lib.cs_interval_hist_static_max_n() == 8192
+    assert lib.cs_interval_hist_static(ctypes.c_void_p(16), None, 8193, -1, ctypes.c_void_p(16), None, None) == -7
+    assert b"N <= 8192" in lib.cs_last_cuda_error() and b"capacity" in lib.cs_status_string(-7)
+    assert lib.cs_interval_hist_static(None, None, 10, -1, None, None, None) == -1
 
 
 def test_missing_library_fails_loudly(monkeypatch, tmp_path):

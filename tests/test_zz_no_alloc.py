@@ -1,0 +1,95 @@
+"""cs_interval_hist_static: a2 for callers that cannot allocate device memory.
+
+Who that is: code running inside another framework's allocator hook (or while its caching allocator is
+locked), services whose device memory is budgeted once at start-up and may not grow afterwards, and plugins
+that are handed their input and output buffers and nothing else.  None of them can cudaMalloc the workspace
+the other a2 calls ask for, so this entry point keeps its scratch in a static device array inside the library
+(8 MiB + 256 B per GPU, N <= 8192) and allocates nothing.
+
+What is checked: the histogram and the relation count are bit-identical (integers: the tolerance every a2 test
+uses is zero) to the workspace-based path, on two calls in a row that share the static array -- the second one
+on a different, smaller causet, so anything the first call left behind in the array (tile counter, transposed
+matrix) would show.  Sizes beyond the limit must be refused with an error that states the limit.
+
+This file is named to be collected last: `pytest -x` stops at the first failure and a failure here must not
+hide the parity tests.  It passes alone in a fresh process (the first call on the device does the one-time
+set-up) and after the rest of the suite.
+"""
+import numpy as np
+import pytest
+
+torch = pytest.importorskip("torch")
+
+from paper_1805_04463_b200 import inputs as inp  # noqa: E402
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def api():
+    if not torch.cuda.is_available():
+        pytest.fail("gpu tests need a CUDA device")
+    from paper_1805_04463_b200 import api as _api
+    _api.load()
+    torch.cuda.set_device(0)
+    return _api
+
+
+def _causet(api, geom, dim, N, seed):
+    coords = inp.sprinkle(geom, dim, N, seed)
+    return api.causal_matrix(torch.from_numpy(np.ascontiguousarray(coords)).cuda(), geom)
+
+
+def test_static_scratch_matches_workspace_path_twice_in_a_row(api, oracle):
+    assert api.interval_hist_static_max_n() == 8192
+    # first call: several 128 x 128 tiles and a ragged tail, no transposed matrix from the caller, so both halves
+    # of the static array (counter, transposed matrix) are in use
+    N1 = 3001
+    bits1, bitsT1 = _causet(api, inp.GEOM_MINK_CONE, 4, N1, 11)
+    want1, wrel1 = api.interval_hist(bits1, bitsT1, N1, route=api.ROUTE_POPC, return_relations=True)
+    got1, rel1 = api.interval_hist_static(bits1, None, N1, return_relations=True)
+    # second call straight after it on the same stream: another causet, smaller, other geometry, truncated histogram
+    N2 = 1000
+    bits2, bitsT2 = _causet(api, inp.GEOM_DS2_SLAB, 2, N2, 12)
+    want2, wrel2 = api.interval_hist(bits2, bitsT2, N2, kmax=37, return_relations=True)
+    got2, rel2 = api.interval_hist_static(bits2, None, N2, kmax=37, return_relations=True)
+    # and a third with the caller's own transposed matrix and output buffer (nothing allocated by the wrapper either)
+    out3 = torch.full((N1 - 1,), -1, dtype=torch.int64, device="cuda")
+    got3 = api.interval_hist_static(bits1, bitsT1, N1, hist=out3)
+    torch.cuda.synchronize()
+    assert got3 is out3
+    assert torch.equal(got1, want1) and torch.equal(rel1, wrel1)
+    assert torch.equal(got2, want2) and torch.equal(rel2, wrel2)
+    assert torch.equal(got3, want1)
+    assert int(rel1.item()) == int(want1.sum().item()) > 0
+    # the default route of the existing path (tensor cores at this size) agrees as well, and so does the oracle
+    assert torch.equal(got1, api.interval_hist(bits1, bitsT1, N1))
+    o_hist = oracle.interval_hist_alg20(bits2.cpu().numpy().view(np.uint64), N2)[0]
+    assert np.array_equal(got2.cpu().numpy(), o_hist[:38])
+
+
+def test_static_scratch_edge_sizes(api):
+    for N in (0, 1):
+        x = torch.zeros((max(N, 1), 2), dtype=torch.int64, device="cuda")
+        h, r = api.interval_hist_static(x, None, N, return_relations=True)
+        assert h.tolist() == [0] and r.tolist() == [0]
+    # the largest size the static array serves (a total order: hist[k] = N - 1 - k)
+    N = api.interval_hist_static_max_n()
+    t = np.arange(N, dtype=np.float64)
+    coords = np.stack([t, np.zeros(N)], axis=1)
+    bits, bitsT = api.causal_matrix(torch.from_numpy(coords).cuda(), inp.GEOM_MINK_CONE)
+    h = api.interval_hist_static(bits, None, N)
+    assert torch.equal(h, torch.arange(N - 1, 0, -1, dtype=torch.int64, device="cuda"))
+
+
+def test_static_scratch_refuses_sizes_beyond_its_capacity(api):
+    N = api.interval_hist_static_max_n() + 1
+    stride = api.row_stride_words(N)
+    bits = torch.zeros((N, stride), dtype=torch.int64, device="cuda")
+    hist = torch.full((N - 1,), 7, dtype=torch.int64, device="cuda")
+    with pytest.raises(RuntimeError, match=r"capacity.*N <= 8192"):
+        api.interval_hist_static(bits, None, N, hist=hist)
+    torch.cuda.synchronize()
+    assert int(hist.min().item()) == 7 and int(hist.max().item()) == 7      # nothing was written
+    # the library still works afterwards
+    assert api.interval_hist_static(bits[:64, :2].contiguous(), None, 64).sum().item() == 0
