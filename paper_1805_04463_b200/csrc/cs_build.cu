@@ -247,13 +247,16 @@ k_causal_matrix(const double *__restrict__ coords, int64_t N, int64_t stride,
         //          conversions, NaN ignored by fmaxf; rounding to nearest is covered by m's 1.001); a point that
         //          may not use the prefilter (Fast::convert) reports +inf, which fails the range test below,
         //   max t_i rounded up and min t_j rounded down, so "max t_i <= min t_j" is only ever claimed when
-        //   it holds for the doubles (a NaN time makes the claim fail or is ignored; either is safe).
+        //   it holds for the doubles (a NaN time makes the claim fail or is ignored: safe where the time is part of
+        //   T, and where it is not -- F::STRICT -- convert() has already refused the point).
         // Inside the diagonal tile i < j must imply t_i <= t_j instead: its points are in time order.
+        // F::STRICT: both claims with < (the header's expression wants d eta > 0 and T does not see eta).
         float fi[NP], hi0, ci = 0.f;
         const bool oki = F::convert(xi0, fi, hi0);
 #pragma unroll
         for (int c = 0; c < NP; c++) ci = fmaxf(ci, fabsf(fi[c]));
-        if (!oki && !(xi0[0] != xi0[0])) ci = __int_as_float(0x7f800000);     // (padding points are NaN: harmless)
+        // a real point that may not use the prefilter takes the tile off it (padding beyond N is NaN and harmless)
+        if (!oki && (int64_t)I * BT + tid < N) ci = __int_as_float(0x7f800000);
         if (GEOM == CS_GEOM_DS2_SLAB) {
             reinterpret_cast<float2 *>(s_f)[tid] = make_float2(fi[0], fi[1]);
         } else {
@@ -270,7 +273,7 @@ k_causal_matrix(const double *__restrict__ coords, int64_t N, int64_t stride,
             const bool okj = F::convert(xj[k], fj[k], hj[k]);
 #pragma unroll
             for (int c = 0; c < NP; c++) cj = fmaxf(cj, fabsf(fj[k][c]));
-            if (!okj && !(xj[k][0] != xj[k][0])) cj = __int_as_float(0x7f800000);
+            if (!okj && act[k] && (int64_t)(JS * NJ + k) * BT + jl < N) cj = __int_as_float(0x7f800000);
             const uint32_t wcj = __reduce_max_sync(0xffffffffu, __float_as_uint(cj));
             const uint32_t wtj = __reduce_max_sync(0xffffffffu, float_key(-__double2float_rd(xj[k][0])));   // -(min t_j)
             if (lane == 0) { s_red[2 + 2 * k][warp] = wcj; s_red[3 + 2 * k][warp] = wtj; }
@@ -286,7 +289,8 @@ k_causal_matrix(const double *__restrict__ coords, int64_t N, int64_t stride,
         bool tile_ordered = false;
         if (any_diag) {   // points beyond N are NaN and only ever sit at the end: their pairs read unrelated either way
             const bool last = tid == BT - 1 || (int64_t)I * BT + tid + 1 >= N;
-            tile_ordered = __syncthreads_and(last || xi0[0] <= s_xi[0][last ? tid : tid + 1]) != 0;
+            const double tnext = s_xi[0][last ? tid : tid + 1];
+            tile_ordered = __syncthreads_and(last || (F::STRICT ? xi0[0] < tnext : xi0[0] <= tnext)) != 0;
         }
         const float Ci = __uint_as_float(r[0]), tmaxI = key_float(r[1]);
 #pragma unroll
@@ -297,7 +301,8 @@ k_causal_matrix(const double *__restrict__ coords, int64_t N, int64_t stride,
                 fast[k] = act[k] && (Cd <= 0x1p100f);
                 m[k] = __fmul_ru(Cd, 0x1p-19f * 1.001f);
             } else {
-                const bool ordered = dg[k] ? tile_ordered : (tmaxI <= -key_float(r[3 + 2 * k]));
+                const float tminJ = -key_float(r[3 + 2 * k]);
+                const bool ordered = dg[k] ? tile_ordered : (F::STRICT ? tmaxI < tminJ : tmaxI <= tminJ);
                 fast[k] = act[k] && ordered && (C >= 0x1p-40f) && (C <= 0x1p40f);
                 m[k] = __fmul_ru(__fmul_ru(C, C), (float)F::MARGIN * 0x1p-24f * 1.001f);
             }

@@ -70,9 +70,7 @@ constexpr int TC_WR0 = TC_EPI0 + TC_EPI_WARPS;   // warps 18..19: writers (stage
 constexpr int TC_WR_WARPS = 2;
 constexpr int TC_THREADS = (TC_WR0 + TC_WR_WARPS) * 32;
 constexpr int TC_PITCH = 9;              // words per staged row (8 + 1: conflict-free 4-byte stores by 32 rows)
-#ifndef TC_NF
-#define TC_NF 12                         // columns of a 32 x 32 block whose sign bit goes through the FMA pipe (0 .. 23)
-#endif
+constexpr int TC_NF = 12;                // columns of a 32 x 32 block whose sign bit goes through the FMA pipe (0 .. 23)
 
 // Per-point data of the tensor route: Fast<> of cs_predicates.cuh for the predicates cs_build.cu already treats as
 // bilinear forms, and two more that are bilinear in derived coordinates only.  F_c is component fcomp(c) of the point's
@@ -88,7 +86,7 @@ struct TcFast : Fast<GEOM, DIM> {
 // du + dv > 0 follows from t_j >= t_i and both differences are positive.
 template <>
 struct TcFast<CS_GEOM_MINK2_LIGHTCONE, 2> {
-    static constexpr bool H = true, RANGE2 = false;
+    static constexpr bool H = true, RANGE2 = false, STRICT = false;
     static constexpr int NP = 2, NNEG = 2, MARGIN = 64;
     __device__ static __forceinline__ double time(const double *x) { return (x[0] + x[1]) * 0.5; }
     __device__ static __forceinline__ constexpr int fcomp(int c) { return 1 - c; }
@@ -106,7 +104,7 @@ struct TcFast<CS_GEOM_MINK2_LIGHTCONE, 2> {
 // span at most 2 pi and its times at most pi (RANGE2); the fp64 rows use the header's expression as everywhere.
 template <>
 struct TcFast<CS_GEOM_DS2_SLAB, 2> {
-    static constexpr bool H = false, RANGE2 = true;
+    static constexpr bool H = false, RANGE2 = true, STRICT = false;
     static constexpr int NP = 4, NNEG = 2, MARGIN = 64;
     __device__ static __forceinline__ double time(const double *x) { return x[0]; }
     __device__ static __forceinline__ constexpr int fcomp(int c) { return c; }
@@ -301,7 +299,7 @@ k_tc_prep(const double *__restrict__ coords, int64_t N, int nA,
         c = fmaxf(c, fabsf(v[q]));
         ok = ok && isfinite(v[q]);
     }
-    ok = ok && isfinite(h);
+    ok = ok && isfinite(h) && isfinite(F::time(x));       // a NaN time would slip through the fmin / fmax of the block summary
     if (!valid) {
 #pragma unroll
         for (int q = 0; q < NP; q++) v[q] = 0.f;
@@ -365,7 +363,10 @@ k_tc_prep(const double *__restrict__ coords, int64_t N, int nA,
     const double tp = F::time(x);
     double tmn = valid ? tp : inf, tmx = valid ? tp : -inf;
     bool sorted = true;                                   // this point <= the next one (fp64; NaN: false)
-    if (valid && gp + 1 < N) sorted = tp <= F::time(coords + (gp + 1) * DIM);
+    if (valid && gp + 1 < N) {                            // F::STRICT: the time is not part of T, d eta > 0 comes from the order alone
+        const double tn = F::time(coords + (gp + 1) * DIM);
+        sorted = F::STRICT ? tp < tn : tp <= tn;
+    }
     float x1lo = __int_as_float(0x7f800000), x1hi = __int_as_float(0xff800000);
     if (F::RANGE2 && valid) { x1lo = __double2float_rd(x[1]); x1hi = __double2float_ru(x[1]); }
 #pragma unroll
@@ -419,7 +420,7 @@ k_tc_prep(const double *__restrict__ coords, int64_t N, int nA,
 //   x = I | J << 16, y = causet, z = margin m (float bits; +inf: every row of the tile goes to fp64), w = unused.
 __global__ void __launch_bounds__(256)
 k_tc_tiles(const TcBlockInfo *__restrict__ info, int nT, uint32_t tiles_per, uint32_t total_tiles, float acc_units,
-           float in_units, int range2, uint4 *__restrict__ tab)
+           float in_units, int range2, int strict, uint4 *__restrict__ tab)
 {
     const uint32_t t = blockIdx.x * 256 + threadIdx.x;
     if (t >= total_tiles) return;
@@ -437,7 +438,8 @@ k_tc_tiles(const TcBlockInfo *__restrict__ info, int nT, uint32_t tiles_per, uin
     const float C = fmaxf(fmaxf(i0.C, i1.C), fmaxf(j0.C, j1.C));
     const bool bad = ((i0.flags | i1.flags | j0.flags | j1.flags) & 4u) != 0;
     const bool ordered = (I == J) ? ((i0.flags & 3u) == 3u && (i1.flags & 1u) != 0)
-                                  : (fmax(i0.tmax, i1.tmax) <= fmin(j0.tmin, j1.tmin));
+                                  : (strict ? fmax(i0.tmax, i1.tmax) < fmin(j0.tmin, j1.tmin)
+                                            : fmax(i0.tmax, i1.tmax) <= fmin(j0.tmin, j1.tmin));
     bool fast = !bad && ordered && C >= 0x1p-40f && C <= 0x1p40f;
     if (range2) {       // 1+1 dS slab: times within pi and angles within 2 pi over the whole tile (both tested a little short)
         const double tspan = fmax(j0.tmax, j1.tmax) - fmin(i0.tmin, i1.tmin);
@@ -857,7 +859,7 @@ int launch_tc_t(const double *coords, int64_t B, int64_t N, int64_t stride, uint
     // IN = the fp32 prefilter's own bound (Fast::MARGIN / 2, conversions included) + the dropped piece products
     k_tc_tiles<<<(unsigned)((total + 255) / 256), 256, 0, st>>>(info, nT, (uint32_t)tiles_per, (uint32_t)total,
                                                                  4.f * (S::K + 2), (float)(TcFast<GEOM, DIM>::MARGIN / 2 + 3 * TcFast<GEOM, DIM>::NP),
-                                                                 TcFast<GEOM, DIM>::RANGE2 ? 1 : 0, tab);
+                                                                 TcFast<GEOM, DIM>::RANGE2 ? 1 : 0, TcFast<GEOM, DIM>::STRICT ? 1 : 0, tab);
     CS_LAUNCHED("k_tc_tiles");
     constexpr size_t smem = SM::BYTES;
     static PerDeviceFlag attr_set;

@@ -108,20 +108,20 @@ struct Pred<CS_GEOM_DS4_SPHERICAL, 7> {
 //                            margin of 2^-18 C^2); anything else falls back to the header's fp64 expression.
 //   3+1 de Sitter, spherical P = (-cos eta, -sin eta, X0..X3), F = (cos eta, sin eta, X0..X3), no h:
 //                            T = cos(omega) - cos(d eta); 12 input roundings + partial sums 1..6 C^2 <= 33 u C^2.
-//                            Unit inputs only (see Fast<DS4_SPHERICAL>::convert: pairs of equal times).
+//                            Unit inputs and finite times only, tiles strictly ordered in time (Fast<DS4_SPHERICAL>).
 // With NP products the bound is (2.01 NP + (NP - 1) + sum of the partial sums) u C^2: 34 (NP = 4), 48 (NP = 5), so the
 // margin is 64 u C^2 up to four products (and for the h-free six of de Sitter) and 96 u C^2 for five.
 // The first NNEG components are stored negated for the past point.  convert() returns false for a point that may not
 // use the prefilter.
 template <int GEOM, int DIM>
 struct Fast {
-    static constexpr bool ok = false, H = false;
+    static constexpr bool ok = false, H = false, STRICT = false;
     static constexpr int NP = 1, NNEG = 0, MARGIN = 64;
     __device__ static __forceinline__ bool convert(const double *, float *, float &) { return false; }
 };
 template <int DIM>
 struct Fast<CS_GEOM_MINK_CONE, DIM> {
-    static constexpr bool ok = true, H = true;
+    static constexpr bool ok = true, H = true, STRICT = false;
     static constexpr int NP = DIM, NNEG = 1, MARGIN = DIM <= 4 ? 64 : 96;
     __device__ static __forceinline__ bool convert(const double *x, float *v, float &h)
     {
@@ -137,7 +137,7 @@ struct Fast<CS_GEOM_MINK_CONE, DIM> {
 };
 template <>
 struct Fast<CS_GEOM_DS2_SLAB, 2> {      // not a bilinear form: its own five-operation expression (above)
-    static constexpr bool ok = true, H = false;
+    static constexpr bool ok = true, H = false, STRICT = false;
     static constexpr int NP = 2, NNEG = 0, MARGIN = 32;
     __device__ static __forceinline__ bool convert(const double *x, float *v, float &h)
     {
@@ -149,24 +149,26 @@ struct Fast<CS_GEOM_DS2_SLAB, 2> {      // not a bilinear form: its own five-ope
 };
 template <>
 struct Fast<CS_GEOM_DS4_SPHERICAL, 7> {
-    static constexpr bool ok = true, H = false;
+    // The time coordinate is not part of T (only its cosine and sine columns are), so the header's "eta_j - eta_i > 0"
+    // must come from the tile test alone: STRICT asks the callers for max eta_i < min eta_j (and strictly increasing
+    // times inside a diagonal tile) instead of <=, and a point whose eta is NaN or infinite -- the header's difference is
+    // then NaN for some partner, "unrelated" whatever the other columns say -- does not take the prefilter.
+    static constexpr bool ok = true, H = false, STRICT = true;
     static constexpr int NP = 6, NNEG = 2, MARGIN = 64;
     __device__ static __forceinline__ bool convert(const double *x, float *v, float &h)
     {
 #pragma unroll
         for (int c = 0; c < 6; c++) v[c] = (float)x[1 + c];
         h = 0.f;
-        // The header's expression also wants eta_j > eta_i; the tile-level time order only gives >=.  With unit
-        // inputs a pair of equal times has T = cos(omega) - 1 <= 2^-29, never above the margin, so it is decided
-        // "unrelated" or re-evaluated; inputs that are not unit vectors do not take the prefilter.
+        // inputs that are not unit vectors do not take the prefilter
         const double n1 = x[1] * x[1] + x[2] * x[2] - 1.0;
         const double n2 = (x[3] * x[3] + x[4] * x[4]) + (x[5] * x[5] + x[6] * x[6]) - 1.0;
-        return fabs(n1) <= 0x1p-30 && fabs(n2) <= 0x1p-30;      // false for NaN
+        return isfinite(x[0]) && fabs(n1) <= 0x1p-30 && fabs(n2) <= 0x1p-30;      // false for NaN
     }
 };
 template <>
 struct Fast<CS_GEOM_FLRW_POLAR, 6> {
-    static constexpr bool ok = true, H = true;
+    static constexpr bool ok = true, H = true, STRICT = false;
     static constexpr int NP = 4, NNEG = 1, MARGIN = 64;
     __device__ static __forceinline__ bool convert(const double *x, float *v, float &h)
     {

@@ -225,7 +225,7 @@ def test_causal_matrix_prefilter_ds4_spherical(api, oracle):
     coords = np.concatenate(sets)
     coords = np.ascontiguousarray(coords[np.lexsort((coords[:, 3], coords[:, 0]))])
     N = coords.shape[0]
-    for variant in range(4):
+    for variant in range(7):
         c = coords.copy()
         if variant == 1:
             c[5, 3] = np.nan; c[300, 0] = np.inf; c[900, 4] = -np.inf; c[1200:1500] = c[1200]
@@ -233,7 +233,23 @@ def test_causal_matrix_prefilter_ds4_spherical(api, oracle):
             c[:, 3:] *= 3.0                                 # not unit vectors: still the header's expression
         if variant == 3:
             c = np.ascontiguousarray(c[rng.permutation(N)])
+        # eta enters the bilinear form through its cosine and sine columns only: whatever the time column itself
+        # decides (d eta > 0, NaN differences) has to survive the prefilter of both a1 routes
+        if variant == 4:                                    # NaN times, every other column still a valid unit vector
+            c[[7, 129, 700, 1300, 2047, 2048, N - 1], 0] = np.nan
+        if variant == 5:                                    # infinite times: inf - inf = NaN (unrelated), inf - finite > 0
+            c[N - 40:, 0] = np.inf; c[:3, 0] = -np.inf
+        if variant == 6:                                    # equal times whose (cos eta, sin eta) columns still differ
+            c[1000:1400, 0] = c[1000, 0]; c[2040:2060, 0] = c[2040, 0]
         o_bits = oracle.causal_matrix_bits(c, inp.GEOM_DS4_SPHERICAL)
+        if variant in (4, 5, 6):                            # the cases bite: the sign of T alone would relate such pairs
+            C = oracle.unpack_bits(o_bits, N)
+            rows = {4: [7, 129, 700, 1300, 2047, 2048, N - 1], 5: list(range(N - 40, N)), 6: list(range(1000, 1400))}[variant]
+            ref = oracle.unpack_bits(oracle.causal_matrix_bits(coords, inp.GEOM_DS4_SPHERICAL), N)
+            if variant == 4:                                # a NaN time is unrelated to everything, in both directions
+                assert ref[rows].any() and ref[:, rows].any() and not C[rows].any() and not C[:, rows].any()
+            else:
+                assert ref[np.ix_(rows, rows)].any() and not C[np.ix_(rows, rows)].any()
         bits, bitsT = gpu_bits(api, c, inp.GEOM_DS4_SPHERICAL)
         assert np.array_equal(to_u64(bits), o_bits), variant
         assert np.array_equal(to_u64(bitsT), oracle.transpose_bits(o_bits, N)), variant
