@@ -66,7 +66,7 @@ enum cs_geometry {
        The spacetime dimension (for the action entry points that take coordinates) is 4. */
     CS_GEOM_FLRW_POLAR = 3,
     /* dim = 7, a point is (eta, cos eta, sin eta, X0, X1, X2, X3): 3+1 de Sitter with spherical foliation,
-       ds^2 = lambda^2 sec^2(eta) (-d eta^2 + d Omega_3^2) (App. A.1.3, PAPER.md:3829-3845), X = (cos psi,
+       ds^2 = lambda^2 sec^2(eta) (-d eta^2 + d Omega_3^2) (App. A.1.3, PAPER.md:3845-3863), X = (cos psi,
        sin psi cos th, sin psi sin th cos ph, sin psi sin th sin ph) the point's unit vector on the 3-sphere.
        Timelike <=> d eta^2 > d Sigma^2 with d Sigma = omega the great-circle angle; for
        0 < d eta <= pi that is cos(d eta) < cos(omega) (reading A18):
@@ -90,7 +90,8 @@ enum cs_status {
 
 /* How a2 is computed.  All routes give identical integers. */
 enum cs_route {
-    CS_ROUTE_AUTO = 0,      /* the library's default for this N */
+    CS_ROUTE_AUTO = 0,      /* the library's default for this N: CS_ROUTE_TENSOR_PAIR for 1024 <= N <= 2^21 on a device that
+                               passed cs_a2_tensor_selfcheck, else CS_ROUTE_POPC */
     CS_ROUTE_POPC = 1,      /* shared-memory tiled AND + POPC (Alg. 20 restated for the GPU) */
     CS_ROUTE_TENSOR = 2,    /* count matrix C.C as a 0/1 int8 contraction on tcgen05 tensor cores */
     CS_ROUTE_TENSOR_FP4 = 3,/* the same contraction with 4-bit (E2M1, unit block scales) operands, fp32 accumulators */
@@ -139,8 +140,11 @@ enum cs_a1_route {
  *              stream-ordered memory pool the library owns on this device.
  * bits / bitsT must be 16-byte aligned.  Errors as cs_causal_matrix, + CS_ERR_WORKSPACE. */
 size_t cs_causal_matrix_workspace(int64_t B, int64_t N, int dim, int geometry, int route);
-/* What CS_A1_AUTO resolves to for B causets of N points: CS_A1_TENSOR once the launch has
- * at least 128 tiles of 256 x 256 pairs (one causet: N >= 3841; ensembles earlier; always N >= 256), else CS_A1_FMA. */
+/* What CS_A1_AUTO resolves to for B causets of N points by size alone: CS_A1_TENSOR once the launch has
+ * at least 128 tiles of 256 x 256 pairs (one causet: N >= 3841; ensembles earlier; always N >= 256), else CS_A1_FMA.
+ * Host logic only: it does not consult the device's self-check (cs_a1_tensor_selfcheck), so on a device that failed
+ * it -- or on which the check could not run -- AUTO runs the FMA route although this call, and
+ * cs_causal_matrix_workspace(route = AUTO), still answer for the tensor route (the workspace is then simply unused). */
 int cs_default_a1_route(int64_t B, int64_t N, int dim, int geometry);
 int cs_causal_matrix_ex(const double *coords, int64_t B, int64_t N, int dim, int geometry, int route,
                         uint64_t *bits, uint64_t *bitsT, void *workspace, size_t workspace_bytes, void *stream);
@@ -153,7 +157,7 @@ int cs_causal_matrix_ex(const double *coords, int64_t B, int64_t N, int dim, int
  *             |a - T| / m, m = the margin of the pair's tile (a decision by sign can only be wrong if this reaches 1),
  *             [4] the largest |a - S| in the unit of [0], S = the exact sum of the products of the bf16 operand pieces
  *             the tensor core was given (its accumulation error alone).
- * Synchronises `stream`.  Errors: CS_ERR_ARG, CS_ERR_DIM, CS_ERR_WORKSPACE, CS_ERR_CUDA. */
+ * Synchronises `stream`.  Errors: CS_ERR_ARG (also N < 256), CS_ERR_DIM, CS_ERR_WORKSPACE, CS_ERR_CUDA. */
 int cs_a1_tensor_probe(const double *coords, int64_t N, int dim, uint64_t *bits, uint64_t *bitsT,
                        void *workspace, size_t workspace_bytes, double *out_host, void *stream);
 
@@ -227,6 +231,18 @@ int cs_interval_hist_ex(const uint64_t *bits, const uint64_t *bitsT, int64_t N, 
 int64_t cs_interval_hist_static_max_n(void);
 int cs_interval_hist_static(const uint64_t *bits, const uint64_t *bitsT, int64_t N, int64_t kmax,
                             int64_t *hist, int64_t *n_relations, void *stream);
+
+/* The self-check behind CS_ROUTE_AUTO.  CS_ROUTE_TENSOR_PAIR reads its counts out of the bit patterns of subnormal
+ * fp32 accumulators, exact only while the tensor cores add subnormals without flushing or rounding them (DESIGN.md,
+ * reading A22: measured, not documented by the vendor).  The first time AUTO would take that route on a device the
+ * library runs it on a built-in total order of 2125 elements (closed form N_k = N-1-k, every count 0..N-2 occurs) and
+ * on a seeded 3+1 causet against the POPC route (whole histogram, and kmax = 3); on any difference AUTO keeps the POPC
+ * route on that device (the workspace AUTO asked for is large enough for it) and cs_last_cuda_error() says what
+ * differed.  This call runs the check if it has not run yet and reports it: 1 exact, 0 not (AUTO = POPC there;
+ * CS_ROUTE_TENSOR_PAIR by name still runs), < 0 a cs_status.  The first time it takes ~2 MiB from the library's
+ * stream-ordered pool and synchronises `stream` (about 1 ms); then it returns the cached answer.  Like
+ * cs_a1_tensor_selfcheck it should first run outside any stream capture. */
+int cs_a2_tensor_selfcheck(void *stream);
 
 /* What the last cs_interval_hist* call that used `workspace` executed (for the roofline on executed work):
  *   stats_host  host, int64[4], overwritten:

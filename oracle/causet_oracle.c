@@ -24,7 +24,7 @@
  *      (Algorithm 13).
  *   6. (NEXT-4) the FLRW relation of Eq. 7.7 as a fourth predicate of stage 1; the flat cone
  *      in 4+1 dimensions (the 4+1 diamond of App. A.1.2); the 3+1 de Sitter slab with
- *      spherical foliation (App. A.1.3, PAPER.md:3829-3845) as a fifth predicate.
+ *      spherical foliation (App. A.1.3, PAPER.md:3845-3863) as a fifth predicate.
  *
  * Floating point: every predicate is evaluated in fp64 exactly in the order
  * written below; compile with -ffp-contract=off (no FMA), no -ffast-math.
@@ -68,7 +68,7 @@ static const double ORC_TWO_PI = 6.283185307179586476925286766559;
  *                   cos ph_i cos ph_j + sin ph_i sin ph_j, so the predicate is additions and multiplications
  *                   only (reading A17).  j is in the future of i only if eta_j > eta_i.
  *  DS4_SPHERICAL:   (NEXT-4) 3+1 de Sitter, spherical foliation: ds^2 = lambda^2 sec^2(eta) (-d eta^2 + d Omega_3^2)
- *                   (PAPER.md:3829-3831), conformal to R x S^3.  In conformal time "timelike ... intervals
+ *                   (PAPER.md:3845-3847), conformal to R x S^3.  In conformal time "timelike ... intervals
  *                   correspond to d eta^2 > d Sigma^2"; on the unit 3-sphere d Sigma is the
  *                   great-circle angle omega between the two points, cos omega = X_i . X_j with X the unit
  *                   4-vector (cos psi, sin psi cos th, sin psi sin th cos ph, sin psi sin th sin ph).  For

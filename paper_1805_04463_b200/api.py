@@ -32,8 +32,7 @@ A1_FMA = 1
 A1_TENSOR = 2
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-# CAUSALSET_LIB selects another build of the same library (A/B timing of kernel variants); default: in-tree
-LIB_PATH = os.environ.get("CAUSALSET_LIB") or os.path.join(_HERE, "libcausalset.so")
+LIB_PATH = os.path.join(_HERE, "libcausalset.so")       # the in-tree build, nothing else
 HEADER_PATH = os.path.join(os.path.dirname(_HERE), "include", "causalset.h")
 
 _i64 = ctypes.c_int64
@@ -52,6 +51,7 @@ _SIGNATURES = {
     "cs_default_a1_route": (_int, [_i64, _i64, _int, _int]),
     "cs_causal_matrix_ex": (_int, [_p, _i64, _i64, _int, _int, _int, _p, _p, _p, _sz, _p]),
     "cs_a1_tensor_selfcheck": (_int, [_p]),
+    "cs_a2_tensor_selfcheck": (_int, [_p]),
     "cs_a1_tensor_probe": (_int, [_p, _i64, _int, _p, _p, _p, _sz, _p, _p]),
     "cs_transpose_bits": (_int, [_p, _i64, _p, _p]),
     "cs_degrees": (_int, [_p, _p, _i64, _p, _p, _p]),
@@ -190,6 +190,14 @@ def a1_tensor_selfcheck() -> bool:
     rc = load().cs_a1_tensor_selfcheck(_stream())
     if rc < 0:
         _check(rc, "cs_a1_tensor_selfcheck")
+    return rc == 1
+
+
+def a2_tensor_selfcheck() -> bool:
+    """True if this device's tensor cores add subnormal fp32 partial sums exactly, which the tensor a2 route rests on."""
+    rc = load().cs_a2_tensor_selfcheck(_stream())
+    if rc < 0:
+        _check(rc, "cs_a2_tensor_selfcheck")
     return rc == 1
 
 

@@ -1,6 +1,6 @@
 // cs_api.cu -- the extern "C" boundary of libcausalset.so (include/causalset.h).
 // Argument checking, workspace carving and kernel sequencing only; the arithmetic lives in
-// cs_poset.cu (NEXT-3), cs_build.cu (a1), cs_interval_popc.cu / cs_interval_tensor.cu / cs_interval_fp4.cu / cs_interval_pair.cu (a2) and cs_action.cu (a3).
+// cs_poset.cu (NEXT-3), cs_build.cu (a1), cs_selfcheck.cu (the a2 self-check), cs_interval_popc.cu / cs_interval_tensor.cu / cs_interval_fp4.cu / cs_interval_pair.cu (a2) and cs_action.cu (a3).
 #include <mutex>
 
 #include "cs_common.cuh"
@@ -63,8 +63,19 @@ static int interval_hist_impl(const uint64_t *bits, const uint64_t *bitsT, int64
     if (row_begin < 0) row_begin = 0;
     if (row_end > N) row_end = N;
     if (row_begin >= row_end) return CS_OK;
+    const bool by_default = route == CS_ROUTE_AUTO;
     route = resolve_route(N, route);
     if (route < 0) return CS_ERR_ARG;
+    if (by_default && route == CS_ROUTE_TENSOR_PAIR) {
+        // the tensor route reads integers out of subnormal accumulators (reading A22): checked once per
+        // device; a device that fails the check -- or on which it could not run -- gets the bit route
+        bool trusted = false;
+        if (interval_pair_trusted(st, &trusted) != CS_OK) {
+            cudaGetLastError();
+            trusted = false;
+        }
+        if (!trusted) route = CS_ROUTE_POPC;
+    }
     const size_t need = interval_ws_bytes(B, N, bitsT != nullptr, route);
     if (!workspace || workspace_bytes < need || ((uintptr_t)workspace & 255)) return CS_ERR_WORKSPACE;
     unsigned char *ws = static_cast<unsigned char *>(workspace);
@@ -131,7 +142,8 @@ int cs_default_route(int64_t N)
     // measured on B200: the 4-bit tensor route on CTA pairs wins from N ~ 1024 up (12.5 ms
     // against 20.3 ms single-CTA and 327 ms POPC at N = 65536); below that a few 256 x 256 tiles cannot
     // fill the machine and the bit route is as fast
-    return interval_tensor_available() && N >= 1024 ? CS_ROUTE_TENSOR_PAIR : CS_ROUTE_POPC;
+    // beyond N = 2^21 the tensor route's 8 * count no longer fits the exact range of its accumulators: bit route
+    return interval_tensor_available() && N >= 1024 && N <= ((int64_t)1 << 21) ? CS_ROUTE_TENSOR_PAIR : CS_ROUTE_POPC;
 }
 
 static int check_a1_args(const double *coords, int64_t B, int64_t N, int dim, int geometry, const uint64_t *bits)
@@ -143,6 +155,17 @@ static int check_a1_args(const double *coords, int64_t B, int64_t N, int dim, in
     if (N == 0 || B == 0) return 1;      // nothing to do
     if (!coords || !bits) return CS_ERR_ARG;
     return CS_OK;
+}
+
+// a1 -> a2 -> a3 entry points: the arguments of a1 and a spacetime dimension the action is defined for (Eq. 4.10-4.12:
+// 2, 3, 4), checked before any work is enqueued
+static int check_pipeline_args(int64_t N, int dim, int geometry)
+{
+    const int rc = check_a1_args(reinterpret_cast<const double *>(16), 1, N > 0 ? N : 1, dim, geometry,
+                                 reinterpret_cast<const uint64_t *>(16));
+    if (rc < 0) return rc;
+    const int sd = spacetime_dim(geometry, dim);
+    return (sd < 2 || sd > 4) ? CS_ERR_DIM : CS_OK;
 }
 
 size_t cs_causal_matrix_workspace(int64_t B, int64_t N, int dim, int geometry, int route)
@@ -188,10 +211,17 @@ int cs_a1_tensor_selfcheck(void *stream)
     return rc ? rc : (trusted ? 1 : 0);
 }
 
+int cs_a2_tensor_selfcheck(void *stream)
+{
+    bool trusted = false;
+    const int rc = interval_pair_trusted(static_cast<cudaStream_t>(stream), &trusted);
+    return rc ? rc : (trusted ? 1 : 0);
+}
+
 int cs_a1_tensor_probe(const double *coords, int64_t N, int dim, uint64_t *bits, uint64_t *bitsT,
                        void *workspace, size_t workspace_bytes, double *out_host, void *stream)
 {
-    if (!coords || !bits || !out_host || N < 1) return CS_ERR_ARG;
+    if (!coords || !bits || !out_host || N < 256) return CS_ERR_ARG;     // the tensor route wants rows of >= 32 bytes
     if (dim != 4 && dim != 5) return CS_ERR_DIM;
     if (misaligned16(bits, bitsT)) return CS_ERR_ARG;
     if (!causal_tc_supported(CS_GEOM_MINK_CONE, dim)) return CS_ERR_ARG;
@@ -376,6 +406,10 @@ int cs_bd_action_batched(const double *coords, int64_t B, int64_t N, int dim, in
     if (B < 0 || N < 0) return CS_ERR_ARG;
     if (B == 0) return CS_OK;
     if (!coords || !actions) return CS_ERR_ARG;
+    {   // geometry, dim and the action's dimension before any chunk is built
+        const int rc = check_pipeline_args(N, dim, geometry);
+        if (rc) return rc;
+    }
     if (!workspace || workspace_bytes < cs_bd_action_batched_workspace(B, N) || ((uintptr_t)workspace & 255))
         return CS_ERR_WORKSPACE;
     cudaStream_t st = static_cast<cudaStream_t>(stream);
@@ -462,7 +496,10 @@ int cs_bd_action_batched_host(const double *coords_host, int64_t B, int64_t N, i
     if (B < 0 || N < 0) return CS_ERR_ARG;
     if (B == 0) return CS_OK;
     if (!coords_host || !actions_host) return CS_ERR_ARG;
-    if (dim < 2 || dim > 7) return CS_ERR_DIM;
+    {
+        const int rc = check_pipeline_args(N, dim, geometry);
+        if (rc) return rc;
+    }
     if (!workspace || workspace_bytes < cs_bd_action_batched_host_workspace(B, N, dim) || ((uintptr_t)workspace & 255))
         return CS_ERR_WORKSPACE;
     cudaStream_t st = static_cast<cudaStream_t>(stream);
@@ -498,22 +535,27 @@ int cs_bd_action_batched_host(const double *coords_host, int64_t B, int64_t N, i
     for (int64_t b0 = 0; b0 < B; b0 += CB, c++) {
         const int64_t nb = (B - b0 < CB) ? B - b0 : CB;
         const int buf = (int)(c & 1);
-        if (c >= 2) CS_CUDA(cudaStreamWaitEvent(copy_stream, consumed[buf], 0));
-        CS_CUDA(cudaMemcpyAsync(cdev[buf], coords_host + b0 * N * dim, (size_t)nb * N * dim * 8,
-                                cudaMemcpyHostToDevice, copy_stream));
-        CS_CUDA(cudaEventRecord(copied[buf], copy_stream));
-        CS_CUDA(cudaStreamWaitEvent(st, copied[buf], 0));
-        const bool fits = cs_causal_matrix_workspace(nb, N, dim, geometry, CS_A1_AUTO) <= a1_bytes;
-        int rc = cs_causal_matrix_ex(cdev[buf], nb, N, dim, geometry, CS_A1_AUTO, bits, bitsT, fits ? a1ws : nullptr,
-                                     fits ? a1_bytes : 0, stream);
-        if (rc) return rc;
-        CS_CUDA(cudaEventRecord(consumed[buf], st));
-        if (kmax < 3) CS_CUDA(cudaMemsetAsync(hist, 0, (size_t)nb * 4 * 8, st));
-        rc = interval_hist_impl(bits, bitsT, nb, N, kmax, 0, N, CS_ROUTE_AUTO, hist, nullptr, ws, left, st, b0 > 0);
-        if (rc) return rc;
-        rc = launch_bd_action(hist, kmax + 1, nb, kmax, N, spacetime_dim(geometry, dim), actions + b0, nullptr,
-                              hist4 + b0 * 4, st);
-        if (rc) return rc;
+        const int rc = [&]() -> int {
+            if (c >= 2) CS_CUDA(cudaStreamWaitEvent(copy_stream, consumed[buf], 0));
+            CS_CUDA(cudaMemcpyAsync(cdev[buf], coords_host + b0 * N * dim, (size_t)nb * N * dim * 8,
+                                    cudaMemcpyHostToDevice, copy_stream));
+            CS_CUDA(cudaEventRecord(copied[buf], copy_stream));
+            CS_CUDA(cudaStreamWaitEvent(st, copied[buf], 0));
+            const bool fits = cs_causal_matrix_workspace(nb, N, dim, geometry, CS_A1_AUTO) <= a1_bytes;
+            int r = cs_causal_matrix_ex(cdev[buf], nb, N, dim, geometry, CS_A1_AUTO, bits, bitsT, fits ? a1ws : nullptr,
+                                        fits ? a1_bytes : 0, stream);
+            if (r) return r;
+            CS_CUDA(cudaEventRecord(consumed[buf], st));
+            if (kmax < 3) CS_CUDA(cudaMemsetAsync(hist, 0, (size_t)nb * 4 * 8, st));
+            r = interval_hist_impl(bits, bitsT, nb, N, kmax, 0, N, CS_ROUTE_AUTO, hist, nullptr, ws, left, st, b0 > 0);
+            if (r) return r;
+            return launch_bd_action(hist, kmax + 1, nb, kmax, N, spacetime_dim(geometry, dim), actions + b0, nullptr,
+                                    hist4 + b0 * 4, st);
+        }();
+        if (rc) {   // do not hand the caller's coords_host back while the copy stream may still be reading it
+            cudaStreamSynchronize(copy_stream);
+            return rc;
+        }
     }
     CS_CUDA(cudaMemcpyAsync(actions_host, actions, (size_t)B * 8, cudaMemcpyDeviceToHost, st));
     if (hist4_host) CS_CUDA(cudaMemcpyAsync(hist4_host, hist4, (size_t)B * 4 * 8, cudaMemcpyDeviceToHost, st));
@@ -537,7 +579,10 @@ int cs_action_host(const double *coords_host, int64_t N, int dim, int geometry, 
                    void *workspace, size_t workspace_bytes, void *stream)
 {
     if (N < 0 || !hist_host || !action_host || (N > 0 && !coords_host)) return CS_ERR_ARG;
-    if (dim < 2 || dim > 7) return CS_ERR_DIM;
+    {
+        const int rc = check_pipeline_args(N, dim, geometry);
+        if (rc) return rc;
+    }
     if (!workspace || workspace_bytes < cs_action_host_workspace(N, kmax) || ((uintptr_t)workspace & 255))
         return CS_ERR_WORKSPACE;
     cudaStream_t st = static_cast<cudaStream_t>(stream);

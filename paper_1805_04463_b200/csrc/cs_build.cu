@@ -497,7 +497,7 @@ size_t causal_matrix_scratch_bytes(int64_t B, int64_t N, int dim, int geometry, 
 
 // Stream-ordered scratch for callers that pass no workspace: one memory pool per device, owned by the library, which
 // keeps what it has allocated (release threshold = never), so that after the first call an allocation is a pointer bump.
-static int scratch_pool(cudaMemPool_t *out)
+int scratch_pool(cudaMemPool_t *out)
 {
     static cudaMemPool_t pools[MAX_DEVICES];
     static bool ready[MAX_DEVICES];
@@ -563,11 +563,13 @@ int tensor_route_trusted(cudaStream_t st, bool *trusted)
                 unsigned char *p = nullptr;
                 CS_CUDA(cudaMallocFromPoolAsync(reinterpret_cast<void **>(&p), cb + 2 * mb + sb, pool, st));
                 double *coords = reinterpret_cast<double *>(p);
-                k_selfcheck_coords<<<(unsigned)((N + 255) / 256), 256, 0, st>>>(coords, (int)N, dim);
-                CS_LAUNCHED("k_selfcheck_coords");
                 double out[5] = {0, 0, 0, 0, 0};
-                rc = launch_causal_tc_probe(coords, N, dim, reinterpret_cast<uint64_t *>(p + cb),
-                                            reinterpret_cast<uint64_t *>(p + cb + mb), p + cb + 2 * mb, out, st);   // synchronises
+                rc = [&]() -> int {                       // every exit passes the cudaFreeAsync below
+                    k_selfcheck_coords<<<(unsigned)((N + 255) / 256), 256, 0, st>>>(coords, (int)N, dim);
+                    CS_LAUNCHED("k_selfcheck_coords");
+                    return launch_causal_tc_probe(coords, N, dim, reinterpret_cast<uint64_t *>(p + cb),
+                                                  reinterpret_cast<uint64_t *>(p + cb + mb), p + cb + 2 * mb, out, st);   // synchronises
+                }();
                 cudaFreeAsync(p, st);
                 if (rc) return rc;
                 ok = out[3] > 0.0 && out[3] < 0.25;
@@ -587,8 +589,12 @@ int launch_causal_matrix(const double *coords, int64_t B, int64_t N, int dim, in
     if (r < 0) return CS_ERR_ARG;
     if (r == CS_A1_TENSOR && route == CS_A1_AUTO) {
         bool trusted = false;
-        const int rc = tensor_route_trusted(st, &trusted);
-        if (rc) return rc;
+        // a self-check that could not run (say, its pool allocation failed) is no reason to fail the caller: AUTO
+        // takes the route that needs no trust, and the check is tried again on the next call
+        if (tensor_route_trusted(st, &trusted) != CS_OK) {
+            cudaGetLastError();
+            trusted = false;
+        }
         if (!trusted) r = CS_A1_FMA;
     }
     if (r == CS_A1_FMA) return launch_causal_fma(coords, B, N, dim, geometry, bits, bitsT, st);

@@ -885,7 +885,7 @@ int launch_tc_t(const double *coords, int64_t B, int64_t N, int64_t stride, uint
 
 bool causal_tc_supported(int geometry, int dim)
 {
-    if (!interval_tensor_available()) return false;      // tcgen05: compute capability 10.x
+    if (!interval_tensor_available()) return false;      // (a constant true: the library is built for sm_100a only)
     switch (geometry) {
     case CS_GEOM_MINK2_LIGHTCONE: return dim == 2;
     case CS_GEOM_DS2_SLAB: return dim == 2;
@@ -949,16 +949,19 @@ int launch_causal_tc_probe(const double *coords, int64_t N, int dim, uint64_t *b
     const int64_t stride = row_stride_words(N);
     TcProbe *dp = nullptr;
     CS_CUDA(cudaMallocAsync(reinterpret_cast<void **>(&dp), sizeof(TcProbe), st));
-    CS_CUDA(cudaMemsetAsync(dp, 0, sizeof(TcProbe), st));
-    int rc = CS_ERR_DIM;
-    if (dim == 4) rc = launch_tc_t<CS_GEOM_MINK_CONE, 4, true>(coords, 1, N, stride, bits, bitsT, scratch, dp, st);
-    if (dim == 5) rc = launch_tc_t<CS_GEOM_MINK_CONE, 5, true>(coords, 1, N, stride, bits, bitsT, scratch, dp, st);
     TcProbe hp;
     memset(&hp, 0, sizeof(hp));
-    if (rc == CS_OK) {
+    // every exit below passes the cudaFreeAsync: the counters are not leaked when a step fails
+    int rc = [&]() -> int {
+        CS_CUDA(cudaMemsetAsync(dp, 0, sizeof(TcProbe), st));
+        int r = CS_ERR_DIM;
+        if (dim == 4) r = launch_tc_t<CS_GEOM_MINK_CONE, 4, true>(coords, 1, N, stride, bits, bitsT, scratch, dp, st);
+        if (dim == 5) r = launch_tc_t<CS_GEOM_MINK_CONE, 5, true>(coords, 1, N, stride, bits, bitsT, scratch, dp, st);
+        if (r) return r;
         CS_CUDA(cudaMemcpyAsync(&hp, dp, sizeof(hp), cudaMemcpyDeviceToHost, st));
         CS_CUDA(cudaStreamSynchronize(st));
-    }
+        return CS_OK;
+    }();
     cudaFreeAsync(dp, st);
     if (rc) return rc;
     float err;

@@ -85,6 +85,8 @@ int launch_causal_matrix(const double *coords, int64_t B, int64_t N, int dim, in
                          uint64_t *bits, uint64_t *bitsT, void *scratch, size_t scratch_bytes, cudaStream_t st);
 size_t causal_matrix_scratch_bytes(int64_t B, int64_t N, int dim, int geometry, int route);
 int tensor_route_trusted(cudaStream_t st, bool *trusted);   // one-time self-check of the tensor a1 route on this device
+int interval_pair_trusted(cudaStream_t st, bool *trusted);  // the same for the tensor a2 route (cs_selfcheck.cu)
+int scratch_pool(cudaMemPool_t *out);                       // the library's stream-ordered pool on the current device (cs_build.cu)
 bool causal_tc_supported(int geometry, int dim);
 size_t causal_tc_scratch_bytes(int64_t B, int64_t N, int dim, int geometry);
 int launch_causal_tc(const double *coords, int64_t B, int64_t N, int dim, int geometry,

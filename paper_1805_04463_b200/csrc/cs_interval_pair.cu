@@ -20,9 +20,10 @@
 //    the accumulator is the integer 8 * count -- no float-to-integer step in the epilogue (the tally of the
 //    ensemble case shifts by it directly: 2 instead of 4 instructions per pair).  Exact while
 //    8 * count < 2^24 (the fp32 grid stays 2^-149 up to there): count < 2^21.  Measured: the tensor cores
-//    accumulate subnormals without flushing; every a2 parity test runs on this path.
-//  * tiles are visited in a table order (longest K first in bands of 8 diagonals, I-major inside
-//    a band) so that the ~74 tiles in flight share a few row panels in L2.
+//    accumulate subnormals without flushing; every a2 parity test runs on this path, and CS_ROUTE_AUTO takes it on a
+//    device only after the self-check of cs_selfcheck.cu (reading A22).
+//  * tiles are visited in a table order (longest K first; single diagonals up to nT = 160, bands of 32 diagonals with
+//    snake rows beyond, see launch_interval_pair) so that the ~74 tiles in flight share a few row panels in L2.
 //
 // Products are 0 or 2^-146 and the fp32 accumulators are exact for counts < 2^21.
 #include <cuda.h>
@@ -60,7 +61,7 @@ constexpr int HS_BATCHED = 2048;        // bins when several causets share a CTA
 constexpr int EPI_WARPS = 8, EXPA_WARP0 = 8, EXPB_WARP0 = 12, EXP_WARPS = 8, MMA_WARP = 16, LOAD_WARP = 17;
 constexpr int THREADS = 20 * 32;
 constexpr int SMEM_BYTES = SMEM_FIXED + HS_MAX * 4;
-constexpr uint32_t SF_COL = 256;        // three 16-column regions of constant scale factors: 2^1, 2^0, 2^-1
+constexpr uint32_t SF_COL = 256;        // three 16-column regions of constant scale factors: 2^-72, 2^-73, 2^-74
 constexpr uint32_t A_COL = 320;         // TMEM ring of the A operand: NS x 32 columns
 static_assert(A_COL + NS * 32 <= 512, "TMEM columns");
 static_assert(SMEM_BYTES <= 227 * 1024, "shared memory");
@@ -490,7 +491,7 @@ k_interval_pair(const __grid_constant__ CUtensorMap mapU, const __grid_constant_
     cluster_sync();           // barriers of the peer are initialised before anyone arrives on them
     tc_fence_after();
     const uint32_t tmem_base = *s_tmem;
-    if (warp < 4) {           // constant UE8M0 block scales: 2^1, 2^0, 2^-1 in every byte of their region
+    if (warp < 4) {           // constant UE8M0 block scales, one value in every byte of its region
         const uint32_t sf = tmem_base + ((uint32_t)(warp * 32) << 16) + SF_COL;
         tmem_st16_const(sf, 0x37373737u);          // 2^-72, 2^-73, 2^-74 on both operands
         tmem_st16_const(sf + 16, 0x36363636u);

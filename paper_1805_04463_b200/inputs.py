@@ -161,7 +161,7 @@ def sprinkle_mink5_diamond(N: int, seed: int) -> np.ndarray:
 
 
 def sprinkle_ds4_spherical(N: int, seed: int, eta0: float = 1.0) -> np.ndarray:
-    """3+1 de Sitter slab, spherical foliation (PAPER.md:3829-3845): eta in [0, eta0] with density ~ sec^4 eta, psi with
+    """3+1 de Sitter slab, spherical foliation (PAPER.md:3845-3863): eta in [0, eta0] with density ~ sec^4 eta, psi with
     density ~ sin^2 psi (u = (2 psi - sin 2 psi) / 2 pi "must be inverted numerically"), theta* = arccos(1 - 2u),
     phi* = 2 pi u; draws per point in the order eta, psi, theta, phi.  The eta CDF is (tan eta + tan^3 eta / 3) /
     (tan eta0 + tan^3 eta0 / 3) (the integral of sec^4), inverted numerically as well.

@@ -52,6 +52,21 @@ def test_argument_errors_need_no_gpu(lib):
     assert lib.cs_causal_matrix_workspace(1, 4096, 4, 1, 1) == 0                             # FMA route: no scratch
     assert lib.cs_causal_matrix_workspace(1, 4096, 4, 1, 2) >= 4096 * (128 + 32)             # operand rows + coordinates
     assert lib.cs_a1_tensor_probe(None, 8, 4, None, None, None, 0, None, None) == -1
+    # the probe runs the tensor route, which needs N >= 256 (rows of at least one 32-byte TMA box)
+    out5 = (ctypes.c_double * 5)()
+    p16 = ctypes.c_void_p(16)
+    assert lib.cs_a1_tensor_probe(p16, 255, 4, p16, None, None, 0, ctypes.addressof(out5), None) == -1
+    assert lib.cs_a1_tensor_probe(p16, 256, 3, p16, None, None, 0, ctypes.addressof(out5), None) == -2
+    assert lib.cs_a1_tensor_probe(p16, 256, 4, p16, None, None, 0, ctypes.addressof(out5), None) == -5   # no workspace
+    # the pipeline entry points check geometry, dim and the action's dimension before any chunk is built:
+    # the 4+1 cone has a causal matrix but no action (Eq. 4.10-4.12 stop at d = 4)
+    assert lib.cs_bd_action_batched(p16, 2, 100, 5, 1, p16, None, None, 0, None) == -2
+    assert lib.cs_bd_action_batched(p16, 2, 100, 4, 9, p16, None, None, 0, None) == -3
+    assert lib.cs_bd_action_batched(p16, 2, 100, 4, 1, p16, None, None, 0, None) == -5                    # then the workspace
+    assert lib.cs_bd_action_batched_host(p16, 2, 100, 5, 1, p16, None, None, 0, None) == -2
+    assert lib.cs_bd_action_batched_host(p16, 2, 100, 6, 4, p16, None, None, 0, None) == -2              # dS4 points have 7 numbers
+    assert lib.cs_action_host(p16, 100, 5, 1, -1, p16, p16, None, 0, None) == -2
+    assert lib.cs_action_host(p16, 100, 2, 7, -1, p16, p16, None, 0, None) == -3
     # CS_A1_AUTO: the tensor route from 128 tiles of 256 x 256 pairs up, never below N = 256 (host logic only)
     assert lib.cs_default_a1_route(1, 65536, 4, 1) == 2 and lib.cs_default_a1_route(1, 131072, 2, 2) == 2
     assert lib.cs_default_a1_route(1, 3840, 4, 1) == 1 and lib.cs_default_a1_route(1, 3841, 4, 1) == 2
@@ -64,6 +79,8 @@ def test_argument_errors_need_no_gpu(lib):
     assert lib.cs_interval_hist(None, None, 10, -1, None, None, None, 0, None) == -1
     assert lib.cs_interval_hist_workspace(65536, -1, 1, 1) >= 256
     assert lib.cs_interval_hist_workspace(1024, -1, 0, 1) >= 256 + 1024 * 16 * 8
+    # CS_ROUTE_AUTO: the tensor route for 1024 <= N <= 2^21, the bit route outside (host logic)
+    assert [lib.cs_default_route(n) for n in (0, 1023, 1024, 65536, 1 << 21, (1 << 21) + 1, 1 << 23)] == [1, 1, 4, 4, 4, 1, 1]
     # the entry point with static scratch refuses what its array cannot hold, before touching the device
     assert lib.cs_interval_hist_static_max_n() == 8192
     assert lib.cs_interval_hist_static(ctypes.c_void_p(16), None, 8193, -1, ctypes.c_void_p(16), None, None) == -7

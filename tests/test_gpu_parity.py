@@ -21,7 +21,7 @@ GEOMS = [
     (inp.GEOM_DS2_SLAB, 2),
     (inp.GEOM_FLRW_POLAR, 6),          # NEXT-4: Eq. 7.7
     (inp.GEOM_MINK_CONE, 5),           # NEXT-4: 4+1 diamond
-    (inp.GEOM_DS4_SPHERICAL, 7),       # NEXT-4: 3+1 de Sitter, spherical foliation (PAPER.md:3829-3845)
+    (inp.GEOM_DS4_SPHERICAL, 7),       # NEXT-4: 3+1 de Sitter, spherical foliation (PAPER.md:3845-3863)
 ]
 
 
@@ -625,6 +625,10 @@ def _full_size_check(api, oracle, cfg):
     assert int((np.arange(N - 1, dtype=np.int64) * h).sum()) == int((outdeg * indeg).sum())
     o_hist, _, _ = oracle.interval_hist_alg20(o_bits, N)
     assert np.array_equal(h, o_hist)
+    # the two single-CTA tensor routes (kept as measured alternatives) at the size they were measured at: their
+    # global-atomic tail, the 16/32-bit schedule limits and the int8 route's N <= 131072 bound are live here
+    for r in (api.ROUTE_TENSOR, api.ROUTE_TENSOR_FP4, api.ROUTE_POPC if N <= 16384 else api.ROUTE_TENSOR_PAIR):
+        assert np.array_equal(api.interval_hist(bits, bitsT, N, route=r).cpu().numpy(), o_hist), "route %d" % r
     rng = np.random.default_rng(cfg.index)
     for r0 in sorted(rng.integers(0, N - 64, 3).tolist()):
         part = api.interval_hist(bits, bitsT, N, row_begin=r0, row_end=r0 + 40).cpu().numpy()
@@ -664,6 +668,8 @@ def test_headline_size_routes_agree_on_device(api):
     executed, total, empty, examined = api.interval_hist_stats(ws)
     popc = api.interval_hist(bits, bitsT, N, route=api.ROUTE_POPC)
     assert torch.equal(pair, popc)
+    for r in (api.ROUTE_TENSOR, api.ROUTE_TENSOR_FP4):
+        assert torch.equal(api.interval_hist(bits, bitsT, N, route=r), popc), "route %d" % r
     assert torch.equal(api.interval_hist(bits, bitsT, N, kmax=3), popc[:4])
     a = api.interval_hist(bits, bitsT, N, route=api.ROUTE_TENSOR_PAIR, row_begin=30000, row_end=31000)
     b = api.interval_hist(bits, bitsT, N, route=api.ROUTE_POPC, row_begin=30000, row_end=31000)
@@ -738,6 +744,49 @@ def test_smeared_action_vs_oracle(api, oracle, cfg_id, N, dim):
     bits, bitsT = gpu_bits(api, coords, cfg.geometry)
     h = api.interval_hist(bits, bitsT, N)
     assert float(api.smeared_action(h, N, dim, 2.0 ** -6)[0]) == float(api.smeared_action(d_hist, N, dim, 2.0 ** -6)[0])
+
+
+def test_smeared_action_device_vs_exact_rational(api, oracle):
+    """The DEVICE value against Eq. 4.13-4.15 with Eq. 4.16-4.18 as printed, evaluated in exact
+    rational arithmetic on the same histogram and the same eps (Fraction(float) is exact).  The tolerance is the CUDA
+    side's own: the double-double bracket is rounded to fp64 once and multiplied by an fp64 prefactor, 2^-51 |S| for
+    the rational prefactor of d = 2, 2^-50 |S| where the prefactor is irrational (its few roundings on either side) --
+    four to five orders tighter than the comparison with the oracle's long-double sum, whose error dominates there."""
+    import math
+    from fractions import Fraction
+    N = 1200
+    coords = inp.sprinkle(inp.GEOM_MINK_CONE, 4, N, 4242)
+    _, hist, _, _ = oracle.action_pipeline(coords, inp.GEOM_MINK_CONE, tier=1)
+    d_hist = torch.from_numpy(hist).cuda()
+    for e in (2.0 ** -6, 0.2, 0.75, 0.013):
+        eps = Fraction(e)
+        q = 1 - eps
+        sums = {2: Fraction(0), 3: Fraction(0), 4: Fraction(0)}
+        qm = Fraction(1)                                         # q^m
+        for m in range(hist.shape[0]):                           # the paper's n_{m+1} f(m)
+            n = int(hist[m])
+            if n:
+                r = eps / q
+                sums[2] += n * qm * (1 - 2 * m * r + Fraction(m * (m - 1), 2) * r ** 2)
+                sums[3] += n * qm * (1 - Fraction(27, 8) * m * r + Fraction(9, 8) * m * (m - 1) * r ** 2)
+                sums[4] += n * qm * (1 - 9 * m * r + 8 * m * (m - 1) * r ** 2 - Fraction(4, 3) * m * (m - 1) * (m - 2) * r ** 3)
+            qm *= q
+        want = {2: (float(2 * eps * (N - 2 * eps * sums[2])), 2.0 ** -51),
+                3: ((1 / math.gamma(5 / 3)) * (math.pi * e / (3 * math.sqrt(2))) ** (2 / 3) * float(N - eps * sums[3]), 2.0 ** -50),
+                4: (4 * math.sqrt(e / 6) * float(N - eps * sums[4]), 2.0 ** -50)}
+        for dim in (2, 3, 4):
+            S = float(api.smeared_action(d_hist, N, dim, e)[0])
+            w, tol = want[dim]
+            assert abs(S - w) <= tol * abs(w), (dim, e, S, w)
+            # the bracket really cancels: the test would not see a sloppy sum otherwise
+            assert abs(float(N - (2 if dim == 2 else 1) * eps * sums[dim])) < 0.2 * float(sum(abs(int(x)) for x in hist)) or e > 0.5
+
+
+def test_tensor_selfchecks_pass_on_this_device(api):
+    """CS_ROUTE_AUTO / CS_A1_AUTO take the tensor routes only on a device that passed these; on a B200 both must."""
+    assert api.a2_tensor_selfcheck() is True
+    assert api.a1_tensor_selfcheck() is True
+    assert api.a2_tensor_selfcheck() is True                     # the cached answer
 
 
 @pytest.mark.parametrize("dim", [2, 3, 4])

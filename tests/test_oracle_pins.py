@@ -236,6 +236,30 @@ def test_tier1_equals_tier0_and_moments(oracle, geom, dim, seed, N):
     assert np.array_equal(ha + hb, h1)
 
 
+@pytest.mark.parametrize("geom,dim,N,step", [(inp.GEOM_MINK_CONE, 4, 1000, 7), (inp.GEOM_DS2_SLAB, 2, 777, 5),
+                                             (inp.GEOM_MINK2_LIGHTCONE, 2, 130, 64)])
+def test_tier1_row_step_partitions_the_rows(oracle, geom, dim, N, step):
+    """The stride of Alg. 20's outer loop (`row_step`, the sample bench.py times for the CPU
+    baseline and the reference arm): rows row_begin + m * row_step, nothing else.  The residue classes add up to the
+    whole histogram and the whole word count; one class equals the sum of its rows taken one at a time, from an
+    offset start too; N is not a multiple of the stride."""
+    coords = inp.sprinkle(geom, dim, N, 900 + N)
+    bits = oracle.causal_matrix_bits(coords, geom)
+    full, wfull, _ = oracle.interval_hist_alg20(bits, N)
+    parts = [oracle.interval_hist_alg20(bits, N, s0, N, row_step=step) for s0 in range(step)]
+    assert np.array_equal(sum(p[0] for p in parts), full)
+    assert sum(p[1] for p in parts) == wfull
+    assert full.sum() > 0 and sum(1 for p in parts if p[0].sum() > 0) >= min(step, 3)
+    for s0, row_end in ((0, N), (step - 1, N), (3, N - 11)):
+        got, wgot, _ = oracle.interval_hist_alg20(bits, N, s0, row_end, row_step=step)
+        rows = [oracle.interval_hist_alg20(bits, N, i, i + 1) for i in range(s0, row_end, step)]
+        assert np.array_equal(got, sum(r[0] for r in rows)) and wgot == sum(r[1] for r in rows)
+    # a stride larger than the range touches its first row only
+    one, wone, _ = oracle.interval_hist_alg20(bits, N, 2, 10, row_step=100)
+    ref, wref, _ = oracle.interval_hist_alg20(bits, N, 2, 3)
+    assert np.array_equal(one, ref) and wone == wref
+
+
 def test_tier1_equals_tier0_N2048(oracle):
     cfg = inp.CONFIGS[5]
     coords = inp.make_config_coords(cfg, batch_index=1)
@@ -488,7 +512,7 @@ def _ds4_point(eta, psi, th, ph):
 
 
 def test_ds4_spherical_relation(oracle):
-    """3+1 de Sitter, spherical foliation (PAPER.md:3829-3845; d eta^2 > d Sigma^2, PAPER.md:3168).  Hand cases; the
+    """3+1 de Sitter, spherical foliation (PAPER.md:3845-3863; d eta^2 > d Sigma^2, PAPER.md:3168).  Hand cases; the
     arccos form of the great-circle distance away from the cone; on a great circle of the 3-sphere the relation is
     the 1+1 slab's periodic one (GEOM_DS2_SLAB, strictness aside); transitivity; the sprinkler's marginals."""
     g = inp.GEOM_DS4_SPHERICAL
