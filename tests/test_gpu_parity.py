@@ -370,6 +370,35 @@ def test_causal_matrix_tensor_route_degenerate(api, oracle):
                           oracle.causal_matrix_bits(mixed, inp.GEOM_MINK_CONE))
 
 
+@pytest.mark.parametrize("dim", [4, 5])
+def test_causal_matrix_tensor_route_mixed_exponents(api, oracle, dim):
+    """The tensor route's error band (reading A21) inside its accepted range 2^-40 .. 2^40 but with the exponents
+    mixed within every tile: points scaled by 2^-15, 1 and 2^15 at random (the margin follows the largest addend of the
+    tile while most pairs have a tiny T), and near-null pairs far from the origin, where |h_i|, |h_j| and the products
+    are ~2^24 times the value they cancel to.  Every a1 route against the oracle (gpu_bits), and the probe's measured
+    error stays inside the margin on such input."""
+    rng = np.random.default_rng(50 + dim)
+    n = 2600
+    mixed = inp.sprinkle(inp.GEOM_MINK_CONE, dim, n, 70 + dim)
+    mixed *= np.array([2.0 ** -15, 1.0, 2.0 ** 15])[rng.integers(0, 3, n)][:, None]
+    mixed = np.ascontiguousarray(mixed[np.lexsort((mixed[:, 1], mixed[:, 0]))])
+    far = _near_null_set(rng, 650, dim)                      # 2600 points: partners on the cone and one ulp off it
+    far[:, 0] += 4096.0                                     # h = (t^2 - |x|^2) / 2 ~ 2^20 for every point
+    far[:, 1] += 3900.0
+    far = np.ascontiguousarray(far[np.lexsort((far[:, 1], far[:, 0]))])
+    both = np.concatenate([mixed[: n // 2], far[: n // 2] * 2.0 ** 3])
+    both = np.ascontiguousarray(both[np.lexsort((both[:, 1], both[:, 0]))])
+    for c in (mixed, far, both):
+        o_bits = oracle.causal_matrix_bits(c, inp.GEOM_MINK_CONE)
+        bits, bitsT = gpu_bits(api, c, inp.GEOM_MINK_CONE)
+        assert np.array_equal(to_u64(bits), o_bits)
+        assert np.array_equal(to_u64(bitsT), oracle.transpose_bits(o_bits, c.shape[0]))
+        b2, _, st = api.a1_tensor_probe(torch.from_numpy(c).cuda())
+        assert np.array_equal(to_u64(b2), o_bits)
+        assert st["max_err_over_margin"] < 0.5, st
+        assert 0 < st["rows_fp64"] <= st["rows_total"], st
+
+
 def test_causal_matrix_lightcone_ties(api, oracle):
     """1+1 light cone (two strict fp64 comparisons): coordinates that differ by one fp64 ulp, exact ties, values
     beyond the fp32 range, denormals and NaN.  (An fp32 prefilter was measured for this predicate too and
