@@ -261,6 +261,96 @@ def sprinkle_ds2_diamond_spherical(N: int, seed: int, w0: float = 0.8) -> np.nda
     return _sort_rows(c, (u + v) / 2.0, u)
 
 
+def _polar6(t, rad, r_theta, r_phi):
+    """(eta, r, cos th, sin th, cos ph, sin ph) rows with theta* = arccos(1 - 2u), phi* = 2 pi u."""
+    ct = 1.0 - 2.0 * r_theta
+    st = np.sqrt(np.maximum(0.0, 1.0 - ct * ct))
+    ph = (2.0 * np.pi) * r_phi
+    return np.stack([t, rad, ct, st, np.cos(ph), np.sin(ph)], axis=1)
+
+
+def ds4_diamond_flat_mu(w: float, u0: float) -> float:
+    """mu of the 3+1 dS diamond, flat foliation: ln[(w + 2u0)^2 / (4 u0 (w + u0))] - (w / (w + 2u0))^2."""
+    return float(np.log((w + 2.0 * u0) ** 2 / (4.0 * u0 * (w + u0))) - (w / (w + 2.0 * u0)) ** 2)
+
+
+def sprinkle_ds4_diamond_flat(N: int, seed: int, w: float = 0.5) -> np.ndarray:
+    """3+1 de Sitter diamond, flat foliation: rho(u, v) = (6 / mu) (u - v)^2 / (u + v)^4 on
+    u in [u0, u0 + w], v in [u0, u], u0 = -1/sqrt 2 (as in the 1+1 diamond; w < 1/sqrt 2).  The
+    printed u*, v* (Lambert W, a cubic) are garbled in the extracted text; both are inverse CDFs of the stated
+    density, which has them in closed form (reading A23), inverted here by bisection:
+      F(u)     = (6 / mu) [G(u) - G(u0)],  G(x) = ln|x + u0| / 3 + 2 u0 / (3 (x + u0)) - 2 u0^2 / (3 (x + u0)^2) - ln|x| / 6
+      F(v | u) = [K(u + v) - K(u + u0)] / [K(2u) - K(u + u0)],  K(s) = -4 u^2 / (3 s^3) + 2 u / s^2 - 1 / s.
+    Conformally flat with eta = (u + v) / sqrt 2 < 0, r = (u - v) / sqrt 2: [N][6] for GEOM_FLRW_POLAR."""
+    r = uniform01(seed, 0, 4 * N).reshape(N, 4)
+    u0 = -1.0 / np.sqrt(2.0)
+    mu = ds4_diamond_flat_mu(w, u0)
+
+    def G(x):
+        a = x + u0
+        return np.log(np.abs(a)) / 3.0 + 2.0 * u0 / (3.0 * a) - 2.0 * u0 * u0 / (3.0 * a * a) - np.log(np.abs(x)) / 6.0
+    u = _invert_monotone(lambda x: 6.0 * (G(x) - G(u0)) / mu, r[:, 0], u0, u0 + w)
+
+    def K(sv):
+        return -4.0 * u * u / (3.0 * sv ** 3) + 2.0 * u / sv ** 2 - 1.0 / sv
+    span = K(2.0 * u) - K(u + u0)
+    t = _invert_monotone(lambda q: np.where(span > 0, (K(u + u0 + q * (u - u0)) - K(u + u0)) / np.where(span > 0, span, 1.0), q),
+                         r[:, 1], 0.0, 1.0)
+    v = u0 + t * (u - u0)
+    c = _polar6((u + v) / np.sqrt(2.0), (u - v) / np.sqrt(2.0), r[:, 2], r[:, 3])
+    return _sort_rows(c, c[:, 0], c[:, 1])
+
+
+def sprinkle_ds4_diamond_spherical(N: int, seed: int, w0: float = 0.8) -> np.ndarray:
+    """3+1 de Sitter diamond, spherical foliation: rho(u, v) ~ sec^4((u + v)/sqrt 2)
+    sin^2((u - v)/sqrt 2) on u in [0, w0], v in [0, u].  The printed u(u*), u(v*) are cut off in the extracted text and
+    "must be inverted numerically" anyway; the stated density is sampled in eta = (u + v)/sqrt 2, psi = (u - v)/sqrt 2
+    (constant Jacobian; reading A23): 0 <= psi <= psi_m(eta) = min(eta, sqrt 2 w0 - eta),
+      p(eta) ~ sec^4(eta) (psi_m - sin(2 psi_m)/2),  F(psi | eta) = (psi - sin(2 psi)/2) / (psi_m - sin(2 psi_m)/2),
+    the first through a cumulative Simpson table (8192 panels), both inverted by bisection.
+    [N][7] = (eta, cos eta, sin eta, X0..X3) for GEOM_DS4_SPHERICAL (w0 < pi / (2 sqrt 2))."""
+    r = uniform01(seed, 0, 4 * N).reshape(N, 4)
+    top = np.sqrt(2.0) * w0
+
+    def area(pm):
+        return pm - 0.5 * np.sin(2.0 * pm)
+    n = 8192
+    grid = np.linspace(0.0, top, 2 * n + 1)
+    f = area(np.minimum(grid, top - grid)) / np.cos(grid) ** 4
+    h = grid[1] - grid[0]
+    cum = np.concatenate([[0.0], np.cumsum((f[0:-2:2] + 4.0 * f[1:-1:2] + f[2::2]) * (h / 3.0))])
+    eta = _invert_monotone(lambda x: np.interp(x, grid[::2], cum) / cum[-1], r[:, 0], 0.0, top)
+    pm = np.minimum(eta, top - eta)
+    am = area(pm)
+    t = _invert_monotone(lambda q: np.where(am > 0, area(q * pm) / np.where(am > 0, am, 1.0), q), r[:, 1], 0.0, 1.0)
+    psi = t * pm
+    ct = 1.0 - 2.0 * r[:, 2]
+    st = np.sqrt(np.maximum(0.0, 1.0 - ct * ct))
+    ph = (2.0 * np.pi) * r[:, 3]
+    sp = np.sin(psi)
+    c = np.stack([eta, np.cos(eta), np.sin(eta), np.cos(psi), sp * ct, sp * st * np.cos(ph), sp * st * np.sin(ph)], axis=1)
+    return _sort_rows(c, eta, psi)
+
+
+def sprinkle_dust_diamond(N: int, seed: int, u0: float = 1.0) -> np.ndarray:
+    """3+1 dust diamond: rho(u, v) = 5940 / (1981 u0^12) (u + v)^8 (u - v)^2 on u in [0, u0],
+    v in [0, u]; u* = u0 u^(1/12); v* from the printed eleventh-degree polynomial (partly garbled in the extracted text),
+    "must be inverted numerically": it is the conditional CDF of the stated density,
+      F(v | u) = [Q(u + v) - Q(u)] / [Q(2u) - Q(u)],  Q(s) = 4 u^2 s^9 / 9 - 2 u s^10 / 5 + s^11 / 11
+    (reading A23), inverted by bisection.  Conformally flat in eta = (u + v)/sqrt 2, r = (u - v)/sqrt 2
+    (the conformal factor ~ (u + v)^4 does not enter the relation): [N][6] for GEOM_FLRW_POLAR."""
+    r = uniform01(seed, 0, 4 * N).reshape(N, 4)
+    u = u0 * r[:, 0] ** (1.0 / 12.0)
+
+    def Q(sv):
+        return 4.0 * u * u * sv ** 9 / 9.0 - 2.0 * u * sv ** 10 / 5.0 + sv ** 11 / 11.0
+    span = Q(2.0 * u) - Q(u)
+    t = _invert_monotone(lambda q: np.where(span > 0, (Q(u + q * u) - Q(u)) / np.where(span > 0, span, 1.0), q), r[:, 1], 0.0, 1.0)
+    v = t * u
+    c = _polar6((u + v) / np.sqrt(2.0), (u - v) / np.sqrt(2.0), r[:, 2], r[:, 3])
+    return _sort_rows(c, c[:, 0], c[:, 1])
+
+
 def chain_lightcone(N: int) -> np.ndarray:
     """Total order: u_i = v_i = i/N (sorted already)."""
     u = np.arange(N, dtype=np.float64) / max(N, 1)

@@ -1063,6 +1063,25 @@ def test_ds4_spherical_and_cone5_pipelines(api, oracle):
         api.causal_matrix(torch.zeros((10, 6), dtype=torch.float64, device="cuda"), inp.GEOM_DS4_SPHERICAL)
 
 
+def test_appendix_a_3p1_diamonds_pipeline(api, oracle):
+    """NEXT-4, the last three regions of App. A.1 (3+1 dS diamonds, flat and spherical foliation; 3+1
+    dust diamond): each sprinkling through a1 (every route), a2 and a3 against the oracle."""
+    N = 1800
+    for sprinkler, geom in ((inp.sprinkle_ds4_diamond_flat, inp.GEOM_FLRW_POLAR),
+                            (inp.sprinkle_ds4_diamond_spherical, inp.GEOM_DS4_SPHERICAL),
+                            (inp.sprinkle_dust_diamond, inp.GEOM_FLRW_POLAR)):
+        c = sprinkler(N, 21)
+        o_bits, o_hist, o_S, o_I = oracle.action_pipeline(c, geom, tier=1)
+        bits, bitsT = gpu_bits(api, c, geom)
+        assert np.array_equal(to_u64(bits), o_bits), sprinkler.__name__
+        hist = api.interval_hist(bits, bitsT, N)
+        assert np.array_equal(hist.cpu().numpy(), o_hist) and o_hist.sum() > N
+        S, I = api.bd_action(hist, N, 4, return_bracket=True)
+        assert int(I[0]) == o_I and float(S[0]) == o_S
+        h_host, s_host = api.action_host(torch.from_numpy(c).pin_memory(), geom)
+        assert np.array_equal(h_host.numpy(), o_hist) and float(s_host[0]) == o_S
+
+
 @pytest.mark.slow
 def test_larger_N_properties(api, oracle):
     """NEXT-4 'larger N': N = 262144 (8 GiB per bit matrix, 1024 x 1024 tiles) in the 1+1 de Sitter slab.  The oracle's

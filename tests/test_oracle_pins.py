@@ -634,3 +634,67 @@ def test_appendix_a_de_sitter_and_dust_lambda_sprinklers(oracle):
     assert 0 < c[:, 0].min() and c[:, 0].max() <= eta_max + 1e-12
     C = oracle.causal_matrix_bytes(c[:500], inp.GEOM_FLRW_POLAR)
     assert C.sum() > 0
+
+
+def test_appendix_a_diamonds_3p1(oracle):
+    """The last three regions of App. A.1: 3+1 dS diamonds (flat and spherical foliation) and the
+    3+1 dust diamond.  The printed inverse CDFs are garbled in the extracted text (DESIGN.md
+    reading A23); the sprinklers invert the CDFs of the STATED densities, so the pins are those densities integrated
+    numerically (scipy quadrature, nothing shared with the sprinklers' closed forms), the paper's printed volumes /
+    normalisations (mu of PAPER.md:3889 and 3933, 1981/5940 of PAPER.md:3961), the regions, and the relation they feed."""
+    from scipy.integrate import dblquad, quad
+    n = 60000
+    s2 = np.sqrt(2.0)
+
+    def check(uv, dens, ulo, uhi, vlo, total, tol=0.012):
+        u, v = uv
+        assert np.all(u >= ulo - 1e-12) and np.all(u <= uhi + 1e-12) and np.all(v >= vlo - 1e-12) and np.all(v <= u + 1e-12)
+        for q in np.linspace(ulo, uhi, 7)[1:-1]:                   # marginal CDF of u
+            want = dblquad(lambda vv, uu: dens(uu, vv), ulo, q, lambda uu: vlo, lambda uu: uu)[0] / total
+            assert abs((u < q).mean() - want) < tol, (q, (u < q).mean(), want)
+        lo_q, hi_q = np.quantile(u, [0.50, 0.54])                   # conditional CDF of v in a thin band of u (2400 points)
+        band = (u > lo_q) & (u < hi_q)
+        um = u[band].mean()
+        den = quad(lambda vv: dens(um, vv), vlo, um)[0]
+        for q in np.linspace(vlo, um, 6)[1:-1]:
+            want = quad(lambda vv: dens(um, vv), vlo, q)[0] / den
+            assert abs((v[band] < q).mean() - want) < 0.04, (q, (v[band] < q).mean(), want)
+
+    # flat foliation: rho ~ (u - v)^2 / (u + v)^4, total = mu / 6 (PAPER.md:3881, 3889)
+    w, u0 = 0.5, -1 / s2
+    dens = lambda u, v: (u - v) ** 2 / (u + v) ** 4
+    total = dblquad(lambda vv, uu: dens(uu, vv), u0, u0 + w, lambda uu: u0, lambda uu: uu)[0]
+    assert inp.ds4_diamond_flat_mu(w, u0) / 6 == pytest.approx(total, rel=1e-9)
+    c = inp.sprinkle_ds4_diamond_flat(n, 3, w)
+    assert np.all(np.diff(c[:, 0]) >= 0) and c[:, 0].max() < 0 and c[:, 1].min() >= 0
+    check(((c[:, 0] + c[:, 1]) / s2, (c[:, 0] - c[:, 1]) / s2), dens, u0, u0 + w, u0, total)
+    assert abs(c[:, 2].mean()) < 0.01 and np.allclose(c[:, 2] ** 2 + c[:, 3] ** 2, 1) and np.allclose(c[:, 4] ** 2 + c[:, 5] ** 2, 1)
+
+    # spherical foliation: rho ~ sec^4((u + v)/sqrt 2) sin^2((u - v)/sqrt 2), total = mu / 3 (PAPER.md:3917, 3933)
+    w0 = 0.8
+    dens = lambda u, v: np.sin((u - v) / s2) ** 2 / np.cos((u + v) / s2) ** 4
+    total = dblquad(lambda vv, uu: dens(uu, vv), 0, w0, lambda uu: 0, lambda uu: uu)[0]
+    mu = np.log(0.5 * (1 + 1 / np.cos(s2 * w0))) - 1 / np.cos(w0 / s2) ** 2 + 1
+    assert mu / 3 == pytest.approx(total, rel=1e-9)
+    c = inp.sprinkle_ds4_diamond_spherical(n, 4, w0)
+    eta = c[:, 0]
+    psi = np.arccos(np.clip(c[:, 3], -1, 1))
+    assert np.all(np.diff(eta) >= 0) and np.allclose(c[:, 1], np.cos(eta)) and np.allclose(c[:, 2], np.sin(eta))
+    assert np.allclose((c[:, 3:] ** 2).sum(axis=1), 1)
+    check(((eta + psi) / s2, (eta - psi) / s2), dens, 0, w0, 0, total)
+
+    # dust: rho = 5940 / (1981 u0^12) (u + v)^8 (u - v)^2 (PAPER.md:3961)
+    dens = lambda u, v: (u + v) ** 8 * (u - v) ** 2
+    total = dblquad(lambda vv, uu: dens(uu, vv), 0, 1, lambda uu: 0, lambda uu: uu)[0]
+    assert total == pytest.approx(1981 / 5940, rel=1e-9)
+    c = inp.sprinkle_dust_diamond(n, 5, 1.0)
+    assert np.all(np.diff(c[:, 0]) >= 0)
+    check(((c[:, 0] + c[:, 1]) / s2, (c[:, 0] - c[:, 1]) / s2), dens, 0, 1.0, 0, total)
+
+    # each feeds a predicate that is already pinned: upper triangular, transitive, a non-trivial relation density
+    for cc, g in ((inp.sprinkle_ds4_diamond_flat(400, 7), inp.GEOM_FLRW_POLAR),
+                  (inp.sprinkle_ds4_diamond_spherical(400, 8), inp.GEOM_DS4_SPHERICAL),
+                  (inp.sprinkle_dust_diamond(400, 9), inp.GEOM_FLRW_POLAR)):
+        C = oracle.causal_matrix_bytes(cc, g).astype(bool)
+        assert np.array_equal(C, np.triu(C, 1)) and 0.02 < C.sum() / (400 * 399 / 2) < 0.9
+        assert not (C.astype(np.int32) @ C.astype(np.int32) > 0)[~C & np.triu(np.ones_like(C), 1)].any()
