@@ -240,8 +240,10 @@ int cs_interval_hist_static(const uint64_t *bits, const uint64_t *bitsT, int64_t
  * route on that device (the workspace AUTO asked for is large enough for it) and cs_last_cuda_error() says what
  * differed.  This call runs the check if it has not run yet and reports it: 1 exact, 0 not (AUTO = POPC there;
  * CS_ROUTE_TENSOR_PAIR by name still runs), < 0 a cs_status.  The first time it takes ~2 MiB from the library's
- * stream-ordered pool and synchronises `stream` (about 1 ms); then it returns the cached answer.  Like
- * cs_a1_tensor_selfcheck it should first run outside any stream capture. */
+ * stream-ordered pool and synchronises `stream` (about 1 ms); then it returns the cached answer.  Neither self-check
+ * runs while `stream` is being captured into a CUDA graph (it would invalidate the capture): an AUTO call made during
+ * capture on a device that has not been checked yet records the POPC (a1: FMA) route into the graph, and this call then
+ * reports 0 without caching it.  Call it once at start-up, outside any capture, to have the tensor routes in graphs. */
 int cs_a2_tensor_selfcheck(void *stream);
 
 /* What the last cs_interval_hist* call that used `workspace` executed (for the roofline on executed work):

@@ -67,6 +67,19 @@ struct PerDeviceFlag {
 
 int sm_count();   // SMs of the current device (cached per device)
 
+// true while `st` is being captured into a CUDA graph (or the query itself fails, which a capture elsewhere can cause):
+// the one-time self-checks synchronise the stream and take pool memory, which would invalidate the caller's capture,
+// so they do not run then and the AUTO routes take the path that needs no trust for that call
+inline bool stream_is_capturing(cudaStream_t st)
+{
+    cudaStreamCaptureStatus status = cudaStreamCaptureStatusNone;
+    if (cudaStreamIsCapturing(st, &status) != cudaSuccess) {
+        cudaGetLastError();
+        return true;
+    }
+    return status != cudaStreamCaptureStatusNone;
+}
+
 // First 256 bytes of every a2 workspace: scheduling counters of the route and what the launch executed
 // (read back through cs_interval_hist_stats).
 struct IntervalStats {

@@ -86,6 +86,10 @@ int interval_pair_trusted(cudaStream_t st, bool *trusted)
     static std::mutex mu;
     const int dev = current_device();
     int s0 = state[dev].load(std::memory_order_acquire);
+    if (s0 == 0 && stream_is_capturing(st)) {         // not now: the check would break the caller's capture
+        *trusted = false;
+        return CS_OK;
+    }
     if (s0 == 0) {
         std::lock_guard<std::mutex> lock(mu);
         s0 = state[dev].load(std::memory_order_acquire);

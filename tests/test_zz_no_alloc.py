@@ -93,3 +93,4 @@ def test_static_scratch_refuses_sizes_beyond_its_capacity(api):
     assert int(hist.min().item()) == 7 and int(hist.max().item()) == 7      # nothing was written
     # the library still works afterwards
     assert api.interval_hist_static(bits[:64, :2].contiguous(), None, 64).sum().item() == 0
+
